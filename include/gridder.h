@@ -1,0 +1,148 @@
+/*
+ * gridder.h -- C ABI of the B200 convolutional gridder (libgridder.so).
+ *
+ * The operation (section 5, Eq. 1, :174-183): every calibrated visibility V_i at
+ * (u_i, v_i) is convolved with a compact gridding convolution function (GCF) f and added to a
+ * regular uv grid,
+ *        V_grid(u, v) = sum_i f_i(r) * V_i delta(u - u_i, v - v_i),
+ * i.e. "compute the distance from the visibility to the centre of a given pixel, and then add the
+ * value of f_i(r) V_i to that grid cell" (:181) for the S x S patch of cells the GCF reaches
+ * (:183, "added the weighted values to those pixels").  The GCF is looked up in an oversampled
+ * table (BASELINE.json north_star).  The exact arithmetic -- rounding of the position to the 1/O
+ * sub-cell lattice, patch origin, w-plane choice, drop rule -- is stated in DESIGN.md section 3
+ * (readings R1-R16) and is what oracle/gridder_oracle.c restates independently in double.
+ *
+ * Pipeline behind the four calls (PAPER.md :197-199 "binned" gridder is the prior art):
+ *   gridder_plan    validate, size and carve the workspace, re-lay the GCF table     (host + 1 kernel)
+ *   gridder_bin     map  uvw x freq -> (tile, patch origin, sub-cell offset) keys    (FP64, exact)
+ *                   sort stable device radix sort of (key, visibility index)         (:199)
+ *                   tile 'first/last' tables and the work-item table                 (:197)
+ *   gridder_grid    grid each warp owns a uv tile (+halo) region in shared memory, FP32 FMA
+ *                   flush fixed-order FP64 sum of the partial regions -> HBM grid
+ *   gridder_destroy
+ *
+ * Conventions
+ *   - Pointers are DEVICE pointers unless marked HOST.  The library allocates no device memory:
+ *     the caller owns every buffer, including the workspace.
+ *   - Calls only enqueue work on `cuda_stream` (a cudaStream_t passed as void*; NULL = default
+ *     stream).  gridder_plan, gridder_destroy, gridder_get_stats and gridder_run_host synchronise.
+ *   - Buffers given to gridder_bin / gridder_grid must stay valid until that work has completed.
+ *   - A plan may be binned and gridded any number of times; one gridder_bin serves any number of
+ *     gridder_grid calls (same uv geometry, new visibilities).  Not thread-safe per plan.
+ *   - Layouts: uvw_m double [n_time][n_baseline][3] (metres); freq_hz double [n_chan];
+ *     vis float [n_time][n_baseline][n_chan][4 pol][re, im], polarisation order XX, XY, YX, YY;
+ *     weight float [n_time][n_baseline][n_chan] (one weight per sample, shared by the 4 pols);
+ *     grid float [4 pol][N][N][re, im]; (u, v) = (0, 0) is cell (N/2, N/2), u along x (fastest).
+ *   - Visibilities whose patch would leave the grid are dropped whole and counted (not an error).
+ *     Inputs are assumed finite.  Results are bit-identical from run to run.
+ *   - Return value: 0 on success, a negative gridder_status otherwise.  Nothing aborts or throws.
+ */
+#ifndef GRIDDER_H
+#define GRIDDER_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define GRIDDER_API __attribute__((visibility("default")))
+#else
+#define GRIDDER_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    GRIDDER_OK = 0,
+    GRIDDER_ERR_INVALID_ARG = -1,      /* null pointer, bad size, odd grid, S*O odd, n_pol != 4 ...  */
+    GRIDDER_ERR_CAPACITY = -2,         /* n_time*n_baseline*n_chan > max_vis                          */
+    GRIDDER_ERR_WORKSPACE = -3,        /* workspace_bytes too small (needed size is reported)         */
+    GRIDDER_ERR_CUDA = -4,             /* a CUDA runtime call failed (see gridder_last_cuda_error)    */
+    GRIDDER_ERR_NOT_BINNED = -5,       /* gridder_grid before a successful gridder_bin                */
+    GRIDDER_ERR_UNSUPPORTED = -6       /* configuration outside what this build implements            */
+} gridder_status;
+
+typedef struct gridder_plan_s gridder_plan_t;      /* opaque host object */
+
+/* Problem statement (PAPER.md :174-183) + table/grid geometry (BASELINE.json north_star). */
+typedef struct {
+    int32_t grid_size;          /* N: square grid, even                                             */
+    double cell_size;           /* du = dv in wavelengths per cell, > 0                             */
+    int32_t n_pol;              /* must be 4                                                        */
+    int32_t oversample;         /* O >= 1 table samples per cell; S_p * O must be even              */
+    int32_t n_wplanes;          /* P >= 1                                                           */
+    const int32_t *support;     /* HOST [P]: S_p taps per axis of plane p, 1 <= S_p <= 32           */
+    double w_max;               /* wavelengths; plane = min(P-1, floor(|w| / w_max * P)); P = 1: unused */
+    int32_t kernel_is_complex;  /* 0: float table; 1: (re, im) float pairs, conjugated for w < 0    */
+    const void *kernel;         /* DEVICE: plane-major, plane p is [S_p O][S_p O] samples, sample
+                                   (jy, jx) is the GCF at r = (j - S_p O / 2) / O cells; read once,
+                                   during gridder_plan                                              */
+    int64_t max_vis;            /* capacity: upper bound of n_time * n_baseline * n_chan            */
+    void *workspace;            /* DEVICE scratch, 256-byte aligned, owned by the caller            */
+    size_t workspace_bytes;
+} gridder_config;
+
+typedef struct {
+    int64_t n_vis;              /* visibilities given to the last gridder_bin                        */
+    int64_t n_dropped;          /* of those, dropped because the patch leaves the grid               */
+    int64_t n_entries;          /* sort entries (= gridded visibilities x sub-patches)               */
+    int64_t vis_taps;           /* sum of S_p^2 over gridded visibilities (the metric's numerator)   */
+    int64_t n_tiles;            /* uv tiles of the plan                                              */
+    int64_t n_tiles_occupied;
+    int64_t max_tile_load;      /* entries in the fullest tile                                       */
+    int64_t n_work_items;       /* (tile, chunk) work items: occupied tiles + hot-tile splits        */
+    int32_t tile_size;          /* T cells per tile edge                                             */
+    int32_t patch_size;         /* padded patch edge handled per entry (8 or 16)                     */
+    int32_t chunk_size;         /* K: most entries per work item                                     */
+    int32_t grid_warps_per_sm;  /* launch shape of the grid kernel                                   */
+} gridder_stats;
+
+/* Bytes of workspace a plan for `cfg` needs (cfg->workspace / workspace_bytes / kernel ignored). */
+GRIDDER_API int gridder_workspace_size(const gridder_config *cfg, size_t *bytes_needed);
+
+/* Create a plan.  On GRIDDER_ERR_WORKSPACE *workspace_needed holds the required size.
+ * `workspace_needed` may be NULL.  Synchronises the device once (table re-layout). */
+GRIDDER_API int gridder_plan(const gridder_config *cfg, gridder_plan_t **plan_out, size_t *workspace_needed);
+
+/* Map + sort + tile tables for n_time*n_baseline*n_chan visibilities (index (t*B + b)*F + f).
+ * u_lambda = u_m * (f / c), c = 299792458 m/s.  Asynchronous on `cuda_stream`. */
+GRIDDER_API int gridder_bin(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
+                const double *freq_hz, int32_t n_chan, void *cuda_stream);
+
+/* Grid + flush.  weight may be NULL (all 1).  accumulate == 0 overwrites all 4*N*N cells,
+ * otherwise the result is added to `grid`.  Asynchronous on `cuda_stream`. */
+GRIDDER_API int gridder_grid(gridder_plan_t *plan, const float *vis, const float *weight, float *grid,
+                 int32_t accumulate, void *cuda_stream);
+
+GRIDDER_API int gridder_destroy(gridder_plan_t *plan);
+
+/* ---- helpers outside the timed path -------------------------------------------------------- */
+
+/* Statistics of the last gridder_bin (synchronises the stream it ran on). */
+GRIDDER_API int gridder_get_stats(gridder_plan_t *plan, gridder_stats *out);
+
+/* The mapping alone, for tests: out is DEVICE int32 [n][6] = x0, y0, qx, qy, plane | conj << 8,
+ * dropped -- per visibility, same device function as gridder_bin's map kernel. */
+GRIDDER_API int gridder_map(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
+                const double *freq_hz, int32_t n_chan, int32_t *out, void *cuda_stream);
+
+/* End-to-end convenience with HOST buffers (pinned or pageable): copies uvw, freq, vis, weight to
+ * the caller's device staging buffers, runs gridder_bin + gridder_grid and copies the grid back,
+ * all on `cuda_stream`, then synchronises it.  d_* are DEVICE buffers at least as large as their
+ * host counterparts (d_weight may be NULL iff h_weight is NULL). */
+GRIDDER_API int gridder_run_host(gridder_plan_t *plan, const double *h_uvw_m, int32_t n_time, int32_t n_baseline,
+                     const double *h_freq_hz, int32_t n_chan, const float *h_vis,
+                     const float *h_weight, float *h_grid, double *d_uvw_m, double *d_freq_hz,
+                     float *d_vis, float *d_weight, float *d_grid, void *cuda_stream);
+
+GRIDDER_API const char *gridder_strerror(int code);
+/* cudaError_t of the most recent failing CUDA call made on behalf of `plan` (0 if none). */
+GRIDDER_API int gridder_last_cuda_error(const gridder_plan_t *plan);
+/* "major.minor.patch" of the library. */
+GRIDDER_API const char *gridder_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRIDDER_H */

@@ -1,0 +1,274 @@
+// The C ABI of include/gridder.h: plan management, argument checks, error codes.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "gridder_internal.cuh"
+
+using namespace gridder;
+
+namespace {
+
+size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+int env_int(const char *name, int dflt) {
+    const char *v = getenv(name);
+    if (!v || !*v) return dflt;
+    return atoi(v);
+}
+
+int ceil_log2(unsigned long long v) {   // smallest b with 2^b >= v
+    int b = 0;
+    while ((1ull << b) < v) ++b;
+    return b;
+}
+
+// Everything that follows from the config alone (no device access).
+int derive(const gridder_config *cfg, Plan &p) {
+    if (!cfg) return GRIDDER_ERR_INVALID_ARG;
+    if (cfg->grid_size < 2 || (cfg->grid_size & 1) || cfg->grid_size > 32768) return GRIDDER_ERR_INVALID_ARG;
+    if (!(cfg->cell_size > 0.0) || cfg->n_pol != 4) return GRIDDER_ERR_INVALID_ARG;
+    if (cfg->oversample < 1 || cfg->oversample > 64) return GRIDDER_ERR_INVALID_ARG;
+    if (cfg->n_wplanes < 1 || cfg->n_wplanes > 64 || !cfg->support) return GRIDDER_ERR_INVALID_ARG;
+    if (cfg->max_vis < 0 || cfg->max_vis > 0xFFFFFFF0ll) return GRIDDER_ERR_INVALID_ARG;
+    for (int i = 0; i < cfg->n_wplanes; ++i) {
+        const int s = cfg->support[i];
+        if (s < 1 || s > 32 || ((s * cfg->oversample) & 1)) return GRIDDER_ERR_INVALID_ARG;
+        if (s > cfg->grid_size) return GRIDDER_ERR_INVALID_ARG;
+    }
+    if (cfg->n_wplanes > 1 && !(cfg->w_max > 0.0)) return GRIDDER_ERR_INVALID_ARG;
+    // this build: one real table, support <= 16 (w-planes / complex tables: DESIGN.md section 9)
+    if (cfg->n_wplanes != 1 || cfg->kernel_is_complex || cfg->support[0] > 16) return GRIDDER_ERR_UNSUPPORTED;
+
+    p.cfg = *cfg;
+    memcpy(p.support_copy, cfg->support, sizeof(int32_t) * cfg->n_wplanes);
+    p.cfg.support = p.support_copy;
+    p.S = cfg->support[0];
+    if (p.S <= 8) { p.NA = 1; p.NB = 2; } else { p.NA = 2; p.NB = 4; }
+    p.tlog = env_int("GRIDDER_TILE_LOG2", 3);
+    if (p.tlog < 2 || p.tlog > 4) return GRIDDER_ERR_INVALID_ARG;
+    p.T = 1 << p.tlog;
+    p.ntx = (cfg->grid_size + p.T - 1) / p.T;
+    p.nty = p.ntx;
+    p.n_tiles = p.ntx * p.nty;
+    p.RW = p.T + 8 * p.NA - 1;
+    p.RH = p.T + 4 * p.NB - 1;
+    p.region_f4 = 2 * p.RW * p.RH;
+    p.chunk = env_int("GRIDDER_CHUNK", 2048);
+    if (p.chunk < 32 || p.chunk > (1 << 20)) return GRIDDER_ERR_INVALID_ARG;
+    p.warps = env_int("GRIDDER_WARPS", 0);
+
+    KeyLayout k;
+    k.bits_q = ceil_log2((unsigned long long)cfg->oversample);
+    k.tlog = p.tlog;
+    k.aux_bits = 2 * k.bits_q + 1;
+    k.tile_shift = k.aux_bits + 2 * k.tlog;
+    k.tile_bits = ceil_log2((unsigned long long)p.n_tiles);
+    if (k.tile_bits < 1) k.tile_bits = 1;
+    k.total_bits = k.tile_shift + k.tile_bits;
+    if (k.total_bits > 32) return GRIDDER_ERR_UNSUPPORTED;
+    p.key = k;
+
+    const int64_t n = cfg->max_vis;
+    int64_t occ = n < p.n_tiles ? n : p.n_tiles;
+    p.max_items = occ + n / p.chunk + 1;
+    p.coef_f4 = cfg->oversample * cfg->oversample * p.NA * p.NB * 32 / 4;
+    return GRIDDER_OK;
+}
+
+// Lay the workspace out; with base == nullptr only the size is computed.
+cudaError_t carve(Plan &p, char *base) {
+    size_t off = 0;
+    auto take = [&](size_t bytes) { char *ptr = base ? base + off : nullptr; off += align_up(bytes); return ptr; };
+    const size_t n = (size_t)(p.cfg.max_vis > 0 ? p.cfg.max_vis : 1);
+    for (int i = 0; i < 2; ++i) p.keys[i] = (uint32_t *)take(n * sizeof(uint32_t));
+    for (int i = 0; i < 2; ++i) p.vals[i] = (uint32_t *)take(n * sizeof(uint32_t));
+    size_t t1 = 0, t2 = 0;
+    cudaError_t e = sort_temp_bytes((int64_t)n, p.key.aux_bits, p.key.total_bits, &t1);
+    if (e == cudaSuccess) e = scan_temp_bytes(p.n_tiles + 1, &t2);
+    if (e != cudaSuccess) return e;
+    p.cub_temp_bytes = align_up(t1 > t2 ? t1 : t2);
+    p.cub_temp = take(p.cub_temp_bytes);
+    p.tile_start = (uint32_t *)take(sizeof(uint32_t) * 2 * (size_t)p.n_tiles);        // [start | end]
+    p.tile_chunks = (unsigned long long *)take(sizeof(unsigned long long) * ((size_t)p.n_tiles + 1));
+    p.tile_chunks_scan = (unsigned long long *)take(sizeof(unsigned long long) * ((size_t)p.n_tiles + 1));
+    p.tile_info = (TileInfo *)take(sizeof(TileInfo) * (size_t)p.n_tiles);
+    p.items = (WorkItem *)take(sizeof(WorkItem) * (size_t)p.max_items);
+    p.partials = (float4 *)take(sizeof(float4) * (size_t)p.region_f4 * (size_t)p.max_items);
+    p.coef = (float4 *)take(sizeof(float4) * (size_t)p.coef_f4);
+    p.counters = (Counters *)take(sizeof(Counters));
+    p.workspace_needed = off;
+    return cudaSuccess;
+}
+
+int cuda_fail(Plan *p, cudaError_t e) {
+    if (p) p->last_cuda_error = (int)e;
+    return GRIDDER_ERR_CUDA;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gridder_workspace_size(const gridder_config *cfg, size_t *bytes_needed) {
+    if (!bytes_needed) return GRIDDER_ERR_INVALID_ARG;
+    Plan p;
+    memset(&p, 0, sizeof(p));
+    const int rc = derive(cfg, p);
+    if (rc != GRIDDER_OK) return rc;
+    if (carve(p, nullptr) != cudaSuccess) return GRIDDER_ERR_CUDA;
+    *bytes_needed = p.workspace_needed;
+    return GRIDDER_OK;
+}
+
+int gridder_plan(const gridder_config *cfg, gridder_plan_t **plan_out, size_t *workspace_needed) {
+    if (!plan_out) return GRIDDER_ERR_INVALID_ARG;
+    *plan_out = nullptr;
+    Plan *p = new (std::nothrow) Plan;
+    if (!p) return GRIDDER_ERR_INVALID_ARG;
+    memset(p, 0, sizeof(Plan));
+    int rc = derive(cfg, *p);
+    if (rc != GRIDDER_OK) { delete p; return rc; }
+    if (carve(*p, nullptr) != cudaSuccess) { delete p; return GRIDDER_ERR_CUDA; }
+    if (workspace_needed) *workspace_needed = p->workspace_needed;
+    if (!cfg->kernel || !cfg->workspace || ((uintptr_t)cfg->workspace & 255)) { delete p; return GRIDDER_ERR_INVALID_ARG; }
+    if (cfg->workspace_bytes < p->workspace_needed) { delete p; return GRIDDER_ERR_WORKSPACE; }
+    if (carve(*p, (char *)cfg->workspace) != cudaSuccess) { delete p; return GRIDDER_ERR_CUDA; }
+
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = configure_grid_kernel(*p);
+    if (e == cudaSuccess) e = launch_relayout(*p, 0);
+    if (e == cudaSuccess) e = cudaMemsetAsync(p->counters, 0, sizeof(Counters), 0);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(0);
+    if (e != cudaSuccess) { delete p; return GRIDDER_ERR_CUDA; }
+    *plan_out = reinterpret_cast<gridder_plan_t *>(p);
+    return GRIDDER_OK;
+}
+
+int gridder_bin(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
+                const double *freq_hz, int32_t n_chan, void *cuda_stream) {
+    Plan *p = reinterpret_cast<Plan *>(plan);
+    if (!p || n_time < 0 || n_baseline < 0 || n_chan < 0) return GRIDDER_ERR_INVALID_ARG;
+    const int64_t n = (int64_t)n_time * n_baseline * n_chan;
+    if (n > 0 && (!uvw_m || !freq_hz)) return GRIDDER_ERR_INVALID_ARG;
+    if (n > p->cfg.max_vis) return GRIDDER_ERR_CAPACITY;
+    p->binned = false;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaError_t e = launch_bin(*p, uvw_m, n_time, n_baseline, freq_hz, n_chan, s);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    p->n_vis = n;
+    p->binned = true;
+    p->last_stream = s;
+    return GRIDDER_OK;
+}
+
+int gridder_grid(gridder_plan_t *plan, const float *vis, const float *weight, float *grid,
+                 int32_t accumulate, void *cuda_stream) {
+    Plan *p = reinterpret_cast<Plan *>(plan);
+    if (!p || !grid) return GRIDDER_ERR_INVALID_ARG;
+    if (!p->binned) return GRIDDER_ERR_NOT_BINNED;
+    if (p->n_vis > 0 && !vis) return GRIDDER_ERR_INVALID_ARG;
+    if (((uintptr_t)vis & 15) || ((uintptr_t)grid & 7)) return GRIDDER_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaError_t e = launch_grid(*p, vis, weight, grid, accumulate ? 1 : 0, s);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    p->last_stream = s;
+    return GRIDDER_OK;
+}
+
+int gridder_destroy(gridder_plan_t *plan) {
+    Plan *p = reinterpret_cast<Plan *>(plan);
+    if (!p) return GRIDDER_ERR_INVALID_ARG;
+    cudaError_t e = cudaDeviceSynchronize();     // the caller may free the workspace after this
+    delete p;
+    return e == cudaSuccess ? GRIDDER_OK : GRIDDER_ERR_CUDA;
+}
+
+int gridder_get_stats(gridder_plan_t *plan, gridder_stats *out) {
+    Plan *p = reinterpret_cast<Plan *>(plan);
+    if (!p || !out) return GRIDDER_ERR_INVALID_ARG;
+    if (!p->binned) return GRIDDER_ERR_NOT_BINNED;
+    Counters c;
+    cudaError_t e = cudaMemcpyAsync(&c, p->counters, sizeof(Counters), cudaMemcpyDeviceToHost, p->last_stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->last_stream);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    memset(out, 0, sizeof(*out));
+    out->n_vis = p->n_vis;
+    out->n_dropped = (int64_t)c.n_dropped;
+    out->n_entries = p->n_vis - (int64_t)c.n_dropped;
+    out->vis_taps = out->n_entries * (int64_t)p->S * p->S;
+    out->n_tiles = p->n_tiles;
+    out->n_tiles_occupied = c.n_occupied;
+    out->max_tile_load = c.max_tile_load;
+    out->n_work_items = c.n_items;
+    out->tile_size = p->T;
+    out->patch_size = 8 * p->NA;
+    out->chunk_size = p->chunk;
+    out->grid_warps_per_sm = p->warps;
+    return GRIDDER_OK;
+}
+
+int gridder_map(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
+                const double *freq_hz, int32_t n_chan, int32_t *out, void *cuda_stream) {
+    Plan *p = reinterpret_cast<Plan *>(plan);
+    if (!p || !uvw_m || !freq_hz || !out || n_time < 0 || n_baseline < 0 || n_chan < 0)
+        return GRIDDER_ERR_INVALID_ARG;
+    if ((int64_t)n_time * n_baseline * n_chan == 0) return GRIDDER_OK;
+    cudaError_t e = launch_map_debug(*p, uvw_m, n_time, n_baseline, freq_hz, n_chan, out, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    return GRIDDER_OK;
+}
+
+int gridder_run_host(gridder_plan_t *plan, const double *h_uvw_m, int32_t n_time, int32_t n_baseline,
+                     const double *h_freq_hz, int32_t n_chan, const float *h_vis, const float *h_weight,
+                     float *h_grid, double *d_uvw_m, double *d_freq_hz, float *d_vis, float *d_weight,
+                     float *d_grid, void *cuda_stream) {
+    Plan *p = reinterpret_cast<Plan *>(plan);
+    if (!p || !h_uvw_m || !h_freq_hz || !h_vis || !h_grid || !d_uvw_m || !d_freq_hz || !d_vis || !d_grid)
+        return GRIDDER_ERR_INVALID_ARG;
+    if (h_weight && !d_weight) return GRIDDER_ERR_INVALID_ARG;
+    if (n_time < 0 || n_baseline < 0 || n_chan < 0) return GRIDDER_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t n_tb = (size_t)n_time * n_baseline, n = n_tb * n_chan;
+    cudaError_t e = cudaMemcpyAsync(d_uvw_m, h_uvw_m, n_tb * 3 * sizeof(double), cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_freq_hz, h_freq_hz, (size_t)n_chan * sizeof(double), cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    // the binning only needs uvw and freq: it runs while the visibilities are still on the wire
+    int rc = gridder_bin(plan, d_uvw_m, n_time, n_baseline, d_freq_hz, n_chan, cuda_stream);
+    if (rc != GRIDDER_OK) return rc;
+    e = cudaMemcpyAsync(d_vis, h_vis, n * 8 * sizeof(float), cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess && h_weight) e = cudaMemcpyAsync(d_weight, h_weight, n * sizeof(float), cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    rc = gridder_grid(plan, d_vis, h_weight ? d_weight : nullptr, d_grid, 0, cuda_stream);
+    if (rc != GRIDDER_OK) return rc;
+    const size_t gbytes = (size_t)4 * p->cfg.grid_size * p->cfg.grid_size * 2 * sizeof(float);
+    e = cudaMemcpyAsync(h_grid, d_grid, gbytes, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    return GRIDDER_OK;
+}
+
+const char *gridder_strerror(int code) {
+    switch (code) {
+        case GRIDDER_OK: return "ok";
+        case GRIDDER_ERR_INVALID_ARG: return "invalid argument";
+        case GRIDDER_ERR_CAPACITY: return "more visibilities than the plan's max_vis";
+        case GRIDDER_ERR_WORKSPACE: return "workspace too small";
+        case GRIDDER_ERR_CUDA: return "CUDA runtime error";
+        case GRIDDER_ERR_NOT_BINNED: return "gridder_bin has not been called on this plan";
+        case GRIDDER_ERR_UNSUPPORTED: return "configuration not supported by this build";
+        default: return "unknown gridder status";
+    }
+}
+
+int gridder_last_cuda_error(const gridder_plan_t *plan) {
+    const Plan *p = reinterpret_cast<const Plan *>(plan);
+    return p ? p->last_cuda_error : 0;
+}
+
+const char *gridder_version(void) { return "0.1.0"; }
+
+}  // extern "C"

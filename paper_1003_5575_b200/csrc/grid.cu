@@ -1,0 +1,361 @@
+// gridder_grid: the gridding kernel (FP32 FMA, registers + shared memory) and the deterministic flush.
+//
+// Grid kernel.  PAPER.md :197-199 gathers per pixel from 9 bins; here the work
+// is turned round so that every lane does useful FMAs on every visibility:
+//   * a work item is <= K consecutive entries of one uv tile's sorted list; ONE WARP owns it;
+//   * the warp keeps the item's (T + SP - 1)^2-cell region (tile + halo) in shared memory;
+//   * for the current patch origin the SP x SP patch lives in REGISTERS, NA*NB cells (x 4 pol
+//     complex = 8 floats) per lane; entries are sorted by origin, so the patch is exchanged with
+//     the shared region only when the origin changes;
+//   * per entry a lane does 3 broadcast LDS.128 (visibility + meta), NA vector LDS (its taps of the
+//     GCF sub-table) and 8*NA*NB FFMA; visibilities are fetched one batch of 32 ahead with
+//     128-bit loads (float4 per polarisation pair) and pre-multiplied by their weight;
+//   * no atomics anywhere: every region cell has one owner lane, every work item its own partial
+//     region in HBM.
+// Flush kernel: each grid cell sums, in FP64 and in a fixed (tile row, tile column, chunk) order,
+// the partial regions that cover it, and writes the complex64 grid once.
+#include "gridder_internal.cuh"
+
+namespace gridder {
+
+template <int NA, int NB, int TLOG>
+struct Geo {
+    static constexpr int SPX = 8 * NA, SPY = 4 * NB;         // padded patch
+    static constexpr int T = 1 << TLOG;
+    static constexpr int RW = T + SPX - 1, RH = T + SPY - 1;   // region = tile + halo
+    static constexpr int CELLS = RW * RH;
+    static constexpr int STAGE_F4 = 2 * 32 * 3;                // 2 buffers x 32 records x 3 float4
+    static constexpr int WARP_F4 = 2 * CELLS + STAGE_F4;       // shared float4 per warp
+};
+
+__device__ __forceinline__ float4 ldg_stream(const float4 *p) {
+    float4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+    return r;
+}
+
+__device__ __forceinline__ void stg_stream(float4 *p, const float4 &v) {
+    asm volatile("st.global.L1::no_allocate.v4.f32 [%0], {%1,%2,%3,%4};"
+                 :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+
+// A staged record: the weighted visibility and where it goes.
+struct Rec {
+    float4 a, b;     // XX.re XX.im XY.re XY.im | YX.re YX.im YY.re YY.im, times weight
+    int coff;        // float offset of its GCF sub-table (q) in the shared table
+    int poff;        // cell offset of its patch origin in the region
+};
+
+template <int NA, int NB, int TLOG>
+__device__ __forceinline__ Rec load_record(const GridParams &p, uint32_t e, bool valid) {
+    using G = Geo<NA, NB, TLOG>;
+    Rec r;
+    r.a = make_float4(0.f, 0.f, 0.f, 0.f);
+    r.b = r.a;
+    r.coff = 0;
+    r.poff = 0;
+    if (valid) {
+        const uint32_t key = p.keys[e];
+        const uint32_t idx = p.vals[e];
+        const uint32_t qmask = (1u << (2 * p.key.bits_q)) - 1u;
+        const uint32_t tmask = (1u << TLOG) - 1u;
+        const uint32_t x0l = (key >> p.key.aux_bits) & tmask;
+        const uint32_t y0l = (key >> (p.key.aux_bits + TLOG)) & tmask;
+        r.coff = (int)((key & qmask) * (NA * 32 * NB));
+        r.poff = (int)(y0l * G::RW + x0l);
+        const bool dropped = (key >> (2 * p.key.bits_q)) & 1u;
+        if (!dropped) {
+            const float4 a = ldg_stream(p.vis + 2 * (size_t)idx);
+            const float4 b = ldg_stream(p.vis + 2 * (size_t)idx + 1);
+            const float w = p.weight ? __ldg(p.weight + idx) : 1.0f;
+            r.a = make_float4(a.x * w, a.y * w, a.z * w, a.w * w);
+            r.b = make_float4(b.x * w, b.y * w, b.z * w, b.w * w);
+        }
+    }
+    return r;
+}
+
+template <int NB> struct CoefVec;
+template <> struct CoefVec<4> {
+    float c[4];
+    __device__ __forceinline__ void load(const float *p) {
+        const float4 v = *reinterpret_cast<const float4 *>(p);
+        c[0] = v.x; c[1] = v.y; c[2] = v.z; c[3] = v.w;
+    }
+};
+template <> struct CoefVec<2> {
+    float c[2];
+    __device__ __forceinline__ void load(const float *p) {
+        const float2 v = *reinterpret_cast<const float2 *>(p);
+        c[0] = v.x; c[1] = v.y;
+    }
+};
+
+template <int NA, int NB, int TLOG, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32, 1) grid_kernel(const GridParams p) {
+    using G = Geo<NA, NB, TLOG>;
+    extern __shared__ float4 smem[];
+    float4 *coef4 = smem;
+    const float *coef = reinterpret_cast<const float *>(smem);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float4 *region = smem + p.coef_f4 + warp * G::WARP_F4;     // plane A then plane B
+    float4 *regA = region, *regB = region + G::CELLS;
+    float4 *stage = region + 2 * G::CELLS;
+
+    for (int i = threadIdx.x; i < p.coef_f4; i += WARPS * 32) coef4[i] = p.coef[i];
+    for (int i = lane; i < 2 * G::CELLS; i += 32) region[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncthreads();
+
+    const unsigned int n_items = p.counters_ro->n_items;
+    const int lane_cell = (lane >> 3) * G::RW + (lane & 7);      // tap (a=0, b=0) of this lane
+    const float *coef_lane = coef + lane * NB;
+
+    float acc[NA][NB][8];
+
+    while (true) {
+        unsigned int item = 0;
+        if (lane == 0) item = atomicAdd(&p.counters->queue_head, 1u);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        if (item >= n_items) break;
+        const WorkItem wi = p.items[item];
+        const int len = (int)wi.len;
+        const int n_batches = (len + 31) >> 5;
+
+        Rec rec = load_record<NA, NB, TLOG>(p, wi.start + lane, lane < len);
+        stage[lane * 3 + 0] = rec.a;
+        stage[lane * 3 + 1] = rec.b;
+        stage[lane * 3 + 2] = make_float4(__int_as_float(rec.coff), __int_as_float(rec.poff), 0.f, 0.f);
+        __syncwarp();
+        if (n_batches > 1) rec = load_record<NA, NB, TLOG>(p, wi.start + 32 + lane, 32 + lane < len);
+
+        int cur = -1;
+        for (int bi = 0; bi < n_batches; ++bi) {
+            const float4 *st = stage + (bi & 1) * 96;
+            const int cnt = min(32, len - bi * 32);
+            for (int r = 0; r < cnt; ++r) {
+                const float4 meta = st[r * 3 + 2];
+                const int coff = __float_as_int(meta.x), poff = __float_as_int(meta.y);
+                if (poff != cur) {                                  // warp-uniform
+                    if (cur >= 0) {
+#pragma unroll
+                        for (int a = 0; a < NA; ++a)
+#pragma unroll
+                            for (int b = 0; b < NB; ++b) {
+                                const int o = cur + lane_cell + 4 * b * G::RW + 8 * a;
+                                regA[o] = make_float4(acc[a][b][0], acc[a][b][1], acc[a][b][2], acc[a][b][3]);
+                                regB[o] = make_float4(acc[a][b][4], acc[a][b][5], acc[a][b][6], acc[a][b][7]);
+                            }
+                    }
+#pragma unroll
+                    for (int a = 0; a < NA; ++a)
+#pragma unroll
+                        for (int b = 0; b < NB; ++b) {
+                            const int o = poff + lane_cell + 4 * b * G::RW + 8 * a;
+                            const float4 x = regA[o], y = regB[o];
+                            acc[a][b][0] = x.x; acc[a][b][1] = x.y; acc[a][b][2] = x.z; acc[a][b][3] = x.w;
+                            acc[a][b][4] = y.x; acc[a][b][5] = y.y; acc[a][b][6] = y.z; acc[a][b][7] = y.w;
+                        }
+                    cur = poff;
+                }
+                const float4 va = st[r * 3 + 0], vb = st[r * 3 + 1];
+                const float v[8] = {va.x, va.y, va.z, va.w, vb.x, vb.y, vb.z, vb.w};
+                CoefVec<NB> c[NA];
+#pragma unroll
+                for (int a = 0; a < NA; ++a) c[a].load(coef_lane + coff + a * 32 * NB);
+#pragma unroll
+                for (int a = 0; a < NA; ++a)
+#pragma unroll
+                    for (int b = 0; b < NB; ++b)
+#pragma unroll
+                        for (int k = 0; k < 8; ++k) acc[a][b][k] = fmaf(c[a].c[b], v[k], acc[a][b][k]);
+            }
+            if (bi + 1 < n_batches) {
+                __syncwarp();
+                float4 *sn = stage + ((bi + 1) & 1) * 96;
+                sn[lane * 3 + 0] = rec.a;
+                sn[lane * 3 + 1] = rec.b;
+                sn[lane * 3 + 2] = make_float4(__int_as_float(rec.coff), __int_as_float(rec.poff), 0.f, 0.f);
+                __syncwarp();
+                if (bi + 2 < n_batches) {
+                    const int off = (bi + 2) * 32 + lane;
+                    rec = load_record<NA, NB, TLOG>(p, wi.start + off, off < len);
+                }
+            }
+        }
+        // put the last patch back, then move the region to this item's partial and clear it
+#pragma unroll
+        for (int a = 0; a < NA; ++a)
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                const int o = cur + lane_cell + 4 * b * G::RW + 8 * a;
+                regA[o] = make_float4(acc[a][b][0], acc[a][b][1], acc[a][b][2], acc[a][b][3]);
+                regB[o] = make_float4(acc[a][b][4], acc[a][b][5], acc[a][b][6], acc[a][b][7]);
+            }
+        __syncwarp();
+        float4 *dst = p.partials + (size_t)item * (2 * G::CELLS);
+        for (int i = lane; i < 2 * G::CELLS; i += 32) {
+            stg_stream(dst + i, region[i]);
+            region[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        __syncwarp();
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Flush: one thread per grid cell.  The partial regions covering cell (x, y) belong to the tiles
+// (ty, tx) with tx*T <= x < tx*T + RW (same in y); each tile's work items are added in id order
+// (full chunks, then the tail).  FP64 accumulation, one rounding to FP32 at the end.
+// ------------------------------------------------------------------------------------------
+template <int NA, int NB, int TLOG>
+__global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
+    using G = Geo<NA, NB, TLOG>;
+    const int x = blockIdx.x * 32 + threadIdx.x;
+    const int y = blockIdx.y * 8 + threadIdx.y;
+    if (x >= p.n_grid || y >= p.n_grid) return;
+    double acc[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) acc[k] = 0.0;
+    const int tx_hi = min(x >> TLOG, p.ntx - 1), ty_hi = min(y >> TLOG, p.nty - 1);
+    const int tx_lo = max(0, (x - G::RW + G::T) >> TLOG), ty_lo = max(0, (y - G::RH + G::T) >> TLOG);
+    for (int ty = ty_lo; ty <= ty_hi; ++ty)
+        for (int tx = tx_lo; tx <= tx_hi; ++tx) {
+            const TileInfo ti = p.tiles[ty * p.ntx + tx];
+            if (ti.count == 0) continue;
+            const int cell = (y - (ty << TLOG)) * G::RW + (x - (tx << TLOG));
+            const uint32_t n_it = ti.n_full + (ti.tail_item != 0xFFFFFFFFu ? 1u : 0u);
+            for (uint32_t c = 0; c < n_it; ++c) {
+                const uint32_t item = c < ti.n_full ? ti.full_base + c : ti.tail_item;
+                const float4 *part = p.partials + (size_t)item * (2 * G::CELLS);
+                const float4 a = __ldcs(part + cell), b = __ldcs(part + G::CELLS + cell);
+                acc[0] += (double)a.x; acc[1] += (double)a.y; acc[2] += (double)a.z; acc[3] += (double)a.w;
+                acc[4] += (double)b.x; acc[5] += (double)b.y; acc[6] += (double)b.z; acc[7] += (double)b.w;
+            }
+        }
+    const size_t nn = (size_t)p.n_grid * p.n_grid;
+    const size_t c0 = (size_t)y * p.n_grid + x;
+#pragma unroll
+    for (int pol = 0; pol < 4; ++pol) {
+        double re = acc[2 * pol], im = acc[2 * pol + 1];
+        if (p.accumulate) {
+            const float2 old = p.grid[pol * nn + c0];
+            re += (double)old.x;
+            im += (double)old.y;
+        }
+        p.grid[pol * nn + c0] = make_float2((float)re, (float)im);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Host side: kernel selection.  NA x NB is fixed by the padded patch (16: 2x4, 8: 1x2), TLOG and
+// the number of warps per block are plan parameters.
+// ------------------------------------------------------------------------------------------
+size_t grid_smem_bytes(int NA, int NB, int tlog, int oversample, int warps) {
+    const int T = 1 << tlog;
+    const int RW = T + 8 * NA - 1, RH = T + 4 * NB - 1;
+    const size_t coef = (size_t)oversample * oversample * NA * NB * 32 * sizeof(float);
+    const size_t per_warp = (size_t)(2 * RW * RH + 2 * 32 * 3) * sizeof(float4);
+    return coef + per_warp * warps;
+}
+
+typedef void (*grid_fn_t)(const GridParams);
+typedef void (*flush_fn_t)(const FlushParams);
+
+template <int NA, int NB, int TLOG>
+static grid_fn_t pick_warps(int warps) {
+    switch (warps) {
+        case 4: return grid_kernel<NA, NB, TLOG, 4>;
+        case 6: return grid_kernel<NA, NB, TLOG, 6>;
+        case 8: return grid_kernel<NA, NB, TLOG, 8>;
+        case 10: return grid_kernel<NA, NB, TLOG, 10>;
+        case 12: return grid_kernel<NA, NB, TLOG, 12>;
+        case 16: return grid_kernel<NA, NB, TLOG, 16>;
+        default: return nullptr;
+    }
+}
+
+static grid_fn_t pick_grid(int NA, int tlog, int warps) {
+    if (NA == 2) {
+        if (tlog == 2) return pick_warps<2, 4, 2>(warps);
+        if (tlog == 3) return pick_warps<2, 4, 3>(warps);
+        if (tlog == 4) return pick_warps<2, 4, 4>(warps);
+    } else {
+        if (tlog == 2) return pick_warps<1, 2, 2>(warps);
+        if (tlog == 3) return pick_warps<1, 2, 3>(warps);
+        if (tlog == 4) return pick_warps<1, 2, 4>(warps);
+    }
+    return nullptr;
+}
+
+static flush_fn_t pick_flush(int NA, int tlog) {
+    if (NA == 2) {
+        if (tlog == 2) return flush_kernel<2, 4, 2>;
+        if (tlog == 3) return flush_kernel<2, 4, 3>;
+        if (tlog == 4) return flush_kernel<2, 4, 4>;
+    } else {
+        if (tlog == 2) return flush_kernel<1, 2, 2>;
+        if (tlog == 3) return flush_kernel<1, 2, 3>;
+        if (tlog == 4) return flush_kernel<1, 2, 4>;
+    }
+    return nullptr;
+}
+
+static const int kWarpChoices[] = {16, 12, 10, 8, 6, 4};
+
+cudaError_t configure_grid_kernel(Plan &p) {
+    int dev = 0, smem_max = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return e;
+    int chosen = 0;
+    for (int w : kWarpChoices) {
+        if (p.warps > 0 && w != p.warps) continue;             // forced by the caller (tuning)
+        if (grid_smem_bytes(p.NA, p.NB, p.tlog, p.cfg.oversample, w) <= (size_t)smem_max) { chosen = w; break; }
+    }
+    if (!chosen) return cudaErrorInvalidConfiguration;
+    p.warps = chosen;
+    p.smem_bytes = (int)grid_smem_bytes(p.NA, p.NB, p.tlog, p.cfg.oversample, chosen);
+    grid_fn_t fn = pick_grid(p.NA, p.tlog, p.warps);
+    if (!fn) return cudaErrorInvalidConfiguration;
+    return cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, p.smem_bytes);
+}
+
+cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *grid, int accumulate,
+                        cudaStream_t s) {
+    grid_fn_t gfn = pick_grid(p.NA, p.tlog, p.warps);
+    flush_fn_t ffn = pick_flush(p.NA, p.tlog);
+    if (!gfn || !ffn) return cudaErrorInvalidConfiguration;
+    // reset the work queue (bin leaves it at 0, a previous grid call leaves it past the end)
+    cudaError_t e = cudaMemsetAsync(&p.counters->queue_head, 0, sizeof(unsigned int), s);
+    if (e != cudaSuccess) return e;
+    GridParams gp;
+    gp.keys = p.keys[p.sorted_sel];
+    gp.vals = p.vals[p.sorted_sel];
+    gp.items = p.items;
+    gp.counters_ro = p.counters;
+    gp.counters = p.counters;
+    gp.vis = reinterpret_cast<const float4 *>(vis);
+    gp.weight = weight;
+    gp.coef = p.coef;
+    gp.partials = p.partials;
+    gp.coef_f4 = p.coef_f4;
+    gp.key = p.key;
+    gfn<<<p.n_sm, p.warps * 32, p.smem_bytes, s>>>(gp);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    FlushParams fp;
+    fp.tiles = p.tile_info;
+    fp.counters = p.counters;
+    fp.partials = p.partials;
+    fp.grid = reinterpret_cast<float2 *>(grid);
+    fp.n_grid = p.cfg.grid_size;
+    fp.ntx = p.ntx;
+    fp.nty = p.nty;
+    fp.accumulate = accumulate;
+    dim3 blk(32, 8), grd((p.cfg.grid_size + 31) / 32, (p.cfg.grid_size + 7) / 8);
+    ffn<<<grd, blk, 0, s>>>(fp);
+    return cudaGetLastError();
+}
+
+}  // namespace gridder

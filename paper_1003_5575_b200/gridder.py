@@ -1,0 +1,226 @@
+"""Thin ctypes binding of include/gridder.h -- argument marshalling only.
+
+Every step of the path (map, sort, tile tables, grid, flush) runs inside libgridder.so's CUDA
+kernels.  torch is used for device memory and streams and nothing else.  There is no CPU
+fallback: if the shared library is missing or cannot be loaded this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from dataclasses import dataclass
+from pathlib import Path
+
+import torch
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "libgridder.so"
+
+OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_WORKSPACE, ERR_CUDA, ERR_NOT_BINNED, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
+
+EXPORTS = ("gridder_workspace_size", "gridder_plan", "gridder_bin", "gridder_grid", "gridder_destroy",
+           "gridder_get_stats", "gridder_map", "gridder_run_host", "gridder_strerror",
+           "gridder_last_cuda_error", "gridder_version")
+
+
+class GridderError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        super().__init__(f"{what}: {strerror(code)} ({code})")
+        self.code = code
+
+
+class _Config(C.Structure):
+    _fields_ = [("grid_size", C.c_int32), ("cell_size", C.c_double), ("n_pol", C.c_int32),
+                ("oversample", C.c_int32), ("n_wplanes", C.c_int32), ("support", C.POINTER(C.c_int32)),
+                ("w_max", C.c_double), ("kernel_is_complex", C.c_int32), ("kernel", C.c_void_p),
+                ("max_vis", C.c_int64), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+
+
+class _Stats(C.Structure):
+    _fields_ = [("n_vis", C.c_int64), ("n_dropped", C.c_int64), ("n_entries", C.c_int64),
+                ("vis_taps", C.c_int64), ("n_tiles", C.c_int64), ("n_tiles_occupied", C.c_int64),
+                ("max_tile_load", C.c_int64), ("n_work_items", C.c_int64), ("tile_size", C.c_int32),
+                ("patch_size", C.c_int32), ("chunk_size", C.c_int32), ("grid_warps_per_sm", C.c_int32)]
+
+
+_lib = None
+
+
+def load_library() -> C.CDLL:
+    """dlopen libgridder.so (built by ``python -m paper_1003_5575_b200.build``).  Fails loudly."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_1003_5575_b200.build` "
+                              "(there is no CPU fallback)")
+        lib = C.CDLL(str(LIB_PATH))
+        lib.gridder_workspace_size.argtypes = [C.POINTER(_Config), C.POINTER(C.c_size_t)]
+        lib.gridder_plan.argtypes = [C.POINTER(_Config), C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
+        lib.gridder_bin.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p]
+        lib.gridder_grid.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+        lib.gridder_destroy.argtypes = [C.c_void_p]
+        lib.gridder_get_stats.argtypes = [C.c_void_p, C.POINTER(_Stats)]
+        lib.gridder_map.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
+                                    C.c_void_p, C.c_void_p]
+        lib.gridder_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
+                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.gridder_strerror.argtypes = [C.c_int]
+        lib.gridder_strerror.restype = C.c_char_p
+        lib.gridder_last_cuda_error.argtypes = [C.c_void_p]
+        lib.gridder_version.restype = C.c_char_p
+        for name in EXPORTS:
+            getattr(lib, name)
+        _lib = lib
+    return _lib
+
+
+def strerror(code: int) -> str:
+    return load_library().gridder_strerror(int(code)).decode()
+
+
+def version() -> str:
+    return load_library().gridder_version().decode()
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def _dev_ptr(t, dtype, what):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise TypeError(f"{what} must be a contiguous CUDA tensor of {dtype}")
+    return t.data_ptr()
+
+
+@dataclass
+class Stats:
+    n_vis: int
+    n_dropped: int
+    n_entries: int
+    vis_taps: int
+    n_tiles: int
+    n_tiles_occupied: int
+    max_tile_load: int
+    n_work_items: int
+    tile_size: int
+    patch_size: int
+    chunk_size: int
+    grid_warps_per_sm: int
+
+
+class Gridder:
+    """gridder_plan / gridder_bin / gridder_grid / gridder_destroy with torch tensors as buffers."""
+
+    def __init__(self, *, grid_size: int, cell_size: float, oversample: int, support, kernel: torch.Tensor,
+                 max_vis: int, n_wplanes: int = 1, w_max: float = 1.0, kernel_is_complex: bool = False,
+                 device=None):
+        lib = load_library()
+        self._lib = lib
+        self._plan = C.c_void_p()
+        self.device = torch.device(device if device is not None else kernel.device)
+        if self.device.type != "cuda":
+            raise RuntimeError("the gridder runs on a CUDA device only (no CPU fallback)")
+        support = [int(s) for s in (support if hasattr(support, "__len__") else [support])]
+        self._support = (C.c_int32 * len(support))(*support)
+        self._kernel = kernel.to(self.device, torch.float32).contiguous()
+        self.grid_size = int(grid_size)
+        cfg = _Config(int(grid_size), float(cell_size), 4, int(oversample), int(n_wplanes), self._support,
+                      float(w_max), int(bool(kernel_is_complex)), self._kernel.data_ptr(), int(max_vis), None, 0)
+        need = C.c_size_t(0)
+        with torch.cuda.device(self.device):
+            rc = lib.gridder_workspace_size(C.byref(cfg), C.byref(need))
+            if rc != OK:
+                raise GridderError(rc, "gridder_workspace_size")
+            self.workspace = torch.empty(need.value + 256, dtype=torch.uint8, device=self.device)
+            base = (self.workspace.data_ptr() + 255) // 256 * 256
+            cfg.workspace = base
+            cfg.workspace_bytes = need.value
+            rc = lib.gridder_plan(C.byref(cfg), C.byref(self._plan), C.byref(need))
+        if rc != OK:
+            self._plan = C.c_void_p()
+            raise GridderError(rc, "gridder_plan")
+        self.workspace_bytes = need.value
+        self._keep = []
+
+    # -- the four calls ---------------------------------------------------------------------
+    def bin(self, uvw_m: torch.Tensor, freq_hz: torch.Tensor, stream=None) -> None:
+        """uvw_m float64 [n_time][n_baseline][3] (metres), freq_hz float64 [n_chan]; asynchronous."""
+        if uvw_m.dim() == 2:
+            uvw_m = uvw_m[None]
+        n_time, n_bl, three = uvw_m.shape
+        if three != 3:
+            raise ValueError("uvw_m must be [n_time][n_baseline][3]")
+        self._keep = [uvw_m, freq_hz]
+        rc = self._lib.gridder_bin(self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m"), n_time, n_bl,
+                                   _dev_ptr(freq_hz, torch.float64, "freq_hz"), freq_hz.numel(), _stream_ptr(stream))
+        if rc != OK:
+            raise GridderError(rc, "gridder_bin")
+
+    def grid(self, vis: torch.Tensor, weight=None, out=None, accumulate: bool = False, stream=None) -> torch.Tensor:
+        """vis float32 [...][4][2]; returns the grid float32 [4][N][N][2]; asynchronous."""
+        if out is None:
+            if accumulate:
+                raise ValueError("accumulate needs an existing grid")
+            out = torch.empty((4, self.grid_size, self.grid_size, 2), dtype=torch.float32, device=self.device)
+        rc = self._lib.gridder_grid(self._plan, _dev_ptr(vis, torch.float32, "vis"),
+                                    _dev_ptr(weight, torch.float32, "weight"),
+                                    _dev_ptr(out, torch.float32, "grid"), int(accumulate), _stream_ptr(stream))
+        if rc != OK:
+            raise GridderError(rc, "gridder_grid")
+        return out
+
+    def destroy(self) -> None:
+        if self._plan:
+            self._lib.gridder_destroy(self._plan)
+            self._plan = C.c_void_p()
+
+    # -- helpers ------------------------------------------------------------------------------
+    def stats(self) -> Stats:
+        st = _Stats()
+        rc = self._lib.gridder_get_stats(self._plan, C.byref(st))
+        if rc != OK:
+            raise GridderError(rc, "gridder_get_stats")
+        return Stats(*[int(getattr(st, f[0])) for f in _Stats._fields_])
+
+    def map(self, uvw_m: torch.Tensor, freq_hz: torch.Tensor, stream=None) -> torch.Tensor:
+        """int32 [n][6] = x0, y0, qx, qy, plane | conj << 8, dropped (the map kernel's device function)."""
+        if uvw_m.dim() == 2:
+            uvw_m = uvw_m[None]
+        n_time, n_bl, _ = uvw_m.shape
+        out = torch.empty((n_time * n_bl * freq_hz.numel(), 6), dtype=torch.int32, device=self.device)
+        rc = self._lib.gridder_map(self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m"), n_time, n_bl,
+                                   _dev_ptr(freq_hz, torch.float64, "freq_hz"), freq_hz.numel(), out.data_ptr(),
+                                   _stream_ptr(stream))
+        if rc != OK:
+            raise GridderError(rc, "gridder_map")
+        return out
+
+    def run_host(self, uvw_m, freq_hz, vis, weight, grid_out, staging: dict, stream=None) -> None:
+        """End to end with HOST tensors (pinned for speed): H2D, bin, grid, D2H, synchronise."""
+        def hp(t, dtype, what):
+            if t is None:
+                return None
+            if t.is_cuda or not t.is_contiguous() or t.dtype != dtype:
+                raise TypeError(f"{what} must be a contiguous host tensor of {dtype}")
+            return t.data_ptr()
+        if uvw_m.dim() == 2:
+            uvw_m = uvw_m[None]
+        n_time, n_bl, _ = uvw_m.shape
+        rc = self._lib.gridder_run_host(
+            self._plan, hp(uvw_m, torch.float64, "uvw_m"), n_time, n_bl, hp(freq_hz, torch.float64, "freq_hz"),
+            freq_hz.numel(), hp(vis, torch.float32, "vis"), hp(weight, torch.float32, "weight"),
+            hp(grid_out, torch.float32, "grid_out"), staging["uvw"].data_ptr(), staging["freq"].data_ptr(),
+            staging["vis"].data_ptr(), staging["weight"].data_ptr() if weight is not None else None,
+            staging["grid"].data_ptr(), _stream_ptr(stream))
+        if rc != OK:
+            raise GridderError(rc, "gridder_run_host")
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

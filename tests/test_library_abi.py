@@ -1,0 +1,67 @@
+"""CPU-side checks of the boundary: the shared library builds, loads and exports every symbol
+include/gridder.h declares; argument checks that need no device return the documented codes."""
+import ctypes as C
+import re
+from pathlib import Path
+
+import pytest
+
+ROOT = Path(__file__).resolve().parents[1]
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1003_5575_b200 import build, gridder
+    build.build()
+    return gridder.load_library()
+
+
+def test_every_declared_symbol_is_exported(lib):
+    header = (ROOT / "include" / "gridder.h").read_text()
+    declared = set(re.findall(r"GRIDDER_API\s+[\w\s\*]+?\b(gridder_\w+)\s*\(", header))
+    assert {"gridder_plan", "gridder_bin", "gridder_grid", "gridder_destroy"} <= declared
+    from paper_1003_5575_b200 import gridder
+    assert declared == set(gridder.EXPORTS)
+    for name in declared:
+        assert getattr(lib, name) is not None
+
+
+def test_version_and_strerror(lib):
+    from paper_1003_5575_b200 import gridder
+    assert re.fullmatch(r"\d+\.\d+\.\d+", gridder.version())
+    assert gridder.strerror(0) == "ok"
+    for code in range(-6, 0):
+        assert "unknown" not in gridder.strerror(code)
+    assert "unknown" in gridder.strerror(-99)
+
+
+def test_null_and_invalid_arguments_need_no_device(lib):
+    from paper_1003_5575_b200 import gridder
+    need = C.c_size_t(0)
+    assert lib.gridder_workspace_size(None, C.byref(need)) == gridder.ERR_INVALID_ARG
+    sup = (C.c_int32 * 1)(16)
+    def cfg(**kw):
+        base = dict(grid_size=256, cell_size=1.0, n_pol=4, oversample=4, n_wplanes=1, support=sup, w_max=1.0,
+                    kernel_is_complex=0, kernel=None, max_vis=1000, workspace=None, workspace_bytes=0)
+        base.update(kw)
+        return gridder._Config(*[base[f[0]] for f in gridder._Config._fields_])
+    for bad in (dict(grid_size=255), dict(grid_size=0), dict(cell_size=0.0), dict(n_pol=2), dict(oversample=0),
+                dict(n_wplanes=0), dict(max_vis=-1), dict(support=(C.c_int32 * 1)(0)),
+                dict(support=(C.c_int32 * 1)(33)), dict(support=(C.c_int32 * 1)(7), oversample=1)):
+        assert lib.gridder_workspace_size(C.byref(cfg(**bad)), C.byref(need)) == gridder.ERR_INVALID_ARG, bad
+    assert lib.gridder_workspace_size(C.byref(cfg(kernel_is_complex=1)), C.byref(need)) == gridder.ERR_UNSUPPORTED
+    plan = C.c_void_p()
+    assert lib.gridder_plan(C.byref(cfg(grid_size=255)), C.byref(plan), None) == gridder.ERR_INVALID_ARG
+    assert lib.gridder_plan(C.byref(cfg()), None, None) == gridder.ERR_INVALID_ARG
+    assert lib.gridder_bin(None, None, 1, 1, None, 1, None) == gridder.ERR_INVALID_ARG
+    assert lib.gridder_grid(None, None, None, None, 0, None) == gridder.ERR_INVALID_ARG
+    assert lib.gridder_destroy(None) == gridder.ERR_INVALID_ARG
+    assert lib.gridder_get_stats(None, None) == gridder.ERR_INVALID_ARG
+
+
+def test_binding_refuses_cpu_tensors():
+    import torch
+    from paper_1003_5575_b200 import gridder
+    with pytest.raises(RuntimeError):
+        gridder.Gridder(grid_size=64, cell_size=1.0, oversample=4, support=[8],
+                        kernel=torch.zeros(32 * 32), max_vis=10)
