@@ -136,6 +136,19 @@ GRIDDER_API int gridder_run_host(gridder_plan_t *plan, const double *h_uvw_m, in
                      const float *h_weight, float *h_grid, double *d_uvw_m, double *d_freq_hz,
                      float *d_vis, float *d_weight, float *d_grid, void *cuda_stream);
 
+/* Stage timers for the benchmark harness (PAPER.md :249 instrumented its pipeline per kernel).
+ * When enabled, gridder_bin / gridder_grid record CUDA events between their stages on the stream
+ * they run on (a few microseconds of host time per call; nothing else changes). */
+GRIDDER_API int gridder_set_profiling(gridder_plan_t *plan, int32_t enable);
+/* Mean device milliseconds per stage over the gridder_bin / gridder_grid calls made since
+ * profiling was enabled (the last 32 of each at most), HOST float [5]: map, sort, tile tables,
+ * grid kernel, flush kernel.  Synchronises on the recorded events.  A stage that has not run
+ * since then reads 0.  Enabling again resets the averages. */
+GRIDDER_API int gridder_get_stage_ms(gridder_plan_t *plan, float *ms_out);
+/* Kernel launches this plan has enqueued so far (the library's own kernels; each CUB
+ * DeviceRadixSort / DeviceScan call counts as one although it launches several). */
+GRIDDER_API int64_t gridder_launch_count(const gridder_plan_t *plan);
+
 GRIDDER_API const char *gridder_strerror(int code);
 /* cudaError_t of the most recent failing CUDA call made on behalf of `plan` (0 if none). */
 GRIDDER_API int gridder_last_cuda_error(const gridder_plan_t *plan);

@@ -183,6 +183,8 @@ int gridder_destroy(gridder_plan_t *plan) {
     Plan *p = reinterpret_cast<Plan *>(plan);
     if (!p) return GRIDDER_ERR_INVALID_ARG;
     cudaError_t e = cudaDeviceSynchronize();     // the caller may free the workspace after this
+    for (int r = 0; r < kProfRing; ++r)
+        for (int i = 0; i < 7; ++i) if (p->ev[r][i]) cudaEventDestroy(p->ev[r][i]);
     delete p;
     return e == cudaSuccess ? GRIDDER_OK : GRIDDER_ERR_CUDA;
 }
@@ -249,6 +251,53 @@ int gridder_run_host(gridder_plan_t *plan, const double *h_uvw_m, int32_t n_time
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return cuda_fail(p, e);
     return GRIDDER_OK;
+}
+
+int gridder_set_profiling(gridder_plan_t *plan, int32_t enable) {
+    Plan *p = reinterpret_cast<Plan *>(plan);
+    if (!p) return GRIDDER_ERR_INVALID_ARG;
+    if (enable && !p->ev[0][0]) {
+        for (int r = 0; r < kProfRing; ++r)
+            for (int i = 0; i < 7; ++i)
+                if (cudaEventCreate(&p->ev[r][i]) != cudaSuccess) return cuda_fail(p, cudaGetLastError());
+    }
+    p->profiling = enable != 0;
+    p->prof_bin_calls = p->prof_grid_calls = 0;
+    return GRIDDER_OK;
+}
+
+int gridder_get_stage_ms(gridder_plan_t *plan, float *ms_out) {
+    Plan *p = reinterpret_cast<Plan *>(plan);
+    if (!p || !ms_out) return GRIDDER_ERR_INVALID_ARG;
+    double sum[5] = {0, 0, 0, 0, 0};
+    const int nb = (int)(p->prof_bin_calls < kProfRing ? p->prof_bin_calls : kProfRing);
+    const int ng = (int)(p->prof_grid_calls < kProfRing ? p->prof_grid_calls : kProfRing);
+    cudaError_t e = cudaSuccess;
+    for (int r = 0; r < nb && e == cudaSuccess; ++r) {
+        e = cudaEventSynchronize(p->ev[r][3]);
+        for (int i = 0; i < 3 && e == cudaSuccess; ++i) {
+            float ms = 0.f;
+            e = cudaEventElapsedTime(&ms, p->ev[r][i], p->ev[r][i + 1]);
+            sum[i] += ms;
+        }
+    }
+    for (int r = 0; r < ng && e == cudaSuccess; ++r) {
+        e = cudaEventSynchronize(p->ev[r][6]);
+        for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+            float ms = 0.f;
+            e = cudaEventElapsedTime(&ms, p->ev[r][4 + i], p->ev[r][5 + i]);
+            sum[3 + i] += ms;
+        }
+    }
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    for (int i = 0; i < 3; ++i) ms_out[i] = nb ? (float)(sum[i] / nb) : 0.f;
+    for (int i = 3; i < 5; ++i) ms_out[i] = ng ? (float)(sum[i] / ng) : 0.f;
+    return GRIDDER_OK;
+}
+
+int64_t gridder_launch_count(const gridder_plan_t *plan) {
+    const Plan *p = reinterpret_cast<const Plan *>(plan);
+    return p ? p->n_launches : 0;
 }
 
 const char *gridder_strerror(int code) {

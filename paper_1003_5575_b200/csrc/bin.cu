@@ -257,19 +257,25 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
     // tile_start and tile_end are adjacent: [2][n_tiles]
     GR_TRY(cudaMemsetAsync(p.tile_start, 0, sizeof(uint32_t) * 2 * (size_t)p.n_tiles, s));
     uint32_t *tile_end = p.tile_start + p.n_tiles;
+    stage_mark(p, 0, s);
     if (n > 0) {
         map_kernel<<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(uvw, freq, n_tb, n_chan, make_map_params(p),
                                                                 p.keys[0], p.vals[0], p.counters);
         GR_TRY(cudaGetLastError());
+        stage_mark(p, 1, s);
         cub::DoubleBuffer<uint32_t> k(p.keys[0], p.keys[1]), v(p.vals[0], p.vals[1]);
         size_t tb = p.cub_temp_bytes;
         GR_TRY(cub::DeviceRadixSort::SortPairs(p.cub_temp, tb, k, v, n, p.key.aux_bits, p.key.total_bits, s));
         p.sorted_sel = k.selector;
+        stage_mark(p, 2, s);
+        p.n_launches += 3;
         tile_bounds_kernel<<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(p.keys[p.sorted_sel], n,
                                                                         p.key.tile_shift, p.tile_start, tile_end);
         GR_TRY(cudaGetLastError());
     } else {
         p.sorted_sel = 0;
+        stage_mark(p, 1, s);
+        stage_mark(p, 2, s);
     }
     const int nt1 = p.n_tiles + 1;
     tile_chunks_kernel<<<(nt1 + 255) / 256, 256, 0, s>>>(p.tile_start, tile_end, p.n_tiles, p.chunk,
@@ -281,6 +287,9 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
     item_fill_kernel<<<(nt1 + 255) / 256, 256, 0, s>>>(p.tile_start, tile_end, p.tile_chunks_scan, p.n_tiles,
                                                          p.chunk, p.tile_info, p.items, p.counters);
     GR_TRY(cudaGetLastError());
+    p.n_launches += 3;
+    stage_mark(p, 3, s);
+    if (p.profiling) p.prof_bin_calls++;
     return cudaSuccess;
 }
 

@@ -15,6 +15,7 @@
 
 namespace gridder {
 
+constexpr int kProfRing = 32;                     // calls remembered by the stage timers
 constexpr double kSpeedOfLight = 299792458.0;     // m/s (gridder.h: u_lambda = u_m * f / c)
 
 // Bit layout of a sort key (LSB first): qx, qy (bits_q each), drop flag, x0l, y0l (tlog each), tile.
@@ -117,7 +118,19 @@ struct Plan {
     bool binned;
     cudaStream_t last_stream;
     int last_cuda_error;
+    // harness support: stage timers and a launch counter
+    bool profiling;
+    cudaEvent_t ev[kProfRing][7];  // per call: bin: 0 map 1 sort 2 tables 3 | grid: 4 grid 5 flush 6
+    int64_t prof_bin_calls, prof_grid_calls;       // since profiling was enabled
+    int64_t n_launches;
 };
+
+// Stage timers: call j of gridder_bin / gridder_grid records into ring slot j % kProfRing.
+inline void stage_mark(Plan &p, int i, cudaStream_t s) {
+    if (!p.profiling) return;
+    const int64_t call = i < 4 ? p.prof_bin_calls : p.prof_grid_calls;
+    cudaEventRecord(p.ev[call % kProfRing][i], s);
+}
 
 // bin.cu
 cudaError_t launch_relayout(const Plan &p, cudaStream_t s);

@@ -18,7 +18,8 @@ LIB_PATH = _HERE / "libgridder.so"
 OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_WORKSPACE, ERR_CUDA, ERR_NOT_BINNED, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = ("gridder_workspace_size", "gridder_plan", "gridder_bin", "gridder_grid", "gridder_destroy",
-           "gridder_get_stats", "gridder_map", "gridder_run_host", "gridder_strerror",
+           "gridder_get_stats", "gridder_map", "gridder_run_host", "gridder_set_profiling",
+           "gridder_get_stage_ms", "gridder_launch_count", "gridder_strerror",
            "gridder_last_cuda_error", "gridder_version")
 
 
@@ -64,6 +65,10 @@ def load_library() -> C.CDLL:
         lib.gridder_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.gridder_set_profiling.argtypes = [C.c_void_p, C.c_int32]
+        lib.gridder_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+        lib.gridder_launch_count.argtypes = [C.c_void_p]
+        lib.gridder_launch_count.restype = C.c_int64
         lib.gridder_strerror.argtypes = [C.c_int]
         lib.gridder_strerror.restype = C.c_char_p
         lib.gridder_last_cuda_error.argtypes = [C.c_void_p]
@@ -185,6 +190,24 @@ class Gridder:
         if rc != OK:
             raise GridderError(rc, "gridder_get_stats")
         return Stats(*[int(getattr(st, f[0])) for f in _Stats._fields_])
+
+    def set_profiling(self, enable: bool = True) -> None:
+        rc = self._lib.gridder_set_profiling(self._plan, int(enable))
+        if rc != OK:
+            raise GridderError(rc, "gridder_set_profiling")
+
+    STAGES = ("map", "sort", "tables", "grid", "flush")
+
+    def stage_ms(self) -> dict:
+        """Device milliseconds of the last bin/grid per stage (synchronises on their events)."""
+        ms = (C.c_float * 5)()
+        rc = self._lib.gridder_get_stage_ms(self._plan, ms)
+        if rc != OK:
+            raise GridderError(rc, "gridder_get_stage_ms")
+        return dict(zip(self.STAGES, [float(x) for x in ms]))
+
+    def launch_count(self) -> int:
+        return int(self._lib.gridder_launch_count(self._plan))
 
     def map(self, uvw_m: torch.Tensor, freq_hz: torch.Tensor, stream=None) -> torch.Tensor:
         """int32 [n][6] = x0, y0, qx, qy, plane | conj << 8, dropped (the map kernel's device function)."""

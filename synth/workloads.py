@@ -100,6 +100,7 @@ class Workload:
     noise_sigma: float = 0.1
     random_weights: bool = False
     w_term: bool = False
+    band: int = 0
 
     @property
     def n_vis(self) -> int:
@@ -114,7 +115,7 @@ class Workload:
         """
         dev = torch.device(device)
         gen = torch.Generator(device=dev)
-        gen.manual_seed((SEED0 + self.cfg) * 1000 + 17 * t + 1)
+        gen.manual_seed((SEED0 + self.cfg) * 1000 + 17 * t + 1 + 100003 * self.band)
         out = torch.empty((self.n_baseline, self.n_chan, 4, 2), dtype=torch.float32, device=dev)
         scale = torch.as_tensor(self.freq / C_M_PER_S, dtype=torch.float64, device=dev)
         uvw_t = torch.as_tensor(self.uvw[t], dtype=torch.float64, device=dev)
@@ -146,7 +147,7 @@ class Workload:
             return None
         dev = torch.device(device)
         gen = torch.Generator(device=dev)
-        gen.manual_seed((SEED0 + self.cfg) * 1000 + 17 * t + 2)
+        gen.manual_seed((SEED0 + self.cfg) * 1000 + 17 * t + 2 + 100003 * self.band)
         w = torch.empty((self.n_baseline, self.n_chan), dtype=torch.float32, device=dev)
         w.normal_(1.0, 0.25, generator=gen)
         return w.clamp_(0.5, 1.5)
@@ -161,9 +162,18 @@ class Workload:
         return torch.stack([self.weight_block(t, device) for t in range(self.n_time)])
 
 
-def make_workload(cfg: int, n_time: int | None = None, n_chan: int | None = None) -> Workload:
+def config_shape(cfg: int) -> dict:
+    """The full sizes of config ``cfg``: n_ant, n_baseline, n_chan, n_time, grid, oversample, wplanes."""
+    sp = dict(_SPEC[cfg])
+    sp["n_baseline"] = sp["n_ant"] * (sp["n_ant"] - 1) // 2
+    return sp
+
+
+def make_workload(cfg: int, n_time: int | None = None, n_chan: int | None = None, band: int = 0) -> Workload:
     """Build config ``cfg``.  ``n_time`` / ``n_chan`` may shrink the sample axes (bounded CPU
-    samples of the same workload); geometry, cell size and tables stay those of the full config."""
+    samples of the same workload); geometry, cell size and tables stay those of the full config.
+    ``band`` > 0 moves the whole band up by ``band`` bandwidths (another GPU's channel block in the
+    paper's channel decomposition, PAPER.md :112-118); the cell size is fitted to that band."""
     sp = _SPEC[cfg]
     rng = np.random.default_rng(SEED0 + cfg)
     enu = _antennas(cfg, rng, sp["n_ant"])
@@ -171,7 +181,7 @@ def make_workload(cfg: int, n_time: int | None = None, n_chan: int | None = None
     dec = lat + np.deg2rad(30.0) if cfg == 3 else np.deg2rad(-27.0)
     hours = np.arange(sp["n_time"]) * sp["dt"] * 2.0 * np.pi / SIDEREAL_DAY_S
     uvw = _uvw(enu, hours, dec)
-    freq = sp["f0"] + sp["df"] * np.arange(sp["n_chan"], dtype=np.float64)
+    freq = sp["f0"] + band * sp["n_chan"] * sp["df"] + sp["df"] * np.arange(sp["n_chan"], dtype=np.float64)
     o = sp["oversample"]
     if sp["wplanes"] > 1:
         support = kernels.wplane_supports(sp["wplanes"])
@@ -199,4 +209,4 @@ def make_workload(cfg: int, n_time: int | None = None, n_chan: int | None = None
         w_max=w_max, kernel_is_complex=is_complex, cell_size=cell,
         uvw=np.ascontiguousarray(uvw[:nt]), freq=np.ascontiguousarray(freq[:nc]),
         kernel=np.ascontiguousarray(table, dtype=np.float32),
-        src_l=src_l, src_m=src_m, src_flux=flux, random_weights=(cfg == 4), w_term=(cfg == 3))
+        src_l=src_l, src_m=src_m, src_flux=flux, random_weights=(cfg == 4), w_term=(cfg == 3), band=band)

@@ -43,7 +43,8 @@ def _gridder(dev, *, N, du, O, S, table, max_vis, env=None):
 
 
 def _run(dev, uvw, freq, vis, weight, *, N, du, O, S, table, env=None, accumulate_onto=None):
-    uvw = np.ascontiguousarray(uvw, np.float64).reshape(-1, uvw.shape[-2], 3)
+    uvw = np.ascontiguousarray(uvw, np.float64)
+    uvw = uvw[None] if uvw.ndim == 2 else uvw
     n = uvw.shape[0] * uvw.shape[1] * len(freq)
     g = _gridder(dev, N=N, du=du, O=O, S=S, table=table, max_vis=max(n, 1), env=env)
     g.bin(torch.from_numpy(uvw).to(dev), torch.tensor(np.asarray(freq, np.float64), device=dev))
@@ -61,7 +62,8 @@ def _run(dev, uvw, freq, vis, weight, *, N, du, O, S, table, env=None, accumulat
 
 
 def _oracle(uvw, freq, vis, weight, *, N, du, O, S, table):
-    uvw = np.ascontiguousarray(uvw, np.float64).reshape(-1, uvw.shape[-2], 3)
+    uvw = np.ascontiguousarray(uvw, np.float64)
+    uvw = uvw[None] if uvw.ndim == 2 else uvw
     return oracle.grid_full(uvw, freq, vis, weight, grid_size=N, cell_size=du, oversample=O, support=[S],
                             kernel=np.ascontiguousarray(table, np.float32).ravel())
 
