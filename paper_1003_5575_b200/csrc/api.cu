@@ -46,7 +46,7 @@ int derive(const gridder_config *cfg, Plan &p) {
     p.cfg.support = p.support_copy;
     p.S = cfg->support[0];
     if (p.S <= 8) { p.NA = 1; p.NB = 2; } else { p.NA = 2; p.NB = 4; }
-    p.tlog = env_int("GRIDDER_TILE_LOG2", 3);
+    p.tlog = env_int("GRIDDER_TILE_LOG2", 2);
     if (p.tlog < 2 || p.tlog > 4) return GRIDDER_ERR_INVALID_ARG;
     p.T = 1 << p.tlog;
     p.ntx = (cfg->grid_size + p.T - 1) / p.T;
@@ -55,9 +55,11 @@ int derive(const gridder_config *cfg, Plan &p) {
     p.RW = p.T + 8 * p.NA - 1;
     p.RH = p.T + 4 * p.NB - 1;
     p.region_f4 = 2 * p.RW * p.RH;
-    p.chunk = env_int("GRIDDER_CHUNK", 2048);
+    p.chunk = env_int("GRIDDER_CHUNK", 4096);
     if (p.chunk < 32 || p.chunk > (1 << 20)) return GRIDDER_ERR_INVALID_ARG;
     p.warps = env_int("GRIDDER_WARPS", 0);
+    p.fold_batches = env_int("GRIDDER_FOLD_BATCHES", 4);
+    if (p.fold_batches < 1 || p.fold_batches > 64 || (p.fold_batches & (p.fold_batches - 1))) return GRIDDER_ERR_INVALID_ARG;
 
     KeyLayout k;
     k.bits_q = ceil_log2((unsigned long long)cfg->oversample);

@@ -24,8 +24,11 @@ struct Geo {
     static constexpr int T = 1 << TLOG;
     static constexpr int RW = T + SPX - 1, RH = T + SPY - 1;   // region = tile + halo
     static constexpr int CELLS = RW * RH;
-    static constexpr int STAGE_F4 = 2 * 32 * 3;                // 2 buffers x 32 records x 3 float4
-    static constexpr int WARP_F4 = 2 * CELLS + STAGE_F4;       // shared float4 per warp
+    static constexpr int HALF_SLOTS = 32 + 3;                  // (3 = the consumer's look-ahead)
+    static constexpr int HALF_SLOTS_UNUSED = 0;                  // a batch + copies of the next batch's first records
+    static constexpr int STAGE_F4 = 2 * HALF_SLOTS * 3;        // 2 halves x slots x 3 float4
+    static constexpr int RAW_F4 = 32 * 3;                      // cp.async landing buffer: one batch
+    static constexpr int WARP_F4 = 2 * CELLS + STAGE_F4 + RAW_F4;   // shared float4 per warp
 };
 
 __device__ __forceinline__ float4 ldg_stream(const float4 *p) {
@@ -40,40 +43,83 @@ __device__ __forceinline__ void stg_stream(float4 *p, const float4 &v) {
                  :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 
-// A staged record: the weighted visibility and where it goes.
-struct Rec {
-    float4 a, b;     // XX.re XX.im XY.re XY.im | YX.re YX.im YY.re YY.im, times weight
-    int coff;        // float offset of its GCF sub-table (q) in the shared table
-    int poff;        // cell offset of its patch origin in the region
+// ---- staging pipeline, three batches deep -------------------------------------------------------
+// Batch j+3: sorted (key, visibility index) loads in flight (two registers).  Batch j+2: its
+// visibilities and weights in flight as cp.async copies into the warp's raw buffer -- no register
+// holds them, so nothing is spilled while the FFMA loop runs.  Batch j+1: read back from the raw
+// buffer by its own lane, multiplied by its weight and written to the record ring while batch j is
+// being gridded.  No load is consumed in the step that issued it.
+struct KeyIdx {
+    uint32_t key, idx;
 };
 
-template <int NA, int NB, int TLOG>
-__device__ __forceinline__ Rec load_record(const GridParams &p, uint32_t e, bool valid) {
-    using G = Geo<NA, NB, TLOG>;
-    Rec r;
-    r.a = make_float4(0.f, 0.f, 0.f, 0.f);
-    r.b = r.a;
-    r.coff = 0;
-    r.poff = 0;
+__device__ __forceinline__ KeyIdx load_keyidx(const GridParams &p, uint32_t e, bool valid) {
+    KeyIdx k;
+    k.key = 0u;
+    k.idx = 0u;
     if (valid) {
-        const uint32_t key = p.keys[e];
-        const uint32_t idx = p.vals[e];
-        const uint32_t qmask = (1u << (2 * p.key.bits_q)) - 1u;
-        const uint32_t tmask = (1u << TLOG) - 1u;
-        const uint32_t x0l = (key >> p.key.aux_bits) & tmask;
-        const uint32_t y0l = (key >> (p.key.aux_bits + TLOG)) & tmask;
-        r.coff = (int)((key & qmask) * (NA * 32 * NB));
-        r.poff = (int)(y0l * G::RW + x0l);
-        const bool dropped = (key >> (2 * p.key.bits_q)) & 1u;
-        if (!dropped) {
-            const float4 a = ldg_stream(p.vis + 2 * (size_t)idx);
-            const float4 b = ldg_stream(p.vis + 2 * (size_t)idx + 1);
-            const float w = p.weight ? __ldg(p.weight + idx) : 1.0f;
-            r.a = make_float4(a.x * w, a.y * w, a.z * w, a.w * w);
-            r.b = make_float4(b.x * w, b.y * w, b.z * w, b.w * w);
-        }
+        k.key = __ldg(p.keys + e);
+        k.idx = __ldg(p.vals + e);
     }
-    return r;
+    return k;
+}
+
+__device__ __forceinline__ void cp_async_16(void *dst_smem, const void *src, bool pred) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst_smem);
+    const int n = pred ? 16 : 0;                      // 0 source bytes: the destination is zero-filled
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(d), "l"(src), "r"(n) : "memory");
+}
+
+__device__ __forceinline__ void cp_async_4(void *dst_smem, const void *src, bool pred) {
+    const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst_smem);
+    const int n = pred ? 4 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" :: "r"(d), "l"(src), "r"(n) : "memory");
+}
+
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// Starts the copies of one batch: lane's record goes to raw[lane] = {a, b, (w, -, -, -)}.
+// A lane past the end of the item, or a dropped visibility, gets zeros (and so adds nothing).
+__device__ __forceinline__ void issue_vis(const GridParams &p, float4 *raw, int lane, const KeyIdx k, bool valid) {
+    const bool dropped = (k.key >> (2 * p.key.bits_q)) & 1u;
+    const bool live = valid && !dropped;
+    const float4 *src = p.vis + 2 * (size_t)(live ? k.idx : 0u);
+    float4 *dst = raw + lane * 3;
+    cp_async_16(dst, src, live);
+    cp_async_16(dst + 1, src + 1, live);
+    if (p.weight) cp_async_4(dst + 2, p.weight + (live ? k.idx : 0u), live);
+    cp_async_commit();
+}
+
+// Moves a landed batch of `cnt` <= 32 records from the raw buffer into `half` of the ring in the
+// consumer's format {w*a, w*b, (table offset, origin)}; lanes past the end write a record that adds
+// nothing (zero visibility, the last record's origin) so that the consumer can work in fours.  The
+// first records are repeated in the extension slots of the other half, where the consumer's
+// look-ahead finds them without wrapping.
+template <int NA, int NB, int TLOG>
+__device__ __forceinline__ void stage_write(const GridParams &p, const float4 *raw, float4 *half, float4 *other_ext,
+                                            int lane, int cnt, uint32_t key) {
+    using G = Geo<NA, NB, TLOG>;
+    const uint32_t qmask = (1u << (2 * p.key.bits_q)) - 1u;
+    const uint32_t tmask = (1u << TLOG) - 1u;
+    const uint32_t x0l = (key >> p.key.aux_bits) & tmask;
+    const uint32_t y0l = (key >> (p.key.aux_bits + TLOG)) & tmask;
+    const int coff = (int)((key & qmask) * (NA * 32 * NB * (uint32_t)sizeof(float)));
+    const int poff = (int)(y0l * G::RW + x0l);
+    const int last_poff = __shfl_sync(0xffffffffu, poff, cnt - 1);
+    const bool pad = lane >= cnt;
+    const float4 ra = raw[lane * 3], rb = raw[lane * 3 + 1];
+    const float w = p.weight ? raw[lane * 3 + 2].x : 1.0f;
+    const float4 a = make_float4(ra.x * w, ra.y * w, ra.z * w, ra.w * w);
+    const float4 b = make_float4(rb.x * w, rb.y * w, rb.z * w, rb.w * w);
+    const float4 m = make_float4(__int_as_float(pad ? 0 : coff), __int_as_float(pad ? last_poff : poff), 0.f, 0.f);
+    float4 *slot = half + lane * 3;
+    slot[0] = a; slot[1] = b; slot[2] = m;
+    if (lane < 3) {
+        float4 *e = other_ext + lane * 3;
+        e[0] = a; e[1] = b; e[2] = m;
+    }
 }
 
 template <int NB> struct CoefVec;
@@ -91,6 +137,27 @@ template <> struct CoefVec<2> {
         c[0] = v.x; c[1] = v.y;
     }
 };
+
+// One staged record in registers: the weighted visibility (broadcast loads) and this lane's taps.
+template <int NA, int NB>
+struct RecRegs {
+    float4 va, vb;
+    CoefVec<NB> c[NA];
+    // `coff` = table byte offset of the record in `slot`, loaded one record earlier (load_meta), so
+    // that no address here waits on a load issued in the same step.
+    __device__ __forceinline__ void fetch(const float4 *slot, const int coff, const char *coef_lane) {
+        va = slot[0];
+        vb = slot[1];
+        const float *cp = reinterpret_cast<const float *>(coef_lane + coff);
+#pragma unroll
+        for (int a = 0; a < NA; ++a) c[a].load(cp + a * 32 * NB);
+    }
+};
+
+__device__ __forceinline__ int2 load_meta(const float4 *slot) {
+    const float2 m = *reinterpret_cast<const float2 *>(slot + 2);
+    return make_int2(__float_as_int(m.x), __float_as_int(m.y));
+}
 
 // Two-level accumulation: the register patch holds a short FP32 chain (one run
 // of equal patch origins, at most 64 entries); it is then ADDED to the shared region and cleared.
@@ -113,24 +180,42 @@ __device__ __forceinline__ void fold_patch(float4 *regA, float4 *regB, int base,
         }
 }
 
+template <int NA, int NB, int RW>
+__device__ __forceinline__ void consume(const RecRegs<NA, NB> &R, const int poff, int &cur, float4 *regA,
+                                        float4 *regB, int lane_cell, float (&acc)[NA][NB][8]) {
+    if (poff != cur) {                                      // warp-uniform
+        if (cur >= 0) fold_patch<NA, NB, RW>(regA, regB, cur + lane_cell, acc);
+        cur = poff;
+    }
+    const float v[8] = {R.va.x, R.va.y, R.va.z, R.va.w, R.vb.x, R.vb.y, R.vb.z, R.vb.w};
+#pragma unroll
+    for (int a = 0; a < NA; ++a)
+#pragma unroll
+        for (int b = 0; b < NB; ++b)
+#pragma unroll
+            for (int k = 0; k < 8; ++k) acc[a][b][k] = fmaf(R.c[a].c[b], v[k], acc[a][b][k]);
+}
+
 template <int NA, int NB, int TLOG, int WARPS>
 __global__ void __launch_bounds__(WARPS * 32, 1) grid_kernel(const GridParams p) {
     using G = Geo<NA, NB, TLOG>;
     extern __shared__ float4 smem[];
     float4 *coef4 = smem;
-    const float *coef = reinterpret_cast<const float *>(smem);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float4 *region = smem + p.coef_f4 + warp * G::WARP_F4;     // plane A then plane B
     float4 *regA = region, *regB = region + G::CELLS;
-    float4 *stage = region + 2 * G::CELLS;
+    float4 *stage = region + 2 * G::CELLS;                     // record ring: 2 halves x 35 slots x 3 float4
+    float4 *raw = stage + G::STAGE_F4;                         // cp.async landing buffer
 
     for (int i = threadIdx.x; i < p.coef_f4; i += WARPS * 32) coef4[i] = p.coef[i];
-    for (int i = lane; i < 2 * G::CELLS; i += 32) region[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    // the ring is cleared too: records are fetched one ahead, also past the end of an item, and
+    // whatever a slot holds must be a valid table offset
+    for (int i = lane; i < G::WARP_F4; i += 32) region[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     __syncthreads();
 
     const unsigned int n_items = p.counters_ro->n_items;
     const int lane_cell = (lane >> 3) * G::RW + (lane & 7);      // tap (a=0, b=0) of this lane
-    const float *coef_lane = coef + lane * NB;
+    const char *coef_lane = reinterpret_cast<const char *>(smem) + lane * NB * sizeof(float);
 
     float acc[NA][NB][8];
 #pragma unroll
@@ -147,54 +232,72 @@ __global__ void __launch_bounds__(WARPS * 32, 1) grid_kernel(const GridParams p)
         if (item >= n_items) break;
         const WorkItem wi = p.items[item];
         const int len = (int)wi.len;
+
         const int n_batches = (len + 31) >> 5;
 
-        Rec rec = load_record<NA, NB, TLOG>(p, wi.start + lane, lane < len);
-        stage[lane * 3 + 0] = rec.a;
-        stage[lane * 3 + 1] = rec.b;
-        stage[lane * 3 + 2] = make_float4(__int_as_float(rec.coff), __int_as_float(rec.poff), 0.f, 0.f);
+        // prologue: batch 0 staged, batch 1's visibilities (cp.async) and batch 2's keys in flight
+        uint32_t key_landing;                                   // key of the batch in the raw buffer
+        KeyIdx ki_next;                                         // batch after that
+        {
+            const KeyIdx k0 = load_keyidx(p, wi.start + lane, lane < len);
+            const KeyIdx k1 = load_keyidx(p, wi.start + 32 + lane, 32 + lane < len);
+            ki_next = load_keyidx(p, wi.start + 64 + lane, 64 + lane < len);
+            issue_vis(p, raw, lane, k0, lane < len);
+            cp_async_wait_all();
+            stage_write<NA, NB, TLOG>(p, raw, stage, stage + (G::HALF_SLOTS + 32) * 3, lane, min(32, len), k0.key);
+            issue_vis(p, raw, lane, k1, 32 + lane < len);
+            key_landing = k1.key;
+        }
         __syncwarp();
-        if (n_batches > 1) rec = load_record<NA, NB, TLOG>(p, wi.start + 32 + lane, 32 + lane < len);
 
+        // The loop body handles four records so that every prefetched (table offset, origin) pair
+        // lands in a register nobody else is still reading: no copy waits on a load just issued.
+        RecRegs<NA, NB> A, B;
+        int2 mA = load_meta(stage);
+        A.fetch(stage, mA.x, coef_lane);
+        int2 mB = load_meta(stage + 3);
         int cur = -1;
-        for (int bi = 0; bi < n_batches; ++bi) {
-            const float4 *st = stage + (bi & 1) * 96;
-            const int cnt = min(32, len - bi * 32);
-            for (int r = 0; r < cnt; ++r) {
-                const float4 meta = st[r * 3 + 2];
-                const int coff = __float_as_int(meta.x), poff = __float_as_int(meta.y);
-                if (poff != cur) {                                  // warp-uniform
-                    if (cur >= 0) fold_patch<NA, NB, G::RW>(regA, regB, cur + lane_cell, acc);
-                    cur = poff;
-                }
-                const float4 va = st[r * 3 + 0], vb = st[r * 3 + 1];
-                const float v[8] = {va.x, va.y, va.z, va.w, vb.x, vb.y, vb.z, vb.w};
-                CoefVec<NB> c[NA];
-#pragma unroll
-                for (int a = 0; a < NA; ++a) c[a].load(coef_lane + coff + a * 32 * NB);
-#pragma unroll
-                for (int a = 0; a < NA; ++a)
-#pragma unroll
-                    for (int b = 0; b < NB; ++b)
-#pragma unroll
-                        for (int k = 0; k < 8; ++k) acc[a][b][k] = fmaf(c[a].c[b], v[k], acc[a][b][k]);
-            }
-            if ((bi & 1) && cur >= 0) {        // bound the register chain to 64 terms
+        for (int jb = 0; jb < n_batches; ++jb) {
+            float4 *half = stage + (jb & 1) * (G::HALF_SLOTS * 3);
+            float4 *other = stage + ((jb + 1) & 1) * (G::HALF_SLOTS * 3);
+            const int n_quads = (min(32, len - 32 * jb) + 3) >> 2;
+            const float4 *sp = half;
+            auto quad_step = [&]() {
+                // in: A = record 0 (origin mA.y), mB = meta of record 1
+                const int2 mC = load_meta(sp + 6);
+                B.fetch(sp + 3, mB.x, coef_lane);
+                consume<NA, NB, G::RW>(A, mA.y, cur, regA, regB, lane_cell, acc);
+                const int2 mD = load_meta(sp + 9);
+                A.fetch(sp + 6, mC.x, coef_lane);
+                consume<NA, NB, G::RW>(B, mB.y, cur, regA, regB, lane_cell, acc);
+                mA = load_meta(sp + 12);
+                B.fetch(sp + 9, mD.x, coef_lane);
+                consume<NA, NB, G::RW>(A, mC.y, cur, regA, regB, lane_cell, acc);
+                mB = load_meta(sp + 15);
+                A.fetch(sp + 12, mA.x, coef_lane);
+                consume<NA, NB, G::RW>(B, mD.y, cur, regA, regB, lane_cell, acc);
+                sp += 12;
+            };
+            const int first = min(n_quads, 4);
+            for (int i = 0; i < first; ++i) quad_step();
+            // mid-batch (warp-uniform): bound the register chain, then move the staging pipeline on
+            if ((jb & p.fold_mask) == p.fold_mask && cur >= 0) {
                 fold_patch<NA, NB, G::RW>(regA, regB, cur + lane_cell, acc);
                 cur = -1;
             }
-            if (bi + 1 < n_batches) {
+            if (jb + 1 < n_batches) {
+                __syncwarp();                                   // the other half was last read in batch jb-1
+                cp_async_wait_all();
+                stage_write<NA, NB, TLOG>(p, raw, other, half + 32 * 3, lane, min(32, len - 32 * (jb + 1)), key_landing);
                 __syncwarp();
-                float4 *sn = stage + ((bi + 1) & 1) * 96;
-                sn[lane * 3 + 0] = rec.a;
-                sn[lane * 3 + 1] = rec.b;
-                sn[lane * 3 + 2] = make_float4(__int_as_float(rec.coff), __int_as_float(rec.poff), 0.f, 0.f);
-                __syncwarp();
-                if (bi + 2 < n_batches) {
-                    const int off = (bi + 2) * 32 + lane;
-                    rec = load_record<NA, NB, TLOG>(p, wi.start + off, off < len);
+                const int o2 = (jb + 2) * 32 + lane, o3 = (jb + 3) * 32 + lane;
+                if ((jb + 2) * 32 < len) {
+                    issue_vis(p, raw, lane, ki_next, o2 < len);
+                    key_landing = ki_next.key;
+                    ki_next = load_keyidx(p, wi.start + o3, o3 < len);
                 }
             }
+            for (int i = 4; i < n_quads; ++i) quad_step();
         }
         // fold the last patch in, then move the region to this item's partial and clear it
         if (cur >= 0) fold_patch<NA, NB, G::RW>(regA, regB, cur + lane_cell, acc);
@@ -260,7 +363,7 @@ size_t grid_smem_bytes(int NA, int NB, int tlog, int oversample, int warps) {
     const int T = 1 << tlog;
     const int RW = T + 8 * NA - 1, RH = T + 4 * NB - 1;
     const size_t coef = (size_t)oversample * oversample * NA * NB * 32 * sizeof(float);
-    const size_t per_warp = (size_t)(2 * RW * RH + 2 * 32 * 3) * sizeof(float4);
+    const size_t per_warp = (size_t)(2 * RW * RH + 2 * (32 + 3) * 3 + 32 * 3) * sizeof(float4);   // Geo::WARP_F4
     return coef + per_warp * warps;
 }
 
@@ -348,6 +451,7 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
     gp.partials = p.partials;
     gp.coef_f4 = p.coef_f4;
     gp.key = p.key;
+    gp.fold_mask = p.fold_batches - 1;
     gfn<<<p.n_sm, p.warps * 32, p.smem_bytes, s>>>(gp);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;

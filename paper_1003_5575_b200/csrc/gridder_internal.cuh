@@ -77,6 +77,7 @@ struct GridParams {
     const float4 *coef;            // re-laid table: [O*O][NA][32 lanes][NB] floats
     float4 *partials;              // [item][2][RH*RW] float4
     int32_t coef_f4;               // float4 count of the table
+    int32_t fold_mask;             // register chains are folded every (fold_mask + 1) batches of 32
     KeyLayout key;
 };
 
@@ -97,6 +98,7 @@ struct Plan {
     int32_t S, NA, NB, tlog, T, ntx, nty, n_tiles;
     int32_t RW, RH, region_f4;     // region_f4 = 2*RH*RW float4 per work item
     int32_t chunk;                 // K
+    int32_t fold_batches;          // longest FP32 register chain, in batches of 32 entries (power of 2)
     int32_t warps, n_sm, smem_bytes;
     int64_t max_items;
     KeyLayout key;
