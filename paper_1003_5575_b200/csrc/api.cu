@@ -30,7 +30,7 @@ int derive(const gridder_config *cfg, Plan &p) {
     if (cfg->grid_size < 2 || (cfg->grid_size & 1) || cfg->grid_size > 32768) return GRIDDER_ERR_INVALID_ARG;
     if (!(cfg->cell_size > 0.0) || cfg->n_pol != 4) return GRIDDER_ERR_INVALID_ARG;
     if (cfg->oversample < 1 || cfg->oversample > 64) return GRIDDER_ERR_INVALID_ARG;
-    if (cfg->n_wplanes < 1 || cfg->n_wplanes > 64 || !cfg->support) return GRIDDER_ERR_INVALID_ARG;
+    if (cfg->n_wplanes < 1 || cfg->n_wplanes > kMaxPlanes || !cfg->support) return GRIDDER_ERR_INVALID_ARG;
     if (cfg->max_vis < 0 || cfg->max_vis > 0xFFFFFFF0ll) return GRIDDER_ERR_INVALID_ARG;
     for (int i = 0; i < cfg->n_wplanes; ++i) {
         const int s = cfg->support[i];
@@ -38,44 +38,80 @@ int derive(const gridder_config *cfg, Plan &p) {
         if (s > cfg->grid_size) return GRIDDER_ERR_INVALID_ARG;
     }
     if (cfg->n_wplanes > 1 && !(cfg->w_max > 0.0)) return GRIDDER_ERR_INVALID_ARG;
-    // this build: one real table, support <= 16 (w-planes / complex tables: DESIGN.md section 9)
-    if (cfg->n_wplanes != 1 || cfg->kernel_is_complex || cfg->support[0] > 16) return GRIDDER_ERR_UNSUPPORTED;
 
     p.cfg = *cfg;
     memcpy(p.support_copy, cfg->support, sizeof(int32_t) * cfg->n_wplanes);
     p.cfg.support = p.support_copy;
-    p.S = cfg->support[0];
-    if (p.S <= 8) { p.NA = 1; p.NB = 2; } else { p.NA = 2; p.NB = 4; }
+    const bool cplx = cfg->kernel_is_complex != 0;
+    // fast path: one real table with S <= 16 (shared-memory table, 32-bit sort values)
+    p.mode = cplx ? 2 : ((cfg->n_wplanes == 1 && cfg->support[0] <= 16 && !env_int("GRIDDER_FORCE_GENERAL", 0)) ? 0 : 1);
     p.tlog = env_int("GRIDDER_TILE_LOG2", 2);
     if (p.tlog < 2 || p.tlog > 4) return GRIDDER_ERR_INVALID_ARG;
     p.T = 1 << p.tlog;
     p.ntx = (cfg->grid_size + p.T - 1) / p.T;
     p.nty = p.ntx;
     p.n_tiles = p.ntx * p.nty;
-    p.RW = p.T + 8 * p.NA - 1;
-    p.RH = p.T + 4 * p.NB - 1;
-    p.region_f4 = 2 * p.RW * p.RH;
+
+    // patch classes in use (ascending), and each plane's slot and table offset
+    int slot_of_class[kMaxClasses] = {-1, -1, -1};
+    bool used[kMaxClasses] = {false, false, false};
+    for (int i = 0; i < cfg->n_wplanes; ++i) {
+        const int s = cfg->support[i];
+        used[s <= 8 ? 0 : (s <= 16 ? 1 : 2)] = true;
+    }
+    p.n_cls = 0;
+    p.region_f4 = 0;
+    for (int c = 0; c < kMaxClasses; ++c) {
+        if (!used[c]) continue;
+        ClassGeo g;
+        memset(&g, 0, sizeof(g));
+        g.NA = c == 0 ? 1 : 2;
+        g.NB = c == 0 ? 2 : 4;
+        g.nsub = c == 2 ? 2 : 1;
+        g.SP = 8 * g.NA * g.nsub;
+        g.RW = g.RH = p.T + g.SP - 1;
+        g.sub_bytes = g.NA * g.NB * 32 * (cplx ? 8 : 4);
+        slot_of_class[c] = p.n_cls;
+        p.cls[p.n_cls++] = g;
+        if (2 * g.RW * g.RH > p.region_f4) p.region_f4 = 2 * g.RW * g.RH;
+    }
+    size_t off = 0;
+    const size_t oo = (size_t)cfg->oversample * cfg->oversample;
+    for (int i = 0; i < cfg->n_wplanes; ++i) {
+        const int s = cfg->support[i];
+        p.plane_slot[i] = slot_of_class[s <= 8 ? 0 : (s <= 16 ? 1 : 2)];
+        const ClassGeo &g = p.cls[p.plane_slot[i]];
+        p.plane_off256[i] = (uint32_t)(off / 256);
+        off += (size_t)g.nsub * g.nsub * oo * g.sub_bytes;
+    }
+    if (off >= (1ull << 31)) return GRIDDER_ERR_UNSUPPORTED;       // table offsets are 32-bit byte offsets
+    p.coef_bytes = off;
+
     p.chunk = env_int("GRIDDER_CHUNK", 4096);
     if (p.chunk < 32 || p.chunk > (1 << 20)) return GRIDDER_ERR_INVALID_ARG;
-    p.warps = env_int("GRIDDER_WARPS", 0);
+    p.warps_forced = env_int("GRIDDER_WARPS", 0);
     p.fold_batches = env_int("GRIDDER_FOLD_BATCHES", 4);
     if (p.fold_batches < 1 || p.fold_batches > 64 || (p.fold_batches & (p.fold_batches - 1))) return GRIDDER_ERR_INVALID_ARG;
 
     KeyLayout k;
     k.bits_q = ceil_log2((unsigned long long)cfg->oversample);
     k.tlog = p.tlog;
-    k.aux_bits = 2 * k.bits_q + 1;
-    k.tile_shift = k.aux_bits + 2 * k.tlog;
-    k.tile_bits = ceil_log2((unsigned long long)p.n_tiles);
+    k.aux_bits = p.mode == 0 ? 2 * k.bits_q + 1 : 0;
+    k.plane_shift = k.aux_bits + 2 * k.tlog;
+    k.plane_bits = cfg->n_wplanes > 1 ? ceil_log2((unsigned long long)cfg->n_wplanes) : 0;
+    k.tile_bits = ceil_log2((unsigned long long)p.n_tiles * p.n_cls);
     if (k.tile_bits < 1) k.tile_bits = 1;
+    // sorting on the plane inside a tile only helps table locality: dropped when the key is full
+    if (k.plane_shift + k.plane_bits + k.tile_bits > 32) k.plane_bits = 0;
+    k.tile_shift = k.plane_shift + k.plane_bits;
     k.total_bits = k.tile_shift + k.tile_bits;
     if (k.total_bits > 32) return GRIDDER_ERR_UNSUPPORTED;
     p.key = k;
 
     const int64_t n = cfg->max_vis;
-    int64_t occ = n < p.n_tiles ? n : p.n_tiles;
+    const int64_t n_vtiles = (int64_t)p.n_tiles * p.n_cls;
+    int64_t occ = n < n_vtiles ? n : n_vtiles;
     p.max_items = occ + n / p.chunk + 1;
-    p.coef_f4 = cfg->oversample * cfg->oversample * p.NA * p.NB * 32 / 4;
     return GRIDDER_OK;
 }
 
@@ -84,21 +120,31 @@ cudaError_t carve(Plan &p, char *base) {
     size_t off = 0;
     auto take = [&](size_t bytes) { char *ptr = base ? base + off : nullptr; off += align_up(bytes); return ptr; };
     const size_t n = (size_t)(p.cfg.max_vis > 0 ? p.cfg.max_vis : 1);
+    const size_t n_vtiles = (size_t)p.n_tiles * p.n_cls;
+    const size_t val_bytes = p.mode == 0 ? sizeof(uint32_t) : sizeof(unsigned long long);
     for (int i = 0; i < 2; ++i) p.keys[i] = (uint32_t *)take(n * sizeof(uint32_t));
-    for (int i = 0; i < 2; ++i) p.vals[i] = (uint32_t *)take(n * sizeof(uint32_t));
+    for (int i = 0; i < 2; ++i) p.vals[i] = (void *)take(n * val_bytes);
     size_t t1 = 0, t2 = 0;
-    cudaError_t e = sort_temp_bytes((int64_t)n, p.key.aux_bits, p.key.total_bits, &t1);
-    if (e == cudaSuccess) e = scan_temp_bytes(p.n_tiles + 1, &t2);
+    cudaError_t e = sort_temp_bytes((int64_t)n, p.key.aux_bits, p.key.total_bits, p.mode != 0, &t1);
+    if (e == cudaSuccess) e = scan_temp_bytes((int64_t)n_vtiles + 1, &t2);
+    if (e == cudaErrorNoDevice || e == cudaErrorInsufficientDriver || e == cudaErrorInvalidDevice) {
+        // no GPU on this machine (size query only): CUB cannot be asked, so report a generous bound
+        (void)cudaGetLastError();
+        t1 = ((size_t)32 << 20) + n / 2;
+        t2 = (size_t)1 << 20;
+        e = cudaSuccess;
+    }
     if (e != cudaSuccess) return e;
     p.cub_temp_bytes = align_up(t1 > t2 ? t1 : t2);
     p.cub_temp = take(p.cub_temp_bytes);
-    p.tile_start = (uint32_t *)take(sizeof(uint32_t) * 2 * (size_t)p.n_tiles);        // [start | end]
-    p.tile_chunks = (unsigned long long *)take(sizeof(unsigned long long) * ((size_t)p.n_tiles + 1));
-    p.tile_chunks_scan = (unsigned long long *)take(sizeof(unsigned long long) * ((size_t)p.n_tiles + 1));
-    p.tile_info = (TileInfo *)take(sizeof(TileInfo) * (size_t)p.n_tiles);
+    p.freq_scale = (double *)take(sizeof(double) * kMaxChannels);
+    p.tile_start = (uint32_t *)take(sizeof(uint32_t) * 2 * n_vtiles);        // [start | end]
+    p.tile_chunks = (unsigned long long *)take(sizeof(unsigned long long) * (n_vtiles + 1));
+    p.tile_chunks_scan = (unsigned long long *)take(sizeof(unsigned long long) * (n_vtiles + 1));
+    p.tile_info = (TileInfo *)take(sizeof(TileInfo) * n_vtiles);
     p.items = (WorkItem *)take(sizeof(WorkItem) * (size_t)p.max_items);
     p.partials = (float4 *)take(sizeof(float4) * (size_t)p.region_f4 * (size_t)p.max_items);
-    p.coef = (float4 *)take(sizeof(float4) * (size_t)p.coef_f4);
+    p.coef = (float4 *)take(p.coef_bytes);
     p.counters = (Counters *)take(sizeof(Counters));
     p.workspace_needed = off;
     return cudaSuccess;
@@ -157,6 +203,7 @@ int gridder_bin(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32
     const int64_t n = (int64_t)n_time * n_baseline * n_chan;
     if (n > 0 && (!uvw_m || !freq_hz)) return GRIDDER_ERR_INVALID_ARG;
     if (n > p->cfg.max_vis) return GRIDDER_ERR_CAPACITY;
+    if (n_chan > kMaxChannels) return GRIDDER_ERR_UNSUPPORTED;
     p->binned = false;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     cudaError_t e = launch_bin(*p, uvw_m, n_time, n_baseline, freq_hz, n_chan, s);
@@ -203,15 +250,15 @@ int gridder_get_stats(gridder_plan_t *plan, gridder_stats *out) {
     out->n_vis = p->n_vis;
     out->n_dropped = (int64_t)c.n_dropped;
     out->n_entries = p->n_vis - (int64_t)c.n_dropped;
-    out->vis_taps = out->n_entries * (int64_t)p->S * p->S;
+    out->vis_taps = (int64_t)c.vis_taps;
     out->n_tiles = p->n_tiles;
-    out->n_tiles_occupied = c.n_occupied;
+    out->n_tiles_occupied = c.n_occupied;      /* (class, tile) pairs when several patch classes are in use */
     out->max_tile_load = c.max_tile_load;
     out->n_work_items = c.n_items;
     out->tile_size = p->T;
-    out->patch_size = 8 * p->NA;
+    out->patch_size = p->cls[p->n_cls - 1].SP;
     out->chunk_size = p->chunk;
-    out->grid_warps_per_sm = p->warps;
+    out->grid_warps_per_sm = p->cls[p->n_cls - 1].warps;
     return GRIDDER_OK;
 }
 

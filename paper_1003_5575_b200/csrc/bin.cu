@@ -5,37 +5,57 @@
 #include <cub/device/device_scan.cuh>
 #include <cub/util_type.cuh>
 
+#include <cstring>
+
 #include "gridder_internal.cuh"
 
 namespace gridder {
 
 // ------------------------------------------------------------------------------------------
-// GCF table re-layout: user table K[jy][jx] ([S*O]^2) -> coef[q = qy*O + qx][a][lane][b], the order
-// the grid kernel's lanes read it in (one vector load per lane per column block a).  Lane
-// (rq = lane >> 3, c8 = lane & 7) owns taps ty = rq + 4 b, tx = c8 + 8 a; taps beyond S are zero
-// (the patch is padded to 8 NA x 4 NB cells).
+// GCF table re-layout, one launch per w-plane: user table K[jy][jx] ([S*O]^2 samples, float or
+// float pairs) -> coef[sub = sy*nsub + sx][q = qy*O + qx][a][lane][b], the order the grid kernel's
+// lanes read it in (one vector load per lane per column block a).  Lane (rq = lane >> 3,
+// c8 = lane & 7) owns taps ty = SPY*sy + rq + 4 b, tx = SPX*sx + c8 + 8 a of sub-patch (sy, sx);
+// taps beyond S are zero (the patch is padded to 8 NA nsub x 4 NB nsub cells).
 // ------------------------------------------------------------------------------------------
 __global__ void relayout_kernel(const float *__restrict__ table, float *__restrict__ coef, int S, int O,
-                                int NA, int NB) {
-    const int total = O * O * NA * 32 * NB;
+                                int NA, int NB, int nsub, int cplx) {
+    const int E = cplx ? 2 : 1;
+    const int total = nsub * nsub * O * O * NA * 32 * NB;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < total; i += gridDim.x * blockDim.x) {
-        int b = i % NB;
-        int lane = (i / NB) % 32;
-        int a = (i / (NB * 32)) % NA;
-        int q = i / (NB * 32 * NA);
-        int qy = q / O, qx = q % O;
-        int ty = (lane >> 3) + 4 * b, tx = (lane & 7) + 8 * a;
-        float v = 0.f;
-        if (ty < S && tx < S) v = table[(size_t)(qy + ty * O) * (S * O) + (qx + tx * O)];
-        coef[i] = v;
+        int r = i;
+        const int b = r % NB; r /= NB;
+        const int lane = r % 32; r /= 32;
+        const int a = r % NA; r /= NA;
+        const int q = r % (O * O); r /= (O * O);
+        const int sub = r;
+        const int qy = q / O, qx = q % O;
+        const int ty = 4 * NB * (sub / nsub) + (lane >> 3) + 4 * b;
+        const int tx = 8 * NA * (sub % nsub) + (lane & 7) + 8 * a;
+        for (int e = 0; e < E; ++e) {
+            float v = 0.f;
+            if (ty < S && tx < S) v = table[((size_t)(qy + ty * O) * (S * O) + (qx + tx * O)) * E + e];
+            coef[(size_t)i * E + e] = v;
+        }
     }
 }
 
 cudaError_t launch_relayout(const Plan &p, cudaStream_t s) {
-    const int total = p.coef_f4 * 4;
-    relayout_kernel<<<(total + 255) / 256, 256, 0, s>>>((const float *)p.cfg.kernel, (float *)p.coef,
-                                                         p.S, p.cfg.oversample, p.NA, p.NB);
-    return cudaGetLastError();
+    const int O = p.cfg.oversample;
+    const int E = p.cfg.kernel_is_complex ? 2 : 1;
+    size_t in_off = 0;
+    for (int pl = 0; pl < p.cfg.n_wplanes; ++pl) {
+        const ClassGeo &g = p.cls[p.plane_slot[pl]];
+        const int S = p.support_copy[pl];
+        const int total = g.nsub * g.nsub * O * O * g.NA * 32 * g.NB;
+        float *out = reinterpret_cast<float *>(reinterpret_cast<char *>(p.coef) + (size_t)p.plane_off256[pl] * 256);
+        relayout_kernel<<<(total + 255) / 256, 256, 0, s>>>((const float *)p.cfg.kernel + in_off, out, S, O, g.NA,
+                                                             g.NB, g.nsub, p.cfg.kernel_is_complex ? 1 : 0);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        in_off += (size_t)S * O * S * O * E;
+    }
+    return cudaSuccess;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -50,103 +70,168 @@ struct AxisMap {
     bool far;       // hopelessly off the grid
 };
 
-__device__ __forceinline__ long long floor_div_ll(long long a, long long b) {
-    long long q = a / b;
-    if ((a % b != 0) && (a < 0)) q -= 1;
-    return q;
+__device__ __noinline__ void map_axis_wide(double r, int S, int O, long long *x0, int *q) {
+    // the same algebra in 64 bits, for positions far outside any grid (always dropped, but the
+    // test interface reports them)
+    const long long X = (long long)r, OO = O;
+    const long long A = X - ((long long)S * OO) / 2;
+    const long long n = A + OO - 1;
+    long long d = n / OO;
+    if ((n % OO != 0) && (n < 0)) d -= 1;
+    *x0 = d;
+    *q = (int)(d * OO - A);
 }
 
-__device__ __forceinline__ AxisMap map_axis(double coord_lambda, const MapParams &p) {
+__device__ __forceinline__ AxisMap map_axis(double coord_lambda, const MapParams &p, int S) {
     AxisMap m;
     const double a = __ddiv_rn(coord_lambda, p.cell_size);
     const double g = __dadd_rn(a, (double)(p.n_grid / 2));
     const double h = __dmul_rn(g, (double)p.oversample);
     const double r = floor(__dadd_rn(h, 0.5));
-    m.far = !(r > -1.0e15 && r < 1.0e15);
-    const long long X = m.far ? 0 : (long long)r;
-    const long long A = X - (long long)p.half_so;
-    const long long O = p.oversample;
-    m.x0 = floor_div_ll(A + O - 1, O);
-    m.q = (int)(m.x0 * O - A);
-    if (m.far) { m.x0 = -(1ll << 61); m.q = 0; }
+    const int O = p.oversample;
+    m.far = false;
+    if (r > -1073741824.0 && r < 1073741824.0) {
+        // |X| < 2^30 sub-cells (N*O <= 2^21 for every accepted plan): 32-bit integer algebra
+        const int X = (int)r;
+        const int A = X - (S * O) / 2;
+        const int n = A + O - 1;              // x0 = ceil(A / O) = floor((A + O - 1) / O)
+        int x0 = n / O;
+        if ((n % O != 0) && (n < 0)) x0 -= 1;
+        m.x0 = x0;
+        m.q = x0 * O - A;
+    } else if (r > -1.0e15 && r < 1.0e15) {
+        map_axis_wide(r, S, O, &m.x0, &m.q);
+    } else {
+        m.far = true;
+        m.x0 = -(1ll << 61);
+        m.q = 0;
+    }
     return m;
 }
 
 struct VisMap {
     long long x0, y0;
-    int qx, qy;
+    int qx, qy, plane, conj, S;
     bool dropped;
 };
 
-__device__ __forceinline__ VisMap map_vis(double u_m, double v_m, double s, const MapParams &p) {
+__device__ __forceinline__ VisMap map_vis(double u_m, double v_m, double w_m, double s, const MapParams &p) {
     const double ul = __dmul_rn(u_m, s), vl = __dmul_rn(v_m, s);
-    const AxisMap mx = map_axis(ul, p), my = map_axis(vl, p);
     VisMap m;
+    m.plane = 0;
+    m.conj = 0;
+    if (p.n_planes > 1 || p.is_complex) {
+        const double wl = __dmul_rn(w_m, s);
+        if (p.n_planes > 1) {
+            const double fp = floor(__dmul_rn(__ddiv_rn(fabs(wl), p.w_max), (double)p.n_planes));
+            m.plane = (fp >= (double)(p.n_planes - 1)) ? p.n_planes - 1 : (int)fp;
+        }
+        m.conj = (p.is_complex && wl < 0.0) ? 1 : 0;
+    }
+    m.S = p.support[m.plane];
+    const AxisMap mx = map_axis(ul, p, m.S), my = map_axis(vl, p, m.S);
     m.x0 = mx.x0; m.y0 = my.x0; m.qx = mx.q; m.qy = my.q;
-    const long long N = p.n_grid, S = p.support;
+    const long long N = p.n_grid, S = m.S;
     m.dropped = mx.far || my.far || m.x0 < 0 || m.x0 + S > N || m.y0 < 0 || m.y0 + S > N;
     return m;
 }
 
-__global__ void __launch_bounds__(256) map_kernel(const double *__restrict__ uvw,
-                                                   const double *__restrict__ freq, long long n_tb,
-                                                   int n_chan, MapParams p, uint32_t *__restrict__ keys,
-                                                   uint32_t *__restrict__ vals, Counters *counters) {
-    const long long n = n_tb * n_chan;
+// s[f] = freq[f] / c, once per gridder_bin
+__global__ void freq_scale_kernel(const double *__restrict__ freq, int n_chan, double *__restrict__ scale) {
+    const int f = blockIdx.x * blockDim.x + threadIdx.x;
+    if (f < n_chan) scale[f] = __ddiv_rn(freq[f], kSpeedOfLight);
+}
+
+template <bool GENERAL>
+__global__ void __launch_bounds__(256) map_kernel(const double *__restrict__ uvw, const double *__restrict__ scale,
+                                                   unsigned int n, unsigned int n_chan, const MapParams p,
+                                                   uint32_t *__restrict__ keys, void *__restrict__ vals,
+                                                   Counters *counters) {
     unsigned int dropped_here = 0;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
-         i += (long long)gridDim.x * blockDim.x) {
-        const long long tb = i / n_chan;
-        const int f = (int)(i - tb * n_chan);
-        const double s = __ddiv_rn(freq[f], kSpeedOfLight);
-        const VisMap m = map_vis(uvw[tb * 3 + 0], uvw[tb * 3 + 1], s, p);
+    unsigned long long taps_here = 0;
+    const unsigned int stride = gridDim.x * blockDim.x;
+    const uint32_t tmask = (1u << p.key.tlog) - 1u;
+    for (unsigned long long ii = blockIdx.x * blockDim.x + threadIdx.x; ii < n; ii += stride) {
+        const unsigned int i = (unsigned int)ii;
+        const unsigned int tb = i / n_chan;
+        const unsigned int f = i - tb * n_chan;
+        const double *L = uvw + (size_t)tb * 3;
+        const VisMap m = map_vis(L[0], L[1], GENERAL ? L[2] : 0.0, scale[f], p);
         uint32_t key;
         if (m.dropped) {
-            key = 1u << (2 * p.key.bits_q);          // tile 0, origin (0,0), drop flag
             dropped_here++;
+            key = (uint32_t)(p.drop_slot * p.n_tiles) << p.key.tile_shift;       // tile 0, origin (0,0)
+            if (!GENERAL) key |= 1u << (2 * p.key.bits_q);
         } else {
+            taps_here += (unsigned long long)(m.S * m.S);
             const uint32_t x0 = (uint32_t)m.x0, y0 = (uint32_t)m.y0;
-            const uint32_t tmask = (1u << p.key.tlog) - 1u;
             const uint32_t tile = (y0 >> p.key.tlog) * (uint32_t)p.ntx + (x0 >> p.key.tlog);
-            key = (tile << p.key.tile_shift) | ((y0 & tmask) << (p.key.aux_bits + p.key.tlog)) |
-                  ((x0 & tmask) << p.key.aux_bits) | ((uint32_t)m.qy << p.key.bits_q) | (uint32_t)m.qx;
+            const uint32_t vtile = (uint32_t)(p.cls_slot[m.plane] * p.n_tiles) + tile;
+            key = (vtile << p.key.tile_shift) | ((y0 & tmask) << (p.key.aux_bits + p.key.tlog)) |
+                  ((x0 & tmask) << p.key.aux_bits);
+            if (p.key.plane_bits) key |= (uint32_t)m.plane << p.key.plane_shift;
+            if (!GENERAL) key |= ((uint32_t)m.qy << p.key.bits_q) | (uint32_t)m.qx;
         }
         keys[i] = key;
-        vals[i] = (uint32_t)i;
+        if (GENERAL) {
+            uint32_t aux = m.dropped ? (1u << 30)
+                                     : p.tab_off256[m.plane] + (uint32_t)(m.qy * p.oversample + m.qx) * p.q_units[m.plane];
+            if (m.conj) aux |= 1u << 31;
+            reinterpret_cast<uint2 *>(vals)[i] = make_uint2(i, aux);
+        } else {
+            reinterpret_cast<uint32_t *>(vals)[i] = i;
+        }
     }
-    // one integer atomic per warp that saw drops (the count does not depend on the order)
-    for (int o = 16; o > 0; o >>= 1) dropped_here += __shfl_xor_sync(0xffffffffu, dropped_here, o);
-    if ((threadIdx.x & 31) == 0 && dropped_here)
-        atomicAdd(&counters->n_dropped, (unsigned long long)dropped_here);
+    // integer atomics, one per warp (the sums do not depend on the order)
+    for (int o = 16; o > 0; o >>= 1) {
+        dropped_here += __shfl_xor_sync(0xffffffffu, dropped_here, o);
+        taps_here += __shfl_xor_sync(0xffffffffu, taps_here, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (dropped_here) atomicAdd(&counters->n_dropped, (unsigned long long)dropped_here);
+        if (taps_here) atomicAdd(&counters->vis_taps, taps_here);
+    }
 }
 
 __global__ void __launch_bounds__(256) map_debug_kernel(const double *__restrict__ uvw,
                                                          const double *__restrict__ freq, long long n_tb,
-                                                         int n_chan, MapParams p, int32_t *__restrict__ out) {
+                                                         int n_chan, const MapParams p, int32_t *__restrict__ out) {
     const long long n = n_tb * n_chan;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
          i += (long long)gridDim.x * blockDim.x) {
         const long long tb = i / n_chan;
         const int f = (int)(i - tb * n_chan);
         const double s = __ddiv_rn(freq[f], kSpeedOfLight);
-        const VisMap m = map_vis(uvw[tb * 3 + 0], uvw[tb * 3 + 1], s, p);
+        const VisMap m = map_vis(uvw[tb * 3 + 0], uvw[tb * 3 + 1], uvw[tb * 3 + 2], s, p);
         const long long lim = 1ll << 30;
         const long long cx = m.x0 < -lim ? -lim : (m.x0 > lim ? lim : m.x0);
         const long long cy = m.y0 < -lim ? -lim : (m.y0 > lim ? lim : m.y0);
         int32_t *o = out + i * 6;
-        o[0] = (int32_t)cx; o[1] = (int32_t)cy; o[2] = m.qx; o[3] = m.qy; o[4] = 0; o[5] = m.dropped ? 1 : 0;
+        o[0] = (int32_t)cx; o[1] = (int32_t)cy; o[2] = m.qx; o[3] = m.qy;
+        o[4] = m.plane | (m.conj << 8); o[5] = m.dropped ? 1 : 0;
     }
 }
 
-static MapParams make_map_params(const Plan &p) {
+MapParams make_map_params(const Plan &p) {
     MapParams mp;
+    memset(&mp, 0, sizeof(mp));
     mp.n_grid = p.cfg.grid_size;
     mp.oversample = p.cfg.oversample;
-    mp.support = p.S;
-    mp.half_so = p.S * p.cfg.oversample / 2;
     mp.ntx = p.ntx;
+    mp.n_tiles = p.n_tiles;
+    mp.n_planes = p.cfg.n_wplanes;
+    mp.general = p.mode != 0;
+    mp.is_complex = p.cfg.kernel_is_complex ? 1 : 0;
+    mp.drop_slot = 0;
     mp.cell_size = p.cfg.cell_size;
+    mp.w_max = p.cfg.w_max;
     mp.key = p.key;
+    for (int i = 0; i < p.cfg.n_wplanes; ++i) {
+        mp.support[i] = p.support_copy[i];
+        mp.cls_slot[i] = p.plane_slot[i];
+        mp.tab_off256[i] = p.plane_off256[i];
+        mp.q_units[i] = (uint32_t)(p.cls[p.plane_slot[i]].sub_bytes / 256);
+    }
     return mp;
 }
 
@@ -167,7 +252,8 @@ cudaError_t launch_map_debug(const Plan &p, const double *uvw, int n_time, int n
 }
 
 // ------------------------------------------------------------------------------------------
-// Tile tables from the sorted keys (the paper's 'first'/'last' look-up tables, :197).
+// Tile tables from the sorted keys (the paper's 'first'/'last' look-up tables, :197), per virtual
+// tile = class slot * n_tiles + tile.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) tile_bounds_kernel(const uint32_t *__restrict__ keys, long long n,
                                                            int tile_shift, uint32_t *__restrict__ tile_start,
@@ -180,16 +266,16 @@ __global__ void __launch_bounds__(256) tile_bounds_kernel(const uint32_t *__rest
     }
 }
 
-// chunks per tile: (full chunks << 32) | has_tail, one extra zero element at [n_tiles] so that the
+// chunks per tile: (full chunks << 32) | has_tail, one extra zero element at [n_vtiles] so that the
 // exclusive scan's last element is the pair of totals.
 __global__ void __launch_bounds__(256) tile_chunks_kernel(const uint32_t *__restrict__ tile_start,
-                                                           const uint32_t *__restrict__ tile_end, int n_tiles,
+                                                           const uint32_t *__restrict__ tile_end, int n_vtiles,
                                                            int chunk, unsigned long long *__restrict__ packed,
                                                            Counters *counters) {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t > n_tiles) return;
+    if (t > n_vtiles) return;
     unsigned long long v = 0;
-    if (t < n_tiles) {
+    if (t < n_vtiles) {
         const uint32_t cnt = tile_end[t] - tile_start[t];
         if (cnt) {
             v = ((unsigned long long)(cnt / chunk) << 32) | (unsigned long long)((cnt % chunk) ? 1 : 0);
@@ -200,44 +286,66 @@ __global__ void __launch_bounds__(256) tile_chunks_kernel(const uint32_t *__rest
     packed[t] = v;
 }
 
+// Work items of class slot c occupy ids [B_c, B_c + F_c + T_c): its F_c full chunks in tile order,
+// then its T_c tails in tile order; B_c = sum over earlier classes.  scan[] is the exclusive scan of
+// the packed (full << 32 | tail) counts over the virtual tiles.
 __global__ void __launch_bounds__(256) item_fill_kernel(const uint32_t *__restrict__ tile_start,
                                                          const uint32_t *__restrict__ tile_end,
                                                          const unsigned long long *__restrict__ scan, int n_tiles,
-                                                         int chunk, TileInfo *__restrict__ info,
+                                                         int n_cls, int chunk, TileInfo *__restrict__ info,
                                                          WorkItem *__restrict__ items, Counters *counters) {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    const unsigned long long totals = scan[n_tiles];
-    const uint32_t n_full_total = (uint32_t)(totals >> 32), n_tail_total = (uint32_t)totals;
+    const int n_vtiles = n_tiles * n_cls;
     if (t == 0) {
-        counters->n_full_total = n_full_total;
-        counters->n_items = n_full_total + n_tail_total;
-        counters->queue_head = 0;
+        uint32_t base = 0;
+        for (int c = 0; c < n_cls; ++c) {
+            const unsigned long long lo = scan[(size_t)c * n_tiles], hi = scan[(size_t)(c + 1) * n_tiles];
+            const uint32_t nf = (uint32_t)(hi >> 32) - (uint32_t)(lo >> 32), nt = (uint32_t)hi - (uint32_t)lo;
+            counters->cls_begin[c] = base;
+            base += nf + nt;
+            counters->cls_end[c] = base;
+        }
+        counters->n_items = base;
     }
-    if (t >= n_tiles) return;
+    if (t >= n_vtiles) return;
+    const int c = t / n_tiles;
+    uint32_t base = 0;
+    for (int k = 0; k < c; ++k) {
+        const unsigned long long lo = scan[(size_t)k * n_tiles], hi = scan[(size_t)(k + 1) * n_tiles];
+        base += ((uint32_t)(hi >> 32) - (uint32_t)(lo >> 32)) + ((uint32_t)hi - (uint32_t)lo);
+    }
+    const unsigned long long c_lo = scan[(size_t)c * n_tiles], c_hi = scan[(size_t)(c + 1) * n_tiles];
+    const uint32_t cls_full = (uint32_t)(c_hi >> 32) - (uint32_t)(c_lo >> 32);
     const uint32_t start = tile_start[t], cnt = tile_end[t] - start;
     const uint32_t nf = cnt / chunk, rem = cnt - nf * chunk;
-    const uint32_t full_base = (uint32_t)(scan[t] >> 32), tail_base = (uint32_t)scan[t];
+    const uint32_t full_base = base + ((uint32_t)(scan[t] >> 32) - (uint32_t)(c_lo >> 32));
+    const uint32_t tail_id = base + cls_full + ((uint32_t)scan[t] - (uint32_t)c_lo);
     TileInfo ti;
     ti.count = cnt;
     ti.full_base = full_base;
     ti.n_full = nf;
-    ti.tail_item = rem ? n_full_total + tail_base : 0xFFFFFFFFu;
+    ti.tail_item = rem ? tail_id : 0xFFFFFFFFu;
     info[t] = ti;
-    for (uint32_t c = 0; c < nf; ++c) {
+    for (uint32_t k = 0; k < nf; ++k) {
         WorkItem w;
-        w.start = start + c * chunk; w.len = chunk; w.tile = t; w.pad = 0;
-        items[full_base + c] = w;
+        w.start = start + k * chunk; w.len = chunk; w.tile = t; w.pad = 0;
+        items[full_base + k] = w;
     }
     if (rem) {
         WorkItem w;
         w.start = start + nf * chunk; w.len = rem; w.tile = t; w.pad = 0;
-        items[n_full_total + tail_base] = w;
+        items[tail_id] = w;
     }
 }
 
-cudaError_t sort_temp_bytes(int64_t n, int begin_bit, int end_bit, size_t *bytes) {
+cudaError_t sort_temp_bytes(int64_t n, int begin_bit, int end_bit, bool wide, size_t *bytes) {
     *bytes = 0;
-    cub::DoubleBuffer<uint32_t> k(nullptr, nullptr), v(nullptr, nullptr);
+    cub::DoubleBuffer<uint32_t> k(nullptr, nullptr);
+    if (wide) {
+        cub::DoubleBuffer<unsigned long long> v(nullptr, nullptr);
+        return cub::DeviceRadixSort::SortPairs(nullptr, *bytes, k, v, (long long)n, begin_bit, end_bit, (cudaStream_t)0);
+    }
+    cub::DoubleBuffer<uint32_t> v(nullptr, nullptr);
     return cub::DeviceRadixSort::SortPairs(nullptr, *bytes, k, v, (long long)n, begin_bit, end_bit, (cudaStream_t)0);
 }
 
@@ -253,22 +361,37 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
                        cudaStream_t s) {
     const long long n_tb = (long long)n_time * n_bl;
     const long long n = n_tb * n_chan;
+    const int n_vtiles = p.n_tiles * p.n_cls;
     GR_TRY(cudaMemsetAsync(p.counters, 0, sizeof(Counters), s));
-    // tile_start and tile_end are adjacent: [2][n_tiles]
-    GR_TRY(cudaMemsetAsync(p.tile_start, 0, sizeof(uint32_t) * 2 * (size_t)p.n_tiles, s));
-    uint32_t *tile_end = p.tile_start + p.n_tiles;
+    // tile_start and tile_end are adjacent: [2][n_vtiles]
+    GR_TRY(cudaMemsetAsync(p.tile_start, 0, sizeof(uint32_t) * 2 * (size_t)n_vtiles, s));
+    uint32_t *tile_end = p.tile_start + n_vtiles;
     stage_mark(p, 0, s);
     if (n > 0) {
-        map_kernel<<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(uvw, freq, n_tb, n_chan, make_map_params(p),
-                                                                p.keys[0], p.vals[0], p.counters);
+        double *scale = p.freq_scale;
+        freq_scale_kernel<<<(n_chan + 255) / 256, 256, 0, s>>>(freq, n_chan, scale);
+        GR_TRY(cudaGetLastError());
+        const MapParams mp = make_map_params(p);
+        if (p.mode == 0)
+            map_kernel<false><<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp,
+                                                                          p.keys[0], p.vals[0], p.counters);
+        else
+            map_kernel<true><<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp,
+                                                                         p.keys[0], p.vals[0], p.counters);
         GR_TRY(cudaGetLastError());
         stage_mark(p, 1, s);
-        cub::DoubleBuffer<uint32_t> k(p.keys[0], p.keys[1]), v(p.vals[0], p.vals[1]);
+        cub::DoubleBuffer<uint32_t> k(p.keys[0], p.keys[1]);
         size_t tb = p.cub_temp_bytes;
-        GR_TRY(cub::DeviceRadixSort::SortPairs(p.cub_temp, tb, k, v, n, p.key.aux_bits, p.key.total_bits, s));
+        if (p.mode == 0) {
+            cub::DoubleBuffer<uint32_t> v((uint32_t *)p.vals[0], (uint32_t *)p.vals[1]);
+            GR_TRY(cub::DeviceRadixSort::SortPairs(p.cub_temp, tb, k, v, n, p.key.aux_bits, p.key.total_bits, s));
+        } else {
+            cub::DoubleBuffer<unsigned long long> v((unsigned long long *)p.vals[0], (unsigned long long *)p.vals[1]);
+            GR_TRY(cub::DeviceRadixSort::SortPairs(p.cub_temp, tb, k, v, n, p.key.aux_bits, p.key.total_bits, s));
+        }
         p.sorted_sel = k.selector;
         stage_mark(p, 2, s);
-        p.n_launches += 3;
+        p.n_launches += 4;
         tile_bounds_kernel<<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(p.keys[p.sorted_sel], n,
                                                                         p.key.tile_shift, p.tile_start, tile_end);
         GR_TRY(cudaGetLastError());
@@ -277,15 +400,15 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
         stage_mark(p, 1, s);
         stage_mark(p, 2, s);
     }
-    const int nt1 = p.n_tiles + 1;
-    tile_chunks_kernel<<<(nt1 + 255) / 256, 256, 0, s>>>(p.tile_start, tile_end, p.n_tiles, p.chunk,
+    const int nt1 = n_vtiles + 1;
+    tile_chunks_kernel<<<(nt1 + 255) / 256, 256, 0, s>>>(p.tile_start, tile_end, n_vtiles, p.chunk,
                                                            p.tile_chunks, p.counters);
     GR_TRY(cudaGetLastError());
     size_t tb = p.cub_temp_bytes;
     GR_TRY(cub::DeviceScan::ExclusiveSum(p.cub_temp, tb, (const unsigned long long *)p.tile_chunks,
                                          p.tile_chunks_scan, (long long)nt1, s));
     item_fill_kernel<<<(nt1 + 255) / 256, 256, 0, s>>>(p.tile_start, tile_end, p.tile_chunks_scan, p.n_tiles,
-                                                         p.chunk, p.tile_info, p.items, p.counters);
+                                                         p.n_cls, p.chunk, p.tile_info, p.items, p.counters);
     GR_TRY(cudaGetLastError());
     p.n_launches += 3;
     stage_mark(p, 3, s);

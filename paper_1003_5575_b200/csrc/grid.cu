@@ -1,67 +1,54 @@
 // gridder_grid: the gridding kernel (FP32 FMA, registers + shared memory) and the deterministic flush.
 //
-// Grid kernel (DESIGN.md section 5).  PAPER.md :197-199 gathers per pixel from 9 bins; here the work
+// Grid kernel (DESIGN.md section 6).  PAPER.md :197-199 gathers per pixel from 9 bins; here the work
 // is turned round so that every lane does useful FMAs on every visibility:
 //   * a work item is <= K consecutive entries of one uv tile's sorted list; ONE WARP owns it;
 //   * the warp keeps the item's (T + SP - 1)^2-cell region (tile + halo) in shared memory;
 //   * for the current patch origin the SP x SP patch lives in REGISTERS, NA*NB cells (x 4 pol
 //     complex = 8 floats) per lane; entries are sorted by origin, so the patch is exchanged with
-//     the shared region only when the origin changes;
-//   * per entry a lane does 3 broadcast LDS.128 (visibility + meta), NA vector LDS (its taps of the
-//     GCF sub-table) and 8*NA*NB FFMA; visibilities are fetched one batch of 32 ahead with
-//     128-bit loads (float4 per polarisation pair) and pre-multiplied by their weight;
-//   * no atomics anywhere: every region cell has one owner lane, every work item its own partial
-//     region in HBM.
-// Flush kernel: each grid cell sums, in FP64 and in a fixed (tile row, tile column, chunk) order,
-// the partial regions that cover it, and writes the complex64 grid once.
+//     the shared region only when the origin changes ("fold");
+//   * per entry a lane does broadcast LDS.128 of the staged visibility, NA vector loads of its
+//     taps of the GCF sub-table and 8*NA*NB FFMA (16*NA*NB for a complex table);
+//   * a warp runs ONE software pipeline over the whole stream of its work items: keys three
+//     batches ahead, visibilities (cp.async, 128-bit) two ahead, weighting and record staging one
+//     ahead, so the start of an item costs no exposed memory latency;
+//   * no atomics on data anywhere: every region cell has one owner lane, every work item its own
+//     partial region in HBM (the only atomic is the integer work-queue counter).
+// Flush kernel: each grid cell sums, in FP64 and in a fixed (class, tile row, tile column, chunk)
+// order, the partial regions that cover it, and writes the complex64 grid once.
+#include <climits>
+
 #include "gridder_internal.cuh"
 
 namespace gridder {
 
-template <int NA, int NB, int TLOG>
-struct Geo {
-    static constexpr int SPX = 8 * NA, SPY = 4 * NB;         // padded patch
-    static constexpr int T = 1 << TLOG;
-    static constexpr int RW = T + SPX - 1, RH = T + SPY - 1;   // region = tile + halo
-    static constexpr int CELLS = RW * RH;
-    static constexpr int HALF_SLOTS = 32 + 3;                  // (3 = the consumer's look-ahead)
-    static constexpr int HALF_SLOTS_UNUSED = 0;                  // a batch + copies of the next batch's first records
-    static constexpr int STAGE_F4 = 2 * HALF_SLOTS * 3;        // 2 halves x slots x 3 float4
-    static constexpr int RAW_F4 = 32 * 3;                      // cp.async landing buffer: one batch
-    static constexpr int WARP_F4 = 2 * CELLS + STAGE_F4 + RAW_F4;   // shared float4 per warp
-};
+// MODE 0: one real table with S <= 16, resident in shared memory, 32-bit (key, index) entries.
+// MODE 1: real tables read from global memory (any number of planes, sub-patches), wide entries.
+// MODE 2: complex tables (w-planes), conjugated for w < 0, read from global memory, wide entries.
+// NSUB > 1: an entry covers NSUB x NSUB register patches (supports 17..32), gridded one after the other.
+constexpr int kSentinel = -(1 << 20);   // origin of the record that ends a work item
+constexpr int kForce = INT_MIN;         // never an origin: forces a fold at the next record
 
-__device__ __forceinline__ float4 ldg_stream(const float4 *p) {
-    float4 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
-                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
-    return r;
-}
+template <int NA, int NB, int NSUB, int TLOG, int MODE>
+struct Geo {
+    static constexpr bool CPLX = MODE == 2;
+    static constexpr bool GEN = MODE != 0;
+    static constexpr int SPX = 8 * NA, SPY = 4 * NB;           // register patch
+    static constexpr int T = 1 << TLOG;
+    static constexpr int RW = T + SPX * NSUB - 1, RH = T + SPY * NSUB - 1;   // region = tile + halo
+    static constexpr int CELLS = RW * RH;
+    static constexpr int VF4 = CPLX ? 4 : 2;                   // float4 per staged visibility
+    static constexpr int SLOT_F4 = VF4 + 1;                    // + (table offset of the NEXT record, origin)
+    static constexpr int SLOTS = 36;                           // 32 records + sentinel + pad + look-ahead
+    static constexpr int RING_F4 = 2 * SLOTS * SLOT_F4;        // two halves
+    static constexpr int RAW_F4 = 32 * 2 + 8;                  // cp.async landing: 32 x {a, b}, 32 weights
+    static constexpr int WARP_F4 = 2 * CELLS + RING_F4 + RAW_F4;
+    static constexpr int SUB_BYTES = NA * NB * 32 * (CPLX ? 8 : 4);   // one (plane, sub-patch, q) sub-table
+};
 
 __device__ __forceinline__ void stg_stream(float4 *p, const float4 &v) {
     asm volatile("st.global.L1::no_allocate.v4.f32 [%0], {%1,%2,%3,%4};"
                  :: "l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
-}
-
-// ---- staging pipeline, three batches deep -------------------------------------------------------
-// Batch j+3: sorted (key, visibility index) loads in flight (two registers).  Batch j+2: its
-// visibilities and weights in flight as cp.async copies into the warp's raw buffer -- no register
-// holds them, so nothing is spilled while the FFMA loop runs.  Batch j+1: read back from the raw
-// buffer by its own lane, multiplied by its weight and written to the record ring while batch j is
-// being gridded.  No load is consumed in the step that issued it.
-struct KeyIdx {
-    uint32_t key, idx;
-};
-
-__device__ __forceinline__ KeyIdx load_keyidx(const GridParams &p, uint32_t e, bool valid) {
-    KeyIdx k;
-    k.key = 0u;
-    k.idx = 0u;
-    if (valid) {
-        k.key = __ldg(p.keys + e);
-        k.idx = __ldg(p.vals + e);
-    }
-    return k;
 }
 
 __device__ __forceinline__ void cp_async_16(void *dst_smem, const void *src, bool pred) {
@@ -79,90 +66,208 @@ __device__ __forceinline__ void cp_async_4(void *dst_smem, const void *src, bool
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// Starts the copies of one batch: lane's record goes to raw[lane] = {a, b, (w, -, -, -)}.
-// A lane past the end of the item, or a dropped visibility, gets zeros (and so adds nothing).
-__device__ __forceinline__ void issue_vis(const GridParams &p, float4 *raw, int lane, const KeyIdx k, bool valid) {
-    const bool dropped = (k.key >> (2 * p.key.bits_q)) & 1u;
+// ---- the per-warp stream of batches ---------------------------------------------------------------
+// A batch is <= 32 consecutive entries of one work item.  bits: count (0..32) | last batch of its
+// item << 6 | end of stream << 7 | batch index inside the item << 8.
+struct Desc {
+    int bits;
+    unsigned item;
+    __device__ __forceinline__ int cnt() const { return bits & 63; }
+    __device__ __forceinline__ bool last() const { return bits & 64; }
+    __device__ __forceinline__ bool end() const { return bits & 128; }
+    __device__ __forceinline__ int bidx() const { return bits >> 8; }
+};
+
+constexpr int kClaim = 4;       // work items claimed per queue access (descriptors live in lanes 0..3)
+
+struct Producer {
+    WorkItem grp, nxt;                   // lane l: descriptor l of the current / the next claimed group
+    unsigned grp_base, nxt_base;
+    int grp_cnt, nxt_cnt, grp_pos;
+    unsigned it_start, it_len, it_off, it_id;
+    unsigned item_begin, item_end;       // this launch's (patch class's) range of the work-item table
+    bool ended;
+
+    __device__ __forceinline__ void claim(const GridParams &p, int lane) {
+        unsigned b = 0;
+        if (lane == 0) b = atomicAdd(&p.counters->queue_head[p.cls], (unsigned)kClaim);
+        b = __shfl_sync(0xffffffffu, b, 0);
+        nxt_base = item_begin + b;
+        nxt_cnt = nxt_base < item_end ? (int)min((unsigned)kClaim, item_end - nxt_base) : 0;
+        WorkItem w;
+        w.start = w.len = w.tile = w.pad = 0;
+        if (lane < nxt_cnt) w = p.items[nxt_base + lane];
+        nxt = w;
+    }
+
+    __device__ __forceinline__ void init(const GridParams &p, int lane) {
+        ended = false;
+        it_len = it_off = it_start = it_id = 0;
+        item_begin = p.counters->cls_begin[p.cls];
+        item_end = p.counters->cls_end[p.cls];
+        claim(p, lane);
+        grp = nxt; grp_base = nxt_base; grp_cnt = nxt_cnt; grp_pos = 0;
+        if (grp_cnt > 0) claim(p, lane); else ended = true;
+    }
+
+    // Descriptor of the next batch of this warp's stream and the position of its first entry.
+    __device__ __forceinline__ Desc next(const GridParams &p, int lane, unsigned &start) {
+        Desc d;
+        d.bits = 128; d.item = 0; start = 0;
+        if (ended) return d;
+        if (it_off >= it_len) {
+            if (grp_pos >= grp_cnt) {
+                grp = nxt; grp_base = nxt_base; grp_cnt = nxt_cnt; grp_pos = 0;
+                if (grp_cnt == 0) { ended = true; return d; }
+                claim(p, lane);
+            }
+            it_start = __shfl_sync(0xffffffffu, grp.start, grp_pos);
+            it_len = __shfl_sync(0xffffffffu, grp.len, grp_pos);
+            it_id = grp_base + grp_pos;
+            ++grp_pos;
+            it_off = 0;
+        }
+        const unsigned left = it_len - it_off;
+        d.bits = (int)min(32u, left) | (left <= 32u ? 64 : 0) | (int)((it_off >> 5) << 8);
+        d.item = it_id;
+        start = it_start + it_off;
+        it_off += 32;
+        return d;
+    }
+};
+
+// One sorted entry as the grid kernel sees it.
+struct Entry {
+    uint32_t key, idx, aux;
+};
+
+template <bool GEN>
+__device__ __forceinline__ Entry load_entry(const GridParams &p, unsigned e, bool valid) {
+    Entry k;
+    k.key = k.idx = k.aux = 0u;
+    if (valid) {
+        k.key = __ldg(p.keys + e);
+        if (GEN) {
+            const uint2 v = __ldg(reinterpret_cast<const uint2 *>(p.vals) + e);
+            k.idx = v.x;
+            k.aux = v.y;
+        } else {
+            k.idx = __ldg(reinterpret_cast<const uint32_t *>(p.vals) + e);
+        }
+    }
+    return k;
+}
+
+// Starts the copies of one batch: lane's visibility goes to raw[2 lane .. 2 lane + 1], its weight to
+// the float array behind.  A lane past the end of the batch, or a dropped visibility, gets zeros.
+template <bool GEN>
+__device__ __forceinline__ void issue_vis(const GridParams &p, float4 *raw, int lane, const Entry k, bool valid) {
+    const bool dropped = GEN ? ((k.aux >> 30) & 1u) : ((k.key >> (2 * p.key.bits_q)) & 1u);
     const bool live = valid && !dropped;
     const float4 *src = p.vis + 2 * (size_t)(live ? k.idx : 0u);
-    float4 *dst = raw + lane * 3;
-    cp_async_16(dst, src, live);
-    cp_async_16(dst + 1, src + 1, live);
-    if (p.weight) cp_async_4(dst + 2, p.weight + (live ? k.idx : 0u), live);
+    cp_async_16(raw + 2 * lane, src, live);
+    cp_async_16(raw + 2 * lane + 1, src + 1, live);
+    if (p.weight) cp_async_4(reinterpret_cast<float *>(raw + 64) + lane, p.weight + (live ? k.idx : 0u), live);
     cp_async_commit();
 }
 
-// Moves a landed batch of `cnt` <= 32 records from the raw buffer into `half` of the ring in the
-// consumer's format {w*a, w*b, (table offset, origin)}; lanes past the end write a record that adds
-// nothing (zero visibility, the last record's origin) so that the consumer can work in fours.  The
-// first records are repeated in the extension slots of the other half, where the consumer's
-// look-ahead finds them without wrapping.
-template <int NA, int NB, int TLOG>
-__device__ __forceinline__ void stage_write(const GridParams &p, const float4 *raw, float4 *half, float4 *other_ext,
-                                            int lane, int cnt, uint32_t key) {
-    using G = Geo<NA, NB, TLOG>;
-    const uint32_t qmask = (1u << (2 * p.key.bits_q)) - 1u;
+// Moves a landed batch from the raw buffer into one half of the record ring in the consumer's format:
+// the weighted visibility (VF4 float4) and (table byte offset, region offset of the patch origin).
+// Lanes past the end write records that add nothing; the last batch of an item is followed by a
+// sentinel record with origin -1, which makes the consumer fold the last patch into the region.
+template <int NA, int NB, int NSUB, int TLOG, int MODE>
+__device__ __forceinline__ void stage_write(const GridParams &p, const float4 *raw, float4 *half, int lane,
+                                            const Desc d, const Entry k) {
+    using G = Geo<NA, NB, NSUB, TLOG, MODE>;
+    const int cnt = d.cnt();
     const uint32_t tmask = (1u << TLOG) - 1u;
-    const uint32_t x0l = (key >> p.key.aux_bits) & tmask;
-    const uint32_t y0l = (key >> (p.key.aux_bits + TLOG)) & tmask;
-    const int coff = (int)((key & qmask) * (NA * 32 * NB * (uint32_t)sizeof(float)));
+    uint32_t x0l, y0l;
+    int coff;
+    float sg = 1.0f;
+    if (G::GEN) {
+        x0l = k.key & tmask;
+        y0l = (k.key >> TLOG) & tmask;
+        coff = (int)((k.aux & 0x3fffffffu) << 8);          // table offset in 256-byte units
+        if (k.aux >> 31) sg = -1.0f;
+    } else {
+        const uint32_t qmask = (1u << (2 * p.key.bits_q)) - 1u;
+        x0l = (k.key >> p.key.aux_bits) & tmask;
+        y0l = (k.key >> (p.key.aux_bits + TLOG)) & tmask;
+        coff = (int)((k.key & qmask) * (uint32_t)G::SUB_BYTES);
+    }
     const int poff = (int)(y0l * G::RW + x0l);
     const int last_poff = __shfl_sync(0xffffffffu, poff, cnt - 1);
     const bool pad = lane >= cnt;
-    const float4 ra = raw[lane * 3], rb = raw[lane * 3 + 1];
-    const float w = p.weight ? raw[lane * 3 + 2].x : 1.0f;
+    const float4 ra = raw[2 * lane], rb = raw[2 * lane + 1];
+    const float w = p.weight ? reinterpret_cast<const float *>(raw + 64)[lane] : 1.0f;
     const float4 a = make_float4(ra.x * w, ra.y * w, ra.z * w, ra.w * w);
     const float4 b = make_float4(rb.x * w, rb.y * w, rb.z * w, rb.w * w);
-    const float4 m = make_float4(__int_as_float(pad ? 0 : coff), __int_as_float(pad ? last_poff : poff), 0.f, 0.f);
-    float4 *slot = half + lane * 3;
-    slot[0] = a; slot[1] = b; slot[2] = m;
-    if (lane < 3) {
-        float4 *e = other_ext + lane * 3;
-        e[0] = a; e[1] = b; e[2] = m;
+    float4 *slot = half + lane * G::SLOT_F4;
+    slot[0] = a;
+    slot[1] = b;
+    if (G::CPLX) {      // (-s im, s re) pairs: the complex product then needs no sign handling
+        slot[2] = make_float4(-sg * a.y, sg * a.x, -sg * a.w, sg * a.z);
+        slot[3] = make_float4(-sg * b.y, sg * b.x, -sg * b.w, sg * b.z);
+    }
+    // slot r carries the table offset of record r + 1 (the consumer loads taps one record ahead)
+    // and the origin of record r; slot 0 also carries its own table offset
+    const int my_coff = pad ? 0 : coff;
+    const int next_coff = __shfl_down_sync(0xffffffffu, my_coff, 1);
+    const int my_poff = pad ? (d.last() ? kSentinel : last_poff) : poff;
+    slot[G::VF4] = make_float4(__int_as_float(lane == 31 ? 0 : next_coff), __int_as_float(my_poff),
+                               __int_as_float(my_coff), 0.f);
+    if (d.last() && lane < 2) {
+        float4 *s2 = half + (32 + lane) * G::SLOT_F4;
+#pragma unroll
+        for (int i = 0; i < G::VF4; ++i) s2[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        s2[G::VF4] = make_float4(__int_as_float(0), __int_as_float(kSentinel), __int_as_float(0), 0.f);
     }
 }
-
-template <int NB> struct CoefVec;
-template <> struct CoefVec<4> {
-    float c[4];
-    __device__ __forceinline__ void load(const float *p) {
-        const float4 v = *reinterpret_cast<const float4 *>(p);
-        c[0] = v.x; c[1] = v.y; c[2] = v.z; c[3] = v.w;
-    }
-};
-template <> struct CoefVec<2> {
-    float c[2];
-    __device__ __forceinline__ void load(const float *p) {
-        const float2 v = *reinterpret_cast<const float2 *>(p);
-        c[0] = v.x; c[1] = v.y;
-    }
-};
 
 // One staged record in registers: the weighted visibility (broadcast loads) and this lane's taps.
-template <int NA, int NB>
+template <int NA, int NB, int MODE>
 struct RecRegs {
-    float4 va, vb;
-    CoefVec<NB> c[NA];
-    // `coff` = table byte offset of the record in `slot`, loaded one record earlier (load_meta), so
-    // that no address here waits on a load issued in the same step.
+    static constexpr bool CPLX = MODE == 2;
+    static constexpr int VF4 = CPLX ? 4 : 2;
+    static constexpr int CF = NB * (CPLX ? 2 : 1);            // floats per column block
+    float4 v[VF4];
+    float c[NA][CF];
+    // MODE 0: `coef_lane` is the shared-space address of this lane's taps of sub-table 0 (the table
+    // sits at the start of dynamic shared memory), else a global pointer.
     __device__ __forceinline__ void fetch(const float4 *slot, const int coff, const char *coef_lane) {
-        va = slot[0];
-        vb = slot[1];
-        const float *cp = reinterpret_cast<const float *>(coef_lane + coff);
 #pragma unroll
-        for (int a = 0; a < NA; ++a) c[a].load(cp + a * 32 * NB);
+        for (int i = 0; i < VF4; ++i) v[i] = slot[i];
+        const char *cp = coef_lane + coff;
+#pragma unroll
+        for (int a = 0; a < NA; ++a) {
+            const char *ca = cp + a * 32 * CF * (int)sizeof(float);
+            if (MODE == 0) {                                   // shared memory, explicit state space
+                const uint32_t sa = (uint32_t)(uintptr_t)ca;
+                if (CF == 4) {
+                    asm("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];"
+                        : "=f"(c[a][0]), "=f"(c[a][1]), "=f"(c[a][2]), "=f"(c[a][3]) : "r"(sa));
+                } else {
+                    asm("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(c[a][0]), "=f"(c[a][1]) : "r"(sa));
+                }
+            } else {                                           // global memory through L1
+#pragma unroll
+                for (int j = 0; j < CF / 4; ++j) {
+                    const float4 t = __ldg(reinterpret_cast<const float4 *>(ca) + j);
+                    c[a][4 * j] = t.x; c[a][4 * j + 1] = t.y; c[a][4 * j + 2] = t.z; c[a][4 * j + 3] = t.w;
+                }
+                if (CF == 2) {
+                    const float2 t = __ldg(reinterpret_cast<const float2 *>(ca));
+                    c[a][0] = t.x; c[a][1] = t.y;
+                }
+            }
+        }
     }
 };
 
-__device__ __forceinline__ int2 load_meta(const float4 *slot) {
-    const float2 m = *reinterpret_cast<const float2 *>(slot + 2);
-    return make_int2(__float_as_int(m.x), __float_as_int(m.y));
-}
-
-// Two-level accumulation (DESIGN.md section 6): the register patch holds a short FP32 chain (one run
-// of equal patch origins, at most 64 entries); it is then ADDED to the shared region and cleared.
-// A long single chain is not good enough: neighbouring channels of one baseline give nearly equal
-// terms, whose rounding errors do not cancel (measured 1.2e-5 relative at 2048 terms).
+// Two-level accumulation (DESIGN.md section 7): the register patch holds a short FP32 chain (one run
+// of equal patch origins, at most fold_batches*32 entries); it is then ADDED to the shared region and
+// cleared.  A long single chain is not good enough: neighbouring channels of one baseline give
+// nearly equal terms, whose rounding errors do not cancel (measured 1.2e-5 relative at 2048 terms).
 template <int NA, int NB, int RW>
 __device__ __forceinline__ void fold_patch(float4 *regA, float4 *regB, int base, float (&acc)[NA][NB][8]) {
     __syncwarp();       // a cell changes owner lane from one origin to the next
@@ -180,42 +285,72 @@ __device__ __forceinline__ void fold_patch(float4 *regA, float4 *regB, int base,
         }
 }
 
-template <int NA, int NB, int RW>
-__device__ __forceinline__ void consume(const RecRegs<NA, NB> &R, const int poff, int &cur, float4 *regA,
-                                        float4 *regB, int lane_cell, float (&acc)[NA][NB][8]) {
-    if (poff != cur) {                                      // warp-uniform
+// `cmp` is the origin the patch was last matched against (kForce forces a fold at the next record, used
+// to bound the chain length); `cur` is the origin the registers really belong to (-1: none).
+template <int NA, int NB, int RW, int MODE>
+__device__ __forceinline__ void consume(const RecRegs<NA, NB, MODE> &R, const int poff, int &cur, int &cmp,
+                                        float4 *regA, float4 *regB, int lane_cell, float (&acc)[NA][NB][8]) {
+    if (poff != cmp) {                                      // warp-uniform
         if (cur >= 0) fold_patch<NA, NB, RW>(regA, regB, cur + lane_cell, acc);
-        cur = poff;
+        cur = cmp = poff;
     }
-    const float v[8] = {R.va.x, R.va.y, R.va.z, R.va.w, R.vb.x, R.vb.y, R.vb.z, R.vb.w};
+    if (MODE == 2) {
+        const float vr[4] = {R.v[0].x, R.v[0].z, R.v[1].x, R.v[1].z};
+        const float vi[4] = {R.v[0].y, R.v[0].w, R.v[1].y, R.v[1].w};
+        const float pp[4] = {R.v[2].x, R.v[2].z, R.v[3].x, R.v[3].z};
+        const float qq[4] = {R.v[2].y, R.v[2].w, R.v[3].y, R.v[3].w};
 #pragma unroll
-    for (int a = 0; a < NA; ++a)
+        for (int a = 0; a < NA; ++a)
 #pragma unroll
-        for (int b = 0; b < NB; ++b)
+            for (int b = 0; b < NB; ++b) {
+                const float cr = R.c[a][2 * b], ci = R.c[a][2 * b + 1];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) acc[a][b][k] = fmaf(R.c[a].c[b], v[k], acc[a][b][k]);
+                for (int k = 0; k < 4; ++k) {
+                    acc[a][b][2 * k] = fmaf(cr, vr[k], acc[a][b][2 * k]);
+                    acc[a][b][2 * k + 1] = fmaf(cr, vi[k], acc[a][b][2 * k + 1]);
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    acc[a][b][2 * k] = fmaf(ci, pp[k], acc[a][b][2 * k]);
+                    acc[a][b][2 * k + 1] = fmaf(ci, qq[k], acc[a][b][2 * k + 1]);
+                }
+            }
+    } else {
+        const float v[8] = {R.v[0].x, R.v[0].y, R.v[0].z, R.v[0].w, R.v[1].x, R.v[1].y, R.v[1].z, R.v[1].w};
+#pragma unroll
+        for (int a = 0; a < NA; ++a)
+#pragma unroll
+            for (int b = 0; b < NB; ++b)
+#pragma unroll
+                for (int k = 0; k < 8; ++k) acc[a][b][k] = fmaf(R.c[a][b], v[k], acc[a][b][k]);
+    }
 }
 
-template <int NA, int NB, int TLOG, int WARPS>
-__global__ void __launch_bounds__(WARPS * 32, 1) grid_kernel(const GridParams p) {
-    using G = Geo<NA, NB, TLOG>;
+template <int NA, int NB, int NSUB, int TLOG, int MODE, int MAXW>
+__global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) {
+    using G = Geo<NA, NB, NSUB, TLOG, MODE>;
     extern __shared__ float4 smem[];
-    float4 *coef4 = smem;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float4 *region = smem + p.coef_f4 + warp * G::WARP_F4;     // plane A then plane B
+    const int table_f4 = MODE == 0 ? p.coef_f4 : 0;
+    float4 *region = smem + table_f4 + warp * G::WARP_F4;      // plane A (XX, XY) then plane B (YX, YY)
     float4 *regA = region, *regB = region + G::CELLS;
-    float4 *stage = region + 2 * G::CELLS;                     // record ring: 2 halves x 35 slots x 3 float4
-    float4 *raw = stage + G::STAGE_F4;                         // cp.async landing buffer
+    float4 *ring = region + 2 * G::CELLS;                      // 2 halves x SLOTS x VF4
+    float4 *raw = ring + G::RING_F4;                           // cp.async landing buffer
 
-    for (int i = threadIdx.x; i < p.coef_f4; i += WARPS * 32) coef4[i] = p.coef[i];
-    // the ring is cleared too: records are fetched one ahead, also past the end of an item, and
+    if (MODE == 0)
+        for (int i = threadIdx.x; i < p.coef_f4; i += blockDim.x) smem[i] = p.coef[i];
+    // everything is cleared: records are fetched one ahead, also past the end of a batch, and
     // whatever a slot holds must be a valid table offset
     for (int i = lane; i < G::WARP_F4; i += 32) region[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     __syncthreads();
 
-    const unsigned int n_items = p.counters_ro->n_items;
     const int lane_cell = (lane >> 3) * G::RW + (lane & 7);      // tap (a=0, b=0) of this lane
-    const char *coef_lane = reinterpret_cast<const char *>(smem) + lane * NB * sizeof(float);
+    const char *coef_lane;
+    if constexpr (MODE == 0)
+        coef_lane = reinterpret_cast<const char *>((uintptr_t)((uint32_t)__cvta_generic_to_shared(smem) +
+                                                              lane * RecRegs<NA, NB, MODE>::CF * (int)sizeof(float)));
+    else
+        coef_lane = reinterpret_cast<const char *>(p.coef) + lane * RecRegs<NA, NB, MODE>::CF * (int)sizeof(float);
 
     float acc[NA][NB][8];
 #pragma unroll
@@ -225,100 +360,101 @@ __global__ void __launch_bounds__(WARPS * 32, 1) grid_kernel(const GridParams p)
 #pragma unroll
             for (int k = 0; k < 8; ++k) acc[a][b][k] = 0.f;
 
+    Producer prod;
+    prod.init(p, lane);
+    Desc dC, dL, dK;                     // being consumed | landing in the raw buffer | keys in flight
+    dC.bits = 0; dC.item = 0;
+    dL = dC;
+    unsigned start;
+    dK = prod.next(p, lane, start);
+    Entry eK = load_entry<G::GEN>(p, start + lane, lane < dK.cnt());
+    Entry eL;
+    eL.key = eL.idx = eL.aux = 0u;
+    int par = 0, cur = -1, cmp = kSentinel;
+
     while (true) {
-        unsigned int item = 0;
-        if (lane == 0) item = atomicAdd(&p.counters->queue_head, 1u);
-        item = __shfl_sync(0xffffffffu, item, 0);
-        if (item >= n_items) break;
-        const WorkItem wi = p.items[item];
-        const int len = (int)wi.len;
-
-        const int n_batches = (len + 31) >> 5;
-
-        // prologue: batch 0 staged, batch 1's visibilities (cp.async) and batch 2's keys in flight
-        uint32_t key_landing;                                   // key of the batch in the raw buffer
-        KeyIdx ki_next;                                         // batch after that
-        {
-            const KeyIdx k0 = load_keyidx(p, wi.start + lane, lane < len);
-            const KeyIdx k1 = load_keyidx(p, wi.start + 32 + lane, 32 + lane < len);
-            ki_next = load_keyidx(p, wi.start + 64 + lane, 64 + lane < len);
-            issue_vis(p, raw, lane, k0, lane < len);
-            cp_async_wait_all();
-            stage_write<NA, NB, TLOG>(p, raw, stage, stage + (G::HALF_SLOTS + 32) * 3, lane, min(32, len), k0.key);
-            issue_vis(p, raw, lane, k1, 32 + lane < len);
-            key_landing = k1.key;
-        }
+        const float4 *half = ring + par * (G::SLOTS * G::SLOT_F4);
+        // the batch that landed goes to the other half (last read one iteration ago)
+        cp_async_wait_all();
         __syncwarp();
+        const Desc dS = dL;
+        if (dS.cnt() > 0)
+            stage_write<NA, NB, NSUB, TLOG, MODE>(p, raw, ring + (par ^ 1) * (G::SLOTS * G::SLOT_F4), lane, dS, eL);
+        __syncwarp();
+        // next batch's visibilities start to move, the one after that gets its keys
+        issue_vis<G::GEN>(p, raw, lane, eK, lane < dK.cnt());
+        dL = dK;
+        eL = eK;
+        dK = prod.next(p, lane, start);
+        eK = load_entry<G::GEN>(p, start + lane, lane < dK.cnt());
 
-        // The loop body handles four records so that every prefetched (table offset, origin) pair
-        // lands in a register nobody else is still reading: no copy waits on a load just issued.
-        RecRegs<NA, NB> A, B;
-        int2 mA = load_meta(stage);
-        A.fetch(stage, mA.x, coef_lane);
-        int2 mB = load_meta(stage + 3);
-        int cur = -1;
-        for (int jb = 0; jb < n_batches; ++jb) {
-            float4 *half = stage + (jb & 1) * (G::HALF_SLOTS * 3);
-            float4 *other = stage + ((jb + 1) & 1) * (G::HALF_SLOTS * 3);
-            const int n_quads = (min(32, len - 32 * jb) + 3) >> 2;
-            const float4 *sp = half;
-            auto quad_step = [&]() {
-                // in: A = record 0 (origin mA.y), mB = meta of record 1
-                const int2 mC = load_meta(sp + 6);
-                B.fetch(sp + 3, mB.x, coef_lane);
-                consume<NA, NB, G::RW>(A, mA.y, cur, regA, regB, lane_cell, acc);
-                const int2 mD = load_meta(sp + 9);
-                A.fetch(sp + 6, mC.x, coef_lane);
-                consume<NA, NB, G::RW>(B, mB.y, cur, regA, regB, lane_cell, acc);
-                mA = load_meta(sp + 12);
-                B.fetch(sp + 9, mD.x, coef_lane);
-                consume<NA, NB, G::RW>(A, mC.y, cur, regA, regB, lane_cell, acc);
-                mB = load_meta(sp + 15);
-                A.fetch(sp + 12, mA.x, coef_lane);
-                consume<NA, NB, G::RW>(B, mD.y, cur, regA, regB, lane_cell, acc);
-                sp += 12;
-            };
-            const int first = min(n_quads, 4);
-            for (int i = 0; i < first; ++i) quad_step();
-            // mid-batch (warp-uniform): bound the register chain, then move the staging pipeline on
-            if ((jb & p.fold_mask) == p.fold_mask && cur >= 0) {
-                fold_patch<NA, NB, G::RW>(regA, regB, cur + lane_cell, acc);
-                cur = -1;
-            }
-            if (jb + 1 < n_batches) {
-                __syncwarp();                                   // the other half was last read in batch jb-1
-                cp_async_wait_all();
-                stage_write<NA, NB, TLOG>(p, raw, other, half + 32 * 3, lane, min(32, len - 32 * (jb + 1)), key_landing);
-                __syncwarp();
-                const int o2 = (jb + 2) * 32 + lane, o3 = (jb + 3) * 32 + lane;
-                if ((jb + 2) * 32 < len) {
-                    issue_vis(p, raw, lane, ki_next, o2 < len);
-                    key_landing = ki_next.key;
-                    ki_next = load_keyidx(p, wi.start + o3, o3 < len);
+        if (dC.end()) break;
+        const int cnt = dC.cnt();
+        if (cnt > 0) {
+            const int cntp = dC.last() ? ((cnt + 2) & ~1) : cnt;        // + sentinel, even
+            const float4 *send = half + cntp * G::SLOT_F4;
+#pragma unroll 1
+            for (int sub = 0; sub < NSUB * NSUB; ++sub) {
+                // sub-patch (sy, sx): its origin in the region and its part of the table
+                const int sub_poff = NSUB > 1 ? (sub / NSUB) * (G::SPY * G::RW) + (sub % NSUB) * G::SPX : 0;
+                const char *cl = NSUB > 1 ? coef_lane + sub * p.sub_stride_bytes : coef_lane;
+                if (NSUB > 1) cmp = kForce;
+                RecRegs<NA, NB, MODE> A, B;
+                const float4 *sp = half;
+                // meta of a slot: x = table offset of the next record, y = origin of this one
+                int2 mA, mB;
+                {
+                    const float4 m0 = sp[G::VF4];
+                    A.fetch(sp, __float_as_int(m0.z), cl);
+                    mA = make_int2(__float_as_int(m0.x), __float_as_int(m0.y));
                 }
+                do {
+                    mB = *reinterpret_cast<const int2 *>(sp + G::SLOT_F4 + G::VF4);
+                    B.fetch(sp + G::SLOT_F4, mA.x, cl);
+                    consume<NA, NB, G::RW, MODE>(A, mA.y + sub_poff, cur, cmp, regA, regB, lane_cell, acc);
+                    mA = *reinterpret_cast<const int2 *>(sp + 2 * G::SLOT_F4 + G::VF4);
+                    A.fetch(sp + 2 * G::SLOT_F4, mB.x, cl);
+                    consume<NA, NB, G::RW, MODE>(B, mB.y + sub_poff, cur, cmp, regA, regB, lane_cell, acc);
+                    sp += 2 * G::SLOT_F4;
+                } while (sp < send);
             }
-            for (int i = 4; i < n_quads; ++i) quad_step();
+            if (dC.last()) {
+                // the sentinel has folded the last patch in; move the region to this item's
+                // partial and clear it
+                cur = -1;
+                cmp = kSentinel;
+                __syncwarp();
+                float4 *dst = p.partials + (size_t)dC.item * p.region_f4;
+                for (int i = lane; i < 2 * G::CELLS; i += 32) {
+                    stg_stream(dst + i, region[i]);
+                    region[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+                __syncwarp();
+            } else if ((dC.bidx() & p.fold_mask) == p.fold_mask) {
+                cmp = kForce;                               // bound the register chain
+            }
         }
-        // fold the last patch in, then move the region to this item's partial and clear it
-        if (cur >= 0) fold_patch<NA, NB, G::RW>(regA, regB, cur + lane_cell, acc);
-        __syncwarp();
-        float4 *dst = p.partials + (size_t)item * (2 * G::CELLS);
-        for (int i = lane; i < 2 * G::CELLS; i += 32) {
-            stg_stream(dst + i, region[i]);
-            region[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-        }
-        __syncwarp();
+        dC = dS;
+        par ^= 1;
     }
+    cp_async_wait_all();
 }
 
 // ------------------------------------------------------------------------------------------
 // Flush: one thread per grid cell.  The partial regions covering cell (x, y) belong to the tiles
 // (ty, tx) with tx*T <= x < tx*T + RW (same in y); each tile's work items are added in id order
-// (full chunks, then the tail).  FP64 accumulation, one rounding to FP32 at the end.
+// (full chunks, then the tail).  FP64 accumulation, one rounding to FP32 at the end.  One launch
+// per patch class (its tile table, its region geometry); the second class adds to the first.
 // ------------------------------------------------------------------------------------------
-template <int NA, int NB, int TLOG>
+template <int SP, int TLOG>
+struct FlushGeo {
+    static constexpr int T = 1 << TLOG;
+    static constexpr int RW = T + SP - 1, RH = T + SP - 1, CELLS = RW * RH;
+};
+
+template <int SP, int TLOG>
 __global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
-    using G = Geo<NA, NB, TLOG>;
+    using G = FlushGeo<SP, TLOG>;
     const int x = blockIdx.x * 32 + threadIdx.x;
     const int y = blockIdx.y * 8 + threadIdx.y;
     if (x >= p.n_grid || y >= p.n_grid) return;
@@ -335,7 +471,7 @@ __global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
             const uint32_t n_it = ti.n_full + (ti.tail_item != 0xFFFFFFFFu ? 1u : 0u);
             for (uint32_t c = 0; c < n_it; ++c) {
                 const uint32_t item = c < ti.n_full ? ti.full_base + c : ti.tail_item;
-                const float4 *part = p.partials + (size_t)item * (2 * G::CELLS);
+                const float4 *part = p.partials + (size_t)item * p.region_f4;
                 const float4 a = __ldcs(part + cell), b = __ldcs(part + G::CELLS + cell);
                 acc[0] += (double)a.x; acc[1] += (double)a.y; acc[2] += (double)a.z; acc[3] += (double)a.w;
                 acc[4] += (double)b.x; acc[5] += (double)b.y; acc[6] += (double)b.z; acc[7] += (double)b.w;
@@ -356,60 +492,70 @@ __global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
 }
 
 // ------------------------------------------------------------------------------------------
-// Host side: kernel selection.  NA x NB is fixed by the padded patch (16: 2x4, 8: 1x2), TLOG and
-// the number of warps per block are plan parameters.
+// Host side: kernel selection.  The register patch (NA x NB), the sub-patch count and the table
+// mode follow from the plan; TLOG is a plan parameter; the block size is chosen at run time.
 // ------------------------------------------------------------------------------------------
-size_t grid_smem_bytes(int NA, int NB, int tlog, int oversample, int warps) {
-    const int T = 1 << tlog;
-    const int RW = T + 8 * NA - 1, RH = T + 4 * NB - 1;
-    const size_t coef = (size_t)oversample * oversample * NA * NB * 32 * sizeof(float);
-    const size_t per_warp = (size_t)(2 * RW * RH + 2 * (32 + 3) * 3 + 32 * 3) * sizeof(float4);   // Geo::WARP_F4
-    return coef + per_warp * warps;
+size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps) {
+    const int vf4 = mode == 2 ? 4 : 2;
+    const size_t per_warp = (size_t)(2 * g.RW * g.RH + 2 * 36 * (vf4 + 1) + 32 * 2 + 8) * sizeof(float4);   // Geo::WARP_F4
+    (void)tlog;
+    return (mode == 0 ? table_bytes : 0) + per_warp * warps;
 }
 
 typedef void (*grid_fn_t)(const GridParams);
 typedef void (*flush_fn_t)(const FlushParams);
 
-template <int NA, int NB, int TLOG>
-static grid_fn_t pick_warps(int warps) {
-    switch (warps) {
-        case 4: return grid_kernel<NA, NB, TLOG, 4>;
-        case 6: return grid_kernel<NA, NB, TLOG, 6>;
-        case 8: return grid_kernel<NA, NB, TLOG, 8>;
-        case 10: return grid_kernel<NA, NB, TLOG, 10>;
-        case 12: return grid_kernel<NA, NB, TLOG, 12>;
-        case 16: return grid_kernel<NA, NB, TLOG, 16>;
+constexpr int kMaxWarpsFast = 12, kMaxWarpsGeneral = 8;     // launch bounds: 168 / 255 registers
+
+template <int NA, int NB, int NSUB, int MODE, int MAXW>
+static grid_fn_t pick_tlog(int tlog) {
+    switch (tlog) {
+        case 2: return grid_kernel<NA, NB, NSUB, 2, MODE, MAXW>;
+        case 3: return grid_kernel<NA, NB, NSUB, 3, MODE, MAXW>;
+        case 4: return grid_kernel<NA, NB, NSUB, 4, MODE, MAXW>;
         default: return nullptr;
     }
 }
 
-static grid_fn_t pick_grid(int NA, int tlog, int warps) {
-    if (NA == 2) {
-        if (tlog == 2) return pick_warps<2, 4, 2>(warps);
-        if (tlog == 3) return pick_warps<2, 4, 3>(warps);
-        if (tlog == 4) return pick_warps<2, 4, 4>(warps);
-    } else {
-        if (tlog == 2) return pick_warps<1, 2, 2>(warps);
-        if (tlog == 3) return pick_warps<1, 2, 3>(warps);
-        if (tlog == 4) return pick_warps<1, 2, 4>(warps);
+template <int MODE, int MAXW>
+static grid_fn_t pick_shape(const ClassGeo &g, int tlog) {
+    if (g.NA == 1 && g.nsub == 1) return pick_tlog<1, 2, 1, MODE, MAXW>(tlog);
+    if (g.NA == 2 && g.nsub == 1) return pick_tlog<2, 4, 1, MODE, MAXW>(tlog);
+    if constexpr (MODE != 0) {
+        if (g.NA == 2 && g.nsub == 2) return pick_tlog<2, 4, 2, MODE, MAXW>(tlog);
     }
     return nullptr;
 }
 
-static flush_fn_t pick_flush(int NA, int tlog) {
-    if (NA == 2) {
-        if (tlog == 2) return flush_kernel<2, 4, 2>;
-        if (tlog == 3) return flush_kernel<2, 4, 3>;
-        if (tlog == 4) return flush_kernel<2, 4, 4>;
-    } else {
-        if (tlog == 2) return flush_kernel<1, 2, 2>;
-        if (tlog == 3) return flush_kernel<1, 2, 3>;
-        if (tlog == 4) return flush_kernel<1, 2, 4>;
+static grid_fn_t pick_grid(const ClassGeo &g, int tlog, int mode) {
+    switch (mode) {
+        case 0: return pick_shape<0, kMaxWarpsFast>(g, tlog);
+        case 1: return pick_shape<1, kMaxWarpsGeneral>(g, tlog);
+        case 2: return pick_shape<2, kMaxWarpsGeneral>(g, tlog);
+        default: return nullptr;
     }
-    return nullptr;
 }
 
-static const int kWarpChoices[] = {16, 12, 10, 8, 6, 4};
+template <int SP>
+static flush_fn_t pick_flush_tlog(int tlog) {
+    switch (tlog) {
+        case 2: return flush_kernel<SP, 2>;
+        case 3: return flush_kernel<SP, 3>;
+        case 4: return flush_kernel<SP, 4>;
+        default: return nullptr;
+    }
+}
+
+static flush_fn_t pick_flush(const ClassGeo &g, int tlog) {
+    switch (g.SP) {
+        case 8: return pick_flush_tlog<8>(tlog);
+        case 16: return pick_flush_tlog<16>(tlog);
+        case 32: return pick_flush_tlog<32>(tlog);
+        default: return nullptr;
+    }
+}
+
+static const int kWarpChoices[] = {12, 10, 8, 6, 4, 2, 1};
 
 cudaError_t configure_grid_kernel(Plan &p) {
     int dev = 0, smem_max = 0;
@@ -417,61 +563,79 @@ cudaError_t configure_grid_kernel(Plan &p) {
     if (e != cudaSuccess) return e;
     e = cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     if (e != cudaSuccess) return e;
-    int chosen = 0;
-    for (int w : kWarpChoices) {
-        if (p.warps > 0 && w != p.warps) continue;             // forced by the caller (tuning)
-        if (grid_smem_bytes(p.NA, p.NB, p.tlog, p.cfg.oversample, w) <= (size_t)smem_max) { chosen = w; break; }
+    const int cap = p.mode == 0 ? kMaxWarpsFast : kMaxWarpsGeneral;
+    for (int c = 0; c < p.n_cls; ++c) {
+        ClassGeo &g = p.cls[c];
+        int chosen = 0;
+        for (int w : kWarpChoices) {
+            if (w > cap) continue;
+            if (p.warps_forced > 0 && w > p.warps_forced) continue;      // the caller's limit (tuning, tests)
+            if (grid_smem_bytes(g, p.tlog, p.mode, p.coef_bytes, w) <= (size_t)smem_max) { chosen = w; break; }
+        }
+        if (!chosen) return cudaErrorInvalidConfiguration;
+        g.warps = chosen;
+        g.smem_bytes = (int)grid_smem_bytes(g, p.tlog, p.mode, p.coef_bytes, chosen);
+        grid_fn_t fn = pick_grid(g, p.tlog, p.mode);
+        if (!fn) return cudaErrorInvalidConfiguration;
+        e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes);
+        if (e != cudaSuccess) return e;
     }
-    if (!chosen) return cudaErrorInvalidConfiguration;
-    p.warps = chosen;
-    p.smem_bytes = (int)grid_smem_bytes(p.NA, p.NB, p.tlog, p.cfg.oversample, chosen);
-    grid_fn_t fn = pick_grid(p.NA, p.tlog, p.warps);
-    if (!fn) return cudaErrorInvalidConfiguration;
-    return cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, p.smem_bytes);
+    return cudaSuccess;
 }
 
 cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *grid, int accumulate,
                         cudaStream_t s) {
-    grid_fn_t gfn = pick_grid(p.NA, p.tlog, p.warps);
-    flush_fn_t ffn = pick_flush(p.NA, p.tlog);
-    if (!gfn || !ffn) return cudaErrorInvalidConfiguration;
     stage_mark(p, 4, s);
-    // reset the work queue (bin leaves it at 0, a previous grid call leaves it past the end)
-    cudaError_t e = cudaMemsetAsync(&p.counters->queue_head, 0, sizeof(unsigned int), s);
+    // reset the work queues (a previous grid call leaves them past the end)
+    cudaError_t e = cudaMemsetAsync(p.counters->queue_head, 0, sizeof(unsigned int) * kMaxClasses, s);
     if (e != cudaSuccess) return e;
-    GridParams gp;
-    gp.keys = p.keys[p.sorted_sel];
-    gp.vals = p.vals[p.sorted_sel];
-    gp.items = p.items;
-    gp.counters_ro = p.counters;
-    gp.counters = p.counters;
-    gp.vis = reinterpret_cast<const float4 *>(vis);
-    gp.weight = weight;
-    gp.coef = p.coef;
-    gp.partials = p.partials;
-    gp.coef_f4 = p.coef_f4;
-    gp.key = p.key;
-    gp.fold_mask = p.fold_batches - 1;
-    gfn<<<p.n_sm, p.warps * 32, p.smem_bytes, s>>>(gp);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
+    for (int c = 0; c < p.n_cls; ++c) {
+        const ClassGeo &g = p.cls[c];
+        grid_fn_t gfn = pick_grid(g, p.tlog, p.mode);
+        if (!gfn) return cudaErrorInvalidConfiguration;
+        GridParams gp;
+        gp.keys = p.keys[p.sorted_sel];
+        gp.vals = p.vals[p.sorted_sel];
+        gp.items = p.items;
+        gp.counters = p.counters;
+        gp.vis = reinterpret_cast<const float4 *>(vis);
+        gp.weight = weight;
+        gp.coef = p.coef;
+        gp.partials = p.partials;
+        gp.coef_f4 = p.mode == 0 ? (int)(p.coef_bytes / sizeof(float4)) : 0;
+        gp.key = p.key;
+        gp.fold_mask = p.fold_batches - 1;
+        gp.region_f4 = p.region_f4;
+        gp.cls = c;
+        gp.sub_stride_bytes = p.cfg.oversample * p.cfg.oversample * g.sub_bytes;
+        gfn<<<p.n_sm, g.warps * 32, g.smem_bytes, s>>>(gp);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        p.n_launches += 1;
+    }
     stage_mark(p, 5, s);
-    FlushParams fp;
-    fp.tiles = p.tile_info;
-    fp.counters = p.counters;
-    fp.partials = p.partials;
-    fp.grid = reinterpret_cast<float2 *>(grid);
-    fp.n_grid = p.cfg.grid_size;
-    fp.ntx = p.ntx;
-    fp.nty = p.nty;
-    fp.accumulate = accumulate;
-    dim3 blk(32, 8), grd((p.cfg.grid_size + 31) / 32, (p.cfg.grid_size + 7) / 8);
-    ffn<<<grd, blk, 0, s>>>(fp);
-    e = cudaGetLastError();
+    for (int c = 0; c < p.n_cls; ++c) {
+        const ClassGeo &g = p.cls[c];
+        flush_fn_t ffn = pick_flush(g, p.tlog);
+        if (!ffn) return cudaErrorInvalidConfiguration;
+        FlushParams fp;
+        fp.tiles = p.tile_info + (size_t)c * p.n_tiles;
+        fp.partials = p.partials;
+        fp.grid = reinterpret_cast<float2 *>(grid);
+        fp.n_grid = p.cfg.grid_size;
+        fp.ntx = p.ntx;
+        fp.nty = p.nty;
+        fp.accumulate = (c > 0 || accumulate) ? 1 : 0;
+        fp.region_f4 = p.region_f4;
+        dim3 blk(32, 8), grd((p.cfg.grid_size + 31) / 32, (p.cfg.grid_size + 7) / 8);
+        ffn<<<grd, blk, 0, s>>>(fp);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        p.n_launches += 1;
+    }
     stage_mark(p, 6, s);
     if (p.profiling) p.prof_grid_calls++;
-    p.n_launches += 2;
-    return e;
+    return cudaSuccess;
 }
 
 }  // namespace gridder

@@ -1,10 +1,14 @@
 // Internal declarations of libgridder.so (not part of the C ABI; see include/gridder.h).
 //
-// Data flow:
-//   map kernel   : visibility i=(t,b,f) -> 32-bit key  [tile | y0l | x0l | drop | qy | qx]  + value i
-//   radix sort   : stable, on the [tile | y0l | x0l] bits only (CUB DeviceRadixSort)
-//   tile tables  : per tile first entry / count -> (tile, chunk) work items, full chunks first
-//   grid kernel  : one warp per work item, patch accumulators in registers, region in shared memory
+// Data flow (DESIGN.md sections 5-6):
+//   map kernel   : visibility i=(t,b,f) -> 32-bit key [class | tile | (plane) | y0l | x0l | aux] + value
+//                  fast path (one real table, S <= 16): aux = drop, qy, qx in the key, value = i (u32)
+//                  general path (w-planes, complex tables, S <= 32): value = (i, table offset | flags) (u64)
+//   radix sort   : stable, on the [class | tile | plane | y0l | x0l] bits only (CUB DeviceRadixSort)
+//   tile tables  : per (class, tile) first entry / count -> (tile, chunk) work items, per class:
+//                  full chunks first, then the ragged tails
+//   grid kernel  : one launch per patch class; one warp per work item, patch accumulators in
+//                  registers, region in shared memory
 //   flush kernel : per grid cell, FP64 sum of the partial regions that cover it, in a fixed order
 #pragma once
 #include <cuda_runtime.h>
@@ -17,25 +21,49 @@ namespace gridder {
 
 constexpr int kProfRing = 32;                     // calls remembered by the stage timers
 constexpr double kSpeedOfLight = 299792458.0;     // m/s (gridder.h: u_lambda = u_m * f / c)
+constexpr int kMaxPlanes = 64;
+constexpr int kMaxChannels = 1 << 16;              // per gridder_bin call (frequency scale table)
+constexpr int kMaxClasses = 3;                    // padded patch 8 (S <= 8), 16 (S <= 16), 32 = 2x2 x 16
 
-// Bit layout of a sort key (LSB first): qx, qy (bits_q each), drop flag, x0l, y0l (tlog each), tile.
+// Bit layout of a sort key (LSB first): [aux: qx, qy (bits_q each), drop flag -- fast path only],
+// x0l, y0l (tlog each), plane (plane_bits, may be 0), virtual tile = class slot * n_tiles + tile.
 struct KeyLayout {
     int bits_q;        // bits of one sub-cell offset
     int tlog;          // log2 of the tile edge T
-    int aux_bits;      // 2*bits_q + 1: not sorted on
-    int tile_shift;    // aux_bits + 2*tlog
-    int tile_bits;     // bits of the tile id
+    int aux_bits;      // 2*bits_q + 1 (fast path) or 0: not sorted on
+    int plane_shift;   // aux_bits + 2*tlog
+    int plane_bits;
+    int tile_shift;    // plane_shift + plane_bits
+    int tile_bits;     // bits of the virtual tile id
     int total_bits;    // tile_shift + tile_bits  (<= 32)
+};
+
+// Patch class: how a lane's register patch and the warp's shared region are shaped.
+struct ClassGeo {
+    int32_t NA, NB;          // register patch = 8 NA x 4 NB cells
+    int32_t nsub;            // sub-patches per axis handled per entry (1, or 2 for 16 < S <= 32)
+    int32_t SP;              // cells per axis covered per entry = 8 NA nsub
+    int32_t RW, RH;          // region = tile + halo
+    int32_t sub_bytes;       // one (plane, sub-patch, q) sub-table of the re-laid GCF
+    int32_t warps, smem_bytes;
 };
 
 struct MapParams {
     int32_t n_grid;          // N
     int32_t oversample;      // O
-    int32_t support;         // S (single plane)
-    int32_t half_so;         // S*O/2
     int32_t ntx;             // tiles per grid row
+    int32_t n_tiles;
+    int32_t n_planes;
+    int32_t general;         // 0: fast path key/value format
+    int32_t is_complex;
+    int32_t drop_slot;       // class slot dropped visibilities are filed under
     double cell_size;        // du
+    double w_max;
     KeyLayout key;
+    int32_t support[kMaxPlanes];
+    int32_t cls_slot[kMaxPlanes];       // class slot of the plane (index into the plan's classes)
+    uint32_t tab_off256[kMaxPlanes];    // byte offset / 256 of the plane's re-laid table
+    uint32_t q_units[kMaxPlanes];       // sub_bytes / 256 of the plane's class
 };
 
 // One (tile, chunk) work item: entries [start, start+len) of the sorted list.
@@ -46,8 +74,7 @@ struct WorkItem {
     uint32_t pad;
 };
 
-// Per tile: where its work items are.  Items [0, n_full_total) are the full chunks (len == K) in
-// tile order, items [n_full_total, n_items) the ragged tails in tile order.
+// Per virtual tile: where its work items are.
 struct TileInfo {
     uint32_t count;          // entries in the tile
     uint32_t full_base;      // id of its first full-chunk item
@@ -58,60 +85,71 @@ struct TileInfo {
 // Device-side counters, all integer (order-independent, so deterministic).
 struct Counters {
     unsigned long long n_dropped;
-    unsigned int n_items;          // full + tail
-    unsigned int n_full_total;
+    unsigned long long vis_taps;              // sum of S_p^2 over gridded visibilities
+    unsigned int n_items;
     unsigned int n_occupied;
     unsigned int max_tile_load;
-    unsigned int queue_head;       // work-item queue of the grid kernel
-    unsigned int pad[9];
+    unsigned int cls_begin[kMaxClasses];      // work-item range of each class slot
+    unsigned int cls_end[kMaxClasses];
+    unsigned int queue_head[kMaxClasses];     // work queues of the grid kernel launches
+    unsigned int pad[2];
 };
 
 struct GridParams {
     const uint32_t *keys;          // sorted keys
-    const uint32_t *vals;          // sorted visibility indices
+    const void *vals;              // sorted values: u32 index (fast path) or u64 (index, aux)
     const WorkItem *items;
-    const Counters *counters_ro;
     Counters *counters;
     const float4 *vis;             // [n][2] float4
     const float *weight;           // [n] or null
-    const float4 *coef;            // re-laid table: [O*O][NA][32 lanes][NB] floats
-    float4 *partials;              // [item][2][RH*RW] float4
-    int32_t coef_f4;               // float4 count of the table
+    const float4 *coef;            // re-laid table(s)
+    float4 *partials;              // [item][region_f4] float4
+    int32_t coef_f4;               // float4 count of the table staged in shared memory (fast path)
     int32_t fold_mask;             // register chains are folded every (fold_mask + 1) batches of 32
+    int32_t region_f4;             // stride of one partial region
+    int32_t cls;                   // class slot of this launch
+    int32_t sub_stride_bytes;      // table distance between sub-patches (O^2 sub-tables)
     KeyLayout key;
 };
 
 struct FlushParams {
-    const TileInfo *tiles;
-    const Counters *counters;
+    const TileInfo *tiles;         // this class's table
     const float4 *partials;
     float2 *grid;                  // [4][N][N]
     int32_t n_grid;
     int32_t ntx, nty;
     int32_t accumulate;
+    int32_t region_f4;
 };
 
 struct Plan {
     gridder_config cfg;            // copy (support pointer re-targeted to support_copy)
-    int32_t support_copy[64];
+    int32_t support_copy[kMaxPlanes];
     // derived
-    int32_t S, NA, NB, tlog, T, ntx, nty, n_tiles;
-    int32_t RW, RH, region_f4;     // region_f4 = 2*RH*RW float4 per work item
+    int32_t mode;                  // 0 fast real, 1 general real, 2 general complex
+    int32_t n_cls;                 // class slots in use
+    ClassGeo cls[kMaxClasses];
+    int32_t plane_slot[kMaxPlanes];
+    uint32_t plane_off256[kMaxPlanes];
+    int32_t tlog, T, ntx, nty, n_tiles;
+    int32_t region_f4;             // largest region of the classes in use = partial stride
     int32_t chunk;                 // K
     int32_t fold_batches;          // longest FP32 register chain, in batches of 32 entries (power of 2)
-    int32_t warps, n_sm, smem_bytes;
+    int32_t warps_forced, n_sm;
     int64_t max_items;
     KeyLayout key;
     // workspace carve-up (device pointers into cfg.workspace)
-    uint32_t *keys[2], *vals[2];
+    uint32_t *keys[2];
+    void *vals[2];
     void *cub_temp; size_t cub_temp_bytes;
-    uint32_t *tile_start;          // [2][n_tiles]: first entry | one past the last entry
-    unsigned long long *tile_chunks, *tile_chunks_scan;   // packed (n_full << 32 | has_tail), [n_tiles+1]
-    TileInfo *tile_info;           // [n_tiles]
+    double *freq_scale;            // [kMaxChannels]: freq / c of the last bin
+    uint32_t *tile_start;          // [2][n_vtiles]: first entry | one past the last entry
+    unsigned long long *tile_chunks, *tile_chunks_scan;   // packed (n_full << 32 | has_tail), [n_vtiles+1]
+    TileInfo *tile_info;           // [n_vtiles]
     WorkItem *items;               // [max_items]
     float4 *partials;              // [max_items][region_f4]
-    float4 *coef;                  // re-laid table
-    int32_t coef_f4;
+    float4 *coef;                  // re-laid table(s)
+    size_t coef_bytes;
     Counters *counters;
     size_t workspace_needed;
     // state
@@ -135,18 +173,19 @@ inline void stage_mark(Plan &p, int i, cudaStream_t s) {
 }
 
 // bin.cu
+MapParams make_map_params(const Plan &p);
 cudaError_t launch_relayout(const Plan &p, cudaStream_t s);
 cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const double *freq, int n_chan,
                        cudaStream_t s);
 cudaError_t launch_map_debug(const Plan &p, const double *uvw, int n_time, int n_bl, const double *freq,
                              int n_chan, int32_t *out, cudaStream_t s);
-cudaError_t sort_temp_bytes(int64_t n, int begin_bit, int end_bit, size_t *bytes);
+cudaError_t sort_temp_bytes(int64_t n, int begin_bit, int end_bit, bool wide, size_t *bytes);
 cudaError_t scan_temp_bytes(int64_t n, size_t *bytes);
 
 // grid.cu
-cudaError_t configure_grid_kernel(Plan &p);          // picks warps/smem, sets the smem attribute
+cudaError_t configure_grid_kernel(Plan &p);          // picks warps/smem per class, sets the smem attribute
 cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *grid, int accumulate,
                         cudaStream_t s);
-size_t grid_smem_bytes(int NA, int NB, int tlog, int oversample, int warps);
+size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps);
 
 }  // namespace gridder

@@ -250,6 +250,6 @@ def test_error_paths_on_device(dev):
     assert e.value.code == gridder.ERR_NOT_BINNED
     g.destroy()
     with pytest.raises(gridder.GridderError) as e:
-        gridder.Gridder(grid_size=64, cell_size=1.0, oversample=4, support=[20], kernel=torch.zeros(80 * 80, device=dev),
+        gridder.Gridder(grid_size=32768, cell_size=1.0, oversample=4, support=[16], kernel=torch.zeros(64 * 64, device=dev),
                         max_vis=100)
     assert e.value.code == gridder.ERR_UNSUPPORTED

@@ -1,0 +1,151 @@
+"""GPU parity of the general path: several w-planes, variable support 1..32 (8-, 16- and 2x2x16-cell
+patch classes), complex tables conjugated for w < 0 (BASELINE.json config 3; R13), and real
+tables read from global memory.  Same bar as test_gpu_parity.py: integer work bit-exact, grid cells
+within 1e-5 * sum|w V C| + 1e-6, reruns bit-identical."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+from _util import assert_parity
+
+pytestmark = pytest.mark.gpu
+C = 299_792_458.0
+
+
+@pytest.fixture(scope="module")
+def dev():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1003_5575_b200 import gridder
+    gridder.load_library()
+    return torch.device("cuda:0")
+
+
+class _Env:
+    def __init__(self, **kw):
+        self.kw = {k: str(v) for k, v in kw.items()}
+
+    def __enter__(self):
+        self.old = {k: os.environ.get(k) for k in self.kw}
+        os.environ.update(self.kw)
+
+    def __exit__(self, *a):
+        for k, v in self.old.items():
+            if v is None:
+                os.environ.pop(k, None)
+            else:
+                os.environ[k] = v
+
+
+def _tables(rng, supports, O, cplx):
+    parts = []
+    for s in supports:
+        shape = (s * O, s * O, 2) if cplx else (s * O, s * O)
+        parts.append(rng.standard_normal(shape).astype(np.float32).ravel())
+    return np.concatenate(parts)
+
+
+def _case(rng, n, N, w_max, n_tie=40):
+    uvw = np.zeros((1, n, 3))
+    uvw[0, :, :2] = rng.uniform(-N / 2 - 1, N / 2 + 1, (n, 2))
+    uvw[0, :, 2] = rng.uniform(-1.05 * w_max, 1.05 * w_max, n)          # beyond w_max: clamps to the last plane
+    uvw[0, :n_tie, :2] = (np.floor(uvw[0, :n_tie, :2] * 4) + 0.5) / 4    # rounding ties
+    uvw[0, n_tie:2 * n_tie, 2] = 0.0                                     # w = 0: plane 0, not conjugated
+    vis = rng.standard_normal((n, 4, 2)).astype(np.float32)
+    w = rng.uniform(0.5, 1.5, n).astype(np.float32)
+    return uvw, vis, w
+
+
+def _both(dev, uvw, freq, vis, weight, *, N, du, O, supports, table, w_max, cplx, env=None):
+    from paper_1003_5575_b200 import gridder
+    n = uvw.shape[0] * uvw.shape[1] * len(freq)
+    with _Env(**(env or {})):
+        g = gridder.Gridder(grid_size=N, cell_size=du, oversample=O, support=list(supports),
+                            kernel=torch.from_numpy(table).to(dev), max_vis=max(n, 1), n_wplanes=len(supports),
+                            w_max=w_max, kernel_is_complex=cplx)
+    d_uvw = torch.from_numpy(np.ascontiguousarray(uvw)).to(dev)
+    d_f = torch.tensor(np.asarray(freq, np.float64), device=dev)
+    got_map = g.map(d_uvw, d_f).cpu().numpy()
+    g.bin(d_uvw, d_f)
+    d_vis = torch.from_numpy(np.ascontiguousarray(vis)).to(dev)
+    d_w = None if weight is None else torch.from_numpy(np.ascontiguousarray(weight)).to(dev)
+    out1 = g.grid(d_vis, d_w).cpu().numpy()
+    out2 = g.grid(d_vis, d_w).cpu().numpy()
+    st = g.stats()
+    g.destroy()
+    kw = dict(grid_size=N, cell_size=du, oversample=O, support=list(supports), kernel=table, w_max=w_max,
+              kernel_is_complex=cplx)
+    ref_map = oracle.map_visibilities(uvw, freq, **kw)
+    ref, ab, ost = oracle.grid_full(uvw, freq, vis, weight, **kw)
+    assert np.array_equal(got_map, ref_map), "map (x0, y0, qx, qy, plane|conj, dropped) differs from the oracle"
+    assert st.n_dropped == ost["n_dropped"] and st.vis_taps == ost["vis_taps"]
+    assert np.array_equal(out1, out2), "rerun is not bit-identical"
+    return out1, ref, ab, st, ost
+
+
+@pytest.mark.parametrize("S,O,N,n", [(16, 4, 96, 5000), (7, 8, 64, 4000), (15, 8, 80, 3000), (3, 2, 34, 500)])
+def test_general_path_equals_oracle_on_single_real_table(dev, S, O, N, n):
+    """The global-table kernels (MODE 1) on the shapes the fast path also handles."""
+    rng = np.random.default_rng(S * 7 + N)
+    table = _tables(rng, [S], O, False)
+    uvw, vis, w = _case(rng, n, N, 1.0)
+    got, ref, ab, st, _ = _both(dev, uvw, [C], vis, w, N=N, du=1.0, O=O, supports=[S], table=table, w_max=1.0,
+                                cplx=False, env={"GRIDDER_FORCE_GENERAL": 1})
+    assert st.n_dropped > 0
+    assert_parity(got, ref, ab, f"general real S={S}")
+
+
+@pytest.mark.parametrize("S,O,N,n", [(17, 2, 80, 3000), (24, 4, 96, 3000), (32, 4, 120, 3000), (31, 2, 100, 2000)])
+def test_large_support_uses_four_sub_patches(dev, S, O, N, n):
+    rng = np.random.default_rng(S)
+    table = _tables(rng, [S], O, False)
+    uvw, vis, w = _case(rng, n, N, 1.0)
+    got, ref, ab, st, _ = _both(dev, uvw, [C], vis, w, N=N, du=1.0, O=O, supports=[S], table=table, w_max=1.0,
+                                cplx=False)
+    assert st.patch_size == 32
+    assert_parity(got, ref, ab, f"real S={S}")
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+@pytest.mark.parametrize("tlog", [2, 3])
+def test_wplanes_mixed_supports_all_three_patch_classes(dev, cplx, tlog):
+    rng = np.random.default_rng(5 + tlog + 10 * cplx)
+    supports = [4, 8, 8, 10, 14, 16, 18, 26, 32]
+    O, N, n, w_max = 4, 128, 12000, 37.5
+    table = _tables(rng, supports, O, cplx)
+    uvw, vis, w = _case(rng, n, N, w_max)
+    vis2 = np.stack([vis, vis[::-1]], 1).copy()               # [n][2 channels][4][2]
+    w2 = np.stack([w, w[::-1]], 1).copy()
+    got, ref, ab, st, ost = _both(dev, uvw, [C, 0.9 * C], vis2, w2, N=N, du=1.0, O=O, supports=supports, table=table,
+                                  w_max=w_max, cplx=cplx, env={"GRIDDER_TILE_LOG2": tlog})
+    assert st.tile_size == 1 << tlog and 0 < st.n_dropped < 2 * n
+    assert_parity(got, ref, ab, f"w-planes cplx={cplx} T={1 << tlog}")
+
+
+def test_wplanes_hot_tile_chunks_and_unit_weights(dev):
+    rng = np.random.default_rng(77)
+    supports = [8, 12, 20]
+    O, N, n, w_max = 2, 64, 9000, 3.0
+    table = _tables(rng, supports, O, True)
+    uvw = np.zeros((1, n, 3))
+    uvw[0, :, :2] = rng.uniform(-2.0, 2.0, (n, 2))
+    uvw[0, :, 2] = rng.uniform(-3.0, 3.0, n)
+    vis = (rng.standard_normal((n, 4, 2)) + 2.0).astype(np.float32)
+    got, ref, ab, st, _ = _both(dev, uvw, [C], vis, None, N=N, du=1.0, O=O, supports=supports, table=table, w_max=w_max,
+                                cplx=True, env={"GRIDDER_CHUNK": 256})
+    assert st.chunk_size == 256 and st.max_tile_load > 256 and st.n_work_items > n // 256
+    assert_parity(got, ref, ab, "w-planes hot tile")
+
+
+def test_config3_reduced_full_grid(dev):
+    """BASELINE.json config 3 (32 complex w-planes, support 8..32, 4096^2 grid), first 2 channels."""
+    wl = synth.make_workload(3, n_chan=2)
+    vis = wl.visibilities("cpu").numpy()
+    got, ref, ab, st, ost = _both(dev, wl.uvw, wl.freq, vis, None, N=wl.grid_size, du=wl.cell_size, O=wl.oversample,
+                                  supports=wl.support, table=wl.kernel, w_max=wl.w_max, cplx=True)
+    assert st.n_dropped == 0 and st.n_vis == wl.n_vis
+    assert_parity(got, ref, ab, "config 3 (2 channels)")

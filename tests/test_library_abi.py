@@ -49,7 +49,13 @@ def test_null_and_invalid_arguments_need_no_device(lib):
                 dict(n_wplanes=0), dict(max_vis=-1), dict(support=(C.c_int32 * 1)(0)),
                 dict(support=(C.c_int32 * 1)(33)), dict(support=(C.c_int32 * 1)(7), oversample=1)):
         assert lib.gridder_workspace_size(C.byref(cfg(**bad)), C.byref(need)) == gridder.ERR_INVALID_ARG, bad
-    assert lib.gridder_workspace_size(C.byref(cfg(kernel_is_complex=1)), C.byref(need)) == gridder.ERR_UNSUPPORTED
+    # complex tables, w-planes and supports up to 32 are sized without a device
+    assert lib.gridder_workspace_size(C.byref(cfg(kernel_is_complex=1)), C.byref(need)) == gridder.OK and need.value > 0
+    sup3 = (C.c_int32 * 3)(8, 16, 32)
+    assert lib.gridder_workspace_size(C.byref(cfg(n_wplanes=3, support=sup3, w_max=10.0)), C.byref(need)) == gridder.OK
+    assert lib.gridder_workspace_size(C.byref(cfg(n_wplanes=3, support=sup3, w_max=0.0)), C.byref(need)) == gridder.ERR_INVALID_ARG
+    # a sort key that does not fit 32 bits (2^26 tiles of 4 x 4 cells + origin + sub-cell bits)
+    assert lib.gridder_workspace_size(C.byref(cfg(grid_size=32768)), C.byref(need)) == gridder.ERR_UNSUPPORTED
     plan = C.c_void_p()
     assert lib.gridder_plan(C.byref(cfg(grid_size=255)), C.byref(plan), None) == gridder.ERR_INVALID_ARG
     assert lib.gridder_plan(C.byref(cfg()), None, None) == gridder.ERR_INVALID_ARG
