@@ -60,7 +60,6 @@ int derive(const gridder_config *cfg, Plan &p) {
         used[s <= 8 ? 0 : (s <= 16 ? 1 : 2)] = true;
     }
     p.n_cls = 0;
-    p.region_f4 = 0;
     for (int c = 0; c < kMaxClasses; ++c) {
         if (!used[c]) continue;
         ClassGeo g;
@@ -71,9 +70,9 @@ int derive(const gridder_config *cfg, Plan &p) {
         g.SP = 8 * g.NA * g.nsub;
         g.RW = g.RH = p.T + g.SP - 1;
         g.sub_bytes = g.NA * g.NB * 32 * (cplx ? 8 : 4);
+        g.region_f4 = 2 * g.RW * g.RH;
         slot_of_class[c] = p.n_cls;
         p.cls[p.n_cls++] = g;
-        if (2 * g.RW * g.RH > p.region_f4) p.region_f4 = 2 * g.RW * g.RH;
     }
     size_t off = 0;
     const size_t oo = (size_t)cfg->oversample * cfg->oversample;
@@ -112,6 +111,13 @@ int derive(const gridder_config *cfg, Plan &p) {
     const int64_t n_vtiles = (int64_t)p.n_tiles * p.n_cls;
     int64_t occ = n < n_vtiles ? n : n_vtiles;
     p.max_items = occ + n / p.chunk + 1;
+    // each class has its own partial-region array, sized for the case that every entry is of that class
+    p.max_items_cls = (n < p.n_tiles ? n : p.n_tiles) + n / p.chunk + 1;
+    p.partials_f4 = 0;
+    for (int c = 0; c < p.n_cls; ++c) {
+        p.cls[c].part_off_f4 = p.partials_f4;
+        p.partials_f4 += p.max_items_cls * p.cls[c].region_f4;
+    }
     return GRIDDER_OK;
 }
 
@@ -143,7 +149,7 @@ cudaError_t carve(Plan &p, char *base) {
     p.tile_chunks_scan = (unsigned long long *)take(sizeof(unsigned long long) * (n_vtiles + 1));
     p.tile_info = (TileInfo *)take(sizeof(TileInfo) * n_vtiles);
     p.items = (WorkItem *)take(sizeof(WorkItem) * (size_t)p.max_items);
-    p.partials = (float4 *)take(sizeof(float4) * (size_t)p.region_f4 * (size_t)p.max_items);
+    p.partials = (float4 *)take(sizeof(float4) * (size_t)p.partials_f4);
     p.coef = (float4 *)take(p.coef_bytes);
     p.counters = (Counters *)take(sizeof(Counters));
     p.workspace_needed = off;

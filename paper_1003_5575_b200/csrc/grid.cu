@@ -424,7 +424,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
                 cur = -1;
                 cmp = kSentinel;
                 __syncwarp();
-                float4 *dst = p.partials + (size_t)dC.item * p.region_f4;
+                float4 *dst = p.partials + (size_t)(dC.item - prod.item_begin) * (2 * G::CELLS);
                 for (int i = lane; i < 2 * G::CELLS; i += 32) {
                     stg_stream(dst + i, region[i]);
                     region[i] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -461,6 +461,7 @@ __global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
     double acc[8];
 #pragma unroll
     for (int k = 0; k < 8; ++k) acc[k] = 0.0;
+    const uint32_t first_item = p.counters->cls_begin[p.cls];
     const int tx_hi = min(x >> TLOG, p.ntx - 1), ty_hi = min(y >> TLOG, p.nty - 1);
     const int tx_lo = max(0, (x - G::RW + G::T) >> TLOG), ty_lo = max(0, (y - G::RH + G::T) >> TLOG);
     for (int ty = ty_lo; ty <= ty_hi; ++ty)
@@ -471,7 +472,7 @@ __global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
             const uint32_t n_it = ti.n_full + (ti.tail_item != 0xFFFFFFFFu ? 1u : 0u);
             for (uint32_t c = 0; c < n_it; ++c) {
                 const uint32_t item = c < ti.n_full ? ti.full_base + c : ti.tail_item;
-                const float4 *part = p.partials + (size_t)item * p.region_f4;
+                const float4 *part = p.partials + (size_t)(item - first_item) * (2 * G::CELLS);
                 const float4 a = __ldcs(part + cell), b = __ldcs(part + G::CELLS + cell);
                 acc[0] += (double)a.x; acc[1] += (double)a.y; acc[2] += (double)a.z; acc[3] += (double)a.w;
                 acc[4] += (double)b.x; acc[5] += (double)b.y; acc[6] += (double)b.z; acc[7] += (double)b.w;
@@ -601,11 +602,10 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         gp.vis = reinterpret_cast<const float4 *>(vis);
         gp.weight = weight;
         gp.coef = p.coef;
-        gp.partials = p.partials;
+        gp.partials = p.partials + g.part_off_f4;
         gp.coef_f4 = p.mode == 0 ? (int)(p.coef_bytes / sizeof(float4)) : 0;
         gp.key = p.key;
         gp.fold_mask = p.fold_batches - 1;
-        gp.region_f4 = p.region_f4;
         gp.cls = c;
         gp.sub_stride_bytes = p.cfg.oversample * p.cfg.oversample * g.sub_bytes;
         gfn<<<p.n_sm, g.warps * 32, g.smem_bytes, s>>>(gp);
@@ -620,13 +620,14 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         if (!ffn) return cudaErrorInvalidConfiguration;
         FlushParams fp;
         fp.tiles = p.tile_info + (size_t)c * p.n_tiles;
-        fp.partials = p.partials;
+        fp.partials = p.partials + g.part_off_f4;
+        fp.counters = p.counters;
+        fp.cls = c;
         fp.grid = reinterpret_cast<float2 *>(grid);
         fp.n_grid = p.cfg.grid_size;
         fp.ntx = p.ntx;
         fp.nty = p.nty;
         fp.accumulate = (c > 0 || accumulate) ? 1 : 0;
-        fp.region_f4 = p.region_f4;
         dim3 blk(32, 8), grd((p.cfg.grid_size + 31) / 32, (p.cfg.grid_size + 7) / 8);
         ffn<<<grd, blk, 0, s>>>(fp);
         e = cudaGetLastError();

@@ -46,6 +46,8 @@ struct ClassGeo {
     int32_t RW, RH;          // region = tile + halo
     int32_t sub_bytes;       // one (plane, sub-patch, q) sub-table of the re-laid GCF
     int32_t warps, smem_bytes;
+    int32_t region_f4;       // 2 RW RH: float4 per partial region of this class
+    int64_t part_off_f4;     // where this class's partial regions start in the workspace array
 };
 
 struct MapParams {
@@ -103,10 +105,9 @@ struct GridParams {
     const float4 *vis;             // [n][2] float4
     const float *weight;           // [n] or null
     const float4 *coef;            // re-laid table(s)
-    float4 *partials;              // [item][region_f4] float4
+    float4 *partials;              // this class's partial regions: [item - first item of the class][region_f4]
     int32_t coef_f4;               // float4 count of the table staged in shared memory (fast path)
     int32_t fold_mask;             // register chains are folded every (fold_mask + 1) batches of 32
-    int32_t region_f4;             // stride of one partial region
     int32_t cls;                   // class slot of this launch
     int32_t sub_stride_bytes;      // table distance between sub-patches (O^2 sub-tables)
     KeyLayout key;
@@ -114,12 +115,13 @@ struct GridParams {
 
 struct FlushParams {
     const TileInfo *tiles;         // this class's table
-    const float4 *partials;
+    const float4 *partials;        // this class's partial regions
+    const Counters *counters;
+    int32_t cls;
     float2 *grid;                  // [4][N][N]
     int32_t n_grid;
     int32_t ntx, nty;
     int32_t accumulate;
-    int32_t region_f4;
 };
 
 struct Plan {
@@ -132,11 +134,12 @@ struct Plan {
     int32_t plane_slot[kMaxPlanes];
     uint32_t plane_off256[kMaxPlanes];
     int32_t tlog, T, ntx, nty, n_tiles;
-    int32_t region_f4;             // largest region of the classes in use = partial stride
     int32_t chunk;                 // K
     int32_t fold_batches;          // longest FP32 register chain, in batches of 32 entries (power of 2)
     int32_t warps_forced, n_sm;
-    int64_t max_items;
+    int64_t max_items;             // capacity of the work-item table (all classes)
+    int64_t max_items_cls;         // capacity of one class's partial-region array
+    int64_t partials_f4;           // float4 in all partial-region arrays
     KeyLayout key;
     // workspace carve-up (device pointers into cfg.workspace)
     uint32_t *keys[2];
@@ -147,7 +150,7 @@ struct Plan {
     unsigned long long *tile_chunks, *tile_chunks_scan;   // packed (n_full << 32 | has_tail), [n_vtiles+1]
     TileInfo *tile_info;           // [n_vtiles]
     WorkItem *items;               // [max_items]
-    float4 *partials;              // [max_items][region_f4]
+    float4 *partials;              // per class: [max_items_cls][region_f4 of the class]
     float4 *coef;                  // re-laid table(s)
     size_t coef_bytes;
     Counters *counters;
