@@ -86,6 +86,16 @@ int derive(const gridder_config *cfg, Plan &p) {
     if (off >= (1ull << 31)) return GRIDDER_ERR_UNSUPPORTED;       // table offsets are 32-bit byte offsets
     p.coef_bytes = off;
 
+    // fast path, opt-in (GRIDDER_TMEM=1): the table in tensor memory (512 columns x 32 bit per lane) when it
+    // fits.  Measured on B200: same speed as the shared-memory table, so off by default.
+    p.tmem_cols = 0;
+    if (p.mode == 0 && env_int("GRIDDER_TMEM", 0)) {
+        const size_t cols = oo * p.cls[0].NA * p.cls[0].NB;
+        if (cols <= 512) {
+            p.tmem_cols = 32;
+            while ((size_t)p.tmem_cols < cols) p.tmem_cols *= 2;
+        }
+    }
     p.chunk = env_int("GRIDDER_CHUNK", 4096);
     if (p.chunk < 32 || p.chunk > (1 << 20)) return GRIDDER_ERR_INVALID_ARG;
     p.warps_forced = env_int("GRIDDER_WARPS", 0);

@@ -25,6 +25,9 @@ namespace gridder {
 // MODE 0: one real table with S <= 16, resident in shared memory, 32-bit (key, index) entries.
 // MODE 1: real tables read from global memory (any number of planes, sub-patches), wide entries.
 // MODE 2: complex tables (w-planes), conjugated for w < 0, read from global memory, wide entries.
+// MODE 3: as MODE 0, but the table lives in TENSOR MEMORY: lane l of every warp reads its NA*NB taps of
+//         sub-table q with one tcgen05.ld (32 lanes x 32 bit x NA*NB columns at column q*NA*NB), which
+//         takes the taps off the shared-memory return path -- the path this kernel is bound by.
 // NSUB > 1: an entry covers NSUB x NSUB register patches (supports 17..32), gridded one after the other.
 constexpr int kSentinel = -(1 << 20);   // origin of the record that ends a work item
 constexpr int kForce = INT_MIN;         // never an origin: forces a fold at the next record
@@ -32,7 +35,8 @@ constexpr int kForce = INT_MIN;         // never an origin: forces a fold at the
 template <int NA, int NB, int NSUB, int TLOG, int MODE>
 struct Geo {
     static constexpr bool CPLX = MODE == 2;
-    static constexpr bool GEN = MODE != 0;
+    static constexpr bool GEN = MODE == 1 || MODE == 2;
+    static constexpr bool TMEM = MODE == 3;
     static constexpr int SPX = 8 * NA, SPY = 4 * NB;           // register patch
     static constexpr int T = 1 << TLOG;
     static constexpr int RW = T + SPX * NSUB - 1, RH = T + SPY * NSUB - 1;   // region = tile + halo
@@ -193,7 +197,7 @@ __device__ __forceinline__ void stage_write(const GridParams &p, const float4 *r
         const uint32_t qmask = (1u << (2 * p.key.bits_q)) - 1u;
         x0l = (k.key >> p.key.aux_bits) & tmask;
         y0l = (k.key >> (p.key.aux_bits + TLOG)) & tmask;
-        coff = (int)((k.key & qmask) * (uint32_t)G::SUB_BYTES);
+        coff = (int)((k.key & qmask) * (uint32_t)(G::TMEM ? NA * NB : G::SUB_BYTES));   // bytes, or TMEM columns
     }
     const int poff = (int)(y0l * G::RW + x0l);
     const int last_poff = __shfl_sync(0xffffffffu, poff, cnt - 1);
@@ -237,6 +241,17 @@ struct RecRegs {
     __device__ __forceinline__ void fetch(const float4 *slot, const int coff, const char *coef_lane) {
 #pragma unroll
         for (int i = 0; i < VF4; ++i) v[i] = slot[i];
+        if (MODE == 3) {                                       // tensor memory: one load for all NA*NB taps
+            const uint32_t ta = (uint32_t)(uintptr_t)coef_lane + (uint32_t)coff;
+            if (NA * NB == 8) {
+                asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                             : "=f"(c[0][0]), "=f"(c[0][1]), "=f"(c[0][2]), "=f"(c[0][3]),
+                               "=f"(c[NA - 1][0]), "=f"(c[NA - 1][1]), "=f"(c[NA - 1][2]), "=f"(c[NA - 1][3]) : "r"(ta));
+            } else {
+                asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=f"(c[0][0]), "=f"(c[0][1]) : "r"(ta));
+            }
+            return;
+        }
         const char *cp = coef_lane + coff;
 #pragma unroll
         for (int a = 0; a < NA; ++a) {
@@ -259,6 +274,19 @@ struct RecRegs {
                     const float2 t = __ldg(reinterpret_cast<const float2 *>(ca));
                     c[a][0] = t.x; c[a][1] = t.y;
                 }
+            }
+        }
+    }
+    // MODE 3: the taps are usable only after this (it waits for the warp's outstanding tcgen05.ld);
+    // the registers go through the statement so that no use is scheduled above it.
+    __device__ __forceinline__ void wait() {
+        if (MODE == 3) {
+            if (NA * NB == 8) {
+                asm volatile("tcgen05.wait::ld.sync.aligned;"
+                             : "+f"(c[0][0]), "+f"(c[0][1]), "+f"(c[0][2]), "+f"(c[0][3]),
+                               "+f"(c[NA - 1][0]), "+f"(c[NA - 1][1]), "+f"(c[NA - 1][2]), "+f"(c[NA - 1][3]));
+            } else {
+                asm volatile("tcgen05.wait::ld.sync.aligned;" : "+f"(c[0][0]), "+f"(c[0][1]));
             }
         }
     }
@@ -285,6 +313,16 @@ __device__ __forceinline__ void fold_patch(float4 *regA, float4 *regB, int base,
         }
 }
 
+// (d0, d1) += c * (v0, v1), each product-sum rounded once (two independent IEEE FMAs in one instruction).
+__device__ __forceinline__ void ffma2(float &d0, float &d1, float c, float v0, float v1) {
+    unsigned long long d, a, b;
+    asm("mov.b64 %0, {%1,%2};" : "=l"(d) : "f"(d0), "f"(d1));
+    asm("mov.b64 %0, {%1,%2};" : "=l"(a) : "f"(c), "f"(c));
+    asm("mov.b64 %0, {%1,%2};" : "=l"(b) : "f"(v0), "f"(v1));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b));
+    asm("mov.b64 {%0,%1}, %2;" : "=f"(d0), "=f"(d1) : "l"(d));
+}
+
 // `cmp` is the origin the patch was last matched against (kForce forces a fold at the next record, used
 // to bound the chain length); `cur` is the origin the registers really belong to (-1: none).
 template <int NA, int NB, int RW, int MODE>
@@ -294,35 +332,34 @@ __device__ __forceinline__ void consume(const RecRegs<NA, NB, MODE> &R, const in
         if (cur >= 0) fold_patch<NA, NB, RW>(regA, regB, cur + lane_cell, acc);
         cur = cmp = poff;
     }
+    // Packed FP32 pairs (Blackwell fma.rn.f32x2 -> FFMA2 with the tap as a scalar broadcast operand): one
+    // instruction updates (re, im) of one polarisation of one cell, halving the issue slots of the loop.
     if (MODE == 2) {
-        const float vr[4] = {R.v[0].x, R.v[0].z, R.v[1].x, R.v[1].z};
-        const float vi[4] = {R.v[0].y, R.v[0].w, R.v[1].y, R.v[1].w};
-        const float pp[4] = {R.v[2].x, R.v[2].z, R.v[3].x, R.v[3].z};
-        const float qq[4] = {R.v[2].y, R.v[2].w, R.v[3].y, R.v[3].w};
 #pragma unroll
         for (int a = 0; a < NA; ++a)
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
                 const float cr = R.c[a][2 * b], ci = R.c[a][2 * b + 1];
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    acc[a][b][2 * k] = fmaf(cr, vr[k], acc[a][b][2 * k]);
-                    acc[a][b][2 * k + 1] = fmaf(cr, vi[k], acc[a][b][2 * k + 1]);
-                }
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    acc[a][b][2 * k] = fmaf(ci, pp[k], acc[a][b][2 * k]);
-                    acc[a][b][2 * k + 1] = fmaf(ci, qq[k], acc[a][b][2 * k + 1]);
-                }
+                ffma2(acc[a][b][0], acc[a][b][1], cr, R.v[0].x, R.v[0].y);
+                ffma2(acc[a][b][2], acc[a][b][3], cr, R.v[0].z, R.v[0].w);
+                ffma2(acc[a][b][4], acc[a][b][5], cr, R.v[1].x, R.v[1].y);
+                ffma2(acc[a][b][6], acc[a][b][7], cr, R.v[1].z, R.v[1].w);
+                ffma2(acc[a][b][0], acc[a][b][1], ci, R.v[2].x, R.v[2].y);
+                ffma2(acc[a][b][2], acc[a][b][3], ci, R.v[2].z, R.v[2].w);
+                ffma2(acc[a][b][4], acc[a][b][5], ci, R.v[3].x, R.v[3].y);
+                ffma2(acc[a][b][6], acc[a][b][7], ci, R.v[3].z, R.v[3].w);
             }
     } else {
-        const float v[8] = {R.v[0].x, R.v[0].y, R.v[0].z, R.v[0].w, R.v[1].x, R.v[1].y, R.v[1].z, R.v[1].w};
 #pragma unroll
         for (int a = 0; a < NA; ++a)
 #pragma unroll
-            for (int b = 0; b < NB; ++b)
-#pragma unroll
-                for (int k = 0; k < 8; ++k) acc[a][b][k] = fmaf(R.c[a][b], v[k], acc[a][b][k]);
+            for (int b = 0; b < NB; ++b) {
+                const float c = R.c[a][b];
+                ffma2(acc[a][b][0], acc[a][b][1], c, R.v[0].x, R.v[0].y);
+                ffma2(acc[a][b][2], acc[a][b][3], c, R.v[0].z, R.v[0].w);
+                ffma2(acc[a][b][4], acc[a][b][5], c, R.v[1].x, R.v[1].y);
+                ffma2(acc[a][b][6], acc[a][b][7], c, R.v[1].z, R.v[1].w);
+            }
     }
 }
 
@@ -346,7 +383,44 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
 
     const int lane_cell = (lane >> 3) * G::RW + (lane & 7);      // tap (a=0, b=0) of this lane
     const char *coef_lane;
-    if constexpr (MODE == 0)
+    uint32_t tmem_base = 0;
+    if constexpr (MODE == 3) {
+        // the table goes to tensor memory: warp w (< 4) fills lane quadrant w, lane l its own taps
+        __shared__ uint32_t tmem_base_s;
+        if (warp == 0) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                         :: "r"((uint32_t)__cvta_generic_to_shared(&tmem_base_s)), "r"((uint32_t)p.tmem_cols) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        tmem_base = tmem_base_s;
+        if (warp < 4) {
+            const uint32_t tl = tmem_base + ((uint32_t)(warp * 32) << 16);
+            const float *tab = reinterpret_cast<const float *>(p.coef);
+            for (int q = 0; q < p.n_q; ++q) {
+                float t[NA * NB];
+#pragma unroll
+                for (int a = 0; a < NA; ++a)
+#pragma unroll
+                    for (int b = 0; b < NB; ++b) t[a * NB + b] = tab[((q * NA + a) * 32 + lane) * NB + b];
+                const uint32_t ta = tl + (uint32_t)(q * NA * NB);
+                if (NA * NB == 8) {
+                    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                                 :: "r"(ta), "f"(t[0]), "f"(t[1]), "f"(t[2]), "f"(t[3]), "f"(t[4 % (NA * NB)]),
+                                    "f"(t[5 % (NA * NB)]), "f"(t[6 % (NA * NB)]), "f"(t[7 % (NA * NB)]) : "memory");
+                } else {
+                    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" :: "r"(ta), "f"(t[0]), "f"(t[1]) : "memory");
+                }
+            }
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        coef_lane = reinterpret_cast<const char *>((uintptr_t)(tmem_base + ((uint32_t)((warp & 3) * 32) << 16)));
+    } else if constexpr (MODE == 0)
         coef_lane = reinterpret_cast<const char *>((uintptr_t)((uint32_t)__cvta_generic_to_shared(smem) +
                                                               lane * RecRegs<NA, NB, MODE>::CF * (int)sizeof(float)));
     else
@@ -410,9 +484,11 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
                 }
                 do {
                     mB = *reinterpret_cast<const int2 *>(sp + G::SLOT_F4 + G::VF4);
+                    A.wait();
                     B.fetch(sp + G::SLOT_F4, mA.x, cl);
                     consume<NA, NB, G::RW, MODE>(A, mA.y + sub_poff, cur, cmp, regA, regB, lane_cell, acc);
                     mA = *reinterpret_cast<const int2 *>(sp + 2 * G::SLOT_F4 + G::VF4);
+                    B.wait();
                     A.fetch(sp + 2 * G::SLOT_F4, mB.x, cl);
                     consume<NA, NB, G::RW, MODE>(B, mB.y + sub_poff, cur, cmp, regA, regB, lane_cell, acc);
                     sp += 2 * G::SLOT_F4;
@@ -438,6 +514,13 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
         par ^= 1;
     }
     cp_async_wait_all();
+    if constexpr (MODE == 3) {
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (warp == 0)
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base), "r"((uint32_t)p.tmem_cols) : "memory");
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -522,15 +605,18 @@ template <int MODE, int MAXW>
 static grid_fn_t pick_shape(const ClassGeo &g, int tlog) {
     if (g.NA == 1 && g.nsub == 1) return pick_tlog<1, 2, 1, MODE, MAXW>(tlog);
     if (g.NA == 2 && g.nsub == 1) return pick_tlog<2, 4, 1, MODE, MAXW>(tlog);
-    if constexpr (MODE != 0) {
+    if constexpr (MODE == 1 || MODE == 2) {
         if (g.NA == 2 && g.nsub == 2) return pick_tlog<2, 4, 2, MODE, MAXW>(tlog);
     }
     return nullptr;
 }
 
+static int kernel_mode(const Plan &p) { return (p.mode == 0 && p.tmem_cols > 0) ? 3 : p.mode; }
+
 static grid_fn_t pick_grid(const ClassGeo &g, int tlog, int mode) {
     switch (mode) {
         case 0: return pick_shape<0, kMaxWarpsFast>(g, tlog);
+        case 3: return pick_shape<3, kMaxWarpsFast>(g, tlog);
         case 1: return pick_shape<1, kMaxWarpsGeneral>(g, tlog);
         case 2: return pick_shape<2, kMaxWarpsGeneral>(g, tlog);
         default: return nullptr;
@@ -571,12 +657,12 @@ cudaError_t configure_grid_kernel(Plan &p) {
         for (int w : kWarpChoices) {
             if (w > cap) continue;
             if (p.warps_forced > 0 && w > p.warps_forced) continue;      // the caller's limit (tuning, tests)
-            if (grid_smem_bytes(g, p.tlog, p.mode, p.coef_bytes, w) <= (size_t)smem_max) { chosen = w; break; }
+            if (grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, w) <= (size_t)smem_max) { chosen = w; break; }
         }
         if (!chosen) return cudaErrorInvalidConfiguration;
         g.warps = chosen;
-        g.smem_bytes = (int)grid_smem_bytes(g, p.tlog, p.mode, p.coef_bytes, chosen);
-        grid_fn_t fn = pick_grid(g, p.tlog, p.mode);
+        g.smem_bytes = (int)grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, chosen);
+        grid_fn_t fn = pick_grid(g, p.tlog, kernel_mode(p));
         if (!fn) return cudaErrorInvalidConfiguration;
         e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes);
         if (e != cudaSuccess) return e;
@@ -592,7 +678,7 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
     if (e != cudaSuccess) return e;
     for (int c = 0; c < p.n_cls; ++c) {
         const ClassGeo &g = p.cls[c];
-        grid_fn_t gfn = pick_grid(g, p.tlog, p.mode);
+        grid_fn_t gfn = pick_grid(g, p.tlog, kernel_mode(p));
         if (!gfn) return cudaErrorInvalidConfiguration;
         GridParams gp;
         gp.keys = p.keys[p.sorted_sel];
@@ -608,6 +694,8 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         gp.fold_mask = p.fold_batches - 1;
         gp.cls = c;
         gp.sub_stride_bytes = p.cfg.oversample * p.cfg.oversample * g.sub_bytes;
+        gp.tmem_cols = p.tmem_cols;
+        gp.n_q = p.cfg.oversample * p.cfg.oversample;
         gfn<<<p.n_sm, g.warps * 32, g.smem_bytes, s>>>(gp);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;

@@ -110,6 +110,8 @@ struct GridParams {
     int32_t fold_mask;             // register chains are folded every (fold_mask + 1) batches of 32
     int32_t cls;                   // class slot of this launch
     int32_t sub_stride_bytes;      // table distance between sub-patches (O^2 sub-tables)
+    int32_t tmem_cols;             // tensor-memory columns to allocate (MODE 3)
+    int32_t n_q;                   // O^2 sub-tables
     KeyLayout key;
 };
 
@@ -129,6 +131,7 @@ struct Plan {
     int32_t support_copy[kMaxPlanes];
     // derived
     int32_t mode;                  // 0 fast real, 1 general real, 2 general complex
+    int32_t tmem_cols;             // > 0: fast path with the table in tensor memory (columns to allocate)
     int32_t n_cls;                 // class slots in use
     ClassGeo cls[kMaxClasses];
     int32_t plane_slot[kMaxPlanes];
