@@ -127,6 +127,17 @@ GRIDDER_API int gridder_get_stats(gridder_plan_t *plan, gridder_stats *out);
 GRIDDER_API int gridder_map(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
                 const double *freq_hz, int32_t n_chan, int32_t *out, void *cuda_stream);
 
+/* the arithmetic of the paper's OpenGL gridder (PAPER.md :185-191: one
+ * screen-aligned GCF quad per visibility, additive blending) as plain CUDA: every (visibility, tap,
+ * polarisation) is an FP32 atomic add into `grid`.  No binning, no workspace use beyond the plan; needs
+ * no gridder_bin.  NOT deterministic (the order of the atomic additions is not fixed) and FP32 chains
+ * are unbounded, so heavily loaded cells drift beyond the binned path's tolerance: a same-box
+ * comparison path, not the product path.  cfg.kernel (the caller's table) must still be valid.
+ * Asynchronous on `cuda_stream`. */
+GRIDDER_API int gridder_scatter_atomic(gridder_plan_t *plan, const double *uvw_m, int32_t n_time,
+                                       int32_t n_baseline, const double *freq_hz, int32_t n_chan, const float *vis,
+                                       const float *weight, float *grid, int32_t accumulate, void *cuda_stream);
+
 /* End-to-end convenience with HOST buffers (pinned or pageable): copies uvw, freq, vis, weight to
  * the caller's device staging buffers, runs gridder_bin + gridder_grid and copies the grid back,
  * all on `cuda_stream`, then synchronises it.  d_* are DEVICE buffers at least as large as their

@@ -289,6 +289,23 @@ int gridder_map(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32
     return GRIDDER_OK;
 }
 
+int gridder_scatter_atomic(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
+                           const double *freq_hz, int32_t n_chan, const float *vis, const float *weight, float *grid,
+                           int32_t accumulate, void *cuda_stream) {
+    Plan *p = reinterpret_cast<Plan *>(plan);
+    if (!p || !grid || n_time < 0 || n_baseline < 0 || n_chan < 0) return GRIDDER_ERR_INVALID_ARG;
+    const int64_t n = (int64_t)n_time * n_baseline * n_chan;
+    if (n > 0 && (!uvw_m || !freq_hz || !vis)) return GRIDDER_ERR_INVALID_ARG;
+    if (n > 0xFFFFFFF0ll) return GRIDDER_ERR_CAPACITY;
+    if (((uintptr_t)vis & 15) || ((uintptr_t)grid & 7)) return GRIDDER_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaError_t e = launch_scatter_atomic(*p, uvw_m, n_time, n_baseline, freq_hz, n_chan, vis, weight, grid,
+                                          accumulate ? 1 : 0, s);
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    p->last_stream = s;
+    return GRIDDER_OK;
+}
+
 int gridder_run_host(gridder_plan_t *plan, const double *h_uvw_m, int32_t n_time, int32_t n_baseline,
                      const double *h_freq_hz, int32_t n_chan, const float *h_vis, const float *h_weight,
                      float *h_grid, double *d_uvw_m, double *d_freq_hz, float *d_vis, float *d_weight,

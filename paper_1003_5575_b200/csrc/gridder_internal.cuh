@@ -188,6 +188,11 @@ cudaError_t launch_map_debug(const Plan &p, const double *uvw, int n_time, int n
 cudaError_t sort_temp_bytes(int64_t n, int begin_bit, int end_bit, bool wide, size_t *bytes);
 cudaError_t scan_temp_bytes(int64_t n, size_t *bytes);
 
+// scatter.cu
+cudaError_t launch_scatter_atomic(Plan &p, const double *uvw, int n_time, int n_bl, const double *freq, int n_chan,
+                                  const float *vis, const float *weight, float *grid, int accumulate,
+                                  cudaStream_t s);
+
 // grid.cu
 cudaError_t configure_grid_kernel(Plan &p);          // picks warps/smem per class, sets the smem attribute
 cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *grid, int accumulate,

@@ -1,0 +1,86 @@
+// The uvw -> (patch origin, sub-cell offset, w-plane) mapping shared by the library's kernels
+// (map kernel of gridder_bin, gridder_map, the atomic-scatter gridder).  Not shared with the oracle.
+#pragma once
+#include "gridder_internal.cuh"
+
+namespace gridder {
+
+// ------------------------------------------------------------------------------------------
+// The mapping (steps 1-4).  Every FP64 operation is an explicit
+// round-to-nearest intrinsic, so no FMA contraction can change a result: this must agree with the
+// definition to the last bit, because one visibility in the wrong sub-cell is far outside the
+// tolerance.
+// ------------------------------------------------------------------------------------------
+struct AxisMap {
+    long long x0;   // patch origin
+    int q;          // sub-cell table offset in [0, O)
+    bool far;       // hopelessly off the grid
+};
+
+static __device__ __noinline__ void map_axis_wide(double r, int S, int O, long long *x0, int *q) {
+    // the same algebra in 64 bits, for positions far outside any grid (always dropped, but the
+    // test interface reports them)
+    const long long X = (long long)r, OO = O;
+    const long long A = X - ((long long)S * OO) / 2;
+    const long long n = A + OO - 1;
+    long long d = n / OO;
+    if ((n % OO != 0) && (n < 0)) d -= 1;
+    *x0 = d;
+    *q = (int)(d * OO - A);
+}
+
+__device__ __forceinline__ AxisMap map_axis(double coord_lambda, const MapParams &p, int S) {
+    AxisMap m;
+    const double a = __ddiv_rn(coord_lambda, p.cell_size);
+    const double g = __dadd_rn(a, (double)(p.n_grid / 2));
+    const double h = __dmul_rn(g, (double)p.oversample);
+    const double r = floor(__dadd_rn(h, 0.5));
+    const int O = p.oversample;
+    m.far = false;
+    if (r > -1073741824.0 && r < 1073741824.0) {
+        // |X| < 2^30 sub-cells (N*O <= 2^21 for every accepted plan): 32-bit integer algebra
+        const int X = (int)r;
+        const int A = X - (S * O) / 2;
+        const int n = A + O - 1;              // x0 = ceil(A / O) = floor((A + O - 1) / O)
+        int x0 = n / O;
+        if ((n % O != 0) && (n < 0)) x0 -= 1;
+        m.x0 = x0;
+        m.q = x0 * O - A;
+    } else if (r > -1.0e15 && r < 1.0e15) {
+        map_axis_wide(r, S, O, &m.x0, &m.q);
+    } else {
+        m.far = true;
+        m.x0 = -(1ll << 61);
+        m.q = 0;
+    }
+    return m;
+}
+
+struct VisMap {
+    long long x0, y0;
+    int qx, qy, plane, conj, S;
+    bool dropped;
+};
+
+__device__ __forceinline__ VisMap map_vis(double u_m, double v_m, double w_m, double s, const MapParams &p) {
+    const double ul = __dmul_rn(u_m, s), vl = __dmul_rn(v_m, s);
+    VisMap m;
+    m.plane = 0;
+    m.conj = 0;
+    if (p.n_planes > 1 || p.is_complex) {
+        const double wl = __dmul_rn(w_m, s);
+        if (p.n_planes > 1) {
+            const double fp = floor(__dmul_rn(__ddiv_rn(fabs(wl), p.w_max), (double)p.n_planes));
+            m.plane = (fp >= (double)(p.n_planes - 1)) ? p.n_planes - 1 : (int)fp;
+        }
+        m.conj = (p.is_complex && wl < 0.0) ? 1 : 0;
+    }
+    m.S = p.support[m.plane];
+    const AxisMap mx = map_axis(ul, p, m.S), my = map_axis(vl, p, m.S);
+    m.x0 = mx.x0; m.y0 = my.x0; m.qx = mx.q; m.qy = my.q;
+    const long long N = p.n_grid, S = m.S;
+    m.dropped = mx.far || my.far || m.x0 < 0 || m.x0 + S > N || m.y0 < 0 || m.y0 + S > N;
+    return m;
+}
+
+}  // namespace gridder

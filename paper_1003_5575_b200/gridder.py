@@ -18,7 +18,7 @@ LIB_PATH = _HERE / "libgridder.so"
 OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_WORKSPACE, ERR_CUDA, ERR_NOT_BINNED, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = ("gridder_workspace_size", "gridder_plan", "gridder_bin", "gridder_grid", "gridder_destroy",
-           "gridder_get_stats", "gridder_map", "gridder_run_host", "gridder_set_profiling",
+           "gridder_get_stats", "gridder_map", "gridder_scatter_atomic", "gridder_run_host", "gridder_set_profiling",
            "gridder_get_stage_ms", "gridder_launch_count", "gridder_strerror",
            "gridder_last_cuda_error", "gridder_version")
 
@@ -62,6 +62,8 @@ def load_library() -> C.CDLL:
         lib.gridder_get_stats.argtypes = [C.c_void_p, C.POINTER(_Stats)]
         lib.gridder_map.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
                                     C.c_void_p, C.c_void_p]
+        lib.gridder_scatter_atomic.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
+                                               C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
         lib.gridder_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -220,6 +222,23 @@ class Gridder:
                                    _stream_ptr(stream))
         if rc != OK:
             raise GridderError(rc, "gridder_map")
+        return out
+
+    def scatter_atomic(self, uvw_m, freq_hz, vis, weight=None, out=None, accumulate: bool = False, stream=None):
+        """per-visibility FP32 atomic scatter (the OpenGL gridder's arithmetic); not deterministic."""
+        if uvw_m.dim() == 2:
+            uvw_m = uvw_m[None]
+        n_time, n_bl, _ = uvw_m.shape
+        if out is None:
+            if accumulate:
+                raise ValueError("accumulate needs an existing grid")
+            out = torch.empty((4, self.grid_size, self.grid_size, 2), dtype=torch.float32, device=self.device)
+        rc = self._lib.gridder_scatter_atomic(
+            self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m"), n_time, n_bl, _dev_ptr(freq_hz, torch.float64, "freq_hz"),
+            freq_hz.numel(), _dev_ptr(vis, torch.float32, "vis"), _dev_ptr(weight, torch.float32, "weight"),
+            _dev_ptr(out, torch.float32, "grid"), int(accumulate), _stream_ptr(stream))
+        if rc != OK:
+            raise GridderError(rc, "gridder_scatter_atomic")
         return out
 
     def run_host(self, uvw_m, freq_hz, vis, weight, grid_out, staging: dict, stream=None) -> None:

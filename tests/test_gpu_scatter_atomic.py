@@ -1,0 +1,72 @@
+"""the atomic-scatter gridder (the OpenGL gridder's arithmetic, PAPER.md :185-191) against
+the oracle.  The additions are FP32 atomics in no fixed order, so only the tolerance is checked (never
+bit-identity), on inputs whose cells carry short sums; config 1 at full size is reported, not asserted
+beyond a loose bound -- the point the paper makes about scatter (:185) and the reason the product path bins."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+from _util import as_complex, assert_parity, oracle_kwargs
+
+pytestmark = pytest.mark.gpu
+C = 299_792_458.0
+
+
+@pytest.fixture(scope="module")
+def dev():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1003_5575_b200 import gridder
+    gridder.load_library()
+    return torch.device("cuda:0")
+
+
+def _plan(dev, *, N, du, O, supports, table, w_max=1.0, cplx=False, max_vis=1):
+    from paper_1003_5575_b200 import gridder
+    return gridder.Gridder(grid_size=N, cell_size=du, oversample=O, support=list(supports),
+                           kernel=torch.from_numpy(np.ascontiguousarray(table, np.float32).ravel()).to(dev),
+                           max_vis=max_vis, n_wplanes=len(supports), w_max=w_max, kernel_is_complex=cplx)
+
+
+@pytest.mark.parametrize("S,O,N,cplx", [(16, 4, 96, False), (7, 8, 64, False), (15, 8, 80, False), (24, 2, 90, True)])
+def test_atomic_scatter_matches_oracle_on_sparse_inputs(dev, S, O, N, cplx):
+    rng = np.random.default_rng(S + N)
+    n = 3000
+    shape = (S * O, S * O, 2) if cplx else (S * O, S * O)
+    table = rng.standard_normal(shape).astype(np.float32).ravel()
+    uvw = np.zeros((1, n, 3))
+    uvw[0, :, :2] = rng.uniform(-N / 2 - 1, N / 2 + 1, (n, 2))
+    uvw[0, :, 2] = rng.uniform(-1.0, 1.0, n)
+    vis = rng.standard_normal((n, 4, 2)).astype(np.float32)
+    w = rng.uniform(0.5, 1.5, n).astype(np.float32)
+    g = _plan(dev, N=N, du=1.0, O=O, supports=[S], table=table, cplx=cplx, max_vis=n)
+    d_uvw, d_f = torch.from_numpy(uvw).to(dev), torch.tensor([C], dtype=torch.float64, device=dev)
+    got = g.scatter_atomic(d_uvw, d_f, torch.from_numpy(vis).to(dev), torch.from_numpy(w).to(dev)).cpu().numpy()
+    base = rng.standard_normal((4, N, N, 2)).astype(np.float32)
+    acc = g.scatter_atomic(d_uvw, d_f, torch.from_numpy(vis).to(dev), torch.from_numpy(w).to(dev),
+                           out=torch.from_numpy(base.copy()).to(dev), accumulate=True).cpu().numpy()
+    g.destroy()
+    ref, ab, ost = oracle.grid_full(uvw, [C], vis, w, grid_size=N, cell_size=1.0, oversample=O, support=[S], kernel=table,
+                                    kernel_is_complex=cplx)
+    assert ost["n_dropped"] > 0
+    assert_parity(got, ref, ab, f"atomic scatter S={S}")
+    assert_parity(acc, ref + as_complex(base), ab + np.abs(as_complex(base)), "atomic scatter, accumulate")
+
+
+def test_atomic_scatter_config1_and_binned_path_agree(dev):
+    wl = synth.make_workload(1)
+    vis = wl.visibilities("cpu")
+    g = _plan(dev, N=wl.grid_size, du=wl.cell_size, O=wl.oversample, supports=wl.support, table=wl.kernel, max_vis=wl.n_vis)
+    d_uvw, d_f, d_v = torch.from_numpy(wl.uvw).to(dev), torch.from_numpy(wl.freq).to(dev), vis.to(dev)
+    got = g.scatter_atomic(d_uvw, d_f, d_v).cpu().numpy()
+    g.bin(d_uvw, d_f)
+    binned = g.grid(d_v).cpu().numpy()
+    g.destroy()
+    ref, ab, _ = oracle.grid_full(wl.uvw, wl.freq, vis.numpy(), None, **oracle_kwargs(wl))
+    assert_parity(binned, ref, ab, "binned path, config 1")
+    err = np.abs(as_complex(got) - ref) / (1e-5 * ab + 1e-6)
+    print(f"atomic scatter on config 1: worst err/tol {err.max():.2f} (binned path: "
+          f"{(np.abs(as_complex(binned) - ref) / (1e-5 * ab + 1e-6)).max():.3f})")
+    assert err.max() < 50.0          # unbounded FP32 chains: reported, loosely bounded, not held to 1e-5
