@@ -38,7 +38,10 @@ FP32_LANES_PER_SM = 128          # guide: 4 SMSP x 32 lanes, one FFMA per lane p
 BAND_HZ = 768 * 40.0e3           # one rank's band; rank r starts at 140 MHz + r * BAND_HZ
 # dram__bytes_read.sum + dram__bytes_write.sum of one grid_kernel launch from the committed
 # `ncu --set full` capture (profiles/), keyed by config; None until a capture exists for it.
-NCU_GRID_KERNEL_TRAFFIC_BYTES = {}
+NCU_GRID_KERNEL_TRAFFIC_BYTES = {
+    4: 53_944_551_000,    # profiles/r01b_grid_kernel_config4_ncu_full.csv: 47.322367 GB read + 6.622184 GB written
+    2: 9_348_989_000,     # profiles/r01_grid_kernel_config2_ncu_full.csv: 4.109023 GB read + 5.239966 GB written
+}
 
 
 def parse_args():
@@ -51,6 +54,8 @@ def parse_args():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (development only)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle leg (development only)")
+    ap.add_argument("--atomic", action="store_true",
+                    help="also time the atomic-scatter gridder (SURVEY row f1) once on the same workload")
     return ap.parse_args()
 
 
@@ -333,6 +338,18 @@ def run_ours(args) -> dict | None:
                "d2h_bytes_per_step": int(h_grid.numel() * 4), "ms_per_step": agg_e["ms_per_step"],
                "steps": e_steps, "n_time": nt_e, "result_checksum": float(h_grid[0, wl.grid_size // 2, wl.grid_size // 2, 0])}
         del h_vis, h_w, h_grid
+    f1 = None
+    if args.atomic:
+        # row f1: per-visibility FP32 atomic scatter, same inputs, one warm-up and one timed pass
+        g.scatter_atomic(d_uvw, d_freq, vis, weight, out=grid)
+        barrier()
+        e0.record()
+        g.scatter_atomic(d_uvw, d_freq, vis, weight, out=grid)
+        e1.record()
+        barrier()
+        ms_f1 = e0.elapsed_time(e1)
+        f1 = {"ms": ms_f1, "value": st.vis_taps / (ms_f1 * 1e-3), "unit": UNIT,
+              "note": "gridder_scatter_atomic: no binning, red.global.add.v2.f32 per (tap, pol); not deterministic"}
     g.destroy()
     if world > 1:
         dist.destroy_process_group()
@@ -378,6 +395,8 @@ def run_ours(args) -> dict | None:
         "stage_ms": stage, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
         "cadence_budget_s": 8.0, "result_checksum": checksum,
     }
+    if f1 is not None:
+        out["f1_atomic_scatter"] = f1
     if e2e is not None:
         out["e2e"] = e2e
     if world == 1 and not args.no_cpu:

@@ -138,6 +138,17 @@ GRIDDER_API int gridder_scatter_atomic(gridder_plan_t *plan, const double *uvw_m
                                        int32_t n_baseline, const double *freq_hz, int32_t n_chan, const float *vis,
                                        const float *weight, float *grid, int32_t accumulate, void *cuda_stream);
 
+/* the imaging step that follows the gridder (PAPER.md :75, :211, :217): centred
+ * unnormalised 2-D inverse DFT of the 4 polarisation planes with the grid correction fused in,
+ *   image[pol][y][x] = corr[y] corr[x] sum_{v,u} grid[pol][v][u] exp(+2 pi i ((u-N/2)(x-N/2) + (v-N/2)(y-N/2)) / N).
+ * grid, image: DEVICE float [4][N][N][2] (may be the same buffer); corr: DEVICE float [N] (1 / Fourier
+ * transform of the separable GCF at pixel k; NULL = no correction); work: DEVICE scratch of
+ * gridder_image_workspace_size bytes for the FFT (cuFFT, loaded on first use; GRIDDER_ERR_UNSUPPORTED
+ * if it cannot be loaded).  Asynchronous on `cuda_stream`; the first call builds the FFT plan. */
+GRIDDER_API int gridder_image_workspace_size(gridder_plan_t *plan, size_t *bytes);
+GRIDDER_API int gridder_image(gridder_plan_t *plan, const float *grid, float *image, const float *corr, void *work,
+                              size_t work_bytes, void *cuda_stream);
+
 /* End-to-end convenience with HOST buffers (pinned or pageable): copies uvw, freq, vis, weight to
  * the caller's device staging buffers, runs gridder_bin + gridder_grid and copies the grid back,
  * all on `cuda_stream`, then synchronises it.  d_* are DEVICE buffers at least as large as their

@@ -167,3 +167,30 @@ def grid_full(uvw_m, freq_hz, vis, weight=None, *, grid_size, cell_size, oversam
     if rc:
         raise RuntimeError("oracle_grid_windows: invalid argument")
     return g, ab, {"n_dropped": int(stats[0]), "vis_taps": int(stats[1]), "threads": nb}
+
+
+# ---- row f2: the imaging step after the gridder (test infrastructure, like everything here) --------------
+def grid_correction(table_1d, support: int, oversample: int, grid_size: int) -> np.ndarray:
+    """1 / c_hat(l_k) for image pixels k = 0..N-1 (l_k = (k - N/2) / N cycles per cell), where
+    c_hat(l) = (1/O) sum_j T1[j] cos(2 pi r_j l), r_j = (j - S O / 2) / O: the Fourier transform of the
+    (separable, even) tabulated GCF itself (R4; PAPER.md :75 "grid correction")."""
+    t1 = np.asarray(table_1d, dtype=np.float64)
+    r = (np.arange(support * oversample) - (support * oversample) / 2.0) / oversample
+    lk = (np.arange(grid_size) - grid_size // 2) / grid_size
+    chat = (t1[None, :] * np.cos(2.0 * np.pi * r[None, :] * lk[:, None])).sum(1) / oversample
+    return 1.0 / chat
+
+
+def image(grid_c: np.ndarray, corr=None) -> np.ndarray:
+    """Dirty image of a gridded plane set, complex128 [..., N, N]: the unnormalised inverse DFT with both
+    planes centred on cell N/2, times corr[y] corr[x] (PAPER.md :75, :211):
+        image[y][x] = corr[y] corr[x] sum_{v,u} G[v][u] exp(+2 pi i ((u-N/2)(x-N/2) + (v-N/2)(y-N/2)) / N).
+    Written with the library FFT as the step the definition names; pinned in tests/test_oracle_pins.py against
+    the O(N^4) sum written out and (P4) against the direct DFT of a point source."""
+    g = np.asarray(grid_c, dtype=np.complex128)
+    n = g.shape[-1]
+    img = np.fft.fftshift(np.fft.ifft2(np.fft.ifftshift(g, axes=(-2, -1)), axes=(-2, -1)), axes=(-2, -1)) * (n * n)
+    if corr is not None:
+        c = np.asarray(corr, dtype=np.float64)
+        img = img * (c[:, None] * c[None, :])
+    return img

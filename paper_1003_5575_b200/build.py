@@ -14,7 +14,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libgridder.so"
-SOURCES = ["api.cu", "bin.cu", "grid.cu", "scatter.cu"]
+SOURCES = ["api.cu", "bin.cu", "grid.cu", "scatter.cu", "image.cu"]
 HEADERS = [CSRC / "gridder_internal.cuh", CSRC / "map.cuh", HERE.parent / "include" / "gridder.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]
@@ -49,7 +49,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
     if force or procs or _stale(LIB, objs):
         tmp = LIB.with_suffix(f".{os.getpid()}.tmp")
-        cmd = [_nvcc(), "-shared", "-o", str(tmp)] + [str(o) for o in objs] + ["-lcudart"]
+        cmd = [_nvcc(), "-shared", "-o", str(tmp)] + [str(o) for o in objs] + ["-lcudart", "-ldl"]
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)
     return LIB

@@ -248,6 +248,7 @@ int gridder_destroy(gridder_plan_t *plan) {
     Plan *p = reinterpret_cast<Plan *>(plan);
     if (!p) return GRIDDER_ERR_INVALID_ARG;
     cudaError_t e = cudaDeviceSynchronize();     // the caller may free the workspace after this
+    image_destroy(*p);
     for (int r = 0; r < kProfRing; ++r)
         for (int i = 0; i < 7; ++i) if (p->ev[r][i]) cudaEventDestroy(p->ev[r][i]);
     delete p;
@@ -304,6 +305,23 @@ int gridder_scatter_atomic(gridder_plan_t *plan, const double *uvw_m, int32_t n_
     if (e != cudaSuccess) return cuda_fail(p, e);
     p->last_stream = s;
     return GRIDDER_OK;
+}
+
+int gridder_image_workspace_size(gridder_plan_t *plan, size_t *bytes) {
+    Plan *p = reinterpret_cast<Plan *>(plan);
+    if (!p || !bytes) return GRIDDER_ERR_INVALID_ARG;
+    return image_workspace(*p, bytes);
+}
+
+int gridder_image(gridder_plan_t *plan, const float *grid, float *image, const float *corr, void *work,
+                  size_t work_bytes, void *cuda_stream) {
+    Plan *p = reinterpret_cast<Plan *>(plan);
+    if (!p || !grid || !image) return GRIDDER_ERR_INVALID_ARG;
+    if (((uintptr_t)grid & 15) || ((uintptr_t)image & 15)) return GRIDDER_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const int rc = launch_image(*p, grid, image, corr, work, work_bytes, s);
+    if (rc == GRIDDER_OK) p->last_stream = s;
+    return rc;
 }
 
 int gridder_run_host(gridder_plan_t *plan, const double *h_uvw_m, int32_t n_time, int32_t n_baseline,

@@ -169,6 +169,10 @@ struct Plan {
     cudaEvent_t ev[kProfRing][7];  // per call: bin: 0 map 1 sort 2 tables 3 | grid: 4 grid 5 flush 6
     int64_t prof_bin_calls, prof_grid_calls;       // since profiling was enabled
     int64_t n_launches;
+    // imager (row f2)
+    bool fft_ready;
+    int fft_handle;
+    size_t fft_work_bytes;
 };
 
 // Stage timers: call j of gridder_bin / gridder_grid records into ring slot j % kProfRing.
@@ -187,6 +191,12 @@ cudaError_t launch_map_debug(const Plan &p, const double *uvw, int n_time, int n
                              int n_chan, int32_t *out, cudaStream_t s);
 cudaError_t sort_temp_bytes(int64_t n, int begin_bit, int end_bit, bool wide, size_t *bytes);
 cudaError_t scan_temp_bytes(int64_t n, size_t *bytes);
+
+// image.cu
+int image_workspace(Plan &p, size_t *bytes);
+void image_destroy(Plan &p);
+int launch_image(Plan &p, const float *grid, float *image, const float *corr, void *work, size_t work_bytes,
+                 cudaStream_t s);
 
 // scatter.cu
 cudaError_t launch_scatter_atomic(Plan &p, const double *uvw, int n_time, int n_bl, const double *freq, int n_chan,

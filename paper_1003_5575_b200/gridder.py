@@ -18,7 +18,8 @@ LIB_PATH = _HERE / "libgridder.so"
 OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_WORKSPACE, ERR_CUDA, ERR_NOT_BINNED, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = ("gridder_workspace_size", "gridder_plan", "gridder_bin", "gridder_grid", "gridder_destroy",
-           "gridder_get_stats", "gridder_map", "gridder_scatter_atomic", "gridder_run_host", "gridder_set_profiling",
+           "gridder_get_stats", "gridder_map", "gridder_scatter_atomic", "gridder_image_workspace_size", "gridder_image",
+           "gridder_run_host", "gridder_set_profiling",
            "gridder_get_stage_ms", "gridder_launch_count", "gridder_strerror",
            "gridder_last_cuda_error", "gridder_version")
 
@@ -64,6 +65,8 @@ def load_library() -> C.CDLL:
                                     C.c_void_p, C.c_void_p]
         lib.gridder_scatter_atomic.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
                                                C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+        lib.gridder_image_workspace_size.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
+        lib.gridder_image.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         lib.gridder_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -239,6 +242,23 @@ class Gridder:
             _dev_ptr(out, torch.float32, "grid"), int(accumulate), _stream_ptr(stream))
         if rc != OK:
             raise GridderError(rc, "gridder_scatter_atomic")
+        return out
+
+    def image(self, grid: torch.Tensor, corr=None, out=None, stream=None) -> torch.Tensor:
+        """centred inverse FFT of the 4 planes with the grid correction fused in (cuFFT inside)."""
+        need = C.c_size_t(0)
+        rc = self._lib.gridder_image_workspace_size(self._plan, C.byref(need))
+        if rc != OK:
+            raise GridderError(rc, "gridder_image_workspace_size")
+        if getattr(self, "_fft_work", None) is None or self._fft_work.numel() < need.value:
+            self._fft_work = torch.empty(max(need.value, 16), dtype=torch.uint8, device=self.device)
+        if out is None:
+            out = torch.empty_like(grid)
+        rc = self._lib.gridder_image(self._plan, _dev_ptr(grid, torch.float32, "grid"), _dev_ptr(out, torch.float32, "image"),
+                                     _dev_ptr(corr, torch.float32, "corr"), self._fft_work.data_ptr(), self._fft_work.numel(),
+                                     _stream_ptr(stream))
+        if rc != OK:
+            raise GridderError(rc, "gridder_image")
         return out
 
     def run_host(self, uvw_m, freq_hz, vis, weight, grid_out, staging: dict, stream=None) -> None:

@@ -172,11 +172,9 @@ def test_p4_three_antennas_fft_image_matches_direct_dft(src):
     vis[:, 0, 0], vis[:, 0, 1] = vis_c.real, vis_c.imag
     g, _, st = _grid(uv, vis, N=N, S=S, O=O, table=table)
     assert st["n_dropped"] == 0
-    img = np.fft.fftshift(np.fft.ifft2(np.fft.ifftshift(g[0]))) * N * N
     lk = (np.arange(N) - N // 2) / N                                 # image pixel centres
-    r = (np.arange(S * O) - (S * O) / 2.0) / O
-    chat = (t1.astype(np.float32).astype(np.float64)[None, :] * np.cos(2 * np.pi * r[None, :] * lk[:, None])).sum(1) / O
-    img_c = img / (chat[None, :] * chat[:, None])
+    # the oracle's imager (row f2) is what is pinned here against the direct DFT
+    img_c = oracle.image(g[0], oracle.grid_correction(t1.astype(np.float32), S, O, N))
     v32 = vis[:, 0, 0].astype(np.float64) + 1j * vis[:, 0, 1].astype(np.float64)
     dft = np.zeros((N, N), complex)
     for (u_, v_), vv in zip(uv, v32):
@@ -188,6 +186,21 @@ def test_p4_three_antennas_fft_image_matches_direct_dft(src):
     if max(abs(round(l0 * N)), abs(round(m0 * N))) < N // 4:
         peak = np.unravel_index(np.abs(img_c[inner, inner]).argmax(), (N // 2 - 1, N // 2 - 1))
         assert (peak[1] + N // 4 + 1 - N // 2, peak[0] + N // 4 + 1 - N // 2) == (round(l0 * N), round(m0 * N))
+
+
+def test_p4b_imager_equals_the_centred_inverse_dft_written_out():
+    """oracle.image against the O(N^4) definition on a random 8 x 8 plane, with a non-trivial correction."""
+    N = 8
+    rng = np.random.default_rng(44)
+    g = rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))
+    corr = rng.uniform(0.5, 2.0, N)
+    k = np.arange(N) - N // 2
+    want = np.zeros((N, N), complex)
+    for y in range(N):
+        for x in range(N):
+            ph = np.exp(2j * np.pi * (k[None, :] * k[x] + k[:, None] * k[y]) / N)       # [v][u]
+            want[y, x] = corr[y] * corr[x] * (g * ph).sum()
+    assert np.abs(oracle.image(g, corr) - want).max() < 1e-12 * np.abs(want).max()
 
 
 # ----------------------------------------------------------------------------------------- P5
