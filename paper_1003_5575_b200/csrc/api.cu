@@ -96,6 +96,12 @@ int derive(const gridder_config *cfg, Plan &p) {
             while ((size_t)p.tmem_cols < cols) p.tmem_cols *= 2;
         }
     }
+    // fast path: bin by channel runs when the key's unsorted bits fit one byte (runs.cu)
+    p.run_cap = 0;
+    if (p.mode == 0 && env_int("GRIDDER_RUNS", 1) && 2 * ceil_log2((unsigned long long)cfg->oversample) + 1 <= 8) {
+        p.run_cap = cfg->max_vis / 4;
+        if (p.run_cap < 1024) p.run_cap = 1024;
+    }
     p.chunk = env_int("GRIDDER_CHUNK", 4096);
     if (p.chunk < 32 || p.chunk > (1 << 20)) return GRIDDER_ERR_INVALID_ARG;
     p.warps_forced = env_int("GRIDDER_WARPS", 0);
@@ -143,6 +149,11 @@ cudaError_t carve(Plan &p, char *base) {
     size_t t1 = 0, t2 = 0;
     cudaError_t e = sort_temp_bytes((int64_t)n, p.key.aux_bits, p.key.total_bits, p.mode != 0, &t1);
     if (e == cudaSuccess) e = scan_temp_bytes((int64_t)n_vtiles + 1, &t2);
+    if (e == cudaSuccess && p.run_cap > 0) {
+        size_t t3 = 0;
+        e = runs_temp_bytes(p.run_cap, p.key.aux_bits, p.key.total_bits, &t3);
+        if (t3 > t1) t1 = t3;
+    }
     if (e == cudaErrorNoDevice || e == cudaErrorInsufficientDriver || e == cudaErrorInvalidDevice) {
         // no GPU on this machine (size query only): CUB cannot be asked, so report a generous bound
         (void)cudaGetLastError();
@@ -154,6 +165,15 @@ cudaError_t carve(Plan &p, char *base) {
     p.cub_temp_bytes = align_up(t1 > t2 ? t1 : t2);
     p.cub_temp = take(p.cub_temp_bytes);
     p.freq_scale = (double *)take(sizeof(double) * kMaxChannels);
+    if (p.run_cap > 0) {
+        const size_t cap = (size_t)p.run_cap;
+        p.qaux = (unsigned char *)take(n);
+        for (int i = 0; i < 2; ++i) p.run_key[i] = (uint32_t *)take(cap * sizeof(uint32_t));
+        for (int i = 0; i < 2; ++i) p.run_val[i] = (unsigned long long *)take(cap * sizeof(unsigned long long));
+        p.run_start = (uint32_t *)take(cap * sizeof(uint32_t));
+        p.run_cum = (uint32_t *)take(cap * sizeof(uint32_t));
+        p.run_blk = (unsigned int *)take(3 * ((n + 1023) / 1024 + 1) * sizeof(unsigned int));
+    }
     p.tile_start = (uint32_t *)take(sizeof(uint32_t) * 2 * n_vtiles);        // [start | end]
     p.tile_chunks = (unsigned long long *)take(sizeof(unsigned long long) * (n_vtiles + 1));
     p.tile_chunks_scan = (unsigned long long *)take(sizeof(unsigned long long) * (n_vtiles + 1));

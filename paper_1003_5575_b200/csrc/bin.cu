@@ -294,30 +294,45 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
         double *scale = p.freq_scale;
         freq_scale_kernel<<<(n_chan + 255) / 256, 256, 0, s>>>(freq, n_chan, scale);
         GR_TRY(cudaGetLastError());
-        const MapParams mp = make_map_params(p);
-        if (p.mode == 0)
-            map_kernel<false><<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp,
-                                                                          p.keys[0], p.vals[0], p.counters);
-        else
-            map_kernel<true><<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp,
-                                                                         p.keys[0], p.vals[0], p.counters);
-        GR_TRY(cudaGetLastError());
-        stage_mark(p, 1, s);
-        cub::DoubleBuffer<uint32_t> k(p.keys[0], p.keys[1]);
-        size_t tb = p.cub_temp_bytes;
-        if (p.mode == 0) {
-            cub::DoubleBuffer<uint32_t> v((uint32_t *)p.vals[0], (uint32_t *)p.vals[1]);
-            GR_TRY(cub::DeviceRadixSort::SortPairs(p.cub_temp, tb, k, v, n, p.key.aux_bits, p.key.total_bits, s));
-        } else {
-            cub::DoubleBuffer<unsigned long long> v((unsigned long long *)p.vals[0], (unsigned long long *)p.vals[1]);
-            GR_TRY(cub::DeviceRadixSort::SortPairs(p.cub_temp, tb, k, v, n, p.key.aux_bits, p.key.total_bits, s));
+        bool by_runs = false;
+        p.n_runs = 0;
+        if (p.run_cap > 0) {
+            GR_TRY(launch_bin_runs(p, uvw, scale, n, n_chan, s, &by_runs));
+            if (by_runs) {
+                stage_mark(p, 2, s);
+            } else {
+                p.n_runs = 0;
+                GR_TRY(cudaMemsetAsync(p.counters, 0, 2 * sizeof(unsigned long long), s));   // counted again below
+            }
         }
-        p.sorted_sel = k.selector;
-        stage_mark(p, 2, s);
-        p.n_launches += 4;
-        tile_bounds_kernel<<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(p.keys[p.sorted_sel], n,
-                                                                        p.key.tile_shift, p.tile_start, tile_end);
-        GR_TRY(cudaGetLastError());
+        if (!by_runs) {
+            const MapParams mp = make_map_params(p);
+            if (p.mode == 0)
+                map_kernel<false><<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp,
+                                                                              p.keys[0], p.vals[0], p.counters);
+            else
+                map_kernel<true><<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp,
+                                                                             p.keys[0], p.vals[0], p.counters);
+            GR_TRY(cudaGetLastError());
+            stage_mark(p, 1, s);
+            cub::DoubleBuffer<uint32_t> k(p.keys[0], p.keys[1]);
+            size_t tb = p.cub_temp_bytes;
+            if (p.mode == 0) {
+                cub::DoubleBuffer<uint32_t> v((uint32_t *)p.vals[0], (uint32_t *)p.vals[1]);
+                GR_TRY(cub::DeviceRadixSort::SortPairs(p.cub_temp, tb, k, v, n, p.key.aux_bits, p.key.total_bits, s));
+            } else {
+                cub::DoubleBuffer<unsigned long long> v((unsigned long long *)p.vals[0], (unsigned long long *)p.vals[1]);
+                GR_TRY(cub::DeviceRadixSort::SortPairs(p.cub_temp, tb, k, v, n, p.key.aux_bits, p.key.total_bits, s));
+            }
+            p.sorted_sel = k.selector;
+            stage_mark(p, 2, s);
+            p.n_launches += 4;
+        }
+        if (!by_runs) {       // (the runs path has built the 'first' / 'last' tables from the runs)
+            tile_bounds_kernel<<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(p.keys[p.sorted_sel], n,
+                                                                            p.key.tile_shift, p.tile_start, tile_end);
+            GR_TRY(cudaGetLastError());
+        }
     } else {
         p.sorted_sel = 0;
         stage_mark(p, 1, s);

@@ -149,6 +149,13 @@ struct Plan {
     void *vals[2];
     void *cub_temp; size_t cub_temp_bytes;
     double *freq_scale;            // [kMaxChannels]: freq / c of the last bin
+    // binning by channel runs (runs.cu); run_cap == 0: not used by this plan
+    int64_t run_cap;               // room for this many runs (more: the bin falls back to per-visibility sorting)
+    unsigned char *qaux;           // [n]: the key's unsorted low bits (sub-cell offsets, drop flag) per visibility
+    uint32_t *run_key[2];          // [run_cap] x 2 (sort double buffer)
+    unsigned long long *run_val[2];// [run_cap] x 2: first index | length << 32
+    uint32_t *run_start, *run_cum; // [run_cap]
+    unsigned int *run_blk;         // [3][ceil(n / 1024) + 1]: runs per map block, their scan, expand partition
     uint32_t *tile_start;          // [2][n_vtiles]: first entry | one past the last entry
     unsigned long long *tile_chunks, *tile_chunks_scan;   // packed (n_full << 32 | has_tail), [n_vtiles+1]
     TileInfo *tile_info;           // [n_vtiles]
@@ -161,6 +168,7 @@ struct Plan {
     // state
     int sorted_sel;                // which of keys[]/vals[] holds the sorted list
     int64_t n_vis;                 // of the last bin
+    int64_t n_runs;                // of the last bin (0: per-visibility path)
     bool binned;
     cudaStream_t last_stream;
     int last_cuda_error;
@@ -190,6 +198,11 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
 cudaError_t launch_map_debug(const Plan &p, const double *uvw, int n_time, int n_bl, const double *freq,
                              int n_chan, int32_t *out, cudaStream_t s);
 cudaError_t sort_temp_bytes(int64_t n, int begin_bit, int end_bit, bool wide, size_t *bytes);
+
+// runs.cu
+cudaError_t runs_temp_bytes(int64_t cap, int begin_bit, int end_bit, size_t *bytes);
+cudaError_t launch_bin_runs(Plan &p, const double *uvw, const double *scale, long long n, int n_chan, cudaStream_t s,
+                            bool *used);
 cudaError_t scan_temp_bytes(int64_t n, size_t *bytes);
 
 // image.cu

@@ -83,4 +83,17 @@ __device__ __forceinline__ VisMap map_vis(double u_m, double v_m, double w_m, do
     return m;
 }
 
+// Fast-path sort key of a mapped visibility (KeyLayout): tile, origin inside the
+// tile, and -- not sorted on -- drop flag and sub-cell offsets.
+__device__ __forceinline__ uint32_t fast_key(const VisMap &m, const MapParams &p) {
+    if (m.dropped)      // filed under tile 0, origin (0, 0)
+        return ((uint32_t)(p.drop_slot * p.n_tiles) << p.key.tile_shift) | (1u << (2 * p.key.bits_q));
+    const uint32_t tmask = (1u << p.key.tlog) - 1u;
+    const uint32_t x0 = (uint32_t)m.x0, y0 = (uint32_t)m.y0;
+    const uint32_t tile = (y0 >> p.key.tlog) * (uint32_t)p.ntx + (x0 >> p.key.tlog);
+    const uint32_t vtile = (uint32_t)(p.cls_slot[m.plane] * p.n_tiles) + tile;
+    return (vtile << p.key.tile_shift) | ((y0 & tmask) << (p.key.aux_bits + p.key.tlog)) |
+           ((x0 & tmask) << p.key.aux_bits) | ((uint32_t)m.qy << p.key.bits_q) | (uint32_t)m.qx;
+}
+
 }  // namespace gridder
