@@ -146,7 +146,12 @@ MapParams make_map_params(const Plan &p) {
     mp.general = p.mode != 0;
     mp.is_complex = p.cfg.kernel_is_complex ? 1 : 0;
     mp.drop_slot = 0;
+    mp.o_shift = -1;
+    for (int b = 0; b < 7; ++b)
+        if ((1 << b) == p.cfg.oversample) mp.o_shift = b;
     mp.cell_size = p.cfg.cell_size;
+    mp.rcp_cell = 1.0 / p.cfg.cell_size;
+    mp.span = (double)p.cfg.grid_size * p.cfg.oversample;
     mp.w_max = p.cfg.w_max;
     mp.key = p.key;
     for (int i = 0; i < p.cfg.n_wplanes; ++i) {

@@ -59,7 +59,10 @@ struct MapParams {
     int32_t general;         // 0: fast path key/value format
     int32_t is_complex;
     int32_t drop_slot;       // class slot dropped visibilities are filed under
+    int32_t o_shift;         // log2 O when O is a power of two, else -1
     double cell_size;        // du
+    double rcp_cell;         // RN(1 / du): screening value only, never decides a rounding (map.cuh)
+    double span;             // N O: scale of the screening margin
     double w_max;
     KeyLayout key;
     int32_t support[kMaxPlanes];

@@ -29,21 +29,41 @@ static __device__ __noinline__ void map_axis_wide(double r, int S, int O, long l
     *q = (int)(d * OO - A);
 }
 
+// Steps 3 of the definition for one axis.  The definition divides by the cell size; a correctly rounded
+// FP64 division is ~4x the cost of everything else here, so the position is first computed with a
+// multiplication by RN(1 / du).  That value differs from the definition's by less than
+// 2^-48 (|h| + N O) (two roundings more, each <= 1 ulp, carried through the same monotone steps), so
+// it rounds to the same sub-cell unless h + 0.5 lies within that distance of an integer: only then
+// (about one visibility in 10^7, and every exact tie) is the division done.  The result is the
+// definition's, bit for bit, by construction -- not "almost always".
 __device__ __forceinline__ AxisMap map_axis(double coord_lambda, const MapParams &p, int S) {
     AxisMap m;
-    const double a = __ddiv_rn(coord_lambda, p.cell_size);
-    const double g = __dadd_rn(a, (double)(p.n_grid / 2));
-    const double h = __dmul_rn(g, (double)p.oversample);
-    const double r = floor(__dadd_rn(h, 0.5));
     const int O = p.oversample;
+    const double half_n = (double)(p.n_grid / 2), dO = (double)O;
+    const double h1 = __dmul_rn(__dadd_rn(__dmul_rn(coord_lambda, p.rcp_cell), half_n), dO);
+    const double t1 = __dadd_rn(h1, 0.5);
+    double r = floor(t1);
+    const double fr = t1 - r;                                  // exact (Sterbenz), in [0, 1)
+    const double eps = __dadd_rn(__dmul_rn(fabs(h1) + p.span, 3.5527136788005009e-15), 1.0e-30);   // 2^-48
+    if (!(fr > eps && fr < 1.0 - eps) || !(fabs(h1) < 1073741824.0)) {
+        const double a = __ddiv_rn(coord_lambda, p.cell_size);
+        const double g = __dadd_rn(a, half_n);
+        const double h = __dmul_rn(g, dO);
+        r = floor(__dadd_rn(h, 0.5));
+    }
     m.far = false;
     if (r > -1073741824.0 && r < 1073741824.0) {
         // |X| < 2^30 sub-cells (N*O <= 2^21 for every accepted plan): 32-bit integer algebra
         const int X = (int)r;
-        const int A = X - (S * O) / 2;
+        const int A = X - ((S * O) >> 1);
         const int n = A + O - 1;              // x0 = ceil(A / O) = floor((A + O - 1) / O)
-        int x0 = n / O;
-        if ((n % O != 0) && (n < 0)) x0 -= 1;
+        int x0;
+        if (p.o_shift >= 0) {                 // O a power of two: floor division is an arithmetic shift
+            x0 = n >> p.o_shift;
+        } else {
+            x0 = n / O;
+            if ((n % O != 0) && (n < 0)) x0 -= 1;
+        }
         m.x0 = x0;
         m.q = x0 * O - A;
     } else if (r > -1.0e15 && r < 1.0e15) {

@@ -53,13 +53,17 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
     unsigned char q[kRunItems];
     unsigned int dropped_here = 0;
     unsigned long long taps_here = 0;
+    // (integration, baseline) row and channel of the thread's first visibility; the next ones by increment
+    unsigned int tb = 0, f = 0;
+    if (base < n) {
+        tb = (unsigned int)base / n_chan;
+        f = (unsigned int)base - tb * n_chan;
+    }
 #pragma unroll
     for (int k = 0; k < kRunItems; ++k) {
         const unsigned long long ii = base + k;
         sk[k] = 0xFFFFFFFFu; fch[k] = 1; q[k] = 0;
         if (ii < n) {
-            const unsigned int i = (unsigned int)ii;
-            const unsigned int tb = i / n_chan, f = i - tb * n_chan;
             const double *L = uvw + (size_t)tb * 3;
             const VisMap m = map_vis(L[0], L[1], 0.0, scale[f], p);
             const uint32_t key = fast_key(m, p);
@@ -67,6 +71,7 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
             sk[k] = key >> p.key.aux_bits;
             q[k] = (unsigned char)(key & aux_mask);
             fch[k] = f;
+            if (++f == n_chan) { f = 0; ++tb; }
         }
     }
     if (base + kRunItems <= n) {
