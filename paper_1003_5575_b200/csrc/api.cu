@@ -31,7 +31,7 @@ int derive(const gridder_config *cfg, Plan &p) {
     if (!(cfg->cell_size > 0.0) || cfg->n_pol != 4) return GRIDDER_ERR_INVALID_ARG;
     if (cfg->oversample < 1 || cfg->oversample > 64) return GRIDDER_ERR_INVALID_ARG;
     if (cfg->n_wplanes < 1 || cfg->n_wplanes > kMaxPlanes || !cfg->support) return GRIDDER_ERR_INVALID_ARG;
-    if (cfg->max_vis < 0 || cfg->max_vis > 0xFFFFFFF0ll) return GRIDDER_ERR_INVALID_ARG;
+    if (cfg->max_vis < 0 || cfg->max_vis > 0xFFFFF000ll) return GRIDDER_ERR_INVALID_ARG;
     for (int i = 0; i < cfg->n_wplanes; ++i) {
         const int s = cfg->support[i];
         if (s < 1 || s > 32 || ((s * cfg->oversample) & 1)) return GRIDDER_ERR_INVALID_ARG;
@@ -317,7 +317,7 @@ int gridder_scatter_atomic(gridder_plan_t *plan, const double *uvw_m, int32_t n_
     if (!p || !grid || n_time < 0 || n_baseline < 0 || n_chan < 0) return GRIDDER_ERR_INVALID_ARG;
     const int64_t n = (int64_t)n_time * n_baseline * n_chan;
     if (n > 0 && (!uvw_m || !freq_hz || !vis)) return GRIDDER_ERR_INVALID_ARG;
-    if (n > 0xFFFFFFF0ll) return GRIDDER_ERR_CAPACITY;
+    if (n > 0xFFFFF000ll) return GRIDDER_ERR_CAPACITY;
     if (((uintptr_t)vis & 15) || ((uintptr_t)grid & 7)) return GRIDDER_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     cudaError_t e = launch_scatter_atomic(*p, uvw_m, n_time, n_baseline, freq_hz, n_chan, vis, weight, grid,

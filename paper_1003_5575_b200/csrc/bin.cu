@@ -126,11 +126,8 @@ __global__ void __launch_bounds__(256) map_debug_kernel(const double *__restrict
         const int f = (int)(i - tb * n_chan);
         const double s = __ddiv_rn(freq[f], kSpeedOfLight);
         const VisMap m = map_vis(uvw[tb * 3 + 0], uvw[tb * 3 + 1], uvw[tb * 3 + 2], s, p);
-        const long long lim = 1ll << 30;
-        const long long cx = m.x0 < -lim ? -lim : (m.x0 > lim ? lim : m.x0);
-        const long long cy = m.y0 < -lim ? -lim : (m.y0 > lim ? lim : m.y0);
         int32_t *o = out + i * 6;
-        o[0] = (int32_t)cx; o[1] = (int32_t)cy; o[2] = m.qx; o[3] = m.qy;
+        o[0] = m.x0; o[1] = m.y0; o[2] = m.qx; o[3] = m.qy;      // origins are clamped to +-2^30 by the map
         o[4] = m.plane | (m.conj << 8); o[5] = m.dropped ? 1 : 0;
     }
 }

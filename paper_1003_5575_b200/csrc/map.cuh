@@ -12,12 +12,12 @@ namespace gridder {
 // tolerance.
 // ------------------------------------------------------------------------------------------
 struct AxisMap {
-    long long x0;   // patch origin
+    int x0;         // patch origin (clamped to +-2^30 for positions far outside any grid)
     int q;          // sub-cell table offset in [0, O)
     bool far;       // hopelessly off the grid
 };
 
-static __device__ __noinline__ void map_axis_wide(double r, int S, int O, long long *x0, int *q) {
+static __device__ __noinline__ void map_axis_wide(double r, int S, int O, int *x0, int *q) {
     // the same algebra in 64 bits, for positions far outside any grid (always dropped, but the
     // test interface reports them)
     const long long X = (long long)r, OO = O;
@@ -25,7 +25,8 @@ static __device__ __noinline__ void map_axis_wide(double r, int S, int O, long l
     const long long n = A + OO - 1;
     long long d = n / OO;
     if ((n % OO != 0) && (n < 0)) d -= 1;
-    *x0 = d;
+    const long long lim = 1ll << 30;
+    *x0 = (int)(d < -lim ? -lim : (d > lim ? lim : d));
     *q = (int)(d * OO - A);
 }
 
@@ -70,14 +71,14 @@ __device__ __forceinline__ AxisMap map_axis(double coord_lambda, const MapParams
         map_axis_wide(r, S, O, &m.x0, &m.q);
     } else {
         m.far = true;
-        m.x0 = -(1ll << 61);
+        m.x0 = -(1 << 30);
         m.q = 0;
     }
     return m;
 }
 
 struct VisMap {
-    long long x0, y0;
+    int x0, y0;     // patch origin, 32-bit (a visibility beyond +-2^30 cells is dropped either way)
     int qx, qy, plane, conj, S;
     bool dropped;
 };
@@ -98,7 +99,7 @@ __device__ __forceinline__ VisMap map_vis(double u_m, double v_m, double w_m, do
     m.S = p.support[m.plane];
     const AxisMap mx = map_axis(ul, p, m.S), my = map_axis(vl, p, m.S);
     m.x0 = mx.x0; m.y0 = my.x0; m.qx = mx.q; m.qy = my.q;
-    const long long N = p.n_grid, S = m.S;
+    const int N = p.n_grid, S = m.S;
     m.dropped = mx.far || my.far || m.x0 < 0 || m.x0 + S > N || m.y0 < 0 || m.y0 + S > N;
     return m;
 }

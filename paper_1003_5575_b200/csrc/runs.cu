@@ -36,14 +36,14 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
     __shared__ unsigned int s_warp[kRunThreads / 32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned int bid = blockIdx.x;
-    const unsigned long long base = (unsigned long long)bid * kRunTile + (unsigned long long)tid * kRunItems;
+    const unsigned int base = bid * (unsigned)kRunTile + (unsigned)tid * kRunItems;    // n <= 2^32 - 4096: no wrap
     const uint32_t aux_mask = (1u << p.key.aux_bits) - 1u;
 
     // thread 0 also maps the visibility just before the block's first one (its key decides whether the
     // block starts inside a run); done before the barrier so that it costs no extra phase
     uint32_t prev = 0xFFFFFFFFu;
     if (tid == 0 && base > 0 && base < n) {
-        const unsigned int i = (unsigned int)(base - 1);
+        const unsigned int i = base - 1;
         const unsigned int tb = i / n_chan, f = i - tb * n_chan;
         const double *L = uvw + (size_t)tb * 3;
         prev = fast_key(map_vis(L[0], L[1], 0.0, scale[f], p), p) >> p.key.aux_bits;
@@ -56,14 +56,13 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
     // (integration, baseline) row and channel of the thread's first visibility; the next ones by increment
     unsigned int tb = 0, f = 0;
     if (base < n) {
-        tb = (unsigned int)base / n_chan;
-        f = (unsigned int)base - tb * n_chan;
+        tb = base / n_chan;
+        f = base - tb * n_chan;
     }
 #pragma unroll
     for (int k = 0; k < kRunItems; ++k) {
-        const unsigned long long ii = base + k;
         sk[k] = 0xFFFFFFFFu; fch[k] = 1; q[k] = 0;
-        if (ii < n) {
+        if (base + k < n) {
             const double *L = uvw + (size_t)tb * 3;
             const VisMap m = map_vis(L[0], L[1], 0.0, scale[f], p);
             const uint32_t key = fast_key(m, p);
@@ -114,7 +113,7 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
     for (int k = 0; k < kRunItems; ++k)
         if (flags & (1u << k)) {
             stage_key[pos] = sk[k] << p.key.aux_bits;
-            stage_start[pos] = (unsigned int)(base + k);
+            stage_start[pos] = base + k;
             ++pos;
         }
     for (int o = 16; o > 0; o >>= 1) {
