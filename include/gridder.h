@@ -25,7 +25,10 @@
  *   - Pointers are DEVICE pointers unless marked HOST.  The library allocates no device memory:
  *     the caller owns every buffer, including the workspace.
  *   - Calls only enqueue work on `cuda_stream` (a cudaStream_t passed as void*; NULL = default
- *     stream).  gridder_plan, gridder_destroy, gridder_get_stats and gridder_run_host synchronise.
+ *     stream).  gridder_plan, gridder_destroy, gridder_get_stats and gridder_run_host synchronise;
+ *     gridder_bin synchronises the stream ONCE in the middle when it bins by channel runs (plans
+ *     with one real table, S <= 16, O <= 8): the number of runs sizes the sort.  What it enqueues
+ *     after that is asynchronous again.
  *   - Buffers given to gridder_bin / gridder_grid must stay valid until that work has completed.
  *   - A plan may be binned and gridded any number of times; one gridder_bin serves any number of
  *     gridder_grid calls (same uv geometry, new visibilities).  Not thread-safe per plan.
@@ -86,7 +89,7 @@ typedef struct {
 typedef struct {
     int64_t n_vis;              /* visibilities given to the last gridder_bin                        */
     int64_t n_dropped;          /* of those, dropped because the patch leaves the grid               */
-    int64_t n_entries;          /* sort entries (= gridded visibilities x sub-patches)               */
+    int64_t n_entries;          /* gridded (not dropped) visibilities                                */
     int64_t vis_taps;           /* sum of S_p^2 over gridded visibilities (the metric's numerator)   */
     int64_t n_tiles;            /* uv tiles of the plan                                              */
     int64_t n_tiles_occupied;
@@ -106,7 +109,8 @@ GRIDDER_API int gridder_workspace_size(const gridder_config *cfg, size_t *bytes_
 GRIDDER_API int gridder_plan(const gridder_config *cfg, gridder_plan_t **plan_out, size_t *workspace_needed);
 
 /* Map + sort + tile tables for n_time*n_baseline*n_chan visibilities (index (t*B + b)*F + f).
- * u_lambda = u_m * (f / c), c = 299792458 m/s.  Asynchronous on `cuda_stream`. */
+ * u_lambda = u_m * (f / c), c = 299792458 m/s.  n_chan <= 65536.  Enqueued on `cuda_stream` (one
+ * internal synchronisation, see above). */
 GRIDDER_API int gridder_bin(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
                 const double *freq_hz, int32_t n_chan, void *cuda_stream);
 
