@@ -253,3 +253,33 @@ def test_error_paths_on_device(dev):
         gridder.Gridder(grid_size=32768, cell_size=1.0, oversample=4, support=[16], kernel=torch.zeros(64 * 64, device=dev),
                         max_vis=100)
     assert e.value.code == gridder.ERR_UNSUPPORTED
+
+
+# ------------------------------------------------------------------------------------ binning by channel runs
+def test_run_binning_gives_the_same_bits_as_the_per_visibility_sort(dev):
+    """The fast path sorts channel runs and expands them (csrc/runs.cu); the result must be the list the
+    per-visibility sort produces, hence the same grid to the last bit -- on a multi-channel workload
+    whose size is not a multiple of the 1024-visibility blocks and whose runs straddle them."""
+    rng = np.random.default_rng(21)
+    N, S, O, nb, nf = 256, 16, 4, 517, 100
+    table = synth.spheroidal_table(S, O)
+    uvw = np.zeros((2, nb, 3))
+    uvw[:, :, :2] = rng.uniform(-112.0, 112.0, (2, nb, 2))
+    uvw[0, :5, :2] = 0.0                                            # one run per row, same origin for all
+    freq = C * (1.0 + 2.0e-3 * np.arange(nf))                       # 20 % band: long and short runs
+    vis = rng.standard_normal((2, nb, nf, 4, 2)).astype(np.float32)
+    w = rng.uniform(0.5, 1.5, (2, nb, nf)).astype(np.float32)
+    kw = dict(N=N, du=1.0, O=O, S=S, table=table)
+    a, st_a = _run(dev, uvw, freq, vis, w, **kw)
+    b, st_b = _run(dev, uvw, freq, vis, w, env={"GRIDDER_RUNS": 0}, **kw)
+    assert np.array_equal(a, b)
+    assert (st_a.n_dropped, st_a.vis_taps, st_a.n_work_items, st_a.max_tile_load) == \
+           (st_b.n_dropped, st_b.vis_taps, st_b.n_work_items, st_b.max_tile_load)
+    assert 0 < st_a.n_dropped < 2 * nb * nf                         # the 1.2x band pushes some off the grid
+    ref, ab, ost = _oracle(uvw, freq, vis, w, **kw)
+    assert ost["n_dropped"] == st_a.n_dropped
+    assert_parity(a, ref, ab, "run binning")
+    # single-channel input: every visibility is its own run -> the plan falls back to the per-visibility sort
+    c, _ = _run(dev, uvw[:, :, :], freq[:1], vis[:, :, :1].copy(), w[:, :, :1].copy(), **kw)
+    d, _ = _run(dev, uvw[:, :, :], freq[:1], vis[:, :, :1].copy(), w[:, :, :1].copy(), env={"GRIDDER_RUNS": 0}, **kw)
+    assert np.array_equal(c, d)
