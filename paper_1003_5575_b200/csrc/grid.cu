@@ -41,7 +41,7 @@ struct Geo {
     static constexpr int T = 1 << TLOG;
     static constexpr int RW = T + SPX * NSUB - 1, RH = T + SPY * NSUB - 1;   // region = tile + halo
     static constexpr int CELLS = RW * RH;
-    static constexpr int VF4 = CPLX ? 4 : 2;                   // float4 per staged visibility
+    static constexpr int VF4 = 2;                              // float4 per staged visibility
     static constexpr int SLOT_F4 = VF4 + 1;                    // + (table offset of the NEXT record, origin)
     static constexpr int SLOTS = 36;                           // 32 records + sentinel + pad + look-ahead
     static constexpr int RING_F4 = 2 * SLOTS * SLOT_F4;        // two halves
@@ -187,12 +187,11 @@ __device__ __forceinline__ void stage_write(const GridParams &p, const float4 *r
     const uint32_t tmask = (1u << TLOG) - 1u;
     uint32_t x0l, y0l;
     int coff;
-    float sg = 1.0f;
     if (G::GEN) {
         x0l = k.key & tmask;
         y0l = (k.key >> TLOG) & tmask;
         coff = (int)((k.aux & 0x3fffffffu) << 8);          // table offset in 256-byte units
-        if (k.aux >> 31) sg = -1.0f;
+        if (G::CPLX) coff |= (int)(k.aux >> 31);           // bit 0: use the conjugate table (w < 0)
     } else {
         const uint32_t qmask = (1u << (2 * p.key.bits_q)) - 1u;
         x0l = (k.key >> p.key.aux_bits) & tmask;
@@ -209,10 +208,6 @@ __device__ __forceinline__ void stage_write(const GridParams &p, const float4 *r
     float4 *slot = half + lane * G::SLOT_F4;
     slot[0] = a;
     slot[1] = b;
-    if (G::CPLX) {      // (-s im, s re) pairs: the complex product then needs no sign handling
-        slot[2] = make_float4(-sg * a.y, sg * a.x, -sg * a.w, sg * a.z);
-        slot[3] = make_float4(-sg * b.y, sg * b.x, -sg * b.w, sg * b.z);
-    }
     // slot r carries the table offset of record r + 1 (the consumer loads taps one record ahead)
     // and the origin of record r; slot 0 also carries its own table offset
     const int my_coff = pad ? 0 : coff;
@@ -232,15 +227,20 @@ __device__ __forceinline__ void stage_write(const GridParams &p, const float4 *r
 template <int NA, int NB, int MODE>
 struct RecRegs {
     static constexpr bool CPLX = MODE == 2;
-    static constexpr int VF4 = CPLX ? 4 : 2;
+    static constexpr int VF4 = 2;
     static constexpr int CF = NB * (CPLX ? 2 : 1);            // floats per column block
     float4 v[VF4];
+    uint32_t sgn;                                             // MODE 2: sign bit of s (s = -1: conjugate table)
     float c[NA][CF];
     // MODE 0: `coef_lane` is the shared-space address of this lane's taps of sub-table 0 (the table
     // sits at the start of dynamic shared memory), else a global pointer.
-    __device__ __forceinline__ void fetch(const float4 *slot, const int coff, const char *coef_lane) {
+    __device__ __forceinline__ void fetch(const float4 *slot, int coff, const char *coef_lane) {
 #pragma unroll
         for (int i = 0; i < VF4; ++i) v[i] = slot[i];
+        if (MODE == 2) {
+            sgn = (uint32_t)coff << 31;
+            coff &= ~1;
+        }
         if (MODE == 3) {                                       // tensor memory: one load for all NA*NB taps
             const uint32_t ta = (uint32_t)(uintptr_t)coef_lane + (uint32_t)coff;
             if (NA * NB == 8) {
@@ -335,19 +335,28 @@ __device__ __forceinline__ void consume(const RecRegs<NA, NB, MODE> &R, const in
     // Packed FP32 pairs (Blackwell fma.rn.f32x2 -> FFMA2 with the tap as a scalar broadcast operand): one
     // instruction updates (re, im) of one polarisation of one cell, halving the issue slots of the loop.
     if (MODE == 2) {
+        // (re, im) += cr (v.re, v.im) + ci (-s v.im, s v.re), s = -1 for the conjugate table: the second
+        // pair is made here with sign-bit XORs (ALU pipe, idle in this loop) instead of being staged,
+        // which keeps the shared-memory traffic of a complex entry at that of a real one
+        const uint32_t sq = R.sgn, sp = R.sgn ^ 0x80000000u;
+        const float4 va = R.v[0], vb = R.v[1];
+        const float p0 = __uint_as_float(__float_as_uint(va.y) ^ sp), q0 = __uint_as_float(__float_as_uint(va.x) ^ sq);
+        const float p1 = __uint_as_float(__float_as_uint(va.w) ^ sp), q1 = __uint_as_float(__float_as_uint(va.z) ^ sq);
+        const float p2 = __uint_as_float(__float_as_uint(vb.y) ^ sp), q2 = __uint_as_float(__float_as_uint(vb.x) ^ sq);
+        const float p3 = __uint_as_float(__float_as_uint(vb.w) ^ sp), q3 = __uint_as_float(__float_as_uint(vb.z) ^ sq);
 #pragma unroll
         for (int a = 0; a < NA; ++a)
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
                 const float cr = R.c[a][2 * b], ci = R.c[a][2 * b + 1];
-                ffma2(acc[a][b][0], acc[a][b][1], cr, R.v[0].x, R.v[0].y);
-                ffma2(acc[a][b][2], acc[a][b][3], cr, R.v[0].z, R.v[0].w);
-                ffma2(acc[a][b][4], acc[a][b][5], cr, R.v[1].x, R.v[1].y);
-                ffma2(acc[a][b][6], acc[a][b][7], cr, R.v[1].z, R.v[1].w);
-                ffma2(acc[a][b][0], acc[a][b][1], ci, R.v[2].x, R.v[2].y);
-                ffma2(acc[a][b][2], acc[a][b][3], ci, R.v[2].z, R.v[2].w);
-                ffma2(acc[a][b][4], acc[a][b][5], ci, R.v[3].x, R.v[3].y);
-                ffma2(acc[a][b][6], acc[a][b][7], ci, R.v[3].z, R.v[3].w);
+                ffma2(acc[a][b][0], acc[a][b][1], cr, va.x, va.y);
+                ffma2(acc[a][b][2], acc[a][b][3], cr, va.z, va.w);
+                ffma2(acc[a][b][4], acc[a][b][5], cr, vb.x, vb.y);
+                ffma2(acc[a][b][6], acc[a][b][7], cr, vb.z, vb.w);
+                ffma2(acc[a][b][0], acc[a][b][1], ci, p0, q0);
+                ffma2(acc[a][b][2], acc[a][b][3], ci, p1, q1);
+                ffma2(acc[a][b][4], acc[a][b][5], ci, p2, q2);
+                ffma2(acc[a][b][6], acc[a][b][7], ci, p3, q3);
             }
     } else {
 #pragma unroll
@@ -580,7 +589,8 @@ __global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
 // mode follow from the plan; TLOG is a plan parameter; the block size is chosen at run time.
 // ------------------------------------------------------------------------------------------
 size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps) {
-    const int vf4 = mode == 2 ? 4 : 2;
+    const int vf4 = 2;
+    (void)mode;
     const size_t per_warp = (size_t)(2 * g.RW * g.RH + 2 * 36 * (vf4 + 1) + 32 * 2 + 8) * sizeof(float4);   // Geo::WARP_F4
     (void)tlog;
     return (mode == 0 ? table_bytes : 0) + per_warp * warps;
