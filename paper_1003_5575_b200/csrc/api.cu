@@ -68,9 +68,9 @@ int derive(const gridder_config *cfg, Plan &p) {
         g.NB = c == 0 ? 2 : 4;
         g.nsub = c == 2 ? 2 : 1;
         g.SP = 8 * g.NA * g.nsub;
-        g.RW = g.RH = p.T + g.SP - 1;
+        g.RW = g.RH = p.T + 8 * g.NA - 1;            // region of ONE register patch (tile + halo)
         g.sub_bytes = g.NA * g.NB * 32 * (cplx ? 8 : 4);
-        g.region_f4 = 2 * g.RW * g.RH;
+        g.region_f4 = g.nsub * g.nsub * 2 * g.RW * g.RH;     // nsub^2 virtual items per work item
         slot_of_class[c] = p.n_cls;
         p.cls[p.n_cls++] = g;
     }
@@ -105,7 +105,7 @@ int derive(const gridder_config *cfg, Plan &p) {
     p.chunk = env_int("GRIDDER_CHUNK", 4096);
     if (p.chunk < 32 || p.chunk > (1 << 20)) return GRIDDER_ERR_INVALID_ARG;
     p.warps_forced = env_int("GRIDDER_WARPS", 0);
-    p.fold_batches = env_int("GRIDDER_FOLD_BATCHES", 4);
+    p.fold_batches = env_int("GRIDDER_FOLD_BATCHES", 8);
     if (p.fold_batches < 1 || p.fold_batches > 64 || (p.fold_batches & (p.fold_batches - 1))) return GRIDDER_ERR_INVALID_ARG;
 
     KeyLayout k;

@@ -28,7 +28,9 @@ namespace gridder {
 // MODE 3: as MODE 0, but the table lives in TENSOR MEMORY: lane l of every warp reads its NA*NB taps of
 //         sub-table q with one tcgen05.ld (32 lanes x 32 bit x NA*NB columns at column q*NA*NB), which
 //         takes the taps off the shared-memory return path -- the path this kernel is bound by.
-// NSUB > 1: an entry covers NSUB x NSUB register patches (supports 17..32), gridded one after the other.
+// NSUB == 2: an entry covers 2 x 2 register patches (supports 17..32).  Sub-patch (sy, sx) of a work item is
+//         gridded as a VIRTUAL work item of its own (same entries, its quarter of the table, its own
+//         tile + halo region, anchored 16 (sx, sy) cells up the grid), so the region stays 19 x 19.
 constexpr int kSentinel = -(1 << 20);   // origin of the record that ends a work item
 constexpr int kForce = INT_MIN;         // never an origin: forces a fold at the next record
 
@@ -39,7 +41,8 @@ struct Geo {
     static constexpr bool TMEM = MODE == 3;
     static constexpr int SPX = 8 * NA, SPY = 4 * NB;           // register patch
     static constexpr int T = 1 << TLOG;
-    static constexpr int RW = T + SPX * NSUB - 1, RH = T + SPY * NSUB - 1;   // region = tile + halo
+    static constexpr int RW = T + SPX - 1, RH = T + SPY - 1;   // region = tile + halo of ONE register patch
+    static constexpr int VSHIFT = NSUB > 1 ? 2 : 0;            // log2 of the virtual items per work item
     static constexpr int CELLS = RW * RH;
     static constexpr int VF4 = 2;                              // float4 per staged visibility
     static constexpr int SLOT_F4 = VF4 + 1;                    // + (table offset of the NEXT record, origin)
@@ -90,25 +93,29 @@ struct Producer {
     int grp_cnt, nxt_cnt, grp_pos;
     unsigned it_start, it_len, it_off, it_id;
     unsigned item_begin, item_end;       // this launch's (patch class's) range of the work-item table
+    unsigned v_end;                      // virtual items of the launch (work items << vshift)
+    int vshift;
     bool ended;
 
     __device__ __forceinline__ void claim(const GridParams &p, int lane) {
         unsigned b = 0;
         if (lane == 0) b = atomicAdd(&p.counters->queue_head[p.cls], (unsigned)kClaim);
         b = __shfl_sync(0xffffffffu, b, 0);
-        nxt_base = item_begin + b;
-        nxt_cnt = nxt_base < item_end ? (int)min((unsigned)kClaim, item_end - nxt_base) : 0;
+        nxt_base = b;                    // virtual item ids, relative to the class
+        nxt_cnt = nxt_base < v_end ? (int)min((unsigned)kClaim, v_end - nxt_base) : 0;
         WorkItem w;
         w.start = w.len = w.tile = w.pad = 0;
-        if (lane < nxt_cnt) w = p.items[nxt_base + lane];
+        if (lane < nxt_cnt) w = p.items[item_begin + ((nxt_base + lane) >> vshift)];
         nxt = w;
     }
 
-    __device__ __forceinline__ void init(const GridParams &p, int lane) {
+    __device__ __forceinline__ void init(const GridParams &p, int lane, int vshift_) {
         ended = false;
         it_len = it_off = it_start = it_id = 0;
         item_begin = p.counters->cls_begin[p.cls];
         item_end = p.counters->cls_end[p.cls];
+        vshift = vshift_;
+        v_end = (item_end - item_begin) << vshift;
         claim(p, lane);
         grp = nxt; grp_base = nxt_base; grp_cnt = nxt_cnt; grp_pos = 0;
         if (grp_cnt > 0) claim(p, lane); else ended = true;
@@ -444,7 +451,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
             for (int k = 0; k < 8; ++k) acc[a][b][k] = 0.f;
 
     Producer prod;
-    prod.init(p, lane);
+    prod.init(p, lane, G::VSHIFT);
     Desc dC, dL, dK;                     // being consumed | landing in the raw buffer | keys in flight
     dC.bits = 0; dC.item = 0;
     dL = dC;
@@ -476,12 +483,10 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
         if (cnt > 0) {
             const int cntp = dC.last() ? ((cnt + 2) & ~1) : cnt;        // + sentinel, even
             const float4 *send = half + cntp * G::SLOT_F4;
-#pragma unroll 1
-            for (int sub = 0; sub < NSUB * NSUB; ++sub) {
-                // sub-patch (sy, sx): its origin in the region and its part of the table
-                const int sub_poff = NSUB > 1 ? (sub / NSUB) * (G::SPY * G::RW) + (sub % NSUB) * G::SPX : 0;
-                const char *cl = NSUB > 1 ? coef_lane + sub * p.sub_stride_bytes : coef_lane;
-                if (NSUB > 1) cmp = kForce;
+            {
+                // NSUB == 2: the virtual item's sub-patch selects its quarter of the table
+                constexpr int sub_poff = 0;
+                const char *cl = NSUB > 1 ? coef_lane + (int)(dC.item & 3u) * p.sub_stride_bytes : coef_lane;
                 RecRegs<NA, NB, MODE> A, B;
                 const float4 *sp = half;
                 // meta of a slot: x = table offset of the next record, y = origin of this one
@@ -509,7 +514,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
                 cur = -1;
                 cmp = kSentinel;
                 __syncwarp();
-                float4 *dst = p.partials + (size_t)(dC.item - prod.item_begin) * (2 * G::CELLS);
+                float4 *dst = p.partials + (size_t)dC.item * (2 * G::CELLS);      // (virtual) item id inside the class
                 for (int i = lane; i < 2 * G::CELLS; i += 32) {
                     stg_stream(dst + i, region[i]);
                     region[i] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -541,7 +546,9 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
 template <int SP, int TLOG>
 struct FlushGeo {
     static constexpr int T = 1 << TLOG;
-    static constexpr int RW = T + SP - 1, RH = T + SP - 1, CELLS = RW * RH;
+    static constexpr int NSUB = SP > 16 ? 2 : 1;               // 32-cell class: 2 x 2 virtual items per work item
+    static constexpr int PATCH = SP / NSUB;
+    static constexpr int RW = T + PATCH - 1, RH = T + PATCH - 1, CELLS = RW * RH;
 };
 
 template <int SP, int TLOG>
@@ -554,22 +561,30 @@ __global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
 #pragma unroll
     for (int k = 0; k < 8; ++k) acc[k] = 0.0;
     const uint32_t first_item = p.counters->cls_begin[p.cls];
-    const int tx_hi = min(x >> TLOG, p.ntx - 1), ty_hi = min(y >> TLOG, p.nty - 1);
-    const int tx_lo = max(0, (x - G::RW + G::T) >> TLOG), ty_lo = max(0, (y - G::RH + G::T) >> TLOG);
-    for (int ty = ty_lo; ty <= ty_hi; ++ty)
-        for (int tx = tx_lo; tx <= tx_hi; ++tx) {
-            const TileInfo ti = p.tiles[ty * p.ntx + tx];
-            if (ti.count == 0) continue;
-            const int cell = (y - (ty << TLOG)) * G::RW + (x - (tx << TLOG));
-            const uint32_t n_it = ti.n_full + (ti.tail_item != 0xFFFFFFFFu ? 1u : 0u);
-            for (uint32_t c = 0; c < n_it; ++c) {
-                const uint32_t item = c < ti.n_full ? ti.full_base + c : ti.tail_item;
-                const float4 *part = p.partials + (size_t)(item - first_item) * (2 * G::CELLS);
-                const float4 a = __ldcs(part + cell), b = __ldcs(part + G::CELLS + cell);
-                acc[0] += (double)a.x; acc[1] += (double)a.y; acc[2] += (double)a.z; acc[3] += (double)a.w;
-                acc[4] += (double)b.x; acc[5] += (double)b.y; acc[6] += (double)b.z; acc[7] += (double)b.w;
+#pragma unroll 1
+    for (int sub = 0; sub < G::NSUB * G::NSUB; ++sub) {
+        // sub-patch (sy, sx) regions are anchored PATCH (sx, sy) cells above their tile
+        const int xs = x - (sub % G::NSUB) * G::PATCH, ys = y - (sub / G::NSUB) * G::PATCH;
+        if (xs < 0 || ys < 0) continue;
+        const int tx_hi = min(xs >> TLOG, p.ntx - 1), ty_hi = min(ys >> TLOG, p.nty - 1);
+        const int tx_lo = max(0, (xs - G::RW + G::T) >> TLOG), ty_lo = max(0, (ys - G::RH + G::T) >> TLOG);
+        for (int ty = ty_lo; ty <= ty_hi; ++ty)
+            for (int tx = tx_lo; tx <= tx_hi; ++tx) {
+                const TileInfo ti = p.tiles[ty * p.ntx + tx];
+                if (ti.count == 0) continue;
+                const int cell = (ys - (ty << TLOG)) * G::RW + (xs - (tx << TLOG));
+                if (xs - (tx << TLOG) >= G::RW || ys - (ty << TLOG) >= G::RH) continue;
+                const uint32_t n_it = ti.n_full + (ti.tail_item != 0xFFFFFFFFu ? 1u : 0u);
+                for (uint32_t c = 0; c < n_it; ++c) {
+                    const uint32_t item = c < ti.n_full ? ti.full_base + c : ti.tail_item;
+                    const size_t vitem = (size_t)(item - first_item) * (G::NSUB * G::NSUB) + sub;
+                    const float4 *part = p.partials + vitem * (2 * G::CELLS);
+                    const float4 a = __ldcs(part + cell), b = __ldcs(part + G::CELLS + cell);
+                    acc[0] += (double)a.x; acc[1] += (double)a.y; acc[2] += (double)a.z; acc[3] += (double)a.w;
+                    acc[4] += (double)b.x; acc[5] += (double)b.y; acc[6] += (double)b.z; acc[7] += (double)b.w;
+                }
             }
-        }
+    }
     const size_t nn = (size_t)p.n_grid * p.n_grid;
     const size_t c0 = (size_t)y * p.n_grid + x;
 #pragma unroll
