@@ -325,7 +325,7 @@ def run_ours(args) -> dict | None:
         staging = {"uvw": d_uvw, "freq": d_freq, "vis": vis, "weight": weight, "grid": grid}
         e_steps = max(1, min(args.steps, 3))
         g.run_host(h_uvw, h_freq, h_vis, h_w, h_grid, staging)            # warm-up
-        taps_e = g.stats().vis_taps
+        taps_e = st.vis_taps * nt_e // nt        # (run_host grids in slices; the plan's stats are the last slice's)
         barrier()
         e0.record()
         for _ in range(e_steps):

@@ -153,9 +153,13 @@ GRIDDER_API int gridder_image_workspace_size(gridder_plan_t *plan, size_t *bytes
 GRIDDER_API int gridder_image(gridder_plan_t *plan, const float *grid, float *image, const float *corr, void *work,
                               size_t work_bytes, void *cuda_stream);
 
-/* End-to-end convenience with HOST buffers (pinned or pageable): copies uvw, freq, vis, weight to
- * the caller's device staging buffers, runs gridder_bin + gridder_grid and copies the grid back,
- * all on `cuda_stream`, then synchronises it.  d_* are DEVICE buffers at least as large as their
+/* End-to-end convenience with HOST buffers (pinned for overlap; pageable works): copies uvw, freq,
+ * vis, weight to the caller's device staging buffers, runs gridder_bin + gridder_grid and copies the
+ * grid back, then synchronises `cuda_stream`.  Inputs of 256 MB and more are moved and gridded in 8
+ * slices of the (integration, baseline) axis: the copy of slice k+1 (on an internal second stream)
+ * overlaps the binning and gridding of slice k, whose result is added to the grid.  The sum is the same
+ * grid up to one more FP32 rounding per slice; it is deterministic, but not bit-identical to a single
+ * gridder_bin + gridder_grid over the whole input.  Afterwards the plan is binned for the last slice only.  d_* are DEVICE buffers at least as large as their
  * host counterparts (d_weight may be NULL iff h_weight is NULL). */
 GRIDDER_API int gridder_run_host(gridder_plan_t *plan, const double *h_uvw_m, int32_t n_time, int32_t n_baseline,
                      const double *h_freq_hz, int32_t n_chan, const float *h_vis,

@@ -269,6 +269,7 @@ int gridder_destroy(gridder_plan_t *plan) {
     if (!p) return GRIDDER_ERR_INVALID_ARG;
     cudaError_t e = cudaDeviceSynchronize();     // the caller may free the workspace after this
     image_destroy(*p);
+    if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
     for (int r = 0; r < kProfRing; ++r)
         for (int i = 0; i < 7; ++i) if (p->ev[r][i]) cudaEventDestroy(p->ev[r][i]);
     delete p;
@@ -355,18 +356,65 @@ int gridder_run_host(gridder_plan_t *plan, const double *h_uvw_m, int32_t n_time
     if (n_time < 0 || n_baseline < 0 || n_chan < 0) return GRIDDER_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const size_t n_tb = (size_t)n_time * n_baseline, n = n_tb * n_chan;
+    const size_t gbytes = (size_t)4 * p->cfg.grid_size * p->cfg.grid_size * 2 * sizeof(float);
     cudaError_t e = cudaMemcpyAsync(d_uvw_m, h_uvw_m, n_tb * 3 * sizeof(double), cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_freq_hz, h_freq_hz, (size_t)n_chan * sizeof(double), cudaMemcpyHostToDevice, s);
     if (e != cudaSuccess) return cuda_fail(p, e);
-    // the binning only needs uvw and freq: it runs while the visibilities are still on the wire
-    int rc = gridder_bin(plan, d_uvw_m, n_time, n_baseline, d_freq_hz, n_chan, cuda_stream);
-    if (rc != GRIDDER_OK) return rc;
-    e = cudaMemcpyAsync(d_vis, h_vis, n * 8 * sizeof(float), cudaMemcpyHostToDevice, s);
-    if (e == cudaSuccess && h_weight) e = cudaMemcpyAsync(d_weight, h_weight, n * sizeof(float), cudaMemcpyHostToDevice, s);
-    if (e != cudaSuccess) return cuda_fail(p, e);
-    rc = gridder_grid(plan, d_vis, h_weight ? d_weight : nullptr, d_grid, 0, cuda_stream);
-    if (rc != GRIDDER_OK) return rc;
-    const size_t gbytes = (size_t)4 * p->cfg.grid_size * p->cfg.grid_size * 2 * sizeof(float);
+
+    // Large inputs are copied and gridded in slices of the flattened (integration, baseline) axis: the
+    // copies run on a second stream, slice k is binned and gridded (added to the grid) while slice k+1
+    // is still on the wire.  Gridding is linear, so the slices sum to the same grid (each slice's
+    // result is rounded to FP32 once more when it is added; deterministic all the same).
+    const int n_slices = (n * 32 >= ((size_t)env_int("GRIDDER_HOST_SLICE_MIN_MB", 256) << 20) && n_tb >= 8 &&
+                          env_int("GRIDDER_HOST_SLICES", 8) > 1)
+                             ? (int)(n_tb < (size_t)env_int("GRIDDER_HOST_SLICES", 8) ? n_tb : (size_t)(env_int("GRIDDER_HOST_SLICES", 8) > 64 ? 64 : env_int("GRIDDER_HOST_SLICES", 8)))
+                             : 1;
+    if (n_slices == 1) {
+        // the binning only needs uvw and freq: it is enqueued ahead of the visibility copy
+        int rc = gridder_bin(plan, d_uvw_m, n_time, n_baseline, d_freq_hz, n_chan, cuda_stream);
+        if (rc != GRIDDER_OK) return rc;
+        e = cudaMemcpyAsync(d_vis, h_vis, n * 8 * sizeof(float), cudaMemcpyHostToDevice, s);
+        if (e == cudaSuccess && h_weight) e = cudaMemcpyAsync(d_weight, h_weight, n * sizeof(float), cudaMemcpyHostToDevice, s);
+        if (e != cudaSuccess) return cuda_fail(p, e);
+        rc = gridder_grid(plan, d_vis, h_weight ? d_weight : nullptr, d_grid, 0, cuda_stream);
+        if (rc != GRIDDER_OK) return rc;
+    } else {
+        if (!p->copy_stream && cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking) != cudaSuccess)
+            return cuda_fail(p, cudaGetLastError());
+        cudaEvent_t ev[64], ev_start;
+        int n_ev = 0;
+        int rc = GRIDDER_OK;
+        // the copy stream starts after whatever the caller's stream was doing with the staging buffers
+        e = cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming);
+        if (e != cudaSuccess) return cuda_fail(p, e);
+        e = cudaEventRecord(ev_start, s);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(p->copy_stream, ev_start, 0);
+        cudaEventDestroy(ev_start);
+        // all copies are enqueued first (their stream never waits for the compute stream)
+        for (int k = 0; k < n_slices && e == cudaSuccess; ++k) {
+            const size_t r0 = n_tb * k / n_slices, r1 = n_tb * (k + 1) / n_slices, cnt = (r1 - r0) * n_chan;
+            e = cudaMemcpyAsync(d_vis + r0 * n_chan * 8, h_vis + r0 * n_chan * 8, cnt * 8 * sizeof(float),
+                                cudaMemcpyHostToDevice, p->copy_stream);
+            if (e == cudaSuccess && h_weight)
+                e = cudaMemcpyAsync(d_weight + r0 * n_chan, h_weight + r0 * n_chan, cnt * sizeof(float),
+                                    cudaMemcpyHostToDevice, p->copy_stream);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev[k], cudaEventDisableTiming);
+            if (e == cudaSuccess) { ++n_ev; e = cudaEventRecord(ev[k], p->copy_stream); }
+        }
+        for (int k = 0; k < n_slices && e == cudaSuccess && rc == GRIDDER_OK; ++k) {
+            const size_t r0 = n_tb * k / n_slices, r1 = n_tb * (k + 1) / n_slices;
+            e = cudaStreamWaitEvent(s, ev[k], 0);
+            if (e != cudaSuccess) break;
+            rc = gridder_bin(plan, d_uvw_m + r0 * 3, 1, (int32_t)(r1 - r0), d_freq_hz, n_chan, cuda_stream);
+            if (rc == GRIDDER_OK)
+                rc = gridder_grid(plan, d_vis + r0 * n_chan * 8, h_weight ? d_weight + r0 * n_chan : nullptr, d_grid,
+                                  k > 0 ? 1 : 0, cuda_stream);
+        }
+        if (e != cudaSuccess || rc != GRIDDER_OK) cudaStreamSynchronize(p->copy_stream);
+        for (int k = 0; k < n_ev; ++k) cudaEventDestroy(ev[k]);
+        if (e != cudaSuccess) return cuda_fail(p, e);
+        if (rc != GRIDDER_OK) return rc;
+    }
     e = cudaMemcpyAsync(h_grid, d_grid, gbytes, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return cuda_fail(p, e);
