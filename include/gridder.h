@@ -114,6 +114,15 @@ GRIDDER_API int gridder_plan(const gridder_config *cfg, gridder_plan_t **plan_ou
 GRIDDER_API int gridder_bin(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
                 const double *freq_hz, int32_t n_chan, void *cuda_stream);
 
+/* per-baseline GCFs (PAPER.md :73, :179: "a unique GCF for each visibility" is the
+ * paper's stated end state).  As gridder_bin, but the table of every (integration, baseline) is the
+ * caller's choice: table_index DEVICE int32 [n_time][n_baseline], each in [0, n_wplanes) -- the plan's
+ * "w-planes" are then simply a bank of tables with their own supports, and w only decides conjugation
+ * (complex tables).  An index outside the bank drops the baseline (counted).  NULL = gridder_bin. */
+GRIDDER_API int gridder_bin_tables(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
+                                   const double *freq_hz, int32_t n_chan, const int32_t *table_index,
+                                   void *cuda_stream);
+
 /* Grid + flush.  weight may be NULL (all 1).  accumulate == 0 overwrites all 4*N*N cells,
  * otherwise the result is added to `grid`.  Asynchronous on `cuda_stream`. */
 GRIDDER_API int gridder_grid(gridder_plan_t *plan, const float *vis, const float *weight, float *grid,
@@ -129,7 +138,8 @@ GRIDDER_API int gridder_get_stats(gridder_plan_t *plan, gridder_stats *out);
 /* The mapping alone, for tests: out is DEVICE int32 [n][6] = x0, y0, qx, qy, plane | conj << 8,
  * dropped -- per visibility, same device function as gridder_bin's map kernel. */
 GRIDDER_API int gridder_map(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
-                const double *freq_hz, int32_t n_chan, int32_t *out, void *cuda_stream);
+                const double *freq_hz, int32_t n_chan, const int32_t *table_index /* or NULL */, int32_t *out,
+                void *cuda_stream);
 
 /* the arithmetic of the paper's OpenGL gridder (PAPER.md :185-191: one
  * screen-aligned GCF quad per visibility, additive blending) as plain CUDA: every (visibility, tap,

@@ -33,7 +33,8 @@ def build(force: bool = False) -> Path:
 class _Params(C.Structure):
     _fields_ = [("grid_size", C.c_int32), ("cell_size", C.c_double), ("oversample", C.c_int32),
                 ("n_wplanes", C.c_int32), ("support", C.POINTER(C.c_int32)), ("w_max", C.c_double),
-                ("kernel_is_complex", C.c_int32), ("kernel", C.POINTER(C.c_float))]
+                ("kernel_is_complex", C.c_int32), ("kernel", C.POINTER(C.c_float)),
+                ("table_index", C.POINTER(C.c_int32))]
 
 
 def _load():
@@ -58,7 +59,7 @@ class _Args:
     """Keeps the numpy buffers alive next to the C struct that points at them."""
 
     def __init__(self, grid_size, cell_size, oversample, support, kernel, w_max=1.0,
-                 kernel_is_complex=False):
+                 kernel_is_complex=False, table_index=None):
         self.support = np.ascontiguousarray(support, dtype=np.int32).ravel()
         self.kernel = np.ascontiguousarray(kernel, dtype=np.float32).ravel()
         need = int(sum((int(s) * oversample) ** 2 for s in self.support)) * (2 if kernel_is_complex else 1)
@@ -66,9 +67,11 @@ class _Args:
             raise ValueError(f"kernel table has {self.kernel.size} floats, expected {need}")
         if grid_size % 2 or any((int(s) * oversample) % 2 for s in self.support):
             raise ValueError("grid_size and every S*O must be even")
+        self.table_index = None if table_index is None else np.ascontiguousarray(table_index, dtype=np.int32).ravel()
         self.p = _Params(int(grid_size), float(cell_size), int(oversample), int(self.support.size),
                          _ptr(self.support, C.c_int32), float(w_max), int(bool(kernel_is_complex)),
-                         _ptr(self.kernel, C.c_float))
+                         _ptr(self.kernel, C.c_float),
+                         None if self.table_index is None else _ptr(self.table_index, C.c_int32))
 
 
 def _inputs(uvw_m, freq_hz, vis=None, weight=None):
@@ -91,9 +94,9 @@ def _inputs(uvw_m, freq_hz, vis=None, weight=None):
 
 
 def map_visibilities(uvw_m, freq_hz, *, grid_size, cell_size, oversample, support, kernel,
-                     w_max=1.0, kernel_is_complex=False) -> np.ndarray:
+                     w_max=1.0, kernel_is_complex=False, table_index=None) -> np.ndarray:
     """Steps 1-4 of the definition per visibility: int32 [n][6] = x0, y0, qx, qy, plane|conj<<8, dropped."""
-    a = _Args(grid_size, cell_size, oversample, support, kernel, w_max, kernel_is_complex)
+    a = _Args(grid_size, cell_size, oversample, support, kernel, w_max, kernel_is_complex, table_index)
     uvw, freq, _, _, n_time, n_bl = _inputs(uvw_m, freq_hz)
     out = np.empty((n_time * n_bl * freq.size, 6), dtype=np.int32)
     rc = _load().oracle_map(C.byref(a.p), _ptr(uvw, C.c_double), n_time, n_bl, _ptr(freq, C.c_double),
@@ -104,15 +107,18 @@ def map_visibilities(uvw_m, freq_hz, *, grid_size, cell_size, oversample, suppor
 
 
 def grid_windows(uvw_m, freq_hz, vis, weight, windows, *, grid_size, cell_size, oversample, support,
-                 kernel, w_max=1.0, kernel_is_complex=False, want_abs=True, n_threads=0, out=None):
+                 kernel, w_max=1.0, kernel_is_complex=False, want_abs=True, n_threads=0, out=None,
+                 table_index=None):
     """Direct scatter restricted to each window (y_lo, y_hi, x_lo, x_hi).
 
     Returns (list of complex128 [4][h][w], list of float64 [4][h][w] or None, stats dict).  With
     ``out=(G_list, A_list)`` from an earlier call the sums are added to (used to feed the
     integrations of config 4 one at a time).
     """
-    a = _Args(grid_size, cell_size, oversample, support, kernel, w_max, kernel_is_complex)
+    a = _Args(grid_size, cell_size, oversample, support, kernel, w_max, kernel_is_complex, table_index)
     uvw, freq, v, w, n_time, n_bl = _inputs(uvw_m, freq_hz, vis, weight)
+    if a.table_index is not None and a.table_index.size != n_time * n_bl:
+        raise ValueError("table_index must have n_time * n_baseline entries")
     wins = [tuple(int(x) for x in win) for win in windows]
     sizes = [4 * (y1 - y0) * (x1 - x0) for (y0, y1, x0, x1) in wins]
     offs = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
@@ -142,14 +148,16 @@ def grid_windows(uvw_m, freq_hz, vis, weight, windows, *, grid_size, cell_size, 
 
 
 def grid_full(uvw_m, freq_hz, vis, weight=None, *, grid_size, cell_size, oversample, support, kernel,
-              w_max=1.0, kernel_is_complex=False, want_abs=True, n_threads=0):
+              w_max=1.0, kernel_is_complex=False, want_abs=True, n_threads=0, table_index=None):
     """The whole grid: complex128 [4][N][N], float64 [4][N][N] (or None), stats.
 
     Threads own disjoint row bands of the one shared grid (one writer per cell, so the result is
     the same for any thread count); each band is the same direct scatter over all visibilities.
     """
-    a = _Args(grid_size, cell_size, oversample, support, kernel, w_max, kernel_is_complex)
+    a = _Args(grid_size, cell_size, oversample, support, kernel, w_max, kernel_is_complex, table_index)
     uvw, freq, v, w, n_time, n_bl = _inputs(uvw_m, freq_hz, vis, weight)
+    if a.table_index is not None and a.table_index.size != n_time * n_bl:
+        raise ValueError("table_index must have n_time * n_baseline entries")
     n = int(grid_size)
     nt = n_threads if n_threads > 0 else max_threads()
     nb = max(1, min(n, nt))

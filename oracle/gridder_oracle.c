@@ -41,6 +41,9 @@ typedef struct {
     double w_max;               /* wavelengths                                                  */
     int32_t kernel_is_complex;  /* 0: float table; 1: (re, im) float pairs, conj for w < 0      */
     const float *kernel;        /* plane-major; plane p is [S_p O][S_p O] samples               */
+    const int32_t *table_index; /* NULL, or [n_time][n_baseline]: the GCF of each baseline, chosen by
+                                   the caller instead of by |w| (PAPER.md :73, :179 "a unique GCF for
+                                   each visibility").  Out of range: dropped.           */
 } oracle_params;
 
 typedef struct {
@@ -75,11 +78,15 @@ static void map_axis(double coord_lambda, const oracle_params *p, int S, int64_t
 }
 
 /* Steps 1-4 of the definition for one (baseline vector in metres, frequency scale s = f / c). */
-static oracle_map_t map_one(const oracle_params *p, double u_m, double v_m, double w_m, double s) {
+static oracle_map_t map_one(const oracle_params *p, double u_m, double v_m, double w_m, double s, int64_t tb) {
     oracle_map_t m;
     double ul = u_m * s, vl = v_m * s, wl = w_m * s;
     m.plane = 0;
-    if (p->n_wplanes > 1) {
+    int bad_table = 0;
+    if (p->table_index) {
+        m.plane = p->table_index[tb];
+        if (m.plane < 0 || m.plane >= p->n_wplanes) { bad_table = 1; m.plane = 0; }
+    } else if (p->n_wplanes > 1) {
         double fp = floor(fabs(wl) / p->w_max * (double)p->n_wplanes);
         m.plane = (fp >= (double)(p->n_wplanes - 1)) ? p->n_wplanes - 1 : (int32_t)fp;
     }
@@ -88,7 +95,7 @@ static oracle_map_t map_one(const oracle_params *p, double u_m, double v_m, doub
     map_axis(ul, p, m.support, &m.x0, &m.qx);
     map_axis(vl, p, m.support, &m.y0, &m.qy);
     const int64_t N = p->grid_size;
-    m.dropped = (m.x0 < 0 || m.x0 + m.support > N || m.y0 < 0 || m.y0 + m.support > N) ? 1 : 0;
+    m.dropped = (bad_table || m.x0 < 0 || m.x0 + m.support > N || m.y0 < 0 || m.y0 + m.support > N) ? 1 : 0;
     return m;
 }
 
@@ -110,7 +117,7 @@ int oracle_map(const oracle_params *p, const double *uvw_m, int32_t n_time, int3
             const double *L = uvw_m + (t * n_baseline + b) * 3;
             for (int64_t f = 0; f < n_chan; ++f) {
                 double s = freq_hz[f] / ORACLE_C_M_PER_S;
-                oracle_map_t m = map_one(p, L[0], L[1], L[2], s);
+                oracle_map_t m = map_one(p, L[0], L[1], L[2], s, t * n_baseline + b);
                 int32_t *o = out + ((t * n_baseline + b) * n_chan + f) * 6;
                 int64_t cx = m.x0, cy = m.y0;
                 if (cx < -(1 << 30)) cx = -(1 << 30);
@@ -144,7 +151,7 @@ static void scatter_window(const oracle_params *p, const double *uvw_m, int32_t 
             for (int64_t f = 0; f < n_chan; ++f) {
                 const int64_t i = (t * n_baseline + b) * n_chan + f;
                 double s = freq_hz[f] / ORACLE_C_M_PER_S;
-                oracle_map_t m = map_one(p, L[0], L[1], L[2], s);
+                oracle_map_t m = map_one(p, L[0], L[1], L[2], s, t * n_baseline + b);
                 if (m.dropped) { n_drop++; continue; }
                 const int64_t S = m.support;
                 n_taps += S * S;

@@ -234,6 +234,11 @@ int gridder_plan(const gridder_config *cfg, gridder_plan_t **plan_out, size_t *w
 
 int gridder_bin(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
                 const double *freq_hz, int32_t n_chan, void *cuda_stream) {
+    return gridder_bin_tables(plan, uvw_m, n_time, n_baseline, freq_hz, n_chan, nullptr, cuda_stream);
+}
+
+int gridder_bin_tables(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
+                       const double *freq_hz, int32_t n_chan, const int32_t *table_index, void *cuda_stream) {
     Plan *p = reinterpret_cast<Plan *>(plan);
     if (!p || n_time < 0 || n_baseline < 0 || n_chan < 0) return GRIDDER_ERR_INVALID_ARG;
     const int64_t n = (int64_t)n_time * n_baseline * n_chan;
@@ -242,7 +247,9 @@ int gridder_bin(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32
     if (n_chan > kMaxChannels) return GRIDDER_ERR_UNSUPPORTED;
     p->binned = false;
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    cudaError_t e = launch_bin(*p, uvw_m, n_time, n_baseline, freq_hz, n_chan, s);
+    // a bank of one real table on the fast path: there is nothing to choose
+    if (table_index && p->mode == 0 && p->cfg.n_wplanes == 1) table_index = nullptr;
+    cudaError_t e = launch_bin(*p, uvw_m, n_time, n_baseline, freq_hz, n_chan, table_index, s);
     if (e != cudaSuccess) return cuda_fail(p, e);
     p->n_vis = n;
     p->binned = true;
@@ -301,12 +308,13 @@ int gridder_get_stats(gridder_plan_t *plan, gridder_stats *out) {
 }
 
 int gridder_map(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
-                const double *freq_hz, int32_t n_chan, int32_t *out, void *cuda_stream) {
+                const double *freq_hz, int32_t n_chan, const int32_t *table_index, int32_t *out, void *cuda_stream) {
     Plan *p = reinterpret_cast<Plan *>(plan);
     if (!p || !uvw_m || !freq_hz || !out || n_time < 0 || n_baseline < 0 || n_chan < 0)
         return GRIDDER_ERR_INVALID_ARG;
     if ((int64_t)n_time * n_baseline * n_chan == 0) return GRIDDER_OK;
-    cudaError_t e = launch_map_debug(*p, uvw_m, n_time, n_baseline, freq_hz, n_chan, out, (cudaStream_t)cuda_stream);
+    cudaError_t e = launch_map_debug(*p, uvw_m, n_time, n_baseline, freq_hz, n_chan, table_index, out,
+                                     (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(p, e);
     return GRIDDER_OK;
 }

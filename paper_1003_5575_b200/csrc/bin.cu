@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(256) map_kernel(const double *__restrict__ uvw
         const unsigned int tb = i / n_chan;
         const unsigned int f = i - tb * n_chan;
         const double *L = uvw + (size_t)tb * 3;
-        const VisMap m = map_vis(L[0], L[1], GENERAL ? L[2] : 0.0, scale[f], p);
+        const VisMap m = map_vis(L[0], L[1], GENERAL ? L[2] : 0.0, scale[f], p, tb);
         uint32_t key;
         if (m.dropped) {
             dropped_here++;
@@ -125,7 +125,7 @@ __global__ void __launch_bounds__(256) map_debug_kernel(const double *__restrict
         const long long tb = i / n_chan;
         const int f = (int)(i - tb * n_chan);
         const double s = __ddiv_rn(freq[f], kSpeedOfLight);
-        const VisMap m = map_vis(uvw[tb * 3 + 0], uvw[tb * 3 + 1], uvw[tb * 3 + 2], s, p);
+        const VisMap m = map_vis(uvw[tb * 3 + 0], uvw[tb * 3 + 1], uvw[tb * 3 + 2], s, p, (unsigned int)tb);
         int32_t *o = out + i * 6;
         o[0] = m.x0; o[1] = m.y0; o[2] = m.qx; o[3] = m.qy;      // origins are clamped to +-2^30 by the map
         o[4] = m.plane | (m.conj << 8); o[5] = m.dropped ? 1 : 0;
@@ -169,10 +169,11 @@ static int blocks_for(long long n, int threads, int n_sm) {
 }
 
 cudaError_t launch_map_debug(const Plan &p, const double *uvw, int n_time, int n_bl, const double *freq,
-                             int n_chan, int32_t *out, cudaStream_t s) {
+                             int n_chan, const int32_t *table_index, int32_t *out, cudaStream_t s) {
     const long long n_tb = (long long)n_time * n_bl;
-    map_debug_kernel<<<blocks_for(n_tb * n_chan, 256, p.n_sm), 256, 0, s>>>(uvw, freq, n_tb, n_chan,
-                                                                             make_map_params(p), out);
+    MapParams mp = make_map_params(p);
+    mp.table_index = table_index;
+    map_debug_kernel<<<blocks_for(n_tb * n_chan, 256, p.n_sm), 256, 0, s>>>(uvw, freq, n_tb, n_chan, mp, out);
     return cudaGetLastError();
 }
 
@@ -283,7 +284,7 @@ cudaError_t scan_temp_bytes(int64_t n, size_t *bytes) {
 #define GR_TRY(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return e_; } while (0)
 
 cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const double *freq, int n_chan,
-                       cudaStream_t s) {
+                       const int32_t *table_index, cudaStream_t s) {
     const long long n_tb = (long long)n_time * n_bl;
     const long long n = n_tb * n_chan;
     const int n_vtiles = p.n_tiles * p.n_cls;
@@ -308,7 +309,8 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
             }
         }
         if (!by_runs) {
-            const MapParams mp = make_map_params(p);
+            MapParams mp = make_map_params(p);
+            mp.table_index = p.mode != 0 ? table_index : nullptr;
             if (p.mode == 0)
                 map_kernel<false><<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp,
                                                                               p.keys[0], p.vals[0], p.counters);

@@ -64,6 +64,7 @@ struct MapParams {
     double rcp_cell;         // RN(1 / du): screening value only, never decides a rounding (map.cuh)
     double span;             // N O: scale of the screening margin
     double w_max;
+    const int32_t *table_index;   // null, or DEVICE [n_time][n_baseline]: the table of each baseline (row f3)
     KeyLayout key;
     int32_t support[kMaxPlanes];
     int32_t cls_slot[kMaxPlanes];       // class slot of the plane (index into the plan's classes)
@@ -198,9 +199,9 @@ inline void stage_mark(Plan &p, int i, cudaStream_t s) {
 MapParams make_map_params(const Plan &p);
 cudaError_t launch_relayout(const Plan &p, cudaStream_t s);
 cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const double *freq, int n_chan,
-                       cudaStream_t s);
+                       const int32_t *table_index, cudaStream_t s);
 cudaError_t launch_map_debug(const Plan &p, const double *uvw, int n_time, int n_bl, const double *freq,
-                             int n_chan, int32_t *out, cudaStream_t s);
+                             int n_chan, const int32_t *table_index, int32_t *out, cudaStream_t s);
 cudaError_t sort_temp_bytes(int64_t n, int begin_bit, int end_bit, bool wide, size_t *bytes);
 
 // runs.cu

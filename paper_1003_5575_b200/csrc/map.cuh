@@ -83,24 +83,33 @@ struct VisMap {
     bool dropped;
 };
 
-__device__ __forceinline__ VisMap map_vis(double u_m, double v_m, double w_m, double s, const MapParams &p) {
+__device__ __forceinline__ VisMap map_vis(double u_m, double v_m, double w_m, double s, const MapParams &p,
+                                          unsigned int tb = 0) {
     const double ul = __dmul_rn(u_m, s), vl = __dmul_rn(v_m, s);
     VisMap m;
     m.plane = 0;
     m.conj = 0;
     if (p.n_planes > 1 || p.is_complex) {
         const double wl = __dmul_rn(w_m, s);
-        if (p.n_planes > 1) {
+        if (p.table_index) {
+            // (handled below: the caller chose the table)
+        } else if (p.n_planes > 1) {
             const double fp = floor(__dmul_rn(__ddiv_rn(fabs(wl), p.w_max), (double)p.n_planes));
             m.plane = (fp >= (double)(p.n_planes - 1)) ? p.n_planes - 1 : (int)fp;
         }
         m.conj = (p.is_complex && wl < 0.0) ? 1 : 0;
     }
+    bool bad_table = false;
+    if (p.table_index) {           // row f3: per-baseline GCF; an index outside the bank drops the baseline
+        const int t = p.table_index[tb];
+        bad_table = t < 0 || t >= p.n_planes;
+        m.plane = bad_table ? 0 : t;
+    }
     m.S = p.support[m.plane];
     const AxisMap mx = map_axis(ul, p, m.S), my = map_axis(vl, p, m.S);
     m.x0 = mx.x0; m.y0 = my.x0; m.qx = mx.q; m.qy = my.q;
     const int N = p.n_grid, S = m.S;
-    m.dropped = mx.far || my.far || m.x0 < 0 || m.x0 + S > N || m.y0 < 0 || m.y0 + S > N;
+    m.dropped = bad_table || mx.far || my.far || m.x0 < 0 || m.x0 + S > N || m.y0 < 0 || m.y0 + S > N;
     return m;
 }
 

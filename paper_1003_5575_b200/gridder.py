@@ -17,7 +17,7 @@ LIB_PATH = _HERE / "libgridder.so"
 
 OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_WORKSPACE, ERR_CUDA, ERR_NOT_BINNED, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 
-EXPORTS = ("gridder_workspace_size", "gridder_plan", "gridder_bin", "gridder_grid", "gridder_destroy",
+EXPORTS = ("gridder_workspace_size", "gridder_plan", "gridder_bin", "gridder_bin_tables", "gridder_grid", "gridder_destroy",
            "gridder_get_stats", "gridder_map", "gridder_scatter_atomic", "gridder_image_workspace_size", "gridder_image",
            "gridder_run_host", "gridder_set_profiling",
            "gridder_get_stage_ms", "gridder_launch_count", "gridder_strerror",
@@ -58,11 +58,13 @@ def load_library() -> C.CDLL:
         lib.gridder_workspace_size.argtypes = [C.POINTER(_Config), C.POINTER(C.c_size_t)]
         lib.gridder_plan.argtypes = [C.POINTER(_Config), C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
         lib.gridder_bin.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p]
+        lib.gridder_bin_tables.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
+                                           C.c_void_p, C.c_void_p]
         lib.gridder_grid.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
         lib.gridder_destroy.argtypes = [C.c_void_p]
         lib.gridder_get_stats.argtypes = [C.c_void_p, C.POINTER(_Stats)]
         lib.gridder_map.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
-                                    C.c_void_p, C.c_void_p]
+                                    C.c_void_p, C.c_void_p, C.c_void_p]
         lib.gridder_scatter_atomic.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
                                                C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
         lib.gridder_image_workspace_size.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
@@ -157,16 +159,18 @@ class Gridder:
         self._keep = []
 
     # -- the four calls ---------------------------------------------------------------------
-    def bin(self, uvw_m: torch.Tensor, freq_hz: torch.Tensor, stream=None) -> None:
-        """uvw_m float64 [n_time][n_baseline][3] (metres), freq_hz float64 [n_chan]; asynchronous."""
+    def bin(self, uvw_m: torch.Tensor, freq_hz: torch.Tensor, stream=None, table_index=None) -> None:
+        """uvw_m float64 [n_time][n_baseline][3] (metres), freq_hz float64 [n_chan]; table_index (row f3):
+        int32 [n_time][n_baseline] choosing each baseline's table from the plan's bank, or None."""
         if uvw_m.dim() == 2:
             uvw_m = uvw_m[None]
         n_time, n_bl, three = uvw_m.shape
         if three != 3:
             raise ValueError("uvw_m must be [n_time][n_baseline][3]")
-        self._keep = [uvw_m, freq_hz]
-        rc = self._lib.gridder_bin(self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m"), n_time, n_bl,
-                                   _dev_ptr(freq_hz, torch.float64, "freq_hz"), freq_hz.numel(), _stream_ptr(stream))
+        self._keep = [uvw_m, freq_hz, table_index]
+        rc = self._lib.gridder_bin_tables(self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m"), n_time, n_bl,
+                                          _dev_ptr(freq_hz, torch.float64, "freq_hz"), freq_hz.numel(),
+                                          _dev_ptr(table_index, torch.int32, "table_index"), _stream_ptr(stream))
         if rc != OK:
             raise GridderError(rc, "gridder_bin")
 
@@ -214,15 +218,15 @@ class Gridder:
     def launch_count(self) -> int:
         return int(self._lib.gridder_launch_count(self._plan))
 
-    def map(self, uvw_m: torch.Tensor, freq_hz: torch.Tensor, stream=None) -> torch.Tensor:
+    def map(self, uvw_m: torch.Tensor, freq_hz: torch.Tensor, stream=None, table_index=None) -> torch.Tensor:
         """int32 [n][6] = x0, y0, qx, qy, plane | conj << 8, dropped (the map kernel's device function)."""
         if uvw_m.dim() == 2:
             uvw_m = uvw_m[None]
         n_time, n_bl, _ = uvw_m.shape
         out = torch.empty((n_time * n_bl * freq_hz.numel(), 6), dtype=torch.int32, device=self.device)
         rc = self._lib.gridder_map(self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m"), n_time, n_bl,
-                                   _dev_ptr(freq_hz, torch.float64, "freq_hz"), freq_hz.numel(), out.data_ptr(),
-                                   _stream_ptr(stream))
+                                   _dev_ptr(freq_hz, torch.float64, "freq_hz"), freq_hz.numel(),
+                                   _dev_ptr(table_index, torch.int32, "table_index"), out.data_ptr(), _stream_ptr(stream))
         if rc != OK:
             raise GridderError(rc, "gridder_map")
         return out

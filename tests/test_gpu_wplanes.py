@@ -149,3 +149,39 @@ def test_config3_reduced_full_grid(dev):
                                   supports=wl.support, table=wl.kernel, w_max=wl.w_max, cplx=True)
     assert st.n_dropped == 0 and st.n_vis == wl.n_vis
     assert_parity(got, ref, ab, "config 3 (2 channels)")
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+def test_per_baseline_tables_row_f3(dev, cplx):
+    """gridder_bin_tables: every (integration, baseline) names its own table of the plan's bank
+    (PAPER.md :73, :179); indices outside the bank drop the baseline; w only decides conjugation."""
+    from paper_1003_5575_b200 import gridder
+    rng = np.random.default_rng(61 + cplx)
+    supports = [6, 8, 12, 16, 22, 32]
+    O, N, nb, nf, w_max = 2, 128, 3000, 3, 1.0
+    table = _tables(rng, supports, O, cplx)
+    uvw = np.zeros((2, nb, 3))
+    uvw[:, :, :2] = rng.uniform(-N / 2 - 1, N / 2 + 1, (2, nb, 2)) / 1.1
+    uvw[:, :, 2] = rng.uniform(-3.0, 3.0, (2, nb))
+    freq = C * np.array([1.0, 1.05, 1.1])
+    idx = rng.integers(0, len(supports), (2, nb)).astype(np.int32)
+    idx[0, :4] = (-1, len(supports), 1 << 20, -(1 << 20))
+    vis = rng.standard_normal((2, nb, nf, 4, 2)).astype(np.float32)
+    w = rng.uniform(0.5, 1.5, (2, nb, nf)).astype(np.float32)
+    g = gridder.Gridder(grid_size=N, cell_size=1.0, oversample=O, support=supports, kernel=torch.from_numpy(table).to(dev),
+                        max_vis=2 * nb * nf, n_wplanes=len(supports), w_max=w_max, kernel_is_complex=cplx)
+    d_uvw, d_f = torch.from_numpy(uvw).to(dev), torch.from_numpy(freq).to(dev)
+    d_idx = torch.from_numpy(idx).to(dev)
+    got_map = g.map(d_uvw, d_f, table_index=d_idx).cpu().numpy()
+    g.bin(d_uvw, d_f, table_index=d_idx)
+    out1 = g.grid(torch.from_numpy(vis).to(dev), torch.from_numpy(w).to(dev)).cpu().numpy()
+    out2 = g.grid(torch.from_numpy(vis).to(dev), torch.from_numpy(w).to(dev)).cpu().numpy()
+    st = g.stats()
+    g.destroy()
+    kw = dict(grid_size=N, cell_size=1.0, oversample=O, support=supports, kernel=table, w_max=w_max,
+              kernel_is_complex=cplx, table_index=idx)
+    assert np.array_equal(got_map, oracle.map_visibilities(uvw, freq, **kw))
+    ref, ab, ost = oracle.grid_full(uvw, freq, vis, w, **kw)
+    assert st.n_dropped == ost["n_dropped"] >= 4 * nf and st.vis_taps == ost["vis_taps"]
+    assert np.array_equal(out1, out2)
+    assert_parity(out1, ref, ab, f"per-baseline tables, complex={cplx}")

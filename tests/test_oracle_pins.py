@@ -355,6 +355,39 @@ def test_wplanes_variable_support_and_conjugate():
     assert np.allclose(g[1, k - s // 2:k + s // 2, k - s // 2:k + s // 2], exp, rtol=1e-15)
 
 
+def test_per_baseline_tables_reduce_to_single_table_gridding():
+    """Row f3 (PAPER.md :73, :179 "a unique GCF for each visibility"): with table_index the GCF of a baseline
+    is the caller's choice, not |w|'s.  Pin: by linearity the grid equals the sum, over the tables j, of
+    gridding the baselines that use j with a single-table problem -- the case P1-P5 pin; an index outside
+    the bank drops the baseline; the conjugate is still taken for w < 0."""
+    rng = np.random.default_rng(33)
+    N, O, nb = 48, 2, 300
+    supports = [5, 8, 12, 20]
+    tabs = [(rng.standard_normal((s * O, s * O)) + 1j * rng.standard_normal((s * O, s * O))).astype(np.complex64)
+            for s in supports]
+    kernel = np.concatenate([t.view(np.float32).ravel() for t in tabs])
+    uv = rng.uniform(-N / 2 + 1, N / 2 - 1, (nb, 2))
+    w = rng.uniform(-5.0, 5.0, nb)
+    idx = rng.integers(0, len(supports), nb).astype(np.int32)
+    idx[:3] = (-1, len(supports), 99)                              # not in the bank: dropped
+    vis, wt = _vis(nb, rng), rng.uniform(0.5, 1.5, nb).astype(np.float32)
+    g, a, st = _grid(uv, vis, wt, N=N, S=supports, O=O, table=kernel, w=w, w_max=1.0, kernel_is_complex=True,
+                     table_index=idx)
+    want, want_a, taps, dropped = np.zeros_like(g), np.zeros_like(a), 0, 3
+    for j, s_j in enumerate(supports):
+        m = idx == j
+        gj, aj, sj = _grid(uv[m], vis[m], wt[m], N=N, S=[s_j], O=O, table=tabs[j].view(np.float32).ravel(), w=w[m],
+                           kernel_is_complex=True)
+        want += gj; want_a += aj; taps += sj["vis_taps"]; dropped += sj["n_dropped"]
+    assert st["vis_taps"] == taps and st["n_dropped"] == dropped
+    assert np.abs(g - want).max() <= 1e-12 * np.abs(want).max()
+    assert np.abs(a - want_a).max() <= 1e-12 * want_a.max()
+    m = oracle.map_visibilities(np.concatenate([uv, w[:, None]], 1)[None], [C], grid_size=N, cell_size=1.0, oversample=O,
+                                support=supports, kernel=kernel, kernel_is_complex=True, table_index=idx)
+    assert np.array_equal(m[3:, 4] & 0xFF, idx[3:]) and np.array_equal(m[3:, 4] >> 8, (w[3:] < 0).astype(np.int32))
+    assert m[:3, 5].all()
+
+
 def test_map_matches_gather_algebra():
     """oracle.map_visibilities (what the CUDA map kernel is compared with) against the gather view:
     the patch is exactly the set of cells whose centre the table reaches."""
