@@ -17,7 +17,8 @@
  * Pins (tests/test_oracle_pins.py, all -m "not gpu"): P1 unit visibility reproduces the table at
  * every sub-cell shift; P2 linearity; P3 total-sum identity; P4 grid -> inverse FFT -> grid
  * correction vs brute-force direct DFT; P5 brute-force gather restatement (:181, :195);
- * P6 the paper's "around 60 visibilities per pixel" (:183).  No function here is "parity unpinned".
+ * P6 the paper's "around 60 visibilities per pixel" (:183); w-planes and per-baseline tables (row f3)
+ * against single-table gridding by linearity.  No function here is "parity unpinned".
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC   (no FMA contraction: every operation
  * below rounds once, in the order written, so the mapping is reproducible bit for bit).

@@ -7,8 +7,8 @@
 //   * for the current patch origin the SP x SP patch lives in REGISTERS, NA*NB cells (x 4 pol
 //     complex = 8 floats) per lane; entries are sorted by origin, so the patch is exchanged with
 //     the shared region only when the origin changes ("fold");
-//   * per entry a lane does broadcast LDS.128 of the staged visibility, NA vector loads of its
-//     taps of the GCF sub-table and 8*NA*NB FFMA (16*NA*NB for a complex table);
+//   * per entry a lane does two broadcast LDS.128 of the staged visibility, NA vector loads of its
+//     taps of the GCF sub-table and 4*NA*NB packed FFMA2 (fma.rn.f32x2; 8*NA*NB for a complex table);
 //   * a warp runs ONE software pipeline over the whole stream of its work items: keys three
 //     batches ahead, visibilities (cp.async, 128-bit) two ahead, weighting and record staging one
 //     ahead, so the start of an item costs no exposed memory latency;
