@@ -102,7 +102,11 @@ int derive(const gridder_config *cfg, Plan &p) {
         p.run_cap = cfg->max_vis / 4;
         if (p.run_cap < 1024) p.run_cap = 1024;
     }
-    p.chunk = env_int("GRIDDER_CHUNK", 4096);
+    // K: most entries per work item.  4096 for big inputs; small inputs get shorter items so that a hot
+    // tile still spreads over the ~1800 resident warps (K ~ max_vis / 2^14, a power of two >= 256)
+    int k_auto = 4096;
+    while (k_auto > 256 && (int64_t)k_auto * 16384 > cfg->max_vis) k_auto >>= 1;
+    p.chunk = env_int("GRIDDER_CHUNK", k_auto);
     if (p.chunk < 32 || p.chunk > (1 << 20)) return GRIDDER_ERR_INVALID_ARG;
     p.warps_forced = env_int("GRIDDER_WARPS", 0);
     p.fold_batches = env_int("GRIDDER_FOLD_BATCHES", 8);
