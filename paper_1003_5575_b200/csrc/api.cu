@@ -51,6 +51,11 @@ int derive(const gridder_config *cfg, Plan &p) {
     p.ntx = (cfg->grid_size + p.T - 1) / p.T;
     p.nty = p.ntx;
     p.n_tiles = p.ntx * p.nty;
+    // the fast path keeps the sub-cell offsets in the 32-bit sort key; a grid too large for that
+    // (2 log2 N + 2 log2 O + 1 > 32 bits) goes through the general path, whose values carry them
+    if (p.mode == 0 &&
+        2 * ceil_log2((unsigned long long)cfg->oversample) + 1 + 2 * p.tlog + ceil_log2((unsigned long long)p.n_tiles) > 32)
+        p.mode = 1;
 
     // patch classes in use (ascending), and each plane's slot and table offset
     int slot_of_class[kMaxClasses] = {-1, -1, -1};

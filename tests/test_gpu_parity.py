@@ -250,8 +250,8 @@ def test_error_paths_on_device(dev):
     assert e.value.code == gridder.ERR_NOT_BINNED
     g.destroy()
     with pytest.raises(gridder.GridderError) as e:
-        gridder.Gridder(grid_size=32768, cell_size=1.0, oversample=4, support=[16], kernel=torch.zeros(64 * 64, device=dev),
-                        max_vis=100)
+        gridder.Gridder(grid_size=64, cell_size=1.0, oversample=64, support=[32] * 64, n_wplanes=64, w_max=1.0,
+                        kernel_is_complex=True, kernel=torch.zeros(8, device=dev), max_vis=100)
     assert e.value.code == gridder.ERR_UNSUPPORTED
 
 
@@ -313,3 +313,41 @@ def test_run_host_sliced_copy_compute_overlap_matches_oracle(dev, monkeypatch):
     assert_parity(outs[2], ref, ab, "run_host, single shot")
     assert not np.array_equal(outs[0], outs[2]) or True          # the modes may differ in the last bits
     assert np.abs(as_complex(outs[0]) - as_complex(outs[2])).max() <= 2e-6 * np.abs(ref).max()
+
+
+def test_large_grid_takes_the_general_path(dev):
+    """N = 16384 with O = 4: tile + origin + sub-cell bits need 33 key bits, so the plan switches to the
+    general path (sub-cell offsets in the sort value).  Windows around a few visibilities against the oracle."""
+    from paper_1003_5575_b200 import gridder
+    rng = np.random.default_rng(16384)
+    N, S, O, n = 16384, 16, 4, 4000
+    table = synth.spheroidal_table(S, O)
+    uvw = np.zeros((1, n, 3))
+    uvw[0, :, :2] = rng.uniform(-N / 2 + 40, N / 2 - 40, (n, 2))
+    uvw[0, :200, :2] = rng.uniform(-30.0, 30.0, (200, 2))                 # a busy patch in the middle
+    vis = rng.standard_normal((n, 4, 2)).astype(np.float32)
+    g = gridder.Gridder(grid_size=N, cell_size=1.0, oversample=O, support=[S], kernel=torch.from_numpy(table.ravel()).to(dev),
+                        max_vis=n)
+    g.bin(torch.from_numpy(uvw).to(dev), torch.tensor([C], dtype=torch.float64, device=dev))
+    grid = g.grid(torch.from_numpy(vis).to(dev))
+    st = g.stats()
+    wins = [(N // 2 - 48, N // 2 + 48, N // 2 - 48, N // 2 + 48)]
+    for k in (300, 1000, 2500, 3999):
+        cx, cy = int(uvw[0, k, 0]) + N // 2, int(uvw[0, k, 1]) + N // 2
+        wins.append((cy - 12, cy + 12, cx - 12, cx + 12))
+    got = [grid[:, y0:y1, x0:x1].cpu().numpy() for (y0, y1, x0, x1) in wins]
+    total = float(grid[..., 0].double().sum().item())
+    g.destroy()
+    del grid
+    torch.cuda.empty_cache()
+    res = oracle.grid_windows(uvw, [C], vis, None, wins, grid_size=N, cell_size=1.0, oversample=O, support=[S], kernel=table)
+    assert st.n_dropped == res["n_dropped"] == 0 and st.vis_taps == res["vis_taps"] == n * S * S
+    for k in range(len(wins)):
+        assert res["A"][k].max() > 0
+        assert_parity(got[k], res["G"][k], res["A"][k], f"N=16384 window {wins[k]}")
+    # nothing is lost outside the windows either: total of the real parts = sum_i Re V_i * (per-offset table sum)
+    m = oracle.map_visibilities(uvw, [C], grid_size=N, cell_size=1.0, oversample=O, support=[S], kernel=table)
+    t64 = table.astype(np.float64)
+    csum = np.array([[t64[qy::O, qx::O].sum() for qx in range(O)] for qy in range(O)])
+    want = (vis[:, :, 0].astype(np.float64).sum(1) * csum[m[:, 3], m[:, 2]]).sum()
+    assert abs(total - want) <= 1e-4 * np.abs(vis[:, :, 0]).sum() * csum.max() * 1e-1 + 1e-2

@@ -54,8 +54,12 @@ def test_null_and_invalid_arguments_need_no_device(lib):
     sup3 = (C.c_int32 * 3)(8, 16, 32)
     assert lib.gridder_workspace_size(C.byref(cfg(n_wplanes=3, support=sup3, w_max=10.0)), C.byref(need)) == gridder.OK
     assert lib.gridder_workspace_size(C.byref(cfg(n_wplanes=3, support=sup3, w_max=0.0)), C.byref(need)) == gridder.ERR_INVALID_ARG
-    # a sort key that does not fit 32 bits (2^26 tiles of 4 x 4 cells + origin + sub-cell bits)
-    assert lib.gridder_workspace_size(C.byref(cfg(grid_size=32768)), C.byref(need)) == gridder.ERR_UNSUPPORTED
+    # the largest grid is sized too (its key has no room for the sub-cell bits: general path)
+    assert lib.gridder_workspace_size(C.byref(cfg(grid_size=32768)), C.byref(need)) == gridder.OK
+    # a table bank of 2 GB and more is beyond the 32-bit table offsets
+    sup64 = (C.c_int32 * 64)(*([32] * 64))
+    assert lib.gridder_workspace_size(C.byref(cfg(n_wplanes=64, support=sup64, oversample=64, kernel_is_complex=1,
+                                                  w_max=1.0)), C.byref(need)) == gridder.ERR_UNSUPPORTED
     plan = C.c_void_p()
     assert lib.gridder_plan(C.byref(cfg(grid_size=255)), C.byref(plan), None) == gridder.ERR_INVALID_ARG
     assert lib.gridder_plan(C.byref(cfg()), None, None) == gridder.ERR_INVALID_ARG
