@@ -99,6 +99,11 @@ typedef struct {
     int32_t patch_size;         /* padded patch edge handled per entry (8 or 16)                     */
     int32_t chunk_size;         /* K: most entries per work item                                     */
     int32_t grid_warps_per_sm;  /* launch shape of the grid kernel                                   */
+    /* of the last gridder_grid (0 before the first): */
+    int64_t n_records_gridded;  /* records the grid kernels processed: entries with equal patch origin and
+                                   table offset inside a batch of 32 are summed first (exact by linearity) */
+    int64_t fma_executed;       /* FP32 FMAs those records cost, padded taps included: records x patch cells
+                                   x 8 (real table) or 16 (complex): what the roofline fraction is claimed on */
 } gridder_stats;
 
 /* Bytes of workspace a plan for `cfg` needs (cfg->workspace / workspace_bytes / kernel ignored). */

@@ -114,6 +114,7 @@ int derive(const gridder_config *cfg, Plan &p) {
     p.chunk = env_int("GRIDDER_CHUNK", k_auto);
     if (p.chunk < 32 || p.chunk > (1 << 20)) return GRIDDER_ERR_INVALID_ARG;
     p.warps_forced = env_int("GRIDDER_WARPS", 0);
+    p.merge = env_int("GRIDDER_MERGE", 1) ? 1 : 0;
     p.fold_batches = env_int("GRIDDER_FOLD_BATCHES", 8);
     if (p.fold_batches < 1 || p.fold_batches > 64 || (p.fold_batches & (p.fold_batches - 1))) return GRIDDER_ERR_INVALID_ARG;
 
@@ -313,6 +314,11 @@ int gridder_get_stats(gridder_plan_t *plan, gridder_stats *out) {
     out->patch_size = p->cls[p->n_cls - 1].SP;
     out->chunk_size = p->chunk;
     out->grid_warps_per_sm = p->cls[p->n_cls - 1].warps;
+    for (int k = 0; k < p->n_cls; ++k) {
+        const ClassGeo &g = p->cls[k];
+        out->n_records_gridded += (int64_t)c.n_exec[k];
+        out->fma_executed += (int64_t)c.n_exec[k] * (8 * g.NA) * (4 * g.NB) * (p->cfg.kernel_is_complex ? 16 : 8);
+    }
     return GRIDDER_OK;
 }
 

@@ -99,6 +99,7 @@ struct Counters {
     unsigned int cls_end[kMaxClasses];
     unsigned int queue_head[kMaxClasses];     // work queues of the grid kernel launches
     unsigned int pad[2];
+    unsigned long long n_exec[kMaxClasses];   // records gridded per class by the last gridder_grid (after merging)
 };
 
 struct GridParams {
@@ -116,6 +117,7 @@ struct GridParams {
     int32_t sub_stride_bytes;      // table distance between sub-patches (O^2 sub-tables)
     int32_t tmem_cols;             // tensor-memory columns to allocate (MODE 3)
     int32_t n_q;                   // O^2 sub-tables
+    int32_t merge;                 // sum entries of a batch with equal origin and table offset before gridding
     KeyLayout key;
 };
 
@@ -142,6 +144,7 @@ struct Plan {
     uint32_t plane_off256[kMaxPlanes];
     int32_t tlog, T, ntx, nty, n_tiles;
     int32_t chunk;                 // K
+    int32_t merge;                 // GRIDDER_MERGE (default 1)
     int32_t fold_batches;          // longest FP32 register chain, in batches of 32 entries (power of 2)
     int32_t warps_forced, n_sm;
     int64_t max_items;             // capacity of the work-item table (all classes)

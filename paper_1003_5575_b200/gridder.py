@@ -41,7 +41,8 @@ class _Stats(C.Structure):
     _fields_ = [("n_vis", C.c_int64), ("n_dropped", C.c_int64), ("n_entries", C.c_int64),
                 ("vis_taps", C.c_int64), ("n_tiles", C.c_int64), ("n_tiles_occupied", C.c_int64),
                 ("max_tile_load", C.c_int64), ("n_work_items", C.c_int64), ("tile_size", C.c_int32),
-                ("patch_size", C.c_int32), ("chunk_size", C.c_int32), ("grid_warps_per_sm", C.c_int32)]
+                ("patch_size", C.c_int32), ("chunk_size", C.c_int32), ("grid_warps_per_sm", C.c_int32),
+                ("n_records_gridded", C.c_int64), ("fma_executed", C.c_int64)]
 
 
 _lib = None
@@ -122,6 +123,8 @@ class Stats:
     patch_size: int
     chunk_size: int
     grid_warps_per_sm: int
+    n_records_gridded: int = 0
+    fma_executed: int = 0
 
 
 class Gridder:
