@@ -351,3 +351,29 @@ def test_large_grid_takes_the_general_path(dev):
     csum = np.array([[t64[qy::O, qx::O].sum() for qx in range(O)] for qy in range(O)])
     want = (vis[:, :, 0].astype(np.float64).sum(1) * csum[m[:, 3], m[:, 2]]).sum()
     assert abs(total - want) <= 1e-4 * np.abs(vis[:, :, 0]).sum() * csum.max() * 1e-1 + 1e-2
+
+
+# ------------------------------------------------------------------------------------ merging
+def test_merging_of_equal_origin_and_offset_entries(dev):
+    """The grid kernel sums entries of a batch that share patch origin and sub-cell offset before gridding
+    them (exact by linearity).  Many visibilities on few lattice points: the merged and the unmerged runs
+    both match the oracle, the counters say what was executed, and a dense case really is merged."""
+    rng = np.random.default_rng(91)
+    N, S, O, n = 64, 16, 4, 20_000
+    table = synth.spheroidal_table(S, O)
+    uvw = np.zeros((1, n, 3))
+    uvw[0, :, :2] = rng.integers(-6, 7, (n, 2)) / 2.0               # 13 x 13 lattice points: heavy duplication
+    uvw[0, ::7, :2] += rng.uniform(-0.2, 0.2, (len(uvw[0, ::7]), 2))
+    vis = (rng.standard_normal((n, 4, 2)) + 1.0).astype(np.float32)
+    w = rng.uniform(0.5, 1.5, n).astype(np.float32)
+    kw = dict(N=N, du=1.0, O=O, S=S, table=table)
+    ref, ab, _ = _oracle(uvw, [C], vis, w, **kw)
+    a, st_a = _run(dev, uvw, [C], vis, w, **kw)
+    a2, _ = _run(dev, uvw, [C], vis, w, **kw)
+    b, st_b = _run(dev, uvw, [C], vis, w, env={"GRIDDER_MERGE": 0}, **kw)
+    assert np.array_equal(a, a2)
+    assert_parity(a, ref, ab, "merging on")
+    assert_parity(b, ref, ab, "merging off")
+    assert st_b.n_records_gridded == st_b.n_vis == n                 # unmerged: one record per entry (none dropped)
+    assert st_b.fma_executed == n * 256 * 8
+    assert st_a.n_records_gridded < n // 3 and st_a.fma_executed == st_a.n_records_gridded * 256 * 8
