@@ -188,6 +188,7 @@ cudaError_t carve(Plan &p, char *base) {
     p.tile_chunks = (unsigned long long *)take(sizeof(unsigned long long) * (n_vtiles + 1));
     p.tile_chunks_scan = (unsigned long long *)take(sizeof(unsigned long long) * (n_vtiles + 1));
     p.tile_info = (TileInfo *)take(sizeof(TileInfo) * n_vtiles);
+    p.tile_cover = (unsigned char *)take((size_t)p.n_tiles);
     p.items = (WorkItem *)take(sizeof(WorkItem) * (size_t)p.max_items);
     p.partials = (float4 *)take(sizeof(float4) * (size_t)p.partials_f4);
     p.coef = (float4 *)take(p.coef_bytes);

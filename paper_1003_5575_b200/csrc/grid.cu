@@ -596,12 +596,27 @@ struct FlushGeo {
     static constexpr int RW = T + PATCH - 1, RH = T + PATCH - 1, CELLS = RW * RH;
 };
 
+// cover[tile] = 1 when some occupied tile's region (all its sub-patches) can reach a cell of `tile`:
+// the later classes' flushes (which only add to the grid) skip every cell of an uncovered tile.
+__global__ void __launch_bounds__(256) tile_cover_kernel(const TileInfo *__restrict__ tiles, int ntx, int nty, int reach,
+                                                          unsigned char *__restrict__ cover) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ntx * nty) return;
+    const int tx = t % ntx, ty = t / ntx;
+    unsigned char c = 0;
+    for (int yy = max(0, ty - reach); yy <= ty && !c; ++yy)
+        for (int xx = max(0, tx - reach); xx <= tx; ++xx)
+            if (tiles[yy * ntx + xx].count) { c = 1; break; }
+    cover[t] = c;
+}
+
 template <int SP, int TLOG>
 __global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
     using G = FlushGeo<SP, TLOG>;
     const int x = blockIdx.x * 32 + threadIdx.x;
     const int y = blockIdx.y * 8 + threadIdx.y;
     if (x >= p.n_grid || y >= p.n_grid) return;
+    if (p.cover && !p.cover[min(y >> TLOG, p.nty - 1) * p.ntx + min(x >> TLOG, p.ntx - 1)]) return;
     double acc[8];
 #pragma unroll
     for (int k = 0; k < 8; ++k) acc[k] = 0.0;
@@ -788,6 +803,16 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         fp.ntx = p.ntx;
         fp.nty = p.nty;
         fp.accumulate = (c > 0 || accumulate) ? 1 : 0;
+        fp.cover = nullptr;
+        if (c > 0) {
+            // a later class only adds: cells no region of the class can reach are skipped (sparse classes)
+            const int reach = (g.RW - 1 + (g.nsub - 1) * 8 * g.NA + p.T - 1) / p.T;
+            tile_cover_kernel<<<(p.n_tiles + 255) / 256, 256, 0, s>>>(fp.tiles, p.ntx, p.nty, reach, p.tile_cover);
+            e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+            fp.cover = p.tile_cover;
+            p.n_launches += 1;
+        }
         dim3 blk(32, 8), grd((p.cfg.grid_size + 31) / 32, (p.cfg.grid_size + 7) / 8);
         ffn<<<grd, blk, 0, s>>>(fp);
         e = cudaGetLastError();

@@ -130,6 +130,7 @@ struct FlushParams {
     int32_t n_grid;
     int32_t ntx, nty;
     int32_t accumulate;
+    const unsigned char *cover;    // null, or [n_tiles]: 0 = no region of this class reaches the tile's cells
 };
 
 struct Plan {
@@ -166,6 +167,7 @@ struct Plan {
     uint32_t *tile_start;          // [2][n_vtiles]: first entry | one past the last entry
     unsigned long long *tile_chunks, *tile_chunks_scan;   // packed (n_full << 32 | has_tail), [n_vtiles+1]
     TileInfo *tile_info;           // [n_vtiles]
+    unsigned char *tile_cover;     // [n_tiles] scratch of the later classes' flushes
     WorkItem *items;               // [max_items]
     float4 *partials;              // per class: [max_items_cls][region_f4 of the class]
     float4 *coef;                  // re-laid table(s)
