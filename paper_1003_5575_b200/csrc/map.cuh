@@ -126,4 +126,56 @@ __device__ __forceinline__ uint32_t fast_key(const VisMap &m, const MapParams &p
            ((x0 & tmask) << p.key.aux_bits) | ((uint32_t)m.qy << p.key.bits_q) | (uint32_t)m.qx;
 }
 
+// The fast path's mapper with its constants in registers (one real table, power-of-two oversampling).
+// Bit for bit the result of map_vis + fast_key: it accepts a position only under a STRICTER screening
+// margin than map_axis (2^-48 * 2 N O >= 2^-48 (|h| + N O) for |h| < N O), where map_axis takes the same
+// multiply-by-reciprocal value and the same 32-bit algebra; everything else goes to map_vis itself.
+struct FastMap {
+    double rcp_cell, half_n, d_o, eps, one_minus_eps, span;
+    int o_shift, o_minus_1, half_so, n_minus_s, s2;
+    uint32_t ntx, tmask, tlog, aux_bits, bits_q, tile_shift;
+
+    __device__ __forceinline__ void init(const MapParams &p) {
+        rcp_cell = p.rcp_cell; half_n = (double)(p.n_grid / 2); d_o = (double)p.oversample; span = p.span;
+        eps = p.span * 7.1054273576010019e-15;                 // 2^-48 * 2 N O
+        one_minus_eps = 1.0 - eps;
+        o_shift = p.o_shift; o_minus_1 = p.oversample - 1;
+        half_so = (p.support[0] * p.oversample) >> 1;
+        n_minus_s = p.n_grid - p.support[0];
+        s2 = p.support[0] * p.support[0];
+        ntx = (uint32_t)p.ntx; tlog = (uint32_t)p.key.tlog; tmask = (1u << p.key.tlog) - 1u;
+        aux_bits = (uint32_t)p.key.aux_bits; bits_q = (uint32_t)p.key.bits_q; tile_shift = (uint32_t)p.key.tile_shift;
+    }
+    __device__ __forceinline__ bool axis(double coord_lambda, int &x0, int &q) const {
+        const double h1 = __dmul_rn(__dadd_rn(__dmul_rn(coord_lambda, rcp_cell), half_n), d_o);
+        const double t1 = __dadd_rn(h1, 0.5);
+        const double r = floor(t1);
+        const double fr = t1 - r;
+        if (!(fabs(h1) < span && fr > eps && fr < one_minus_eps)) return false;
+        const int a = (int)r - half_so;
+        x0 = (a + o_minus_1) >> o_shift;                        // ceil(a / O), arithmetic shift = floor division
+        q = (x0 << o_shift) - a;
+        return true;
+    }
+    // sort key of the visibility (fast_key's layout); `taps` gets S^2 or 0 (dropped)
+    __device__ __forceinline__ uint32_t key(double u_m, double v_m, double s, const MapParams &p, int &taps) const {
+        int x0, y0, qx, qy;
+        const bool okx = axis(__dmul_rn(u_m, s), x0, qx), oky = axis(__dmul_rn(v_m, s), y0, qy);
+        if (okx && oky) {
+            if ((unsigned)x0 > (unsigned)n_minus_s || (unsigned)y0 > (unsigned)n_minus_s) {     // off the grid
+                taps = 0;
+                return 1u << (2 * bits_q);                      // drop slot 0, tile 0, origin (0, 0)
+            }
+            taps = s2;
+            const uint32_t ux = (uint32_t)x0, uy = (uint32_t)y0;
+            const uint32_t tile = (uy >> tlog) * ntx + (ux >> tlog);
+            return (tile << tile_shift) | ((uy & tmask) << (aux_bits + tlog)) | ((ux & tmask) << aux_bits) |
+                   ((uint32_t)qy << bits_q) | (uint32_t)qx;
+        }
+        const VisMap m = map_vis(u_m, v_m, 0.0, s, p);          // rare: near a rounding boundary, or far away
+        taps = m.dropped ? 0 : m.S * m.S;
+        return fast_key(m, p);
+    }
+};
+
 }  // namespace gridder

@@ -24,6 +24,7 @@ namespace gridder {
 
 constexpr int kRunThreads = 256, kRunItems = 4, kRunTile = kRunThreads * kRunItems;
 
+template <bool FAST>
 __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__restrict__ uvw,
                                                                 const double *__restrict__ scale, unsigned int n,
                                                                 unsigned int n_chan, const MapParams p,
@@ -38,6 +39,14 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
     const unsigned int bid = blockIdx.x;
     const unsigned int base = bid * (unsigned)kRunTile + (unsigned)tid * kRunItems;    // n <= 2^32 - 4096: no wrap
     const uint32_t aux_mask = (1u << p.key.aux_bits) - 1u;
+    FastMap fm;
+    if (FAST) fm.init(p);
+    auto key_of = [&](const double *L, double s, int &taps) -> uint32_t {
+        if (FAST) return fm.key(L[0], L[1], s, p, taps);
+        const VisMap m = map_vis(L[0], L[1], 0.0, s, p);
+        taps = m.dropped ? 0 : m.S * m.S;
+        return fast_key(m, p);
+    };
 
     // thread 0 also maps the visibility just before the block's first one (its key decides whether the
     // block starts inside a run); done before the barrier so that it costs no extra phase
@@ -46,7 +55,8 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
         const unsigned int i = base - 1;
         const unsigned int tb = i / n_chan, f = i - tb * n_chan;
         const double *L = uvw + (size_t)tb * 3;
-        prev = fast_key(map_vis(L[0], L[1], 0.0, scale[f], p), p) >> p.key.aux_bits;
+        int taps;
+        prev = key_of(L, scale[f], taps) >> p.key.aux_bits;
     }
     uint32_t sk[kRunItems];
     unsigned int fch[kRunItems];
@@ -64,9 +74,9 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
         sk[k] = 0xFFFFFFFFu; fch[k] = 1; q[k] = 0;
         if (base + k < n) {
             const double *L = uvw + (size_t)tb * 3;
-            const VisMap m = map_vis(L[0], L[1], 0.0, scale[f], p);
-            const uint32_t key = fast_key(m, p);
-            if (m.dropped) dropped_here++; else taps_here += (unsigned long long)(m.S * m.S);
+            int taps;
+            const uint32_t key = key_of(L, scale[f], taps);
+            if (taps == 0) dropped_here++; else taps_here += (unsigned long long)taps;
             sk[k] = key >> p.key.aux_bits;
             q[k] = (unsigned char)(key & aux_mask);
             fch[k] = f;
@@ -280,8 +290,12 @@ cudaError_t launch_bin_runs(Plan &p, const double *uvw, const double *scale, lon
     uint32_t *stage_key = p.keys[1], *stage_start = (uint32_t *)p.vals[1];
     unsigned int *block_count = p.run_blk, *block_prefix = p.run_blk + (n_blocks + 1), *part = p.run_blk + 2 * (n_blocks + 1);
     GR_TRY(cudaMemsetAsync(block_count + n_blocks, 0, sizeof(unsigned int), s));
-    map_runs_kernel<<<n_blocks, kRunThreads, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp, p.qaux, stage_key,
-                                                      stage_start, block_count, p.counters);
+    if (mp.o_shift >= 0 && mp.drop_slot == 0)
+        map_runs_kernel<true><<<n_blocks, kRunThreads, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp, p.qaux,
+                                                                stage_key, stage_start, block_count, p.counters);
+    else
+        map_runs_kernel<false><<<n_blocks, kRunThreads, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp, p.qaux,
+                                                                 stage_key, stage_start, block_count, p.counters);
     GR_TRY(cudaGetLastError());
     size_t tb = p.cub_temp_bytes;
     GR_TRY(cub::DeviceScan::ExclusiveSum(p.cub_temp, tb, (const unsigned int *)block_count, block_prefix,
