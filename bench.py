@@ -39,7 +39,7 @@ BAND_HZ = 768 * 40.0e3           # one rank's band; rank r starts at 140 MHz + r
 # dram__bytes_read.sum + dram__bytes_write.sum of one grid_kernel launch from the committed
 # `ncu --set full` capture (profiles/), keyed by config; None until a capture exists for it.
 NCU_GRID_KERNEL_TRAFFIC_BYTES = {
-    4: 53_909_963_000,    # profiles/r01d_grid_kernel_config4_ncu_full.csv: 47.290430 GB read + 6.619533 GB written
+    4: 53_910_878_000,    # profiles/r01d_grid_kernel_config4_ncu_full.csv: 47.291082 GB read + 6.619796 GB written
     2: 9_348_989_000,     # profiles/r01_grid_kernel_config2_ncu_full.csv: 4.109023 GB read + 5.239966 GB written
 }
 
