@@ -27,7 +27,7 @@
  *   - Calls only enqueue work on `cuda_stream` (a cudaStream_t passed as void*; NULL = default
  *     stream).  gridder_plan, gridder_destroy, gridder_get_stats and gridder_run_host synchronise;
  *     gridder_bin synchronises the stream ONCE in the middle when it bins by channel runs (plans
- *     with one real table, S <= 16, O <= 8): the number of runs sizes the sort.  What it enqueues
+ *     with one real table, S <= 16, O <= 8 and max_vis >= 4 Mi): the number of runs sizes the sort.  What it enqueues
  *     after that is asynchronous again.
  *   - Buffers given to gridder_bin / gridder_grid must stay valid until that work has completed.
  *   - A plan may be binned and gridded any number of times; one gridder_bin serves any number of

@@ -103,7 +103,11 @@ int derive(const gridder_config *cfg, Plan &p) {
     }
     // fast path: bin by channel runs when the key's unsorted bits fit one byte (runs.cu)
     p.run_cap = 0;
-    if (p.mode == 0 && env_int("GRIDDER_RUNS", 1) && 2 * ceil_log2((unsigned long long)cfg->oversample) + 1 <= 8) {
+    // GRIDDER_RUNS: 0 never, 1 (default) for plans of 4 M visibilities and more -- below that the per-visibility
+    // sort is cheap and the run path's one host synchronisation is not --, 2 always
+    const int runs_mode = env_int("GRIDDER_RUNS", 1);
+    if (p.mode == 0 && (runs_mode >= 2 || (runs_mode == 1 && cfg->max_vis >= (4ll << 20))) &&
+        2 * ceil_log2((unsigned long long)cfg->oversample) + 1 <= 8) {
         p.run_cap = cfg->max_vis / 4;
         if (p.run_cap < 1024) p.run_cap = 1024;
     }

@@ -270,7 +270,7 @@ def test_run_binning_gives_the_same_bits_as_the_per_visibility_sort(dev):
     vis = rng.standard_normal((2, nb, nf, 4, 2)).astype(np.float32)
     w = rng.uniform(0.5, 1.5, (2, nb, nf)).astype(np.float32)
     kw = dict(N=N, du=1.0, O=O, S=S, table=table)
-    a, st_a = _run(dev, uvw, freq, vis, w, **kw)
+    a, st_a = _run(dev, uvw, freq, vis, w, env={"GRIDDER_RUNS": 2}, **kw)        # 2: also for a plan this small
     b, st_b = _run(dev, uvw, freq, vis, w, env={"GRIDDER_RUNS": 0}, **kw)
     assert np.array_equal(a, b)
     assert (st_a.n_dropped, st_a.vis_taps, st_a.n_work_items, st_a.max_tile_load) == \
@@ -280,7 +280,7 @@ def test_run_binning_gives_the_same_bits_as_the_per_visibility_sort(dev):
     assert ost["n_dropped"] == st_a.n_dropped
     assert_parity(a, ref, ab, "run binning")
     # single-channel input: every visibility is its own run -> the plan falls back to the per-visibility sort
-    c, _ = _run(dev, uvw[:, :, :], freq[:1], vis[:, :, :1].copy(), w[:, :, :1].copy(), **kw)
+    c, _ = _run(dev, uvw[:, :, :], freq[:1], vis[:, :, :1].copy(), w[:, :, :1].copy(), env={"GRIDDER_RUNS": 2}, **kw)
     d, _ = _run(dev, uvw[:, :, :], freq[:1], vis[:, :, :1].copy(), w[:, :, :1].copy(), env={"GRIDDER_RUNS": 0}, **kw)
     assert np.array_equal(c, d)
 
