@@ -111,9 +111,11 @@ int derive(const gridder_config *cfg, Plan &p) {
         p.run_cap = cfg->max_vis / 4;
         if (p.run_cap < 1024) p.run_cap = 1024;
     }
-    // K: most entries per work item.  4096 for big inputs; small inputs get shorter items so that a hot
-    // tile still spreads over the ~1800 resident warps (K ~ max_vis / 2^14, a power of two >= 256)
-    int k_auto = 4096;
+    // K: most entries per work item, ~ max_vis / 2^14 as a power of two in [256, 8192]: small inputs get
+    // short items so that a hot tile still spreads over the ~1800 resident warps; the largest get 8192,
+    // which halves the number of partial regions the flush has to sum for the cells of a hot tile
+    // (the accuracy budget of DESIGN.md section 7 holds up to 8192)
+    int k_auto = 8192;
     while (k_auto > 256 && (int64_t)k_auto * 16384 > cfg->max_vis) k_auto >>= 1;
     p.chunk = env_int("GRIDDER_CHUNK", k_auto);
     if (p.chunk < 32 || p.chunk > (1 << 20)) return GRIDDER_ERR_INVALID_ARG;
