@@ -16,7 +16,7 @@ CSRC = HERE / "csrc"
 LIB = HERE / "libgridder.so"
 SOURCES = ["api.cu", "bin.cu", "grid.cu", "runs.cu", "scatter.cu", "image.cu"]
 HEADERS = [CSRC / "gridder_internal.cuh", CSRC / "map.cuh", HERE.parent / "include" / "gridder.h"]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Wno-deprecated-gpu-targets",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]
 
 
@@ -49,7 +49,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
     if force or procs or _stale(LIB, objs):
         tmp = LIB.with_suffix(f".{os.getpid()}.tmp")
-        cmd = [_nvcc(), "-shared", "-o", str(tmp)] + [str(o) for o in objs] + ["-lcudart", "-ldl"]
+        cmd = [_nvcc(), "-shared", "-Wno-deprecated-gpu-targets", "-o", str(tmp)] + [str(o) for o in objs] + ["-lcudart", "-ldl"]
         subprocess.check_call(cmd)
         os.replace(tmp, LIB)
     return LIB

@@ -15,7 +15,7 @@
 // everything downstream (tile tables, grid kernel, flush) and every output bit is unchanged.
 #include <cub/device/device_radix_sort.cuh>
 #include <cub/device/device_scan.cuh>
-#include <cub/iterator/transform_input_iterator.cuh>
+#include <thrust/iterator/transform_iterator.h>
 
 #include "gridder_internal.cuh"
 #include "map.cuh"
@@ -270,7 +270,7 @@ cudaError_t runs_temp_bytes(int64_t cap, int begin_bit, int end_bit, size_t *byt
     cub::DoubleBuffer<unsigned long long> v(nullptr, nullptr);
     cudaError_t e = cub::DeviceRadixSort::SortPairs(nullptr, a, k, v, (long long)cap, begin_bit, end_bit, (cudaStream_t)0);
     if (e != cudaSuccess) return e;
-    cub::TransformInputIterator<unsigned int, RunLen, const unsigned long long *> it(nullptr, RunLen());
+    auto it = thrust::make_transform_iterator((const unsigned long long *)nullptr, RunLen());
     e = cub::DeviceScan::ExclusiveSum(nullptr, b, it, (unsigned int *)nullptr, (long long)cap, (cudaStream_t)0);
     *bytes = a > b ? a : b;
     return e;
@@ -316,7 +316,7 @@ cudaError_t launch_bin_runs(Plan &p, const double *uvw, const double *scale, lon
     cub::DoubleBuffer<unsigned long long> v(rval[0], rval[1]);
     tb = p.cub_temp_bytes;
     GR_TRY(cub::DeviceRadixSort::SortPairs(p.cub_temp, tb, k, v, (long long)n_runs, p.key.aux_bits, p.key.total_bits, s));
-    cub::TransformInputIterator<unsigned int, RunLen, const unsigned long long *> it(v.Current(), RunLen());
+    auto it = thrust::make_transform_iterator((const unsigned long long *)v.Current(), RunLen());
     tb = p.cub_temp_bytes;
     GR_TRY(cub::DeviceScan::ExclusiveSum(p.cub_temp, tb, it, p.run_cum, (long long)n_runs, s));
     expand_partition_kernel<<<(n_blocks + 255) / 256, 256, 0, s>>>(p.run_cum, n_runs, n_blocks, part);
