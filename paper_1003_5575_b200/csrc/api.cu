@@ -121,6 +121,14 @@ int derive(const gridder_config *cfg, Plan &p) {
     if (p.chunk < 32 || p.chunk > (1 << 20)) return GRIDDER_ERR_INVALID_ARG;
     p.warps_forced = env_int("GRIDDER_WARPS", 0);
     p.merge = env_int("GRIDDER_MERGE", 1) ? 1 : 0;
+    // fast path with per-origin bins (grid.cu): one real table, 16-cell patch, O^2 <= 64 offsets
+    // GRIDDER_QBINS: 0 never, 1 (default) for dense plans -- 256 visibilities per tile and more, where an
+    // origin gathers many entries per sub-cell offset; sparser inputs merge as well per batch --, 2 always
+    p.qbins = 0;
+    const int qb_mode = env_int("GRIDDER_QBINS", 1);
+    if (p.mode == 0 && p.merge && p.tmem_cols == 0 && p.cls[0].NA == 2 && oo <= 64 &&
+        (qb_mode >= 2 || (qb_mode == 1 && cfg->max_vis / p.n_tiles >= 256)))
+        p.qbins = (int)oo;
     p.fold_batches = env_int("GRIDDER_FOLD_BATCHES", 8);
     if (p.fold_batches < 1 || p.fold_batches > 64 || (p.fold_batches & (p.fold_batches - 1))) return GRIDDER_ERR_INVALID_ARG;
 

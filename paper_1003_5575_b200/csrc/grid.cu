@@ -583,6 +583,176 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
 }
 
 // ------------------------------------------------------------------------------------------
+// The fast path with PER-ORIGIN BINS (one real table in shared memory, 16 x 16 patch, merging on).
+// Entries of a work item are sorted by patch origin, and for one origin there are only O^2 possible
+// sub-cell offsets, i.e. O^2 different sets of taps.  So the weighted visibilities of an origin are
+// first summed into O^2 bins of shared memory (512 B per warp at O = 4) and only when the origin
+// changes are the non-empty bins gridded (256 FMAs each) -- at most O^2 records per (item, origin)
+// however many entries it has; exact by linearity like the per-batch merging of stage_write, of
+// which this is the complete form.  Fixed order: inside a batch the first lane of a group adds the
+// others in ascending lane order, batches are added to the bins in sequence, bins are gridded in
+// offset order: bit-identical reruns.  FP32 chains: <= 32 (batch), <= K/32 (bin), <= O^2 records
+// in registers per origin, then the fold: inside the budget of DESIGN.md section 7.
+// Pipeline per warp: sorted (key, index) pairs three batches ahead in registers, visibilities two
+// batches ahead (cp.async into three landing buffers); a batch is accumulated straight out of its
+// landing buffer, there is no record ring.
+// ------------------------------------------------------------------------------------------
+template <int TLOG, int MAXW>
+__global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel_qbins(const GridParams p) {
+    constexpr int NA = 2, NB = 4, NRAW = 3;
+    using G = Geo<NA, NB, 1, TLOG, 0>;
+    extern __shared__ float4 smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n_q = p.n_q;                                     // O^2 <= 64 bins
+    const int warp_f4 = 2 * G::CELLS + 2 * n_q + NRAW * G::RAW_F4;
+    float4 *region = smem + p.coef_f4 + warp * warp_f4;        // plane A (XX, XY) then plane B (YX, YY)
+    float4 *regA = region, *regB = region + G::CELLS;
+    float4 *bins = region + 2 * G::CELLS;                      // [q][2] float4: sum of w V of the current origin
+    float4 *raw = bins + 2 * n_q;                              // NRAW cp.async landing buffers
+
+    for (int i = threadIdx.x; i < p.coef_f4; i += blockDim.x) smem[i] = p.coef[i];
+    for (int i = lane; i < warp_f4; i += 32) region[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncthreads();
+
+    const int lane_cell = (lane >> 3) * G::RW + (lane & 7);
+    const char *coef_lane = reinterpret_cast<const char *>((uintptr_t)((uint32_t)__cvta_generic_to_shared(smem) +
+                                                                        lane * NB * (int)sizeof(float)));
+    float acc[NA][NB][8];
+#pragma unroll
+    for (int a = 0; a < NA; ++a)
+#pragma unroll
+        for (int b = 0; b < NB; ++b)
+#pragma unroll
+            for (int k = 0; k < 8; ++k) acc[a][b][k] = 0.f;
+
+    Producer prod;
+    prod.init(p, lane, 0);
+    // batch i is processed while i+1 and i+2 are landing and i+3 has its pairs in flight
+    Desc d0, d1, d2, d3;
+    Entry e0, e1, e2, e3;
+    d0.bits = 0; d0.item = 0; d1 = d0; d2 = d0;
+    e0.key = e0.idx = e0.aux = 0u; e1 = e0; e2 = e0;
+    {
+        unsigned start;
+        d3 = prod.next(p, lane, start);
+        e3 = load_entry<false>(p, start + lane, lane < d3.cnt());
+    }
+    unsigned long long n_exec = 0;
+    const uint32_t tmask = (1u << TLOG) - 1u, qmask = (1u << (2 * p.key.bits_q)) - 1u;
+    int cur = -1, cmp = kSentinel;
+    int bin_org = kSentinel;             // origin the bins belong to
+    unsigned long long occ = 0;          // its non-empty bins
+    int slot = 0;                        // landing buffer of batch i
+
+    while (true) {
+        // batch i+2's visibilities start to move; batch i+3 gets its pairs; then batch i must have landed
+        d0 = d1; e0 = e1; d1 = d2; e1 = e2; d2 = d3; e2 = e3;
+        issue_vis<false>(p, raw + ((slot + 2) % NRAW) * G::RAW_F4, lane, e2, lane < d2.cnt());
+        {
+            unsigned start;
+            d3 = prod.next(p, lane, start);
+            e3 = load_entry<false>(p, start + lane, lane < d3.cnt());
+        }
+        asm volatile("cp.async.wait_group 2;" ::: "memory");
+        __syncwarp();
+        if (d0.end()) break;
+        const int cnt = d0.cnt();
+        if (cnt > 0) {
+            const float4 *rw = raw + slot * G::RAW_F4;
+            const uint32_t x0l = (e0.key >> p.key.aux_bits) & tmask, y0l = (e0.key >> (p.key.aux_bits + TLOG)) & tmask;
+            const bool valid = lane < cnt;
+            const int poff = valid ? (int)(y0l * G::RW + x0l) : kForce;
+            const int q = (int)(e0.key & qmask);
+            const float4 ra = rw[2 * lane], rb = rw[2 * lane + 1];
+            const float w = p.weight ? reinterpret_cast<const float *>(rw + 64)[lane] : 1.0f;
+            const float o[8] = {ra.x * w, ra.y * w, ra.z * w, ra.w * w, rb.x * w, rb.y * w, rb.z * w, rb.w * w};
+            float sum[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) sum[k] = o[k];
+            // groups of equal (origin, offset) inside the batch: the first lane adds the others
+            const unsigned gkey = valid ? (((unsigned)poff << 8) | (unsigned)q) : (0xFFFF0000u | lane);
+            const unsigned grp = __match_any_sync(0xffffffffu, gkey);
+            const bool keep = valid && (__ffs(grp) - 1 == lane);
+            unsigned rest = keep ? (grp & ~(1u << lane)) : 0u;
+            while (__any_sync(0xffffffffu, rest != 0u)) {
+                const int src = rest ? __ffs(rest) - 1 : lane;
+                const bool add = rest != 0u;
+                rest &= rest - 1u;
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const float t = __shfl_sync(0xffffffffu, o[k], src);
+                    if (add) sum[k] += t;
+                }
+            }
+            // origin by origin (the batch is sorted by origin); one more round with no origin ends the item
+            int lp = 0;
+            const bool last = d0.last();
+            while (lp < cnt || (last && lp == cnt)) {
+                const int seg = lp < cnt ? __shfl_sync(0xffffffffu, poff, lp) : kSentinel;
+                if (seg != bin_org) {
+                    // ---- grid the bins of the finished origin ------------------------------------------
+                    if (occ) {
+                        RecRegs<NA, NB, 0> A, B;
+                        unsigned long long m = occ;
+                        int qa = __ffsll((long long)m) - 1, qb;
+                        m &= m - 1ull;
+                        A.fetch(bins + 2 * qa, qa * G::SUB_BYTES, coef_lane);
+                        while (true) {
+                            qb = m ? __ffsll((long long)m) - 1 : -1;
+                            m &= m - 1ull;
+                            if (qb >= 0) B.fetch(bins + 2 * qb, qb * G::SUB_BYTES, coef_lane);
+                            consume<NA, NB, G::RW, 0>(A, bin_org, cur, cmp, regA, regB, lane_cell, acc);
+                            if (qb < 0) break;
+                            qa = m ? __ffsll((long long)m) - 1 : -1;
+                            m &= m - 1ull;
+                            if (qa >= 0) A.fetch(bins + 2 * qa, qa * G::SUB_BYTES, coef_lane);
+                            consume<NA, NB, G::RW, 0>(B, bin_org, cur, cmp, regA, regB, lane_cell, acc);
+                            if (qa < 0) break;
+                        }
+                        n_exec += (unsigned)__popcll(occ);
+                        __syncwarp();
+                        for (int k = lane; k < 2 * n_q; k += 32) bins[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        occ = 0;
+                        __syncwarp();
+                    }
+                    bin_org = seg;
+                }
+                if (lp >= cnt) break;
+                // ---- this origin's lanes of the batch go into the bins ---------------------------------
+                const bool in_seg = poff == seg;
+                const bool put = in_seg && keep;
+                if (put) {               // the kept lanes of one origin have distinct offsets
+                    float4 x = bins[2 * q], y = bins[2 * q + 1];
+                    x.x += sum[0]; x.y += sum[1]; x.z += sum[2]; x.w += sum[3];
+                    y.x += sum[4]; y.y += sum[5]; y.z += sum[6]; y.w += sum[7];
+                    bins[2 * q] = x; bins[2 * q + 1] = y;
+                }
+                const unsigned lo = __reduce_or_sync(0xffffffffu, (put && q < 32) ? (1u << q) : 0u);
+                const unsigned hi = __reduce_or_sync(0xffffffffu, (put && q >= 32) ? (1u << (q - 32)) : 0u);
+                occ |= ((unsigned long long)hi << 32) | lo;
+                lp += __popc(__ballot_sync(0xffffffffu, in_seg));
+                __syncwarp();
+            }
+            if (last) {
+                // the item's last origin has been gridded; fold it, write the region out, clear it
+                if (cur >= 0) fold_patch<NA, NB, G::RW>(regA, regB, cur + lane_cell, acc);
+                cur = -1; cmp = kSentinel; bin_org = kSentinel;
+                __syncwarp();
+                float4 *dst = p.partials + (size_t)d0.item * (2 * G::CELLS);
+                for (int k = lane; k < 2 * G::CELLS; k += 32) {
+                    stg_stream(dst + k, region[k]);
+                    region[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+                __syncwarp();
+            }
+        }
+        slot = (slot + 1) % NRAW;
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (lane == 0 && n_exec) atomicAdd(&p.counters->n_exec[p.cls], n_exec);
+}
+
+// ------------------------------------------------------------------------------------------
 // Flush: one thread per grid cell.  The partial regions covering cell (x, y) belong to the tiles
 // (ty, tx) with tx*T <= x < tx*T + RW (same in y); each tile's work items are added in id order
 // (full chunks, then the tail).  FP64 accumulation, one rounding to FP32 at the end.  One launch
@@ -663,8 +833,10 @@ __global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
 // Host side: kernel selection.  The register patch (NA x NB), the sub-patch count and the table
 // mode follow from the plan; TLOG is a plan parameter; the block size is chosen at run time.
 // ------------------------------------------------------------------------------------------
-size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps) {
+size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps, int qbins) {
     const int vf4 = 2;
+    if (qbins > 0)      // grid_kernel_qbins: region, O^2 bins, three landing buffers
+        return table_bytes + (size_t)(2 * g.RW * g.RH + 2 * qbins + 3 * (32 * 2 + 8)) * sizeof(float4) * warps;
     (void)mode;
     const size_t per_warp = (size_t)(2 * g.RW * g.RH + 2 * 36 * (vf4 + 1) + 32 * 2 + 8) * sizeof(float4);   // Geo::WARP_F4
     (void)tlog;
@@ -698,7 +870,17 @@ static grid_fn_t pick_shape(const ClassGeo &g, int tlog) {
 
 static int kernel_mode(const Plan &p) { return (p.mode == 0 && p.tmem_cols > 0) ? 3 : p.mode; }
 
-static grid_fn_t pick_grid(const ClassGeo &g, int tlog, int mode) {
+static grid_fn_t pick_qbins(int tlog) {
+    switch (tlog) {
+        case 2: return grid_kernel_qbins<2, kMaxWarpsFast>;
+        case 3: return grid_kernel_qbins<3, kMaxWarpsFast>;
+        case 4: return grid_kernel_qbins<4, kMaxWarpsFast>;
+        default: return nullptr;
+    }
+}
+
+static grid_fn_t pick_grid(const ClassGeo &g, int tlog, int mode, int qbins = 0) {
+    if (qbins > 0) return pick_qbins(tlog);
     switch (mode) {
         case 0: return pick_shape<0, kMaxWarpsFast>(g, tlog);
         case 3: return pick_shape<3, kMaxWarpsFast>(g, tlog);
@@ -742,12 +924,12 @@ cudaError_t configure_grid_kernel(Plan &p) {
         for (int w : kWarpChoices) {
             if (w > cap) continue;
             if (p.warps_forced > 0 && w > p.warps_forced) continue;      // the caller's limit (tuning, tests)
-            if (grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, w) <= (size_t)smem_max) { chosen = w; break; }
+            if (grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, w, p.qbins) <= (size_t)smem_max) { chosen = w; break; }
         }
         if (!chosen) return cudaErrorInvalidConfiguration;
         g.warps = chosen;
-        g.smem_bytes = (int)grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, chosen);
-        grid_fn_t fn = pick_grid(g, p.tlog, kernel_mode(p));
+        g.smem_bytes = (int)grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, chosen, p.qbins);
+        grid_fn_t fn = pick_grid(g, p.tlog, kernel_mode(p), p.qbins);
         if (!fn) return cudaErrorInvalidConfiguration;
         e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes);
         if (e != cudaSuccess) return e;
@@ -764,7 +946,7 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
     if (e != cudaSuccess) return e;
     for (int c = 0; c < p.n_cls; ++c) {
         const ClassGeo &g = p.cls[c];
-        grid_fn_t gfn = pick_grid(g, p.tlog, kernel_mode(p));
+        grid_fn_t gfn = pick_grid(g, p.tlog, kernel_mode(p), p.qbins);
         if (!gfn) return cudaErrorInvalidConfiguration;
         GridParams gp;
         gp.keys = p.keys[p.sorted_sel];

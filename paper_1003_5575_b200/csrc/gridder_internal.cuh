@@ -146,6 +146,7 @@ struct Plan {
     int32_t tlog, T, ntx, nty, n_tiles;
     int32_t chunk;                 // K
     int32_t merge;                 // GRIDDER_MERGE (default 1)
+    int32_t qbins;                 // > 0: fast path with per-origin bins (O^2 of them), grid_kernel_qbins
     int32_t fold_batches;          // longest FP32 register chain, in batches of 32 entries (power of 2)
     int32_t warps_forced, n_sm;
     int64_t max_items;             // capacity of the work-item table (all classes)
@@ -230,6 +231,6 @@ cudaError_t launch_scatter_atomic(Plan &p, const double *uvw, int n_time, int n_
 cudaError_t configure_grid_kernel(Plan &p);          // picks warps/smem per class, sets the smem attribute
 cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *grid, int accumulate,
                         cudaStream_t s);
-size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps);
+size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps, int qbins = 0);
 
 }  // namespace gridder

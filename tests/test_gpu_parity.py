@@ -377,3 +377,43 @@ def test_merging_of_equal_origin_and_offset_entries(dev):
     assert st_b.n_records_gridded == st_b.n_vis == n                 # unmerged: one record per entry (none dropped)
     assert st_b.fma_executed == n * 256 * 8
     assert st_a.n_records_gridded < n // 3 and st_a.fma_executed == st_a.n_records_gridded * 256 * 8
+
+
+# ------------------------------------------------------------------------------------ per-origin bins
+@pytest.mark.parametrize("S,O,N,n", [(16, 4, 96, 6000), (15, 8, 80, 5000), (12, 4, 66, 3000), (9, 2, 70, 3000)])
+def test_per_origin_bins_kernel_random(dev, S, O, N, n):
+    """grid_kernel_qbins (chosen by default only for dense plans) forced on the random cases."""
+    rng = np.random.default_rng(S * 1000 + N + 1)
+    table = rng.standard_normal((S * O, S * O)).astype(np.float32)
+    uvw, vis, w = _random_case(rng, n, N, S)
+    got, st = _run(dev, uvw, [C], vis, w, N=N, du=1.0, O=O, S=S, table=table, env={"GRIDDER_QBINS": 2})
+    got2, _ = _run(dev, uvw, [C], vis, w, N=N, du=1.0, O=O, S=S, table=table, env={"GRIDDER_QBINS": 2, "GRIDDER_WARPS": 4})
+    ref, ab, ost = _oracle(uvw, [C], vis, w, N=N, du=1.0, O=O, S=S, table=table)
+    assert st.n_dropped == ost["n_dropped"] > 0 and st.vis_taps == ost["vis_taps"]
+    assert np.array_equal(got, got2)
+    assert_parity(got, ref, ab, f"qbins S={S} O={O}")
+
+
+def test_per_origin_bins_kernel_dense_lattice_chunks_and_tiles(dev):
+    """Many visibilities on few lattice points (every bin of an origin fills, chunks of 256 split the hot
+    tiles, T = 4 and 8): the bins kernel against the oracle and against the ring kernel's record counts."""
+    rng = np.random.default_rng(92)
+    N, S, O, n = 64, 16, 4, 30_000
+    table = synth.spheroidal_table(S, O)
+    uvw = np.zeros((1, n, 3))
+    uvw[0, :, :2] = rng.integers(-24, 25, (n, 2)) / 8.0              # 49 x 49 points on the 1/8 lattice (ties too)
+    vis = (rng.standard_normal((n, 4, 2)) + 1.0).astype(np.float32)
+    w = rng.uniform(0.5, 1.5, n).astype(np.float32)
+    kw = dict(N=N, du=1.0, O=O, S=S, table=table)
+    ref, ab, _ = _oracle(uvw, [C], vis, w, **kw)
+    for tlog in (2, 3):
+        env = {"GRIDDER_QBINS": 2, "GRIDDER_CHUNK": 256, "GRIDDER_TILE_LOG2": tlog}
+        a, st_a = _run(dev, uvw, [C], vis, w, env=env, **kw)
+        a2, _ = _run(dev, uvw, [C], vis, w, env=env, **kw)
+        b, st_b = _run(dev, uvw, [C], vis, w, env=dict(env, GRIDDER_QBINS=0), **kw)
+        assert np.array_equal(a, a2)
+        assert_parity(a, ref, ab, f"qbins dense T={1 << tlog}")
+        assert_parity(b, ref, ab, f"ring kernel dense T={1 << tlog}")
+        assert st_a.n_work_items == st_b.n_work_items and st_a.max_tile_load > 256
+        assert 0 < st_a.n_records_gridded <= st_b.n_records_gridded < n        # bins merge at least as much
+        assert st_a.fma_executed == st_a.n_records_gridded * 256 * 8
