@@ -169,15 +169,15 @@ __device__ __forceinline__ Entry load_entry(const GridParams &p, unsigned e, boo
     return k;
 }
 
-// Starts the copies of one batch: lane's visibility goes to raw[2 lane .. 2 lane + 1], its weight to
+// Starts the copies of one batch: lane's visibility goes to raw[lane] and raw[32 + lane], its weight to
 // the float array behind.  A lane past the end of the batch, or a dropped visibility, gets zeros.
 template <bool GEN>
 __device__ __forceinline__ void issue_vis(const GridParams &p, float4 *raw, int lane, const Entry k, bool valid) {
     const bool dropped = GEN ? ((k.aux >> 30) & 1u) : ((k.key >> (2 * p.key.bits_q)) & 1u);
     const bool live = valid && !dropped;
     const float4 *src = p.vis + 2 * (size_t)(live ? k.idx : 0u);
-    cp_async_16(raw + 2 * lane, src, live);
-    cp_async_16(raw + 2 * lane + 1, src + 1, live);
+    cp_async_16(raw + lane, src, live);                // two planes of 32 float4: conflict-free to read back
+    cp_async_16(raw + 32 + lane, src + 1, live);
     if (p.weight) cp_async_4(reinterpret_cast<float *>(raw + 64) + lane, p.weight + (live ? k.idx : 0u), live);
     cp_async_commit();
 }
@@ -218,7 +218,7 @@ __device__ __forceinline__ int stage_write(const GridParams &p, const float4 *ra
     }
     const int poff = (int)(y0l * G::RW + x0l);
     const bool valid = lane < cnt;
-    const float4 ra = raw[2 * lane], rb = raw[2 * lane + 1];
+    const float4 ra = raw[lane], rb = raw[32 + lane];
     const float w = p.weight ? reinterpret_cast<const float *>(raw + 64)[lane] : 1.0f;
     const float o[8] = {ra.x * w, ra.y * w, ra.z * w, ra.w * w, rb.x * w, rb.y * w, rb.z * w, rb.w * w};
     float sum[8];
@@ -283,6 +283,15 @@ struct RecRegs {
     __device__ __forceinline__ void fetch(const float4 *slot, int coff, const char *coef_lane) {
 #pragma unroll
         for (int i = 0; i < VF4; ++i) v[i] = slot[i];
+        fetch_taps(coff, coef_lane);
+    }
+    // the two halves of the weighted visibility from two places (the per-origin bins are kept as planes)
+    __device__ __forceinline__ void fetch2(const float4 *lo, const float4 *hi, int coff, const char *coef_lane) {
+        v[0] = *lo;
+        v[1] = *hi;
+        fetch_taps(coff, coef_lane);
+    }
+    __device__ __forceinline__ void fetch_taps(int coff, const char *coef_lane) {
         if (MODE == 2) {
             sgn = (uint32_t)coff << 31;
             coff &= ~1;
@@ -607,7 +616,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel_qbins(const GridPara
     const int warp_f4 = 2 * G::CELLS + 2 * n_q + NRAW * G::RAW_F4;
     float4 *region = smem + p.coef_f4 + warp * warp_f4;        // plane A (XX, XY) then plane B (YX, YY)
     float4 *regA = region, *regB = region + G::CELLS;
-    float4 *bins = region + 2 * G::CELLS;                      // [q][2] float4: sum of w V of the current origin
+    float4 *bins = region + 2 * G::CELLS;                      // [2][q] float4: sum of w V of the current origin
     float4 *raw = bins + 2 * n_q;                              // NRAW cp.async landing buffers
 
     for (int i = threadIdx.x; i < p.coef_f4; i += blockDim.x) smem[i] = p.coef[i];
@@ -663,26 +672,48 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel_qbins(const GridPara
             const bool valid = lane < cnt;
             const int poff = valid ? (int)(y0l * G::RW + x0l) : kForce;
             const int q = (int)(e0.key & qmask);
-            const float4 ra = rw[2 * lane], rb = rw[2 * lane + 1];
+            const float4 ra = rw[lane], rb = rw[32 + lane];
             const float w = p.weight ? reinterpret_cast<const float *>(rw + 64)[lane] : 1.0f;
             const float o[8] = {ra.x * w, ra.y * w, ra.z * w, ra.w * w, rb.x * w, rb.y * w, rb.z * w, rb.w * w};
             float sum[8];
 #pragma unroll
             for (int k = 0; k < 8; ++k) sum[k] = o[k];
-            // groups of equal (origin, offset) inside the batch: the first lane adds the others
+            // Sum inside the batch.  Neighbouring channels of a baseline are neighbours in the sorted list and
+            // mostly share (origin, offset): first a segmented tree reduction over RUNS of equal lanes (five
+            // shuffle steps whatever the run lengths), then the heads of runs with equal (origin, offset) --
+            // rare -- are added into the first of them one by one.  Fixed order, so reruns are bit-identical.
             const unsigned gkey = valid ? (((unsigned)poff << 8) | (unsigned)q) : (0xFFFF0000u | lane);
-            const unsigned grp = __match_any_sync(0xffffffffu, gkey);
-            const bool keep = valid && (__ffs(grp) - 1 == lane);
-            unsigned rest = keep ? (grp & ~(1u << lane)) : 0u;
-            while (__any_sync(0xffffffffu, rest != 0u)) {
-                const int src = rest ? __ffs(rest) - 1 : lane;
-                const bool add = rest != 0u;
-                rest &= rest - 1u;
+            const unsigned gprev = __shfl_up_sync(0xffffffffu, gkey, 1);
+            const bool head = lane == 0 || gprev != gkey;
+            const unsigned heads = __ballot_sync(0xffffffffu, head);
+            const unsigned above = lane == 31 ? 0u : (heads & (0xFFFFFFFEu << lane));
+            const int run_end = above ? __ffs(above) - 1 : 32;         // first lane of the next run
+#pragma unroll
+            for (int dlt = 1; dlt < 32; dlt <<= 1) {
+                const bool add = lane + dlt < run_end;
 #pragma unroll
                 for (int k = 0; k < 8; ++k) {
-                    const float t = __shfl_sync(0xffffffffu, o[k], src);
+                    const float t = __shfl_down_sync(0xffffffffu, sum[k], dlt);
                     if (add) sum[k] += t;
                 }
+            }
+            const unsigned grp = __match_any_sync(0xffffffffu, head ? gkey : (0xFFFF0000u | lane));
+            const bool keep = valid && head && (__ffs(grp) - 1 == lane);
+            unsigned rest = keep ? (grp & ~(1u << lane)) : 0u;
+            if (__any_sync(0xffffffffu, rest != 0u)) {
+                float hs[8];                                           // the run sums as the heads hold them now
+#pragma unroll
+                for (int k = 0; k < 8; ++k) hs[k] = sum[k];
+                do {
+                    const int src = rest ? __ffs(rest) - 1 : lane;
+                    const bool add = rest != 0u;
+                    rest &= rest - 1u;
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) {
+                        const float t = __shfl_sync(0xffffffffu, hs[k], src);
+                        if (add) sum[k] += t;
+                    }
+                } while (__any_sync(0xffffffffu, rest != 0u));
             }
             // origin by origin (the batch is sorted by origin); one more round with no origin ends the item
             int lp = 0;
@@ -696,16 +727,16 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel_qbins(const GridPara
                         unsigned long long m = occ;
                         int qa = __ffsll((long long)m) - 1, qb;
                         m &= m - 1ull;
-                        A.fetch(bins + 2 * qa, qa * G::SUB_BYTES, coef_lane);
+                        A.fetch2(bins + qa, bins + n_q + qa, qa * G::SUB_BYTES, coef_lane);
                         while (true) {
                             qb = m ? __ffsll((long long)m) - 1 : -1;
                             m &= m - 1ull;
-                            if (qb >= 0) B.fetch(bins + 2 * qb, qb * G::SUB_BYTES, coef_lane);
+                            if (qb >= 0) B.fetch2(bins + qb, bins + n_q + qb, qb * G::SUB_BYTES, coef_lane);
                             consume<NA, NB, G::RW, 0>(A, bin_org, cur, cmp, regA, regB, lane_cell, acc);
                             if (qb < 0) break;
                             qa = m ? __ffsll((long long)m) - 1 : -1;
                             m &= m - 1ull;
-                            if (qa >= 0) A.fetch(bins + 2 * qa, qa * G::SUB_BYTES, coef_lane);
+                            if (qa >= 0) A.fetch2(bins + qa, bins + n_q + qa, qa * G::SUB_BYTES, coef_lane);
                             consume<NA, NB, G::RW, 0>(B, bin_org, cur, cmp, regA, regB, lane_cell, acc);
                             if (qa < 0) break;
                         }
@@ -722,10 +753,10 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel_qbins(const GridPara
                 const bool in_seg = poff == seg;
                 const bool put = in_seg && keep;
                 if (put) {               // the kept lanes of one origin have distinct offsets
-                    float4 x = bins[2 * q], y = bins[2 * q + 1];
+                    float4 x = bins[q], y = bins[n_q + q];
                     x.x += sum[0]; x.y += sum[1]; x.z += sum[2]; x.w += sum[3];
                     y.x += sum[4]; y.y += sum[5]; y.z += sum[6]; y.w += sum[7];
-                    bins[2 * q] = x; bins[2 * q + 1] = y;
+                    bins[q] = x; bins[n_q + q] = y;
                 }
                 const unsigned lo = __reduce_or_sync(0xffffffffu, (put && q < 32) ? (1u << q) : 0u);
                 const unsigned hi = __reduce_or_sync(0xffffffffu, (put && q >= 32) ? (1u << (q - 32)) : 0u);
