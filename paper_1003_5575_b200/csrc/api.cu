@@ -153,6 +153,15 @@ int derive(const gridder_config *cfg, Plan &p) {
     p.max_items = occ + n / p.chunk + 1;
     // each class has its own partial-region array, sized for the case that every entry is of that class
     p.max_items_cls = (n < p.n_tiles ? n : p.n_tiles) + n / p.chunk + 1;
+    // GRIDDER_REDUCE (with the bins): 1 (default) a separate kernel sums the entries into records
+    // (reduce.cu) and the grid kernel runs on those; 0: one kernel does both (grid_kernel_qbins)
+    p.reduce = 0; p.rec_cap = 0; p.rec_slot = 0;
+    if (p.qbins > 0 && p.qbins <= 16 && env_int("GRIDDER_REDUCE", 1)) {
+        const int64_t per_item = (int64_t)p.T * p.T * p.qbins;          // (origin, offset) pairs of a tile
+        p.rec_slot = p.max_items * per_item <= n ? per_item : 0;
+        p.rec_cap = p.rec_slot ? p.max_items * per_item : n;
+        if (p.rec_cap < (1ll << 32)) p.reduce = 1;
+    }
     p.partials_f4 = 0;
     for (int c = 0; c < p.n_cls; ++c) {
         p.cls[c].part_off_f4 = p.partials_f4;
@@ -205,6 +214,11 @@ cudaError_t carve(Plan &p, char *base) {
     p.tile_cover = (unsigned char *)take((size_t)p.n_tiles);
     p.items = (WorkItem *)take(sizeof(WorkItem) * (size_t)p.max_items);
     p.partials = (float4 *)take(sizeof(float4) * (size_t)p.partials_f4);
+    if (p.reduce) {
+        p.rec_key = (uint32_t *)take(sizeof(uint32_t) * (size_t)p.rec_cap);
+        p.rec_sum = (float4 *)take(sizeof(float4) * 2 * (size_t)p.rec_cap);
+        p.rec_items = (WorkItem *)take(sizeof(WorkItem) * (size_t)p.max_items);
+    }
     p.coef = (float4 *)take(p.coef_bytes);
     p.counters = (Counters *)take(sizeof(Counters));
     p.workspace_needed = off;

@@ -163,7 +163,7 @@ __device__ __forceinline__ Entry load_entry(const GridParams &p, unsigned e, boo
             k.idx = v.x;
             k.aux = v.y;
         } else {
-            k.idx = __ldg(reinterpret_cast<const uint32_t *>(p.vals) + e);
+            k.idx = p.vals ? __ldg(reinterpret_cast<const uint32_t *>(p.vals) + e) : e;     // null: records, in place
         }
     }
     return k;
@@ -784,6 +784,231 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel_qbins(const GridPara
 }
 
 // ------------------------------------------------------------------------------------------
+// PRE-SUMMATION of a dense plan's entries (fast path, O^2 <= 16 sub-cell offsets).
+// When a tile holds many more entries than it has (origin, offset) pairs -- T^2 O^2 = 256 at
+// T = O = 4 -- it pays to add the weighted visibilities of every pair first (8 FMAs per entry) and to
+// grid each non-empty pair once (2048 FMAs): sum_i C_q w_i V_i = C_q sum_i w_i V_i, exact by
+// linearity like the per-batch merging of stage_write, of which this is the complete form.  This
+// kernel does the adding: per work item it writes RECORDS (origin | offset, sum of w V), origin by
+// origin; grid_kernel then runs on the records exactly as it runs on entries (keys = record keys,
+// visibilities = record sums, no weights, nothing left to merge).  BASELINE.json config 4: 16.5
+// entries per record.
+//
+// A warp walks its items' entries 32 at a time (same queue and batch stream as the grid kernel; the
+// visibilities of three batches are landing in shared memory by cp.async while one is added).  Entries of one origin are consecutive.
+// Every LANE keeps private bins for the O^2 offsets of the current origin in shared memory
+// ([offset][half][lane] float4: conflict-free whatever the offsets are) and adds its entry to its own
+// bin: no two lanes ever touch the same word, so there is nothing to match, merge or serialise.
+// When the origin changes (or after 64 batches, which bounds the FP32 chain of a bin) the 32 private
+// copies of each touched bin are added in a fixed order -- 8 serial additions in each of four lane
+// groups, then a butterfly -- into registers, and at the end of the origin the non-empty bins are
+// written out as records in offset order.  All orders are fixed: reruns are bit-identical.
+// ------------------------------------------------------------------------------------------
+constexpr int kRedWarps = 10, kRedPiece = 64;
+constexpr int kRedBins = 16;                                   // O^2 <= 16
+constexpr int kRedVis = 4, kRedVisF4 = 32 * 2 + 8;             // landing ring of the visibilities (a, b, weight)
+constexpr int kRedKey = 8, kRedKeyF4 = 16;                     // ring of the sorted pairs: 32 keys, 32 indices
+constexpr int kRedWarpF4 = kRedBins * 2 * 32 + kRedVis * kRedVisF4 + kRedKey * kRedKeyF4 + kRedKey;
+
+__global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridParams p) {
+    extern __shared__ float4 smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float4 *priv = smem + (size_t)warp * kRedWarpF4;           // [q][half][lane]
+    float4 *vring = priv + kRedBins * 2 * 32;                  // kRedVis x {a[32], b[32], w[32]}
+    uint32_t *kring = reinterpret_cast<uint32_t *>(vring + kRedVis * kRedVisF4);   // kRedKey x {key[32], idx[32]}
+    uint4 *dring = reinterpret_cast<uint4 *>(kring + kRedKey * 64);                 // kRedKey batch descriptors
+    for (int i = lane; i < kRedWarpF4; i += 32) priv[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncwarp();
+
+    const int tl2 = 2 * p.key.tlog;
+    const uint32_t omask = (1u << tl2) - 1u, qmask = (1u << (2 * p.key.bits_q)) - 1u;
+    const uint32_t dropbit = 1u << (2 * p.key.bits_q);
+    const unsigned item_begin = p.counters->cls_begin[p.cls], item_end = p.counters->cls_end[p.cls];
+    const uint32_t *idx_sorted = reinterpret_cast<const uint32_t *>(p.vals);
+    // the lane's part in adding the private copies: bin 4 pass + bs, half h, source lanes 8 g .. 8 g + 7
+    const int g = lane & 3, h = (lane >> 2) & 1, bs = lane >> 3;
+
+    float4 bacc[4];                      // sums of the bins 4 pass + bs (half h) over the pieces of the origin
+#pragma unroll
+    for (int i = 0; i < 4; ++i) bacc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    unsigned touched = 0;                // this lane's private bins that hold something
+    unsigned occ = 0;                    // bins of the origin that hold something (all pieces)
+    int bin_org = -1, piece = 0;
+    unsigned n_rec = 0;
+    size_t rec_base = 0;
+
+    // ---- the warp's stream of batches: <= 32 consecutive entries of one work item ---------------------
+    // descriptor: x = first entry, y = count | first batch of its item << 8 | last << 9 | end of stream << 10,
+    // z = item (relative to the class)
+    unsigned cur_id = 0, cur_start = 0, cur_len = 0, cur_off = 0;      // the item the batches are cut from
+    unsigned nxt_id = 0, nxt_start = 0, nxt_len = 0;                   // claimed one item ahead
+    bool nxt_ok = false, gen_end = false;
+    auto claim = [&]() {
+        unsigned it = 0;
+        if (lane == 0) it = atomicAdd(&p.counters->queue_head[p.cls], 1u);
+        nxt_id = __shfl_sync(0xffffffffu, it, 0);
+        nxt_ok = item_begin + nxt_id < item_end;
+        nxt_start = nxt_len = 0;
+        if (nxt_ok) {
+            const WorkItem w = p.items[item_begin + nxt_id];
+            nxt_start = w.start;
+            nxt_len = w.len;
+        }
+    };
+    // batch m: its descriptor into the ring, the copies of its sorted pairs started
+    auto gen_batch = [&](int m) {
+        if (!gen_end && cur_off >= cur_len) {
+            if (!nxt_ok) gen_end = true;
+            else {
+                cur_id = nxt_id; cur_start = nxt_start; cur_len = nxt_len; cur_off = 0;
+                claim();
+            }
+        }
+        uint4 d = make_uint4(0u, 1u << 10, 0u, 0u);
+        if (!gen_end) {
+            const unsigned left = cur_len - cur_off;
+            d.x = cur_start + cur_off;
+            d.y = min(32u, left) | (cur_off == 0u ? 256u : 0u) | (left <= 32u ? 512u : 0u);
+            d.z = cur_id;
+            cur_off += 32u;
+        }
+        const int ks = m & (kRedKey - 1);
+        if (lane == 0) dring[ks] = d;
+        const bool v = lane < (int)(d.y & 63u);
+        cp_async_4(kring + ks * 64 + lane, p.keys + d.x + lane, v);
+        cp_async_4(kring + ks * 64 + 32 + lane, idx_sorted + d.x + lane, v);
+    };
+    // batch m (its pairs have landed): the copies of its visibilities started
+    auto gen_vis = [&](int m) {
+        const int ks = m & (kRedKey - 1);
+        const uint4 d = dring[ks];
+        const uint32_t key = kring[ks * 64 + lane], idx = kring[ks * 64 + 32 + lane];
+        const bool live = lane < (int)(d.y & 63u) && !(key & dropbit);
+        float4 *dst = vring + (m & (kRedVis - 1)) * kRedVisF4;
+        const float4 *src = p.vis + 2 * (size_t)(live ? idx : 0u);
+        cp_async_16(dst + lane, src, live);
+        cp_async_16(dst + 32 + lane, src + 1, live);
+        if (p.weight) cp_async_4(reinterpret_cast<float *>(dst + 64) + lane, p.weight + (live ? idx : 0u), live);
+    };
+
+    claim();
+    // prologue: batches 0..5 have their pairs moving, then 0..2 their visibilities
+    for (int m = 0; m < 6; ++m) {
+        gen_batch(m);
+        cp_async_commit();
+    }
+    asm volatile("cp.async.wait_group 3;" ::: "memory");          // pairs of batches 0..2
+    __syncwarp();
+    for (int m = 0; m < 3; ++m) {
+        gen_vis(m);
+        cp_async_commit();
+    }
+
+    // iteration n: pairs of batch n+6 and visibilities of batch n+3 start to move (one group), batch n is added
+#pragma unroll 1
+    for (int n = 0;; ++n) {
+        asm volatile("cp.async.wait_group 2;" ::: "memory");      // groups up to iteration n-3: pairs(n+3), vis(n)
+        __syncwarp();
+        gen_batch(n + 6);
+        gen_vis(n + 3);
+        cp_async_commit();
+        const uint4 d = dring[n & (kRedKey - 1)];
+        if (d.y & 1024u) break;
+        const int cnt = (int)(d.y & 63u);
+        {
+            const float4 *rw = vring + (n & (kRedVis - 1)) * kRedVisF4;
+            if (d.y & 256u) {            // first batch of an item: where its records go
+                n_rec = 0;
+                rec_base = p.rec_slot ? (size_t)d.z * p.rec_slot : (size_t)d.x;
+            }
+            const uint32_t key = kring[(n & (kRedKey - 1)) * 64 + lane];
+            const bool valid = lane < cnt;
+            const int org = valid ? (int)((key >> p.key.aux_bits) & omask) : -2;
+            const int q = (int)(key & qmask);
+            const float w = p.weight ? reinterpret_cast<const float *>(rw + 64)[lane] : 1.0f;
+            const float4 a = rw[lane], b = rw[32 + lane];
+            const bool last = d.y & 512u;
+            int lp = 0;
+            // origin by origin; one more round with no origin ends the item
+#pragma unroll 1
+            while (lp < cnt || (last && lp == cnt)) {
+                const int seg = lp < cnt ? __shfl_sync(0xffffffffu, org, lp) : -1;
+                const bool change = seg != bin_org;
+                if ((change && bin_org >= 0) || piece >= kRedPiece) {
+                    // ---- the 32 private copies of every touched bin are added into bacc and cleared --------
+                    __syncwarp();
+                    const unsigned u = __reduce_or_sync(0xffffffffu, touched);
+                    occ |= u;
+#pragma unroll
+                    for (int pass = 0; pass < 4; ++pass) {
+                        if (((u >> (4 * pass)) & 15u) == 0u) continue;
+                        const float4 *src = priv + ((4 * pass + bs) * 2 + h) * 32 + 8 * g;
+                        float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            const float4 v = src[(j + lane) & 7];
+                            t.x += v.x; t.y += v.y; t.z += v.z; t.w += v.w;
+                        }
+#pragma unroll
+                        for (int dd = 1; dd < 4; dd <<= 1) {
+                            t.x += __shfl_xor_sync(0xffffffffu, t.x, dd); t.y += __shfl_xor_sync(0xffffffffu, t.y, dd);
+                            t.z += __shfl_xor_sync(0xffffffffu, t.z, dd); t.w += __shfl_xor_sync(0xffffffffu, t.w, dd);
+                        }
+                        bacc[pass].x += t.x; bacc[pass].y += t.y; bacc[pass].z += t.z; bacc[pass].w += t.w;
+                    }
+                    __syncwarp();
+                    for (unsigned m = touched; m; m &= m - 1u) {
+                        const int qq = __ffs(m) - 1;
+                        priv[(qq * 2) * 32 + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        priv[(qq * 2 + 1) * 32 + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+                    touched = 0;
+                    piece = 0;
+                    __syncwarp();
+                    if (change) {
+                        // ---- the origin is complete: its non-empty bins become records, in offset order ----
+#pragma unroll
+                        for (int pass = 0; pass < 4; ++pass) {
+                            const int qq = 4 * pass + bs;
+                            if (g == 0 && ((occ >> qq) & 1u)) {
+                                const size_t r = rec_base + n_rec + (unsigned)__popc(occ & ((1u << qq) - 1u));
+                                p.rec_sum[2 * r + h] = bacc[pass];
+                                if (h == 0) p.rec_key[r] = ((uint32_t)bin_org << p.key.aux_bits) | (uint32_t)qq;
+                            }
+                            bacc[pass] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        }
+                        n_rec += (unsigned)__popc(occ);
+                        occ = 0;
+                    }
+                }
+                bin_org = seg;
+                if (lp >= cnt) break;
+                const bool in_seg = org == seg;
+                if (in_seg) {
+                    float4 *pa = priv + (q * 2) * 32 + lane, *pb = pa + 32;
+                    float4 x = *pa, y = *pb;
+                    x.x = fmaf(w, a.x, x.x); x.y = fmaf(w, a.y, x.y); x.z = fmaf(w, a.z, x.z); x.w = fmaf(w, a.w, x.w);
+                    y.x = fmaf(w, b.x, y.x); y.y = fmaf(w, b.y, y.y); y.z = fmaf(w, b.z, y.z); y.w = fmaf(w, b.w, y.w);
+                    *pa = x; *pb = y;
+                    touched |= 1u << q;
+                }
+                ++piece;
+                lp += __popc(__ballot_sync(0xffffffffu, in_seg));
+            }
+            if (last && lane == 0) {     // the item's entry in the record items
+                WorkItem ri;
+                ri.start = (uint32_t)rec_base;
+                ri.len = n_rec;
+                ri.tile = 0;
+                ri.pad = 0;
+                p.rec_items[item_begin + d.z] = ri;
+            }
+        }
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+}
+
+// ------------------------------------------------------------------------------------------
 // Flush: one thread per grid cell.  The partial regions covering cell (x, y) belong to the tiles
 // (ty, tx) with tx*T <= x < tx*T + RW (same in y); each tile's work items are added in id order
 // (full chunks, then the tail).  FP64 accumulation, one rounding to FP32 at the end.  One launch
@@ -899,6 +1124,7 @@ static grid_fn_t pick_shape(const ClassGeo &g, int tlog) {
     return nullptr;
 }
 
+static int kernel_qbins(const Plan &p) { return p.reduce ? 0 : p.qbins; }      // the kernel with its own bins
 static int kernel_mode(const Plan &p) { return (p.mode == 0 && p.tmem_cols > 0) ? 3 : p.mode; }
 
 static grid_fn_t pick_qbins(int tlog) {
@@ -955,14 +1181,19 @@ cudaError_t configure_grid_kernel(Plan &p) {
         for (int w : kWarpChoices) {
             if (w > cap) continue;
             if (p.warps_forced > 0 && w > p.warps_forced) continue;      // the caller's limit (tuning, tests)
-            if (grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, w, p.qbins) <= (size_t)smem_max) { chosen = w; break; }
+            if (grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, w, kernel_qbins(p)) <= (size_t)smem_max) { chosen = w; break; }
         }
         if (!chosen) return cudaErrorInvalidConfiguration;
         g.warps = chosen;
-        g.smem_bytes = (int)grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, chosen, p.qbins);
-        grid_fn_t fn = pick_grid(g, p.tlog, kernel_mode(p), p.qbins);
+        g.smem_bytes = (int)grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, chosen, kernel_qbins(p));
+        grid_fn_t fn = pick_grid(g, p.tlog, kernel_mode(p), kernel_qbins(p));
         if (!fn) return cudaErrorInvalidConfiguration;
         e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes);
+        if (e != cudaSuccess) return e;
+    }
+    if (p.reduce) {
+        e = cudaFuncSetAttribute((const void *)reduce_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)(kRedWarps * kRedWarpF4 * sizeof(float4)));
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
@@ -975,9 +1206,30 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
     cudaError_t e = cudaMemsetAsync(p.counters->queue_head, 0, sizeof(unsigned int) * kMaxClasses, s);
     if (e == cudaSuccess) e = cudaMemsetAsync(p.counters->n_exec, 0, sizeof(unsigned long long) * kMaxClasses, s);
     if (e != cudaSuccess) return e;
+    if (p.reduce) {                  // sum the entries into records first; the grid kernel then takes those
+        GridParams rp;
+        memset(&rp, 0, sizeof(rp));
+        rp.keys = p.keys[p.sorted_sel];
+        rp.vals = p.vals[p.sorted_sel];
+        rp.items = p.items;
+        rp.counters = p.counters;
+        rp.vis = reinterpret_cast<const float4 *>(vis);
+        rp.weight = weight;
+        rp.key = p.key;
+        rp.cls = 0;
+        rp.rec_key = p.rec_key;
+        rp.rec_sum = p.rec_sum;
+        rp.rec_items = p.rec_items;
+        rp.rec_slot = (uint32_t)p.rec_slot;
+        reduce_kernel<<<p.n_sm, kRedWarps * 32, kRedWarps * kRedWarpF4 * sizeof(float4), s>>>(rp);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaMemsetAsync(p.counters->queue_head, 0, sizeof(unsigned int) * kMaxClasses, s);
+        if (e != cudaSuccess) return e;
+        p.n_launches += 1;
+    }
     for (int c = 0; c < p.n_cls; ++c) {
         const ClassGeo &g = p.cls[c];
-        grid_fn_t gfn = pick_grid(g, p.tlog, kernel_mode(p), p.qbins);
+        grid_fn_t gfn = pick_grid(g, p.tlog, kernel_mode(p), kernel_qbins(p));
         if (!gfn) return cudaErrorInvalidConfiguration;
         GridParams gp;
         gp.keys = p.keys[p.sorted_sel];
@@ -996,6 +1248,15 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         gp.tmem_cols = p.tmem_cols;
         gp.merge = p.merge;
         gp.n_q = p.cfg.oversample * p.cfg.oversample;
+        if (p.reduce) {              // the entries were summed into records: grid those, as they are
+            gp.keys = p.rec_key;
+            gp.vals = nullptr;
+            gp.items = p.rec_items;
+            gp.vis = p.rec_sum;
+            gp.weight = nullptr;
+            gp.merge = 0;
+            if (gp.fold_mask > 3) gp.fold_mask = 3;      // a record is a sum already: shorter register chains
+        }
         gfn<<<p.n_sm, g.warps * 32, g.smem_bytes, s>>>(gp);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;

@@ -119,6 +119,11 @@ struct GridParams {
     int32_t n_q;                   // O^2 sub-tables
     int32_t merge;                 // sum entries of a batch with equal origin and table offset before gridding
     KeyLayout key;
+    // reduce_kernel only: the records it writes (the grid kernel then reads them as keys / vis / items)
+    uint32_t *rec_key;             // [record]
+    float4 *rec_sum;               // [record][2]
+    WorkItem *rec_items;           // [item]
+    uint32_t rec_slot;             // > 0: item i owns records [i rec_slot, (i + 1) rec_slot); 0: [start, start + len)
 };
 
 struct FlushParams {
@@ -147,6 +152,12 @@ struct Plan {
     int32_t chunk;                 // K
     int32_t merge;                 // GRIDDER_MERGE (default 1)
     int32_t qbins;                 // > 0: fast path with per-origin bins (O^2 of them), grid_kernel_qbins
+    int32_t reduce;                // with qbins: the bins are filled by reduce_kernel (reduce.cu), which writes records
+    int64_t rec_cap;               // records the arrays below hold
+    int64_t rec_slot;              // > 0: records per work item (item i owns [i rec_slot, (i+1) rec_slot)); 0: item.start
+    uint32_t *rec_key;             // [rec_cap]
+    float4 *rec_sum;               // [rec_cap][2]
+    WorkItem *rec_items;           // [max_items]: the work items over the record arrays
     int32_t fold_batches;          // longest FP32 register chain, in batches of 32 entries (power of 2)
     int32_t warps_forced, n_sm;
     int64_t max_items;             // capacity of the work-item table (all classes)
