@@ -39,8 +39,12 @@ BAND_HZ = 768 * 40.0e3           # one rank's band; rank r starts at 140 MHz + r
 # dram__bytes_read.sum + dram__bytes_write.sum of one grid_kernel launch from the committed
 # `ncu --set full` capture (profiles/), keyed by config; None until a capture exists for it.
 NCU_GRID_KERNEL_TRAFFIC_BYTES = {
-    4: 53_910_878_000,    # profiles/r01d_grid_kernel_config4_ncu_full.csv: 47.291082 GB read + 6.619796 GB written
+    4: 7_679_000_000,     # profiles/r01f: grid_kernel on the records of config 4: 1.820 GB read + 5.859 GB written
     2: 9_348_989_000,     # profiles/r01_grid_kernel_config2_ncu_full.csv: 4.109023 GB read + 5.239966 GB written
+}
+# the same for reduce_kernel (dense plans: it is the longest kernel of the step there)
+NCU_REDUCE_KERNEL_TRAFFIC_BYTES = {
+    4: 42_588_000_000,    # profiles/r01f_reduce_kernel_config4_ncu_full.csv: 40.829 GB read + 1.759 GB written
 }
 
 
@@ -415,6 +419,25 @@ def run_ours(args) -> dict | None:
                 "peak_gbs": peaks.get("hbm_gbs", 6650.0),
                 "peak_source": "MEASURED_PEAKS.json" if "hbm_gbs" in peaks else "fallback (B200_PROFILING.md)"},
     }
+    reduce_ms = stage.get("reduce", 0.0)
+    if reduce_ms > grid_ms:
+        # Dense plan: the pre-summation (reduce_kernel) is the longest kernel.  It streams every sorted
+        # (key, index) pair, gathers the visibility (and weight) it names, and writes the records:
+        # HBM-bound.  Algorithmic bytes per launch: 8 + 32 (+ 4) per entry, 36 per record.
+        red_bytes = st.n_entries * (8 + 32 + (4 if weight is not None else 0)) + st_exec.n_records_gridded * 36
+        gbs = red_bytes / (reduce_ms * 1e-3) / 1e9
+        hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+        roofline = {
+            "bound": "hbm", "kernel": "reduce_kernel", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
+            "frac": gbs / hbm_peak, "traffic": NCU_REDUCE_KERNEL_TRAFFIC_BYTES.get(args.config),
+            "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy bandwidth)" if "hbm_gbs" in peaks
+                           else "fallback (B200_PROFILING.md)",
+            "kernel_ms": reduce_ms, "kernel_share_of_step": reduce_ms / agg["ms_per_step"] if agg["ms_per_step"] else None,
+            "bytes_per_launch": int(red_bytes), "entries": st.n_entries, "records": st_exec.n_records_gridded,
+            "merge_factor": roofline["merge_factor"],
+            "grid_kernel": roofline,              # the second kernel of the stage, on the records: FP32-FMA bound
+            "hbm": roofline["hbm"],
+        }
     out = {
         "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": agg["ms_per_step"], "higher_is_better": True,
@@ -427,7 +450,7 @@ def run_ours(args) -> dict | None:
                    "tile": st.tile_size, "chunk": st.chunk_size, "work_items": st.n_work_items,
                    "grid_warps_per_sm": st.grid_warps_per_sm},
         "gflops": flop_per_tap * agg["value"] / 1e9,
-        "stage_ms": stage, "grid_only_ms": stage["grid"] + stage["flush"],     # gridder_grid alone (a bin serves many)
+        "stage_ms": stage, "grid_only_ms": stage["grid"] + stage["flush"] + stage.get("reduce", 0.0),     # gridder_grid alone (a bin serves many)
         "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
         "cadence_budget_s": 8.0, "result_checksum": checksum,
     }

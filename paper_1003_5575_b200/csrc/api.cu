@@ -317,7 +317,7 @@ int gridder_destroy(gridder_plan_t *plan) {
     image_destroy(*p);
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
     for (int r = 0; r < kProfRing; ++r)
-        for (int i = 0; i < 7; ++i) if (p->ev[r][i]) cudaEventDestroy(p->ev[r][i]);
+        for (int i = 0; i < 8; ++i) if (p->ev[r][i]) cudaEventDestroy(p->ev[r][i]);
     delete p;
     return e == cudaSuccess ? GRIDDER_OK : GRIDDER_ERR_CUDA;
 }
@@ -478,7 +478,7 @@ int gridder_set_profiling(gridder_plan_t *plan, int32_t enable) {
     if (!p) return GRIDDER_ERR_INVALID_ARG;
     if (enable && !p->ev[0][0]) {
         for (int r = 0; r < kProfRing; ++r)
-            for (int i = 0; i < 7; ++i)
+            for (int i = 0; i < 8; ++i)
                 if (cudaEventCreate(&p->ev[r][i]) != cudaSuccess) return cuda_fail(p, cudaGetLastError());
     }
     p->profiling = enable != 0;
@@ -489,7 +489,7 @@ int gridder_set_profiling(gridder_plan_t *plan, int32_t enable) {
 int gridder_get_stage_ms(gridder_plan_t *plan, float *ms_out) {
     Plan *p = reinterpret_cast<Plan *>(plan);
     if (!p || !ms_out) return GRIDDER_ERR_INVALID_ARG;
-    double sum[5] = {0, 0, 0, 0, 0};
+    double sum[6] = {0, 0, 0, 0, 0, 0};
     const int nb = (int)(p->prof_bin_calls < kProfRing ? p->prof_bin_calls : kProfRing);
     const int ng = (int)(p->prof_grid_calls < kProfRing ? p->prof_grid_calls : kProfRing);
     cudaError_t e = cudaSuccess;
@@ -508,10 +508,16 @@ int gridder_get_stage_ms(gridder_plan_t *plan, float *ms_out) {
             e = cudaEventElapsedTime(&ms, p->ev[r][4 + i], p->ev[r][5 + i]);
             sum[3 + i] += ms;
         }
+        if (p->reduce && e == cudaSuccess) {           // the pre-summation's share of the grid stage
+            float ms = 0.f;
+            e = cudaEventElapsedTime(&ms, p->ev[r][4], p->ev[r][7]);
+            sum[5] += ms;
+            sum[3] -= ms;
+        }
     }
     if (e != cudaSuccess) return cuda_fail(p, e);
     for (int i = 0; i < 3; ++i) ms_out[i] = nb ? (float)(sum[i] / nb) : 0.f;
-    for (int i = 3; i < 5; ++i) ms_out[i] = ng ? (float)(sum[i] / ng) : 0.f;
+    for (int i = 3; i < 6; ++i) ms_out[i] = ng ? (float)(sum[i] / ng) : 0.f;
     return GRIDDER_OK;
 }
 

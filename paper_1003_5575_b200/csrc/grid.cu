@@ -794,8 +794,8 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel_qbins(const GridPara
 // visibilities = record sums, no weights, nothing left to merge).  BASELINE.json config 4: 16.5
 // entries per record.
 //
-// A warp walks its items' entries 32 at a time (same queue and batch stream as the grid kernel; the
-// visibilities of three batches are landing in shared memory by cp.async while one is added).  Entries of one origin are consecutive.
+// A warp walks its items' entries 64 at a time, two per lane (its own queue of work items; sorted pairs
+// and visibilities land in rings of shared memory by cp.async, two to four batches ahead).  Entries of one origin are consecutive.
 // Every LANE keeps private bins for the O^2 offsets of the current origin in shared memory
 // ([offset][half][lane] float4: conflict-free whatever the offsets are) and adds its entry to its own
 // bin: no two lanes ever touch the same word, so there is nothing to match, merge or serialise.
@@ -804,19 +804,20 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel_qbins(const GridPara
 // groups, then a butterfly -- into registers, and at the end of the origin the non-empty bins are
 // written out as records in offset order.  All orders are fixed: reruns are bit-identical.
 // ------------------------------------------------------------------------------------------
-constexpr int kRedWarps = 10, kRedPiece = 64;
+constexpr int kRedWarps = 8, kRedPiece = 64;
 constexpr int kRedBins = 16;                                   // O^2 <= 16
-constexpr int kRedVis = 4, kRedVisF4 = 32 * 2 + 8;             // landing ring of the visibilities (a, b, weight)
-constexpr int kRedKey = 8, kRedKeyF4 = 16;                     // ring of the sorted pairs: 32 keys, 32 indices
-constexpr int kRedWarpF4 = kRedBins * 2 * 32 + kRedVis * kRedVisF4 + kRedKey * kRedKeyF4 + kRedKey;
+constexpr int kRedBatch = 64;                                  // entries per batch: two per lane
+constexpr int kRedVis = 3, kRedVisF4 = 2 * (32 * 2 + 8);       // landing ring of the visibilities: 2 x (a, b, weight)
+constexpr int kRedKey = 6, kRedKeyF4 = 32;                     // ring of the sorted pairs: 64 keys, 64 indices
+constexpr int kRedWarpF4 = kRedBins * 2 * 32 + kRedVis * kRedVisF4 + kRedKey * kRedKeyF4 + 8;
 
 __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridParams p) {
     extern __shared__ float4 smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float4 *priv = smem + (size_t)warp * kRedWarpF4;           // [q][half][lane]
-    float4 *vring = priv + kRedBins * 2 * 32;                  // kRedVis x {a[32], b[32], w[32]}
-    uint32_t *kring = reinterpret_cast<uint32_t *>(vring + kRedVis * kRedVisF4);   // kRedKey x {key[32], idx[32]}
-    uint4 *dring = reinterpret_cast<uint4 *>(kring + kRedKey * 64);                 // kRedKey batch descriptors
+    float4 *vring = priv + kRedBins * 2 * 32;                  // kRedVis x 2 x {a[32], b[32], w[32]}
+    uint32_t *kring = reinterpret_cast<uint32_t *>(vring + kRedVis * kRedVisF4);   // kRedKey x {key[64], idx[64]}
+    uint4 *dring = reinterpret_cast<uint4 *>(kring + kRedKey * 128);                // kRedKey batch descriptors
     for (int i = lane; i < kRedWarpF4; i += 32) priv[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     __syncwarp();
 
@@ -837,7 +838,7 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
     unsigned n_rec = 0;
     size_t rec_base = 0;
 
-    // ---- the warp's stream of batches: <= 32 consecutive entries of one work item ---------------------
+    // ---- the warp's stream of batches: <= 64 consecutive entries of one work item (lane: e and e + 32) ---
     // descriptor: x = first entry, y = count | first batch of its item << 8 | last << 9 | end of stream << 10,
     // z = item (relative to the class)
     unsigned cur_id = 0, cur_start = 0, cur_len = 0, cur_off = 0;      // the item the batches are cut from
@@ -856,7 +857,7 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
         }
     };
     // batch m: its descriptor into the ring, the copies of its sorted pairs started
-    auto gen_batch = [&](int m) {
+    auto gen_batch = [&](int ks) {
         if (!gen_end && cur_off >= cur_len) {
             if (!nxt_ok) gen_end = true;
             else {
@@ -868,71 +869,79 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
         if (!gen_end) {
             const unsigned left = cur_len - cur_off;
             d.x = cur_start + cur_off;
-            d.y = min(32u, left) | (cur_off == 0u ? 256u : 0u) | (left <= 32u ? 512u : 0u);
+            d.y = min((unsigned)kRedBatch, left) | (cur_off == 0u ? 256u : 0u) | (left <= (unsigned)kRedBatch ? 512u : 0u);
             d.z = cur_id;
-            cur_off += 32u;
+            cur_off += (unsigned)kRedBatch;
         }
-        const int ks = m & (kRedKey - 1);
         if (lane == 0) dring[ks] = d;
-        const bool v = lane < (int)(d.y & 63u);
-        cp_async_4(kring + ks * 64 + lane, p.keys + d.x + lane, v);
-        cp_async_4(kring + ks * 64 + 32 + lane, idx_sorted + d.x + lane, v);
+        const int cnt = (int)(d.y & 255u);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const bool v = lane + 32 * u < cnt;
+            cp_async_4(kring + ks * 128 + 32 * u + lane, p.keys + d.x + (v ? 32 * u + lane : 0), v);
+            cp_async_4(kring + ks * 128 + 64 + 32 * u + lane, idx_sorted + d.x + (v ? 32 * u + lane : 0), v);
+        }
     };
     // batch m (its pairs have landed): the copies of its visibilities started
-    auto gen_vis = [&](int m) {
-        const int ks = m & (kRedKey - 1);
-        const uint4 d = dring[ks];
-        const uint32_t key = kring[ks * 64 + lane], idx = kring[ks * 64 + 32 + lane];
-        const bool live = lane < (int)(d.y & 63u) && !(key & dropbit);
-        float4 *dst = vring + (m & (kRedVis - 1)) * kRedVisF4;
-        const float4 *src = p.vis + 2 * (size_t)(live ? idx : 0u);
-        cp_async_16(dst + lane, src, live);
-        cp_async_16(dst + 32 + lane, src + 1, live);
-        if (p.weight) cp_async_4(reinterpret_cast<float *>(dst + 64) + lane, p.weight + (live ? idx : 0u), live);
+    auto gen_vis = [&](int ks, int vs) {
+        const int cnt = (int)(dring[ks].y & 255u);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const uint32_t key = kring[ks * 128 + 32 * u + lane], idx = kring[ks * 128 + 64 + 32 * u + lane];
+            const bool live = lane + 32 * u < cnt && !(key & dropbit);
+            float4 *dst = vring + vs * kRedVisF4 + u * (kRedVisF4 / 2);
+            const float4 *src = p.vis + 2 * (size_t)(live ? idx : 0u);
+            cp_async_16(dst + lane, src, live);
+            cp_async_16(dst + 32 + lane, src + 1, live);
+            if (p.weight) cp_async_4(reinterpret_cast<float *>(dst + 64) + lane, p.weight + (live ? idx : 0u), live);
+        }
     };
 
     claim();
-    // prologue: batches 0..5 have their pairs moving, then 0..2 their visibilities
-    for (int m = 0; m < 6; ++m) {
+    // prologue: batches 0..3 have their pairs moving, then 0 and 1 their visibilities
+    for (int m = 0; m < 4; ++m) {
         gen_batch(m);
         cp_async_commit();
     }
-    asm volatile("cp.async.wait_group 3;" ::: "memory");          // pairs of batches 0..2
+    asm volatile("cp.async.wait_group 2;" ::: "memory");          // pairs of batches 0 and 1
     __syncwarp();
-    for (int m = 0; m < 3; ++m) {
-        gen_vis(m);
+    for (int m = 0; m < 2; ++m) {
+        gen_vis(m, m);
         cp_async_commit();
     }
 
-    // iteration n: pairs of batch n+6 and visibilities of batch n+3 start to move (one group), batch n is added
+    // iteration n: pairs of batch n+4 and visibilities of batch n+2 start to move (one group), batch n is added
+    int kn = 0, vn = 0;                  // ring slots of batch n
 #pragma unroll 1
-    for (int n = 0;; ++n) {
-        asm volatile("cp.async.wait_group 2;" ::: "memory");      // groups up to iteration n-3: pairs(n+3), vis(n)
+    while (true) {
+        asm volatile("cp.async.wait_group 1;" ::: "memory");      // groups up to iteration n-2: pairs(n+2), vis(n)
         __syncwarp();
-        gen_batch(n + 6);
-        gen_vis(n + 3);
+        gen_batch(kn + 4 < kRedKey ? kn + 4 : kn + 4 - kRedKey);
+        gen_vis(kn + 2 < kRedKey ? kn + 2 : kn + 2 - kRedKey, vn + 2 < kRedVis ? vn + 2 : vn + 2 - kRedVis);
         cp_async_commit();
-        const uint4 d = dring[n & (kRedKey - 1)];
+        const uint4 d = dring[kn];
         if (d.y & 1024u) break;
-        const int cnt = (int)(d.y & 63u);
+        const int cnt = (int)(d.y & 255u);
         {
-            const float4 *rw = vring + (n & (kRedVis - 1)) * kRedVisF4;
+            const float4 *rw = vring + vn * kRedVisF4;
             if (d.y & 256u) {            // first batch of an item: where its records go
                 n_rec = 0;
                 rec_base = p.rec_slot ? (size_t)d.z * p.rec_slot : (size_t)d.x;
             }
-            const uint32_t key = kring[(n & (kRedKey - 1)) * 64 + lane];
-            const bool valid = lane < cnt;
-            const int org = valid ? (int)((key >> p.key.aux_bits) & omask) : -2;
-            const int q = (int)(key & qmask);
-            const float w = p.weight ? reinterpret_cast<const float *>(rw + 64)[lane] : 1.0f;
-            const float4 a = rw[lane], b = rw[32 + lane];
+            const uint32_t key0 = kring[kn * 128 + lane], key1 = kring[kn * 128 + 32 + lane];
+            const int org0 = lane < cnt ? (int)((key0 >> p.key.aux_bits) & omask) : -2;
+            const int org1 = lane + 32 < cnt ? (int)((key1 >> p.key.aux_bits) & omask) : -2;
+            const int q0 = (int)(key0 & qmask), q1 = (int)(key1 & qmask);
+            const float w0 = p.weight ? reinterpret_cast<const float *>(rw + 64)[lane] : 1.0f;
+            const float w1 = p.weight ? reinterpret_cast<const float *>(rw + kRedVisF4 / 2 + 64)[lane] : 1.0f;
+            const float4 a0 = rw[lane], b0 = rw[32 + lane];
+            const float4 a1 = rw[kRedVisF4 / 2 + lane], b1 = rw[kRedVisF4 / 2 + 32 + lane];
             const bool last = d.y & 512u;
             int lp = 0;
             // origin by origin; one more round with no origin ends the item
 #pragma unroll 1
             while (lp < cnt || (last && lp == cnt)) {
-                const int seg = lp < cnt ? __shfl_sync(0xffffffffu, org, lp) : -1;
+                const int seg = lp < cnt ? __shfl_sync(0xffffffffu, lp < 32 ? org0 : org1, lp & 31) : -1;
                 const bool change = seg != bin_org;
                 if ((change && bin_org >= 0) || piece >= kRedPiece) {
                     // ---- the 32 private copies of every touched bin are added into bacc and cleared --------
@@ -983,17 +992,26 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
                 }
                 bin_org = seg;
                 if (lp >= cnt) break;
-                const bool in_seg = org == seg;
-                if (in_seg) {
-                    float4 *pa = priv + (q * 2) * 32 + lane, *pb = pa + 32;
-                    float4 x = *pa, y = *pb;
-                    x.x = fmaf(w, a.x, x.x); x.y = fmaf(w, a.y, x.y); x.z = fmaf(w, a.z, x.z); x.w = fmaf(w, a.w, x.w);
-                    y.x = fmaf(w, b.x, y.x); y.y = fmaf(w, b.y, y.y); y.z = fmaf(w, b.z, y.z); y.w = fmaf(w, b.w, y.w);
-                    *pa = x; *pb = y;
-                    touched |= 1u << q;
-                }
-                ++piece;
-                lp += __popc(__ballot_sync(0xffffffffu, in_seg));
+                // the lane's two entries: into its own bins (one read-modify-write when they share the offset)
+                const bool in0 = org0 == seg, in1 = org1 == seg;
+                const bool same = in0 && in1 && q0 == q1;
+                const bool sep1 = in1 && !same;
+                float4 *pa0 = priv + (q0 * 2) * 32 + lane, *pa1 = priv + (q1 * 2) * 32 + lane;
+                float4 x0, y0, x1, y1;
+                x0 = y0 = x1 = y1 = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (in0) { x0 = pa0[0]; y0 = pa0[32]; }
+                if (sep1) { x1 = pa1[0]; y1 = pa1[32]; }
+                x0.x = fmaf(w0, a0.x, x0.x); x0.y = fmaf(w0, a0.y, x0.y); x0.z = fmaf(w0, a0.z, x0.z); x0.w = fmaf(w0, a0.w, x0.w);
+                y0.x = fmaf(w0, b0.x, y0.x); y0.y = fmaf(w0, b0.y, y0.y); y0.z = fmaf(w0, b0.z, y0.z); y0.w = fmaf(w0, b0.w, y0.w);
+                if (same) { x1 = x0; y1 = y0; }
+                x1.x = fmaf(w1, a1.x, x1.x); x1.y = fmaf(w1, a1.y, x1.y); x1.z = fmaf(w1, a1.z, x1.z); x1.w = fmaf(w1, a1.w, x1.w);
+                y1.x = fmaf(w1, b1.x, y1.x); y1.y = fmaf(w1, b1.y, y1.y); y1.z = fmaf(w1, b1.z, y1.z); y1.w = fmaf(w1, b1.w, y1.w);
+                if (in0 && !same) { pa0[0] = x0; pa0[32] = y0; }
+                if (in1) { pa1[0] = x1; pa1[32] = y1; }
+                if (in0) touched |= 1u << q0;
+                if (in1) touched |= 1u << q1;
+                piece += 2;
+                lp += __popc(__ballot_sync(0xffffffffu, in0)) + __popc(__ballot_sync(0xffffffffu, in1));
             }
             if (last && lane == 0) {     // the item's entry in the record items
                 WorkItem ri;
@@ -1004,6 +1022,8 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
                 p.rec_items[item_begin + d.z] = ri;
             }
         }
+        kn = kn + 1 < kRedKey ? kn + 1 : 0;
+        vn = vn + 1 < kRedVis ? vn + 1 : 0;
     }
     asm volatile("cp.async.wait_group 0;" ::: "memory");
 }
@@ -1226,6 +1246,7 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         if (e == cudaSuccess) e = cudaMemsetAsync(p.counters->queue_head, 0, sizeof(unsigned int) * kMaxClasses, s);
         if (e != cudaSuccess) return e;
         p.n_launches += 1;
+        stage_mark(p, 7, s);
     }
     for (int c = 0; c < p.n_cls; ++c) {
         const ClassGeo &g = p.cls[c];

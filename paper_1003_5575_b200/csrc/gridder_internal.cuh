@@ -195,7 +195,7 @@ struct Plan {
     int last_cuda_error;
     // harness support: stage timers and a launch counter
     bool profiling;
-    cudaEvent_t ev[kProfRing][7];  // per call: bin: 0 map 1 sort 2 tables 3 | grid: 4 grid 5 flush 6
+    cudaEvent_t ev[kProfRing][8];  // per call: bin: 0 map 1 sort 2 tables 3 | grid: 4 (reduce 7) grid 5 flush 6
     int64_t prof_bin_calls, prof_grid_calls;       // since profiling was enabled
     int64_t n_launches;
     cudaStream_t copy_stream;      // gridder_run_host: host-to-device copies of the next slice

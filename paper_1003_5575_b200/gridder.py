@@ -208,11 +208,11 @@ class Gridder:
         if rc != OK:
             raise GridderError(rc, "gridder_set_profiling")
 
-    STAGES = ("map", "sort", "tables", "grid", "flush")
+    STAGES = ("map", "sort", "tables", "grid", "flush", "reduce")
 
     def stage_ms(self) -> dict:
         """Device milliseconds of the last bin/grid per stage (synchronises on their events)."""
-        ms = (C.c_float * 5)()
+        ms = (C.c_float * 6)()
         rc = self._lib.gridder_get_stage_ms(self._plan, ms)
         if rc != OK:
             raise GridderError(rc, "gridder_get_stage_ms")
