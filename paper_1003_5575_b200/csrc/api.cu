@@ -45,7 +45,16 @@ int derive(const gridder_config *cfg, Plan &p) {
     const bool cplx = cfg->kernel_is_complex != 0;
     // fast path: one real table with S <= 16 (shared-memory table, 32-bit sort values)
     p.mode = cplx ? 2 : ((cfg->n_wplanes == 1 && cfg->support[0] <= 16 && !env_int("GRIDDER_FORCE_GENERAL", 0)) ? 0 : 1);
-    p.tlog = env_int("GRIDDER_TILE_LOG2", 2);
+    // DENSE plans -- fast path, 16-cell patch, O^2 <= 64, 256 visibilities and more per 4 x 4 cells -- sum the
+    // entries of equal (origin, offset) before gridding (GRIDDER_QBINS: 0 never, 1 by density, 2 always)
+    const int64_t oo_early = (int64_t)cfg->oversample * cfg->oversample;
+    const int qb_mode = env_int("GRIDDER_QBINS", 1);
+    const bool dense = p.mode == 0 && cfg->support[0] > 8 && oo_early <= 64 && env_int("GRIDDER_MERGE", 1) &&
+                       (qb_mode >= 2 || (qb_mode == 1 && cfg->max_vis * 16 / ((int64_t)cfg->grid_size * cfg->grid_size) >= 256));
+    // ... and with the pre-summation kernel (O^2 <= 16) larger tiles and longer work items pay: the work per
+    // item follows its (origin, offset) pairs, not its entries, and the flush has fewer regions to add
+    const bool dense_reduce = dense && oo_early <= 16 && env_int("GRIDDER_REDUCE", 1);
+    p.tlog = env_int("GRIDDER_TILE_LOG2", dense_reduce ? 3 : 2);
     if (p.tlog < 2 || p.tlog > 4) return GRIDDER_ERR_INVALID_ARG;
     p.T = 1 << p.tlog;
     p.ntx = (cfg->grid_size + p.T - 1) / p.T;
@@ -115,20 +124,16 @@ int derive(const gridder_config *cfg, Plan &p) {
     // short items so that a hot tile still spreads over the ~1800 resident warps; the largest get 8192,
     // which halves the number of partial regions the flush has to sum for the cells of a hot tile
     // (the accuracy budget of DESIGN.md section 7 holds up to 8192)
-    int k_auto = 8192;
+    int k_auto = dense_reduce ? 32768 : 8192;
     while (k_auto > 256 && (int64_t)k_auto * 16384 > cfg->max_vis) k_auto >>= 1;
     p.chunk = env_int("GRIDDER_CHUNK", k_auto);
     if (p.chunk < 32 || p.chunk > (1 << 20)) return GRIDDER_ERR_INVALID_ARG;
     p.warps_forced = env_int("GRIDDER_WARPS", 0);
     p.merge = env_int("GRIDDER_MERGE", 1) ? 1 : 0;
     // fast path with per-origin bins (grid.cu): one real table, 16-cell patch, O^2 <= 64 offsets
-    // GRIDDER_QBINS: 0 never, 1 (default) for dense plans -- 256 visibilities per tile and more, where an
-    // origin gathers many entries per sub-cell offset; sparser inputs merge as well per batch --, 2 always
+    // (sparser inputs merge as well per batch of 32)
     p.qbins = 0;
-    const int qb_mode = env_int("GRIDDER_QBINS", 1);
-    if (p.mode == 0 && p.merge && p.tmem_cols == 0 && p.cls[0].NA == 2 && oo <= 64 &&
-        (qb_mode >= 2 || (qb_mode == 1 && cfg->max_vis / p.n_tiles >= 256)))
-        p.qbins = (int)oo;
+    if (dense && p.mode == 0 && p.merge && p.tmem_cols == 0 && p.cls[0].NA == 2) p.qbins = (int)oo;
     p.fold_batches = env_int("GRIDDER_FOLD_BATCHES", 8);
     if (p.fold_batches < 1 || p.fold_batches > 64 || (p.fold_batches & (p.fold_batches - 1))) return GRIDDER_ERR_INVALID_ARG;
 
