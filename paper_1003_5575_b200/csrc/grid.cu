@@ -796,26 +796,28 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel_qbins(const GridPara
 //
 // A warp walks its items' entries 64 at a time, two per lane (its own queue of work items; sorted pairs
 // and visibilities land in rings of shared memory by cp.async, two to four batches ahead).  Entries of one origin are consecutive.
-// Every LANE keeps private bins for the O^2 offsets of the current origin in shared memory
-// ([offset][half][lane] float4: conflict-free whatever the offsets are) and adds its entry to its own
-// bin: no two lanes ever touch the same word, so there is nothing to match, merge or serialise.
-// When the origin changes (or after 64 batches, which bounds the FP32 chain of a bin) the 32 private
-// copies of each touched bin are added in a fixed order -- 8 serial additions in each of four lane
-// groups, then a butterfly -- into registers, and at the end of the origin the non-empty bins are
+// Every lane PAIR (l, l + 16) keeps private bins for the O^2 offsets of the current origin in shared
+// memory ([offset][half][l] float4: conflict-free whatever the offsets are); the two half-warps add
+// their entries to their bins in turn, so no two lanes ever touch the same word at the same time and
+// there is nothing to match, merge or serialise.
+// When the origin changes (or after 1024 entries, which bounds the FP32 chain of a bin copy at 64) the 16
+// private copies of each touched bin are added in a fixed order -- 4 serial additions in each of four
+// lane groups, then a butterfly -- into registers, and at the end of the origin the non-empty bins are
 // written out as records in offset order.  All orders are fixed: reruns are bit-identical.
 // ------------------------------------------------------------------------------------------
-constexpr int kRedWarps = 8, kRedPiece = 64;
+constexpr int kRedWarps = 12, kRedPiece = 32;      // (a copy is shared by two lanes: chains <= 64)
 constexpr int kRedBins = 16;                                   // O^2 <= 16
+constexpr int kRedCopies = 16;                                 // private copies of a bin: lanes l and l + 16 share one
 constexpr int kRedBatch = 64;                                  // entries per batch: two per lane
 constexpr int kRedVis = 3, kRedVisF4 = 2 * (32 * 2 + 8);       // landing ring of the visibilities: 2 x (a, b, weight)
 constexpr int kRedKey = 6, kRedKeyF4 = 32;                     // ring of the sorted pairs: 64 keys, 64 indices
-constexpr int kRedWarpF4 = kRedBins * 2 * 32 + kRedVis * kRedVisF4 + kRedKey * kRedKeyF4 + 8;
+constexpr int kRedWarpF4 = kRedBins * 2 * kRedCopies + kRedVis * kRedVisF4 + kRedKey * kRedKeyF4 + 8;
 
 __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridParams p) {
     extern __shared__ float4 smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float4 *priv = smem + (size_t)warp * kRedWarpF4;           // [q][half][lane]
-    float4 *vring = priv + kRedBins * 2 * 32;                  // kRedVis x 2 x {a[32], b[32], w[32]}
+    float4 *priv = smem + (size_t)warp * kRedWarpF4;           // [q][half][lane & 15]
+    float4 *vring = priv + kRedBins * 2 * kRedCopies;                  // kRedVis x 2 x {a[32], b[32], w[32]}
     uint32_t *kring = reinterpret_cast<uint32_t *>(vring + kRedVis * kRedVisF4);   // kRedKey x {key[64], idx[64]}
     uint4 *dring = reinterpret_cast<uint4 *>(kring + kRedKey * 128);                // kRedKey batch descriptors
     for (int i = lane; i < kRedWarpF4; i += 32) priv[i] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -826,8 +828,9 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
     const uint32_t dropbit = 1u << (2 * p.key.bits_q);
     const unsigned item_begin = p.counters->cls_begin[p.cls], item_end = p.counters->cls_end[p.cls];
     const uint32_t *idx_sorted = reinterpret_cast<const uint32_t *>(p.vals);
-    // the lane's part in adding the private copies: bin 4 pass + bs, half h, source lanes 8 g .. 8 g + 7
+    // the lane's part in adding the private copies: bin 4 pass + bs, half h, copies 4 g .. 4 g + 3
     const int g = lane & 3, h = (lane >> 2) & 1, bs = lane >> 3;
+    const int cl = lane & (kRedCopies - 1), rot = h + 2 * (g >> 1);      // (rot: conflict-free reads)
 
     float4 bacc[4];                      // sums of the bins 4 pass + bs (half h) over the pieces of the origin
 #pragma unroll
@@ -951,11 +954,11 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
 #pragma unroll
                     for (int pass = 0; pass < 4; ++pass) {
                         if (((u >> (4 * pass)) & 15u) == 0u) continue;
-                        const float4 *src = priv + ((4 * pass + bs) * 2 + h) * 32 + 8 * g;
+                        const float4 *src = priv + ((4 * pass + bs) * 2 + h) * kRedCopies + 4 * g;
                         float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-                        for (int j = 0; j < 8; ++j) {
-                            const float4 v = src[(j + lane) & 7];
+                        for (int j = 0; j < 4; ++j) {
+                            const float4 v = src[(j + rot) & 3];
                             t.x += v.x; t.y += v.y; t.z += v.z; t.w += v.w;
                         }
 #pragma unroll
@@ -966,10 +969,10 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
                         bacc[pass].x += t.x; bacc[pass].y += t.y; bacc[pass].z += t.z; bacc[pass].w += t.w;
                     }
                     __syncwarp();
-                    for (unsigned m = touched; m; m &= m - 1u) {
+                    for (unsigned m = touched; m; m &= m - 1u) {     // (lanes l and l + 16 may clear the same words)
                         const int qq = __ffs(m) - 1;
-                        priv[(qq * 2) * 32 + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
-                        priv[(qq * 2 + 1) * 32 + lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        priv[(qq * 2) * kRedCopies + cl] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        priv[(qq * 2 + 1) * kRedCopies + cl] = make_float4(0.f, 0.f, 0.f, 0.f);
                     }
                     touched = 0;
                     piece = 0;
@@ -992,22 +995,29 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
                 }
                 bin_org = seg;
                 if (lp >= cnt) break;
-                // the lane's two entries: into its own bins (one read-modify-write when they share the offset)
+                // the lane's two entries: into its copy of the bins (one read-modify-write when they share the
+                // offset); lanes l and l + 16 share a copy, so the two half-warps take turns
                 const bool in0 = org0 == seg, in1 = org1 == seg;
                 const bool same = in0 && in1 && q0 == q1;
                 const bool sep1 = in1 && !same;
-                float4 *pa0 = priv + (q0 * 2) * 32 + lane, *pa1 = priv + (q1 * 2) * 32 + lane;
-                float4 x0, y0, x1, y1;
-                x0 = y0 = x1 = y1 = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (in0) { x0 = pa0[0]; y0 = pa0[32]; }
-                if (sep1) { x1 = pa1[0]; y1 = pa1[32]; }
-                x0.x = fmaf(w0, a0.x, x0.x); x0.y = fmaf(w0, a0.y, x0.y); x0.z = fmaf(w0, a0.z, x0.z); x0.w = fmaf(w0, a0.w, x0.w);
-                y0.x = fmaf(w0, b0.x, y0.x); y0.y = fmaf(w0, b0.y, y0.y); y0.z = fmaf(w0, b0.z, y0.z); y0.w = fmaf(w0, b0.w, y0.w);
-                if (same) { x1 = x0; y1 = y0; }
-                x1.x = fmaf(w1, a1.x, x1.x); x1.y = fmaf(w1, a1.y, x1.y); x1.z = fmaf(w1, a1.z, x1.z); x1.w = fmaf(w1, a1.w, x1.w);
-                y1.x = fmaf(w1, b1.x, y1.x); y1.y = fmaf(w1, b1.y, y1.y); y1.z = fmaf(w1, b1.z, y1.z); y1.w = fmaf(w1, b1.w, y1.w);
-                if (in0 && !same) { pa0[0] = x0; pa0[32] = y0; }
-                if (in1) { pa1[0] = x1; pa1[32] = y1; }
+                float4 *pa0 = priv + (q0 * 2) * kRedCopies + cl, *pa1 = priv + (q1 * 2) * kRedCopies + cl;
+#pragma unroll 1
+                for (int ph = 0; ph < 2; ++ph) {
+                    if ((lane >> 4) == ph) {
+                        float4 x0, y0, x1, y1;
+                        x0 = y0 = x1 = y1 = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (in0) { x0 = pa0[0]; y0 = pa0[kRedCopies]; }
+                        if (sep1) { x1 = pa1[0]; y1 = pa1[kRedCopies]; }
+                        x0.x = fmaf(w0, a0.x, x0.x); x0.y = fmaf(w0, a0.y, x0.y); x0.z = fmaf(w0, a0.z, x0.z); x0.w = fmaf(w0, a0.w, x0.w);
+                        y0.x = fmaf(w0, b0.x, y0.x); y0.y = fmaf(w0, b0.y, y0.y); y0.z = fmaf(w0, b0.z, y0.z); y0.w = fmaf(w0, b0.w, y0.w);
+                        if (same) { x1 = x0; y1 = y0; }
+                        x1.x = fmaf(w1, a1.x, x1.x); x1.y = fmaf(w1, a1.y, x1.y); x1.z = fmaf(w1, a1.z, x1.z); x1.w = fmaf(w1, a1.w, x1.w);
+                        y1.x = fmaf(w1, b1.x, y1.x); y1.y = fmaf(w1, b1.y, y1.y); y1.z = fmaf(w1, b1.z, y1.z); y1.w = fmaf(w1, b1.w, y1.w);
+                        if (in0 && !same) { pa0[0] = x0; pa0[kRedCopies] = y0; }
+                        if (in1) { pa1[0] = x1; pa1[kRedCopies] = y1; }
+                    }
+                    __syncwarp();
+                }
                 if (in0) touched |= 1u << q0;
                 if (in1) touched |= 1u << q1;
                 piece += 2;
