@@ -417,3 +417,28 @@ def test_per_origin_bins_kernel_dense_lattice_chunks_and_tiles(dev):
         assert st_a.n_work_items == st_b.n_work_items and st_a.max_tile_load > 256
         assert 0 < st_a.n_records_gridded <= st_b.n_records_gridded < n        # bins merge at least as much
         assert st_a.fma_executed == st_a.n_records_gridded * 256 * 8
+
+
+def test_pre_summation_long_origins_pieces_and_unit_weights(dev):
+    """reduce_kernel: a few origins with thousands of entries each (the 1024-entry piece limit adds the bin
+    copies several times per origin), no weights, and items of one and of many batches; and the one-kernel
+    form of the same plan (GRIDDER_REDUCE=0: grid_kernel_qbins) gives a grid inside the same tolerance."""
+    rng = np.random.default_rng(93)
+    N, S, O, n = 64, 16, 4, 20_000
+    table = synth.spheroidal_table(S, O)
+    uvw = np.zeros((1, n, 3))
+    uvw[0, :, :2] = rng.uniform(-1.2, 1.2, (n, 2))                   # 3 x 3 origins, ~2200 entries each
+    uvw[0, :50, :2] = rng.uniform(-20.0, 20.0, (50, 2))              # and a few lonely ones (items of one entry)
+    vis = (rng.standard_normal((n, 4, 2)) + 1.0).astype(np.float32)
+    kw = dict(N=N, du=1.0, O=O, S=S, table=table)
+    ref, ab, _ = _oracle(uvw, [C], vis, None, **kw)
+    env = {"GRIDDER_QBINS": 2, "GRIDDER_TILE_LOG2": 2, "GRIDDER_CHUNK": 8192}
+    a, st_a = _run(dev, uvw, [C], vis, None, env=env, **kw)
+    a2, _ = _run(dev, uvw, [C], vis, None, env=env, **kw)
+    b, st_b = _run(dev, uvw, [C], vis, None, env=dict(env, GRIDDER_REDUCE=0), **kw)
+    assert np.array_equal(a, a2)
+    assert_parity(a, ref, ab, "pre-summation, long origins")
+    assert_parity(b, ref, ab, "per-origin bins in the grid kernel, long origins")
+    assert st_a.max_tile_load > 2048 and st_a.chunk_size == 8192
+    # both count one record per non-empty (item, origin, offset)
+    assert st_a.n_records_gridded == st_b.n_records_gridded < n // 10
