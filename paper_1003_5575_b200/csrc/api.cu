@@ -100,10 +100,12 @@ int derive(const gridder_config *cfg, Plan &p) {
     if (off >= (1ull << 31)) return GRIDDER_ERR_UNSUPPORTED;       // table offsets are 32-bit byte offsets
     p.coef_bytes = off;
 
-    // fast path, opt-in (GRIDDER_TMEM=1): the table in tensor memory (512 columns x 32 bit per lane) when it
-    // fits.  Measured on B200: same speed as the shared-memory table, so off by default.
+    // fast path (GRIDDER_TMEM=0/1): the table in tensor memory (512 columns x 32 bit per lane) when it fits.
+    // Measured on B200: same speed as the shared-memory table while the kernel is FMA-bound (DESIGN.md section
+    // 10), 8 % faster on the records of a dense plan, where the shared-memory path is the busiest unit: on by
+    // default there, off elsewhere.
     p.tmem_cols = 0;
-    if (p.mode == 0 && env_int("GRIDDER_TMEM", 0)) {
+    if (p.mode == 0 && env_int("GRIDDER_TMEM", dense_reduce ? 1 : 0)) {
         const size_t cols = oo * p.cls[0].NA * p.cls[0].NB;
         if (cols <= 512) {
             p.tmem_cols = 32;
@@ -133,7 +135,7 @@ int derive(const gridder_config *cfg, Plan &p) {
     // fast path with per-origin bins (grid.cu): one real table, 16-cell patch, O^2 <= 64 offsets
     // (sparser inputs merge as well per batch of 32)
     p.qbins = 0;
-    if (dense && p.mode == 0 && p.merge && p.tmem_cols == 0 && p.cls[0].NA == 2) p.qbins = (int)oo;
+    if (dense && p.mode == 0 && p.merge && (p.tmem_cols == 0 || dense_reduce) && p.cls[0].NA == 2) p.qbins = (int)oo;
     p.fold_batches = env_int("GRIDDER_FOLD_BATCHES", 8);
     if (p.fold_batches < 1 || p.fold_batches > 64 || (p.fold_batches & (p.fold_batches - 1))) return GRIDDER_ERR_INVALID_ARG;
 
@@ -167,6 +169,7 @@ int derive(const gridder_config *cfg, Plan &p) {
         p.rec_cap = p.rec_slot ? p.max_items * per_item : n;
         if (p.rec_cap < (1ll << 32)) p.reduce = 1;
     }
+    if (!p.reduce && p.tmem_cols > 0) p.qbins = 0;       // (grid_kernel_qbins reads its table from shared memory)
     p.partials_f4 = 0;
     for (int c = 0; c < p.n_cls; ++c) {
         p.cls[c].part_off_f4 = p.partials_f4;

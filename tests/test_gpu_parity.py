@@ -442,3 +442,19 @@ def test_pre_summation_long_origins_pieces_and_unit_weights(dev):
     assert st_a.max_tile_load > 2048 and st_a.chunk_size == 8192
     # both count one record per non-empty (item, origin, offset)
     assert st_a.n_records_gridded == st_b.n_records_gridded < n // 10
+
+
+@pytest.mark.parametrize("S,O,N,n,env", [(16, 4, 96, 6000, {}), (12, 4, 66, 3000, {"GRIDDER_MERGE": 0}),
+                                         (16, 4, 80, 8000, {"GRIDDER_QBINS": 2}), (7, 8, 64, 3000, {})])
+def test_table_in_tensor_memory(dev, S, O, N, n, env):
+    """GRIDDER_TMEM=1: the GCF table is read with tcgen05.ld instead of LDS (the default for dense plans,
+    where the grid kernel runs on pre-summed records); same bits as the shared-memory table."""
+    rng = np.random.default_rng(S + N + n)
+    table = rng.standard_normal((S * O, S * O)).astype(np.float32)
+    uvw, vis, w = _random_case(rng, n, N, S)
+    kw = dict(N=N, du=1.0, O=O, S=S, table=table)
+    a, _ = _run(dev, uvw, [C], vis, w, env=dict(env, GRIDDER_TMEM=1), **kw)
+    b, _ = _run(dev, uvw, [C], vis, w, env=dict(env, GRIDDER_TMEM=0), **kw)
+    ref, ab, _ = _oracle(uvw, [C], vis, w, **kw)
+    assert np.array_equal(a, b)
+    assert_parity(a, ref, ab, f"tensor-memory table S={S} O={O}")
