@@ -805,12 +805,12 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel_qbins(const GridPara
 // lane groups, then a butterfly -- into registers, and at the end of the origin the non-empty bins are
 // written out as records in offset order.  All orders are fixed: reruns are bit-identical.
 // ------------------------------------------------------------------------------------------
-constexpr int kRedWarps = 12, kRedPiece = 32;      // (a copy is shared by two lanes: chains <= 64)
+constexpr int kRedWarps = 13, kRedPiece = 32;      // (a copy is shared by two lanes: chains <= 64)
 constexpr int kRedBins = 16;                                   // O^2 <= 16
 constexpr int kRedCopies = 16;                                 // private copies of a bin: lanes l and l + 16 share one
 constexpr int kRedBatch = 64;                                  // entries per batch: two per lane
 constexpr int kRedVis = 3, kRedVisF4 = 2 * (32 * 2 + 8);       // landing ring of the visibilities: 2 x (a, b, weight)
-constexpr int kRedKey = 6, kRedKeyF4 = 32;                     // ring of the sorted pairs: 64 keys, 64 indices
+constexpr int kRedKey = 5, kRedKeyF4 = 32;                     // ring of the sorted pairs: 64 keys, 64 indices
 constexpr int kRedWarpF4 = kRedBins * 2 * kRedCopies + kRedVis * kRedVisF4 + kRedKey * kRedKeyF4 + 8;
 
 __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridParams p) {
