@@ -59,6 +59,9 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (development only)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle leg (development only)")
     ap.add_argument("--no-unmerged", action="store_true", help="skip the merging-off leg (development only)")
+    ap.add_argument("--mfs", action="store_true",
+                    help="row f4: with N > 1 ranks also sum the per-rank grids inside every timed step "
+                         "(deterministic all-to-all + FP64 sum + all-gather); default: no collective")
     ap.add_argument("--atomic", action="store_true",
                     help="also time the atomic-scatter gridder (SURVEY row f1) once on the same workload")
     return ap.parse_args()
@@ -272,9 +275,15 @@ def run_ours(args) -> dict | None:
                         n_wplanes=wl.n_wplanes, w_max=wl.w_max, kernel_is_complex=wl.kernel_is_complex)
     grid = torch.empty((4, wl.grid_size, wl.grid_size, 2), dtype=torch.float32, device=dev)
 
+    mfs_on = bool(args.mfs and world > 1)
+    if mfs_on:
+        from paper_1003_5575_b200 import mfs
+
     def step():
         g.bin(d_uvw, d_freq)
         g.grid(vis, weight, out=grid)
+        if mfs_on:
+            mfs.reduce_grids(grid)
 
     def barrier():
         torch.cuda.synchronize()
@@ -300,7 +309,7 @@ def run_ours(args) -> dict | None:
     ms_rank = e0.elapsed_time(e1)
     stage = g.stage_ms()
     st_exec = g.stats()                   # records gridded / FMAs executed by the last gridder_grid
-    launches = g.launch_count() - launches0
+    launches = g.launch_count() - launches0 + (args.steps if mfs_on else 0)      # + gridder_sum_parts per step
     g.set_profiling(False)
     checksum = float(grid[0, wl.grid_size // 2, wl.grid_size // 2, 0].item())
 
@@ -445,7 +454,8 @@ def run_ours(args) -> dict | None:
         "config": {"workload": f"config{wl.cfg}", "n_antennas": wl.n_ant, "n_baselines": nb, "n_chan": nf,
                    "n_time": nt, "n_vis_per_gpu": n, "grid": wl.grid_size, "support": max(wl.support),
                    "oversample": wl.oversample, "n_wplanes": wl.n_wplanes, "weights": weight is not None,
-                   "parallelism": f"channel-block x{world} (no collective)",
+                   "parallelism": (f"channel-block x{world} + grid sum (all-to-all, FP64 fixed-order sum, all-gather)"
+                                   if mfs_on else f"channel-block x{world} (no collective)"),
                    "l2": "inputs per step exceed the 126 MB L2" if n * 32 > (126 << 20) else "L2-resident inputs",
                    "tile": st.tile_size, "chunk": st.chunk_size, "work_items": st.n_work_items,
                    "grid_warps_per_sm": st.grid_warps_per_sm},

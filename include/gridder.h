@@ -157,6 +157,17 @@ GRIDDER_API int gridder_scatter_atomic(gridder_plan_t *plan, const double *uvw_m
                                        int32_t n_baseline, const double *freq_hz, int32_t n_chan, const float *vis,
                                        const float *weight, float *grid, int32_t accumulate, void *cuda_stream);
 
+/* the summation step of a channel-sharded deployment (PAPER.md :108-120: every
+ * GPU grids its own block of channels; a multi-frequency-synthesis image needs the sum of the per-GPU
+ * grids).  out[i] = (float) sum_{p = 0 .. n_parts-1, in this order, in double} parts[p * stride + i],
+ * i < len: the part-p slices of all ranks, as an all-to-all leaves them in one buffer, become the rank's
+ * slice of the summed grid -- a fixed order, so the result does not depend on the collective's algorithm
+ * and is bit-identical from run to run and from rank to rank.  parts, out: DEVICE float, 16-byte
+ * aligned, len and stride multiples of 4; out may alias parts (part 0).  No plan is needed.
+ * Asynchronous on `cuda_stream`.  Returns GRIDDER_OK / GRIDDER_ERR_INVALID_ARG / GRIDDER_ERR_CUDA. */
+GRIDDER_API int gridder_sum_parts(const float *parts, int32_t n_parts, int64_t len, int64_t stride, float *out,
+                                  void *cuda_stream);
+
 /* the imaging step that follows the gridder (PAPER.md :75, :211, :217): centred
  * unnormalised 2-D inverse DFT of the 4 polarisation planes with the grid correction fused in,
  *   image[pol][y][x] = corr[y] corr[x] sum_{v,u} grid[pol][v][u] exp(+2 pi i ((u-N/2)(x-N/2) + (v-N/2)(y-N/2)) / N).

@@ -388,6 +388,15 @@ int gridder_scatter_atomic(gridder_plan_t *plan, const double *uvw_m, int32_t n_
     return GRIDDER_OK;
 }
 
+int gridder_sum_parts(const float *parts, int32_t n_parts, int64_t len, int64_t stride, float *out,
+                      void *cuda_stream) {
+    if (!parts || !out || n_parts < 1 || len < 0 || stride < len || (len & 3) || (stride & 3)) return GRIDDER_ERR_INVALID_ARG;
+    if (((uintptr_t)parts & 15) || ((uintptr_t)out & 15)) return GRIDDER_ERR_INVALID_ARG;
+    if (len == 0) return GRIDDER_OK;
+    const cudaError_t e = launch_sum_parts(parts, n_parts, len, stride, out, (cudaStream_t)cuda_stream);
+    return e == cudaSuccess ? GRIDDER_OK : GRIDDER_ERR_CUDA;
+}
+
 int gridder_image_workspace_size(gridder_plan_t *plan, size_t *bytes) {
     Plan *p = reinterpret_cast<Plan *>(plan);
     if (!p || !bytes) return GRIDDER_ERR_INVALID_ARG;

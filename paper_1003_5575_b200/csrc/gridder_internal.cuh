@@ -221,6 +221,9 @@ cudaError_t launch_map_debug(const Plan &p, const double *uvw, int n_time, int n
                              int n_chan, const int32_t *table_index, int32_t *out, cudaStream_t s);
 cudaError_t sort_temp_bytes(int64_t n, int begin_bit, int end_bit, bool wide, size_t *bytes);
 
+// scatter.cu (row f4's summation kernel lives beside row f1)
+cudaError_t launch_sum_parts(const float *parts, int n_parts, long long len, long long stride, float *out, cudaStream_t s);
+
 // runs.cu
 cudaError_t runs_temp_bytes(int64_t cap, int begin_bit, int end_bit, size_t *bytes);
 cudaError_t launch_bin_runs(Plan &p, const double *uvw, const double *scale, long long n, int n_chan, cudaStream_t s,

@@ -89,4 +89,29 @@ cudaError_t launch_scatter_atomic(Plan &p, const double *uvw, int n_time, int n_
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------
+// Row f4: out[i] = (float) sum over the parts, in part order, in double (include/gridder.h).  One float4
+// per thread and part: HBM-bound, (n_parts + 1) x 4 len bytes.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) sum_parts_kernel(const float4 *__restrict__ parts, int n_parts, long long len4,
+                                                         long long stride4, float4 *__restrict__ out) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < len4; i += (long long)gridDim.x * blockDim.x) {
+        double a = 0.0, b = 0.0, c = 0.0, d = 0.0;
+        for (int p = 0; p < n_parts; ++p) {
+            const float4 v = parts[(long long)p * stride4 + i];
+            a += (double)v.x; b += (double)v.y; c += (double)v.z; d += (double)v.w;
+        }
+        out[i] = make_float4((float)a, (float)b, (float)c, (float)d);
+    }
+}
+
+cudaError_t launch_sum_parts(const float *parts, int n_parts, long long len, long long stride, float *out, cudaStream_t s) {
+    const long long len4 = len / 4;
+    long long blocks = (len4 + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    sum_parts_kernel<<<(int)blocks, 256, 0, s>>>(reinterpret_cast<const float4 *>(parts), n_parts, len4, stride / 4,
+                                                 reinterpret_cast<float4 *>(out));
+    return cudaGetLastError();
+}
+
 }  // namespace gridder

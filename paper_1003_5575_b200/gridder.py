@@ -19,7 +19,7 @@ OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_WORKSPACE, ERR_CUDA, ERR_NOT_BINNED, ERR_
 
 EXPORTS = ("gridder_workspace_size", "gridder_plan", "gridder_bin", "gridder_bin_tables", "gridder_grid", "gridder_destroy",
            "gridder_get_stats", "gridder_map", "gridder_scatter_atomic", "gridder_image_workspace_size", "gridder_image",
-           "gridder_run_host", "gridder_set_profiling",
+           "gridder_run_host", "gridder_sum_parts", "gridder_set_profiling",
            "gridder_get_stage_ms", "gridder_launch_count", "gridder_strerror",
            "gridder_last_cuda_error", "gridder_version")
 
@@ -68,6 +68,7 @@ def load_library() -> C.CDLL:
                                     C.c_void_p, C.c_void_p, C.c_void_p]
         lib.gridder_scatter_atomic.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
                                                C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+        lib.gridder_sum_parts.argtypes = [C.c_void_p, C.c_int32, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
         lib.gridder_image_workspace_size.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
         lib.gridder_image.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
         lib.gridder_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,

@@ -458,3 +458,47 @@ def test_table_in_tensor_memory(dev, S, O, N, n, env):
     ref, ab, _ = _oracle(uvw, [C], vis, w, **kw)
     assert np.array_equal(a, b)
     assert_parity(a, ref, ab, f"tensor-memory table S={S} O={O}")
+
+
+def test_pre_summation_edge_cases(dev):
+    """The dense path (reduce_kernel + grid_kernel on records, forced) on the degenerate inputs: empty,
+    one visibility, everything dropped, zero weights, accumulate onto a grid, bin once / grid twice / re-bin."""
+    env = {"GRIDDER_QBINS": 2}
+    N, S, O = 48, 16, 4
+    table = synth.spheroidal_table(S, O)
+    kw = dict(N=N, du=1.0, O=O, S=S, table=table)
+    got, st = _run(dev, np.zeros((1, 0, 3)), [C], np.zeros((0, 4, 2), np.float32), None, env=env, **kw)
+    assert st.n_vis == 0 and st.n_work_items == 0 and not got.any()
+    uvw = np.zeros((1, 1, 3))
+    vis = np.zeros((1, 4, 2), np.float32)
+    vis[0, 1] = (-3.0, 0.5)
+    got, st = _run(dev, uvw, [C], vis, None, env=env, **kw)
+    ref, ab, _ = _oracle(uvw, [C], vis, None, **kw)
+    assert st.n_work_items == 1 and st.n_records_gridded == 1
+    assert_parity(got, ref, ab, "dense path, single")
+    uvw[0, 0, :2] = (100.0, 0.0)
+    got, st = _run(dev, uvw, [C], vis, None, env=env, **kw)
+    assert st.n_dropped == 1 and st.vis_taps == 0 and not got.any()
+
+    rng = np.random.default_rng(94)
+    n = 5000
+    uvw, vis, w = _random_case(rng, n, N, S, spread=6)
+    w[::3] = 0.0
+    base = rng.standard_normal((4, N, N, 2)).astype(np.float32)
+    got, st = _run(dev, uvw, [C], vis, w, env=env, accumulate_onto=base, **kw)
+    ref, ab, ost = _oracle(uvw, [C], vis, w, **kw)
+    assert st.n_dropped == ost["n_dropped"] and st.vis_taps == ost["vis_taps"]
+    assert_parity(got, ref + as_complex(base), ab + np.abs(as_complex(base)), "dense path, accumulate")
+
+    g = _gridder(dev, max_vis=n, env=env, **kw)
+    d_uvw, d_f = torch.from_numpy(uvw).to(dev), torch.tensor([C], dtype=torch.float64, device=dev)
+    d_v, d_w = torch.from_numpy(vis).to(dev), torch.from_numpy(w).to(dev)
+    g.bin(d_uvw, d_f)
+    o1 = g.grid(d_v, d_w).cpu().numpy()
+    o2 = g.grid(d_v, d_w).cpu().numpy()
+    o4 = g.grid(2.0 * d_v, d_w).cpu().numpy()                 # new visibilities on the same binning
+    g.bin(d_uvw, d_f)
+    o3 = g.grid(d_v, d_w).cpu().numpy()
+    g.destroy()
+    assert np.array_equal(o1, o2) and np.array_equal(o1, o3) and np.array_equal(o4, 2.0 * o1)
+    assert_parity(o1, ref, ab, "dense path, bin once grid twice")

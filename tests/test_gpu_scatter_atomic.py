@@ -70,3 +70,18 @@ def test_atomic_scatter_config1_and_binned_path_agree(dev):
     print(f"atomic scatter on config 1: worst err/tol {err.max():.2f} (binned path: "
           f"{(np.abs(as_complex(binned) - ref) / (1e-5 * ab + 1e-6)).max():.3f})")
     assert err.max() < 50.0          # unbounded FP32 chains: reported, loosely bounded, not held to 1e-5
+
+
+def test_sum_parts_is_the_fixed_order_double_sum(dev):
+    """Row f4's kernel: out = (float) sum over parts, in part order, in double; also in place over part 0."""
+    from paper_1003_5575_b200 import mfs
+    rng = np.random.default_rng(41)
+    for n_parts, length in ((1, 4), (2, 1000), (8, 4 * 333), (3, 1 << 20)):
+        parts = (rng.standard_normal((n_parts, length)) * 10.0 ** rng.integers(-3, 4, (n_parts, 1))).astype(np.float32)
+        got = mfs.sum_parts_cuda(torch.from_numpy(parts).to(dev)).cpu().numpy()
+        acc = np.zeros(length, np.float64)
+        for p in range(n_parts):
+            acc += parts[p].astype(np.float64)
+        assert np.array_equal(got, acc.astype(np.float32))
+    with pytest.raises(Exception):
+        mfs.sum_parts_cuda(torch.zeros((2, 6), dtype=torch.float32, device=dev))     # 6 is not a multiple of 4

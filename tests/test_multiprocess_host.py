@@ -75,3 +75,49 @@ def test_shard_plan_rejects_bad_rank_and_reference_arm_is_rank0_only():
     a1 = bench.aggregate([20.0], [1e9], steps=2)
     a2 = bench.aggregate([20.0, 20.0], [1e9, 1e9], steps=2)
     assert np.isclose(a2["value"], 2 * a1["value"])
+
+
+# ---- row f4: the deterministic sum of the per-rank grids (paper_1003_5575_b200/mfs.py) ----------------
+def _sum_parts_cpu(parts):
+    """What gridder_sum_parts computes, written out with torch CPU ops (the tests' stand-in for the kernel)."""
+    acc = torch.zeros(parts.shape[1], dtype=torch.float64)
+    for p in range(parts.shape[0]):
+        acc += parts[p].double()
+    return acc.float()
+
+
+def _mfs_worker(rank, world, port, out_dir, shape):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, str(ROOT))
+    from paper_1003_5575_b200 import mfs
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        grids = [torch.from_numpy(np.random.default_rng(100 + r).standard_normal(shape).astype(np.float32) * 10.0 ** r)
+                 for r in range(world)]
+        mine = grids[rank].clone()
+        out = mfs.reduce_grids(mine, sum_parts=_sum_parts_cpu)
+        assert out is mine
+        expect = torch.zeros(shape, dtype=torch.float64)
+        for r in range(world):                               # rank order, double, one rounding
+            expect += grids[r].double()
+        assert torch.equal(mine, expect.float()), "not the fixed-order FP64 sum"
+        np.save(Path(out_dir) / f"sum{rank}.npy", mine.numpy())
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,shape", [(2, (4, 6, 6, 2)), (3, (4, 5, 5, 2)), (2, (1, 1, 1, 2))])
+def test_reduce_grids_is_the_fixed_order_sum_on_every_rank(tmp_path, world, shape):
+    mp.spawn(_mfs_worker, args=(world, _free_port(), str(tmp_path), shape), nprocs=world, join=True)
+    sums = [np.load(tmp_path / f"sum{r}.npy") for r in range(world)]
+    for s in sums[1:]:
+        assert np.array_equal(s, sums[0])                    # the same bits on every rank
+
+
+def test_slice_len_covers_and_is_float4_aligned():
+    sys.path.insert(0, str(ROOT))
+    from paper_1003_5575_b200 import mfs
+    for numel in (1, 2, 7, 8, 288, 4 * 4096 * 4096 * 2):
+        for world in (1, 2, 3, 8):
+            L = mfs.slice_len(numel, world)
+            assert L % 4 == 0 and world * L >= numel and world * (L - 4) < numel
