@@ -299,6 +299,7 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
         GR_TRY(cudaGetLastError());
         bool by_runs = false;
         p.n_runs = 0;
+        p.fused_bin = 0;
         if (p.run_cap > 0) {
             GR_TRY(launch_bin_runs(p, uvw, scale, n, n_chan, s, &by_runs));
             if (by_runs) {

@@ -1038,6 +1038,269 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
     asm volatile("cp.async.wait_group 0;" ::: "memory");
 }
 
+// The same pre-summation straight from the SORTED CHANNEL RUNS (runs.cu), so that the per-entry sorted
+// list never has to be written (expand_kernel: 3.7 ms and 6.4 GB on config 4) or read.  Entry e of the
+// sorted order belongs to the run r with rcum[r] <= e < rcum[r + 1]; it is visibility start[r] + (e - rcum[r]),
+// its origin is in the run's key and its sub-cell offsets (and drop flag) are the byte qaux[visibility].
+// Batches are cut at multiples of 64 of the global entry position, and blk_run[e / 64] (block_run_kernel)
+// names the run holding position 64 (e / 64): the 64 runs from there on cover the batch (a run has at least
+// one entry), so a lane finds its run by a 6-step search in a window of shared memory.  Four stages run
+// ahead of the adding, each through its own ring: descriptor + blk_run word (6 batches ahead), run window
+// (4), visibilities + weight + qaux word (2).  Same records, same order of additions, same bits as
+// reduce_kernel.
+constexpr int kRunWin = 4, kRunWinU32 = 192;                   // ring of run windows: cum[64], start[64], key[64]
+constexpr int kRunEnt = 3, kRunEntF4 = 2 * (32 * 2 + 8) + 32;  // ring of entries: 2 x (a, b, weight), then okey[64], qword[64]
+constexpr int kRunDesc = 8;
+constexpr int kRunWarps = 11;
+constexpr int kRunWarpF4 = kRedBins * 2 * kRedCopies + kRunEnt * kRunEntF4 + kRunWin * kRunWinU32 / 4 + kRunDesc;
+
+__global__ void __launch_bounds__(kRunWarps * 32, 1) reduce_runs_kernel(const GridParams p) {
+    extern __shared__ float4 smem[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float4 *priv = smem + (size_t)warp * kRunWarpF4;           // [q][half][lane & 15]
+    float4 *ering = priv + kRedBins * 2 * kRedCopies;
+    uint32_t *wring = reinterpret_cast<uint32_t *>(ering + kRunEnt * kRunEntF4);
+    uint4 *dring = reinterpret_cast<uint4 *>(wring + kRunWin * kRunWinU32);
+    for (int i = lane; i < kRunWarpF4; i += 32) priv[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncwarp();
+
+    const int tl2 = 2 * p.key.tlog;
+    const uint32_t omask = (1u << tl2) - 1u, qmask = (1u << (2 * p.key.bits_q)) - 1u;
+    const int dropshift = 2 * p.key.bits_q;
+    const unsigned item_begin = p.counters->cls_begin[p.cls], item_end = p.counters->cls_end[p.cls];
+    // the lane's part in adding the private copies: bin 4 pass + bs, half h, copies 4 g .. 4 g + 3
+    const int g = lane & 3, h = (lane >> 2) & 1, bs = lane >> 3;
+    const int cl = lane & (kRedCopies - 1), rot = h + 2 * (g >> 1);      // (rot: conflict-free reads)
+
+    float4 bacc[4];                      // sums of the bins 4 pass + bs (half h) over the pieces of the origin
+#pragma unroll
+    for (int i = 0; i < 4; ++i) bacc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    unsigned touched = 0;                // this lane's private bins that hold something
+    unsigned occ = 0;                    // bins of the origin that hold something (all pieces)
+    int bin_org = -1, piece = 0;
+    unsigned n_rec = 0;
+    size_t rec_base = 0;
+
+    // ---- the warp's stream of batches: consecutive entries of one work item up to the next multiple of 64
+    // of the global position (lane: positions x + lane and x + 32 + lane).  descriptor: x = first position,
+    // y = count | first batch of its item << 8 | last << 9 | end of stream << 10, z = item, w = blk_run[x / 64]
+    unsigned cur_id = 0, cur_pos = 0, cur_end = 0;                     // the item the batches are cut from
+    bool cur_first = false;
+    unsigned nxt_id = 0, nxt_start = 0, nxt_len = 0;                   // claimed one item ahead
+    bool nxt_ok = false, gen_end = false;
+    auto claim = [&]() {
+        unsigned it = 0;
+        if (lane == 0) it = atomicAdd(&p.counters->queue_head[p.cls], 1u);
+        nxt_id = __shfl_sync(0xffffffffu, it, 0);
+        nxt_ok = item_begin + nxt_id < item_end;
+        nxt_start = nxt_len = 0;
+        if (nxt_ok) {
+            const WorkItem w = p.items[item_begin + nxt_id];
+            nxt_start = w.start;
+            nxt_len = w.len;
+        }
+    };
+    // stage 1, batch m: its descriptor into the ring, the copy of its blk_run word started
+    auto gen_desc = [&](int m) {
+        if (!gen_end && cur_pos >= cur_end) {
+            if (!nxt_ok) gen_end = true;
+            else {
+                cur_id = nxt_id; cur_pos = nxt_start; cur_end = nxt_start + nxt_len; cur_first = true;
+                claim();
+            }
+        }
+        uint4 d = make_uint4(0u, 1u << 10, 0u, 0u);
+        if (!gen_end) {
+            const unsigned stop = min(cur_end, (cur_pos | 63u) + 1u);
+            d.x = cur_pos;
+            d.y = (stop - cur_pos) | (cur_first ? 256u : 0u) | (stop == cur_end ? 512u : 0u);
+            d.z = cur_id;
+            cur_pos = stop;
+            cur_first = false;
+        }
+        uint4 *slot = dring + (m & (kRunDesc - 1));
+        if (lane == 0) {
+            *reinterpret_cast<uint3 *>(slot) = make_uint3(d.x, d.y, d.z);
+            cp_async_4(&slot->w, p.blk_run + (d.x >> 6), !(d.y & 1024u));
+        }
+    };
+    // stage 2, batch m (its blk_run word has landed): the copies of its window of 64 runs started
+    auto gen_window = [&](int m) {
+        const uint4 d = dring[m & (kRunDesc - 1)];
+        uint32_t *w = wring + (m & (kRunWin - 1)) * kRunWinU32;
+        const bool live = !(d.y & 1024u);
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const unsigned r = d.w + 32 * u + lane;
+            const bool v = live && r < p.n_runs;
+            if (v) cp_async_4(w + 32 * u + lane, p.rcum + r, true);
+            else w[32 * u + lane] = 0xFFFFFFFFu;             // beyond the last run: never chosen by the search
+            cp_async_4(w + 64 + 32 * u + lane, p.rstart + 2 * (size_t)(v ? r : 0u), v);
+            cp_async_4(w + 128 + 32 * u + lane, p.rkey + (v ? r : 0u), v);
+        }
+    };
+    // stage 3, batch m (its window has landed): every lane finds the runs of its two entries, notes origin
+    // and byte position, and starts the copies of visibility, weight and the qaux word
+    auto gen_entries = [&](int m, int es) {
+        const uint4 d = dring[m & (kRunDesc - 1)];
+        const uint32_t *w = wring + (m & (kRunWin - 1)) * kRunWinU32;
+        const int cnt = (int)(d.y & 255u);
+        float4 *dst0 = ering + es * kRunEntF4;
+        uint32_t *okey = reinterpret_cast<uint32_t *>(dst0 + 2 * (32 * 2 + 8));
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const bool v = lane + 32 * u < cnt;
+            const unsigned pos = d.x + 32 * u + lane;
+            int j = 0;
+#pragma unroll
+            for (int st = 32; st >= 1; st >>= 1)
+                if (w[j + st] <= pos) j += st;
+            const unsigned idx = v ? w[64 + j] + (pos - w[j]) : 0u;
+            okey[32 * u + lane] = ((w[128 + j] >> p.key.aux_bits) & omask) | ((idx & 3u) << 16);
+            float4 *dst = dst0 + u * (32 * 2 + 8);
+            const float4 *src = p.vis + 2 * (size_t)idx;
+            cp_async_16(dst + lane, src, v);
+            cp_async_16(dst + 32 + lane, src + 1, v);
+            if (p.weight) cp_async_4(reinterpret_cast<float *>(dst + 64) + lane, p.weight + idx, v);
+            cp_async_4(okey + 64 + 32 * u + lane, p.qaux + (idx & ~3u), v);
+        }
+    };
+
+    claim();
+    // iteration n: stages 1, 2, 3 for batches n + 6, n + 4, n + 2 (one cp.async group), batch n is added; the
+    // first six iterations only fill the pipeline
+    int es_n = 0, es_n2 = 2;             // entry-ring slots of batches n and n + 2 (n = -6: any)
+#pragma unroll 1
+    for (int n = -6;; ++n) {
+        asm volatile("cp.async.wait_group 1;" ::: "memory");      // everything up to iteration n - 2 has landed
+        __syncwarp();
+        gen_desc(n + 6);
+        if (n + 4 >= 0) gen_window(n + 4);
+        if (n + 2 >= 0) gen_entries(n + 2, es_n2);
+        cp_async_commit();
+        if (n >= 0) {
+        const uint4 d = dring[n & (kRunDesc - 1)];
+        if (d.y & 1024u) break;
+        const int cnt = (int)(d.y & 255u);
+        {
+            const float4 *rw = ering + es_n * kRunEntF4;
+            const uint32_t *okey = reinterpret_cast<const uint32_t *>(rw + 2 * (32 * 2 + 8));
+            if (d.y & 256u) {            // first batch of an item: where its records go
+                n_rec = 0;
+                rec_base = p.rec_slot ? (size_t)d.z * p.rec_slot : (size_t)d.x;
+            }
+            const uint32_t k0 = okey[lane], k1 = okey[32 + lane];
+            const uint32_t qb0 = (okey[64 + lane] >> (8 * (k0 >> 16))) & 255u;
+            const uint32_t qb1 = (okey[96 + lane] >> (8 * (k1 >> 16))) & 255u;
+            const int org0 = lane < cnt ? (int)(k0 & 0xFFFFu) : -2;
+            const int org1 = lane + 32 < cnt ? (int)(k1 & 0xFFFFu) : -2;
+            const int q0 = (int)(qb0 & qmask), q1 = (int)(qb1 & qmask);
+            const bool drop0 = (qb0 >> dropshift) & 1u, drop1 = (qb1 >> dropshift) & 1u;      // dropped: adds nothing
+            const float w0 = drop0 ? 0.0f : (p.weight ? reinterpret_cast<const float *>(rw + 64)[lane] : 1.0f);
+            const float w1 = drop1 ? 0.0f : (p.weight ? reinterpret_cast<const float *>(rw + (32 * 2 + 8) + 64)[lane] : 1.0f);
+            const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+            const float4 a0 = drop0 ? z4 : rw[lane], b0 = drop0 ? z4 : rw[32 + lane];
+            const float4 a1 = drop1 ? z4 : rw[(32 * 2 + 8) + lane], b1 = drop1 ? z4 : rw[(32 * 2 + 8) + 32 + lane];
+            const bool last = d.y & 512u;
+            int lp = 0;
+            // origin by origin; one more round with no origin ends the item
+#pragma unroll 1
+            while (lp < cnt || (last && lp == cnt)) {
+                const int seg = lp < cnt ? __shfl_sync(0xffffffffu, lp < 32 ? org0 : org1, lp & 31) : -1;
+                const bool change = seg != bin_org;
+                if ((change && bin_org >= 0) || piece >= kRedPiece) {
+                    // ---- the 32 private copies of every touched bin are added into bacc and cleared --------
+                    __syncwarp();
+                    const unsigned u = __reduce_or_sync(0xffffffffu, touched);
+                    occ |= u;
+#pragma unroll
+                    for (int pass = 0; pass < 4; ++pass) {
+                        if (((u >> (4 * pass)) & 15u) == 0u) continue;
+                        const float4 *src = priv + ((4 * pass + bs) * 2 + h) * kRedCopies + 4 * g;
+                        float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            const float4 v = src[(j + rot) & 3];
+                            t.x += v.x; t.y += v.y; t.z += v.z; t.w += v.w;
+                        }
+#pragma unroll
+                        for (int dd = 1; dd < 4; dd <<= 1) {
+                            t.x += __shfl_xor_sync(0xffffffffu, t.x, dd); t.y += __shfl_xor_sync(0xffffffffu, t.y, dd);
+                            t.z += __shfl_xor_sync(0xffffffffu, t.z, dd); t.w += __shfl_xor_sync(0xffffffffu, t.w, dd);
+                        }
+                        bacc[pass].x += t.x; bacc[pass].y += t.y; bacc[pass].z += t.z; bacc[pass].w += t.w;
+                    }
+                    __syncwarp();
+                    for (unsigned m = touched; m; m &= m - 1u) {     // (lanes l and l + 16 may clear the same words)
+                        const int qq = __ffs(m) - 1;
+                        priv[(qq * 2) * kRedCopies + cl] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        priv[(qq * 2 + 1) * kRedCopies + cl] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+                    touched = 0;
+                    piece = 0;
+                    __syncwarp();
+                    if (change) {
+                        // ---- the origin is complete: its non-empty bins become records, in offset order ----
+#pragma unroll
+                        for (int pass = 0; pass < 4; ++pass) {
+                            const int qq = 4 * pass + bs;
+                            if (g == 0 && ((occ >> qq) & 1u)) {
+                                const size_t r = rec_base + n_rec + (unsigned)__popc(occ & ((1u << qq) - 1u));
+                                p.rec_sum[2 * r + h] = bacc[pass];
+                                if (h == 0) p.rec_key[r] = ((uint32_t)bin_org << p.key.aux_bits) | (uint32_t)qq;
+                            }
+                            bacc[pass] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        }
+                        n_rec += (unsigned)__popc(occ);
+                        occ = 0;
+                    }
+                }
+                bin_org = seg;
+                if (lp >= cnt) break;
+                // the lane's two entries: into its copy of the bins (one read-modify-write when they share the
+                // offset); lanes l and l + 16 share a copy, so the two half-warps take turns
+                const bool in0 = org0 == seg, in1 = org1 == seg;
+                const bool same = in0 && in1 && q0 == q1;
+                const bool sep1 = in1 && !same;
+                float4 *pa0 = priv + (q0 * 2) * kRedCopies + cl, *pa1 = priv + (q1 * 2) * kRedCopies + cl;
+#pragma unroll 1
+                for (int ph = 0; ph < 2; ++ph) {
+                    if ((lane >> 4) == ph) {
+                        float4 x0, y0, x1, y1;
+                        x0 = y0 = x1 = y1 = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if (in0) { x0 = pa0[0]; y0 = pa0[kRedCopies]; }
+                        if (sep1) { x1 = pa1[0]; y1 = pa1[kRedCopies]; }
+                        x0.x = fmaf(w0, a0.x, x0.x); x0.y = fmaf(w0, a0.y, x0.y); x0.z = fmaf(w0, a0.z, x0.z); x0.w = fmaf(w0, a0.w, x0.w);
+                        y0.x = fmaf(w0, b0.x, y0.x); y0.y = fmaf(w0, b0.y, y0.y); y0.z = fmaf(w0, b0.z, y0.z); y0.w = fmaf(w0, b0.w, y0.w);
+                        if (same) { x1 = x0; y1 = y0; }
+                        x1.x = fmaf(w1, a1.x, x1.x); x1.y = fmaf(w1, a1.y, x1.y); x1.z = fmaf(w1, a1.z, x1.z); x1.w = fmaf(w1, a1.w, x1.w);
+                        y1.x = fmaf(w1, b1.x, y1.x); y1.y = fmaf(w1, b1.y, y1.y); y1.z = fmaf(w1, b1.z, y1.z); y1.w = fmaf(w1, b1.w, y1.w);
+                        if (in0 && !same) { pa0[0] = x0; pa0[kRedCopies] = y0; }
+                        if (in1) { pa1[0] = x1; pa1[kRedCopies] = y1; }
+                    }
+                    __syncwarp();
+                }
+                if (in0) touched |= 1u << q0;
+                if (in1) touched |= 1u << q1;
+                piece += 2;
+                lp += __popc(__ballot_sync(0xffffffffu, in0)) + __popc(__ballot_sync(0xffffffffu, in1));
+            }
+            if (last && lane == 0) {     // the item's entry in the record items
+                WorkItem ri;
+                ri.start = (uint32_t)rec_base;
+                ri.len = n_rec;
+                ri.tile = 0;
+                ri.pad = 0;
+                p.rec_items[item_begin + d.z] = ri;
+            }
+        }
+        }
+        es_n = es_n + 1 < kRunEnt ? es_n + 1 : 0;
+        es_n2 = es_n2 + 1 < kRunEnt ? es_n2 + 1 : 0;
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+}
+
 // ------------------------------------------------------------------------------------------
 // Flush: one thread per grid cell.  The partial regions covering cell (x, y) belong to the tiles
 // (ty, tx) with tx*T <= x < tx*T + RW (same in y); each tile's work items are added in id order
@@ -1224,6 +1487,9 @@ cudaError_t configure_grid_kernel(Plan &p) {
     if (p.reduce) {
         e = cudaFuncSetAttribute((const void *)reduce_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)(kRedWarps * kRedWarpF4 * sizeof(float4)));
+        if (e == cudaSuccess && p.fuse)
+            e = cudaFuncSetAttribute((const void *)reduce_runs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)(kRunWarps * kRunWarpF4 * sizeof(float4)));
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
@@ -1251,7 +1517,17 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         rp.rec_sum = p.rec_sum;
         rp.rec_items = p.rec_items;
         rp.rec_slot = (uint32_t)p.rec_slot;
-        reduce_kernel<<<p.n_sm, kRedWarps * 32, kRedWarps * kRedWarpF4 * sizeof(float4), s>>>(rp);
+        if (p.fused_bin) {           // binned by runs and not expanded: straight from the sorted runs
+            rp.rkey = p.srun_key;
+            rp.rstart = reinterpret_cast<const uint32_t *>(p.srun_val);
+            rp.rcum = p.run_cum;
+            rp.n_runs = (uint32_t)p.n_runs;
+            rp.qaux = p.qaux;
+            rp.blk_run = p.blk_run;
+            reduce_runs_kernel<<<p.n_sm, kRunWarps * 32, kRunWarps * kRunWarpF4 * sizeof(float4), s>>>(rp);
+        } else {
+            reduce_kernel<<<p.n_sm, kRedWarps * 32, kRedWarps * kRedWarpF4 * sizeof(float4), s>>>(rp);
+        }
         e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaMemsetAsync(p.counters->queue_head, 0, sizeof(unsigned int) * kMaxClasses, s);
         if (e != cudaSuccess) return e;

@@ -124,6 +124,13 @@ struct GridParams {
     float4 *rec_sum;               // [record][2]
     WorkItem *rec_items;           // [item]
     uint32_t rec_slot;             // > 0: item i owns records [i rec_slot, (i + 1) rec_slot); 0: [start, start + len)
+    // reduce_runs_kernel only: the sorted channel runs it reads instead of the per-entry list
+    const uint32_t *rkey;          // [run] sorted key (tile | origin bits, offsets zero)
+    const uint32_t *rstart;        // [run][2]: first visibility (low word of first | length << 32)
+    const uint32_t *rcum;          // [run] position of the run's first entry in the sorted order
+    uint32_t n_runs;
+    const unsigned char *qaux;     // [visibility] sub-cell offsets | drop flag
+    const uint32_t *blk_run;       // [position / 64] last run with rcum <= 64 (position / 64)
 };
 
 struct FlushParams {
@@ -155,6 +162,11 @@ struct Plan {
     int32_t reduce;                // with qbins: the bins are filled by reduce_kernel (reduce.cu), which writes records
     int64_t rec_cap;               // records the arrays below hold
     int64_t rec_slot;              // > 0: records per work item (item i owns [i rec_slot, (i+1) rec_slot)); 0: item.start
+    int32_t fuse;                  // reduce straight from the sorted runs when the bin went by runs (no expansion)
+    int32_t fused_bin;             // the last gridder_bin did: keys[0] / vals[0] were NOT written
+    const uint32_t *srun_key;      // the sorted runs of the last bin (inside run_key / run_val)
+    const unsigned long long *srun_val;
+    uint32_t *blk_run;             // [max_vis / 64 + 2]
     uint32_t *rec_key;             // [rec_cap]
     float4 *rec_sum;               // [rec_cap][2]
     WorkItem *rec_items;           // [max_items]: the work items over the record arrays

@@ -184,6 +184,21 @@ __global__ void __launch_bounds__(256) expand_partition_kernel(const uint32_t *_
     part[b] = lo;
 }
 
+// blk_run[g] = last run with rcum <= 64 g: where reduce_runs_kernel (grid.cu) starts looking for the runs of
+// the entries 64 g .. 64 g + 63 (dense plans read the sorted runs themselves; nothing is expanded)
+__global__ void __launch_bounds__(256) block_run_kernel(const uint32_t *__restrict__ rcum, unsigned int n_runs,
+                                                         unsigned int n_blocks64, uint32_t *__restrict__ blk_run) {
+    const unsigned int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= n_blocks64) return;
+    const unsigned int e0 = g * 64u;
+    unsigned int lo = 0, hi = n_runs;
+    while (hi - lo > 1) {
+        const unsigned int mid = (lo + hi) >> 1;
+        if (rcum[mid] <= e0) lo = mid; else hi = mid;
+    }
+    blk_run[g] = lo;
+}
+
 __global__ void __launch_bounds__(kRunThreads) expand_kernel(const uint32_t *__restrict__ rkey,
                                                               const unsigned long long *__restrict__ rval,
                                                               const uint32_t *__restrict__ rcum, unsigned int n_runs,
@@ -282,6 +297,7 @@ cudaError_t runs_temp_bytes(int64_t cap, int begin_bit, int end_bit, size_t *byt
 cudaError_t launch_bin_runs(Plan &p, const double *uvw, const double *scale, long long n, int n_chan, cudaStream_t s,
                             bool *used) {
     *used = false;
+    p.fused_bin = 0;
     const MapParams mp = make_map_params(p);
     const unsigned int n_blocks = (unsigned int)((n + kRunTile - 1) / kRunTile);
     uint32_t *rkey[2] = {p.run_key[0], p.run_key[1]};
@@ -319,11 +335,21 @@ cudaError_t launch_bin_runs(Plan &p, const double *uvw, const double *scale, lon
     auto it = thrust::make_transform_iterator((const unsigned long long *)v.Current(), RunLen());
     tb = p.cub_temp_bytes;
     GR_TRY(cub::DeviceScan::ExclusiveSum(p.cub_temp, tb, it, p.run_cum, (long long)n_runs, s));
-    expand_partition_kernel<<<(n_blocks + 255) / 256, 256, 0, s>>>(p.run_cum, n_runs, n_blocks, part);
-    GR_TRY(cudaGetLastError());
-    expand_kernel<<<n_blocks, kRunThreads, 0, s>>>(k.Current(), v.Current(), p.run_cum, n_runs, (unsigned)n, part, p.qaux,
-                                                   p.keys[0], (uint32_t *)p.vals[0]);
-    GR_TRY(cudaGetLastError());
+    p.srun_key = k.Current();
+    p.srun_val = v.Current();
+    if (p.fuse) {
+        // dense plan: the pre-summation reads the sorted runs; the per-entry list is never written
+        const unsigned int nb64 = (unsigned int)((n + 63) / 64);
+        block_run_kernel<<<(nb64 + 255) / 256, 256, 0, s>>>(p.run_cum, n_runs, nb64, p.blk_run);
+        GR_TRY(cudaGetLastError());
+        p.fused_bin = 1;
+    } else {
+        expand_partition_kernel<<<(n_blocks + 255) / 256, 256, 0, s>>>(p.run_cum, n_runs, n_blocks, part);
+        GR_TRY(cudaGetLastError());
+        expand_kernel<<<n_blocks, kRunThreads, 0, s>>>(k.Current(), v.Current(), p.run_cum, n_runs, (unsigned)n, part, p.qaux,
+                                                       p.keys[0], (uint32_t *)p.vals[0]);
+        GR_TRY(cudaGetLastError());
+    }
     const int tb_blocks = (int)min((long long)(n_runs + 255) / 256, (long long)p.n_sm * 32);
     tile_bounds_runs_kernel<<<tb_blocks, 256, 0, s>>>(k.Current(), p.run_cum, n_runs, (unsigned)n, p.key.tile_shift,
                                                       p.tile_start, p.tile_start + (size_t)p.n_tiles * p.n_cls);

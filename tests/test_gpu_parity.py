@@ -502,3 +502,25 @@ def test_pre_summation_edge_cases(dev):
     g.destroy()
     assert np.array_equal(o1, o2) and np.array_equal(o1, o3) and np.array_equal(o4, 2.0 * o1)
     assert_parity(o1, ref, ab, "dense path, bin once grid twice")
+
+
+@pytest.mark.parametrize("tlog,chunk", [(2, 256), (3, 4096)])
+def test_pre_summation_straight_from_the_sorted_runs(dev, tlog, chunk):
+    """Dense plan binned by channel runs: reduce_runs_kernel reads the sorted runs (no per-entry list is
+    written) and must produce the same records, hence the same bits, as reduce_kernel on the expanded list."""
+    wl = synth.make_workload(1, n_time=2)
+    vis = wl.visibilities("cpu").numpy()
+    rng = np.random.default_rng(95)
+    w = rng.uniform(0.5, 1.5, vis.shape[:-2]).astype(np.float32)
+    kw = dict(N=wl.grid_size, du=wl.cell_size, O=wl.oversample, S=wl.support[0], table=wl.kernel)
+    env = {"GRIDDER_QBINS": 2, "GRIDDER_RUNS": 2, "GRIDDER_TILE_LOG2": tlog, "GRIDDER_CHUNK": chunk}
+    a, st_a = _run(dev, wl.uvw, wl.freq, vis, w, env=dict(env, GRIDDER_FUSE=1), **kw)
+    a2, _ = _run(dev, wl.uvw, wl.freq, vis, w, env=dict(env, GRIDDER_FUSE=1), **kw)
+    b, st_b = _run(dev, wl.uvw, wl.freq, vis, w, env=dict(env, GRIDDER_FUSE=0), **kw)
+    c, st_c = _run(dev, wl.uvw, wl.freq, vis, w, env=dict(env, GRIDDER_RUNS=0), **kw)
+    assert np.array_equal(a, a2) and np.array_equal(a, b) and np.array_equal(a, c)
+    assert st_a.n_records_gridded == st_b.n_records_gridded == st_c.n_records_gridded
+    assert st_a.n_work_items == st_b.n_work_items and st_a.vis_taps == st_b.vis_taps
+    ref, ab, ost = _oracle(wl.uvw, wl.freq, vis, w, **kw)
+    assert st_a.n_dropped == ost["n_dropped"]
+    assert_parity(a, ref, ab, f"pre-summation from runs T={1 << tlog}")
