@@ -801,8 +801,8 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel_qbins(const GridPara
 // their entries to their bins in turn, so no two lanes ever touch the same word at the same time and
 // there is nothing to match, merge or serialise.
 // When the origin changes (or after 1024 entries, which bounds the FP32 chain of a bin copy at 64) the 16
-// private copies of each touched bin are added in a fixed order -- 4 serial additions in each of four
-// lane groups, then a butterfly -- into registers, and at the end of the origin the non-empty bins are
+// private copies of each bin are added in a fixed order -- lane (q, h) adds the 16 copies of half h of bin
+// q one after the other -- into registers, and at the end of the origin the non-empty bins are
 // written out as records in offset order.  All orders are fixed: reruns are bit-identical.
 // ------------------------------------------------------------------------------------------
 constexpr int kRedWarps = 13, kRedPiece = 32;      // (a copy is shared by two lanes: chains <= 64)
@@ -828,13 +828,11 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
     const uint32_t dropbit = 1u << (2 * p.key.bits_q);
     const unsigned item_begin = p.counters->cls_begin[p.cls], item_end = p.counters->cls_end[p.cls];
     const uint32_t *idx_sorted = reinterpret_cast<const uint32_t *>(p.vals);
-    // the lane's part in adding the private copies: bin 4 pass + bs, half h, copies 4 g .. 4 g + 3
-    const int g = lane & 3, h = (lane >> 2) & 1, bs = lane >> 3;
-    const int cl = lane & (kRedCopies - 1), rot = h + 2 * (g >> 1);      // (rot: conflict-free reads)
+    // the lane's part in adding the private copies: half bh of bin bq (row lane of the [q][half] table)
+    const int bq = lane >> 1, bh = lane & 1;
+    const int cl = lane & (kRedCopies - 1);
 
-    float4 bacc[4];                      // sums of the bins 4 pass + bs (half h) over the pieces of the origin
-#pragma unroll
-    for (int i = 0; i < 4; ++i) bacc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 bacc = make_float4(0.f, 0.f, 0.f, 0.f);     // sum of (bq, bh) over the pieces of the origin
     unsigned touched = 0;                // this lane's private bins that hold something
     unsigned occ = 0;                    // bins of the origin that hold something (all pieces)
     int bin_org = -1, piece = 0;
@@ -947,26 +945,19 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
                 const int seg = lp < cnt ? __shfl_sync(0xffffffffu, lp < 32 ? org0 : org1, lp & 31) : -1;
                 const bool change = seg != bin_org;
                 if ((change && bin_org >= 0) || piece >= kRedPiece) {
-                    // ---- the 32 private copies of every touched bin are added into bacc and cleared --------
+                    // ---- the 16 private copies of every bin are added into bacc and cleared: lane (q, h) adds
+                    // half h of bin q, copy by copy in a fixed (rotated: conflict-free) order
                     __syncwarp();
-                    const unsigned u = __reduce_or_sync(0xffffffffu, touched);
-                    occ |= u;
-#pragma unroll
-                    for (int pass = 0; pass < 4; ++pass) {
-                        if (((u >> (4 * pass)) & 15u) == 0u) continue;
-                        const float4 *src = priv + ((4 * pass + bs) * 2 + h) * kRedCopies + 4 * g;
+                    occ |= __reduce_or_sync(0xffffffffu, touched);
+                    {
+                        const float4 *src = priv + lane * kRedCopies;        // row (q * 2 + h) = lane
                         float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const float4 v = src[(j + rot) & 3];
+                        for (int j = 0; j < kRedCopies; ++j) {
+                            const float4 v = src[(j + lane) & (kRedCopies - 1)];
                             t.x += v.x; t.y += v.y; t.z += v.z; t.w += v.w;
                         }
-#pragma unroll
-                        for (int dd = 1; dd < 4; dd <<= 1) {
-                            t.x += __shfl_xor_sync(0xffffffffu, t.x, dd); t.y += __shfl_xor_sync(0xffffffffu, t.y, dd);
-                            t.z += __shfl_xor_sync(0xffffffffu, t.z, dd); t.w += __shfl_xor_sync(0xffffffffu, t.w, dd);
-                        }
-                        bacc[pass].x += t.x; bacc[pass].y += t.y; bacc[pass].z += t.z; bacc[pass].w += t.w;
+                        bacc.x += t.x; bacc.y += t.y; bacc.z += t.z; bacc.w += t.w;
                     }
                     __syncwarp();
                     for (unsigned m = touched; m; m &= m - 1u) {     // (lanes l and l + 16 may clear the same words)
@@ -979,16 +970,12 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
                     __syncwarp();
                     if (change) {
                         // ---- the origin is complete: its non-empty bins become records, in offset order ----
-#pragma unroll
-                        for (int pass = 0; pass < 4; ++pass) {
-                            const int qq = 4 * pass + bs;
-                            if (g == 0 && ((occ >> qq) & 1u)) {
-                                const size_t r = rec_base + n_rec + (unsigned)__popc(occ & ((1u << qq) - 1u));
-                                p.rec_sum[2 * r + h] = bacc[pass];
-                                if (h == 0) p.rec_key[r] = ((uint32_t)bin_org << p.key.aux_bits) | (uint32_t)qq;
-                            }
-                            bacc[pass] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if ((occ >> bq) & 1u) {
+                            const size_t r = rec_base + n_rec + (unsigned)__popc(occ & ((1u << bq) - 1u));
+                            p.rec_sum[2 * r + bh] = bacc;
+                            if (bh == 0) p.rec_key[r] = ((uint32_t)bin_org << p.key.aux_bits) | (uint32_t)bq;
                         }
+                        bacc = make_float4(0.f, 0.f, 0.f, 0.f);
                         n_rec += (unsigned)__popc(occ);
                         occ = 0;
                     }
@@ -1068,13 +1055,11 @@ __global__ void __launch_bounds__(kRunWarps * 32, 1) reduce_runs_kernel(const Gr
     const uint32_t omask = (1u << tl2) - 1u, qmask = (1u << (2 * p.key.bits_q)) - 1u;
     const int dropshift = 2 * p.key.bits_q;
     const unsigned item_begin = p.counters->cls_begin[p.cls], item_end = p.counters->cls_end[p.cls];
-    // the lane's part in adding the private copies: bin 4 pass + bs, half h, copies 4 g .. 4 g + 3
-    const int g = lane & 3, h = (lane >> 2) & 1, bs = lane >> 3;
-    const int cl = lane & (kRedCopies - 1), rot = h + 2 * (g >> 1);      // (rot: conflict-free reads)
+    // the lane's part in adding the private copies: half bh of bin bq (row lane of the [q][half] table)
+    const int bq = lane >> 1, bh = lane & 1;
+    const int cl = lane & (kRedCopies - 1);
 
-    float4 bacc[4];                      // sums of the bins 4 pass + bs (half h) over the pieces of the origin
-#pragma unroll
-    for (int i = 0; i < 4; ++i) bacc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 bacc = make_float4(0.f, 0.f, 0.f, 0.f);     // sum of (bq, bh) over the pieces of the origin
     unsigned touched = 0;                // this lane's private bins that hold something
     unsigned occ = 0;                    // bins of the origin that hold something (all pieces)
     int bin_org = -1, piece = 0;
@@ -1209,26 +1194,19 @@ __global__ void __launch_bounds__(kRunWarps * 32, 1) reduce_runs_kernel(const Gr
                 const int seg = lp < cnt ? __shfl_sync(0xffffffffu, lp < 32 ? org0 : org1, lp & 31) : -1;
                 const bool change = seg != bin_org;
                 if ((change && bin_org >= 0) || piece >= kRedPiece) {
-                    // ---- the 32 private copies of every touched bin are added into bacc and cleared --------
+                    // ---- the 16 private copies of every bin are added into bacc and cleared: lane (q, h) adds
+                    // half h of bin q, copy by copy in a fixed (rotated: conflict-free) order
                     __syncwarp();
-                    const unsigned u = __reduce_or_sync(0xffffffffu, touched);
-                    occ |= u;
-#pragma unroll
-                    for (int pass = 0; pass < 4; ++pass) {
-                        if (((u >> (4 * pass)) & 15u) == 0u) continue;
-                        const float4 *src = priv + ((4 * pass + bs) * 2 + h) * kRedCopies + 4 * g;
+                    occ |= __reduce_or_sync(0xffffffffu, touched);
+                    {
+                        const float4 *src = priv + lane * kRedCopies;        // row (q * 2 + h) = lane
                         float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const float4 v = src[(j + rot) & 3];
+                        for (int j = 0; j < kRedCopies; ++j) {
+                            const float4 v = src[(j + lane) & (kRedCopies - 1)];
                             t.x += v.x; t.y += v.y; t.z += v.z; t.w += v.w;
                         }
-#pragma unroll
-                        for (int dd = 1; dd < 4; dd <<= 1) {
-                            t.x += __shfl_xor_sync(0xffffffffu, t.x, dd); t.y += __shfl_xor_sync(0xffffffffu, t.y, dd);
-                            t.z += __shfl_xor_sync(0xffffffffu, t.z, dd); t.w += __shfl_xor_sync(0xffffffffu, t.w, dd);
-                        }
-                        bacc[pass].x += t.x; bacc[pass].y += t.y; bacc[pass].z += t.z; bacc[pass].w += t.w;
+                        bacc.x += t.x; bacc.y += t.y; bacc.z += t.z; bacc.w += t.w;
                     }
                     __syncwarp();
                     for (unsigned m = touched; m; m &= m - 1u) {     // (lanes l and l + 16 may clear the same words)
@@ -1241,16 +1219,12 @@ __global__ void __launch_bounds__(kRunWarps * 32, 1) reduce_runs_kernel(const Gr
                     __syncwarp();
                     if (change) {
                         // ---- the origin is complete: its non-empty bins become records, in offset order ----
-#pragma unroll
-                        for (int pass = 0; pass < 4; ++pass) {
-                            const int qq = 4 * pass + bs;
-                            if (g == 0 && ((occ >> qq) & 1u)) {
-                                const size_t r = rec_base + n_rec + (unsigned)__popc(occ & ((1u << qq) - 1u));
-                                p.rec_sum[2 * r + h] = bacc[pass];
-                                if (h == 0) p.rec_key[r] = ((uint32_t)bin_org << p.key.aux_bits) | (uint32_t)qq;
-                            }
-                            bacc[pass] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        if ((occ >> bq) & 1u) {
+                            const size_t r = rec_base + n_rec + (unsigned)__popc(occ & ((1u << bq) - 1u));
+                            p.rec_sum[2 * r + bh] = bacc;
+                            if (bh == 0) p.rec_key[r] = ((uint32_t)bin_org << p.key.aux_bits) | (uint32_t)bq;
                         }
+                        bacc = make_float4(0.f, 0.f, 0.f, 0.f);
                         n_rec += (unsigned)__popc(occ);
                         occ = 0;
                     }
