@@ -986,15 +986,13 @@ __global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridPar
                 // offset); lanes l and l + 16 share a copy, so the two half-warps take turns
                 const bool in0 = org0 == seg, in1 = org1 == seg;
                 const bool same = in0 && in1 && q0 == q1;
-                const bool sep1 = in1 && !same;
                 float4 *pa0 = priv + (q0 * 2) * kRedCopies + cl, *pa1 = priv + (q1 * 2) * kRedCopies + cl;
 #pragma unroll 1
                 for (int ph = 0; ph < 2; ++ph) {
                     if ((lane >> 4) == ph) {
-                        float4 x0, y0, x1, y1;
-                        x0 = y0 = x1 = y1 = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (in0) { x0 = pa0[0]; y0 = pa0[kRedCopies]; }
-                        if (sep1) { x1 = pa1[0]; y1 = pa1[kRedCopies]; }
+                        // (the addresses are valid whatever the lane holds: loads are unconditional, stores are not)
+                        float4 x0 = pa0[0], y0 = pa0[kRedCopies];
+                        float4 x1 = pa1[0], y1 = pa1[kRedCopies];
                         x0.x = fmaf(w0, a0.x, x0.x); x0.y = fmaf(w0, a0.y, x0.y); x0.z = fmaf(w0, a0.z, x0.z); x0.w = fmaf(w0, a0.w, x0.w);
                         y0.x = fmaf(w0, b0.x, y0.x); y0.y = fmaf(w0, b0.y, y0.y); y0.z = fmaf(w0, b0.z, y0.z); y0.w = fmaf(w0, b0.w, y0.w);
                         if (same) { x1 = x0; y1 = y0; }
@@ -1235,15 +1233,13 @@ __global__ void __launch_bounds__(kRunWarps * 32, 1) reduce_runs_kernel(const Gr
                 // offset); lanes l and l + 16 share a copy, so the two half-warps take turns
                 const bool in0 = org0 == seg, in1 = org1 == seg;
                 const bool same = in0 && in1 && q0 == q1;
-                const bool sep1 = in1 && !same;
                 float4 *pa0 = priv + (q0 * 2) * kRedCopies + cl, *pa1 = priv + (q1 * 2) * kRedCopies + cl;
 #pragma unroll 1
                 for (int ph = 0; ph < 2; ++ph) {
                     if ((lane >> 4) == ph) {
-                        float4 x0, y0, x1, y1;
-                        x0 = y0 = x1 = y1 = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (in0) { x0 = pa0[0]; y0 = pa0[kRedCopies]; }
-                        if (sep1) { x1 = pa1[0]; y1 = pa1[kRedCopies]; }
+                        // (the addresses are valid whatever the lane holds: loads are unconditional, stores are not)
+                        float4 x0 = pa0[0], y0 = pa0[kRedCopies];
+                        float4 x1 = pa1[0], y1 = pa1[kRedCopies];
                         x0.x = fmaf(w0, a0.x, x0.x); x0.y = fmaf(w0, a0.y, x0.y); x0.z = fmaf(w0, a0.z, x0.z); x0.w = fmaf(w0, a0.w, x0.w);
                         y0.x = fmaf(w0, b0.x, y0.x); y0.y = fmaf(w0, b0.y, y0.y); y0.z = fmaf(w0, b0.z, y0.z); y0.w = fmaf(w0, b0.w, y0.w);
                         if (same) { x1 = x0; y1 = y0; }
