@@ -39,12 +39,12 @@ BAND_HZ = 768 * 40.0e3           # one rank's band; rank r starts at 140 MHz + r
 # dram__bytes_read.sum + dram__bytes_write.sum of one grid_kernel launch from the committed
 # `ncu --set full` capture (profiles/), keyed by config; None until a capture exists for it.
 NCU_GRID_KERNEL_TRAFFIC_BYTES = {
-    4: 4_180_064_000,     # profiles/r01f_grid_kernel_on_records_config4_ncu_full.csv: 1.765172 GB read + 2.414892 GB written
+    4: 4_177_715_000,     # profiles/r01f_grid_kernel_on_records_config4_ncu_full.csv: 1.763335 GB read + 2.414380 GB written
     2: 9_348_989_000,     # profiles/r01_grid_kernel_config2_ncu_full.csv: 4.109023 GB read + 5.239966 GB written
 }
 # the same for reduce_kernel (dense plans: it is the longest kernel of the step there)
 NCU_REDUCE_KERNEL_TRAFFIC_BYTES = {
-    4: 50_353_096_000,    # profiles/r01f_reduce_kernel_config4_ncu_full.csv: 48.612657 GB read + 1.740439 GB written
+    4: 50_401_785_000,    # profiles/r01f_reduce_kernel_config4_ncu_full.csv: 48.661029 GB read + 1.740756 GB written
 }
 
 
