@@ -45,12 +45,12 @@ int derive(const gridder_config *cfg, Plan &p) {
     const bool cplx = cfg->kernel_is_complex != 0;
     // fast path: one real table with S <= 16 (shared-memory table, 32-bit sort values)
     p.mode = cplx ? 2 : ((cfg->n_wplanes == 1 && cfg->support[0] <= 16 && !env_int("GRIDDER_FORCE_GENERAL", 0)) ? 0 : 1);
-    // DENSE plans -- fast path, 16-cell patch, O^2 <= 64, 256 visibilities and more per 4 x 4 cells -- sum the
+    // DENSE plans -- fast path, 16-cell patch, O^2 <= 64, 64 visibilities and more per 4 x 4 cells -- sum the
     // entries of equal (origin, offset) before gridding (GRIDDER_QBINS: 0 never, 1 by density, 2 always)
     const int64_t oo_early = (int64_t)cfg->oversample * cfg->oversample;
     const int qb_mode = env_int("GRIDDER_QBINS", 1);
     const bool dense = p.mode == 0 && cfg->support[0] > 8 && oo_early <= 64 && env_int("GRIDDER_MERGE", 1) &&
-                       (qb_mode >= 2 || (qb_mode == 1 && cfg->max_vis * 16 / ((int64_t)cfg->grid_size * cfg->grid_size) >= 256));
+                       (qb_mode >= 2 || (qb_mode == 1 && cfg->max_vis * 16 / ((int64_t)cfg->grid_size * cfg->grid_size) >= 64));
     // ... and with the pre-summation kernel (O^2 <= 16) larger tiles and longer work items pay: the work per
     // item follows its (origin, offset) pairs, not its entries, and the flush has fewer regions to add
     const bool dense_reduce = dense && oo_early <= 16 && env_int("GRIDDER_REDUCE", 1);
