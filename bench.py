@@ -40,7 +40,7 @@ BAND_HZ = 768 * 40.0e3           # one rank's band; rank r starts at 140 MHz + r
 # `ncu --set full` capture (profiles/), keyed by config; None until a capture exists for it.
 NCU_GRID_KERNEL_TRAFFIC_BYTES = {
     4: 4_177_715_000,     # profiles/r01f_grid_kernel_on_records_config4_ncu_full.csv: 1.763335 GB read + 2.414380 GB written
-    2: 9_348_989_000,     # profiles/r01_grid_kernel_config2_ncu_full.csv: 4.109023 GB read + 5.239966 GB written
+    2: 3_500_273_000,     # profiles/r01f_grid_kernel_on_records_config2_ncu_full.csv: 1.150321 GB read + 2.349952 GB written
 }
 # the same for reduce_kernel (dense plans: it is the longest kernel of the step there)
 NCU_REDUCE_KERNEL_TRAFFIC_BYTES = {
