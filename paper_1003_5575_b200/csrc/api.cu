@@ -215,7 +215,6 @@ cudaError_t carve(Plan &p, char *base) {
         p.qaux = (unsigned char *)take(n);
         for (int i = 0; i < 2; ++i) p.run_key[i] = (uint32_t *)take(cap * sizeof(uint32_t));
         for (int i = 0; i < 2; ++i) p.run_val[i] = (unsigned long long *)take(cap * sizeof(unsigned long long));
-        p.run_start = (uint32_t *)take(cap * sizeof(uint32_t));
         p.run_cum = (uint32_t *)take(cap * sizeof(uint32_t));
         p.run_blk = (unsigned int *)take(3 * ((n + 1023) / 1024 + 1) * sizeof(unsigned int));
     }

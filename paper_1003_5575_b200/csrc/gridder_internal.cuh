@@ -186,7 +186,7 @@ struct Plan {
     unsigned char *qaux;           // [n]: the key's unsorted low bits (sub-cell offsets, drop flag) per visibility
     uint32_t *run_key[2];          // [run_cap] x 2 (sort double buffer)
     unsigned long long *run_val[2];// [run_cap] x 2: first index | length << 32
-    uint32_t *run_start, *run_cum; // [run_cap]
+    uint32_t *run_cum;             // [run_cap]
     unsigned int *run_blk;         // [3][ceil(n / 1024) + 1]: runs per map block, their scan, expand partition
     uint32_t *tile_start;          // [2][n_vtiles]: first entry | one past the last entry
     unsigned long long *tile_chunks, *tile_chunks_scan;   // packed (n_full << 32 | has_tail), [n_vtiles+1]

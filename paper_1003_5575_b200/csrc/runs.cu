@@ -6,8 +6,8 @@
 //   map_runs_kernel   exact map of every visibility (same device function as the classic path);
 //                     writes its sub-cell offsets / drop flag (1 byte) and, for every run start,
 //                     (sort key, first index) into the block's own staging slots, plus the block's count
-//   exclusive scan    of the block counts; compact_runs_kernel moves the staged runs to their place
-//   run_len_kernel    value = first index | length << 32
+//   exclusive scan    of the block counts; compact_runs_kernel moves the staged runs to their place as
+//                     (key, first index | length << 32)
 //   radix sort        (key u32, value u64) over the runs, stable: equal keys stay in index order
 //   exclusive scan    entries before each sorted run
 //   expand_kernel     sorted runs -> the per-entry sorted (key, index) arrays of the classic path
@@ -136,29 +136,32 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
     }
 }
 
-// One warp per map block: its staged runs move to [prefix, prefix + count) of the compact arrays.
+// One warp per map block: its staged runs move to [prefix, prefix + count) of the compact arrays, as
+// (key, first index | length << 32); a run ends where the next one starts -- the next staged start of the
+// block, or the first start of the next block that has one, or n.
 __global__ void __launch_bounds__(256) compact_runs_kernel(const uint32_t *__restrict__ stage_key,
                                                             const uint32_t *__restrict__ stage_start,
                                                             const unsigned int *__restrict__ block_count,
                                                             const unsigned int *__restrict__ block_prefix,
-                                                            unsigned int n_blocks, uint32_t *__restrict__ rkey,
-                                                            uint32_t *__restrict__ rstart) {
+                                                            unsigned int n_blocks, unsigned int n,
+                                                            uint32_t *__restrict__ rkey,
+                                                            unsigned long long *__restrict__ rval) {
     const unsigned int b = blockIdx.x * 8 + (threadIdx.x >> 5);
     if (b >= n_blocks) return;
     const unsigned int cnt = block_count[b], dst = block_prefix[b], src = b * (unsigned)kRunTile;
-    for (unsigned int j = threadIdx.x & 31; j < cnt; j += 32) {
-        rkey[dst + j] = stage_key[src + j];
-        rstart[dst + j] = stage_start[src + j];
+    if (cnt == 0) return;
+    unsigned int next_first = n;
+    if ((threadIdx.x & 31) == 0) {
+        for (unsigned int bb = b + 1; bb < n_blocks; ++bb)
+            if (block_count[bb] > 0) { next_first = stage_start[bb * (unsigned)kRunTile]; break; }
     }
-}
-
-__global__ void __launch_bounds__(256) run_len_kernel(const uint32_t *__restrict__ rstart, unsigned int n_runs,
-                                                       unsigned int n, unsigned long long *__restrict__ rval) {
-    const unsigned int g = blockIdx.x * blockDim.x + threadIdx.x;
-    if (g >= n_runs) return;
-    const unsigned int st = rstart[g];
-    const unsigned int nx = g + 1 < n_runs ? rstart[g + 1] : n;
-    rval[g] = (unsigned long long)st | ((unsigned long long)(nx - st) << 32);
+    next_first = __shfl_sync(0xffffffffu, next_first, 0);
+    for (unsigned int j = threadIdx.x & 31; j < cnt; j += 32) {
+        const unsigned int st = stage_start[src + j];
+        const unsigned int nx = j + 1 < cnt ? stage_start[src + j + 1] : next_first;
+        rkey[dst + j] = stage_key[src + j];
+        rval[dst + j] = (unsigned long long)st | ((unsigned long long)(nx - st) << 32);
+    }
 }
 
 struct RunLen {
@@ -323,9 +326,7 @@ cudaError_t launch_bin_runs(Plan &p, const double *uvw, const double *scale, lon
     p.n_runs = n_runs;
     if ((long long)n_runs > p.run_cap) return cudaSuccess;          // too fragmented: classic path
     compact_runs_kernel<<<(n_blocks + 7) / 8, 256, 0, s>>>(stage_key, stage_start, block_count, block_prefix, n_blocks,
-                                                           rkey[0], p.run_start);
-    GR_TRY(cudaGetLastError());
-    run_len_kernel<<<(n_runs + 255) / 256, 256, 0, s>>>(p.run_start, n_runs, (unsigned)n, rval[0]);
+                                                           (unsigned)n, rkey[0], rval[0]);
     GR_TRY(cudaGetLastError());
     stage_mark(p, 1, s);
     cub::DoubleBuffer<uint32_t> k(rkey[0], rkey[1]);
@@ -355,7 +356,7 @@ cudaError_t launch_bin_runs(Plan &p, const double *uvw, const double *scale, lon
                                                       p.tile_start, p.tile_start + (size_t)p.n_tiles * p.n_cls);
     GR_TRY(cudaGetLastError());
     p.sorted_sel = 0;
-    p.n_launches += 7;
+    p.n_launches += 6;
     *used = true;
     return cudaSuccess;
 }
