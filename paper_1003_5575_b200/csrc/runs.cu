@@ -207,7 +207,9 @@ __global__ void __launch_bounds__(kRunThreads) expand_kernel(const uint32_t *__r
                                                               const uint32_t *__restrict__ rcum, unsigned int n_runs,
                                                               unsigned int n, const unsigned int *__restrict__ part,
                                                               const unsigned char *__restrict__ qaux,
-                                                              uint32_t *__restrict__ keys, uint32_t *__restrict__ vals) {
+                                                              uint32_t *__restrict__ keys, uint32_t *__restrict__ vals,
+                                                              int tile_shift, uint32_t *__restrict__ tile_start,
+                                                              uint32_t *__restrict__ tile_end) {
     __shared__ uint32_t s_cum[kRunTile + 1], s_key[kRunTile], s_start[kRunTile];
     __shared__ unsigned int s_cnt;
     const unsigned int e0 = blockIdx.x * (unsigned)kRunTile;
@@ -221,10 +223,19 @@ __global__ void __launch_bounds__(kRunThreads) expand_kernel(const uint32_t *__r
             const uint32_t c = rcum[r];
             if (c < e1) {
                 const unsigned long long v = rval[r];
+                const uint32_t key = rkey[r];
                 s_cum[j] = c;
-                s_key[j] = rkey[r];
+                s_key[j] = key;
                 s_start[j] = (unsigned int)v;
                 mine = j + 1;
+                if (c >= e0) {
+                    // the run starts in this block: the block notes where its tile starts and ends (the paper's
+                    // 'first' / 'last' tables, :197; what tile_bounds_runs_kernel does on its own)
+                    const uint32_t t = key >> tile_shift;
+                    if (r == 0 || (rkey[r - 1] >> tile_shift) != t) tile_start[t] = c;
+                    if (r == n_runs - 1) tile_end[t] = n;
+                    else if ((rkey[r + 1] >> tile_shift) != t) tile_end[t] = rcum[r + 1];
+                }
             }
         }
     }
@@ -348,15 +359,18 @@ cudaError_t launch_bin_runs(Plan &p, const double *uvw, const double *scale, lon
         expand_partition_kernel<<<(n_blocks + 255) / 256, 256, 0, s>>>(p.run_cum, n_runs, n_blocks, part);
         GR_TRY(cudaGetLastError());
         expand_kernel<<<n_blocks, kRunThreads, 0, s>>>(k.Current(), v.Current(), p.run_cum, n_runs, (unsigned)n, part, p.qaux,
-                                                       p.keys[0], (uint32_t *)p.vals[0]);
+                                                       p.keys[0], (uint32_t *)p.vals[0], p.key.tile_shift, p.tile_start,
+                                                       p.tile_start + (size_t)p.n_tiles * p.n_cls);
         GR_TRY(cudaGetLastError());
     }
-    const int tb_blocks = (int)min((long long)(n_runs + 255) / 256, (long long)p.n_sm * 32);
-    tile_bounds_runs_kernel<<<tb_blocks, 256, 0, s>>>(k.Current(), p.run_cum, n_runs, (unsigned)n, p.key.tile_shift,
-                                                      p.tile_start, p.tile_start + (size_t)p.n_tiles * p.n_cls);
-    GR_TRY(cudaGetLastError());
+    if (p.fuse) {                    // (expand_kernel builds the tile tables on its way)
+        const int tb_blocks = (int)min((long long)(n_runs + 255) / 256, (long long)p.n_sm * 32);
+        tile_bounds_runs_kernel<<<tb_blocks, 256, 0, s>>>(k.Current(), p.run_cum, n_runs, (unsigned)n, p.key.tile_shift,
+                                                          p.tile_start, p.tile_start + (size_t)p.n_tiles * p.n_cls);
+        GR_TRY(cudaGetLastError());
+    }
     p.sorted_sel = 0;
-    p.n_launches += 6;
+    p.n_launches += 5;
     *used = true;
     return cudaSuccess;
 }
