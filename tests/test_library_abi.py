@@ -67,6 +67,14 @@ def test_null_and_invalid_arguments_need_no_device(lib):
     assert lib.gridder_grid(None, None, None, None, 0, None) == gridder.ERR_INVALID_ARG
     assert lib.gridder_destroy(None) == gridder.ERR_INVALID_ARG
     assert lib.gridder_get_stats(None, None) == gridder.ERR_INVALID_ARG
+    # row f4's summation kernel: argument checks come before any CUDA call
+    buf = C.c_void_p(256)
+    assert lib.gridder_sum_parts(None, 2, 8, 8, buf, None) == gridder.ERR_INVALID_ARG
+    assert lib.gridder_sum_parts(buf, 0, 8, 8, buf, None) == gridder.ERR_INVALID_ARG          # no parts
+    assert lib.gridder_sum_parts(buf, 2, 6, 8, buf, None) == gridder.ERR_INVALID_ARG          # len not a multiple of 4
+    assert lib.gridder_sum_parts(buf, 2, 8, 4, buf, None) == gridder.ERR_INVALID_ARG          # stride < len
+    assert lib.gridder_sum_parts(C.c_void_p(260), 2, 8, 8, buf, None) == gridder.ERR_INVALID_ARG   # misaligned
+    assert lib.gridder_sum_parts(buf, 2, 0, 0, buf, None) == gridder.OK                       # nothing to do
 
 
 def test_binding_refuses_cpu_tensors():
