@@ -524,3 +524,33 @@ def test_pre_summation_straight_from_the_sorted_runs(dev, tlog, chunk):
     ref, ab, ost = _oracle(wl.uvw, wl.freq, vis, w, **kw)
     assert st_a.n_dropped == ost["n_dropped"]
     assert_parity(a, ref, ab, f"pre-summation from runs T={1 << tlog}")
+
+
+def test_dense_path_randomised_sweep(dev):
+    """60 seeded random small problems through every variant of the dense path (pre-summation from the expanded
+    list or from the runs, bins inside the grid kernel, table in shared or tensor memory; tiles 4/8/16; chunks
+    down to one batch; counts around the 32- and 64-entry batch sizes; lattice ties; with and without weights)."""
+    rng = np.random.default_rng(2024)
+    for it in range(60):
+        S = int(rng.choice([9, 10, 12, 13, 15, 16]))
+        O = int(rng.choice([1, 2, 4])) if S % 2 == 0 else int(rng.choice([2, 4]))
+        N = int(rng.choice([48, 64, 96, 130]))
+        n = int(rng.choice([1, 31, 32, 33, 63, 64, 65, 127, 128, 129, 1000, 4097, 20000]))
+        spread = float(rng.choice([0.4, 2.0, 8.0, N / 2 + 1]))
+        table = rng.standard_normal((S * O, S * O)).astype(np.float32)
+        uvw = np.zeros((1, n, 3))
+        uvw[0, :, :2] = rng.uniform(-spread, spread, (n, 2))
+        if rng.random() < 0.3:
+            uvw[0, :, :2] = np.round(uvw[0, :, :2] * O) / O
+        vis = rng.standard_normal((n, 4, 2)).astype(np.float32)
+        w = None if rng.random() < 0.3 else rng.uniform(0.0, 1.5, n).astype(np.float32)
+        kw = dict(N=N, du=1.0, O=O, S=S, table=table)
+        env = {"GRIDDER_QBINS": 2, "GRIDDER_TILE_LOG2": int(rng.choice([2, 3, 4])),
+               "GRIDDER_CHUNK": int(rng.choice([32, 64, 100, 256, 4096])), "GRIDDER_RUNS": int(rng.choice([0, 2])),
+               "GRIDDER_FUSE": int(rng.choice([0, 1])), "GRIDDER_TMEM": int(rng.choice([0, 1])),
+               "GRIDDER_REDUCE": int(rng.choice([0, 1, 1]))}
+        got, st = _run(dev, uvw, [C], vis, w, env=env, **kw)
+        ref, ab, ost = _oracle(uvw, [C], vis, w, **kw)
+        assert st.n_dropped == ost["n_dropped"] and st.vis_taps == ost["vis_taps"], (it, env)
+        assert 0 < st.n_records_gridded <= st.n_vis, (it, env)        # (dropped visibilities end in a record of zeros)
+        assert_parity(got, ref, ab, f"sweep case {it} {env}")
