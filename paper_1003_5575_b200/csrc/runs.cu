@@ -22,7 +22,8 @@
 
 namespace gridder {
 
-constexpr int kRunThreads = 256, kRunItems = 4, kRunTile = kRunThreads * kRunItems;
+constexpr int kRunThreads = 256, kRunItems = 4, kRunTile = kRunThreads * kRunItems;     // expansion: entries per block
+constexpr int kMapItems = 8, kMapTile = kRunThreads * kMapItems;                       // map: visibilities per block
 
 template <bool FAST>
 __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__restrict__ uvw,
@@ -37,7 +38,7 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
     __shared__ unsigned int s_warp[kRunThreads / 32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned int bid = blockIdx.x;
-    const unsigned int base = bid * (unsigned)kRunTile + (unsigned)tid * kRunItems;    // n <= 2^32 - 4096: no wrap
+    const unsigned int base = bid * (unsigned)kMapTile + (unsigned)tid * kMapItems;    // n <= 2^32 - 4096: no wrap
     const uint32_t aux_mask = (1u << p.key.aux_bits) - 1u;
     FastMap fm;
     if (FAST) fm.init(p);
@@ -58,9 +59,9 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
         int taps;
         prev = key_of(L, scale[f], taps) >> p.key.aux_bits;
     }
-    uint32_t sk[kRunItems];
-    unsigned int fch[kRunItems];
-    unsigned char q[kRunItems];
+    uint32_t sk[kMapItems];
+    unsigned int fch[kMapItems];
+    unsigned char q[kMapItems];
     unsigned int dropped_here = 0;
     unsigned long long taps_here = 0;
     // (integration, baseline) row and channel of the thread's first visibility; the next ones by increment
@@ -70,7 +71,7 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
         f = base - tb * n_chan;
     }
 #pragma unroll
-    for (int k = 0; k < kRunItems; ++k) {
+    for (int k = 0; k < kMapItems; ++k) {
         sk[k] = 0xFFFFFFFFu; fch[k] = 1; q[k] = 0;
         if (base + k < n) {
             const double *L = uvw + (size_t)tb * 3;
@@ -83,21 +84,24 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
             if (++f == n_chan) { f = 0; ++tb; }
         }
     }
-    if (base + kRunItems <= n) {
-        *reinterpret_cast<uchar4 *>(qaux + base) = make_uchar4(q[0], q[1], q[2], q[3]);
+    if (base + kMapItems <= n) {
+        static_assert(kMapItems == 8, "the offsets of a thread's visibilities are stored as one 8-byte word");
+        *reinterpret_cast<uint2 *>(qaux + base) =
+            make_uint2((uint32_t)q[0] | ((uint32_t)q[1] << 8) | ((uint32_t)q[2] << 16) | ((uint32_t)q[3] << 24),
+                       (uint32_t)q[4] | ((uint32_t)q[5] << 8) | ((uint32_t)q[6] << 16) | ((uint32_t)q[7] << 24));
     } else {
 #pragma unroll
-        for (int k = 0; k < kRunItems; ++k)
+        for (int k = 0; k < kMapItems; ++k)
             if (base + k < n) qaux[base + k] = q[k];
     }
     // the sort key of the visibility just before this thread's first one
-    s_last[tid] = sk[kRunItems - 1];
+    s_last[tid] = sk[kMapItems - 1];
     __syncthreads();
     if (tid > 0) prev = s_last[tid - 1];
     // run starts: first channel of a (t, b) row, or a different [tile | origin] than the previous channel
     unsigned int flags = 0, cnt = 0;
 #pragma unroll
-    for (int k = 0; k < kRunItems; ++k) {
+    for (int k = 0; k < kMapItems; ++k) {
         const bool st = (base + k < n) && (fch[k] == 0 || sk[k] != prev);
         if (st) { flags |= 1u << k; cnt++; }
         prev = sk[k];
@@ -117,10 +121,10 @@ __global__ void __launch_bounds__(kRunThreads) map_runs_kernel(const double *__r
         total += s_warp[w];
     }
     if (tid == 0) block_count[bid] = total;
-    // the block's runs go to its own slots (a block of kRunTile visibilities has at most kRunTile runs)
-    unsigned int pos = bid * (unsigned)kRunTile + woff + incl - cnt;
+    // the block's runs go to its own slots (a block of kMapTile visibilities has at most kMapTile runs)
+    unsigned int pos = bid * (unsigned)kMapTile + woff + incl - cnt;
 #pragma unroll
-    for (int k = 0; k < kRunItems; ++k)
+    for (int k = 0; k < kMapItems; ++k)
         if (flags & (1u << k)) {
             stage_key[pos] = sk[k] << p.key.aux_bits;
             stage_start[pos] = base + k;
@@ -148,12 +152,12 @@ __global__ void __launch_bounds__(256) compact_runs_kernel(const uint32_t *__res
                                                             unsigned long long *__restrict__ rval) {
     const unsigned int b = blockIdx.x * 8 + (threadIdx.x >> 5);
     if (b >= n_blocks) return;
-    const unsigned int cnt = block_count[b], dst = block_prefix[b], src = b * (unsigned)kRunTile;
+    const unsigned int cnt = block_count[b], dst = block_prefix[b], src = b * (unsigned)kMapTile;
     if (cnt == 0) return;
     unsigned int next_first = n;
     if ((threadIdx.x & 31) == 0) {
         for (unsigned int bb = b + 1; bb < n_blocks; ++bb)
-            if (block_count[bb] > 0) { next_first = stage_start[bb * (unsigned)kRunTile]; break; }
+            if (block_count[bb] > 0) { next_first = stage_start[bb * (unsigned)kMapTile]; break; }
     }
     next_first = __shfl_sync(0xffffffffu, next_first, 0);
     for (unsigned int j = threadIdx.x & 31; j < cnt; j += 32) {
@@ -313,30 +317,31 @@ cudaError_t launch_bin_runs(Plan &p, const double *uvw, const double *scale, lon
     *used = false;
     p.fused_bin = 0;
     const MapParams mp = make_map_params(p);
-    const unsigned int n_blocks = (unsigned int)((n + kRunTile - 1) / kRunTile);
+    const unsigned int n_blocks = (unsigned int)((n + kRunTile - 1) / kRunTile);       // expansion blocks
+    const unsigned int n_mblocks = (unsigned int)((n + kMapTile - 1) / kMapTile);      // map blocks
     uint32_t *rkey[2] = {p.run_key[0], p.run_key[1]};
     unsigned long long *rval[2] = {p.run_val[0], p.run_val[1]};
     // staging slots: the second sort buffers of the classic path, which this path does not sort with
     uint32_t *stage_key = p.keys[1], *stage_start = (uint32_t *)p.vals[1];
     unsigned int *block_count = p.run_blk, *block_prefix = p.run_blk + (n_blocks + 1), *part = p.run_blk + 2 * (n_blocks + 1);
-    GR_TRY(cudaMemsetAsync(block_count + n_blocks, 0, sizeof(unsigned int), s));
+    GR_TRY(cudaMemsetAsync(block_count + n_mblocks, 0, sizeof(unsigned int), s));
     if (mp.o_shift >= 0 && mp.drop_slot == 0)
-        map_runs_kernel<true><<<n_blocks, kRunThreads, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp, p.qaux,
+        map_runs_kernel<true><<<n_mblocks, kRunThreads, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp, p.qaux,
                                                                 stage_key, stage_start, block_count, p.counters);
     else
-        map_runs_kernel<false><<<n_blocks, kRunThreads, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp, p.qaux,
+        map_runs_kernel<false><<<n_mblocks, kRunThreads, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp, p.qaux,
                                                                  stage_key, stage_start, block_count, p.counters);
     GR_TRY(cudaGetLastError());
     size_t tb = p.cub_temp_bytes;
     GR_TRY(cub::DeviceScan::ExclusiveSum(p.cub_temp, tb, (const unsigned int *)block_count, block_prefix,
-                                         (long long)n_blocks + 1, s));
+                                         (long long)n_mblocks + 1, s));
     p.n_launches += 2;
     unsigned int n_runs = 0;
-    GR_TRY(cudaMemcpyAsync(&n_runs, block_prefix + n_blocks, sizeof(unsigned int), cudaMemcpyDeviceToHost, s));
+    GR_TRY(cudaMemcpyAsync(&n_runs, block_prefix + n_mblocks, sizeof(unsigned int), cudaMemcpyDeviceToHost, s));
     GR_TRY(cudaStreamSynchronize(s));
     p.n_runs = n_runs;
     if ((long long)n_runs > p.run_cap) return cudaSuccess;          // too fragmented: classic path
-    compact_runs_kernel<<<(n_blocks + 7) / 8, 256, 0, s>>>(stage_key, stage_start, block_count, block_prefix, n_blocks,
+    compact_runs_kernel<<<(n_mblocks + 7) / 8, 256, 0, s>>>(stage_key, stage_start, block_count, block_prefix, n_mblocks,
                                                            (unsigned)n, rkey[0], rval[0]);
     GR_TRY(cudaGetLastError());
     stage_mark(p, 1, s);
