@@ -223,9 +223,11 @@ __global__ void __launch_bounds__(kRunThreads) expand_kernel(const uint32_t *__r
     unsigned int mine = 0;
     for (unsigned int j = threadIdx.x; j < (unsigned)kRunTile; j += kRunThreads) {
         const unsigned int r = r0 + j;
-        if (r < n_runs) {
+        if (r >= n_runs) break;
+        {
             const uint32_t c = rcum[r];
-            if (c < e1) {
+            if (c >= e1) break;                            // rcum ascends: no later run starts inside the block
+            {
                 const unsigned long long v = rval[r];
                 const uint32_t key = rkey[r];
                 s_cum[j] = c;
