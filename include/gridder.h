@@ -102,6 +102,10 @@ typedef struct {
     /* of the last gridder_grid (0 before the first): */
     int64_t n_records_gridded;  /* records the grid kernels processed: entries with equal patch origin and
                                    table offset inside a batch of 32 are summed first (exact by linearity) */
+    int64_t n_presum_records;   /* > 0: the last gridder_bin pre-summed the visibilities in input order into this
+                                   many partial records (one per lattice point met by a group of 32 channels x 8
+                                   integrations of a baseline); tiles, work items and max_tile_load then count
+                                   records, not visibilities                                                */
     int64_t fma_executed;       /* FP32 FMAs those records cost, padded taps included: records x patch cells
                                    x 8 (real table) or 16 (complex): what the roofline fraction is claimed on */
 } gridder_stats;

@@ -49,12 +49,17 @@ int derive(const gridder_config *cfg, Plan &p) {
     // entries of equal (origin, offset) before gridding (GRIDDER_QBINS: 0 never, 1 by density, 2 always)
     const int64_t oo_early = (int64_t)cfg->oversample * cfg->oversample;
     const int qb_mode = env_int("GRIDDER_QBINS", 1);
-    const bool dense = p.mode == 0 && cfg->support[0] > 8 && oo_early <= 64 && env_int("GRIDDER_MERGE", 1) &&
+    // PRE-SUMMATION IN INPUT ORDER (presum.cu; GRIDDER_PRESUM: 0 never, 1 plans of 4 Mi visibilities and more,
+    // 2 always): replaces the sorted-entry paths below
+    const int ps_mode = env_int("GRIDDER_PRESUM", 1);
+    p.presum = (p.mode == 0 && env_int("GRIDDER_MERGE", 1) && 2 * ceil_log2((unsigned long long)cfg->oversample) + 1 <= 8 &&
+                (ps_mode >= 2 || (ps_mode == 1 && cfg->max_vis >= (4ll << 20)))) ? 1 : 0;
+    const bool dense = !p.presum && p.mode == 0 && cfg->support[0] > 8 && oo_early <= 64 && env_int("GRIDDER_MERGE", 1) &&
                        (qb_mode >= 2 || (qb_mode == 1 && cfg->max_vis * 16 / ((int64_t)cfg->grid_size * cfg->grid_size) >= 64));
     // ... and with the pre-summation kernel (O^2 <= 16) larger tiles and longer work items pay: the work per
     // item follows its (origin, offset) pairs, not its entries, and the flush has fewer regions to add
     const bool dense_reduce = dense && oo_early <= 16 && env_int("GRIDDER_REDUCE", 1);
-    p.tlog = env_int("GRIDDER_TILE_LOG2", dense_reduce ? 3 : 2);
+    p.tlog = env_int("GRIDDER_TILE_LOG2", (dense_reduce || p.presum) ? 3 : 2);
     if (p.tlog < 2 || p.tlog > 4) return GRIDDER_ERR_INVALID_ARG;
     p.T = 1 << p.tlog;
     p.ntx = (cfg->grid_size + p.T - 1) / p.T;
@@ -105,7 +110,7 @@ int derive(const gridder_config *cfg, Plan &p) {
     // 10), 8 % faster on the records of a dense plan, where the shared-memory path is the busiest unit: on by
     // default there, off elsewhere.
     p.tmem_cols = 0;
-    if (p.mode == 0 && env_int("GRIDDER_TMEM", dense_reduce ? 1 : 0)) {
+    if (p.mode == 0 && env_int("GRIDDER_TMEM", (dense_reduce || p.presum) ? 1 : 0)) {
         const size_t cols = oo * p.cls[0].NA * p.cls[0].NB;
         if (cols <= 512) {
             p.tmem_cols = 32;
@@ -117,7 +122,7 @@ int derive(const gridder_config *cfg, Plan &p) {
     // GRIDDER_RUNS: 0 never, 1 (default) for plans of 4 M visibilities and more -- below that the per-visibility
     // sort is cheap and the run path's one host synchronisation is not --, 2 always
     const int runs_mode = env_int("GRIDDER_RUNS", 1);
-    if (p.mode == 0 && (runs_mode >= 2 || (runs_mode == 1 && cfg->max_vis >= (4ll << 20))) &&
+    if (p.mode == 0 && !p.presum && (runs_mode >= 2 || (runs_mode == 1 && cfg->max_vis >= (4ll << 20))) &&
         2 * ceil_log2((unsigned long long)cfg->oversample) + 1 <= 8) {
         p.run_cap = cfg->max_vis / 4;
         if (p.run_cap < 1024) p.run_cap = 1024;
@@ -170,6 +175,13 @@ int derive(const gridder_config *cfg, Plan &p) {
         if (p.rec_cap < (1ll << 32)) p.reduce = 1;
     }
     if (!p.reduce && p.tmem_cols > 0) p.qbins = 0;       // (grid_kernel_qbins reads its table from shared memory)
+    if (p.presum) {
+        // record sums: room for 3/4 of the visibilities (inputs that merge less take the per-visibility path);
+        // the plan kernel's staging slots live in the same array
+        p.rec_cap = n * 3 / 4 + 1024;
+        p.ps_stage_cap = p.rec_cap * 8;
+        p.ps_group_cap = n * 3 / 16 + 1024;
+    }
     // GRIDDER_FUSE=1 (with the pre-summation and the run binning; opt-in): reduce straight from the sorted runs,
     // the per-entry sorted list is not written.  Measured on config 4: binning 3.4 ms shorter, reduce 4.6 ms
     // longer (a run search per entry, one more gather, fewer warps): not a gain, so off by default.
@@ -194,6 +206,11 @@ cudaError_t carve(Plan &p, char *base) {
     size_t t1 = 0, t2 = 0;
     cudaError_t e = sort_temp_bytes((int64_t)n, p.key.aux_bits, p.key.total_bits, p.mode != 0, &t1);
     if (e == cudaSuccess) e = scan_temp_bytes((int64_t)n_vtiles + 1, &t2);
+    if (e == cudaSuccess && p.presum) {
+        size_t t3 = 0;
+        e = presum_scan_temp_bytes(p.ps_group_cap + 1, &t3);
+        if (t3 > t2) t2 = t3;
+    }
     if (e == cudaSuccess && p.run_cap > 0) {
         size_t t3 = 0;
         e = runs_temp_bytes(p.run_cap, p.key.aux_bits, p.key.total_bits, &t3);
@@ -225,6 +242,12 @@ cudaError_t carve(Plan &p, char *base) {
     p.tile_cover = (unsigned char *)take((size_t)p.n_tiles);
     p.items = (WorkItem *)take(sizeof(WorkItem) * (size_t)p.max_items);
     p.partials = (float4 *)take(sizeof(float4) * (size_t)p.partials_f4);
+    if (p.presum) {
+        p.ps_flags = (unsigned char *)take(n);
+        p.ps_count = (uint32_t *)take(sizeof(uint32_t) * (size_t)(p.ps_group_cap + 1));
+        p.ps_base = (uint32_t *)take(sizeof(uint32_t) * (size_t)(p.ps_group_cap + 1));
+        p.rec_sum = (float4 *)take(sizeof(float4) * 2 * (size_t)p.rec_cap);
+    }
     if (p.reduce) {
         p.rec_key = (uint32_t *)take(sizeof(uint32_t) * (size_t)p.rec_cap);
         p.rec_sum = (float4 *)take(sizeof(float4) * 2 * (size_t)p.rec_cap);
@@ -355,6 +378,7 @@ int gridder_get_stats(gridder_plan_t *plan, gridder_stats *out) {
     out->patch_size = p->cls[p->n_cls - 1].SP;
     out->chunk_size = p->chunk;
     out->grid_warps_per_sm = p->cls[p->n_cls - 1].warps;
+    out->n_presum_records = p->presum_active ? p->n_sorted : 0;
     for (int k = 0; k < p->n_cls; ++k) {
         const ClassGeo &g = p->cls[k];
         out->n_records_gridded += (int64_t)c.n_exec[k];
@@ -529,7 +553,7 @@ int gridder_get_stage_ms(gridder_plan_t *plan, float *ms_out) {
             e = cudaEventElapsedTime(&ms, p->ev[r][4 + i], p->ev[r][5 + i]);
             sum[3 + i] += ms;
         }
-        if (p->reduce && e == cudaSuccess) {           // the pre-summation's share of the grid stage
+        if ((p->reduce || p->presum_active) && e == cudaSuccess) {           // the pre-summation's share of the grid stage
             float ms = 0.f;
             e = cudaEventElapsedTime(&ms, p->ev[r][4], p->ev[r][7]);
             sum[5] += ms;

@@ -300,7 +300,36 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
         bool by_runs = false;
         p.n_runs = 0;
         p.fused_bin = 0;
-        if (p.run_cap > 0) {
+        p.presum_active = 0;
+        p.n_sorted = n;
+        if (p.presum && !table_index && presum_fits(p, n_time, n_bl, n_chan)) {
+            // pre-summation in input order (presum.cu): flags per visibility, keys per partial record; the
+            // RECORDS are what is sorted and gridded.  Inputs that merge too little take the per-visibility path.
+            long long n_rec = 0;
+            GR_TRY(launch_presum_plan(p, uvw, scale, n_time, n_bl, n_chan, s, &n_rec));
+            if (n_rec <= p.rec_cap) {
+                stage_mark(p, 1, s);
+                cub::DoubleBuffer<uint32_t> k(p.keys[0], p.keys[1]);
+                cub::DoubleBuffer<uint32_t> v((uint32_t *)p.vals[0], (uint32_t *)p.vals[1]);
+                size_t tb = p.cub_temp_bytes;
+                GR_TRY(cub::DeviceRadixSort::SortPairs(p.cub_temp, tb, k, v, n_rec, p.key.aux_bits, p.key.total_bits, s));
+                p.sorted_sel = k.selector;
+                p.n_launches += 1;
+                stage_mark(p, 2, s);
+                p.presum_active = 1;
+                p.n_sorted = n_rec;
+                p.ps_n_time = n_time; p.ps_n_bl = n_bl; p.ps_n_chan = n_chan;
+                by_runs = true;          // (skips the per-visibility map and sort below)
+                if (n_rec > 0) {
+                    tile_bounds_kernel<<<blocks_for(n_rec, 256, p.n_sm), 256, 0, s>>>(p.keys[p.sorted_sel], n_rec,
+                                                                                      p.key.tile_shift, p.tile_start, tile_end);
+                    GR_TRY(cudaGetLastError());
+                }
+            } else {
+                GR_TRY(cudaMemsetAsync(p.counters, 0, 2 * sizeof(unsigned long long), s));   // counted again below
+            }
+        }
+        if (p.run_cap > 0 && !p.presum_active) {
             GR_TRY(launch_bin_runs(p, uvw, scale, n, n_chan, s, &by_runs));
             if (by_runs) {
                 stage_mark(p, 2, s);

@@ -1504,6 +1504,11 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         p.n_launches += 1;
         stage_mark(p, 7, s);
     }
+    if (p.presum_active) {           // sum the visibilities into the records of the plan, in input order
+        e = launch_presum(p, vis, weight, s);
+        if (e != cudaSuccess) return e;
+        stage_mark(p, 7, s);
+    }
     for (int c = 0; c < p.n_cls; ++c) {
         const ClassGeo &g = p.cls[c];
         grid_fn_t gfn = pick_grid(g, p.tlog, kernel_mode(p), kernel_qbins(p));
@@ -1533,6 +1538,11 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
             gp.weight = nullptr;
             gp.merge = 0;
             if (gp.fold_mask > 3) gp.fold_mask = 3;      // a record is a sum already: shorter register chains
+        }
+        if (p.presum_active) {       // the sorted list names records: their sums are the "visibilities"
+            gp.vis = p.rec_sum;
+            gp.weight = nullptr;
+            if (gp.fold_mask > 3) gp.fold_mask = 3;
         }
         gfn<<<p.n_sm, g.warps * 32, g.smem_bytes, s>>>(gp);
         e = cudaGetLastError();

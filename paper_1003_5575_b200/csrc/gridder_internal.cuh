@@ -170,6 +170,15 @@ struct Plan {
     uint32_t *rec_key;             // [rec_cap]
     float4 *rec_sum;               // [rec_cap][2]
     WorkItem *rec_items;           // [max_items]: the work items over the record arrays
+    // pre-summation in input order (presum.cu); presum == 0: not used by this plan
+    int32_t presum;
+    int32_t presum_active;         // the last gridder_bin took it: keys / vals hold the sorted RECORDS
+    int64_t ps_group_cap;          // room for this many groups (count / base arrays)
+    int64_t ps_stage_cap;          // uint32 staging slots (they live in rec_sum, which is written later)
+    int32_t ps_n_time, ps_n_bl, ps_n_chan;     // shape of the last bin
+    int64_t n_sorted;              // entries of the sorted list of the last bin (records, or visibilities)
+    unsigned char *ps_flags;       // [max_vis] one flag byte per visibility
+    uint32_t *ps_count, *ps_base;  // [ps_group_cap + 1] records per group and their exclusive scan
     int32_t fold_batches;          // longest FP32 register chain, in batches of 32 entries (power of 2)
     int32_t warps_forced, n_sm;
     int64_t max_items;             // capacity of the work-item table (all classes)
@@ -241,6 +250,13 @@ cudaError_t runs_temp_bytes(int64_t cap, int begin_bit, int end_bit, size_t *byt
 cudaError_t launch_bin_runs(Plan &p, const double *uvw, const double *scale, long long n, int n_chan, cudaStream_t s,
                             bool *used);
 cudaError_t scan_temp_bytes(int64_t n, size_t *bytes);
+
+// presum.cu
+bool presum_fits(const Plan &p, int n_time, int n_bl, int n_chan);
+cudaError_t presum_scan_temp_bytes(int64_t n, size_t *bytes);
+cudaError_t launch_presum_plan(Plan &p, const double *uvw, const double *scale, int n_time, int n_bl, int n_chan,
+                               cudaStream_t s, long long *n_rec);
+cudaError_t launch_presum(Plan &p, const float *vis, const float *weight, cudaStream_t s);
 
 // image.cu
 int image_workspace(Plan &p, size_t *bytes);

@@ -42,7 +42,7 @@ class _Stats(C.Structure):
                 ("vis_taps", C.c_int64), ("n_tiles", C.c_int64), ("n_tiles_occupied", C.c_int64),
                 ("max_tile_load", C.c_int64), ("n_work_items", C.c_int64), ("tile_size", C.c_int32),
                 ("patch_size", C.c_int32), ("chunk_size", C.c_int32), ("grid_warps_per_sm", C.c_int32),
-                ("n_records_gridded", C.c_int64), ("fma_executed", C.c_int64)]
+                ("n_records_gridded", C.c_int64), ("n_presum_records", C.c_int64), ("fma_executed", C.c_int64)]
 
 
 _lib = None
@@ -125,6 +125,7 @@ class Stats:
     chunk_size: int
     grid_warps_per_sm: int
     n_records_gridded: int = 0
+    n_presum_records: int = 0
     fma_executed: int = 0
 
 
