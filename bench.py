@@ -460,7 +460,7 @@ def run_ours(args) -> dict | None:
                    "tile": st.tile_size, "chunk": st.chunk_size, "work_items": st.n_work_items,
                    "grid_warps_per_sm": st.grid_warps_per_sm},
         "gflops": flop_per_tap * agg["value"] / 1e9,
-        "stage_ms": stage, "grid_only_ms": stage["grid"] + stage["flush"] + stage.get("reduce", 0.0),     # gridder_grid alone (a bin serves many)
+        "stage_ms": stage, "grid_only_ms": stage["grid"] + stage["flush"] + stage.get("reduce", 0.0) + stage.get("presum", 0.0),     # gridder_grid alone (a bin serves many)
         "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
         "cadence_budget_s": 8.0, "result_checksum": checksum,
     }

@@ -201,8 +201,9 @@ GRIDDER_API int gridder_run_host(gridder_plan_t *plan, const double *h_uvw_m, in
  * they run on (a few microseconds of host time per call; nothing else changes). */
 GRIDDER_API int gridder_set_profiling(gridder_plan_t *plan, int32_t enable);
 /* Mean device milliseconds per stage over the gridder_bin / gridder_grid calls made since
- * profiling was enabled (the last 32 of each at most), HOST float [6]: map, sort, tile tables,
- * grid kernel, flush kernel, pre-summation kernel (dense plans; 0 otherwise).  Synchronises on
+ * profiling was enabled (the last 32 of each at most), HOST float [7]: map, sort, tile tables,
+ * grid kernel, flush kernel, input-order pre-summation kernel, per-origin summation kernel (0 for plans that
+ * do not run them).  Synchronises on
  * the recorded events.  A stage that has not run since then reads 0.  Enabling again resets
  * the averages. */
 GRIDDER_API int gridder_get_stage_ms(gridder_plan_t *plan, float *ms_out);

@@ -178,8 +178,8 @@ int derive(const gridder_config *cfg, Plan &p) {
     if (p.presum) {
         // record sums: room for 3/4 of the visibilities (inputs that merge less take the per-visibility path);
         // the plan kernel's staging slots live in the same array
-        p.rec_cap = n * 3 / 4 + 1024;
-        p.ps_stage_cap = p.rec_cap * 8;
+        p.ps_cap = n * 3 / 4 + 1024;
+        p.ps_stage_cap = p.ps_cap * 8;
         p.ps_group_cap = n * 3 / 16 + 1024;
     }
     // GRIDDER_FUSE=1 (with the pre-summation and the run binning; opt-in): reduce straight from the sorted runs,
@@ -246,7 +246,7 @@ cudaError_t carve(Plan &p, char *base) {
         p.ps_flags = (unsigned char *)take(n);
         p.ps_count = (uint32_t *)take(sizeof(uint32_t) * (size_t)(p.ps_group_cap + 1));
         p.ps_base = (uint32_t *)take(sizeof(uint32_t) * (size_t)(p.ps_group_cap + 1));
-        p.rec_sum = (float4 *)take(sizeof(float4) * 2 * (size_t)p.rec_cap);
+        p.ps_sum = (float4 *)take(sizeof(float4) * 2 * (size_t)p.ps_cap);
     }
     if (p.reduce) {
         p.rec_key = (uint32_t *)take(sizeof(uint32_t) * (size_t)p.rec_cap);
@@ -352,7 +352,7 @@ int gridder_destroy(gridder_plan_t *plan) {
     image_destroy(*p);
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
     for (int r = 0; r < kProfRing; ++r)
-        for (int i = 0; i < 8; ++i) if (p->ev[r][i]) cudaEventDestroy(p->ev[r][i]);
+        for (int i = 0; i < 10; ++i) if (p->ev[r][i]) cudaEventDestroy(p->ev[r][i]);
     delete p;
     return e == cudaSuccess ? GRIDDER_OK : GRIDDER_ERR_CUDA;
 }
@@ -523,7 +523,7 @@ int gridder_set_profiling(gridder_plan_t *plan, int32_t enable) {
     if (!p) return GRIDDER_ERR_INVALID_ARG;
     if (enable && !p->ev[0][0]) {
         for (int r = 0; r < kProfRing; ++r)
-            for (int i = 0; i < 8; ++i)
+            for (int i = 0; i < 10; ++i)
                 if (cudaEventCreate(&p->ev[r][i]) != cudaSuccess) return cuda_fail(p, cudaGetLastError());
     }
     p->profiling = enable != 0;
@@ -534,7 +534,7 @@ int gridder_set_profiling(gridder_plan_t *plan, int32_t enable) {
 int gridder_get_stage_ms(gridder_plan_t *plan, float *ms_out) {
     Plan *p = reinterpret_cast<Plan *>(plan);
     if (!p || !ms_out) return GRIDDER_ERR_INVALID_ARG;
-    double sum[6] = {0, 0, 0, 0, 0, 0};
+    double sum[7] = {0, 0, 0, 0, 0, 0, 0};
     const int nb = (int)(p->prof_bin_calls < kProfRing ? p->prof_bin_calls : kProfRing);
     const int ng = (int)(p->prof_grid_calls < kProfRing ? p->prof_grid_calls : kProfRing);
     cudaError_t e = cudaSuccess;
@@ -548,21 +548,26 @@ int gridder_get_stage_ms(gridder_plan_t *plan, float *ms_out) {
     }
     for (int r = 0; r < ng && e == cudaSuccess; ++r) {
         e = cudaEventSynchronize(p->ev[r][6]);
-        for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
-            float ms = 0.f;
-            e = cudaEventElapsedTime(&ms, p->ev[r][4 + i], p->ev[r][5 + i]);
-            sum[3 + i] += ms;
-        }
-        if ((p->reduce || p->presum_active) && e == cudaSuccess) {           // the pre-summation's share of the grid stage
-            float ms = 0.f;
-            e = cudaEventElapsedTime(&ms, p->ev[r][4], p->ev[r][7]);
+        // events of a grid call, in stream order: 4, [7 after the input-order pre-summation], [8 after the
+        // per-origin summation], 5 after the grid kernels, 6 after the flush
+        int last = 4;
+        float ms = 0.f;
+        if (p->presum_active && e == cudaSuccess) {
+            e = cudaEventElapsedTime(&ms, p->ev[r][last], p->ev[r][7]);
             sum[5] += ms;
-            sum[3] -= ms;
+            last = 7;
         }
+        if (p->reduce && e == cudaSuccess) {
+            e = cudaEventElapsedTime(&ms, p->ev[r][last], p->ev[r][8]);
+            sum[6] += ms;
+            last = 8;
+        }
+        if (e == cudaSuccess) { e = cudaEventElapsedTime(&ms, p->ev[r][last], p->ev[r][5]); sum[3] += ms; }
+        if (e == cudaSuccess) { e = cudaEventElapsedTime(&ms, p->ev[r][5], p->ev[r][6]); sum[4] += ms; }
     }
     if (e != cudaSuccess) return cuda_fail(p, e);
     for (int i = 0; i < 3; ++i) ms_out[i] = nb ? (float)(sum[i] / nb) : 0.f;
-    for (int i = 3; i < 6; ++i) ms_out[i] = ng ? (float)(sum[i] / ng) : 0.f;
+    for (int i = 3; i < 7; ++i) ms_out[i] = ng ? (float)(sum[i] / ng) : 0.f;
     return GRIDDER_OK;
 }
 

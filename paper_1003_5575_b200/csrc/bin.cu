@@ -307,7 +307,7 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
             // RECORDS are what is sorted and gridded.  Inputs that merge too little take the per-visibility path.
             long long n_rec = 0;
             GR_TRY(launch_presum_plan(p, uvw, scale, n_time, n_bl, n_chan, s, &n_rec));
-            if (n_rec <= p.rec_cap) {
+            if (n_rec <= p.ps_cap) {
                 stage_mark(p, 1, s);
                 cub::DoubleBuffer<uint32_t> k(p.keys[0], p.keys[1]);
                 cub::DoubleBuffer<uint32_t> v((uint32_t *)p.vals[0], (uint32_t *)p.vals[1]);

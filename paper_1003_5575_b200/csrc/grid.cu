@@ -1472,6 +1472,11 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
     cudaError_t e = cudaMemsetAsync(p.counters->queue_head, 0, sizeof(unsigned int) * kMaxClasses, s);
     if (e == cudaSuccess) e = cudaMemsetAsync(p.counters->n_exec, 0, sizeof(unsigned long long) * kMaxClasses, s);
     if (e != cudaSuccess) return e;
+    if (p.presum_active) {           // sum the visibilities into the partial records of the plan, in input order
+        e = launch_presum(p, vis, weight, s);
+        if (e != cudaSuccess) return e;
+        stage_mark(p, 7, s);
+    }
     if (p.reduce) {                  // sum the entries into records first; the grid kernel then takes those
         GridParams rp;
         memset(&rp, 0, sizeof(rp));
@@ -1481,6 +1486,10 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         rp.counters = p.counters;
         rp.vis = reinterpret_cast<const float4 *>(vis);
         rp.weight = weight;
+        if (p.presum_active) {       // the sorted list names partial records: their sums are the "visibilities"
+            rp.vis = p.ps_sum;
+            rp.weight = nullptr;
+        }
         rp.key = p.key;
         rp.cls = 0;
         rp.rec_key = p.rec_key;
@@ -1502,12 +1511,7 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         if (e == cudaSuccess) e = cudaMemsetAsync(p.counters->queue_head, 0, sizeof(unsigned int) * kMaxClasses, s);
         if (e != cudaSuccess) return e;
         p.n_launches += 1;
-        stage_mark(p, 7, s);
-    }
-    if (p.presum_active) {           // sum the visibilities into the records of the plan, in input order
-        e = launch_presum(p, vis, weight, s);
-        if (e != cudaSuccess) return e;
-        stage_mark(p, 7, s);
+        stage_mark(p, 8, s);
     }
     for (int c = 0; c < p.n_cls; ++c) {
         const ClassGeo &g = p.cls[c];
@@ -1539,8 +1543,8 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
             gp.merge = 0;
             if (gp.fold_mask > 3) gp.fold_mask = 3;      // a record is a sum already: shorter register chains
         }
-        if (p.presum_active) {       // the sorted list names records: their sums are the "visibilities"
-            gp.vis = p.rec_sum;
+        if (p.presum_active && !p.reduce) {       // the sorted list names partial records: their sums are the "visibilities"
+            gp.vis = p.ps_sum;
             gp.weight = nullptr;
             if (gp.fold_mask > 3) gp.fold_mask = 3;
         }

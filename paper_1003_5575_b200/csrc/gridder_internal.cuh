@@ -174,7 +174,9 @@ struct Plan {
     int32_t presum;
     int32_t presum_active;         // the last gridder_bin took it: keys / vals hold the sorted RECORDS
     int64_t ps_group_cap;          // room for this many groups (count / base arrays)
-    int64_t ps_stage_cap;          // uint32 staging slots (they live in rec_sum, which is written later)
+    int64_t ps_cap;                // partial records the plan has room for
+    float4 *ps_sum;                // [ps_cap][2] sum of w V per partial record (written by gridder_grid)
+    int64_t ps_stage_cap;          // uint32 staging slots (they live in ps_sum, which is written later)
     int32_t ps_n_time, ps_n_bl, ps_n_chan;     // shape of the last bin
     int64_t n_sorted;              // entries of the sorted list of the last bin (records, or visibilities)
     unsigned char *ps_flags;       // [max_vis] one flag byte per visibility
@@ -216,7 +218,7 @@ struct Plan {
     int last_cuda_error;
     // harness support: stage timers and a launch counter
     bool profiling;
-    cudaEvent_t ev[kProfRing][8];  // per call: bin: 0 map 1 sort 2 tables 3 | grid: 4 (reduce 7) grid 5 flush 6
+    cudaEvent_t ev[kProfRing][10]; // per call: bin: 0 map 1 sort 2 tables 3 | grid: 4 (presum 7) (reduce 8) grid 5 flush 6
     int64_t prof_bin_calls, prof_grid_calls;       // since profiling was enabled
     int64_t n_launches;
     cudaStream_t copy_stream;      // gridder_run_host: host-to-device copies of the next slice

@@ -178,4 +178,65 @@ struct FastMap {
     }
 };
 
+// The production mapper of the pre-summed path: ONE fused multiply-add per axis.  Per channel the scale
+// ks = RN(RN(s rcp_cell) O) is formed once (O a power of two: the last product is exact); per visibility and axis
+//     t1 = RN(coord_m ks + (N/2 O + 1/2)).
+// With H = coord_m s / du O + N/2 O the exact position in sub-cells and u = 2^-53:
+//   the definition's t = RN(h + 1/2), h from four roundings, lies within 5.01 u (|H| + N O / 2 + 1) of H + 1/2;
+//   t1 (three roundings in ks, one in the FMA) lies within (3.01 |H| + 2.01 N O / 2 + 1) u of it;
+// so |t1 - t| < 8.1 u (|H| + N O / 2 + 1) < 2^-48.7 N O for |H| < 2 N O, and floor(t1) = floor(t) whenever t1 is
+// farther than eps = 2^-47 N O from every integer -- the same margin FastMap uses, five times the bound.  Anything
+// closer (about one visibility in 10^8, and every exact tie) or farther out than 2 N O goes to map_vis: the result
+// is the definition's bit for bit by construction.  floor and the distance to the nearest integer come from the
+// 1.5 * 2^52 trick: m = RN(t1 + M) holds RN(t1) in its low mantissa bits, d = t1 - (m - M) is exact.
+struct FastMap2 {
+    double rcp_cell, d_o, chalf, eps, span2;
+    int o_shift, o_minus_1, half_so, n_minus_s, s2;
+    uint32_t ntx, tmask, tlog, aux_bits, bits_q, tile_shift;
+
+    __device__ __forceinline__ void init(const MapParams &p) {
+        rcp_cell = p.rcp_cell; d_o = (double)p.oversample;
+        chalf = (double)(p.n_grid / 2) * (double)p.oversample + 0.5;
+        eps = p.span * 7.1054273576010019e-15;                 // 2^-47 N O
+        span2 = 2.0 * p.span;
+        o_shift = p.o_shift; o_minus_1 = p.oversample - 1;
+        half_so = (p.support[0] * p.oversample) >> 1;
+        n_minus_s = p.n_grid - p.support[0];
+        s2 = p.support[0] * p.support[0];
+        ntx = (uint32_t)p.ntx; tlog = (uint32_t)p.key.tlog; tmask = (1u << p.key.tlog) - 1u;
+        aux_bits = (uint32_t)p.key.aux_bits; bits_q = (uint32_t)p.key.bits_q; tile_shift = (uint32_t)p.key.tile_shift;
+    }
+    __device__ __forceinline__ double chan_scale(double s) const { return __dmul_rn(__dmul_rn(s, rcp_cell), d_o); }
+    __device__ __forceinline__ bool axis(double coord_m, double ks, int &x0, int &q) const {
+        const double kMagic = 6755399441055744.0;               // 1.5 * 2^52
+        const double t1 = __fma_rn(coord_m, ks, chalf);
+        const double m = __dadd_rn(t1, kMagic);
+        const double d = __dadd_rn(t1, -__dadd_rn(m, -kMagic));
+        if (!(fabs(t1) < span2 && fabs(d) > eps)) return false;
+        const int a = __double2loint(m) - (d < 0.0 ? 1 : 0) - half_so;     // floor(t1) - S O / 2
+        x0 = (a + o_minus_1) >> o_shift;                        // ceil(a / O)
+        q = (x0 << o_shift) - a;
+        return true;
+    }
+    // sort key of the visibility (fast_key's layout); `taps` gets S^2 or 0 (dropped)
+    __device__ __forceinline__ uint32_t key(double u_m, double v_m, double s, double ks, const MapParams &p, int &taps) const {
+        int x0, y0, qx, qy;
+        const bool okx = axis(u_m, ks, x0, qx), oky = axis(v_m, ks, y0, qy);
+        if (okx && oky) {
+            if ((unsigned)x0 > (unsigned)n_minus_s || (unsigned)y0 > (unsigned)n_minus_s) {     // off the grid
+                taps = 0;
+                return 1u << (2 * bits_q);                      // drop slot 0, tile 0, origin (0, 0)
+            }
+            taps = s2;
+            const uint32_t ux = (uint32_t)x0, uy = (uint32_t)y0;
+            const uint32_t tile = (uy >> tlog) * ntx + (ux >> tlog);
+            return (tile << tile_shift) | ((uy & tmask) << (aux_bits + tlog)) | ((ux & tmask) << aux_bits) |
+                   ((uint32_t)qy << bits_q) | (uint32_t)qx;
+        }
+        const VisMap mv = map_vis(u_m, v_m, 0.0, s, p);         // rare: near a rounding boundary, or far away
+        taps = mv.dropped ? 0 : mv.S * mv.S;
+        return fast_key(mv, p);
+    }
+};
+
 }  // namespace gridder

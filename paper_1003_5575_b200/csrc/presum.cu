@@ -40,20 +40,46 @@ namespace gridder {
 
 constexpr uint32_t kAbsent = 0xFFFFFFFFu;      // no visibility here (ragged group); never a key (see fast_key)
 
+// A group is 8 ROWS x 32 channels; a row is one (integration, baseline).  Rows of a group: rt integrations
+// (rt = min(8, n_time)) of each of rb = 8 / rt consecutive baselines, the integrations of a baseline next to each
+// other -- so 8 integrations of one baseline when there are that many, 8 baselines when there is one integration.
+// (Summing visibilities with equal keys is valid whatever rows they come from.)
 struct PsGeo {
     uint32_t n_time, n_bl, n_chan;
     uint32_t n_fchunk;          // ceil(n_chan / 32)
-    uint32_t rows;              // min(8, n_time): integrations per group
-    uint32_t n_tblock;          // ceil(n_time / rows)
-    uint32_t n_groups;          // n_tblock * n_bl * n_fchunk; group g = (tb * n_bl + b) * n_fchunk + fc
-    uint32_t slots;             // rows * 32: staging slots (most records) of a group
+    uint32_t rt, rb;            // integrations x baselines per group
+    uint32_t n_tblock;          // ceil(n_time / rt)
+    uint32_t n_bgroup;          // ceil(n_bl / rb)
+    uint32_t n_groups;          // n_tblock * n_bgroup * n_fchunk; group g = (tb * n_bgroup + bg) * n_fchunk + fc
 };
+constexpr uint32_t kPsSlots = 256;             // staging slots (most records) of a group
 
-__device__ __forceinline__ void group_coords(const PsGeo &g, uint32_t grp, uint32_t &tb, uint32_t &b, uint32_t &fc) {
-    fc = grp % g.n_fchunk;
-    const uint32_t rb = grp / g.n_fchunk;
-    b = rb % g.n_bl;
-    tb = rb / g.n_bl;
+__device__ __forceinline__ void group_coords(const PsGeo &g, uint32_t grp, uint32_t &t0, uint32_t &b0, uint32_t &f0) {
+    const uint32_t fc = grp % g.n_fchunk, rest = grp / g.n_fchunk;
+    f0 = fc * 32u;
+    b0 = (rest % g.n_bgroup) * g.rb;
+    t0 = (rest / g.n_bgroup) * g.rt;
+}
+
+// Row r of a group: integration t0 + rt of baseline b0 + rb.  RT > 0: the integrations per group are known at
+// compile time (1, 2, 4 or 8: all 8 rows in use), RT == 0: any (geo.rt).
+template <int RT>
+__device__ __forceinline__ void row_of(const PsGeo &g, int r, uint32_t &rt, uint32_t &rb) {
+    if constexpr (RT > 0) {
+        rt = (uint32_t)(r % RT);
+        rb = (uint32_t)(r / RT);
+    } else {
+        rb = (uint32_t)r / g.rt;
+        rt = (uint32_t)r - rb * g.rt;
+    }
+}
+// (all element indices fit 32 bits: a plan holds fewer than 2^32 visibilities)
+template <int RT>
+__device__ __forceinline__ bool row_index(const PsGeo &g, int r, uint32_t t0, uint32_t b0, uint32_t &row) {
+    uint32_t rt, rb;
+    row_of<RT>(g, r, rt, rb);
+    row = (t0 + rt) * g.n_bl + (b0 + rb);
+    return (RT > 0 || rb < g.rb) && t0 + rt < g.n_time && b0 + rb < g.n_bl;
 }
 
 // exclusive prefix of x over the lanes of a warp, and the total
@@ -68,73 +94,75 @@ __device__ __forceinline__ uint32_t warp_excl(uint32_t x, int lane, uint32_t &to
     return incl - x;
 }
 
-template <bool FAST>
-__global__ void __launch_bounds__(256) presum_plan_kernel(const double *__restrict__ uvw, const double *__restrict__ scale,
+template <bool FAST, int RT>
+__global__ void __launch_bounds__(256, 3) presum_plan_kernel(const double *__restrict__ uvw, const double *__restrict__ scale,
                                                            const PsGeo geo, const MapParams p,
                                                            unsigned char *__restrict__ flags, uint32_t *__restrict__ stage,
                                                            uint32_t *__restrict__ count, Counters *counters) {
     const int lane = threadIdx.x & 31;
     const uint32_t gw = blockIdx.x * 8u + (threadIdx.x >> 5), nw = gridDim.x * 8u;
     const uint32_t dropbit = 1u << (2 * p.key.bits_q);
-    FastMap fm;
+    FastMap2 fm;
     if (FAST) fm.init(p);
     unsigned int dropped_here = 0;
     unsigned long long taps_here = 0;
 
     for (uint32_t grp = gw; grp < geo.n_groups; grp += nw) {
-        uint32_t tb, b, fc;
-        group_coords(geo, grp, tb, b, fc);
-        const uint32_t f = fc * 32u + (uint32_t)lane, t0 = tb * geo.rows;
+        uint32_t t0, b0, f0;
+        group_coords(geo, grp, t0, b0, f0);
+        const uint32_t f = f0 + (uint32_t)lane;
         const bool col = f < geo.n_chan;
         const double s = col ? scale[f] : 0.0;
+        const double ks = FAST ? fm.chan_scale(s) : 0.0;
         uint32_t key[8];
+        uint32_t valid = 0;
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
             key[r] = kAbsent;
-            if (col && (uint32_t)r < geo.rows && t0 + r < geo.n_time) {
-                const double *L = uvw + ((size_t)(t0 + r) * geo.n_bl + b) * 3;
+            uint32_t row;
+            if (row_index<RT>(geo, r, t0, b0, row) && col) {
+                const double *L = uvw + (size_t)row * 3;
                 int taps;
                 if (FAST) {
-                    key[r] = fm.key(__ldg(L), __ldg(L + 1), s, p, taps);
+                    key[r] = fm.key(__ldg(L), __ldg(L + 1), s, ks, p, taps);
                 } else {
                     const VisMap m = map_vis(__ldg(L), __ldg(L + 1), 0.0, s, p);
                     taps = m.dropped ? 0 : m.S * m.S;
                     key[r] = fast_key(m, p);
                 }
                 if (taps == 0) dropped_here++; else taps_here += (unsigned long long)taps;
+                valid |= 1u << r;
             }
         }
-        // t-runs, and which of them is the first of its key in the column
-        uint32_t th = 0, fo = 0, drop = 0;
+        // t-runs (bit r of th: a run starts in row r), dropped runs, rows whose key equals the next column's
+        uint32_t th = 0, drop = 0, eq = 0;
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
-            if (key[r] == kAbsent) continue;
-            const bool start = r == 0 || key[r] != key[r - 1];
-            if (!start) continue;
-            th |= 1u << r;
-            if (key[r] & dropbit) { drop |= 1u << r; continue; }
-            bool first = true;
-#pragma unroll
-            for (int r2 = 0; r2 < r; ++r2) first = first && key[r2] != key[r];
-            if (first) fo |= 1u << r;
+            const uint32_t nk = __shfl_down_sync(0xffffffffu, key[r], 1);
+            if (!((valid >> r) & 1u)) continue;
+            if (r == 0 || key[r] != key[r - 1]) {
+                th |= 1u << r;
+                if (key[r] & dropbit) drop |= 1u << r;
+            }
+            if (nk == key[r] && lane < 31) eq |= 1u << r;
         }
-        // forward links into column f + 1 (same warp only: chains do not cross a group)
-        uint32_t nfo = __shfl_down_sync(0xffffffffu, fo, 1);
-        if (lane == 31) nfo = 0u;
-        uint32_t nk[8];
-#pragma unroll
-        for (int r = 0; r < 8; ++r) nk[r] = __shfl_down_sync(0xffffffffu, key[r], 1);
+        // forward links: a run links to the run of the next column that holds the same key in one of the run's
+        // own rows (runs of a lattice point in neighbouring columns overlap in their rows, or they are strangers:
+        // then they stay two records, which is only a record more).  A target is taken once.
+        const uint32_t nth = __shfl_down_sync(0xffffffffu, th, 1);
         uint32_t link = 0;          // 4 bits per row: has a link | the linked row << 1
         uint32_t targets = 0;       // rows of column f + 1 this column links to
-#pragma unroll
-        for (int r = 0; r < 8; ++r) {
-            if (!((fo >> r) & 1u)) continue;
-#pragma unroll
-            for (int r2 = 0; r2 < 8; ++r2)
-                if (((nfo >> r2) & 1u) && nk[r2] == key[r]) {
-                    link |= (1u | ((uint32_t)r2 << 1)) << (4 * r);
-                    targets |= 1u << r2;
-                }
+        for (uint32_t m = th & ~drop; m; m &= m - 1u) {
+            const int r = __ffs(m) - 1;
+            const uint32_t later = th & ~((2u << r) - 1u);                    // starts of the later runs
+            const uint32_t rows = ((later ? (later & (0u - later)) : 256u) - 1u) & ~((1u << r) - 1u);
+            const uint32_t hit = eq & rows;
+            if (!hit) continue;
+            const int rs = __ffs(hit) - 1;
+            const int h = 31 - __clz(nth & ((2u << rs) - 1u));                // start of the neighbour's run through row rs
+            if ((targets >> h) & 1u) continue;
+            targets |= 1u << h;
+            link |= (1u | ((uint32_t)h << 1)) << (4 * r);
         }
         uint32_t pred = __shfl_up_sync(0xffffffffu, targets, 1);
         if (lane == 0) pred = 0;
@@ -143,16 +171,19 @@ __global__ void __launch_bounds__(256) presum_plan_kernel(const double *__restri
         uint32_t total;
         uint32_t idx = warp_excl((uint32_t)__popc(head), lane, total);
         if (lane == 0) count[grp] = total;
-        uint32_t *st = stage + (size_t)grp * geo.slots;
+        uint32_t *st = stage + (size_t)grp * kPsSlots;
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
-            if (key[r] == kAbsent) continue;
             const uint32_t bit = 1u << r;
-            unsigned char fl = 0;
-            if (th & bit)
-                fl = (unsigned char)(1u | ((head & bit) ? 2u : 0u) | ((drop & bit) ? 4u : 0u) | (((link >> (4 * r)) & 15u) << 3));
-            flags[((size_t)(t0 + r) * geo.n_bl + b) * geo.n_chan + f] = fl;
-            if (head & bit) st[idx++] = key[r];
+            if (valid & bit) {
+                uint32_t row;
+                row_index<RT>(geo, r, t0, b0, row);
+                unsigned char fl = 0;
+                if (th & bit)
+                    fl = (unsigned char)(1u | ((head & bit) ? 2u : 0u) | ((drop & bit) ? 4u : 0u) | (((link >> (4 * r)) & 15u) << 3));
+                flags[row * geo.n_chan + f] = fl;
+                if (head & bit) st[idx++] = key[r];
+            }
         }
     }
     for (int o = 16; o > 0; o >>= 1) {
@@ -174,7 +205,7 @@ __global__ void __launch_bounds__(256) presum_compact_kernel(const uint32_t *__r
     const uint32_t nw = gridDim.x * 8u;
     for (uint32_t grp = blockIdx.x * 8u + (threadIdx.x >> 5); grp < geo.n_groups; grp += nw) {
         const uint32_t cnt = count[grp], dst = base[grp];
-        const uint32_t *st = stage + (size_t)grp * geo.slots;
+        const uint32_t *st = stage + (size_t)grp * kPsSlots;
         for (uint32_t j = lane; j < cnt; j += 32) {
             rec_key[dst + j] = st[j];
             rec_idx[dst + j] = dst + j;
@@ -192,8 +223,10 @@ __device__ __forceinline__ float4 ld_stream4(const float4 *p) {
 constexpr int kPsWarps = 4;                          // 33 KB of static shared memory per block
 constexpr int kPsWarpF4 = 2 * 8 * 32 + 16;          // slot planes A and B [row][lane], then 256 flag bytes
 
-// gridder_grid, first kernel of a pre-summed plan: rec_sum[record] = sum over the record's chain of w V.
-template <bool WEIGHTED>
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
+
+// gridder_grid, first kernel of a pre-summed plan: ps_sum[record] = sum over the record's chain of w V.
+template <bool WEIGHTED, int RT>
 __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__restrict__ vis, const float *__restrict__ weight,
                                                                const unsigned char *__restrict__ flags,
                                                                const uint32_t *__restrict__ base, const PsGeo geo,
@@ -203,11 +236,30 @@ __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__r
     float4 *slotA = smem + warp * kPsWarpF4, *slotB = slotA + 8 * 32;
     unsigned char *sflag = reinterpret_cast<unsigned char *>(slotB + 8 * 32);
     const uint32_t nw = gridDim.x * (uint32_t)kPsWarps;
+    // this lane's share of the prefetch of the warp's NEXT group: row pr, 128-byte lines pl and pl + 4 of the
+    // row's 1 KB of visibilities; lanes 0-7 also the row's weights, lanes 8-15 its flags
+    const int pr = lane & 7;
+    const uint32_t pl = (uint32_t)lane >> 3;
 
     for (uint32_t grp = blockIdx.x * (uint32_t)kPsWarps + warp; grp < geo.n_groups; grp += nw) {
-        uint32_t tb, b, fc;
-        group_coords(geo, grp, tb, b, fc);
-        const uint32_t f = fc * 32u + (uint32_t)lane, t0 = tb * geo.rows;
+        uint32_t t0, b0, f0;
+        group_coords(geo, grp, t0, b0, f0);
+        if (grp + nw < geo.n_groups) {
+            // The group this warp takes next is asked into L2 now: a warp has one group's loads in flight at a
+            // time, which alone does not keep HBM busy
+            uint32_t nt0, nb0, nf0;
+            group_coords(geo, grp + nw, nt0, nb0, nf0);
+            uint32_t row;
+            if (row_index<RT>(geo, pr, nt0, nb0, row)) {
+                const size_t i0 = (size_t)(row * geo.n_chan + nf0);
+                const uint32_t nf = min(32u, geo.n_chan - nf0);
+                if (pl * 4u < nf) prefetch_l2(vis + 2 * (i0 + pl * 4u));
+                if ((pl + 4u) * 4u < nf) prefetch_l2(vis + 2 * (i0 + (pl + 4u) * 4u));
+                if (pl == 0 && WEIGHTED) prefetch_l2(weight + i0);
+                if (pl == 1) prefetch_l2(flags + i0);
+            }
+        }
+        const uint32_t f = f0 + (uint32_t)lane;
         const bool col = f < geo.n_chan;
         // everything the group needs is requested at once: 8 rows x (32 B + 4 B + 1 B) per lane
         float4 va[8], vb[8];
@@ -218,8 +270,9 @@ __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__r
             va[r] = vb[r] = make_float4(0.f, 0.f, 0.f, 0.f);
             w[r] = 0.f;
             fl[r] = 0u;
-            if (col && (uint32_t)r < geo.rows && t0 + r < geo.n_time) {
-                const size_t i = ((size_t)(t0 + r) * geo.n_bl + b) * geo.n_chan + f;
+            uint32_t row;
+            if (row_index<RT>(geo, r, t0, b0, row) && col) {
+                const size_t i = (size_t)(row * geo.n_chan + f);
                 va[r] = ld_stream4(vis + 2 * i);
                 vb[r] = ld_stream4(vis + 2 * i + 1);
                 w[r] = WEIGHTED ? __ldcs(weight + i) : 1.0f;
@@ -281,21 +334,22 @@ static PsGeo make_geo(int n_time, int n_bl, int n_chan) {
     PsGeo g;
     g.n_time = (uint32_t)n_time; g.n_bl = (uint32_t)n_bl; g.n_chan = (uint32_t)n_chan;
     g.n_fchunk = (uint32_t)((n_chan + 31) / 32);
-    g.rows = (uint32_t)(n_time < 8 ? n_time : 8);
-    if (g.rows == 0) g.rows = 1;
-    g.n_tblock = (uint32_t)((n_time + (int)g.rows - 1) / (int)g.rows);
-    g.n_groups = g.n_tblock * g.n_bl * g.n_fchunk;
-    g.slots = g.rows * 32u;
+    g.rt = (uint32_t)(n_time < 8 ? (n_time > 0 ? n_time : 1) : 8);
+    g.rb = 8u / g.rt;
+    g.n_tblock = ((uint32_t)n_time + g.rt - 1) / g.rt;
+    g.n_bgroup = ((uint32_t)n_bl + g.rb - 1) / g.rb;
+    g.n_groups = g.n_tblock * g.n_bgroup * g.n_fchunk;
     return g;
 }
 
-// Can this input be pre-summed by the plan?  (Host-side, shapes only.)
+// Can this input be pre-summed by the plan?  (Host-side, shapes only: ragged groups are padded to 8 x 32, and
+// the plan has room for 6 staging slots per visibility of its capacity.)
 bool presum_fits(const Plan &p, int n_time, int n_bl, int n_chan) {
     if (!p.presum || n_time <= 0 || n_bl <= 0 || n_chan <= 0) return false;
     const PsGeo g = make_geo(n_time, n_bl, n_chan);
-    const unsigned long long ng = (unsigned long long)g.n_tblock * g.n_bl * g.n_fchunk;
+    const unsigned long long ng = (unsigned long long)g.n_tblock * g.n_bgroup * g.n_fchunk;
     if (ng > (unsigned long long)p.ps_group_cap) return false;
-    if (ng * g.slots > (unsigned long long)p.ps_stage_cap) return false;        // staging lives in the record sums
+    if (ng * kPsSlots > (unsigned long long)p.ps_stage_cap) return false;       // staging lives in the record sums
     return true;
 }
 
@@ -311,13 +365,20 @@ cudaError_t launch_presum_plan(Plan &p, const double *uvw, const double *scale, 
                                cudaStream_t s, long long *n_rec) {
     const PsGeo geo = make_geo(n_time, n_bl, n_chan);
     const MapParams mp = make_map_params(p);
-    uint32_t *stage = reinterpret_cast<uint32_t *>(p.rec_sum);
+    uint32_t *stage = reinterpret_cast<uint32_t *>(p.ps_sum);
     const int blocks = (int)min((long long)(geo.n_groups + 7) / 8, (long long)p.n_sm * 64);
     GR_TRY(cudaMemsetAsync(p.ps_count + geo.n_groups, 0, sizeof(uint32_t), s));
-    if (mp.o_shift >= 0 && mp.drop_slot == 0)
-        presum_plan_kernel<true><<<blocks, 256, 0, s>>>(uvw, scale, geo, mp, p.ps_flags, stage, p.ps_count, p.counters);
-    else
-        presum_plan_kernel<false><<<blocks, 256, 0, s>>>(uvw, scale, geo, mp, p.ps_flags, stage, p.ps_count, p.counters);
+    const bool fast = mp.o_shift >= 0 && mp.drop_slot == 0;
+#define PS_PLAN(F, R) presum_plan_kernel<F, R><<<blocks, 256, 0, s>>>(uvw, scale, geo, mp, p.ps_flags, stage, p.ps_count, p.counters)
+    switch (fast ? (int)geo.rt : -1) {
+        case 8: PS_PLAN(true, 8); break;
+        case 4: PS_PLAN(true, 4); break;
+        case 2: PS_PLAN(true, 2); break;
+        case 1: PS_PLAN(true, 1); break;
+        case -1: PS_PLAN(false, 0); break;
+        default: PS_PLAN(true, 0); break;
+    }
+#undef PS_PLAN
     GR_TRY(cudaGetLastError());
     size_t tb = p.cub_temp_bytes;
     GR_TRY(cub::DeviceScan::ExclusiveSum(p.cub_temp, tb, (const uint32_t *)p.ps_count, p.ps_base,
@@ -336,12 +397,22 @@ cudaError_t launch_presum_plan(Plan &p, const double *uvw, const double *scale, 
 cudaError_t launch_presum(Plan &p, const float *vis, const float *weight, cudaStream_t s) {
     const PsGeo geo = make_geo(p.ps_n_time, p.ps_n_bl, p.ps_n_chan);
     const int blocks = (int)min((long long)(geo.n_groups + kPsWarps - 1) / kPsWarps, (long long)p.n_sm * 32);
-    if (weight)
-        presum_kernel<true><<<blocks, kPsWarps * 32, 0, s>>>(reinterpret_cast<const float4 *>(vis), weight, p.ps_flags,
-                                                              p.ps_base, geo, p.rec_sum);
-    else
-        presum_kernel<false><<<blocks, kPsWarps * 32, 0, s>>>(reinterpret_cast<const float4 *>(vis), nullptr, p.ps_flags,
-                                                               p.ps_base, geo, p.rec_sum);
+    const float4 *v4 = reinterpret_cast<const float4 *>(vis);
+#define PS_SUM(W, R) presum_kernel<W, R><<<blocks, kPsWarps * 32, 0, s>>>(v4, weight, p.ps_flags, p.ps_base, geo, p.ps_sum)
+    if (weight) {
+        switch (geo.rt) {
+            case 8: PS_SUM(true, 8); break;
+            case 1: PS_SUM(true, 1); break;
+            default: PS_SUM(true, 0); break;
+        }
+    } else {
+        switch (geo.rt) {
+            case 8: PS_SUM(false, 8); break;
+            case 1: PS_SUM(false, 1); break;
+            default: PS_SUM(false, 0); break;
+        }
+    }
+#undef PS_SUM
     p.n_launches += 1;
     return cudaGetLastError();
 }

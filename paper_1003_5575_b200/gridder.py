@@ -210,11 +210,11 @@ class Gridder:
         if rc != OK:
             raise GridderError(rc, "gridder_set_profiling")
 
-    STAGES = ("map", "sort", "tables", "grid", "flush", "reduce")
+    STAGES = ("map", "sort", "tables", "grid", "flush", "presum", "reduce")
 
     def stage_ms(self) -> dict:
         """Device milliseconds of the last bin/grid per stage (synchronises on their events)."""
-        ms = (C.c_float * 6)()
+        ms = (C.c_float * 7)()
         rc = self._lib.gridder_get_stage_ms(self._plan, ms)
         if rc != OK:
             raise GridderError(rc, "gridder_get_stage_ms")
