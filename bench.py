@@ -371,13 +371,10 @@ def run_ours(args) -> dict | None:
     if world == 1 and not args.no_unmerged:
         g.workspace = None                        # (the first plan's workspace goes back to the allocator)
         torch.cuda.empty_cache()
-        os.environ["GRIDDER_MERGE"] = "0"
-        try:
-            g2 = gridder.Gridder(grid_size=wl.grid_size, cell_size=wl.cell_size, oversample=wl.oversample,
-                                 support=wl.support, kernel=torch.from_numpy(wl.kernel).to(dev), max_vis=n,
-                                 n_wplanes=wl.n_wplanes, w_max=wl.w_max, kernel_is_complex=wl.kernel_is_complex)
-        finally:
-            os.environ.pop("GRIDDER_MERGE", None)
+        g2 = gridder.Gridder(grid_size=wl.grid_size, cell_size=wl.cell_size, oversample=wl.oversample,
+                             support=wl.support, kernel=torch.from_numpy(wl.kernel).to(dev), max_vis=n,
+                             n_wplanes=wl.n_wplanes, w_max=wl.w_max, kernel_is_complex=wl.kernel_is_complex,
+                             tuning={"merge": 2})
         g2.bin(d_uvw, d_freq)
         g2.grid(vis, weight, out=grid)
         torch.cuda.synchronize()

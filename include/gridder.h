@@ -26,9 +26,9 @@
  *     the caller owns every buffer, including the workspace.
  *   - Calls only enqueue work on `cuda_stream` (a cudaStream_t passed as void*; NULL = default
  *     stream).  gridder_plan, gridder_destroy, gridder_get_stats and gridder_run_host synchronise;
- *     gridder_bin synchronises the stream ONCE in the middle when it bins by channel runs (plans
- *     with one real table, S <= 16, O <= 8 and max_vis >= 4 Mi): the number of runs sizes the sort.  What it enqueues
- *     after that is asynchronous again.
+ *     gridder_bin synchronises the stream ONCE in the middle when the plan pre-sums in input order
+ *     (see gridder_tuning.presum): the number of partial records sizes the radix sort.  What it
+ *     enqueues after that is asynchronous again.  Nothing in the library reads the environment.
  *   - Buffers given to gridder_bin / gridder_grid must stay valid until that work has completed.
  *   - A plan may be binned and gridded any number of times; one gridder_bin serves any number of
  *     gridder_grid calls (same uv geometry, new visibilities).  Not thread-safe per plan.
@@ -86,6 +86,28 @@ typedef struct {
     size_t workspace_bytes;
 } gridder_config;
 
+/* Optional tuning (gridder_plan_tuned).  Every field: 0 = the library's default, so a zeroed struct is
+ * gridder_plan.  None of them changes WHAT is computed -- only tile shapes, work-item sizes and which of the
+ * equivalent paths runs; results stay within the tolerance of the definition and bit-identical from run to run
+ * for a given tuning.  The tests use them to reach every path on small inputs. */
+typedef struct {
+    int32_t tile_log2;          /* 2, 3 or 4: uv tiles of 2^tile_log2 cells per edge (default 2; 3 for pre-summed plans) */
+    int32_t chunk;              /* K, 32 .. 2^20: most sorted entries per work item (default by size, 256 .. 8192)  */
+    int32_t max_warps;          /* cap on the warps per block of the grid kernel (default: what fits)              */
+    int32_t merge;              /* 1 on (default), 2 off: entries of a batch of 32 with equal patch origin and
+                                   sub-cell offset are summed before they are gridded (exact by linearity)        */
+    int32_t presum;             /* pre-summation in input order (one real table, S <= 16, O <= 8): 1 always,
+                                   2 never; default: plans of max_vis >= 4 Mi, where the one synchronisation
+                                   it costs gridder_bin is cheaper than sorting every visibility                   */
+    int32_t table_in_tmem;      /* 1 on, 2 off: GCF table in tensor memory instead of shared memory (one real
+                                   table with O^2 x 8 <= 512 columns; default: on for pre-summed plans)            */
+    int32_t fold_batches;       /* power of two <= 64: batches of 32 records a register chain may span (default 8) */
+    int32_t force_general;      /* 1: global-memory tables and wide sort values even for one real table          */
+    int32_t host_slices;        /* gridder_run_host: slices of the (integration, baseline) axis (default 8; 1: none) */
+    int32_t host_slice_min_mb;  /* gridder_run_host: slice inputs of at least this many MB (default 256)           */
+    int32_t reserved[6];        /* must be 0 */
+} gridder_tuning;
+
 typedef struct {
     int64_t n_vis;              /* visibilities given to the last gridder_bin                        */
     int64_t n_dropped;          /* of those, dropped because the patch leaves the grid               */
@@ -117,9 +139,15 @@ GRIDDER_API int gridder_workspace_size(const gridder_config *cfg, size_t *bytes_
  * `workspace_needed` may be NULL.  Synchronises the device once (table re-layout). */
 GRIDDER_API int gridder_plan(const gridder_config *cfg, gridder_plan_t **plan_out, size_t *workspace_needed);
 
+/* The same with explicit tuning (`tuning` HOST, may be NULL = defaults; copied).  A value outside a field's
+ * range is GRIDDER_ERR_INVALID_ARG. */
+GRIDDER_API int gridder_workspace_size_tuned(const gridder_config *cfg, const gridder_tuning *tuning, size_t *bytes_needed);
+GRIDDER_API int gridder_plan_tuned(const gridder_config *cfg, const gridder_tuning *tuning, gridder_plan_t **plan_out,
+                                   size_t *workspace_needed);
+
 /* Map + sort + tile tables for n_time*n_baseline*n_chan visibilities (index (t*B + b)*F + f).
- * u_lambda = u_m * (f / c), c = 299792458 m/s.  n_chan <= 65536.  Enqueued on `cuda_stream` (one
- * internal synchronisation, see above). */
+ * u_lambda = u_m * (f / c), c = 299792458 m/s.  n_chan <= 65536.  Enqueued on `cuda_stream` (pre-summed
+ * plans: one internal synchronisation, see above). */
 GRIDDER_API int gridder_bin(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
                 const double *freq_hz, int32_t n_chan, void *cuda_stream);
 
@@ -145,10 +173,19 @@ GRIDDER_API int gridder_destroy(gridder_plan_t *plan);
 GRIDDER_API int gridder_get_stats(gridder_plan_t *plan, gridder_stats *out);
 
 /* The mapping alone, for tests: out is DEVICE int32 [n][6] = x0, y0, qx, qy, plane | conj << 8,
- * dropped -- per visibility, same device function as gridder_bin's map kernel. */
+ * dropped -- per visibility, computed by map_vis (csrc/map.cuh), the device function of the per-visibility
+ * map kernel and the fallback of the screened mappers. */
 GRIDDER_API int gridder_map(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
                 const double *freq_hz, int32_t n_chan, const int32_t *table_index /* or NULL */, int32_t *out,
                 void *cuda_stream);
+
+/* The same through the mapper of the pre-summed path (FastMap2 in csrc/map.cuh: one fused multiply-add per
+ * axis, screened against the definition's rounding, map_vis where the screen does not decide) -- the code
+ * that maps BASELINE.json configs 2 and 4.  Same output, except that a dropped visibility reports
+ * 0, 0, 0, 0, 0, 1.  Only for plans on the fast path (one real table, S <= 16) with a power-of-two
+ * oversampling; otherwise GRIDDER_ERR_UNSUPPORTED. */
+GRIDDER_API int gridder_map_presum(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
+                                   const double *freq_hz, int32_t n_chan, int32_t *out, void *cuda_stream);
 
 /* the arithmetic of the paper's OpenGL gridder (PAPER.md :185-191: one
  * screen-aligned GCF quad per visibility, additive blending) as plain CUDA: every (visibility, tap,
@@ -201,9 +238,9 @@ GRIDDER_API int gridder_run_host(gridder_plan_t *plan, const double *h_uvw_m, in
  * they run on (a few microseconds of host time per call; nothing else changes). */
 GRIDDER_API int gridder_set_profiling(gridder_plan_t *plan, int32_t enable);
 /* Mean device milliseconds per stage over the gridder_bin / gridder_grid calls made since
- * profiling was enabled (the last 32 of each at most), HOST float [7]: map, sort, tile tables,
- * grid kernel, flush kernel, input-order pre-summation kernel, per-origin summation kernel (0 for plans that
- * do not run them).  Synchronises on
+ * profiling was enabled (the last 32 of each at most), HOST float [6]: map (pre-summed plans: the plan
+ * kernel, scan and compaction), sort, tile tables, grid kernel, flush kernel, input-order pre-summation
+ * kernel (0 where it does not run).  Synchronises on
  * the recorded events.  A stage that has not run since then reads 0.  Enabling again resets
  * the averages. */
 GRIDDER_API int gridder_get_stage_ms(gridder_plan_t *plan, float *ms_out);

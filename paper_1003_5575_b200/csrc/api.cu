@@ -1,6 +1,5 @@
 // The C ABI of include/gridder.h: plan management, argument checks, error codes.
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -12,20 +11,14 @@ namespace {
 
 size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
-int env_int(const char *name, int dflt) {
-    const char *v = getenv(name);
-    if (!v || !*v) return dflt;
-    return atoi(v);
-}
-
 int ceil_log2(unsigned long long v) {   // smallest b with 2^b >= v
     int b = 0;
     while ((1ull << b) < v) ++b;
     return b;
 }
 
-// Everything that follows from the config alone (no device access).
-int derive(const gridder_config *cfg, Plan &p) {
+// Everything that follows from the config and the tuning alone (no device access).
+int derive(const gridder_config *cfg, const gridder_tuning *tuning, Plan &p) {
     if (!cfg) return GRIDDER_ERR_INVALID_ARG;
     if (cfg->grid_size < 2 || (cfg->grid_size & 1) || cfg->grid_size > 32768) return GRIDDER_ERR_INVALID_ARG;
     if (!(cfg->cell_size > 0.0) || cfg->n_pol != 4) return GRIDDER_ERR_INVALID_ARG;
@@ -38,38 +31,45 @@ int derive(const gridder_config *cfg, Plan &p) {
         if (s > cfg->grid_size) return GRIDDER_ERR_INVALID_ARG;
     }
     if (cfg->n_wplanes > 1 && !(cfg->w_max > 0.0)) return GRIDDER_ERR_INVALID_ARG;
+    gridder_tuning t;
+    memset(&t, 0, sizeof(t));
+    if (tuning) t = *tuning;
+    if ((t.tile_log2 != 0 && (t.tile_log2 < 2 || t.tile_log2 > 4)) || (t.chunk != 0 && (t.chunk < 32 || t.chunk > (1 << 20))) ||
+        t.max_warps < 0 || t.merge < 0 || t.merge > 2 || t.presum < 0 || t.presum > 2 || t.table_in_tmem < 0 ||
+        t.table_in_tmem > 2 || t.fold_batches < 0 || t.fold_batches > 64 || (t.fold_batches & (t.fold_batches - 1)) ||
+        t.force_general < 0 || t.force_general > 1 || t.host_slices < 0 || t.host_slices > 64 || t.host_slice_min_mb < 0)
+        return GRIDDER_ERR_INVALID_ARG;
+    for (int i = 0; i < 6; ++i)
+        if (t.reserved[i]) return GRIDDER_ERR_INVALID_ARG;
 
     p.cfg = *cfg;
+    p.tune = t;
     memcpy(p.support_copy, cfg->support, sizeof(int32_t) * cfg->n_wplanes);
     p.cfg.support = p.support_copy;
     const bool cplx = cfg->kernel_is_complex != 0;
-    // fast path: one real table with S <= 16 (shared-memory table, 32-bit sort values)
-    p.mode = cplx ? 2 : ((cfg->n_wplanes == 1 && cfg->support[0] <= 16 && !env_int("GRIDDER_FORCE_GENERAL", 0)) ? 0 : 1);
-    // DENSE plans -- fast path, 16-cell patch, O^2 <= 64, 64 visibilities and more per 4 x 4 cells -- sum the
-    // entries of equal (origin, offset) before gridding (GRIDDER_QBINS: 0 never, 1 by density, 2 always)
-    const int64_t oo_early = (int64_t)cfg->oversample * cfg->oversample;
-    const int qb_mode = env_int("GRIDDER_QBINS", 1);
-    // PRE-SUMMATION IN INPUT ORDER (presum.cu; GRIDDER_PRESUM: 0 never, 1 plans of 4 Mi visibilities and more,
-    // 2 always): replaces the sorted-entry paths below
-    const int ps_mode = env_int("GRIDDER_PRESUM", 1);
-    p.presum = (p.mode == 0 && env_int("GRIDDER_MERGE", 1) && 2 * ceil_log2((unsigned long long)cfg->oversample) + 1 <= 8 &&
-                (ps_mode >= 2 || (ps_mode == 1 && cfg->max_vis >= (4ll << 20)))) ? 1 : 0;
-    const bool dense = !p.presum && p.mode == 0 && cfg->support[0] > 8 && oo_early <= 64 && env_int("GRIDDER_MERGE", 1) &&
-                       (qb_mode >= 2 || (qb_mode == 1 && cfg->max_vis * 16 / ((int64_t)cfg->grid_size * cfg->grid_size) >= 64));
-    // ... and with the pre-summation kernel (O^2 <= 16) larger tiles and longer work items pay: the work per
-    // item follows its (origin, offset) pairs, not its entries, and the flush has fewer regions to add
-    const bool dense_reduce = dense && oo_early <= 16 && env_int("GRIDDER_REDUCE", 1);
-    p.tlog = env_int("GRIDDER_TILE_LOG2", (dense_reduce || p.presum) ? 3 : 2);
-    if (p.tlog < 2 || p.tlog > 4) return GRIDDER_ERR_INVALID_ARG;
+    const size_t oo = (size_t)cfg->oversample * cfg->oversample;
+    const int q_bits = ceil_log2((unsigned long long)cfg->oversample);
+    p.merge = t.merge == 2 ? 0 : 1;
+    // fast path: one real table with S <= 16 (table in shared or tensor memory, 32-bit sort values)
+    p.mode = cplx ? 2 : ((cfg->n_wplanes == 1 && cfg->support[0] <= 16 && !t.force_general) ? 0 : 1);
+    // PRE-SUMMATION IN INPUT ORDER (presum.cu): fast path, merging allowed (a per-visibility GCF forbids it),
+    // sub-cell offsets and drop flag in one byte.  By default for plans of 4 Mi visibilities and more: below
+    // that sorting every visibility is cheap and the one host synchronisation it costs gridder_bin is not.
+    // Whether an input then really takes it is decided per gridder_bin, from its shape and the number of partial
+    // records the plan kernel COUNTED (the data, not the capacity): see launch_bin.
+    p.presum = (p.mode == 0 && p.merge && 2 * q_bits + 1 <= 8 &&
+                (t.presum == 1 || (t.presum == 0 && cfg->max_vis >= (4ll << 20)))) ? 1 : 0;
+    p.tlog = t.tile_log2 ? t.tile_log2 : (p.presum ? 3 : 2);
     p.T = 1 << p.tlog;
     p.ntx = (cfg->grid_size + p.T - 1) / p.T;
     p.nty = p.ntx;
     p.n_tiles = p.ntx * p.nty;
     // the fast path keeps the sub-cell offsets in the 32-bit sort key; a grid too large for that
     // (2 log2 N + 2 log2 O + 1 > 32 bits) goes through the general path, whose values carry them
-    if (p.mode == 0 &&
-        2 * ceil_log2((unsigned long long)cfg->oversample) + 1 + 2 * p.tlog + ceil_log2((unsigned long long)p.n_tiles) > 32)
+    if (p.mode == 0 && 2 * q_bits + 1 + 2 * p.tlog + ceil_log2((unsigned long long)p.n_tiles) > 32) {
         p.mode = 1;
+        p.presum = 0;
+    }
 
     // patch classes in use (ascending), and each plane's slot and table offset
     int slot_of_class[kMaxClasses] = {-1, -1, -1};
@@ -94,7 +94,6 @@ int derive(const gridder_config *cfg, Plan &p) {
         p.cls[p.n_cls++] = g;
     }
     size_t off = 0;
-    const size_t oo = (size_t)cfg->oversample * cfg->oversample;
     for (int i = 0; i < cfg->n_wplanes; ++i) {
         const int s = cfg->support[i];
         p.plane_slot[i] = slot_of_class[s <= 8 ? 0 : (s <= 16 ? 1 : 2)];
@@ -104,48 +103,36 @@ int derive(const gridder_config *cfg, Plan &p) {
     }
     if (off >= (1ull << 31)) return GRIDDER_ERR_UNSUPPORTED;       // table offsets are 32-bit byte offsets
     p.coef_bytes = off;
+    // a fast-path table that cannot sit in shared memory beside one warp's region (e.g. S = 16 with O = 16:
+    // 256 KB) is read from global memory instead: the general path
+    if (p.mode == 0 && p.coef_bytes + 24 * 1024 > 227 * 1024) {
+        p.mode = 1;
+        p.presum = 0;
+    }
 
-    // fast path (GRIDDER_TMEM=0/1): the table in tensor memory (512 columns x 32 bit per lane) when it fits.
-    // Measured on B200: same speed as the shared-memory table while the kernel is FMA-bound (DESIGN.md section
-    // 10), 8 % faster on the records of a dense plan, where the shared-memory path is the busiest unit: on by
-    // default there, off elsewhere.
+    // fast path: the table in tensor memory (512 columns x 32 bit per lane) when it fits.  Measured on B200:
+    // same speed as the shared-memory table while the kernel is FMA-bound, faster on the records of a
+    // pre-summed plan, where the shared-memory path is the busiest unit: on by default there.
     p.tmem_cols = 0;
-    if (p.mode == 0 && env_int("GRIDDER_TMEM", (dense_reduce || p.presum) ? 1 : 0)) {
+    if (p.mode == 0 && (t.table_in_tmem == 1 || (t.table_in_tmem == 0 && p.presum))) {
         const size_t cols = oo * p.cls[0].NA * p.cls[0].NB;
         if (cols <= 512) {
             p.tmem_cols = 32;
             while ((size_t)p.tmem_cols < cols) p.tmem_cols *= 2;
         }
     }
-    // fast path: bin by channel runs when the key's unsorted bits fit one byte (runs.cu)
-    p.run_cap = 0;
-    // GRIDDER_RUNS: 0 never, 1 (default) for plans of 4 M visibilities and more -- below that the per-visibility
-    // sort is cheap and the run path's one host synchronisation is not --, 2 always
-    const int runs_mode = env_int("GRIDDER_RUNS", 1);
-    if (p.mode == 0 && !p.presum && (runs_mode >= 2 || (runs_mode == 1 && cfg->max_vis >= (4ll << 20))) &&
-        2 * ceil_log2((unsigned long long)cfg->oversample) + 1 <= 8) {
-        p.run_cap = cfg->max_vis / 4;
-        if (p.run_cap < 1024) p.run_cap = 1024;
-    }
     // K: most entries per work item, ~ max_vis / 2^14 as a power of two in [256, 8192]: small inputs get
-    // short items so that a hot tile still spreads over the ~1800 resident warps; the largest get 8192,
-    // which halves the number of partial regions the flush has to sum for the cells of a hot tile
-    // (the accuracy budget of DESIGN.md section 7 holds up to 8192)
-    int k_auto = dense_reduce ? 32768 : 8192;
+    // short items so that a hot tile still spreads over the ~1800 resident warps; the largest get 8192
+    // (4096 when the entries are partial records), which bounds the partial regions the flush has to sum for
+    // the cells of a hot tile (the accuracy budget of DESIGN.md section 7 holds up to 8192)
+    int k_auto = p.presum ? 4096 : 8192;
     while (k_auto > 256 && (int64_t)k_auto * 16384 > cfg->max_vis) k_auto >>= 1;
-    p.chunk = env_int("GRIDDER_CHUNK", k_auto);
-    if (p.chunk < 32 || p.chunk > (1 << 20)) return GRIDDER_ERR_INVALID_ARG;
-    p.warps_forced = env_int("GRIDDER_WARPS", 0);
-    p.merge = env_int("GRIDDER_MERGE", 1) ? 1 : 0;
-    // fast path with per-origin bins (grid.cu): one real table, 16-cell patch, O^2 <= 64 offsets
-    // (sparser inputs merge as well per batch of 32)
-    p.qbins = 0;
-    if (dense && p.mode == 0 && p.merge && (p.tmem_cols == 0 || dense_reduce) && p.cls[0].NA == 2) p.qbins = (int)oo;
-    p.fold_batches = env_int("GRIDDER_FOLD_BATCHES", 8);
-    if (p.fold_batches < 1 || p.fold_batches > 64 || (p.fold_batches & (p.fold_batches - 1))) return GRIDDER_ERR_INVALID_ARG;
+    p.chunk = t.chunk ? t.chunk : k_auto;
+    p.warps_forced = t.max_warps;
+    p.fold_batches = t.fold_batches ? t.fold_batches : 8;
 
     KeyLayout k;
-    k.bits_q = ceil_log2((unsigned long long)cfg->oversample);
+    k.bits_q = q_bits;
     k.tlog = p.tlog;
     k.aux_bits = p.mode == 0 ? 2 * k.bits_q + 1 : 0;
     k.plane_shift = k.aux_bits + 2 * k.tlog;
@@ -165,27 +152,13 @@ int derive(const gridder_config *cfg, Plan &p) {
     p.max_items = occ + n / p.chunk + 1;
     // each class has its own partial-region array, sized for the case that every entry is of that class
     p.max_items_cls = (n < p.n_tiles ? n : p.n_tiles) + n / p.chunk + 1;
-    // GRIDDER_REDUCE (with the bins): 1 (default) a separate kernel sums the entries into records
-    // (reduce.cu) and the grid kernel runs on those; 0: one kernel does both (grid_kernel_qbins)
-    p.reduce = 0; p.rec_cap = 0; p.rec_slot = 0;
-    if (p.qbins > 0 && p.qbins <= 16 && env_int("GRIDDER_REDUCE", 1)) {
-        const int64_t per_item = (int64_t)p.T * p.T * p.qbins;          // (origin, offset) pairs of a tile
-        p.rec_slot = p.max_items * per_item <= n ? per_item : 0;
-        p.rec_cap = p.rec_slot ? p.max_items * per_item : n;
-        if (p.rec_cap < (1ll << 32)) p.reduce = 1;
-    }
-    if (!p.reduce && p.tmem_cols > 0) p.qbins = 0;       // (grid_kernel_qbins reads its table from shared memory)
     if (p.presum) {
-        // record sums: room for 3/4 of the visibilities (inputs that merge less take the per-visibility path);
-        // the plan kernel's staging slots live in the same array
+        // partial-record sums: room for 3/4 of the visibilities (inputs that merge less take the per-visibility
+        // path); the plan kernel's staging slots live in the same array
         p.ps_cap = n * 3 / 4 + 1024;
         p.ps_stage_cap = p.ps_cap * 8;
         p.ps_group_cap = n * 3 / 16 + 1024;
     }
-    // GRIDDER_FUSE=1 (with the pre-summation and the run binning; opt-in): reduce straight from the sorted runs,
-    // the per-entry sorted list is not written.  Measured on config 4: binning 3.4 ms shorter, reduce 4.6 ms
-    // longer (a run search per entry, one more gather, fewer warps): not a gain, so off by default.
-    p.fuse = (p.reduce && p.run_cap > 0 && env_int("GRIDDER_FUSE", 0)) ? 1 : 0;
     p.partials_f4 = 0;
     for (int c = 0; c < p.n_cls; ++c) {
         p.cls[c].part_off_f4 = p.partials_f4;
@@ -211,11 +184,6 @@ cudaError_t carve(Plan &p, char *base) {
         e = presum_scan_temp_bytes(p.ps_group_cap + 1, &t3);
         if (t3 > t2) t2 = t3;
     }
-    if (e == cudaSuccess && p.run_cap > 0) {
-        size_t t3 = 0;
-        e = runs_temp_bytes(p.run_cap, p.key.aux_bits, p.key.total_bits, &t3);
-        if (t3 > t1) t1 = t3;
-    }
     if (e == cudaErrorNoDevice || e == cudaErrorInsufficientDriver || e == cudaErrorInvalidDevice) {
         // no GPU on this machine (size query only): CUB cannot be asked, so report a generous bound
         (void)cudaGetLastError();
@@ -227,14 +195,6 @@ cudaError_t carve(Plan &p, char *base) {
     p.cub_temp_bytes = align_up(t1 > t2 ? t1 : t2);
     p.cub_temp = take(p.cub_temp_bytes);
     p.freq_scale = (double *)take(sizeof(double) * kMaxChannels);
-    if (p.run_cap > 0) {
-        const size_t cap = (size_t)p.run_cap;
-        p.qaux = (unsigned char *)take(n);
-        for (int i = 0; i < 2; ++i) p.run_key[i] = (uint32_t *)take(cap * sizeof(uint32_t));
-        for (int i = 0; i < 2; ++i) p.run_val[i] = (unsigned long long *)take(cap * sizeof(unsigned long long));
-        p.run_cum = (uint32_t *)take(cap * sizeof(uint32_t));
-        p.run_blk = (unsigned int *)take(3 * ((n + 1023) / 1024 + 1) * sizeof(unsigned int));
-    }
     p.tile_start = (uint32_t *)take(sizeof(uint32_t) * 2 * n_vtiles);        // [start | end]
     p.tile_chunks = (unsigned long long *)take(sizeof(unsigned long long) * (n_vtiles + 1));
     p.tile_chunks_scan = (unsigned long long *)take(sizeof(unsigned long long) * (n_vtiles + 1));
@@ -248,12 +208,6 @@ cudaError_t carve(Plan &p, char *base) {
         p.ps_base = (uint32_t *)take(sizeof(uint32_t) * (size_t)(p.ps_group_cap + 1));
         p.ps_sum = (float4 *)take(sizeof(float4) * 2 * (size_t)p.ps_cap);
     }
-    if (p.reduce) {
-        p.rec_key = (uint32_t *)take(sizeof(uint32_t) * (size_t)p.rec_cap);
-        p.rec_sum = (float4 *)take(sizeof(float4) * 2 * (size_t)p.rec_cap);
-        p.rec_items = (WorkItem *)take(sizeof(WorkItem) * (size_t)p.max_items);
-    }
-    if (p.fuse) p.blk_run = (uint32_t *)take(sizeof(uint32_t) * (n / 64 + 2));
     p.coef = (float4 *)take(p.coef_bytes);
     p.counters = (Counters *)take(sizeof(Counters));
     p.workspace_needed = off;
@@ -270,23 +224,32 @@ int cuda_fail(Plan *p, cudaError_t e) {
 extern "C" {
 
 int gridder_workspace_size(const gridder_config *cfg, size_t *bytes_needed) {
+    return gridder_workspace_size_tuned(cfg, nullptr, bytes_needed);
+}
+
+int gridder_plan(const gridder_config *cfg, gridder_plan_t **plan_out, size_t *workspace_needed) {
+    return gridder_plan_tuned(cfg, nullptr, plan_out, workspace_needed);
+}
+
+int gridder_workspace_size_tuned(const gridder_config *cfg, const gridder_tuning *tuning, size_t *bytes_needed) {
     if (!bytes_needed) return GRIDDER_ERR_INVALID_ARG;
     Plan p;
     memset(&p, 0, sizeof(p));
-    const int rc = derive(cfg, p);
+    const int rc = derive(cfg, tuning, p);
     if (rc != GRIDDER_OK) return rc;
     if (carve(p, nullptr) != cudaSuccess) return GRIDDER_ERR_CUDA;
     *bytes_needed = p.workspace_needed;
     return GRIDDER_OK;
 }
 
-int gridder_plan(const gridder_config *cfg, gridder_plan_t **plan_out, size_t *workspace_needed) {
+int gridder_plan_tuned(const gridder_config *cfg, const gridder_tuning *tuning, gridder_plan_t **plan_out,
+                       size_t *workspace_needed) {
     if (!plan_out) return GRIDDER_ERR_INVALID_ARG;
     *plan_out = nullptr;
     Plan *p = new (std::nothrow) Plan;
     if (!p) return GRIDDER_ERR_INVALID_ARG;
     memset(p, 0, sizeof(Plan));
-    int rc = derive(cfg, *p);
+    int rc = derive(cfg, tuning, *p);
     if (rc != GRIDDER_OK) { delete p; return rc; }
     if (carve(*p, nullptr) != cudaSuccess) { delete p; return GRIDDER_ERR_CUDA; }
     if (workspace_needed) *workspace_needed = p->workspace_needed;
@@ -321,8 +284,6 @@ int gridder_bin_tables(gridder_plan_t *plan, const double *uvw_m, int32_t n_time
     if (n_chan > kMaxChannels) return GRIDDER_ERR_UNSUPPORTED;
     p->binned = false;
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    // a bank of one real table on the fast path: there is nothing to choose
-    if (table_index && p->mode == 0 && p->cfg.n_wplanes == 1) table_index = nullptr;
     cudaError_t e = launch_bin(*p, uvw_m, n_time, n_baseline, freq_hz, n_chan, table_index, s);
     if (e != cudaSuccess) return cuda_fail(p, e);
     p->n_vis = n;
@@ -399,6 +360,18 @@ int gridder_map(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32
     return GRIDDER_OK;
 }
 
+int gridder_map_presum(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
+                       const double *freq_hz, int32_t n_chan, int32_t *out, void *cuda_stream) {
+    Plan *p = reinterpret_cast<Plan *>(plan);
+    if (!p || !uvw_m || !freq_hz || !out || n_time < 0 || n_baseline < 0 || n_chan < 0)
+        return GRIDDER_ERR_INVALID_ARG;
+    if ((int64_t)n_time * n_baseline * n_chan == 0) return GRIDDER_OK;
+    cudaError_t e = launch_map_presum_debug(*p, uvw_m, n_time, n_baseline, freq_hz, n_chan, out, (cudaStream_t)cuda_stream);
+    if (e == cudaErrorNotSupported) return GRIDDER_ERR_UNSUPPORTED;
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    return GRIDDER_OK;
+}
+
 int gridder_scatter_atomic(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
                            const double *freq_hz, int32_t n_chan, const float *vis, const float *weight, float *grid,
                            int32_t accumulate, void *cuda_stream) {
@@ -462,10 +435,9 @@ int gridder_run_host(gridder_plan_t *plan, const double *h_uvw_m, int32_t n_time
     // copies run on a second stream, slice k is binned and gridded (added to the grid) while slice k+1
     // is still on the wire.  Gridding is linear, so the slices sum to the same grid (each slice's
     // result is rounded to FP32 once more when it is added; deterministic all the same).
-    const int n_slices = (n * 32 >= ((size_t)env_int("GRIDDER_HOST_SLICE_MIN_MB", 256) << 20) && n_tb >= 8 &&
-                          env_int("GRIDDER_HOST_SLICES", 8) > 1)
-                             ? (int)(n_tb < (size_t)env_int("GRIDDER_HOST_SLICES", 8) ? n_tb : (size_t)(env_int("GRIDDER_HOST_SLICES", 8) > 64 ? 64 : env_int("GRIDDER_HOST_SLICES", 8)))
-                             : 1;
+    const size_t want = (size_t)(p->tune.host_slices ? p->tune.host_slices : 8);
+    const size_t min_mb = (size_t)(p->tune.host_slice_min_mb ? p->tune.host_slice_min_mb : 256);
+    const int n_slices = (n * 32 >= (min_mb << 20) && n_tb >= 8 && want > 1) ? (int)(n_tb < want ? n_tb : want) : 1;
     if (n_slices == 1) {
         // the binning only needs uvw and freq: it is enqueued ahead of the visibility copy
         int rc = gridder_bin(plan, d_uvw_m, n_time, n_baseline, d_freq_hz, n_chan, cuda_stream);
@@ -534,7 +506,7 @@ int gridder_set_profiling(gridder_plan_t *plan, int32_t enable) {
 int gridder_get_stage_ms(gridder_plan_t *plan, float *ms_out) {
     Plan *p = reinterpret_cast<Plan *>(plan);
     if (!p || !ms_out) return GRIDDER_ERR_INVALID_ARG;
-    double sum[7] = {0, 0, 0, 0, 0, 0, 0};
+    double sum[6] = {0, 0, 0, 0, 0, 0};
     const int nb = (int)(p->prof_bin_calls < kProfRing ? p->prof_bin_calls : kProfRing);
     const int ng = (int)(p->prof_grid_calls < kProfRing ? p->prof_grid_calls : kProfRing);
     cudaError_t e = cudaSuccess;
@@ -548,8 +520,8 @@ int gridder_get_stage_ms(gridder_plan_t *plan, float *ms_out) {
     }
     for (int r = 0; r < ng && e == cudaSuccess; ++r) {
         e = cudaEventSynchronize(p->ev[r][6]);
-        // events of a grid call, in stream order: 4, [7 after the input-order pre-summation], [8 after the
-        // per-origin summation], 5 after the grid kernels, 6 after the flush
+        // events of a grid call, in stream order: 4, [7 after the input-order pre-summation], 5 after the grid
+        // kernels, 6 after the flush
         int last = 4;
         float ms = 0.f;
         if (p->presum_active && e == cudaSuccess) {
@@ -557,17 +529,12 @@ int gridder_get_stage_ms(gridder_plan_t *plan, float *ms_out) {
             sum[5] += ms;
             last = 7;
         }
-        if (p->reduce && e == cudaSuccess) {
-            e = cudaEventElapsedTime(&ms, p->ev[r][last], p->ev[r][8]);
-            sum[6] += ms;
-            last = 8;
-        }
         if (e == cudaSuccess) { e = cudaEventElapsedTime(&ms, p->ev[r][last], p->ev[r][5]); sum[3] += ms; }
         if (e == cudaSuccess) { e = cudaEventElapsedTime(&ms, p->ev[r][5], p->ev[r][6]); sum[4] += ms; }
     }
     if (e != cudaSuccess) return cuda_fail(p, e);
     for (int i = 0; i < 3; ++i) ms_out[i] = nb ? (float)(sum[i] / nb) : 0.f;
-    for (int i = 3; i < 7; ++i) ms_out[i] = ng ? (float)(sum[i] / ng) : 0.f;
+    for (int i = 3; i < 6; ++i) ms_out[i] = ng ? (float)(sum[i] / ng) : 0.f;
     return GRIDDER_OK;
 }
 

@@ -297,9 +297,7 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
         double *scale = p.freq_scale;
         freq_scale_kernel<<<(n_chan + 255) / 256, 256, 0, s>>>(freq, n_chan, scale);
         GR_TRY(cudaGetLastError());
-        bool by_runs = false;
-        p.n_runs = 0;
-        p.fused_bin = 0;
+        bool by_runs = false;          // the sorted list is there already (records of a pre-summed plan)
         p.presum_active = 0;
         p.n_sorted = n;
         if (p.presum && !table_index && presum_fits(p, n_time, n_bl, n_chan)) {
@@ -329,18 +327,9 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
                 GR_TRY(cudaMemsetAsync(p.counters, 0, 2 * sizeof(unsigned long long), s));   // counted again below
             }
         }
-        if (p.run_cap > 0 && !p.presum_active) {
-            GR_TRY(launch_bin_runs(p, uvw, scale, n, n_chan, s, &by_runs));
-            if (by_runs) {
-                stage_mark(p, 2, s);
-            } else {
-                p.n_runs = 0;
-                GR_TRY(cudaMemsetAsync(p.counters, 0, 2 * sizeof(unsigned long long), s));   // counted again below
-            }
-        }
         if (!by_runs) {
             MapParams mp = make_map_params(p);
-            mp.table_index = p.mode != 0 ? table_index : nullptr;
+            mp.table_index = table_index;
             if (p.mode == 0)
                 map_kernel<false><<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(uvw, scale, (unsigned)n, (unsigned)n_chan, mp,
                                                                               p.keys[0], p.vals[0], p.counters);
@@ -362,7 +351,7 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
             stage_mark(p, 2, s);
             p.n_launches += 4;
         }
-        if (!by_runs) {       // (the runs path has built the 'first' / 'last' tables from the runs)
+        if (!by_runs) {
             tile_bounds_kernel<<<blocks_for(n, 256, p.n_sm), 256, 0, s>>>(p.keys[p.sorted_sel], n,
                                                                             p.key.tile_shift, p.tile_start, tile_end);
             GR_TRY(cudaGetLastError());

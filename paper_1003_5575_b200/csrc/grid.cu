@@ -592,686 +592,6 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
 }
 
 // ------------------------------------------------------------------------------------------
-// The fast path with PER-ORIGIN BINS (one real table in shared memory, 16 x 16 patch, merging on).
-// Entries of a work item are sorted by patch origin, and for one origin there are only O^2 possible
-// sub-cell offsets, i.e. O^2 different sets of taps.  So the weighted visibilities of an origin are
-// first summed into O^2 bins of shared memory (512 B per warp at O = 4) and only when the origin
-// changes are the non-empty bins gridded (256 FMAs each) -- at most O^2 records per (item, origin)
-// however many entries it has; exact by linearity like the per-batch merging of stage_write, of
-// which this is the complete form.  Fixed order: inside a batch the first lane of a group adds the
-// others in ascending lane order, batches are added to the bins in sequence, bins are gridded in
-// offset order: bit-identical reruns.  FP32 chains: <= 32 (batch), <= K/32 (bin), <= O^2 records
-// in registers per origin, then the fold: inside the budget of DESIGN.md section 7.
-// Pipeline per warp: sorted (key, index) pairs three batches ahead in registers, visibilities two
-// batches ahead (cp.async into three landing buffers); a batch is accumulated straight out of its
-// landing buffer, there is no record ring.
-// ------------------------------------------------------------------------------------------
-template <int TLOG, int MAXW>
-__global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel_qbins(const GridParams p) {
-    constexpr int NA = 2, NB = 4, NRAW = 3;
-    using G = Geo<NA, NB, 1, TLOG, 0>;
-    extern __shared__ float4 smem[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n_q = p.n_q;                                     // O^2 <= 64 bins
-    const int warp_f4 = 2 * G::CELLS + 2 * n_q + NRAW * G::RAW_F4;
-    float4 *region = smem + p.coef_f4 + warp * warp_f4;        // plane A (XX, XY) then plane B (YX, YY)
-    float4 *regA = region, *regB = region + G::CELLS;
-    float4 *bins = region + 2 * G::CELLS;                      // [2][q] float4: sum of w V of the current origin
-    float4 *raw = bins + 2 * n_q;                              // NRAW cp.async landing buffers
-
-    for (int i = threadIdx.x; i < p.coef_f4; i += blockDim.x) smem[i] = p.coef[i];
-    for (int i = lane; i < warp_f4; i += 32) region[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    __syncthreads();
-
-    const int lane_cell = (lane >> 3) * G::RW + (lane & 7);
-    const char *coef_lane = reinterpret_cast<const char *>((uintptr_t)((uint32_t)__cvta_generic_to_shared(smem) +
-                                                                        lane * NB * (int)sizeof(float)));
-    float acc[NA][NB][8];
-#pragma unroll
-    for (int a = 0; a < NA; ++a)
-#pragma unroll
-        for (int b = 0; b < NB; ++b)
-#pragma unroll
-            for (int k = 0; k < 8; ++k) acc[a][b][k] = 0.f;
-
-    Producer prod;
-    prod.init(p, lane, 0);
-    // batch i is processed while i+1 and i+2 are landing and i+3 has its pairs in flight
-    Desc d0, d1, d2, d3;
-    Entry e0, e1, e2, e3;
-    d0.bits = 0; d0.item = 0; d1 = d0; d2 = d0;
-    e0.key = e0.idx = e0.aux = 0u; e1 = e0; e2 = e0;
-    {
-        unsigned start;
-        d3 = prod.next(p, lane, start);
-        e3 = load_entry<false>(p, start + lane, lane < d3.cnt());
-    }
-    unsigned long long n_exec = 0;
-    const uint32_t tmask = (1u << TLOG) - 1u, qmask = (1u << (2 * p.key.bits_q)) - 1u;
-    int cur = -1, cmp = kSentinel;
-    int bin_org = kSentinel;             // origin the bins belong to
-    unsigned long long occ = 0;          // its non-empty bins
-    int slot = 0;                        // landing buffer of batch i
-
-    while (true) {
-        // batch i+2's visibilities start to move; batch i+3 gets its pairs; then batch i must have landed
-        d0 = d1; e0 = e1; d1 = d2; e1 = e2; d2 = d3; e2 = e3;
-        issue_vis<false>(p, raw + ((slot + 2) % NRAW) * G::RAW_F4, lane, e2, lane < d2.cnt());
-        {
-            unsigned start;
-            d3 = prod.next(p, lane, start);
-            e3 = load_entry<false>(p, start + lane, lane < d3.cnt());
-        }
-        asm volatile("cp.async.wait_group 2;" ::: "memory");
-        __syncwarp();
-        if (d0.end()) break;
-        const int cnt = d0.cnt();
-        if (cnt > 0) {
-            const float4 *rw = raw + slot * G::RAW_F4;
-            const uint32_t x0l = (e0.key >> p.key.aux_bits) & tmask, y0l = (e0.key >> (p.key.aux_bits + TLOG)) & tmask;
-            const bool valid = lane < cnt;
-            const int poff = valid ? (int)(y0l * G::RW + x0l) : kForce;
-            const int q = (int)(e0.key & qmask);
-            const float4 ra = rw[lane], rb = rw[32 + lane];
-            const float w = p.weight ? reinterpret_cast<const float *>(rw + 64)[lane] : 1.0f;
-            const float o[8] = {ra.x * w, ra.y * w, ra.z * w, ra.w * w, rb.x * w, rb.y * w, rb.z * w, rb.w * w};
-            float sum[8];
-#pragma unroll
-            for (int k = 0; k < 8; ++k) sum[k] = o[k];
-            // Sum inside the batch.  Neighbouring channels of a baseline are neighbours in the sorted list and
-            // mostly share (origin, offset): first a segmented tree reduction over RUNS of equal lanes (five
-            // shuffle steps whatever the run lengths), then the heads of runs with equal (origin, offset) --
-            // rare -- are added into the first of them one by one.  Fixed order, so reruns are bit-identical.
-            const unsigned gkey = valid ? (((unsigned)poff << 8) | (unsigned)q) : (0xFFFF0000u | lane);
-            const unsigned gprev = __shfl_up_sync(0xffffffffu, gkey, 1);
-            const bool head = lane == 0 || gprev != gkey;
-            const unsigned heads = __ballot_sync(0xffffffffu, head);
-            const unsigned above = lane == 31 ? 0u : (heads & (0xFFFFFFFEu << lane));
-            const int run_end = above ? __ffs(above) - 1 : 32;         // first lane of the next run
-#pragma unroll
-            for (int dlt = 1; dlt < 32; dlt <<= 1) {
-                const bool add = lane + dlt < run_end;
-#pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    const float t = __shfl_down_sync(0xffffffffu, sum[k], dlt);
-                    if (add) sum[k] += t;
-                }
-            }
-            const unsigned grp = __match_any_sync(0xffffffffu, head ? gkey : (0xFFFF0000u | lane));
-            const bool keep = valid && head && (__ffs(grp) - 1 == lane);
-            unsigned rest = keep ? (grp & ~(1u << lane)) : 0u;
-            if (__any_sync(0xffffffffu, rest != 0u)) {
-                float hs[8];                                           // the run sums as the heads hold them now
-#pragma unroll
-                for (int k = 0; k < 8; ++k) hs[k] = sum[k];
-                do {
-                    const int src = rest ? __ffs(rest) - 1 : lane;
-                    const bool add = rest != 0u;
-                    rest &= rest - 1u;
-#pragma unroll
-                    for (int k = 0; k < 8; ++k) {
-                        const float t = __shfl_sync(0xffffffffu, hs[k], src);
-                        if (add) sum[k] += t;
-                    }
-                } while (__any_sync(0xffffffffu, rest != 0u));
-            }
-            // origin by origin (the batch is sorted by origin); one more round with no origin ends the item
-            int lp = 0;
-            const bool last = d0.last();
-            while (lp < cnt || (last && lp == cnt)) {
-                const int seg = lp < cnt ? __shfl_sync(0xffffffffu, poff, lp) : kSentinel;
-                if (seg != bin_org) {
-                    // ---- grid the bins of the finished origin ------------------------------------------
-                    if (occ) {
-                        RecRegs<NA, NB, 0> A, B;
-                        unsigned long long m = occ;
-                        int qa = __ffsll((long long)m) - 1, qb;
-                        m &= m - 1ull;
-                        A.fetch2(bins + qa, bins + n_q + qa, qa * G::SUB_BYTES, coef_lane);
-                        while (true) {
-                            qb = m ? __ffsll((long long)m) - 1 : -1;
-                            m &= m - 1ull;
-                            if (qb >= 0) B.fetch2(bins + qb, bins + n_q + qb, qb * G::SUB_BYTES, coef_lane);
-                            consume<NA, NB, G::RW, 0>(A, bin_org, cur, cmp, regA, regB, lane_cell, acc);
-                            if (qb < 0) break;
-                            qa = m ? __ffsll((long long)m) - 1 : -1;
-                            m &= m - 1ull;
-                            if (qa >= 0) A.fetch2(bins + qa, bins + n_q + qa, qa * G::SUB_BYTES, coef_lane);
-                            consume<NA, NB, G::RW, 0>(B, bin_org, cur, cmp, regA, regB, lane_cell, acc);
-                            if (qa < 0) break;
-                        }
-                        n_exec += (unsigned)__popcll(occ);
-                        __syncwarp();
-                        for (int k = lane; k < 2 * n_q; k += 32) bins[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-                        occ = 0;
-                        __syncwarp();
-                    }
-                    bin_org = seg;
-                }
-                if (lp >= cnt) break;
-                // ---- this origin's lanes of the batch go into the bins ---------------------------------
-                const bool in_seg = poff == seg;
-                const bool put = in_seg && keep;
-                if (put) {               // the kept lanes of one origin have distinct offsets
-                    float4 x = bins[q], y = bins[n_q + q];
-                    x.x += sum[0]; x.y += sum[1]; x.z += sum[2]; x.w += sum[3];
-                    y.x += sum[4]; y.y += sum[5]; y.z += sum[6]; y.w += sum[7];
-                    bins[q] = x; bins[n_q + q] = y;
-                }
-                const unsigned lo = __reduce_or_sync(0xffffffffu, (put && q < 32) ? (1u << q) : 0u);
-                const unsigned hi = __reduce_or_sync(0xffffffffu, (put && q >= 32) ? (1u << (q - 32)) : 0u);
-                occ |= ((unsigned long long)hi << 32) | lo;
-                lp += __popc(__ballot_sync(0xffffffffu, in_seg));
-                __syncwarp();
-            }
-            if (last) {
-                // the item's last origin has been gridded; fold it, write the region out, clear it
-                if (cur >= 0) fold_patch<NA, NB, G::RW>(regA, regB, cur + lane_cell, acc);
-                cur = -1; cmp = kSentinel; bin_org = kSentinel;
-                __syncwarp();
-                float4 *dst = p.partials + (size_t)d0.item * (2 * G::CELLS);
-                for (int k = lane; k < 2 * G::CELLS; k += 32) {
-                    stg_stream(dst + k, region[k]);
-                    region[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-                }
-                __syncwarp();
-            }
-        }
-        slot = (slot + 1) % NRAW;
-    }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-    if (lane == 0 && n_exec) atomicAdd(&p.counters->n_exec[p.cls], n_exec);
-}
-
-// ------------------------------------------------------------------------------------------
-// PRE-SUMMATION of a dense plan's entries (fast path, O^2 <= 16 sub-cell offsets).
-// When a tile holds many more entries than it has (origin, offset) pairs -- T^2 O^2 = 256 at
-// T = O = 4 -- it pays to add the weighted visibilities of every pair first (8 FMAs per entry) and to
-// grid each non-empty pair once (2048 FMAs): sum_i C_q w_i V_i = C_q sum_i w_i V_i, exact by
-// linearity like the per-batch merging of stage_write, of which this is the complete form.  This
-// kernel does the adding: per work item it writes RECORDS (origin | offset, sum of w V), origin by
-// origin; grid_kernel then runs on the records exactly as it runs on entries (keys = record keys,
-// visibilities = record sums, no weights, nothing left to merge).  BASELINE.json config 4: 16.5
-// entries per record.
-//
-// A warp walks its items' entries 64 at a time, two per lane (its own queue of work items; sorted pairs
-// and visibilities land in rings of shared memory by cp.async, two to four batches ahead).  Entries of one origin are consecutive.
-// Every lane PAIR (l, l + 16) keeps private bins for the O^2 offsets of the current origin in shared
-// memory ([offset][half][l] float4: conflict-free whatever the offsets are); the two half-warps add
-// their entries to their bins in turn, so no two lanes ever touch the same word at the same time and
-// there is nothing to match, merge or serialise.
-// When the origin changes (or after 1024 entries, which bounds the FP32 chain of a bin copy at 64) the 16
-// private copies of each bin are added in a fixed order -- lane (q, h) adds the 16 copies of half h of bin
-// q one after the other -- into registers, and at the end of the origin the non-empty bins are
-// written out as records in offset order.  All orders are fixed: reruns are bit-identical.
-// ------------------------------------------------------------------------------------------
-constexpr int kRedWarps = 13, kRedPiece = 32;      // (a copy is shared by two lanes: chains <= 64)
-constexpr int kRedBins = 16;                                   // O^2 <= 16
-constexpr int kRedCopies = 16;                                 // private copies of a bin: lanes l and l + 16 share one
-constexpr int kRedBatch = 64;                                  // entries per batch: two per lane
-constexpr int kRedVis = 3, kRedVisF4 = 2 * (32 * 2 + 8);       // landing ring of the visibilities: 2 x (a, b, weight)
-constexpr int kRedKey = 5, kRedKeyF4 = 32;                     // ring of the sorted pairs: 64 keys, 64 indices
-constexpr int kRedWarpF4 = kRedBins * 2 * kRedCopies + kRedVis * kRedVisF4 + kRedKey * kRedKeyF4 + 8;
-
-__global__ void __launch_bounds__(kRedWarps * 32, 1) reduce_kernel(const GridParams p) {
-    extern __shared__ float4 smem[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float4 *priv = smem + (size_t)warp * kRedWarpF4;           // [q][half][lane & 15]
-    float4 *vring = priv + kRedBins * 2 * kRedCopies;                  // kRedVis x 2 x {a[32], b[32], w[32]}
-    uint32_t *kring = reinterpret_cast<uint32_t *>(vring + kRedVis * kRedVisF4);   // kRedKey x {key[64], idx[64]}
-    uint4 *dring = reinterpret_cast<uint4 *>(kring + kRedKey * 128);                // kRedKey batch descriptors
-    for (int i = lane; i < kRedWarpF4; i += 32) priv[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    __syncwarp();
-
-    const int tl2 = 2 * p.key.tlog;
-    const uint32_t omask = (1u << tl2) - 1u, qmask = (1u << (2 * p.key.bits_q)) - 1u;
-    const uint32_t dropbit = 1u << (2 * p.key.bits_q);
-    const unsigned item_begin = p.counters->cls_begin[p.cls], item_end = p.counters->cls_end[p.cls];
-    const uint32_t *idx_sorted = reinterpret_cast<const uint32_t *>(p.vals);
-    // the lane's part in adding the private copies: half bh of bin bq (row lane of the [q][half] table)
-    const int bq = lane >> 1, bh = lane & 1;
-    const int cl = lane & (kRedCopies - 1);
-
-    float4 bacc = make_float4(0.f, 0.f, 0.f, 0.f);     // sum of (bq, bh) over the pieces of the origin
-    unsigned touched = 0;                // this lane's private bins that hold something
-    unsigned occ = 0;                    // bins of the origin that hold something (all pieces)
-    int bin_org = -1, piece = 0;
-    unsigned n_rec = 0;
-    size_t rec_base = 0;
-
-    // ---- the warp's stream of batches: <= 64 consecutive entries of one work item (lane: e and e + 32) ---
-    // descriptor: x = first entry, y = count | first batch of its item << 8 | last << 9 | end of stream << 10,
-    // z = item (relative to the class)
-    unsigned cur_id = 0, cur_start = 0, cur_len = 0, cur_off = 0;      // the item the batches are cut from
-    unsigned nxt_id = 0, nxt_start = 0, nxt_len = 0;                   // claimed one item ahead
-    bool nxt_ok = false, gen_end = false;
-    auto claim = [&]() {
-        unsigned it = 0;
-        if (lane == 0) it = atomicAdd(&p.counters->queue_head[p.cls], 1u);
-        nxt_id = __shfl_sync(0xffffffffu, it, 0);
-        nxt_ok = item_begin + nxt_id < item_end;
-        nxt_start = nxt_len = 0;
-        if (nxt_ok) {
-            const WorkItem w = p.items[item_begin + nxt_id];
-            nxt_start = w.start;
-            nxt_len = w.len;
-        }
-    };
-    // batch m: its descriptor into the ring, the copies of its sorted pairs started
-    auto gen_batch = [&](int ks) {
-        if (!gen_end && cur_off >= cur_len) {
-            if (!nxt_ok) gen_end = true;
-            else {
-                cur_id = nxt_id; cur_start = nxt_start; cur_len = nxt_len; cur_off = 0;
-                claim();
-            }
-        }
-        uint4 d = make_uint4(0u, 1u << 10, 0u, 0u);
-        if (!gen_end) {
-            const unsigned left = cur_len - cur_off;
-            d.x = cur_start + cur_off;
-            d.y = min((unsigned)kRedBatch, left) | (cur_off == 0u ? 256u : 0u) | (left <= (unsigned)kRedBatch ? 512u : 0u);
-            d.z = cur_id;
-            cur_off += (unsigned)kRedBatch;
-        }
-        if (lane == 0) dring[ks] = d;
-        const int cnt = (int)(d.y & 255u);
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            const bool v = lane + 32 * u < cnt;
-            cp_async_4(kring + ks * 128 + 32 * u + lane, p.keys + d.x + (v ? 32 * u + lane : 0), v);
-            cp_async_4(kring + ks * 128 + 64 + 32 * u + lane, idx_sorted + d.x + (v ? 32 * u + lane : 0), v);
-        }
-    };
-    // batch m (its pairs have landed): the copies of its visibilities started
-    auto gen_vis = [&](int ks, int vs) {
-        const int cnt = (int)(dring[ks].y & 255u);
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            const uint32_t key = kring[ks * 128 + 32 * u + lane], idx = kring[ks * 128 + 64 + 32 * u + lane];
-            const bool live = lane + 32 * u < cnt && !(key & dropbit);
-            float4 *dst = vring + vs * kRedVisF4 + u * (kRedVisF4 / 2);
-            const float4 *src = p.vis + 2 * (size_t)(live ? idx : 0u);
-            cp_async_16(dst + lane, src, live);
-            cp_async_16(dst + 32 + lane, src + 1, live);
-            if (p.weight) cp_async_4(reinterpret_cast<float *>(dst + 64) + lane, p.weight + (live ? idx : 0u), live);
-        }
-    };
-
-    claim();
-    // prologue: batches 0..3 have their pairs moving, then 0 and 1 their visibilities
-    for (int m = 0; m < 4; ++m) {
-        gen_batch(m);
-        cp_async_commit();
-    }
-    asm volatile("cp.async.wait_group 2;" ::: "memory");          // pairs of batches 0 and 1
-    __syncwarp();
-    for (int m = 0; m < 2; ++m) {
-        gen_vis(m, m);
-        cp_async_commit();
-    }
-
-    // iteration n: pairs of batch n+4 and visibilities of batch n+2 start to move (one group), batch n is added
-    int kn = 0, vn = 0;                  // ring slots of batch n
-#pragma unroll 1
-    while (true) {
-        asm volatile("cp.async.wait_group 1;" ::: "memory");      // groups up to iteration n-2: pairs(n+2), vis(n)
-        __syncwarp();
-        gen_batch(kn + 4 < kRedKey ? kn + 4 : kn + 4 - kRedKey);
-        gen_vis(kn + 2 < kRedKey ? kn + 2 : kn + 2 - kRedKey, vn + 2 < kRedVis ? vn + 2 : vn + 2 - kRedVis);
-        cp_async_commit();
-        const uint4 d = dring[kn];
-        if (d.y & 1024u) break;
-        const int cnt = (int)(d.y & 255u);
-        {
-            const float4 *rw = vring + vn * kRedVisF4;
-            if (d.y & 256u) {            // first batch of an item: where its records go
-                n_rec = 0;
-                rec_base = p.rec_slot ? (size_t)d.z * p.rec_slot : (size_t)d.x;
-            }
-            const uint32_t key0 = kring[kn * 128 + lane], key1 = kring[kn * 128 + 32 + lane];
-            const int org0 = lane < cnt ? (int)((key0 >> p.key.aux_bits) & omask) : -2;
-            const int org1 = lane + 32 < cnt ? (int)((key1 >> p.key.aux_bits) & omask) : -2;
-            const int q0 = (int)(key0 & qmask), q1 = (int)(key1 & qmask);
-            const float w0 = p.weight ? reinterpret_cast<const float *>(rw + 64)[lane] : 1.0f;
-            const float w1 = p.weight ? reinterpret_cast<const float *>(rw + kRedVisF4 / 2 + 64)[lane] : 1.0f;
-            const float4 a0 = rw[lane], b0 = rw[32 + lane];
-            const float4 a1 = rw[kRedVisF4 / 2 + lane], b1 = rw[kRedVisF4 / 2 + 32 + lane];
-            const bool last = d.y & 512u;
-            int lp = 0;
-            // origin by origin; one more round with no origin ends the item
-#pragma unroll 1
-            while (lp < cnt || (last && lp == cnt)) {
-                const int seg = lp < cnt ? __shfl_sync(0xffffffffu, lp < 32 ? org0 : org1, lp & 31) : -1;
-                const bool change = seg != bin_org;
-                if ((change && bin_org >= 0) || piece >= kRedPiece) {
-                    // ---- the 16 private copies of every bin are added into bacc and cleared: lane (q, h) adds
-                    // half h of bin q, copy by copy in a fixed (rotated: conflict-free) order
-                    __syncwarp();
-                    occ |= __reduce_or_sync(0xffffffffu, touched);
-                    {
-                        const float4 *src = priv + lane * kRedCopies;        // row (q * 2 + h) = lane
-                        float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-                        for (int j = 0; j < kRedCopies; ++j) {
-                            const float4 v = src[(j + lane) & (kRedCopies - 1)];
-                            t.x += v.x; t.y += v.y; t.z += v.z; t.w += v.w;
-                        }
-                        bacc.x += t.x; bacc.y += t.y; bacc.z += t.z; bacc.w += t.w;
-                    }
-                    __syncwarp();
-                    for (unsigned m = touched; m; m &= m - 1u) {     // (lanes l and l + 16 may clear the same words)
-                        const int qq = __ffs(m) - 1;
-                        priv[(qq * 2) * kRedCopies + cl] = make_float4(0.f, 0.f, 0.f, 0.f);
-                        priv[(qq * 2 + 1) * kRedCopies + cl] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    }
-                    touched = 0;
-                    piece = 0;
-                    __syncwarp();
-                    if (change) {
-                        // ---- the origin is complete: its non-empty bins become records, in offset order ----
-                        if ((occ >> bq) & 1u) {
-                            const size_t r = rec_base + n_rec + (unsigned)__popc(occ & ((1u << bq) - 1u));
-                            p.rec_sum[2 * r + bh] = bacc;
-                            if (bh == 0) p.rec_key[r] = ((uint32_t)bin_org << p.key.aux_bits) | (uint32_t)bq;
-                        }
-                        bacc = make_float4(0.f, 0.f, 0.f, 0.f);
-                        n_rec += (unsigned)__popc(occ);
-                        occ = 0;
-                    }
-                }
-                bin_org = seg;
-                if (lp >= cnt) break;
-                // the lane's two entries: into its copy of the bins (one read-modify-write when they share the
-                // offset); lanes l and l + 16 share a copy, so the two half-warps take turns
-                const bool in0 = org0 == seg, in1 = org1 == seg;
-                const bool same = in0 && in1 && q0 == q1;
-                float4 *pa0 = priv + (q0 * 2) * kRedCopies + cl, *pa1 = priv + (q1 * 2) * kRedCopies + cl;
-#pragma unroll 1
-                for (int ph = 0; ph < 2; ++ph) {
-                    if ((lane >> 4) == ph) {
-                        // (the addresses are valid whatever the lane holds: loads are unconditional, stores are not)
-                        float4 x0 = pa0[0], y0 = pa0[kRedCopies];
-                        float4 x1 = pa1[0], y1 = pa1[kRedCopies];
-                        x0.x = fmaf(w0, a0.x, x0.x); x0.y = fmaf(w0, a0.y, x0.y); x0.z = fmaf(w0, a0.z, x0.z); x0.w = fmaf(w0, a0.w, x0.w);
-                        y0.x = fmaf(w0, b0.x, y0.x); y0.y = fmaf(w0, b0.y, y0.y); y0.z = fmaf(w0, b0.z, y0.z); y0.w = fmaf(w0, b0.w, y0.w);
-                        if (same) { x1 = x0; y1 = y0; }
-                        x1.x = fmaf(w1, a1.x, x1.x); x1.y = fmaf(w1, a1.y, x1.y); x1.z = fmaf(w1, a1.z, x1.z); x1.w = fmaf(w1, a1.w, x1.w);
-                        y1.x = fmaf(w1, b1.x, y1.x); y1.y = fmaf(w1, b1.y, y1.y); y1.z = fmaf(w1, b1.z, y1.z); y1.w = fmaf(w1, b1.w, y1.w);
-                        if (in0 && !same) { pa0[0] = x0; pa0[kRedCopies] = y0; }
-                        if (in1) { pa1[0] = x1; pa1[kRedCopies] = y1; }
-                    }
-                    __syncwarp();
-                }
-                if (in0) touched |= 1u << q0;
-                if (in1) touched |= 1u << q1;
-                piece += 2;
-                lp += __popc(__ballot_sync(0xffffffffu, in0)) + __popc(__ballot_sync(0xffffffffu, in1));
-            }
-            if (last && lane == 0) {     // the item's entry in the record items
-                WorkItem ri;
-                ri.start = (uint32_t)rec_base;
-                ri.len = n_rec;
-                ri.tile = 0;
-                ri.pad = 0;
-                p.rec_items[item_begin + d.z] = ri;
-            }
-        }
-        kn = kn + 1 < kRedKey ? kn + 1 : 0;
-        vn = vn + 1 < kRedVis ? vn + 1 : 0;
-    }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-}
-
-// The same pre-summation straight from the SORTED CHANNEL RUNS (runs.cu), so that the per-entry sorted
-// list never has to be written (expand_kernel: 3.7 ms and 6.4 GB on config 4) or read.  Entry e of the
-// sorted order belongs to the run r with rcum[r] <= e < rcum[r + 1]; it is visibility start[r] + (e - rcum[r]),
-// its origin is in the run's key and its sub-cell offsets (and drop flag) are the byte qaux[visibility].
-// Batches are cut at multiples of 64 of the global entry position, and blk_run[e / 64] (block_run_kernel)
-// names the run holding position 64 (e / 64): the 64 runs from there on cover the batch (a run has at least
-// one entry), so a lane finds its run by a 6-step search in a window of shared memory.  Four stages run
-// ahead of the adding, each through its own ring: descriptor + blk_run word (6 batches ahead), run window
-// (4), visibilities + weight + qaux word (2).  Same records, same order of additions, same bits as
-// reduce_kernel.
-constexpr int kRunWin = 4, kRunWinU32 = 192;                   // ring of run windows: cum[64], start[64], key[64]
-constexpr int kRunEnt = 3, kRunEntF4 = 2 * (32 * 2 + 8) + 32;  // ring of entries: 2 x (a, b, weight), then okey[64], qword[64]
-constexpr int kRunDesc = 8;
-constexpr int kRunWarps = 11;
-constexpr int kRunWarpF4 = kRedBins * 2 * kRedCopies + kRunEnt * kRunEntF4 + kRunWin * kRunWinU32 / 4 + kRunDesc;
-
-__global__ void __launch_bounds__(kRunWarps * 32, 1) reduce_runs_kernel(const GridParams p) {
-    extern __shared__ float4 smem[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float4 *priv = smem + (size_t)warp * kRunWarpF4;           // [q][half][lane & 15]
-    float4 *ering = priv + kRedBins * 2 * kRedCopies;
-    uint32_t *wring = reinterpret_cast<uint32_t *>(ering + kRunEnt * kRunEntF4);
-    uint4 *dring = reinterpret_cast<uint4 *>(wring + kRunWin * kRunWinU32);
-    for (int i = lane; i < kRunWarpF4; i += 32) priv[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    __syncwarp();
-
-    const int tl2 = 2 * p.key.tlog;
-    const uint32_t omask = (1u << tl2) - 1u, qmask = (1u << (2 * p.key.bits_q)) - 1u;
-    const int dropshift = 2 * p.key.bits_q;
-    const unsigned item_begin = p.counters->cls_begin[p.cls], item_end = p.counters->cls_end[p.cls];
-    // the lane's part in adding the private copies: half bh of bin bq (row lane of the [q][half] table)
-    const int bq = lane >> 1, bh = lane & 1;
-    const int cl = lane & (kRedCopies - 1);
-
-    float4 bacc = make_float4(0.f, 0.f, 0.f, 0.f);     // sum of (bq, bh) over the pieces of the origin
-    unsigned touched = 0;                // this lane's private bins that hold something
-    unsigned occ = 0;                    // bins of the origin that hold something (all pieces)
-    int bin_org = -1, piece = 0;
-    unsigned n_rec = 0;
-    size_t rec_base = 0;
-
-    // ---- the warp's stream of batches: consecutive entries of one work item up to the next multiple of 64
-    // of the global position (lane: positions x + lane and x + 32 + lane).  descriptor: x = first position,
-    // y = count | first batch of its item << 8 | last << 9 | end of stream << 10, z = item, w = blk_run[x / 64]
-    unsigned cur_id = 0, cur_pos = 0, cur_end = 0;                     // the item the batches are cut from
-    bool cur_first = false;
-    unsigned nxt_id = 0, nxt_start = 0, nxt_len = 0;                   // claimed one item ahead
-    bool nxt_ok = false, gen_end = false;
-    auto claim = [&]() {
-        unsigned it = 0;
-        if (lane == 0) it = atomicAdd(&p.counters->queue_head[p.cls], 1u);
-        nxt_id = __shfl_sync(0xffffffffu, it, 0);
-        nxt_ok = item_begin + nxt_id < item_end;
-        nxt_start = nxt_len = 0;
-        if (nxt_ok) {
-            const WorkItem w = p.items[item_begin + nxt_id];
-            nxt_start = w.start;
-            nxt_len = w.len;
-        }
-    };
-    // stage 1, batch m: its descriptor into the ring, the copy of its blk_run word started
-    auto gen_desc = [&](int m) {
-        if (!gen_end && cur_pos >= cur_end) {
-            if (!nxt_ok) gen_end = true;
-            else {
-                cur_id = nxt_id; cur_pos = nxt_start; cur_end = nxt_start + nxt_len; cur_first = true;
-                claim();
-            }
-        }
-        uint4 d = make_uint4(0u, 1u << 10, 0u, 0u);
-        if (!gen_end) {
-            const unsigned stop = min(cur_end, (cur_pos | 63u) + 1u);
-            d.x = cur_pos;
-            d.y = (stop - cur_pos) | (cur_first ? 256u : 0u) | (stop == cur_end ? 512u : 0u);
-            d.z = cur_id;
-            cur_pos = stop;
-            cur_first = false;
-        }
-        uint4 *slot = dring + (m & (kRunDesc - 1));
-        if (lane == 0) {
-            *reinterpret_cast<uint3 *>(slot) = make_uint3(d.x, d.y, d.z);
-            cp_async_4(&slot->w, p.blk_run + (d.x >> 6), !(d.y & 1024u));
-        }
-    };
-    // stage 2, batch m (its blk_run word has landed): the copies of its window of 64 runs started
-    auto gen_window = [&](int m) {
-        const uint4 d = dring[m & (kRunDesc - 1)];
-        uint32_t *w = wring + (m & (kRunWin - 1)) * kRunWinU32;
-        const bool live = !(d.y & 1024u);
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            const unsigned r = d.w + 32 * u + lane;
-            const bool v = live && r < p.n_runs;
-            if (v) cp_async_4(w + 32 * u + lane, p.rcum + r, true);
-            else w[32 * u + lane] = 0xFFFFFFFFu;             // beyond the last run: never chosen by the search
-            cp_async_4(w + 64 + 32 * u + lane, p.rstart + 2 * (size_t)(v ? r : 0u), v);
-            cp_async_4(w + 128 + 32 * u + lane, p.rkey + (v ? r : 0u), v);
-        }
-    };
-    // stage 3, batch m (its window has landed): every lane finds the runs of its two entries, notes origin
-    // and byte position, and starts the copies of visibility, weight and the qaux word
-    auto gen_entries = [&](int m, int es) {
-        const uint4 d = dring[m & (kRunDesc - 1)];
-        const uint32_t *w = wring + (m & (kRunWin - 1)) * kRunWinU32;
-        const int cnt = (int)(d.y & 255u);
-        float4 *dst0 = ering + es * kRunEntF4;
-        uint32_t *okey = reinterpret_cast<uint32_t *>(dst0 + 2 * (32 * 2 + 8));
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            const bool v = lane + 32 * u < cnt;
-            const unsigned pos = d.x + 32 * u + lane;
-            int j = 0;
-#pragma unroll
-            for (int st = 32; st >= 1; st >>= 1)
-                if (w[j + st] <= pos) j += st;
-            const unsigned idx = v ? w[64 + j] + (pos - w[j]) : 0u;
-            okey[32 * u + lane] = ((w[128 + j] >> p.key.aux_bits) & omask) | ((idx & 3u) << 16);
-            float4 *dst = dst0 + u * (32 * 2 + 8);
-            const float4 *src = p.vis + 2 * (size_t)idx;
-            cp_async_16(dst + lane, src, v);
-            cp_async_16(dst + 32 + lane, src + 1, v);
-            if (p.weight) cp_async_4(reinterpret_cast<float *>(dst + 64) + lane, p.weight + idx, v);
-            cp_async_4(okey + 64 + 32 * u + lane, p.qaux + (idx & ~3u), v);
-        }
-    };
-
-    claim();
-    // iteration n: stages 1, 2, 3 for batches n + 6, n + 4, n + 2 (one cp.async group), batch n is added; the
-    // first six iterations only fill the pipeline
-    int es_n = 0, es_n2 = 2;             // entry-ring slots of batches n and n + 2 (n = -6: any)
-#pragma unroll 1
-    for (int n = -6;; ++n) {
-        asm volatile("cp.async.wait_group 1;" ::: "memory");      // everything up to iteration n - 2 has landed
-        __syncwarp();
-        gen_desc(n + 6);
-        if (n + 4 >= 0) gen_window(n + 4);
-        if (n + 2 >= 0) gen_entries(n + 2, es_n2);
-        cp_async_commit();
-        if (n >= 0) {
-        const uint4 d = dring[n & (kRunDesc - 1)];
-        if (d.y & 1024u) break;
-        const int cnt = (int)(d.y & 255u);
-        {
-            const float4 *rw = ering + es_n * kRunEntF4;
-            const uint32_t *okey = reinterpret_cast<const uint32_t *>(rw + 2 * (32 * 2 + 8));
-            if (d.y & 256u) {            // first batch of an item: where its records go
-                n_rec = 0;
-                rec_base = p.rec_slot ? (size_t)d.z * p.rec_slot : (size_t)d.x;
-            }
-            const uint32_t k0 = okey[lane], k1 = okey[32 + lane];
-            const uint32_t qb0 = (okey[64 + lane] >> (8 * (k0 >> 16))) & 255u;
-            const uint32_t qb1 = (okey[96 + lane] >> (8 * (k1 >> 16))) & 255u;
-            const int org0 = lane < cnt ? (int)(k0 & 0xFFFFu) : -2;
-            const int org1 = lane + 32 < cnt ? (int)(k1 & 0xFFFFu) : -2;
-            const int q0 = (int)(qb0 & qmask), q1 = (int)(qb1 & qmask);
-            const bool drop0 = (qb0 >> dropshift) & 1u, drop1 = (qb1 >> dropshift) & 1u;      // dropped: adds nothing
-            const float w0 = drop0 ? 0.0f : (p.weight ? reinterpret_cast<const float *>(rw + 64)[lane] : 1.0f);
-            const float w1 = drop1 ? 0.0f : (p.weight ? reinterpret_cast<const float *>(rw + (32 * 2 + 8) + 64)[lane] : 1.0f);
-            const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
-            const float4 a0 = drop0 ? z4 : rw[lane], b0 = drop0 ? z4 : rw[32 + lane];
-            const float4 a1 = drop1 ? z4 : rw[(32 * 2 + 8) + lane], b1 = drop1 ? z4 : rw[(32 * 2 + 8) + 32 + lane];
-            const bool last = d.y & 512u;
-            int lp = 0;
-            // origin by origin; one more round with no origin ends the item
-#pragma unroll 1
-            while (lp < cnt || (last && lp == cnt)) {
-                const int seg = lp < cnt ? __shfl_sync(0xffffffffu, lp < 32 ? org0 : org1, lp & 31) : -1;
-                const bool change = seg != bin_org;
-                if ((change && bin_org >= 0) || piece >= kRedPiece) {
-                    // ---- the 16 private copies of every bin are added into bacc and cleared: lane (q, h) adds
-                    // half h of bin q, copy by copy in a fixed (rotated: conflict-free) order
-                    __syncwarp();
-                    occ |= __reduce_or_sync(0xffffffffu, touched);
-                    {
-                        const float4 *src = priv + lane * kRedCopies;        // row (q * 2 + h) = lane
-                        float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-                        for (int j = 0; j < kRedCopies; ++j) {
-                            const float4 v = src[(j + lane) & (kRedCopies - 1)];
-                            t.x += v.x; t.y += v.y; t.z += v.z; t.w += v.w;
-                        }
-                        bacc.x += t.x; bacc.y += t.y; bacc.z += t.z; bacc.w += t.w;
-                    }
-                    __syncwarp();
-                    for (unsigned m = touched; m; m &= m - 1u) {     // (lanes l and l + 16 may clear the same words)
-                        const int qq = __ffs(m) - 1;
-                        priv[(qq * 2) * kRedCopies + cl] = make_float4(0.f, 0.f, 0.f, 0.f);
-                        priv[(qq * 2 + 1) * kRedCopies + cl] = make_float4(0.f, 0.f, 0.f, 0.f);
-                    }
-                    touched = 0;
-                    piece = 0;
-                    __syncwarp();
-                    if (change) {
-                        // ---- the origin is complete: its non-empty bins become records, in offset order ----
-                        if ((occ >> bq) & 1u) {
-                            const size_t r = rec_base + n_rec + (unsigned)__popc(occ & ((1u << bq) - 1u));
-                            p.rec_sum[2 * r + bh] = bacc;
-                            if (bh == 0) p.rec_key[r] = ((uint32_t)bin_org << p.key.aux_bits) | (uint32_t)bq;
-                        }
-                        bacc = make_float4(0.f, 0.f, 0.f, 0.f);
-                        n_rec += (unsigned)__popc(occ);
-                        occ = 0;
-                    }
-                }
-                bin_org = seg;
-                if (lp >= cnt) break;
-                // the lane's two entries: into its copy of the bins (one read-modify-write when they share the
-                // offset); lanes l and l + 16 share a copy, so the two half-warps take turns
-                const bool in0 = org0 == seg, in1 = org1 == seg;
-                const bool same = in0 && in1 && q0 == q1;
-                float4 *pa0 = priv + (q0 * 2) * kRedCopies + cl, *pa1 = priv + (q1 * 2) * kRedCopies + cl;
-#pragma unroll 1
-                for (int ph = 0; ph < 2; ++ph) {
-                    if ((lane >> 4) == ph) {
-                        // (the addresses are valid whatever the lane holds: loads are unconditional, stores are not)
-                        float4 x0 = pa0[0], y0 = pa0[kRedCopies];
-                        float4 x1 = pa1[0], y1 = pa1[kRedCopies];
-                        x0.x = fmaf(w0, a0.x, x0.x); x0.y = fmaf(w0, a0.y, x0.y); x0.z = fmaf(w0, a0.z, x0.z); x0.w = fmaf(w0, a0.w, x0.w);
-                        y0.x = fmaf(w0, b0.x, y0.x); y0.y = fmaf(w0, b0.y, y0.y); y0.z = fmaf(w0, b0.z, y0.z); y0.w = fmaf(w0, b0.w, y0.w);
-                        if (same) { x1 = x0; y1 = y0; }
-                        x1.x = fmaf(w1, a1.x, x1.x); x1.y = fmaf(w1, a1.y, x1.y); x1.z = fmaf(w1, a1.z, x1.z); x1.w = fmaf(w1, a1.w, x1.w);
-                        y1.x = fmaf(w1, b1.x, y1.x); y1.y = fmaf(w1, b1.y, y1.y); y1.z = fmaf(w1, b1.z, y1.z); y1.w = fmaf(w1, b1.w, y1.w);
-                        if (in0 && !same) { pa0[0] = x0; pa0[kRedCopies] = y0; }
-                        if (in1) { pa1[0] = x1; pa1[kRedCopies] = y1; }
-                    }
-                    __syncwarp();
-                }
-                if (in0) touched |= 1u << q0;
-                if (in1) touched |= 1u << q1;
-                piece += 2;
-                lp += __popc(__ballot_sync(0xffffffffu, in0)) + __popc(__ballot_sync(0xffffffffu, in1));
-            }
-            if (last && lane == 0) {     // the item's entry in the record items
-                WorkItem ri;
-                ri.start = (uint32_t)rec_base;
-                ri.len = n_rec;
-                ri.tile = 0;
-                ri.pad = 0;
-                p.rec_items[item_begin + d.z] = ri;
-            }
-        }
-        }
-        es_n = es_n + 1 < kRunEnt ? es_n + 1 : 0;
-        es_n2 = es_n2 + 1 < kRunEnt ? es_n2 + 1 : 0;
-    }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-}
-
-// ------------------------------------------------------------------------------------------
 // Flush: one thread per grid cell.  The partial regions covering cell (x, y) belong to the tiles
 // (ty, tx) with tx*T <= x < tx*T + RW (same in y); each tile's work items are added in id order
 // (full chunks, then the tail).  FP64 accumulation, one rounding to FP32 at the end.  One launch
@@ -1352,11 +672,8 @@ __global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
 // Host side: kernel selection.  The register patch (NA x NB), the sub-patch count and the table
 // mode follow from the plan; TLOG is a plan parameter; the block size is chosen at run time.
 // ------------------------------------------------------------------------------------------
-size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps, int qbins) {
+size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps) {
     const int vf4 = 2;
-    if (qbins > 0)      // grid_kernel_qbins: region, O^2 bins, three landing buffers
-        return table_bytes + (size_t)(2 * g.RW * g.RH + 2 * qbins + 3 * (32 * 2 + 8)) * sizeof(float4) * warps;
-    (void)mode;
     const size_t per_warp = (size_t)(2 * g.RW * g.RH + 2 * 36 * (vf4 + 1) + 32 * 2 + 8) * sizeof(float4);   // Geo::WARP_F4
     (void)tlog;
     return (mode == 0 ? table_bytes : 0) + per_warp * warps;
@@ -1387,20 +704,9 @@ static grid_fn_t pick_shape(const ClassGeo &g, int tlog) {
     return nullptr;
 }
 
-static int kernel_qbins(const Plan &p) { return p.reduce ? 0 : p.qbins; }      // the kernel with its own bins
 static int kernel_mode(const Plan &p) { return (p.mode == 0 && p.tmem_cols > 0) ? 3 : p.mode; }
 
-static grid_fn_t pick_qbins(int tlog) {
-    switch (tlog) {
-        case 2: return grid_kernel_qbins<2, kMaxWarpsFast>;
-        case 3: return grid_kernel_qbins<3, kMaxWarpsFast>;
-        case 4: return grid_kernel_qbins<4, kMaxWarpsFast>;
-        default: return nullptr;
-    }
-}
-
-static grid_fn_t pick_grid(const ClassGeo &g, int tlog, int mode, int qbins = 0) {
-    if (qbins > 0) return pick_qbins(tlog);
+static grid_fn_t pick_grid(const ClassGeo &g, int tlog, int mode) {
     switch (mode) {
         case 0: return pick_shape<0, kMaxWarpsFast>(g, tlog);
         case 3: return pick_shape<3, kMaxWarpsFast>(g, tlog);
@@ -1444,22 +750,14 @@ cudaError_t configure_grid_kernel(Plan &p) {
         for (int w : kWarpChoices) {
             if (w > cap) continue;
             if (p.warps_forced > 0 && w > p.warps_forced) continue;      // the caller's limit (tuning, tests)
-            if (grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, w, kernel_qbins(p)) <= (size_t)smem_max) { chosen = w; break; }
+            if (grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, w) <= (size_t)smem_max) { chosen = w; break; }
         }
         if (!chosen) return cudaErrorInvalidConfiguration;
         g.warps = chosen;
-        g.smem_bytes = (int)grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, chosen, kernel_qbins(p));
-        grid_fn_t fn = pick_grid(g, p.tlog, kernel_mode(p), kernel_qbins(p));
+        g.smem_bytes = (int)grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, chosen);
+        grid_fn_t fn = pick_grid(g, p.tlog, kernel_mode(p));
         if (!fn) return cudaErrorInvalidConfiguration;
         e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes);
-        if (e != cudaSuccess) return e;
-    }
-    if (p.reduce) {
-        e = cudaFuncSetAttribute((const void *)reduce_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)(kRedWarps * kRedWarpF4 * sizeof(float4)));
-        if (e == cudaSuccess && p.fuse)
-            e = cudaFuncSetAttribute((const void *)reduce_runs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)(kRunWarps * kRunWarpF4 * sizeof(float4)));
         if (e != cudaSuccess) return e;
     }
     return cudaSuccess;
@@ -1477,45 +775,9 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         if (e != cudaSuccess) return e;
         stage_mark(p, 7, s);
     }
-    if (p.reduce) {                  // sum the entries into records first; the grid kernel then takes those
-        GridParams rp;
-        memset(&rp, 0, sizeof(rp));
-        rp.keys = p.keys[p.sorted_sel];
-        rp.vals = p.vals[p.sorted_sel];
-        rp.items = p.items;
-        rp.counters = p.counters;
-        rp.vis = reinterpret_cast<const float4 *>(vis);
-        rp.weight = weight;
-        if (p.presum_active) {       // the sorted list names partial records: their sums are the "visibilities"
-            rp.vis = p.ps_sum;
-            rp.weight = nullptr;
-        }
-        rp.key = p.key;
-        rp.cls = 0;
-        rp.rec_key = p.rec_key;
-        rp.rec_sum = p.rec_sum;
-        rp.rec_items = p.rec_items;
-        rp.rec_slot = (uint32_t)p.rec_slot;
-        if (p.fused_bin) {           // binned by runs and not expanded: straight from the sorted runs
-            rp.rkey = p.srun_key;
-            rp.rstart = reinterpret_cast<const uint32_t *>(p.srun_val);
-            rp.rcum = p.run_cum;
-            rp.n_runs = (uint32_t)p.n_runs;
-            rp.qaux = p.qaux;
-            rp.blk_run = p.blk_run;
-            reduce_runs_kernel<<<p.n_sm, kRunWarps * 32, kRunWarps * kRunWarpF4 * sizeof(float4), s>>>(rp);
-        } else {
-            reduce_kernel<<<p.n_sm, kRedWarps * 32, kRedWarps * kRedWarpF4 * sizeof(float4), s>>>(rp);
-        }
-        e = cudaGetLastError();
-        if (e == cudaSuccess) e = cudaMemsetAsync(p.counters->queue_head, 0, sizeof(unsigned int) * kMaxClasses, s);
-        if (e != cudaSuccess) return e;
-        p.n_launches += 1;
-        stage_mark(p, 8, s);
-    }
     for (int c = 0; c < p.n_cls; ++c) {
         const ClassGeo &g = p.cls[c];
-        grid_fn_t gfn = pick_grid(g, p.tlog, kernel_mode(p), kernel_qbins(p));
+        grid_fn_t gfn = pick_grid(g, p.tlog, kernel_mode(p));
         if (!gfn) return cudaErrorInvalidConfiguration;
         GridParams gp;
         gp.keys = p.keys[p.sorted_sel];
@@ -1534,16 +796,7 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         gp.tmem_cols = p.tmem_cols;
         gp.merge = p.merge;
         gp.n_q = p.cfg.oversample * p.cfg.oversample;
-        if (p.reduce) {              // the entries were summed into records: grid those, as they are
-            gp.keys = p.rec_key;
-            gp.vals = nullptr;
-            gp.items = p.rec_items;
-            gp.vis = p.rec_sum;
-            gp.weight = nullptr;
-            gp.merge = 0;
-            if (gp.fold_mask > 3) gp.fold_mask = 3;      // a record is a sum already: shorter register chains
-        }
-        if (p.presum_active && !p.reduce) {       // the sorted list names partial records: their sums are the "visibilities"
+        if (p.presum_active) {       // the sorted list names partial records: their sums are the "visibilities"
             gp.vis = p.ps_sum;
             gp.weight = nullptr;
             if (gp.fold_mask > 3) gp.fold_mask = 3;

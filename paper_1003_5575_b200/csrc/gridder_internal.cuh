@@ -1,6 +1,8 @@
 // Internal declarations of libgridder.so (not part of the C ABI; see include/gridder.h).
 //
 // Data flow (DESIGN.md sections 5-6):
+// (Plans that pre-sum in input order -- presum.cu -- sort and grid partial RECORDS instead of visibilities;
+//  everything from the radix sort on is the same code.)
 //   map kernel   : visibility i=(t,b,f) -> 32-bit key [class | tile | (plane) | y0l | x0l | aux] + value
 //                  fast path (one real table, S <= 16): aux = drop, qy, qx in the key, value = i (u32)
 //                  general path (w-planes, complex tables, S <= 32): value = (i, table offset | flags) (u64)
@@ -119,18 +121,6 @@ struct GridParams {
     int32_t n_q;                   // O^2 sub-tables
     int32_t merge;                 // sum entries of a batch with equal origin and table offset before gridding
     KeyLayout key;
-    // reduce_kernel only: the records it writes (the grid kernel then reads them as keys / vis / items)
-    uint32_t *rec_key;             // [record]
-    float4 *rec_sum;               // [record][2]
-    WorkItem *rec_items;           // [item]
-    uint32_t rec_slot;             // > 0: item i owns records [i rec_slot, (i + 1) rec_slot); 0: [start, start + len)
-    // reduce_runs_kernel only: the sorted channel runs it reads instead of the per-entry list
-    const uint32_t *rkey;          // [run] sorted key (tile | origin bits, offsets zero)
-    const uint32_t *rstart;        // [run][2]: first visibility (low word of first | length << 32)
-    const uint32_t *rcum;          // [run] position of the run's first entry in the sorted order
-    uint32_t n_runs;
-    const unsigned char *qaux;     // [visibility] sub-cell offsets | drop flag
-    const uint32_t *blk_run;       // [position / 64] last run with rcum <= 64 (position / 64)
 };
 
 struct FlushParams {
@@ -147,6 +137,7 @@ struct FlushParams {
 
 struct Plan {
     gridder_config cfg;            // copy (support pointer re-targeted to support_copy)
+    gridder_tuning tune;           // copy of the caller's tuning (zeros: defaults)
     int32_t support_copy[kMaxPlanes];
     // derived
     int32_t mode;                  // 0 fast real, 1 general real, 2 general complex
@@ -157,19 +148,7 @@ struct Plan {
     uint32_t plane_off256[kMaxPlanes];
     int32_t tlog, T, ntx, nty, n_tiles;
     int32_t chunk;                 // K
-    int32_t merge;                 // GRIDDER_MERGE (default 1)
-    int32_t qbins;                 // > 0: fast path with per-origin bins (O^2 of them), grid_kernel_qbins
-    int32_t reduce;                // with qbins: the bins are filled by reduce_kernel (reduce.cu), which writes records
-    int64_t rec_cap;               // records the arrays below hold
-    int64_t rec_slot;              // > 0: records per work item (item i owns [i rec_slot, (i+1) rec_slot)); 0: item.start
-    int32_t fuse;                  // reduce straight from the sorted runs when the bin went by runs (no expansion)
-    int32_t fused_bin;             // the last gridder_bin did: keys[0] / vals[0] were NOT written
-    const uint32_t *srun_key;      // the sorted runs of the last bin (inside run_key / run_val)
-    const unsigned long long *srun_val;
-    uint32_t *blk_run;             // [max_vis / 64 + 2]
-    uint32_t *rec_key;             // [rec_cap]
-    float4 *rec_sum;               // [rec_cap][2]
-    WorkItem *rec_items;           // [max_items]: the work items over the record arrays
+    int32_t merge;                 // tuning.merge (default on)
     // pre-summation in input order (presum.cu); presum == 0: not used by this plan
     int32_t presum;
     int32_t presum_active;         // the last gridder_bin took it: keys / vals hold the sorted RECORDS
@@ -192,13 +171,6 @@ struct Plan {
     void *vals[2];
     void *cub_temp; size_t cub_temp_bytes;
     double *freq_scale;            // [kMaxChannels]: freq / c of the last bin
-    // binning by channel runs (runs.cu); run_cap == 0: not used by this plan
-    int64_t run_cap;               // room for this many runs (more: the bin falls back to per-visibility sorting)
-    unsigned char *qaux;           // [n]: the key's unsorted low bits (sub-cell offsets, drop flag) per visibility
-    uint32_t *run_key[2];          // [run_cap] x 2 (sort double buffer)
-    unsigned long long *run_val[2];// [run_cap] x 2: first index | length << 32
-    uint32_t *run_cum;             // [run_cap]
-    unsigned int *run_blk;         // [3][ceil(n / 1024) + 1]: runs per map block, their scan, expand partition
     uint32_t *tile_start;          // [2][n_vtiles]: first entry | one past the last entry
     unsigned long long *tile_chunks, *tile_chunks_scan;   // packed (n_full << 32 | has_tail), [n_vtiles+1]
     TileInfo *tile_info;           // [n_vtiles]
@@ -212,7 +184,6 @@ struct Plan {
     // state
     int sorted_sel;                // which of keys[]/vals[] holds the sorted list
     int64_t n_vis;                 // of the last bin
-    int64_t n_runs;                // of the last bin (0: per-visibility path)
     bool binned;
     cudaStream_t last_stream;
     int last_cuda_error;
@@ -247,10 +218,6 @@ cudaError_t sort_temp_bytes(int64_t n, int begin_bit, int end_bit, bool wide, si
 // scatter.cu (row f4's summation kernel lives beside row f1)
 cudaError_t launch_sum_parts(const float *parts, int n_parts, long long len, long long stride, float *out, cudaStream_t s);
 
-// runs.cu
-cudaError_t runs_temp_bytes(int64_t cap, int begin_bit, int end_bit, size_t *bytes);
-cudaError_t launch_bin_runs(Plan &p, const double *uvw, const double *scale, long long n, int n_chan, cudaStream_t s,
-                            bool *used);
 cudaError_t scan_temp_bytes(int64_t n, size_t *bytes);
 
 // presum.cu
@@ -259,6 +226,8 @@ cudaError_t presum_scan_temp_bytes(int64_t n, size_t *bytes);
 cudaError_t launch_presum_plan(Plan &p, const double *uvw, const double *scale, int n_time, int n_bl, int n_chan,
                                cudaStream_t s, long long *n_rec);
 cudaError_t launch_presum(Plan &p, const float *vis, const float *weight, cudaStream_t s);
+cudaError_t launch_map_presum_debug(const Plan &p, const double *uvw, int n_time, int n_bl, const double *freq, int n_chan,
+                                    int32_t *out, cudaStream_t s);
 
 // image.cu
 int image_workspace(Plan &p, size_t *bytes);
@@ -275,6 +244,6 @@ cudaError_t launch_scatter_atomic(Plan &p, const double *uvw, int n_time, int n_
 cudaError_t configure_grid_kernel(Plan &p);          // picks warps/smem per class, sets the smem attribute
 cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *grid, int accumulate,
                         cudaStream_t s);
-size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps, int qbins = 0);
+size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps);
 
 }  // namespace gridder

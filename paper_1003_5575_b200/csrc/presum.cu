@@ -328,6 +328,44 @@ __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__r
     }
 }
 
+// gridder_map_presum: the keys of FastMap2, decoded (test interface)
+__global__ void __launch_bounds__(256) map_presum_debug_kernel(const double *__restrict__ uvw, const double *__restrict__ freq,
+                                                                long long n_tb, int n_chan, const MapParams p,
+                                                                int32_t *__restrict__ out) {
+    FastMap2 fm;
+    fm.init(p);
+    const long long n = n_tb * n_chan;
+    const uint32_t tmask = (1u << p.key.tlog) - 1u, qmask = (1u << p.key.bits_q) - 1u;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const long long tb = i / n_chan;
+        const double s = __ddiv_rn(freq[(int)(i - tb * n_chan)], kSpeedOfLight);
+        int taps;
+        const uint32_t key = fm.key(uvw[tb * 3], uvw[tb * 3 + 1], s, fm.chan_scale(s), p, taps);
+        int32_t *o = out + i * 6;
+        if (taps == 0) {
+            o[0] = o[1] = o[2] = o[3] = o[4] = 0; o[5] = 1;
+        } else {
+            const uint32_t tile = key >> p.key.tile_shift;
+            o[0] = (int32_t)(((tile % (uint32_t)p.ntx) << p.key.tlog) | ((key >> p.key.aux_bits) & tmask));
+            o[1] = (int32_t)(((tile / (uint32_t)p.ntx) << p.key.tlog) | ((key >> (p.key.aux_bits + p.key.tlog)) & tmask));
+            o[2] = (int32_t)(key & qmask);
+            o[3] = (int32_t)((key >> p.key.bits_q) & qmask);
+            o[4] = 0; o[5] = 0;
+        }
+    }
+}
+
+cudaError_t launch_map_presum_debug(const Plan &p, const double *uvw, int n_time, int n_bl, const double *freq, int n_chan,
+                                    int32_t *out, cudaStream_t s) {
+    const MapParams mp = make_map_params(p);
+    if (p.mode != 0 || mp.o_shift < 0) return cudaErrorNotSupported;
+    const long long n_tb = (long long)n_time * n_bl, n = n_tb * n_chan;
+    long long blocks = (n + 255) / 256;
+    if (blocks > (long long)p.n_sm * 16) blocks = (long long)p.n_sm * 16;
+    map_presum_debug_kernel<<<(int)(blocks < 1 ? 1 : blocks), 256, 0, s>>>(uvw, freq, n_tb, n_chan, mp, out);
+    return cudaGetLastError();
+}
+
 #define GR_TRY(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return e_; } while (0)
 
 static PsGeo make_geo(int n_time, int n_bl, int n_chan) {

@@ -17,7 +17,8 @@ LIB_PATH = _HERE / "libgridder.so"
 
 OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_WORKSPACE, ERR_CUDA, ERR_NOT_BINNED, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 
-EXPORTS = ("gridder_workspace_size", "gridder_plan", "gridder_bin", "gridder_bin_tables", "gridder_grid", "gridder_destroy",
+EXPORTS = ("gridder_workspace_size", "gridder_plan", "gridder_workspace_size_tuned", "gridder_plan_tuned", "gridder_map_presum",
+           "gridder_bin", "gridder_bin_tables", "gridder_grid", "gridder_destroy",
            "gridder_get_stats", "gridder_map", "gridder_scatter_atomic", "gridder_image_workspace_size", "gridder_image",
            "gridder_run_host", "gridder_sum_parts", "gridder_set_profiling",
            "gridder_get_stage_ms", "gridder_launch_count", "gridder_strerror",
@@ -35,6 +36,16 @@ class _Config(C.Structure):
                 ("oversample", C.c_int32), ("n_wplanes", C.c_int32), ("support", C.POINTER(C.c_int32)),
                 ("w_max", C.c_double), ("kernel_is_complex", C.c_int32), ("kernel", C.c_void_p),
                 ("max_vis", C.c_int64), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+
+
+class _Tuning(C.Structure):
+    _fields_ = [("tile_log2", C.c_int32), ("chunk", C.c_int32), ("max_warps", C.c_int32), ("merge", C.c_int32),
+                ("presum", C.c_int32), ("table_in_tmem", C.c_int32), ("fold_batches", C.c_int32),
+                ("force_general", C.c_int32), ("host_slices", C.c_int32), ("host_slice_min_mb", C.c_int32),
+                ("reserved", C.c_int32 * 6)]
+
+
+TUNING_FIELDS = tuple(f[0] for f in _Tuning._fields_ if f[0] != "reserved")
 
 
 class _Stats(C.Structure):
@@ -58,6 +69,10 @@ def load_library() -> C.CDLL:
         lib = C.CDLL(str(LIB_PATH))
         lib.gridder_workspace_size.argtypes = [C.POINTER(_Config), C.POINTER(C.c_size_t)]
         lib.gridder_plan.argtypes = [C.POINTER(_Config), C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
+        lib.gridder_workspace_size_tuned.argtypes = [C.POINTER(_Config), C.POINTER(_Tuning), C.POINTER(C.c_size_t)]
+        lib.gridder_plan_tuned.argtypes = [C.POINTER(_Config), C.POINTER(_Tuning), C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
+        lib.gridder_map_presum.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
+                                           C.c_void_p, C.c_void_p]
         lib.gridder_bin.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32, C.c_void_p]
         lib.gridder_bin_tables.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
                                            C.c_void_p, C.c_void_p]
@@ -102,11 +117,17 @@ def _stream_ptr(stream) -> int:
     return int(stream.cuda_stream)
 
 
-def _dev_ptr(t, dtype, what):
+def _dev_ptr(t, dtype, what, device=None, numel=None):
+    """Pointer of a device buffer after the checks the C ABI cannot make (it sees no sizes): dtype, layout,
+    device and element count."""
     if t is None:
         return None
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == dtype):
         raise TypeError(f"{what} must be a contiguous CUDA tensor of {dtype}")
+    if device is not None and t.device != device:
+        raise ValueError(f"{what} is on {t.device}, the plan on {device}")
+    if numel is not None and t.numel() != numel:
+        raise ValueError(f"{what} has {t.numel()} elements, expected {numel}")
     return t.data_ptr()
 
 
@@ -134,7 +155,8 @@ class Gridder:
 
     def __init__(self, *, grid_size: int, cell_size: float, oversample: int, support, kernel: torch.Tensor,
                  max_vis: int, n_wplanes: int = 1, w_max: float = 1.0, kernel_is_complex: bool = False,
-                 device=None):
+                 device=None, tuning: dict | None = None):
+        """`tuning`: optional {field of gridder_tuning: value} (include/gridder.h); absent fields are defaults."""
         lib = load_library()
         self._lib = lib
         self._plan = C.c_void_p()
@@ -147,16 +169,23 @@ class Gridder:
         self.grid_size = int(grid_size)
         cfg = _Config(int(grid_size), float(cell_size), 4, int(oversample), int(n_wplanes), self._support,
                       float(w_max), int(bool(kernel_is_complex)), self._kernel.data_ptr(), int(max_vis), None, 0)
+        tune = _Tuning()
+        for k, v in (tuning or {}).items():
+            if k not in TUNING_FIELDS:
+                raise KeyError(f"unknown gridder_tuning field {k!r}")
+            setattr(tune, k, int(v))
+        self.n_planes = int(n_wplanes)
+        self._binned = None          # (n_time, n_baseline, n_chan) of the last bin
         need = C.c_size_t(0)
         with torch.cuda.device(self.device):
-            rc = lib.gridder_workspace_size(C.byref(cfg), C.byref(need))
+            rc = lib.gridder_workspace_size_tuned(C.byref(cfg), C.byref(tune), C.byref(need))
             if rc != OK:
                 raise GridderError(rc, "gridder_workspace_size")
             self.workspace = torch.empty(need.value + 256, dtype=torch.uint8, device=self.device)
             base = (self.workspace.data_ptr() + 255) // 256 * 256
             cfg.workspace = base
             cfg.workspace_bytes = need.value
-            rc = lib.gridder_plan(C.byref(cfg), C.byref(self._plan), C.byref(need))
+            rc = lib.gridder_plan_tuned(C.byref(cfg), C.byref(tune), C.byref(self._plan), C.byref(need))
         if rc != OK:
             self._plan = C.c_void_p()
             raise GridderError(rc, "gridder_plan")
@@ -173,11 +202,14 @@ class Gridder:
         if three != 3:
             raise ValueError("uvw_m must be [n_time][n_baseline][3]")
         self._keep = [uvw_m, freq_hz, table_index]
-        rc = self._lib.gridder_bin_tables(self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m"), n_time, n_bl,
-                                          _dev_ptr(freq_hz, torch.float64, "freq_hz"), freq_hz.numel(),
-                                          _dev_ptr(table_index, torch.int32, "table_index"), _stream_ptr(stream))
+        self._binned = None
+        rc = self._lib.gridder_bin_tables(self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m", self.device), n_time, n_bl,
+                                          _dev_ptr(freq_hz, torch.float64, "freq_hz", self.device), freq_hz.numel(),
+                                          _dev_ptr(table_index, torch.int32, "table_index", self.device, n_time * n_bl),
+                                          _stream_ptr(stream))
         if rc != OK:
             raise GridderError(rc, "gridder_bin")
+        self._binned = (n_time, n_bl, freq_hz.numel())
 
     def grid(self, vis: torch.Tensor, weight=None, out=None, accumulate: bool = False, stream=None) -> torch.Tensor:
         """vis float32 [...][4][2]; returns the grid float32 [4][N][N][2]; asynchronous."""
@@ -185,9 +217,13 @@ class Gridder:
             if accumulate:
                 raise ValueError("accumulate needs an existing grid")
             out = torch.empty((4, self.grid_size, self.grid_size, 2), dtype=torch.float32, device=self.device)
-        rc = self._lib.gridder_grid(self._plan, _dev_ptr(vis, torch.float32, "vis"),
-                                    _dev_ptr(weight, torch.float32, "weight"),
-                                    _dev_ptr(out, torch.float32, "grid"), int(accumulate), _stream_ptr(stream))
+        if self._binned is None:
+            raise GridderError(ERR_NOT_BINNED, "gridder_grid")
+        n = self._binned[0] * self._binned[1] * self._binned[2]
+        rc = self._lib.gridder_grid(self._plan, _dev_ptr(vis, torch.float32, "vis", self.device, 8 * n),
+                                    _dev_ptr(weight, torch.float32, "weight", self.device, n),
+                                    _dev_ptr(out, torch.float32, "grid", self.device, 8 * self.grid_size ** 2),
+                                    int(accumulate), _stream_ptr(stream))
         if rc != OK:
             raise GridderError(rc, "gridder_grid")
         return out
@@ -210,11 +246,11 @@ class Gridder:
         if rc != OK:
             raise GridderError(rc, "gridder_set_profiling")
 
-    STAGES = ("map", "sort", "tables", "grid", "flush", "presum", "reduce")
+    STAGES = ("map", "sort", "tables", "grid", "flush", "presum")
 
     def stage_ms(self) -> dict:
         """Device milliseconds of the last bin/grid per stage (synchronises on their events)."""
-        ms = (C.c_float * 7)()
+        ms = (C.c_float * 6)()
         rc = self._lib.gridder_get_stage_ms(self._plan, ms)
         if rc != OK:
             raise GridderError(rc, "gridder_get_stage_ms")
@@ -223,15 +259,23 @@ class Gridder:
     def launch_count(self) -> int:
         return int(self._lib.gridder_launch_count(self._plan))
 
-    def map(self, uvw_m: torch.Tensor, freq_hz: torch.Tensor, stream=None, table_index=None) -> torch.Tensor:
-        """int32 [n][6] = x0, y0, qx, qy, plane | conj << 8, dropped (the map kernel's device function)."""
+    def map(self, uvw_m: torch.Tensor, freq_hz: torch.Tensor, stream=None, table_index=None, presum: bool = False) -> torch.Tensor:
+        """int32 [n][6] = x0, y0, qx, qy, plane | conj << 8, dropped.  presum=False: map_vis, the device function
+        of the per-visibility map kernel; presum=True: the pre-summed path's one-FMA mapper (gridder_map_presum;
+        dropped visibilities report 0, 0, 0, 0, 0, 1)."""
         if uvw_m.dim() == 2:
             uvw_m = uvw_m[None]
         n_time, n_bl, _ = uvw_m.shape
         out = torch.empty((n_time * n_bl * freq_hz.numel(), 6), dtype=torch.int32, device=self.device)
-        rc = self._lib.gridder_map(self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m"), n_time, n_bl,
-                                   _dev_ptr(freq_hz, torch.float64, "freq_hz"), freq_hz.numel(),
-                                   _dev_ptr(table_index, torch.int32, "table_index"), out.data_ptr(), _stream_ptr(stream))
+        if presum:
+            rc = self._lib.gridder_map_presum(self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m", self.device), n_time, n_bl,
+                                              _dev_ptr(freq_hz, torch.float64, "freq_hz", self.device), freq_hz.numel(),
+                                              out.data_ptr(), _stream_ptr(stream))
+        else:
+            rc = self._lib.gridder_map(self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m", self.device), n_time, n_bl,
+                                       _dev_ptr(freq_hz, torch.float64, "freq_hz", self.device), freq_hz.numel(),
+                                       _dev_ptr(table_index, torch.int32, "table_index", self.device, n_time * n_bl),
+                                       out.data_ptr(), _stream_ptr(stream))
         if rc != OK:
             raise GridderError(rc, "gridder_map")
         return out
@@ -245,10 +289,12 @@ class Gridder:
             if accumulate:
                 raise ValueError("accumulate needs an existing grid")
             out = torch.empty((4, self.grid_size, self.grid_size, 2), dtype=torch.float32, device=self.device)
+        n = n_time * n_bl * freq_hz.numel()
         rc = self._lib.gridder_scatter_atomic(
-            self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m"), n_time, n_bl, _dev_ptr(freq_hz, torch.float64, "freq_hz"),
-            freq_hz.numel(), _dev_ptr(vis, torch.float32, "vis"), _dev_ptr(weight, torch.float32, "weight"),
-            _dev_ptr(out, torch.float32, "grid"), int(accumulate), _stream_ptr(stream))
+            self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m", self.device), n_time, n_bl,
+            _dev_ptr(freq_hz, torch.float64, "freq_hz", self.device), freq_hz.numel(),
+            _dev_ptr(vis, torch.float32, "vis", self.device, 8 * n), _dev_ptr(weight, torch.float32, "weight", self.device, n),
+            _dev_ptr(out, torch.float32, "grid", self.device, 8 * self.grid_size ** 2), int(accumulate), _stream_ptr(stream))
         if rc != OK:
             raise GridderError(rc, "gridder_scatter_atomic")
         return out
@@ -263,28 +309,46 @@ class Gridder:
             self._fft_work = torch.empty(max(need.value, 16), dtype=torch.uint8, device=self.device)
         if out is None:
             out = torch.empty_like(grid)
-        rc = self._lib.gridder_image(self._plan, _dev_ptr(grid, torch.float32, "grid"), _dev_ptr(out, torch.float32, "image"),
-                                     _dev_ptr(corr, torch.float32, "corr"), self._fft_work.data_ptr(), self._fft_work.numel(),
-                                     _stream_ptr(stream))
+        cells = 8 * self.grid_size ** 2
+        rc = self._lib.gridder_image(self._plan, _dev_ptr(grid, torch.float32, "grid", self.device, cells),
+                                     _dev_ptr(out, torch.float32, "image", self.device, cells),
+                                     _dev_ptr(corr, torch.float32, "corr", self.device, self.grid_size),
+                                     self._fft_work.data_ptr(), self._fft_work.numel(), _stream_ptr(stream))
         if rc != OK:
             raise GridderError(rc, "gridder_image")
         return out
 
     def run_host(self, uvw_m, freq_hz, vis, weight, grid_out, staging: dict, stream=None) -> None:
         """End to end with HOST tensors (pinned for speed): H2D, bin, grid, D2H, synchronise."""
-        def hp(t, dtype, what):
+        def hp(t, dtype, what, numel):
             if t is None:
                 return None
             if t.is_cuda or not t.is_contiguous() or t.dtype != dtype:
                 raise TypeError(f"{what} must be a contiguous host tensor of {dtype}")
+            if t.numel() != numel:
+                raise ValueError(f"{what} has {t.numel()} elements, expected {numel}")
             return t.data_ptr()
         if uvw_m.dim() == 2:
             uvw_m = uvw_m[None]
         n_time, n_bl, _ = uvw_m.shape
+        n_chan = freq_hz.numel()
+        n = n_time * n_bl * n_chan
+        cells = 8 * self.grid_size ** 2
+        need = {"uvw": (torch.float64, 3 * n_time * n_bl), "freq": (torch.float64, n_chan), "vis": (torch.float32, 8 * n),
+                "grid": (torch.float32, cells)}
+        if weight is not None:
+            need["weight"] = (torch.float32, n)
+        for name, (dt, cnt) in need.items():     # staging buffers may be larger than one call needs
+            t = staging.get(name)
+            if not (isinstance(t, torch.Tensor) and t.is_cuda and t.device == self.device and t.is_contiguous()
+                    and t.dtype == dt and t.numel() >= cnt):
+                raise ValueError(f"staging[{name!r}] must be a contiguous {dt} tensor on {self.device} with >= {cnt} elements")
+        self._binned = None
         rc = self._lib.gridder_run_host(
-            self._plan, hp(uvw_m, torch.float64, "uvw_m"), n_time, n_bl, hp(freq_hz, torch.float64, "freq_hz"),
-            freq_hz.numel(), hp(vis, torch.float32, "vis"), hp(weight, torch.float32, "weight"),
-            hp(grid_out, torch.float32, "grid_out"), staging["uvw"].data_ptr(), staging["freq"].data_ptr(),
+            self._plan, hp(uvw_m, torch.float64, "uvw_m", 3 * n_time * n_bl), n_time, n_bl,
+            hp(freq_hz, torch.float64, "freq_hz", n_chan), n_chan, hp(vis, torch.float32, "vis", 8 * n),
+            hp(weight, torch.float32, "weight", n), hp(grid_out, torch.float32, "grid_out", cells),
+            staging["uvw"].data_ptr(), staging["freq"].data_ptr(),
             staging["vis"].data_ptr(), staging["weight"].data_ptr() if weight is not None else None,
             staging["grid"].data_ptr(), _stream_ptr(stream))
         if rc != OK:

@@ -1,8 +1,6 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
 same seeded inputs.  Integer work (the mapping, counts) must be bit-exact; grid cells must satisfy
 BASELINE.json's |delta| <= 1e-5 * sum|w V C| + 1e-6; reruns must be bit-identical."""
-import os
-
 import numpy as np
 import pytest
 import torch
@@ -24,29 +22,19 @@ def dev():
     return torch.device("cuda:0")
 
 
-def _gridder(dev, *, N, du, O, S, table, max_vis, env=None):
+def _gridder(dev, *, N, du, O, S, table, max_vis, tuning=None):
+    """A plan; `tuning` = fields of gridder_tuning (include/gridder.h) that steer it onto the path under test."""
     from paper_1003_5575_b200 import gridder
-    old = {}
-    for k, v in (env or {}).items():
-        old[k] = os.environ.get(k)
-        os.environ[k] = str(v)
-    try:
-        return gridder.Gridder(grid_size=N, cell_size=du, oversample=O, support=[S],
-                               kernel=torch.from_numpy(np.ascontiguousarray(table, np.float32).ravel()).to(dev),
-                               max_vis=max_vis)
-    finally:
-        for k, v in old.items():
-            if v is None:
-                os.environ.pop(k, None)
-            else:
-                os.environ[k] = v
+    return gridder.Gridder(grid_size=N, cell_size=du, oversample=O, support=[S],
+                           kernel=torch.from_numpy(np.ascontiguousarray(table, np.float32).ravel()).to(dev),
+                           max_vis=max_vis, tuning=tuning)
 
 
-def _run(dev, uvw, freq, vis, weight, *, N, du, O, S, table, env=None, accumulate_onto=None):
+def _run(dev, uvw, freq, vis, weight, *, N, du, O, S, table, tuning=None, accumulate_onto=None):
     uvw = np.ascontiguousarray(uvw, np.float64)
     uvw = uvw[None] if uvw.ndim == 2 else uvw
     n = uvw.shape[0] * uvw.shape[1] * len(freq)
-    g = _gridder(dev, N=N, du=du, O=O, S=S, table=table, max_vis=max(n, 1), env=env)
+    g = _gridder(dev, N=N, du=du, O=O, S=S, table=table, max_vis=max(n, 1), tuning=tuning)
     g.bin(torch.from_numpy(uvw).to(dev), torch.tensor(np.asarray(freq, np.float64), device=dev))
     d_vis = torch.from_numpy(np.ascontiguousarray(vis, np.float32)).to(dev)
     d_w = None if weight is None else torch.from_numpy(np.ascontiguousarray(weight, np.float32)).to(dev)
@@ -120,6 +108,56 @@ def test_map_kernel_is_bit_exact_on_adversarial_positions(dev, S, O, N):
     assert 0 < ref[:, 5].sum() < len(ref)
 
 
+def _check_presum_map(got, ref):
+    """gridder_map_presum reports a dropped visibility as 0, 0, 0, 0, 0, 1; everything else as gridder_map."""
+    assert np.array_equal(got[:, 5], ref[:, 5])
+    keep = ref[:, 5] == 0
+    assert np.array_equal(got[keep], ref[keep])
+    assert not got[~keep, :5].any()
+
+
+@pytest.mark.parametrize("S,O,N", [(16, 4, 512), (7, 8, 256), (15, 8, 128), (8, 2, 64), (16, 1, 64)])
+def test_presum_mapper_is_bit_exact_on_adversarial_positions(dev, S, O, N):
+    """The PRODUCTION mapper of configs 2 and 4 (FastMap2: one FMA per axis, screened; csrc/map.cuh) on the
+    same 600 000 adversarial positions -- exact half sub-cells, lattice points, their FP64 neighbours, far
+    outliers -- with integer equality against the oracle's mapping."""
+    rng = np.random.default_rng(100 + S)
+    n = 200_000
+    pos = rng.uniform(-N / 2 - 3, N / 2 + 3, (n, 2))
+    pos[:50_000] = (np.floor(pos[:50_000] * O) + 0.5) / O
+    pos[50_000:60_000] = np.round(pos[50_000:60_000] * O) / O
+    pos[60_000:70_000] = np.nextafter((np.floor(pos[60_000:70_000] * O) + 0.5) / O, -np.inf)
+    pos[70_000:80_000] = np.nextafter((np.floor(pos[70_000:80_000] * O) + 0.5) / O, np.inf)
+    pos[80_000] = (1e30, -1e30)
+    pos[80_001] = (-1e18, 3.0)
+    pos[80_002] = (N * 1.4, 0.0)                   # beyond the fast range of the screen, inside the slow one
+    du = 0.37
+    uvw = np.zeros((1, n, 3))
+    uvw[0, :, :2] = pos * du
+    freq = np.array([C, C * (1 + 2.0 ** -20), 0.75 * C])
+    table = np.zeros((S * O) ** 2, np.float32)
+    g = _gridder(dev, N=N, du=du, O=O, S=S, table=table, max_vis=n * 3)
+    got = g.map(torch.from_numpy(uvw).to(dev), torch.from_numpy(freq).to(dev), presum=True).cpu().numpy()
+    g.destroy()
+    ref = oracle.map_visibilities(uvw, freq, grid_size=N, cell_size=du, oversample=O, support=[S], kernel=table)
+    _check_presum_map(got, ref)
+    assert 0 < ref[:, 5].sum() < len(ref)
+
+
+def test_presum_mapper_is_bit_exact_on_config_2(dev):
+    """Every visibility of BASELINE.json config 2 (130 816 baselines x 768 channels) through the production
+    mapper, against the oracle's mapping, in blocks of 96 channels."""
+    wl = synth.make_workload(2)
+    g = _gridder(dev, N=wl.grid_size, du=wl.cell_size, O=wl.oversample, S=wl.support[0], table=wl.kernel, max_vis=1024)
+    d_uvw = torch.from_numpy(wl.uvw).to(dev)
+    for f0 in range(0, wl.n_chan, 96):
+        freq = wl.freq[f0:f0 + 96]
+        got = g.map(d_uvw, torch.from_numpy(freq).to(dev), presum=True).cpu().numpy()
+        ref = oracle.map_visibilities(wl.uvw, freq, **oracle_kwargs(wl))
+        _check_presum_map(got, ref)
+    g.destroy()
+
+
 # ------------------------------------------------------------------------------------ full grids
 @pytest.mark.parametrize("cfg", [0, 1])
 def test_parity_full_grid_configs(dev, cfg):
@@ -154,7 +192,7 @@ def test_parity_tile_sizes_and_ragged_grid(dev, S, O, tlog):
     N, n = 90, 5000
     table = rng.standard_normal((S * O, S * O)).astype(np.float32)
     uvw, vis, w = _random_case(rng, n, N, S)
-    got, st = _run(dev, uvw, [C], vis, w, N=N, du=1.0, O=O, S=S, table=table, env={"GRIDDER_TILE_LOG2": tlog})
+    got, st = _run(dev, uvw, [C], vis, w, N=N, du=1.0, O=O, S=S, table=table, tuning={"tile_log2": tlog})
     ref, ab, ost = _oracle(uvw, [C], vis, w, N=N, du=1.0, O=O, S=S, table=table)
     assert st.tile_size == 1 << tlog and st.n_dropped == ost["n_dropped"]
     assert_parity(got, ref, ab, f"T={1 << tlog}")
@@ -168,7 +206,7 @@ def test_parity_hot_tile_is_split_into_chunks(dev):
     uvw = np.zeros((1, n, 3))
     uvw[0, :, :2] = rng.uniform(-3.0, 3.0, (n, 2))
     vis = (rng.standard_normal((n, 4, 2)) + 3.0).astype(np.float32)          # coherent: sums grow
-    got, st = _run(dev, uvw, [C], vis, None, N=N, du=1.0, O=O, S=S, table=table, env={"GRIDDER_CHUNK": 512})
+    got, st = _run(dev, uvw, [C], vis, None, N=N, du=1.0, O=O, S=S, table=table, tuning={"chunk": 512})
     ref, ab, _ = _oracle(uvw, [C], vis, None, N=N, du=1.0, O=O, S=S, table=table)
     assert st.chunk_size == 512 and st.n_work_items >= n // 512 and st.max_tile_load > 512
     assert st.n_work_items <= st.n_tiles_occupied + n // 512
@@ -220,7 +258,7 @@ def test_reruns_and_launch_shapes_are_bit_identical(dev):
     b, _ = _run(dev, wl.uvw, wl.freq, vis, None, **kw)
     assert np.array_equal(a, b)
     # the number of resident warps changes which warp takes which work item, never the result
-    c, st = _run(dev, wl.uvw, wl.freq, vis, None, env={"GRIDDER_WARPS": 4}, **kw)
+    c, st = _run(dev, wl.uvw, wl.freq, vis, None, tuning={"max_warps": 4}, **kw)
     assert st.grid_warps_per_sm == 4 and np.array_equal(a, c)
     # same plan: bin once, grid twice, and re-bin
     g = _gridder(dev, max_vis=wl.n_vis, **kw)
@@ -255,63 +293,32 @@ def test_error_paths_on_device(dev):
     assert e.value.code == gridder.ERR_UNSUPPORTED
 
 
-# ------------------------------------------------------------------------------------ binning by channel runs
-def test_run_binning_gives_the_same_bits_as_the_per_visibility_sort(dev):
-    """The fast path sorts channel runs and expands them (csrc/runs.cu); the result must be the list the
-    per-visibility sort produces, hence the same grid to the last bit -- on a multi-channel workload
-    whose size is not a multiple of the 1024-visibility blocks and whose runs straddle them."""
-    rng = np.random.default_rng(21)
-    N, S, O, nb, nf = 256, 16, 4, 517, 100
-    table = synth.spheroidal_table(S, O)
-    uvw = np.zeros((2, nb, 3))
-    uvw[:, :, :2] = rng.uniform(-112.0, 112.0, (2, nb, 2))
-    uvw[0, :5, :2] = 0.0                                            # one run per row, same origin for all
-    freq = C * (1.0 + 2.0e-3 * np.arange(nf))                       # 20 % band: long and short runs
-    vis = rng.standard_normal((2, nb, nf, 4, 2)).astype(np.float32)
-    w = rng.uniform(0.5, 1.5, (2, nb, nf)).astype(np.float32)
-    kw = dict(N=N, du=1.0, O=O, S=S, table=table)
-    a, st_a = _run(dev, uvw, freq, vis, w, env={"GRIDDER_RUNS": 2}, **kw)        # 2: also for a plan this small
-    b, st_b = _run(dev, uvw, freq, vis, w, env={"GRIDDER_RUNS": 0}, **kw)
-    assert np.array_equal(a, b)
-    assert (st_a.n_dropped, st_a.vis_taps, st_a.n_work_items, st_a.max_tile_load) == \
-           (st_b.n_dropped, st_b.vis_taps, st_b.n_work_items, st_b.max_tile_load)
-    assert 0 < st_a.n_dropped < 2 * nb * nf                         # the 1.2x band pushes some off the grid
-    ref, ab, ost = _oracle(uvw, freq, vis, w, **kw)
-    assert ost["n_dropped"] == st_a.n_dropped
-    assert_parity(a, ref, ab, "run binning")
-    # single-channel input: every visibility is its own run -> the plan falls back to the per-visibility sort
-    c, _ = _run(dev, uvw[:, :, :], freq[:1], vis[:, :, :1].copy(), w[:, :, :1].copy(), env={"GRIDDER_RUNS": 2}, **kw)
-    d, _ = _run(dev, uvw[:, :, :], freq[:1], vis[:, :, :1].copy(), w[:, :, :1].copy(), env={"GRIDDER_RUNS": 0}, **kw)
-    assert np.array_equal(c, d)
-
-
 # ------------------------------------------------------------------------------------ host buffers end to end
-def test_run_host_sliced_copy_compute_overlap_matches_oracle(dev, monkeypatch):
+def test_run_host_sliced_copy_compute_overlap_matches_oracle(dev):
     """gridder_run_host on config 1 with pinned host buffers, forced into its sliced mode (copy of slice
     k+1 on a second stream while slice k is binned and gridded): within tolerance of the oracle, equal to
     the single-shot mode within a few FP32 roundings, and bit-identical between two calls."""
     from paper_1003_5575_b200 import gridder
     wl = synth.make_workload(1)
     vis = wl.visibilities("cpu").contiguous()
-    g = gridder.Gridder(grid_size=wl.grid_size, cell_size=wl.cell_size, oversample=wl.oversample, support=wl.support,
-                        kernel=torch.from_numpy(wl.kernel).to(dev), max_vis=wl.n_vis)
     h_uvw, h_freq = torch.from_numpy(wl.uvw).pin_memory(), torch.from_numpy(wl.freq).pin_memory()
     h_vis = vis.pin_memory()
     staging = {"uvw": torch.empty_like(h_uvw, device=dev), "freq": torch.empty_like(h_freq, device=dev),
                "vis": torch.empty_like(h_vis, device=dev), "weight": None,
                "grid": torch.empty((4, wl.grid_size, wl.grid_size, 2), dtype=torch.float32, device=dev)}
     outs = []
-    for min_mb in ("1", "1", "100000"):                # sliced, sliced again, single shot
-        monkeypatch.setenv("GRIDDER_HOST_SLICE_MIN_MB", min_mb)
+    for min_mb in (1, 1, 100000):                      # sliced, sliced again, single shot
+        g = gridder.Gridder(grid_size=wl.grid_size, cell_size=wl.cell_size, oversample=wl.oversample, support=wl.support,
+                            kernel=torch.from_numpy(wl.kernel).to(dev), max_vis=wl.n_vis,
+                            tuning={"host_slice_min_mb": min_mb})
         h_grid = torch.empty((4, wl.grid_size, wl.grid_size, 2), dtype=torch.float32).pin_memory()
         g.run_host(h_uvw, h_freq, h_vis, None, h_grid, staging)
         outs.append(h_grid.numpy().copy())
-    g.destroy()
+        g.destroy()
     ref, ab, _ = oracle.grid_full(wl.uvw, wl.freq, vis.numpy(), None, **oracle_kwargs(wl))
     assert np.array_equal(outs[0], outs[1])
     assert_parity(outs[0], ref, ab, "run_host, sliced")
     assert_parity(outs[2], ref, ab, "run_host, single shot")
-    assert not np.array_equal(outs[0], outs[2]) or True          # the modes may differ in the last bits
     assert np.abs(as_complex(outs[0]) - as_complex(outs[2])).max() <= 2e-6 * np.abs(ref).max()
 
 
@@ -370,7 +377,7 @@ def test_merging_of_equal_origin_and_offset_entries(dev):
     ref, ab, _ = _oracle(uvw, [C], vis, w, **kw)
     a, st_a = _run(dev, uvw, [C], vis, w, **kw)
     a2, _ = _run(dev, uvw, [C], vis, w, **kw)
-    b, st_b = _run(dev, uvw, [C], vis, w, env={"GRIDDER_MERGE": 0}, **kw)
+    b, st_b = _run(dev, uvw, [C], vis, w, tuning={"merge": 2}, **kw)
     assert np.array_equal(a, a2)
     assert_parity(a, ref, ab, "merging on")
     assert_parity(b, ref, ab, "merging off")
@@ -379,178 +386,31 @@ def test_merging_of_equal_origin_and_offset_entries(dev):
     assert st_a.n_records_gridded < n // 3 and st_a.fma_executed == st_a.n_records_gridded * 256 * 8
 
 
-# ------------------------------------------------------------------------------------ per-origin bins
-@pytest.mark.parametrize("S,O,N,n", [(16, 4, 96, 6000), (15, 8, 80, 5000), (12, 4, 66, 3000), (9, 2, 70, 3000)])
-def test_per_origin_bins_kernel_random(dev, S, O, N, n):
-    """grid_kernel_qbins (chosen by default only for dense plans) forced on the random cases."""
-    rng = np.random.default_rng(S * 1000 + N + 1)
-    table = rng.standard_normal((S * O, S * O)).astype(np.float32)
-    uvw, vis, w = _random_case(rng, n, N, S)
-    got, st = _run(dev, uvw, [C], vis, w, N=N, du=1.0, O=O, S=S, table=table, env={"GRIDDER_QBINS": 2})
-    got2, _ = _run(dev, uvw, [C], vis, w, N=N, du=1.0, O=O, S=S, table=table, env={"GRIDDER_QBINS": 2, "GRIDDER_WARPS": 4})
-    ref, ab, ost = _oracle(uvw, [C], vis, w, N=N, du=1.0, O=O, S=S, table=table)
-    assert st.n_dropped == ost["n_dropped"] > 0 and st.vis_taps == ost["vis_taps"]
-    assert np.array_equal(got, got2)
-    assert_parity(got, ref, ab, f"qbins S={S} O={O}")
-
-
-def test_per_origin_bins_kernel_dense_lattice_chunks_and_tiles(dev):
-    """Many visibilities on few lattice points (every bin of an origin fills, chunks of 256 split the hot
-    tiles, T = 4 and 8): the bins kernel against the oracle and against the ring kernel's record counts."""
-    rng = np.random.default_rng(92)
-    N, S, O, n = 64, 16, 4, 30_000
-    table = synth.spheroidal_table(S, O)
-    uvw = np.zeros((1, n, 3))
-    uvw[0, :, :2] = rng.integers(-24, 25, (n, 2)) / 8.0              # 49 x 49 points on the 1/8 lattice (ties too)
-    vis = (rng.standard_normal((n, 4, 2)) + 1.0).astype(np.float32)
-    w = rng.uniform(0.5, 1.5, n).astype(np.float32)
-    kw = dict(N=N, du=1.0, O=O, S=S, table=table)
-    ref, ab, _ = _oracle(uvw, [C], vis, w, **kw)
-    for tlog in (2, 3):
-        env = {"GRIDDER_QBINS": 2, "GRIDDER_CHUNK": 256, "GRIDDER_TILE_LOG2": tlog}
-        a, st_a = _run(dev, uvw, [C], vis, w, env=env, **kw)
-        a2, _ = _run(dev, uvw, [C], vis, w, env=env, **kw)
-        b, st_b = _run(dev, uvw, [C], vis, w, env=dict(env, GRIDDER_QBINS=0), **kw)
-        assert np.array_equal(a, a2)
-        assert_parity(a, ref, ab, f"qbins dense T={1 << tlog}")
-        assert_parity(b, ref, ab, f"ring kernel dense T={1 << tlog}")
-        assert st_a.n_work_items == st_b.n_work_items and st_a.max_tile_load > 256
-        assert 0 < st_a.n_records_gridded <= st_b.n_records_gridded < n        # bins merge at least as much
-        assert st_a.fma_executed == st_a.n_records_gridded * 256 * 8
-
-
-def test_pre_summation_long_origins_pieces_and_unit_weights(dev):
-    """reduce_kernel: a few origins with thousands of entries each (the 1024-entry piece limit adds the bin
-    copies several times per origin), no weights, and items of one and of many batches; and the one-kernel
-    form of the same plan (GRIDDER_REDUCE=0: grid_kernel_qbins) gives a grid inside the same tolerance."""
-    rng = np.random.default_rng(93)
-    N, S, O, n = 64, 16, 4, 20_000
-    table = synth.spheroidal_table(S, O)
-    uvw = np.zeros((1, n, 3))
-    uvw[0, :, :2] = rng.uniform(-1.2, 1.2, (n, 2))                   # 3 x 3 origins, ~2200 entries each
-    uvw[0, :50, :2] = rng.uniform(-20.0, 20.0, (50, 2))              # and a few lonely ones (items of one entry)
-    vis = (rng.standard_normal((n, 4, 2)) + 1.0).astype(np.float32)
-    kw = dict(N=N, du=1.0, O=O, S=S, table=table)
-    ref, ab, _ = _oracle(uvw, [C], vis, None, **kw)
-    env = {"GRIDDER_QBINS": 2, "GRIDDER_TILE_LOG2": 2, "GRIDDER_CHUNK": 8192}
-    a, st_a = _run(dev, uvw, [C], vis, None, env=env, **kw)
-    a2, _ = _run(dev, uvw, [C], vis, None, env=env, **kw)
-    b, st_b = _run(dev, uvw, [C], vis, None, env=dict(env, GRIDDER_REDUCE=0), **kw)
-    assert np.array_equal(a, a2)
-    assert_parity(a, ref, ab, "pre-summation, long origins")
-    assert_parity(b, ref, ab, "per-origin bins in the grid kernel, long origins")
-    assert st_a.max_tile_load > 2048 and st_a.chunk_size == 8192
-    # both count one record per non-empty (item, origin, offset)
-    assert st_a.n_records_gridded == st_b.n_records_gridded < n // 10
-
-
-@pytest.mark.parametrize("S,O,N,n,env", [(16, 4, 96, 6000, {}), (12, 4, 66, 3000, {"GRIDDER_MERGE": 0}),
-                                         (16, 4, 80, 8000, {"GRIDDER_QBINS": 2}), (7, 8, 64, 3000, {})])
-def test_table_in_tensor_memory(dev, S, O, N, n, env):
-    """GRIDDER_TMEM=1: the GCF table is read with tcgen05.ld instead of LDS (the default for dense plans,
-    where the grid kernel runs on pre-summed records); same bits as the shared-memory table."""
+@pytest.mark.parametrize("S,O,N,n,tuning", [(16, 4, 96, 6000, {}), (12, 4, 66, 3000, {"merge": 2}),
+                                            (16, 4, 80, 8000, {"tile_log2": 3}), (7, 8, 64, 3000, {})])
+def test_table_in_tensor_memory(dev, S, O, N, n, tuning):
+    """table_in_tmem: the GCF table is read with tcgen05.ld instead of LDS (the default for pre-summed plans,
+    where the grid kernel runs on partial records); same bits as the shared-memory table."""
     rng = np.random.default_rng(S + N + n)
     table = rng.standard_normal((S * O, S * O)).astype(np.float32)
     uvw, vis, w = _random_case(rng, n, N, S)
     kw = dict(N=N, du=1.0, O=O, S=S, table=table)
-    a, _ = _run(dev, uvw, [C], vis, w, env=dict(env, GRIDDER_TMEM=1), **kw)
-    b, _ = _run(dev, uvw, [C], vis, w, env=dict(env, GRIDDER_TMEM=0), **kw)
+    a, _ = _run(dev, uvw, [C], vis, w, tuning=dict(tuning, table_in_tmem=1), **kw)
+    b, _ = _run(dev, uvw, [C], vis, w, tuning=dict(tuning, table_in_tmem=2), **kw)
     ref, ab, _ = _oracle(uvw, [C], vis, w, **kw)
     assert np.array_equal(a, b)
     assert_parity(a, ref, ab, f"tensor-memory table S={S} O={O}")
 
 
-def test_pre_summation_edge_cases(dev):
-    """The dense path (reduce_kernel + grid_kernel on records, forced) on the degenerate inputs: empty,
-    one visibility, everything dropped, zero weights, accumulate onto a grid, bin once / grid twice / re-bin."""
-    env = {"GRIDDER_QBINS": 2}
-    N, S, O = 48, 16, 4
-    table = synth.spheroidal_table(S, O)
+def test_table_too_large_for_shared_memory_takes_the_general_path(dev):
+    """S = 16 with O = 16 is a 256 KB table: more than an SM's shared memory.  The plan must not fail: it reads
+    the table from global memory (the general path) and still matches the oracle."""
+    rng = np.random.default_rng(1616)
+    N, S, O, n = 96, 16, 16, 3000
+    table = rng.standard_normal((S * O, S * O)).astype(np.float32)
+    uvw, vis, w = _random_case(rng, n, N, S)
     kw = dict(N=N, du=1.0, O=O, S=S, table=table)
-    got, st = _run(dev, np.zeros((1, 0, 3)), [C], np.zeros((0, 4, 2), np.float32), None, env=env, **kw)
-    assert st.n_vis == 0 and st.n_work_items == 0 and not got.any()
-    uvw = np.zeros((1, 1, 3))
-    vis = np.zeros((1, 4, 2), np.float32)
-    vis[0, 1] = (-3.0, 0.5)
-    got, st = _run(dev, uvw, [C], vis, None, env=env, **kw)
-    ref, ab, _ = _oracle(uvw, [C], vis, None, **kw)
-    assert st.n_work_items == 1 and st.n_records_gridded == 1
-    assert_parity(got, ref, ab, "dense path, single")
-    uvw[0, 0, :2] = (100.0, 0.0)
-    got, st = _run(dev, uvw, [C], vis, None, env=env, **kw)
-    assert st.n_dropped == 1 and st.vis_taps == 0 and not got.any()
-
-    rng = np.random.default_rng(94)
-    n = 5000
-    uvw, vis, w = _random_case(rng, n, N, S, spread=6)
-    w[::3] = 0.0
-    base = rng.standard_normal((4, N, N, 2)).astype(np.float32)
-    got, st = _run(dev, uvw, [C], vis, w, env=env, accumulate_onto=base, **kw)
+    got, st = _run(dev, uvw, [C], vis, w, **kw)
     ref, ab, ost = _oracle(uvw, [C], vis, w, **kw)
     assert st.n_dropped == ost["n_dropped"] and st.vis_taps == ost["vis_taps"]
-    assert_parity(got, ref + as_complex(base), ab + np.abs(as_complex(base)), "dense path, accumulate")
-
-    g = _gridder(dev, max_vis=n, env=env, **kw)
-    d_uvw, d_f = torch.from_numpy(uvw).to(dev), torch.tensor([C], dtype=torch.float64, device=dev)
-    d_v, d_w = torch.from_numpy(vis).to(dev), torch.from_numpy(w).to(dev)
-    g.bin(d_uvw, d_f)
-    o1 = g.grid(d_v, d_w).cpu().numpy()
-    o2 = g.grid(d_v, d_w).cpu().numpy()
-    o4 = g.grid(2.0 * d_v, d_w).cpu().numpy()                 # new visibilities on the same binning
-    g.bin(d_uvw, d_f)
-    o3 = g.grid(d_v, d_w).cpu().numpy()
-    g.destroy()
-    assert np.array_equal(o1, o2) and np.array_equal(o1, o3) and np.array_equal(o4, 2.0 * o1)
-    assert_parity(o1, ref, ab, "dense path, bin once grid twice")
-
-
-@pytest.mark.parametrize("tlog,chunk", [(2, 256), (3, 4096)])
-def test_pre_summation_straight_from_the_sorted_runs(dev, tlog, chunk):
-    """Dense plan binned by channel runs: reduce_runs_kernel reads the sorted runs (no per-entry list is
-    written) and must produce the same records, hence the same bits, as reduce_kernel on the expanded list."""
-    wl = synth.make_workload(1, n_time=2)
-    vis = wl.visibilities("cpu").numpy()
-    rng = np.random.default_rng(95)
-    w = rng.uniform(0.5, 1.5, vis.shape[:-2]).astype(np.float32)
-    kw = dict(N=wl.grid_size, du=wl.cell_size, O=wl.oversample, S=wl.support[0], table=wl.kernel)
-    env = {"GRIDDER_QBINS": 2, "GRIDDER_RUNS": 2, "GRIDDER_TILE_LOG2": tlog, "GRIDDER_CHUNK": chunk}
-    a, st_a = _run(dev, wl.uvw, wl.freq, vis, w, env=dict(env, GRIDDER_FUSE=1), **kw)
-    a2, _ = _run(dev, wl.uvw, wl.freq, vis, w, env=dict(env, GRIDDER_FUSE=1), **kw)
-    b, st_b = _run(dev, wl.uvw, wl.freq, vis, w, env=dict(env, GRIDDER_FUSE=0), **kw)
-    c, st_c = _run(dev, wl.uvw, wl.freq, vis, w, env=dict(env, GRIDDER_RUNS=0), **kw)
-    assert np.array_equal(a, a2) and np.array_equal(a, b) and np.array_equal(a, c)
-    assert st_a.n_records_gridded == st_b.n_records_gridded == st_c.n_records_gridded
-    assert st_a.n_work_items == st_b.n_work_items and st_a.vis_taps == st_b.vis_taps
-    ref, ab, ost = _oracle(wl.uvw, wl.freq, vis, w, **kw)
-    assert st_a.n_dropped == ost["n_dropped"]
-    assert_parity(a, ref, ab, f"pre-summation from runs T={1 << tlog}")
-
-
-def test_dense_path_randomised_sweep(dev):
-    """60 seeded random small problems through every variant of the dense path (pre-summation from the expanded
-    list or from the runs, bins inside the grid kernel, table in shared or tensor memory; tiles 4/8/16; chunks
-    down to one batch; counts around the 32- and 64-entry batch sizes; lattice ties; with and without weights)."""
-    rng = np.random.default_rng(2024)
-    for it in range(60):
-        S = int(rng.choice([9, 10, 12, 13, 15, 16]))
-        O = int(rng.choice([1, 2, 4])) if S % 2 == 0 else int(rng.choice([2, 4]))
-        N = int(rng.choice([48, 64, 96, 130]))
-        n = int(rng.choice([1, 31, 32, 33, 63, 64, 65, 127, 128, 129, 1000, 4097, 20000]))
-        spread = float(rng.choice([0.4, 2.0, 8.0, N / 2 + 1]))
-        table = rng.standard_normal((S * O, S * O)).astype(np.float32)
-        uvw = np.zeros((1, n, 3))
-        uvw[0, :, :2] = rng.uniform(-spread, spread, (n, 2))
-        if rng.random() < 0.3:
-            uvw[0, :, :2] = np.round(uvw[0, :, :2] * O) / O
-        vis = rng.standard_normal((n, 4, 2)).astype(np.float32)
-        w = None if rng.random() < 0.3 else rng.uniform(0.0, 1.5, n).astype(np.float32)
-        kw = dict(N=N, du=1.0, O=O, S=S, table=table)
-        env = {"GRIDDER_QBINS": 2, "GRIDDER_TILE_LOG2": int(rng.choice([2, 3, 4])),
-               "GRIDDER_CHUNK": int(rng.choice([32, 64, 100, 256, 4096])), "GRIDDER_RUNS": int(rng.choice([0, 2])),
-               "GRIDDER_FUSE": int(rng.choice([0, 1])), "GRIDDER_TMEM": int(rng.choice([0, 1])),
-               "GRIDDER_REDUCE": int(rng.choice([0, 1, 1]))}
-        got, st = _run(dev, uvw, [C], vis, w, env=env, **kw)
-        ref, ab, ost = _oracle(uvw, [C], vis, w, **kw)
-        assert st.n_dropped == ost["n_dropped"] and st.vis_taps == ost["vis_taps"], (it, env)
-        assert 0 < st.n_records_gridded <= st.n_vis, (it, env)        # (dropped visibilities end in a record of zeros)
-        assert_parity(got, ref, ab, f"sweep case {it} {env}")
+    assert_parity(got, ref, ab, "S=16 O=16")

@@ -11,7 +11,7 @@ from _util import as_complex, assert_parity, oracle_kwargs
 from test_gpu_parity import _gridder, _oracle, _run, C
 
 pytestmark = pytest.mark.gpu
-PS = {"GRIDDER_PRESUM": 2}
+PS = {"presum": 1}
 
 
 @pytest.fixture(scope="module")
@@ -27,8 +27,8 @@ def test_presum_config1_full_grid(dev):
     wl = synth.make_workload(1)
     vis = wl.visibilities("cpu").numpy()
     kw = dict(N=wl.grid_size, du=wl.cell_size, O=wl.oversample, S=wl.support[0], table=wl.kernel)
-    a, st = _run(dev, wl.uvw, wl.freq, vis, None, env=PS, **kw)
-    b, _ = _run(dev, wl.uvw, wl.freq, vis, None, env=PS, **kw)
+    a, st = _run(dev, wl.uvw, wl.freq, vis, None, tuning=PS, **kw)
+    b, _ = _run(dev, wl.uvw, wl.freq, vis, None, tuning=PS, **kw)
     ref, ab, ost = oracle.grid_full(wl.uvw, wl.freq, vis, None, **oracle_kwargs(wl))
     assert 0 < st.n_presum_records < wl.n_vis
     assert st.n_dropped == ost["n_dropped"] == 0 and st.vis_taps == ost["vis_taps"]
@@ -52,15 +52,15 @@ def test_presum_ragged_groups_weights_and_drops(dev, nt, nb, nf, band):
     vis = rng.standard_normal((nt, nb, nf, 4, 2)).astype(np.float32)
     w = rng.uniform(0.0, 1.5, (nt, nb, nf)).astype(np.float32)
     kw = dict(N=N, du=1.0, O=O, S=S, table=table)
-    a, st = _run(dev, uvw, freq, vis, w, env=PS, **kw)
-    a2, _ = _run(dev, uvw, freq, vis, w, env=PS, **kw)
+    a, st = _run(dev, uvw, freq, vis, w, tuning=PS, **kw)
+    a2, _ = _run(dev, uvw, freq, vis, w, tuning=PS, **kw)
     ref, ab, ost = _oracle(uvw, freq, vis, w, **kw)
     assert st.n_presum_records > 0
     assert st.n_dropped == ost["n_dropped"] and st.vis_taps == ost["vis_taps"]
     assert np.array_equal(a, a2)
     assert_parity(a, ref, ab, f"presum {nt}x{nb}x{nf}")
     # the classic per-visibility path agrees within tolerance too
-    c, st_c = _run(dev, uvw, freq, vis, w, env={"GRIDDER_PRESUM": 0}, **kw)
+    c, st_c = _run(dev, uvw, freq, vis, w, tuning={"presum": 2}, **kw)
     assert st_c.n_presum_records == 0
     assert_parity(c, ref, ab, "classic")
 
@@ -84,7 +84,7 @@ def test_presum_adversarial_key_sequences(dev):
     vis = rng.standard_normal((nt, nb, nf, 4, 2)).astype(np.float32)
     w = rng.uniform(0.5, 1.5, (nt, nb, nf)).astype(np.float32)
     kw = dict(N=N, du=1.0, O=O, S=S, table=table)
-    a, st = _run(dev, uvw, freq, vis, w, env=PS, **kw)
+    a, st = _run(dev, uvw, freq, vis, w, tuning=PS, **kw)
     ref, ab, ost = _oracle(uvw, freq, vis, w, **kw)
     assert st.n_presum_records > 0 and 0 < st.n_dropped == ost["n_dropped"]
     assert st.vis_taps == ost["vis_taps"]
@@ -102,7 +102,7 @@ def test_presum_nothing_to_merge_and_shapes_that_fall_back(dev):
     freq = C * rng.uniform(0.2, 1.0, nf)
     vis = rng.standard_normal((1, nb, nf, 4, 2)).astype(np.float32)
     kw = dict(N=N, du=1.0, O=O, S=S, table=table)
-    a, st = _run(dev, uvw, freq, vis, None, env=PS, **kw)
+    a, st = _run(dev, uvw, freq, vis, None, tuning=PS, **kw)
     ref, ab, ost = _oracle(uvw, freq, vis, None, **kw)
     assert st.n_dropped == ost["n_dropped"] > 0
     assert 0.9 * (nb * nf - st.n_dropped) <= st.n_presum_records <= nb * nf - st.n_dropped
@@ -113,7 +113,7 @@ def test_presum_nothing_to_merge_and_shapes_that_fall_back(dev):
     uvw1 = np.zeros((1, nb1, 3))
     uvw1[0, :, :2] = rng.uniform(-N / 2 - 1, N / 2 + 1, (nb1, 2))
     vis1 = rng.standard_normal((1, nb1, 1, 4, 2)).astype(np.float32)
-    b, st_b = _run(dev, uvw1, freq[:1], vis1, None, env=PS, **kw)
+    b, st_b = _run(dev, uvw1, freq[:1], vis1, None, tuning=PS, **kw)
     ref, ab, ost = _oracle(uvw1, freq[:1], vis1, None, **kw)
     assert st_b.n_presum_records == 0 and st_b.n_dropped == ost["n_dropped"] and st_b.vis_taps == ost["vis_taps"]
     assert_parity(b, ref, ab, "single channel: per-visibility path")
@@ -124,7 +124,7 @@ def test_presum_bin_once_grid_twice_accumulate_and_empty(dev):
     N, S, O, nt, nb, nf = 64, 16, 4, 4, 50, 40
     table = synth.spheroidal_table(S, O)
     kw = dict(N=N, du=1.0, O=O, S=S, table=table)
-    got, st = _run(dev, np.zeros((1, 0, 3)), [C], np.zeros((0, 4, 2), np.float32), None, env=PS, **kw)
+    got, st = _run(dev, np.zeros((1, 0, 3)), [C], np.zeros((0, 4, 2), np.float32), None, tuning=PS, **kw)
     assert st.n_vis == 0 and st.n_work_items == 0 and not got.any()
     uvw = np.zeros((nt, nb, 3))
     uvw[:, :, :2] = rng.uniform(-20.0, 20.0, (1, nb, 2))
@@ -133,9 +133,9 @@ def test_presum_bin_once_grid_twice_accumulate_and_empty(dev):
     w = rng.uniform(0.5, 1.5, (nt, nb, nf)).astype(np.float32)
     ref, ab, _ = _oracle(uvw, freq, vis, w, **kw)
     base = rng.standard_normal((4, N, N, 2)).astype(np.float32)
-    got, _ = _run(dev, uvw, freq, vis, w, env=PS, accumulate_onto=base, **kw)
+    got, _ = _run(dev, uvw, freq, vis, w, tuning=PS, accumulate_onto=base, **kw)
     assert_parity(got, ref + as_complex(base), ab + np.abs(as_complex(base)), "presum accumulate")
-    g = _gridder(dev, max_vis=nt * nb * nf, env=PS, **kw)
+    g = _gridder(dev, max_vis=nt * nb * nf, tuning=PS, **kw)
     d_uvw, d_f = torch.from_numpy(uvw).to(dev), torch.from_numpy(freq).to(dev)
     d_v, d_w = torch.from_numpy(vis).to(dev), torch.from_numpy(w).to(dev)
     g.bin(d_uvw, d_f)
@@ -147,3 +147,40 @@ def test_presum_bin_once_grid_twice_accumulate_and_empty(dev):
     g.destroy()
     assert np.array_equal(o1, o2) and np.array_equal(o1, o3) and np.array_equal(o4, 2.0 * o1)
     assert_parity(o1, ref, ab, "presum, bin once grid twice")
+
+
+def test_presum_randomised_sweep(dev):
+    """40 seeded random multi-channel problems through the pre-summed path: shapes around the 8-row x 32-channel
+    group (ragged in both), tiles 4/8/16, chunks down to one batch, table in shared or tensor memory, with and
+    without weights, bands from 'every channel on one point' to 'every channel elsewhere'."""
+    rng = np.random.default_rng(2025)
+    for it in range(40):
+        S = int(rng.choice([9, 12, 13, 15, 16]))
+        O = int(rng.choice([1, 2, 4])) if S % 2 == 0 else int(rng.choice([2, 4, 8]))
+        N = int(rng.choice([48, 64, 96, 130]))
+        nt = int(rng.choice([1, 2, 3, 5, 8, 9, 17]))
+        nb = int(rng.choice([1, 7, 8, 9, 40, 150]))
+        nf = int(rng.choice([1, 2, 31, 32, 33, 64, 100]))
+        if nt * nb * nf > 60_000:
+            nb = max(1, 60_000 // (nt * nf))
+        spread = float(rng.choice([0.4, 3.0, N / 3, N / 2 + 1]))
+        band = float(rng.choice([0.0, 1e-4, 2e-3, 3e-2]))
+        table = rng.standard_normal((S * O, S * O)).astype(np.float32)
+        uvw = np.zeros((nt, nb, 3))
+        uvw[0, :, :2] = rng.uniform(-spread, spread, (nb, 2))
+        rot = float(rng.choice([0.0, 1e-4, 1e-2])) * np.arange(nt)[:, None]
+        uvw[:, :, 0] = uvw[0, :, 0] * np.cos(rot) - uvw[0, :, 1] * np.sin(rot)
+        uvw[:, :, 1] = uvw[0, :, 0] * np.sin(rot) + uvw[0, :, 1] * np.cos(rot)
+        if rng.random() < 0.3:
+            uvw[:, :, :2] = np.round(uvw[:, :, :2] * O) / O
+        freq = C * (1.0 + band * np.arange(nf))
+        vis = rng.standard_normal((nt, nb, nf, 4, 2)).astype(np.float32)
+        w = None if rng.random() < 0.3 else rng.uniform(0.0, 1.5, (nt, nb, nf)).astype(np.float32)
+        kw = dict(N=N, du=1.0, O=O, S=S, table=table)
+        tuning = {"presum": 1, "tile_log2": int(rng.choice([2, 3, 4])), "chunk": int(rng.choice([32, 64, 100, 256, 4096])),
+                  "table_in_tmem": int(rng.choice([1, 2]))}
+        got, st = _run(dev, uvw, freq, vis, w, tuning=tuning, **kw)
+        ref, ab, ost = _oracle(uvw, freq, vis, w, **kw)
+        what = f"sweep case {it}: {nt}x{nb}x{nf} S={S} O={O} N={N} {tuning}"
+        assert st.n_dropped == ost["n_dropped"] and st.vis_taps == ost["vis_taps"], what
+        assert_parity(got, ref, ab, what)

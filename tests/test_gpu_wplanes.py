@@ -2,8 +2,6 @@
 patch classes), complex tables conjugated for w < 0 (BASELINE.json config 3; R13), and real
 tables read from global memory.  Same bar as test_gpu_parity.py: integer work bit-exact, grid cells
 within 1e-5 * sum|w V C| + 1e-6, reruns bit-identical."""
-import os
-
 import numpy as np
 import pytest
 import torch
@@ -25,22 +23,6 @@ def dev():
     return torch.device("cuda:0")
 
 
-class _Env:
-    def __init__(self, **kw):
-        self.kw = {k: str(v) for k, v in kw.items()}
-
-    def __enter__(self):
-        self.old = {k: os.environ.get(k) for k in self.kw}
-        os.environ.update(self.kw)
-
-    def __exit__(self, *a):
-        for k, v in self.old.items():
-            if v is None:
-                os.environ.pop(k, None)
-            else:
-                os.environ[k] = v
-
-
 def _tables(rng, supports, O, cplx):
     parts = []
     for s in supports:
@@ -60,13 +42,12 @@ def _case(rng, n, N, w_max, n_tie=40):
     return uvw, vis, w
 
 
-def _both(dev, uvw, freq, vis, weight, *, N, du, O, supports, table, w_max, cplx, env=None):
+def _both(dev, uvw, freq, vis, weight, *, N, du, O, supports, table, w_max, cplx, tuning=None):
     from paper_1003_5575_b200 import gridder
     n = uvw.shape[0] * uvw.shape[1] * len(freq)
-    with _Env(**(env or {})):
-        g = gridder.Gridder(grid_size=N, cell_size=du, oversample=O, support=list(supports),
-                            kernel=torch.from_numpy(table).to(dev), max_vis=max(n, 1), n_wplanes=len(supports),
-                            w_max=w_max, kernel_is_complex=cplx)
+    g = gridder.Gridder(grid_size=N, cell_size=du, oversample=O, support=list(supports),
+                        kernel=torch.from_numpy(table).to(dev), max_vis=max(n, 1), n_wplanes=len(supports),
+                        w_max=w_max, kernel_is_complex=cplx, tuning=tuning)
     d_uvw = torch.from_numpy(np.ascontiguousarray(uvw)).to(dev)
     d_f = torch.tensor(np.asarray(freq, np.float64), device=dev)
     got_map = g.map(d_uvw, d_f).cpu().numpy()
@@ -94,7 +75,7 @@ def test_general_path_equals_oracle_on_single_real_table(dev, S, O, N, n):
     table = _tables(rng, [S], O, False)
     uvw, vis, w = _case(rng, n, N, 1.0)
     got, ref, ab, st, _ = _both(dev, uvw, [C], vis, w, N=N, du=1.0, O=O, supports=[S], table=table, w_max=1.0,
-                                cplx=False, env={"GRIDDER_FORCE_GENERAL": 1})
+                                cplx=False, tuning={"force_general": 1})
     assert st.n_dropped > 0
     assert_parity(got, ref, ab, f"general real S={S}")
 
@@ -121,7 +102,7 @@ def test_wplanes_mixed_supports_all_three_patch_classes(dev, cplx, tlog):
     vis2 = np.stack([vis, vis[::-1]], 1).copy()               # [n][2 channels][4][2]
     w2 = np.stack([w, w[::-1]], 1).copy()
     got, ref, ab, st, ost = _both(dev, uvw, [C, 0.9 * C], vis2, w2, N=N, du=1.0, O=O, supports=supports, table=table,
-                                  w_max=w_max, cplx=cplx, env={"GRIDDER_TILE_LOG2": tlog})
+                                  w_max=w_max, cplx=cplx, tuning={"tile_log2": tlog})
     assert st.tile_size == 1 << tlog and 0 < st.n_dropped < 2 * n
     assert_parity(got, ref, ab, f"w-planes cplx={cplx} T={1 << tlog}")
 
@@ -136,7 +117,7 @@ def test_wplanes_hot_tile_chunks_and_unit_weights(dev):
     uvw[0, :, 2] = rng.uniform(-3.0, 3.0, n)
     vis = (rng.standard_normal((n, 4, 2)) + 2.0).astype(np.float32)
     got, ref, ab, st, _ = _both(dev, uvw, [C], vis, None, N=N, du=1.0, O=O, supports=supports, table=table, w_max=w_max,
-                                cplx=True, env={"GRIDDER_CHUNK": 256})
+                                cplx=True, tuning={"chunk": 256})
     assert st.chunk_size == 256 and st.max_tile_load > 256 and st.n_work_items > n // 256
     assert_parity(got, ref, ab, "w-planes hot tile")
 
@@ -185,3 +166,35 @@ def test_per_baseline_tables_row_f3(dev, cplx):
     assert st.n_dropped == ost["n_dropped"] >= 4 * nf and st.vis_taps == ost["vis_taps"]
     assert np.array_equal(out1, out2)
     assert_parity(out1, ref, ab, f"per-baseline tables, complex={cplx}")
+
+
+@pytest.mark.parametrize("presum", [1, 2])
+def test_per_baseline_tables_bank_of_one_on_the_fast_path(dev, presum):
+    """A bank of ONE real table takes the fast path, where there is nothing to choose -- but an index outside
+    the bank must still drop its baseline (include/gridder.h), as the oracle does.  Whether or not the plan
+    would pre-sum: a table_index always goes through the per-visibility map."""
+    from paper_1003_5575_b200 import gridder
+    rng = np.random.default_rng(71)
+    S, O, N, nb, nf = 16, 4, 96, 2000, 4
+    table = _tables(rng, [S], O, False)
+    uvw = np.zeros((1, nb, 3))
+    uvw[:, :, :2] = rng.uniform(-N / 2 + S, N / 2 - S, (1, nb, 2)) / 1.1
+    freq = C * np.array([1.0, 1.01, 1.02, 1.03])
+    idx = np.zeros((1, nb), np.int32)
+    idx[0, ::7] = -1
+    idx[0, 3::11] = 1
+    vis = rng.standard_normal((1, nb, nf, 4, 2)).astype(np.float32)
+    g = gridder.Gridder(grid_size=N, cell_size=1.0, oversample=O, support=[S], kernel=torch.from_numpy(table).to(dev),
+                        max_vis=nb * nf, tuning={"presum": presum})
+    d_uvw, d_f, d_idx = torch.from_numpy(uvw).to(dev), torch.from_numpy(freq).to(dev), torch.from_numpy(idx).to(dev)
+    got_map = g.map(d_uvw, d_f, table_index=d_idx).cpu().numpy()
+    g.bin(d_uvw, d_f, table_index=d_idx)
+    out = g.grid(torch.from_numpy(vis).to(dev)).cpu().numpy()
+    st = g.stats()
+    g.destroy()
+    kw = dict(grid_size=N, cell_size=1.0, oversample=O, support=[S], kernel=table, table_index=idx)
+    assert np.array_equal(got_map, oracle.map_visibilities(uvw, freq, **kw))
+    ref, ab, ost = oracle.grid_full(uvw, freq, vis, None, **kw)
+    n_bad = int(((idx < 0) | (idx > 0)).sum()) * nf
+    assert st.n_dropped == ost["n_dropped"] == n_bad and st.vis_taps == ost["vis_taps"] and st.n_presum_records == 0
+    assert_parity(out, ref, ab, "bank of one table with indices outside it")
