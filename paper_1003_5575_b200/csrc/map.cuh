@@ -207,36 +207,34 @@ struct FastMap2 {
         aux_bits = (uint32_t)p.key.aux_bits; bits_q = (uint32_t)p.key.bits_q; tile_shift = (uint32_t)p.key.tile_shift;
     }
     __device__ __forceinline__ double chan_scale(double s) const { return __dmul_rn(__dmul_rn(s, rcp_cell), d_o); }
-    __device__ __forceinline__ bool axis(double coord_m, double ks, int &x0, int &q) const {
+    // sort key of the visibility (fast_key's layout; a dropped visibility has the drop bit, 1 << 2 bits_q, set).
+    // Both axes are computed first and tested together: one branch per visibility.  Returns kUndecided where the
+    // screen does not decide: the caller then takes slow_key.
+    __device__ __forceinline__ uint32_t key(double u_m, double v_m, double ks) const {
         const double kMagic = 6755399441055744.0;               // 1.5 * 2^52
-        const double t1 = __fma_rn(coord_m, ks, chalf);
-        const double m = __dadd_rn(t1, kMagic);
-        const double d = __dadd_rn(t1, -__dadd_rn(m, -kMagic));
-        if (!(fabs(t1) < span2 && fabs(d) > eps)) return false;
-        const int a = __double2loint(m) - (d < 0.0 ? 1 : 0) - half_so;     // floor(t1) - S O / 2
-        x0 = (a + o_minus_1) >> o_shift;                        // ceil(a / O)
-        q = (x0 << o_shift) - a;
-        return true;
-    }
-    // sort key of the visibility (fast_key's layout); `taps` gets S^2 or 0 (dropped)
-    __device__ __forceinline__ uint32_t key(double u_m, double v_m, double s, double ks, const MapParams &p, int &taps) const {
-        int x0, y0, qx, qy;
-        const bool okx = axis(u_m, ks, x0, qx), oky = axis(v_m, ks, y0, qy);
-        if (okx && oky) {
-            if ((unsigned)x0 > (unsigned)n_minus_s || (unsigned)y0 > (unsigned)n_minus_s) {     // off the grid
-                taps = 0;
+        const double tx = __fma_rn(u_m, ks, chalf), ty = __fma_rn(v_m, ks, chalf);
+        const double mx = __dadd_rn(tx, kMagic), my = __dadd_rn(ty, kMagic);
+        const double dx = __dadd_rn(tx, -__dadd_rn(mx, -kMagic)), dy = __dadd_rn(ty, -__dadd_rn(my, -kMagic));
+        if (fabs(tx) < span2 && fabs(ty) < span2 && fabs(dx) > eps && fabs(dy) > eps) {
+            // floor(t) = RN(t) - (d < 0): the sign of d is the top bit of its high word
+            const int ax = __double2loint(mx) + (__double2hiint(dx) >> 31) - half_so;
+            const int ay = __double2loint(my) + (__double2hiint(dy) >> 31) - half_so;
+            const int x0 = (ax + o_minus_1) >> o_shift, y0 = (ay + o_minus_1) >> o_shift;     // ceil(a / O)
+            if ((unsigned)x0 > (unsigned)n_minus_s || (unsigned)y0 > (unsigned)n_minus_s)     // off the grid
                 return 1u << (2 * bits_q);                      // drop slot 0, tile 0, origin (0, 0)
-            }
-            taps = s2;
+            const uint32_t qx = (uint32_t)((x0 << o_shift) - ax), qy = (uint32_t)((y0 << o_shift) - ay);
             const uint32_t ux = (uint32_t)x0, uy = (uint32_t)y0;
             const uint32_t tile = (uy >> tlog) * ntx + (ux >> tlog);
             return (tile << tile_shift) | ((uy & tmask) << (aux_bits + tlog)) | ((ux & tmask) << aux_bits) |
-                   ((uint32_t)qy << bits_q) | (uint32_t)qx;
+                   (qy << bits_q) | qx;
         }
-        const VisMap mv = map_vis(u_m, v_m, 0.0, s, p);         // rare: near a rounding boundary, or far away
-        taps = mv.dropped ? 0 : mv.S * mv.S;
-        return fast_key(mv, p);
+        return kUndecided;                                      // rare: near a rounding boundary, or far away
     }
+    // what the caller maps such a visibility with (kept out of key() so that unrolled callers inline it once)
+    static __device__ __forceinline__ uint32_t slow_key(double u_m, double v_m, double s, const MapParams &p) {
+        return fast_key(map_vis(u_m, v_m, 0.0, s, p), p);
+    }
+    static constexpr uint32_t kUndecided = 0xFFFFFFFEu;         // never a key (nor kAbsent of presum.cu)
 };
 
 }  // namespace gridder

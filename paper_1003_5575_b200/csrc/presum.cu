@@ -29,8 +29,8 @@
 //     t-runs, added in chain order: a fixed order, so results are bit-identical from run to run.
 //   * records of a group are numbered in (column, row) order of their heads.
 // Flag byte of visibility (t, b, f), meaningful where a t-run starts (0 elsewhere):
-//   bit 0 t-run starts here | bit 1 chain head | bit 2 dropped (off the grid) | bit 3 has a forward link |
-//   bits 4-6 row where the linked t-run of column f + 1 starts.
+//   bit 0 has a forward link | bits 1-3 row where the linked t-run of column f + 1 starts |
+//   bit 4 t-run starts here | bit 5 chain head | bit 6 dropped (off the grid).
 #include <cub/device/device_scan.cuh>
 
 #include "gridder_internal.cuh"
@@ -38,6 +38,7 @@
 
 namespace gridder {
 
+constexpr uint32_t kFlagLink = 1u, kFlagStart = 16u, kFlagHead = 32u, kFlagDrop = 64u;
 constexpr uint32_t kAbsent = 0xFFFFFFFFu;      // no visibility here (ragged group); never a key (see fast_key)
 
 // A group is 8 ROWS x 32 channels; a row is one (integration, baseline).  Rows of a group: rt integrations
@@ -95,7 +96,7 @@ __device__ __forceinline__ uint32_t warp_excl(uint32_t x, int lane, uint32_t &to
 }
 
 template <bool FAST, int RT>
-__global__ void __launch_bounds__(256, 3) presum_plan_kernel(const double *__restrict__ uvw, const double *__restrict__ scale,
+__global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__restrict__ uvw, const double *__restrict__ scale,
                                                            const PsGeo geo, const MapParams p,
                                                            unsigned char *__restrict__ flags, uint32_t *__restrict__ stage,
                                                            uint32_t *__restrict__ count, Counters *counters) {
@@ -104,8 +105,7 @@ __global__ void __launch_bounds__(256, 3) presum_plan_kernel(const double *__res
     const uint32_t dropbit = 1u << (2 * p.key.bits_q);
     FastMap2 fm;
     if (FAST) fm.init(p);
-    unsigned int dropped_here = 0;
-    unsigned long long taps_here = 0;
+    unsigned int dropped_here = 0, mapped_here = 0;
 
     for (uint32_t grp = gw; grp < geo.n_groups; grp += nw) {
         uint32_t t0, b0, f0;
@@ -115,42 +115,48 @@ __global__ void __launch_bounds__(256, 3) presum_plan_kernel(const double *__res
         const double s = col ? scale[f] : 0.0;
         const double ks = FAST ? fm.chan_scale(s) : 0.0;
         uint32_t key[8];
-        uint32_t valid = 0;
+        uint32_t valid = 0, slow = 0;
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
             key[r] = kAbsent;
             uint32_t row;
             if (row_index<RT>(geo, r, t0, b0, row) && col) {
                 const double *L = uvw + (size_t)row * 3;
-                int taps;
-                if (FAST) {
-                    key[r] = fm.key(__ldg(L), __ldg(L + 1), s, ks, p, taps);
-                } else {
-                    const VisMap m = map_vis(__ldg(L), __ldg(L + 1), 0.0, s, p);
-                    taps = m.dropped ? 0 : m.S * m.S;
-                    key[r] = fast_key(m, p);
-                }
-                if (taps == 0) dropped_here++; else taps_here += (unsigned long long)taps;
+                key[r] = FAST ? fm.key(__ldg(L), __ldg(L + 1), ks) : FastMap2::kUndecided;
+                if (key[r] == FastMap2::kUndecided) slow |= 1u << r;
                 valid |= 1u << r;
             }
         }
-        // t-runs (bit r of th: a run starts in row r), dropped runs, rows whose key equals the next column's
-        uint32_t th = 0, drop = 0, eq = 0;
+        while (slow) {              // the screen did not decide (about one visibility in 10^8), or no fast mapper
+            const int r = __ffs(slow) - 1;
+            slow &= slow - 1u;
+            uint32_t row;
+            row_index<RT>(geo, r, t0, b0, row);
+            const double *L = uvw + (size_t)row * 3;
+            const uint32_t k = FastMap2::slow_key(__ldg(L), __ldg(L + 1), s, p);
+#pragma unroll
+            for (int rr = 0; rr < 8; ++rr)
+                if (rr == r) key[rr] = k;
+        }
+        // t-runs (bit r of th: a run starts in row r), dropped visibilities, rows whose key equals the next column's
+        uint32_t th = 0, dropv = 0, eq = 0;
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
             const uint32_t nk = __shfl_down_sync(0xffffffffu, key[r], 1);
             if (!((valid >> r) & 1u)) continue;
-            if (r == 0 || key[r] != key[r - 1]) {
-                th |= 1u << r;
-                if (key[r] & dropbit) drop |= 1u << r;
-            }
+            if (r == 0 || key[r] != key[r - 1]) th |= 1u << r;
+            if (key[r] & dropbit) dropv |= 1u << r;
             if (nk == key[r] && lane < 31) eq |= 1u << r;
         }
+        const uint32_t drop = th & dropv;                   // dropped runs
+        mapped_here += (unsigned)__popc(valid);
+        dropped_here += (unsigned)__popc(dropv);
         // forward links: a run links to the run of the next column that holds the same key in one of the run's
         // own rows (runs of a lattice point in neighbouring columns overlap in their rows, or they are strangers:
         // then they stay two records, which is only a record more).  A target is taken once.
+        // The flag bytes of the 8 rows are assembled in two words, byte r % 4 of word r / 4.
         const uint32_t nth = __shfl_down_sync(0xffffffffu, th, 1);
-        uint32_t link = 0;          // 4 bits per row: has a link | the linked row << 1
+        uint32_t w_lo = 0, w_hi = 0;
         uint32_t targets = 0;       // rows of column f + 1 this column links to
         for (uint32_t m = th & ~drop; m; m &= m - 1u) {
             const int r = __ffs(m) - 1;
@@ -162,11 +168,17 @@ __global__ void __launch_bounds__(256, 3) presum_plan_kernel(const double *__res
             const int h = 31 - __clz(nth & ((2u << rs) - 1u));                // start of the neighbour's run through row rs
             if ((targets >> h) & 1u) continue;
             targets |= 1u << h;
-            link |= (1u | ((uint32_t)h << 1)) << (4 * r);
+            const uint32_t nib = (kFlagLink | ((uint32_t)h << 1)) << (8 * (r & 3));
+            if (r < 4) w_lo |= nib; else w_hi |= nib;
         }
         uint32_t pred = __shfl_up_sync(0xffffffffu, targets, 1);
         if (lane == 0) pred = 0;
         const uint32_t head = th & ~drop & ~pred;
+        // bit k of a 4-bit mask to bit 8 k: the shifted copies of x in x * 0x204081 do not overlap
+        w_lo |= (((th & 15u) * 0x204081u) & 0x01010101u) * kFlagStart | (((head & 15u) * 0x204081u) & 0x01010101u) * kFlagHead |
+                (((drop & 15u) * 0x204081u) & 0x01010101u) * kFlagDrop;
+        w_hi |= (((th >> 4) * 0x204081u) & 0x01010101u) * kFlagStart | (((head >> 4) * 0x204081u) & 0x01010101u) * kFlagHead |
+                (((drop >> 4) * 0x204081u) & 0x01010101u) * kFlagDrop;
         // records of the group in (column, row) order of their heads
         uint32_t total;
         uint32_t idx = warp_excl((uint32_t)__popc(head), lane, total);
@@ -178,21 +190,19 @@ __global__ void __launch_bounds__(256, 3) presum_plan_kernel(const double *__res
             if (valid & bit) {
                 uint32_t row;
                 row_index<RT>(geo, r, t0, b0, row);
-                unsigned char fl = 0;
-                if (th & bit)
-                    fl = (unsigned char)(1u | ((head & bit) ? 2u : 0u) | ((drop & bit) ? 4u : 0u) | (((link >> (4 * r)) & 15u) << 3));
-                flags[row * geo.n_chan + f] = fl;
+                flags[row * geo.n_chan + f] = (unsigned char)((r < 4 ? w_lo : w_hi) >> (8 * (r & 3)));
                 if (head & bit) st[idx++] = key[r];
             }
         }
     }
     for (int o = 16; o > 0; o >>= 1) {
         dropped_here += __shfl_xor_sync(0xffffffffu, dropped_here, o);
-        taps_here += __shfl_xor_sync(0xffffffffu, taps_here, o);
+        mapped_here += __shfl_xor_sync(0xffffffffu, mapped_here, o);
     }
-    if (lane == 0) {
+    if (lane == 0) {      // (fast path: one table, every gridded visibility has S^2 taps)
         if (dropped_here) atomicAdd(&counters->n_dropped, (unsigned long long)dropped_here);
-        if (taps_here) atomicAdd(&counters->vis_taps, taps_here);
+        const unsigned long long taps = (unsigned long long)(mapped_here - dropped_here) * (unsigned)(p.support[0] * p.support[0]);
+        if (taps) atomicAdd(&counters->vis_taps, taps);
     }
 }
 
@@ -288,12 +298,12 @@ __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__r
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
             sflag[r * 32 + lane] = (unsigned char)fl[r];
-            if (fl[r] & 1u) {
+            if (fl[r] & kFlagStart) {
                 if (start >= 0) { slotA[start * 32 + lane] = xa; slotB[start * 32 + lane] = xb; }
                 start = r;
                 xa = make_float4(w[r] * va[r].x, w[r] * va[r].y, w[r] * va[r].z, w[r] * va[r].w);
                 xb = make_float4(w[r] * vb[r].x, w[r] * vb[r].y, w[r] * vb[r].z, w[r] * vb[r].w);
-                if (fl[r] & 2u) head |= 1u << r;
+                if (fl[r] & kFlagHead) head |= 1u << r;
             } else {
                 xa.x = fmaf(w[r], va[r].x, xa.x); xa.y = fmaf(w[r], va[r].y, xa.y);
                 xa.z = fmaf(w[r], va[r].z, xa.z); xa.w = fmaf(w[r], va[r].w, xa.w);
@@ -312,8 +322,8 @@ __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__r
             float4 sa = slotA[r * 32 + lane], sb = slotB[r * 32 + lane];
             uint32_t cf = sflag[r * 32 + lane];
             int c = lane;
-            while (cf & 8u) {
-                const int rr = (int)((cf >> 4) & 7u);
+            while (cf & kFlagLink) {
+                const int rr = (int)((cf >> 1) & 7u);
                 ++c;
                 const float4 ta = slotA[rr * 32 + c], tb4 = slotB[rr * 32 + c];
                 sa.x += ta.x; sa.y += ta.y; sa.z += ta.z; sa.w += ta.w;
@@ -339,10 +349,10 @@ __global__ void __launch_bounds__(256) map_presum_debug_kernel(const double *__r
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
         const long long tb = i / n_chan;
         const double s = __ddiv_rn(freq[(int)(i - tb * n_chan)], kSpeedOfLight);
-        int taps;
-        const uint32_t key = fm.key(uvw[tb * 3], uvw[tb * 3 + 1], s, fm.chan_scale(s), p, taps);
+        uint32_t key = fm.key(uvw[tb * 3], uvw[tb * 3 + 1], fm.chan_scale(s));
+        if (key == FastMap2::kUndecided) key = FastMap2::slow_key(uvw[tb * 3], uvw[tb * 3 + 1], s, p);
         int32_t *o = out + i * 6;
-        if (taps == 0) {
+        if (key & (1u << (2 * p.key.bits_q))) {
             o[0] = o[1] = o[2] = o[3] = o[4] = 0; o[5] = 1;
         } else {
             const uint32_t tile = key >> p.key.tile_shift;
