@@ -153,11 +153,12 @@ int derive(const gridder_config *cfg, const gridder_tuning *tuning, Plan &p) {
     // each class has its own partial-region array, sized for the case that every entry is of that class
     p.max_items_cls = (n < p.n_tiles ? n : p.n_tiles) + n / p.chunk + 1;
     if (p.presum) {
-        // partial-record sums: room for 3/4 of the visibilities (inputs that merge less take the per-visibility
-        // path); the plan kernel's staging slots live in the same array
+        // The sums of a group's partial records live in the group's own visibility slots (presum.cu slot_index), so
+        // they need an array as large as the visibilities.  Inputs that merge into more than 3/4 n records take the per-visibility path (decided
+        // per gridder_bin from the count the plan kernel returns).  The plan kernel stages the record keys in the
+        // sort's second key buffer.
         p.ps_cap = n * 3 / 4 + 1024;
-        p.ps_stage_cap = p.ps_cap * 8;
-        p.ps_group_cap = n * 3 / 16 + 1024;
+        p.ps_group_cap = n / 8 + 1024;
     }
     p.partials_f4 = 0;
     for (int c = 0; c < p.n_cls; ++c) {
@@ -174,8 +175,11 @@ cudaError_t carve(Plan &p, char *base) {
     const size_t n = (size_t)(p.cfg.max_vis > 0 ? p.cfg.max_vis : 1);
     const size_t n_vtiles = (size_t)p.n_tiles * p.n_cls;
     const size_t val_bytes = p.mode == 0 ? sizeof(uint32_t) : sizeof(unsigned long long);
-    for (int i = 0; i < 2; ++i) p.keys[i] = (uint32_t *)take(n * sizeof(uint32_t));
-    for (int i = 0; i < 2; ++i) p.vals[i] = (void *)take(n * val_bytes);
+    // (keys[1] and vals[1] next to each other: together they are the staging area of the pre-summed plans)
+    p.keys[0] = (uint32_t *)take(n * sizeof(uint32_t));
+    p.vals[0] = (void *)take(n * val_bytes);
+    p.keys[1] = (uint32_t *)take(n * sizeof(uint32_t));
+    p.vals[1] = (void *)take(n * val_bytes);
     size_t t1 = 0, t2 = 0;
     cudaError_t e = sort_temp_bytes((int64_t)n, p.key.aux_bits, p.key.total_bits, p.mode != 0, &t1);
     if (e == cudaSuccess) e = scan_temp_bytes((int64_t)n_vtiles + 1, &t2);
@@ -206,7 +210,7 @@ cudaError_t carve(Plan &p, char *base) {
         p.ps_flags = (unsigned char *)take(n);
         p.ps_count = (uint32_t *)take(sizeof(uint32_t) * (size_t)(p.ps_group_cap + 1));
         p.ps_base = (uint32_t *)take(sizeof(uint32_t) * (size_t)(p.ps_group_cap + 1));
-        p.ps_sum = (float4 *)take(sizeof(float4) * 2 * (size_t)p.ps_cap);
+        p.ps_sum = (float4 *)take(sizeof(float4) * 2 * n);
     }
     p.coef = (float4 *)take(p.coef_bytes);
     p.counters = (Counters *)take(sizeof(Counters));

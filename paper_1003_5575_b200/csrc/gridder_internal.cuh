@@ -153,9 +153,8 @@ struct Plan {
     int32_t presum;
     int32_t presum_active;         // the last gridder_bin took it: keys / vals hold the sorted RECORDS
     int64_t ps_group_cap;          // room for this many groups (count / base arrays)
-    int64_t ps_cap;                // partial records the plan has room for
-    float4 *ps_sum;                // [ps_cap][2] sum of w V per partial record (written by gridder_grid)
-    int64_t ps_stage_cap;          // uint32 staging slots (they live in ps_sum, which is written later)
+    int64_t ps_cap;                // most partial records an input may have to take this path (3/4 max_vis)
+    float4 *ps_sum;                // [max_vis][2] sums of w V of the partial records, in their group's visibility slots
     int32_t ps_n_time, ps_n_bl, ps_n_chan;     // shape of the last bin
     int64_t n_sorted;              // entries of the sorted list of the last bin (records, or visibilities)
     unsigned char *ps_flags;       // [max_vis] one flag byte per visibility

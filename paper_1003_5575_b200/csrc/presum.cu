@@ -53,7 +53,6 @@ struct PsGeo {
     uint32_t n_bgroup;          // ceil(n_bl / rb)
     uint32_t n_groups;          // n_tblock * n_bgroup * n_fchunk; group g = (tb * n_bgroup + bg) * n_fchunk + fc
 };
-constexpr uint32_t kPsSlots = 256;             // staging slots (most records) of a group
 
 __device__ __forceinline__ void group_coords(const PsGeo &g, uint32_t grp, uint32_t &t0, uint32_t &b0, uint32_t &f0) {
     const uint32_t fc = grp % g.n_fchunk, rest = grp / g.n_fchunk;
@@ -81,6 +80,25 @@ __device__ __forceinline__ bool row_index(const PsGeo &g, int r, uint32_t t0, ui
     row_of<RT>(g, r, rt, rb);
     row = (t0 + rt) * g.n_bl + (b0 + rb);
     return (RT > 0 || rb < g.rb) && t0 + rt < g.n_time && b0 + rb < g.n_bl;
+}
+
+// Where the sum of record j of a group lives in ps_sum (an array as large as the visibility array): in the group's
+// own visibility slots, filled row segment by row segment -- so a group's records are contiguous runs of up to 32,
+// their places need no scan over the groups, and no two groups share a slot.  (A group has at most as many records
+// as visibilities.)
+__device__ __forceinline__ uint32_t slot_index(const PsGeo &g, uint32_t t0, uint32_t b0, uint32_t f0, uint32_t j) {
+    const uint32_t ncols = min(32u, g.n_chan - f0), nrt = min(g.rt, g.n_time - t0);
+    const uint32_t k = j / ncols, c = j - k * ncols;          // k-th valid row of the group
+    const uint32_t kb = k / nrt, kt = k - kb * nrt;
+    return ((t0 + kt) * g.n_bl + (b0 + kb)) * g.n_chan + f0 + c;
+}
+
+// Where a group's staged record keys start: the number of visibilities of the groups before it (group order: t-block,
+// baseline group, channel chunk) -- a closed form, so the staging area is exactly as large as the visibility count
+// however ragged the groups are.  (A group has at most as many records as visibilities.)
+__device__ __forceinline__ uint32_t stage_offset(const PsGeo &g, uint32_t t0, uint32_t b0, uint32_t f0) {
+    const uint32_t nrt = min(g.rt, g.n_time - t0), nrb = min(g.rb, g.n_bl - b0);
+    return (t0 * g.n_bl + nrt * b0) * g.n_chan + nrt * nrb * f0;
 }
 
 // exclusive prefix of x over the lanes of a warp, and the total
@@ -183,7 +201,7 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
         uint32_t total;
         uint32_t idx = warp_excl((uint32_t)__popc(head), lane, total);
         if (lane == 0) count[grp] = total;
-        uint32_t *st = stage + (size_t)grp * kPsSlots;
+        uint32_t *st = stage + stage_offset(geo, t0, b0, f0);
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
             const uint32_t bit = 1u << r;
@@ -206,7 +224,7 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
     }
 }
 
-// Staged record keys -> their final places (group order); the sort's values are the record indices.
+// Staged record keys -> their final places (group order).  The sort's values name the record's sum (slot_index).
 __global__ void __launch_bounds__(256) presum_compact_kernel(const uint32_t *__restrict__ stage,
                                                               const uint32_t *__restrict__ count,
                                                               const uint32_t *__restrict__ base, const PsGeo geo,
@@ -215,10 +233,12 @@ __global__ void __launch_bounds__(256) presum_compact_kernel(const uint32_t *__r
     const uint32_t nw = gridDim.x * 8u;
     for (uint32_t grp = blockIdx.x * 8u + (threadIdx.x >> 5); grp < geo.n_groups; grp += nw) {
         const uint32_t cnt = count[grp], dst = base[grp];
-        const uint32_t *st = stage + (size_t)grp * kPsSlots;
+        uint32_t t0, b0, f0;
+        group_coords(geo, grp, t0, b0, f0);
+        const uint32_t *st = stage + stage_offset(geo, t0, b0, f0);
         for (uint32_t j = lane; j < cnt; j += 32) {
             rec_key[dst + j] = st[j];
-            rec_idx[dst + j] = dst + j;
+            rec_idx[dst + j] = slot_index(geo, t0, b0, f0, j);
         }
     }
 }
@@ -235,11 +255,11 @@ constexpr int kPsWarpF4 = 2 * 8 * 32 + 16;          // slot planes A and B [row]
 
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" :: "l"(p)); }
 
-// gridder_grid, first kernel of a pre-summed plan: ps_sum[record] = sum over the record's chain of w V.
+// gridder_grid, first kernel of a pre-summed plan: ps_sum[slot_index(group, j)] = sum over the chain of record j
+// of the group of w V.
 template <bool WEIGHTED, int RT>
 __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__restrict__ vis, const float *__restrict__ weight,
-                                                               const unsigned char *__restrict__ flags,
-                                                               const uint32_t *__restrict__ base, const PsGeo geo,
+                                                               const unsigned char *__restrict__ flags, const PsGeo geo,
                                                                float4 *__restrict__ rec_sum) {
     __shared__ float4 smem[kPsWarps * kPsWarpF4];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -289,7 +309,6 @@ __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__r
                 fl[r] = flags[i];
             }
         }
-        const uint32_t rbase = base[grp];
         // t-runs: a column's visibilities are added down the rows; a finished run goes to the slot of the row
         // it started in
         float4 xa = make_float4(0.f, 0.f, 0.f, 0.f), xb = xa;
@@ -315,7 +334,7 @@ __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__r
         __syncwarp();
         // chain heads: walk the chain through the columns, adding the t-run sums in chain order
         uint32_t total;
-        uint32_t idx = rbase + warp_excl((uint32_t)__popc(head), lane, total);
+        uint32_t j = warp_excl((uint32_t)__popc(head), lane, total);       // records in (column, row) order of their heads
         while (head) {
             const int r = __ffs(head) - 1;
             head &= head - 1u;
@@ -330,9 +349,9 @@ __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__r
                 sb.x += tb4.x; sb.y += tb4.y; sb.z += tb4.z; sb.w += tb4.w;
                 cf = sflag[rr * 32 + c];
             }
-            rec_sum[2 * (size_t)idx] = sa;
-            rec_sum[2 * (size_t)idx + 1] = sb;
-            ++idx;
+            const size_t idx = (size_t)slot_index(geo, t0, b0, f0, j++);
+            rec_sum[2 * idx] = sa;
+            rec_sum[2 * idx + 1] = sb;
         }
         __syncwarp();           // the slots are reused by the next group
     }
@@ -382,7 +401,9 @@ static PsGeo make_geo(int n_time, int n_bl, int n_chan) {
     PsGeo g;
     g.n_time = (uint32_t)n_time; g.n_bl = (uint32_t)n_bl; g.n_chan = (uint32_t)n_chan;
     g.n_fchunk = (uint32_t)((n_chan + 31) / 32);
-    g.rt = (uint32_t)(n_time < 8 ? (n_time > 0 ? n_time : 1) : 8);
+    // integrations per group: at most 8, in t-blocks of equal size (9 integrations: 5 + 4, not 8 + 1)
+    const uint32_t blocks = ((uint32_t)(n_time > 0 ? n_time : 1) + 7u) / 8u;
+    g.rt = ((uint32_t)(n_time > 0 ? n_time : 1) + blocks - 1) / blocks;
     g.rb = 8u / g.rt;
     g.n_tblock = ((uint32_t)n_time + g.rt - 1) / g.rt;
     g.n_bgroup = ((uint32_t)n_bl + g.rb - 1) / g.rb;
@@ -390,14 +411,13 @@ static PsGeo make_geo(int n_time, int n_bl, int n_chan) {
     return g;
 }
 
-// Can this input be pre-summed by the plan?  (Host-side, shapes only: ragged groups are padded to 8 x 32, and
-// the plan has room for 6 staging slots per visibility of its capacity.)
+// Can this input be pre-summed by the plan?  (Host-side, shapes only: the plan has room for max_vis / 8 + 1024
+// groups, i.e. for groups of 8 visibilities and more on average.)
 bool presum_fits(const Plan &p, int n_time, int n_bl, int n_chan) {
     if (!p.presum || n_time <= 0 || n_bl <= 0 || n_chan <= 0) return false;
     const PsGeo g = make_geo(n_time, n_bl, n_chan);
     const unsigned long long ng = (unsigned long long)g.n_tblock * g.n_bgroup * g.n_fchunk;
     if (ng > (unsigned long long)p.ps_group_cap) return false;
-    if (ng * kPsSlots > (unsigned long long)p.ps_stage_cap) return false;       // staging lives in the record sums
     return true;
 }
 
@@ -413,7 +433,8 @@ cudaError_t launch_presum_plan(Plan &p, const double *uvw, const double *scale, 
                                cudaStream_t s, long long *n_rec) {
     const PsGeo geo = make_geo(n_time, n_bl, n_chan);
     const MapParams mp = make_map_params(p);
-    uint32_t *stage = reinterpret_cast<uint32_t *>(p.ps_sum);
+    // staging: the sort's second key buffer, which nothing uses before the sort
+    uint32_t *stage = p.keys[1];
     const int blocks = (int)min((long long)(geo.n_groups + 7) / 8, (long long)p.n_sm * 64);
     GR_TRY(cudaMemsetAsync(p.ps_count + geo.n_groups, 0, sizeof(uint32_t), s));
     const bool fast = mp.o_shift >= 0 && mp.drop_slot == 0;
@@ -446,7 +467,7 @@ cudaError_t launch_presum(Plan &p, const float *vis, const float *weight, cudaSt
     const PsGeo geo = make_geo(p.ps_n_time, p.ps_n_bl, p.ps_n_chan);
     const int blocks = (int)min((long long)(geo.n_groups + kPsWarps - 1) / kPsWarps, (long long)p.n_sm * 32);
     const float4 *v4 = reinterpret_cast<const float4 *>(vis);
-#define PS_SUM(W, R) presum_kernel<W, R><<<blocks, kPsWarps * 32, 0, s>>>(v4, weight, p.ps_flags, p.ps_base, geo, p.ps_sum)
+#define PS_SUM(W, R) presum_kernel<W, R><<<blocks, kPsWarps * 32, 0, s>>>(v4, weight, p.ps_flags, geo, p.ps_sum)
     if (weight) {
         switch (geo.rt) {
             case 8: PS_SUM(true, 8); break;

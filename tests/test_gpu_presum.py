@@ -92,8 +92,8 @@ def test_presum_adversarial_key_sequences(dev):
 
 
 def test_presum_nothing_to_merge_and_shapes_that_fall_back(dev):
-    """Channels at unrelated frequencies: every visibility is its own record.  A large single-channel input
-    pads its groups 32-fold, which the plan has no room for: it takes the per-visibility path instead."""
+    """Channels at unrelated frequencies: every visibility is its own record.  A larger input that does not
+    merge either is handed to the per-visibility path."""
     rng = np.random.default_rng(6)
     N, S, O, nb, nf = 96, 15, 8, 100, 32      # (3 200 visibilities: inside the record capacity of 3n/4 + 1024)
     table = rng.standard_normal((S * O, S * O)).astype(np.float32)
@@ -107,16 +107,16 @@ def test_presum_nothing_to_merge_and_shapes_that_fall_back(dev):
     assert st.n_dropped == ost["n_dropped"] > 0
     assert 0.9 * (nb * nf - st.n_dropped) <= st.n_presum_records <= nb * nf - st.n_dropped
     assert_parity(a, ref, ab, "presum, one record per visibility")
-    # one channel: 8 baselines x 1 channel per group, padded 32-fold -- more staging than a plan of 4 000
-    # visibilities has room for, so the per-visibility path takes it
-    nb1 = 4000
+    # one channel, random positions, 20 000 visibilities: nothing merges, the plan kernel counts more than
+    # 3 n / 4 + 1024 records, and gridder_bin takes the per-visibility path instead (decided from the data)
+    nb1 = 20000
     uvw1 = np.zeros((1, nb1, 3))
     uvw1[0, :, :2] = rng.uniform(-N / 2 - 1, N / 2 + 1, (nb1, 2))
     vis1 = rng.standard_normal((1, nb1, 1, 4, 2)).astype(np.float32)
     b, st_b = _run(dev, uvw1, freq[:1], vis1, None, tuning=PS, **kw)
     ref, ab, ost = _oracle(uvw1, freq[:1], vis1, None, **kw)
     assert st_b.n_presum_records == 0 and st_b.n_dropped == ost["n_dropped"] and st_b.vis_taps == ost["vis_taps"]
-    assert_parity(b, ref, ab, "single channel: per-visibility path")
+    assert_parity(b, ref, ab, "nothing merges: per-visibility path")
 
 
 def test_presum_bin_once_grid_twice_accumulate_and_empty(dev):
