@@ -36,15 +36,12 @@ UNIT = "vis*taps/s"
 FLOP_PER_VIS_TAP = 16            # 4 pol x complex x (mul + add), real GCF table
 FP32_LANES_PER_SM = 128          # guide: 4 SMSP x 32 lanes, one FFMA per lane per clock
 BAND_HZ = 768 * 40.0e3           # one rank's band; rank r starts at 140 MHz + r * BAND_HZ
-# dram__bytes_read.sum + dram__bytes_write.sum of one grid_kernel launch from the committed
-# `ncu --set full` capture (profiles/), keyed by config; None until a capture exists for it.
-NCU_GRID_KERNEL_TRAFFIC_BYTES = {
-    4: 4_177_715_000,     # profiles/r01f_grid_kernel_on_records_config4_ncu_full.csv: 1.763335 GB read + 2.414380 GB written
-    2: 3_500_273_000,     # profiles/r01f_grid_kernel_on_records_config2_ncu_full.csv: 1.150321 GB read + 2.349952 GB written
-}
-# the same for reduce_kernel (dense plans: it is the longest kernel of the step there)
-NCU_REDUCE_KERNEL_TRAFFIC_BYTES = {
-    4: 50_401_785_000,    # profiles/r01f_reduce_kernel_config4_ncu_full.csv: 48.661029 GB read + 1.740756 GB written
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures of this round
+# (profiles/r02_*_ncu_full.csv; historical, i.e. not measured by this run), keyed by kernel and config.
+NCU_TRAFFIC_BYTES = {
+    ("presum_kernel", 4): 32_558_710_000,     # 29.794871 GB read + 2.763839 GB written
+    ("grid_kernel", 4): 5_966_465_000,        # 3.673973 GB read + 2.292492 GB written
+    ("presum_plan_kernel", 4): 1_285_268_000,  # 0.122242 GB read + 1.163026 GB written
 }
 
 
@@ -59,6 +56,10 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (development only)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the oracle leg (development only)")
     ap.add_argument("--no-unmerged", action="store_true", help="skip the merging-off leg (development only)")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the compact legs on configs 0-3 (development only)")
+    ap.add_argument("--spawn-check", action="store_true",
+                    help="host-logic check of the launcher (tests): every rank joins a gloo group and reports its "
+                         "shard, rank 0 prints one JSON line; no GPU work")
     ap.add_argument("--mfs", action="store_true",
                     help="row f4: with N > 1 ranks also sum the per-rank grids inside every timed step "
                          "(deterministic all-to-all + FP64 sum + all-gather); default: no collective")
@@ -142,7 +143,7 @@ class OracleSample:
         self.weight = None if w is None else np.ascontiguousarray(w.numpy())
         self.n_time, self.n_chan = n_time, n_chan
 
-    def run(self):
+    def run(self, n_threads: int = 0):
         """One timed oracle gridding (wall clock of the gridding call only) -> (vis_taps, seconds, threads)."""
         import oracle
         wl = self.wl
@@ -150,7 +151,7 @@ class OracleSample:
         _, _, st = oracle.grid_full(wl.uvw, wl.freq, self.vis, self.weight, grid_size=wl.grid_size,
                                     cell_size=wl.cell_size, oversample=wl.oversample, support=wl.support,
                                     kernel=wl.kernel, w_max=wl.w_max, kernel_is_complex=wl.kernel_is_complex,
-                                    want_abs=False)
+                                    want_abs=False, n_threads=n_threads)
         return st["vis_taps"], time.perf_counter() - t0, st["threads"]
 
     def describe(self) -> str:
@@ -240,6 +241,166 @@ def _host_budget_bytes(world: int) -> int:
     return int(0.6 * avail / max(1, world))
 
 
+def _self_spawn(args) -> int:
+    """`python bench.py --gpus N` without a launcher: start the N ranks ourselves (torchrun's own module, one
+    process per GPU, rendezvous on 127.0.0.1) and hand its exit code back.  NCCL's communicator lines stay on."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), str(Path(__file__).resolve())] + sys.argv[1:]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")
+    return subprocess.call(cmd, env=env)
+
+
+def spawn_check(args) -> dict | None:
+    """What every rank of a launched job does before any GPU work, on gloo: join the group, exchange shard plans."""
+    import torch
+    import torch.distributed as dist
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    mine = torch.tensor([float(shard_plan(world, rank)["f0_hz"])], dtype=torch.float64)
+    got = [torch.zeros_like(mine) for _ in range(world)]
+    if world > 1:
+        dist.all_gather(got, mine)
+        dist.destroy_process_group()
+    else:
+        got = [mine]
+    if rank != 0:
+        return None
+    return {"spawn_check": True, "n_gpus": world, "requested_gpus": args.gpus, "f0_hz": [float(x.item()) for x in got]}
+
+
+class Loaded:
+    """One config resident in HBM: inputs, plan, output grid."""
+
+    def __init__(self, cfg: int, dev, band: int = 0, tuning=None):
+        import torch
+        import synth
+        from paper_1003_5575_b200 import gridder
+        wl = synth.make_workload(cfg, band=band)
+        self.wl = wl
+        nt, nb, nf = wl.n_time, wl.n_baseline, wl.n_chan
+        self.vis = torch.empty((nt, nb, nf, 4, 2), dtype=torch.float32, device=dev)
+        self.weight = torch.empty((nt, nb, nf), dtype=torch.float32, device=dev) if wl.random_weights else None
+        for t in range(nt):
+            self.vis[t] = wl.vis_block(t, dev)
+            if self.weight is not None:
+                self.weight[t] = wl.weight_block(t, dev)
+        self.uvw = torch.from_numpy(wl.uvw).to(dev)
+        self.freq = torch.from_numpy(wl.freq).to(dev)
+        self.table = torch.from_numpy(wl.kernel).to(dev)
+        self.grid = torch.empty((4, wl.grid_size, wl.grid_size, 2), dtype=torch.float32, device=dev)
+        self.dev = dev
+        self.g = self.plan(tuning)
+
+    def plan(self, tuning=None):
+        from paper_1003_5575_b200 import gridder
+        wl = self.wl
+        return gridder.Gridder(grid_size=wl.grid_size, cell_size=wl.cell_size, oversample=wl.oversample, support=wl.support,
+                               kernel=self.table, max_vis=wl.n_vis, n_wplanes=wl.n_wplanes, w_max=wl.w_max,
+                               kernel_is_complex=wl.kernel_is_complex, tuning=tuning)
+
+    def step(self):
+        self.g.bin(self.uvw, self.freq)
+        self.g.grid(self.vis, self.weight, out=self.grid)
+
+    def close(self):
+        self.g.destroy()
+        self.g.workspace = None
+
+
+def timed_steps(step, steps: int, barrier) -> list:
+    """Device milliseconds of each of `steps` calls of step(): CUDA events around every step on the current stream
+    (the stream the library launches on), a barrier + synchronise on both sides of the whole region."""
+    import torch
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    barrier()
+    ev[0].record()
+    for k in range(steps):
+        step()
+        ev[k + 1].record()
+    barrier()
+    return [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
+
+
+def _median(xs):
+    xs = sorted(xs)
+    m = len(xs) // 2
+    return xs[m] if len(xs) % 2 else 0.5 * (xs[m - 1] + xs[m])
+
+
+def kernel_rooflines(L: "Loaded", stage: dict, st, st_exec, ms_per_step: float, fma_peak_tf: float, hbm_peak: float,
+                     hbm_source: str, fma_source: str) -> dict:
+    """the longest kernel of the step against the roofline that bounds it -- 16 (32) flop per
+    visibility-tap against the FP32-FMA peak, or 32 B + 4 B per visibility (+ uvw, + the grid once) against HBM --
+    and the same for the whole step.  Every number here reproduces from stage_ms, config and the stats."""
+    wl, cfg = L.wl, L.wl.cfg
+    n, nt, nb, nf = wl.n_vis, wl.n_time, wl.n_baseline, wl.n_chan
+    has_w = L.weight is not None
+    flop_per_tap = FLOP_PER_VIS_TAP * (2 if wl.kernel_is_complex else 1)
+    grid_bytes = 32 * wl.grid_size ** 2
+    alg_bytes = n * (32 + (4 if has_w else 0)) + nt * nb * 24 + nf * 8 + grid_bytes
+    exec_flop = 2.0 * st_exec.fma_executed
+    nominal_flop = float(flop_per_tap * st.vis_taps)
+    kernels = {}
+
+    def alu(name, ms, flop, extra=None):
+        tf = flop / (ms * 1e-3) / 1e12 if ms > 0 else 0.0
+        d = {"bound": "alu", "kernel": name, "achieved": tf, "peak": fma_peak_tf, "unit": "TFLOP/s",
+             "frac": tf / fma_peak_tf if fma_peak_tf else None, "kernel_ms": ms, "flop_per_launch": flop,
+             "kernel_share_of_step": ms / ms_per_step if ms_per_step else None, "peak_source": fma_source,
+             "traffic": NCU_TRAFFIC_BYTES.get((name, cfg)),
+             "traffic_source": "profiles/r02 ncu --set full capture (historical)" if (name, cfg) in NCU_TRAFFIC_BYTES else None}
+        d.update(extra or {})
+        return d
+
+    def hbm(name, ms, nbytes, extra=None):
+        gbs = nbytes / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
+        d = {"bound": "hbm", "kernel": name, "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+             "kernel_ms": ms, "bytes_per_launch": int(nbytes), "kernel_share_of_step": ms / ms_per_step if ms_per_step else None,
+             "peak_source": hbm_source, "frac_of_8tbs": gbs / 8000.0, "traffic": NCU_TRAFFIC_BYTES.get((name, cfg)),
+             "traffic_source": "profiles/r02 ncu --set full capture (historical)" if (name, cfg) in NCU_TRAFFIC_BYTES else None}
+        d.update(extra or {})
+        return d
+
+    # the grid kernel executes FMAs on the records left after merging (exact by linearity): the fraction is claimed
+    # on the FMAs it EXECUTED; the nominal rate (16 flop per visibility-tap gridded) is beside it
+    merged = st.n_entries / st_exec.n_records_gridded if st_exec.n_records_gridded else None
+    kernels["grid_kernel"] = alu("grid_kernel", stage["grid"], exec_flop, {
+        "records_gridded": st_exec.n_records_gridded, "merge_factor": merged,
+        "nominal": {"tflops": nominal_flop / (stage["grid"] * 1e-3) / 1e12 if stage["grid"] > 0 else None,
+                    "flop_per_launch": nominal_flop,
+                    "note": "16 (32) flop per visibility-tap gridded; not a roofline statement once visibilities are pre-summed"}})
+    if stage.get("presum", 0.0) > 0:
+        # SURVEY 8(d) algorithmic bytes of the kernel that streams the visibilities: 32 B + 4 B weight each
+        ps_bytes = n * (32 + (4 if has_w else 0))
+        io_bytes = n * (32 + (4 if has_w else 0) + 1) + st.n_presum_records * 32
+        kernels["presum_kernel"] = hbm("presum_kernel", stage["presum"], ps_bytes, {
+            "partial_records": st.n_presum_records, "vis_per_record": n / st.n_presum_records if st.n_presum_records else None,
+            "frac_kernel_io": io_bytes / (stage["presum"] * 1e-3) / 1e9 / hbm_peak,
+            "kernel_io_bytes": int(io_bytes), "note": "frac: 32 B + 4 B per visibility (SURVEY 8(d)); frac_kernel_io adds the "
+                                                     "flag byte per visibility and the 32 B written per partial record"})
+    longest = max(kernels.values(), key=lambda k: k["kernel_ms"])
+    out = dict(longest)
+    out["kernels"] = kernels
+    out["step"] = {
+        "algorithmic_bytes": int(alg_bytes), "ms_per_step": ms_per_step,
+        "frac_of_hbm_peak": alg_bytes / (ms_per_step * 1e-3) / 1e9 / hbm_peak if ms_per_step else None,
+        "executed_flop": exec_flop, "frac_of_fma_peak": exec_flop / (ms_per_step * 1e-3) / 1e12 / fma_peak_tf if ms_per_step else None,
+        "nominal_flop": nominal_flop,
+        "nominal_frac_of_fma_peak": nominal_flop / (ms_per_step * 1e-3) / 1e12 / fma_peak_tf if ms_per_step else None,
+        "binding": "hbm" if alg_bytes / (hbm_peak * 1e9) > exec_flop / (fma_peak_tf * 1e12) else "alu",
+        "floor_ms": {"hbm": alg_bytes / (hbm_peak * 1e9) * 1e3, "fma_executed": exec_flop / (fma_peak_tf * 1e12) * 1e3,
+                     "fma_nominal": nominal_flop / (fma_peak_tf * 1e12) * 1e3},
+        "note": "after pre-summation the binding roofline of the step is the slower of HBM (inputs once) and the FMAs "
+                "actually executed; the nominal-FMA figure is kept for comparison with a gridder that may not merge"}
+    return out
+
+
 def run_ours(args) -> dict | None:
     import numpy as np
     import torch
@@ -257,61 +418,42 @@ def run_ours(args) -> dict | None:
 
     from paper_1003_5575_b200 import gridder
     gridder.load_library()                       # fails loudly if libgridder.so is missing
-    import synth
 
     shard = shard_plan(world, rank)
-    wl = synth.make_workload(args.config, band=shard["band"])
+    L = Loaded(args.config, dev, band=shard["band"])
+    wl, g = L.wl, L.g
     nt, nb, nf, n = wl.n_time, wl.n_baseline, wl.n_chan, wl.n_vis
-    vis = torch.empty((nt, nb, nf, 4, 2), dtype=torch.float32, device=dev)
-    weight = torch.empty((nt, nb, nf), dtype=torch.float32, device=dev) if wl.random_weights else None
-    for t in range(nt):
-        vis[t] = wl.vis_block(t, dev)
-        if weight is not None:
-            weight[t] = wl.weight_block(t, dev)
-    d_uvw = torch.from_numpy(wl.uvw).to(dev)
-    d_freq = torch.from_numpy(wl.freq).to(dev)
-    g = gridder.Gridder(grid_size=wl.grid_size, cell_size=wl.cell_size, oversample=wl.oversample,
-                        support=wl.support, kernel=torch.from_numpy(wl.kernel).to(dev), max_vis=n,
-                        n_wplanes=wl.n_wplanes, w_max=wl.w_max, kernel_is_complex=wl.kernel_is_complex)
-    grid = torch.empty((4, wl.grid_size, wl.grid_size, 2), dtype=torch.float32, device=dev)
-
     mfs_on = bool(args.mfs and world > 1)
     if mfs_on:
         from paper_1003_5575_b200 import mfs
 
     def step():
-        g.bin(d_uvw, d_freq)
-        g.grid(vis, weight, out=grid)
+        L.step()
         if mfs_on:
-            mfs.reduce_grids(grid)
+            mfs.reduce_grids(L.grid)
 
     def barrier():
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
 
-    for _ in range(max(args.warmup, 3)):
+    warmup = max(args.warmup, 3)
+    for _ in range(warmup):
         step()
     torch.cuda.synchronize()
     st = g.stats()
     g.set_profiling(True)
     launches0 = g.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     sampler = ClockSampler(local)
-    barrier()
     sampler.start()
-    e0.record()
-    for _ in range(args.steps):
-        step()
-    e1.record()
-    barrier()
+    per_step = timed_steps(step, args.steps, barrier)
     clocks = sampler.stop()
-    ms_rank = e0.elapsed_time(e1)
+    ms_rank = float(sum(per_step))
     stage = g.stage_ms()
     st_exec = g.stats()                   # records gridded / FMAs executed by the last gridder_grid
     launches = g.launch_count() - launches0 + (args.steps if mfs_on else 0)      # + gridder_sum_parts per step
     g.set_profiling(False)
-    checksum = float(grid[0, wl.grid_size // 2, wl.grid_size // 2, 0].item())
+    checksum = float(L.grid[0, wl.grid_size // 2, wl.grid_size // 2, 0].item())
 
     def gather(x: float):
         if world == 1:
@@ -323,158 +465,160 @@ def run_ours(args) -> dict | None:
 
     agg = aggregate(gather(ms_rank), gather(float(st.vis_taps)), args.steps)
 
-    # ---- end to end: pinned host buffers through gridder_run_host ---------------------------
+    # ---- end to end: pinned host buffers through gridder_run_host, the same number of steps --------------
     e2e = None
     if not args.no_e2e:
-        per_t = nb * nf * (32 + (4 if weight is not None else 0))
+        per_t = nb * nf * (32 + (4 if L.weight is not None else 0))
         nt_e = int(max(1, min(nt, _host_budget_bytes(world) // max(1, per_t))))
         h_vis = torch.empty((nt_e, nb, nf, 4, 2), dtype=torch.float32, pin_memory=True)
-        h_vis.copy_(vis[:nt_e])
+        h_vis.copy_(L.vis[:nt_e])
         h_w = None
-        if weight is not None:
+        if L.weight is not None:
             h_w = torch.empty((nt_e, nb, nf), dtype=torch.float32, pin_memory=True)
-            h_w.copy_(weight[:nt_e])
+            h_w.copy_(L.weight[:nt_e])
         h_uvw = torch.from_numpy(np.ascontiguousarray(wl.uvw[:nt_e])).pin_memory()
         h_freq = torch.from_numpy(wl.freq).pin_memory()
-        h_grid = torch.empty(grid.shape, dtype=torch.float32, pin_memory=True)
-        staging = {"uvw": d_uvw, "freq": d_freq, "vis": vis, "weight": weight, "grid": grid}
-        e_steps = max(1, min(args.steps, 3))
+        h_grid = torch.empty(L.grid.shape, dtype=torch.float32, pin_memory=True)
+        staging = {"uvw": L.uvw, "freq": L.freq, "vis": L.vis, "weight": L.weight, "grid": L.grid}
         g.run_host(h_uvw, h_freq, h_vis, h_w, h_grid, staging)            # warm-up
         taps_e = st.vis_taps * nt_e // nt        # (run_host grids in slices; the plan's stats are the last slice's)
-        barrier()
-        e0.record()
-        for _ in range(e_steps):
-            g.run_host(h_uvw, h_freq, h_vis, h_w, h_grid, staging)
-        e1.record()
-        barrier()
-        agg_e = aggregate(gather(e0.elapsed_time(e1)), gather(float(taps_e)), e_steps)
+        per_e = timed_steps(lambda: g.run_host(h_uvw, h_freq, h_vis, h_w, h_grid, staging), args.steps, barrier)
+        agg_e = aggregate(gather(float(sum(per_e))), gather(float(taps_e)), args.steps)
         h2d = h_vis.numel() * 4 + (h_w.numel() * 4 if h_w is not None else 0) + h_uvw.numel() * 8 + h_freq.numel() * 8
         e2e = {"value": agg_e["value"], "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(h_grid.numel() * 4), "ms_per_step": agg_e["ms_per_step"],
-               "steps": e_steps, "n_time": nt_e, "result_checksum": float(h_grid[0, wl.grid_size // 2, wl.grid_size // 2, 0])}
+               "ms_per_step_min": min(per_e), "ms_per_step_median": _median(per_e),
+               "steps": args.steps, "n_time": nt_e, "result_checksum": float(h_grid[0, wl.grid_size // 2, wl.grid_size // 2, 0])}
         del h_vis, h_w, h_grid
     f1 = None
     if args.atomic:
         # row f1: per-visibility FP32 atomic scatter, same inputs, one warm-up and one timed pass
-        g.scatter_atomic(d_uvw, d_freq, vis, weight, out=grid)
-        barrier()
-        e0.record()
-        g.scatter_atomic(d_uvw, d_freq, vis, weight, out=grid)
-        e1.record()
-        barrier()
-        ms_f1 = e0.elapsed_time(e1)
+        g.scatter_atomic(L.uvw, L.freq, L.vis, L.weight, out=L.grid)
+        ms_f1 = timed_steps(lambda: g.scatter_atomic(L.uvw, L.freq, L.vis, L.weight, out=L.grid), 1, barrier)[0]
         f1 = {"ms": ms_f1, "value": st.vis_taps / (ms_f1 * 1e-3), "unit": UNIT,
               "note": "gridder_scatter_atomic: no binning, red.global.add.v2.f32 per (tap, pol); not deterministic"}
-    g.destroy()
-    # the same kernel with merging off: every entry gridded on its own (what per-visibility GCFs would need)
+    # the same workload with merging and pre-summation off: every visibility gridded on its own (what per-visibility
+    # GCFs would need) -- the like-for-like FMA-bound number
     unmerged = None
     if world == 1 and not args.no_unmerged:
-        g.workspace = None                        # (the first plan's workspace goes back to the allocator)
+        L.close()
         torch.cuda.empty_cache()
-        g2 = gridder.Gridder(grid_size=wl.grid_size, cell_size=wl.cell_size, oversample=wl.oversample,
-                             support=wl.support, kernel=torch.from_numpy(wl.kernel).to(dev), max_vis=n,
-                             n_wplanes=wl.n_wplanes, w_max=wl.w_max, kernel_is_complex=wl.kernel_is_complex,
-                             tuning={"merge": 2})
-        g2.bin(d_uvw, d_freq)
-        g2.grid(vis, weight, out=grid)
+        L.g = L.plan({"merge": 2})
+        L.step()
         torch.cuda.synchronize()
-        g2.set_profiling(True)
-        for _ in range(2):
-            g2.grid(vis, weight, out=grid)
-        torch.cuda.synchronize()
-        st2, stage2 = g2.stats(), g2.stage_ms()
-        g2.destroy()
-        unmerged = {"grid_kernel_ms": stage2["grid"], "fma_executed": st2.fma_executed,
+        L.g.set_profiling(True)
+        ms_u = timed_steps(L.step, 2, barrier)
+        st2, stage2 = L.g.stats(), L.g.stage_ms()
+        unmerged = {"grid_kernel_ms": stage2["grid"], "fma_executed": st2.fma_executed, "ms_per_step": min(ms_u),
                     "records_gridded": st2.n_records_gridded}
+    L.close()
+    shapes = {"nt": nt, "nb": nb, "nf": nf, "n": n}
+    has_weight = L.weight is not None
+
+    # ---- compact legs on the other configs (after the timed region; development figures for the driver record) --
+    per_config = None
+    if world == 1 and not args.no_per_config and rank == 0:
+        del L
+        torch.cuda.empty_cache()
+        per_config = {}
+        for c in (0, 1, 2, 3):
+            if c == args.config:
+                continue
+            Lc = Loaded(c, dev)
+            for _ in range(3):
+                Lc.step()
+            torch.cuda.synchronize()
+            Lc.g.set_profiling(True)
+            reps = 20 if c < 2 else 10
+            ms_c = timed_steps(Lc.step, reps, barrier)
+            sc, stc = Lc.g.stage_ms(), Lc.g.stats()
+            per_config[f"config{c}"] = {"ms_per_step_min": min(ms_c), "ms_per_step_median": _median(ms_c), "steps": reps,
+                                        "vis_taps": stc.vis_taps, "stage_ms": sc, "fma_executed": stc.fma_executed,
+                                        "records_gridded": stc.n_records_gridded, "presum_records": stc.n_presum_records,
+                                        "complex_table": bool(Lc.wl.kernel_is_complex)}
+            Lc.close()
+            del Lc
+            torch.cuda.empty_cache()
     if world > 1:
         dist.destroy_process_group()
     if rank != 0:
         return None
 
-    # ---- roofline of the dominant kernel (the grid kernel) ----------------------------------
+    # ---- rooflines -------------------------------------------------------------------------
     peaks = measured_peaks()
     props = torch.cuda.get_device_properties(dev)
     sm_max_mhz = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
     fma_peak_tf = props.multi_processor_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
+    fma_source = (f"derived: {props.multi_processor_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x {sm_max_mhz:.0f} MHz "
+                  "(clocks.max.sm); DESIGN.md section 7")
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    hbm_source = "MEASURED_PEAKS.json hbm_gbs (copy bandwidth)" if "hbm_gbs" in peaks else "fallback (B200_PROFILING.md)"
     flop_per_tap = FLOP_PER_VIS_TAP * (2 if wl.kernel_is_complex else 1)
-    grid_ms = stage["grid"]
-    # The grid kernel sums entries with equal patch origin and table offset before gridding them
-    # (exact by linearity), so it executes fewer FMAs than 8 per visibility-tap.  The roofline
-    # fraction is claimed on the FMAs it EXECUTED (gridder_get_stats: records x padded patch cells x
-    # 8 or 16); the nominal rate (16 flop per visibility-tap gridded) is given beside it.
-    alg_bytes = n * (32 + (4 if weight is not None else 0)) + nt * nb * 24 + nf * 8 + 32 * wl.grid_size ** 2
-    exec_flop = 2.0 * st_exec.fma_executed
-    achieved_tf = exec_flop / (grid_ms * 1e-3) / 1e12 if grid_ms > 0 else 0.0
-    nominal_tf = flop_per_tap * st.vis_taps / (grid_ms * 1e-3) / 1e12 if grid_ms > 0 else 0.0
-    roofline = {
-        "bound": "alu", "kernel": "grid_kernel", "achieved": achieved_tf, "peak": fma_peak_tf, "unit": "TFLOP/s",
-        "frac": achieved_tf / fma_peak_tf if fma_peak_tf else None,
-        "traffic": NCU_GRID_KERNEL_TRAFFIC_BYTES.get(args.config),
-        "peak_source": f"derived: {props.multi_processor_count} SMs x {FP32_LANES_PER_SM} FP32 lanes x 2 flop x "
-                       f"{sm_max_mhz:.0f} MHz (clocks.max.sm); DESIGN.md section 7",
-        "kernel_ms": grid_ms, "kernel_share_of_step": grid_ms / agg["ms_per_step"] if agg["ms_per_step"] else None,
-        "flop_per_launch": exec_flop, "records_gridded": st_exec.n_records_gridded,
-        "merge_factor": st.n_entries / st_exec.n_records_gridded if st_exec.n_records_gridded else None,
-        "nominal": {"tflops": nominal_tf, "frac": nominal_tf / fma_peak_tf if fma_peak_tf else None,
-                    "flop_per_launch": flop_per_tap * st.vis_taps,
-                    "note": "16 (32) flop per visibility-tap gridded; above 1 is possible because of the merging"},
-        "frac_at_sampled_clock": (achieved_tf / (fma_peak_tf * clocks["sm_mhz"] / sm_max_mhz)
-                                  if clocks.get("sm_mhz") else None),
-        "hbm": {"algorithmic_bytes_per_step": int(alg_bytes),
-                "gbs_at_step_time": alg_bytes / (agg["ms_per_step"] * 1e-3) / 1e9 if agg["ms_per_step"] else None,
-                "peak_gbs": peaks.get("hbm_gbs", 6650.0),
-                "peak_source": "MEASURED_PEAKS.json" if "hbm_gbs" in peaks else "fallback (B200_PROFILING.md)"},
-    }
-    reduce_ms = stage.get("reduce", 0.0)
-    if reduce_ms > grid_ms:
-        # Dense plan: the pre-summation (reduce_kernel) is the longest kernel.  It streams every sorted
-        # (key, index) pair, gathers the visibility (and weight) it names, and writes the records:
-        # HBM-bound.  Algorithmic bytes per launch: 8 + 32 (+ 4) per entry, 36 per record.
-        red_bytes = st.n_entries * (8 + 32 + (4 if weight is not None else 0)) + st_exec.n_records_gridded * 36
-        gbs = red_bytes / (reduce_ms * 1e-3) / 1e9
-        hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
-        roofline = {
-            "bound": "hbm", "kernel": "reduce_kernel", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
-            "frac": gbs / hbm_peak, "traffic": NCU_REDUCE_KERNEL_TRAFFIC_BYTES.get(args.config),
-            "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy bandwidth)" if "hbm_gbs" in peaks
-                           else "fallback (B200_PROFILING.md)",
-            "kernel_ms": reduce_ms, "kernel_share_of_step": reduce_ms / agg["ms_per_step"] if agg["ms_per_step"] else None,
-            "bytes_per_launch": int(red_bytes), "entries": st.n_entries, "records": st_exec.n_records_gridded,
-            "merge_factor": roofline["merge_factor"],
-            "grid_kernel": roofline,              # the second kernel of the stage, on the records: FP32-FMA bound
-            "hbm": roofline["hbm"],
-        }
+
+    class _Shim:                      # (the Loaded object is gone: what kernel_rooflines needs of it)
+        pass
+    shim = _Shim()
+    shim.wl, shim.weight = wl, (True if has_weight else None)
+    roofline = kernel_rooflines(shim, stage, st, st_exec, agg["ms_per_step"], fma_peak_tf, hbm_peak, hbm_source, fma_source)
+    roofline["frac_at_sampled_clock"] = (roofline["frac"] * sm_max_mhz / clocks["sm_mhz"]
+                                         if roofline["bound"] == "alu" and clocks.get("sm_mhz") else None)
+    if per_config:
+        for name, pc in per_config.items():
+            fpt = FLOP_PER_VIS_TAP * (2 if pc["complex_table"] else 1)
+            t = pc["ms_per_step_min"] * 1e-3
+            pc["vis_taps_per_s"] = pc["vis_taps"] / t
+            pc["nominal_frac_of_fma_peak"] = fpt * pc["vis_taps"] / t / 1e12 / fma_peak_tf
+            pc["executed_frac_of_fma_peak_grid_kernel"] = (2.0 * pc["fma_executed"] / (pc["stage_ms"]["grid"] * 1e-3) / 1e12 / fma_peak_tf
+                                                          if pc["stage_ms"]["grid"] > 0 else None)
     out = {
         "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": agg["ms_per_step"], "higher_is_better": True,
+        "warmup": warmup, "ms_per_step": agg["ms_per_step"], "ms_per_step_min": min(per_step),
+        "ms_per_step_median": _median(per_step), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"config{wl.cfg}", "n_antennas": wl.n_ant, "n_baselines": nb, "n_chan": nf,
                    "n_time": nt, "n_vis_per_gpu": n, "grid": wl.grid_size, "support": max(wl.support),
-                   "oversample": wl.oversample, "n_wplanes": wl.n_wplanes, "weights": weight is not None,
+                   "oversample": wl.oversample, "n_wplanes": wl.n_wplanes, "weights": has_weight,
                    "parallelism": (f"channel-block x{world} + grid sum (all-to-all, FP64 fixed-order sum, all-gather)"
                                    if mfs_on else f"channel-block x{world} (no collective)"),
                    "l2": "inputs per step exceed the 126 MB L2" if n * 32 > (126 << 20) else "L2-resident inputs",
                    "tile": st.tile_size, "chunk": st.chunk_size, "work_items": st.n_work_items,
-                   "grid_warps_per_sm": st.grid_warps_per_sm},
-        "gflops": flop_per_tap * agg["value"] / 1e9,
-        "stage_ms": stage, "grid_only_ms": stage["grid"] + stage["flush"] + stage.get("reduce", 0.0) + stage.get("presum", 0.0),     # gridder_grid alone (a bin serves many)
+                   "grid_warps_per_sm": st.grid_warps_per_sm, "presum_records": st.n_presum_records},
+        "gflops_nominal": flop_per_tap * agg["value"] / 1e9,
+        "stage_ms": stage, "grid_only_ms": stage["grid"] + stage["flush"] + stage.get("presum", 0.0),   # gridder_grid alone (a bin serves many)
         "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
         "cadence_budget_s": 8.0, "result_checksum": checksum,
     }
     if unmerged is not None and unmerged["grid_kernel_ms"] > 0:
         tf = 2.0 * unmerged["fma_executed"] / (unmerged["grid_kernel_ms"] * 1e-3) / 1e12
         unmerged.update({"achieved": tf, "frac": tf / fma_peak_tf, "unit": "TFLOP/s",
-                         "note": "GRIDDER_MERGE=0: every entry gridded on its own, same kernel"})
+                         "step_frac_of_nominal_fma_roofline": (flop_per_tap * st.vis_taps / (fma_peak_tf * 1e12)) / (unmerged["ms_per_step"] * 1e-3),
+                         "note": "tuning merge = off: every visibility gridded on its own, same grid kernel"})
         out["roofline"]["without_merging"] = unmerged
     if f1 is not None:
         out["f1_atomic_scatter"] = f1
     if e2e is not None:
         out["e2e"] = e2e
+    if per_config is not None:
+        out["per_config"] = per_config
     if world == 1 and not args.no_cpu:
         import oracle
         oracle.build()
         out["cpu_baseline"] = cpu_baseline(args.config, args.cpu_seconds)
+        # one oracle thread on the small configs, for comparison with the paper's single Nehalem core
+        # (PAPER.md :216, Table 3: 13 285 ms for 12 channels ~ 68 M visibility-taps/s, derived in BASELINE.md)
+        one = {}
+        for c in (0, 1):
+            s1 = OracleSample(c, 1 if c == 1 else synth_shape(c)["n_time"], min(4, synth_shape(c)["n_chan"]))
+            s1.run(n_threads=1)
+            taps, dt, _ = s1.run(n_threads=1)
+            one[f"config{c}"] = {"value": taps / dt, "unit": UNIT, "cores": 1, "sample": s1.describe(), "seconds": dt}
+        out["cpu_baseline"]["one_thread"] = one
     return out
+
+
+def synth_shape(cfg: int) -> dict:
+    import synth
+    return synth.config_shape(cfg)
 
 
 def main():
@@ -483,6 +627,13 @@ def main():
         if int(os.environ.get("RANK", "0")) != 0:
             return
         print(json.dumps(run_reference(args)), flush=True)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(_self_spawn(args))
+    if args.spawn_check:
+        out = spawn_check(args)
+        if out is not None:
+            print(json.dumps(out), flush=True)
         return
     out = run_ours(args)
     if out is not None:

@@ -121,3 +121,19 @@ def test_slice_len_covers_and_is_float4_aligned():
         for world in (1, 2, 3, 8):
             L = mfs.slice_len(numel, world)
             assert L % 4 == 0 and world * L >= numel and world * (L - 4) < numel
+
+
+def test_bench_gpus_n_starts_its_own_ranks(repo_root):
+    """`python bench.py --gpus 2` with no launcher around it starts 2 ranks itself (torch.distributed.run on
+    127.0.0.1); the line rank 0 prints says n_gpus = 2 and every rank got its own band."""
+    import json
+    import subprocess
+    import sys
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, str(repo_root / "bench.py"), "--gpus", "2", "--spawn-check"], env=env,
+                         capture_output=True, text=True, timeout=300)
+    assert res.returncode == 0, res.stderr[-2000:]
+    line = [l for l in res.stdout.splitlines() if l.startswith("{")][-1]
+    out = json.loads(line)
+    assert out["n_gpus"] == out["requested_gpus"] == 2
+    assert out["f0_hz"] == [140.0e6, 140.0e6 + 768 * 40.0e3]
