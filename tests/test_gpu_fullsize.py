@@ -2,8 +2,12 @@
 bench.py times: default tile, chunk and warps).  The oracle cannot grid 4096^2 x 10^8..10^9 in test
 time, so it computes sampled windows of the grid one by one (oracle.grid_windows: the same direct
 scatter restricted to a window) -- hot centre, mid-radius, sparse outskirts, a strip crossing many
-tiles -- and every cell of every window must satisfy |delta| <= 1e-5 * sum|w V C| + 1e-6.  Counts
-(visibilities, dropped, vis*taps) are compared exactly and the rerun must be bit-identical."""
+tiles, the whole regions of the four hottest tiles (every chunk boundary of their work items falls inside),
+the patches of the outermost visibilities at the four grid edges, and 28 more drawn from a seed -- and every
+cell of every window must satisfy |delta| <= 1e-5 * sum|w V C| + 1e-6.  Nothing can hide outside the windows
+either: per polarisation the sum over ALL cells must equal sum_i w_i V_i * (table sum of visibility i's
+sub-cell offset), the oracle's mapping giving the offsets.  Counts (visibilities, dropped, vis*taps) are
+compared exactly and the rerun must be bit-identical."""
 import numpy as np
 import pytest
 import torch
@@ -15,7 +19,7 @@ from _util import as_complex, oracle_kwargs, RTOL_ABS, ATOL
 pytestmark = pytest.mark.gpu
 
 N = 4096
-WINDOWS = [                       # (y_lo, y_hi, x_lo, x_hi)
+FIXED_WINDOWS = [                 # (y_lo, y_hi, x_lo, x_hi)
     (2032, 2064, 2032, 2064),     # the hottest tiles (18 antennas within 1.5 m of the centre)
     (2060, 2084, 1990, 2014),     # core, off-centre
     (2000, 2008, 1800, 2296),     # a strip across 124 tiles through the core
@@ -38,11 +42,58 @@ def dev():
     return torch.device("cuda:0")
 
 
+def _clip(y0, y1, x0, x1):
+    return (max(0, int(y0)), min(N, int(y1)), max(0, int(x0)), min(N, int(x1)))
+
+
+def _windows(wl, m0):
+    """The fixed windows plus 36 chosen from the ORACLE's mapping of integration 0 (m0: [n][6] = x0, y0, qx, qy,
+    plane, dropped) and a seed: hottest tiles, grid edges, random visibilities, random places."""
+    wins = list(FIXED_WINDOWS)
+    x0, y0 = m0[:, 0].astype(np.int64), m0[:, 1].astype(np.int64)
+    S = max(wl.support)
+    tiles = np.bincount((y0 >> 3) * (N >> 3) + (x0 >> 3), minlength=(N >> 3) ** 2)
+    for t in np.argsort(tiles)[::-1][:4]:                    # the whole region (tile + halo) of the 4 hottest 8 x 8 tiles
+        ty, tx = divmod(int(t), N >> 3)
+        wins.append(_clip(ty * 8, ty * 8 + 8 + S, tx * 8, tx * 8 + 8 + S))
+    for k in (int(np.argmin(x0)), int(np.argmax(x0)), int(np.argmin(y0)), int(np.argmax(y0))):     # the grid edges
+        wins.append(_clip(y0[k] - 4, y0[k] + S + 4, x0[k] - 4, x0[k] + S + 4))
+    rng = np.random.default_rng(10035575 + 100 * wl.cfg)
+    for k in rng.integers(0, len(x0), 14):                   # where visibilities are
+        wins.append(_clip(y0[k], y0[k] + 16, x0[k], x0[k] + 16))
+    r = float(np.hypot(x0 - N / 2, y0 - N / 2).max())
+    for _ in range(14):                                      # anywhere inside the sampled disk
+        rr, th = r * np.sqrt(rng.random()), 2 * np.pi * rng.random()
+        cy, cx = N / 2 + rr * np.sin(th), N / 2 + rr * np.cos(th)
+        wins.append(_clip(cy - 8, cy + 8, cx - 8, cx + 8))
+    return [w for w in wins if w[1] > w[0] and w[3] > w[2]]
+
+
+def _table_sums(wl):
+    """Per w-plane: complex sums of the table over the taps of every sub-cell offset [qy][qx], and of |table|."""
+    O, E = wl.oversample, 2 if wl.kernel_is_complex else 1
+    sums, asums, off = [], [], 0
+    for S in wl.support:
+        t = wl.kernel[off:off + (S * O) ** 2 * E].astype(np.float64).reshape(S * O, S * O, E)
+        off += (S * O) ** 2 * E
+        c = t[..., 0] + (1j * t[..., 1] if E == 2 else 0.0)
+        sums.append(np.array([[c[qy::O, qx::O].sum() for qx in range(O)] for qy in range(O)]))
+        asums.append(np.array([[np.abs(c[qy::O, qx::O]).sum() for qx in range(O)] for qy in range(O)]))
+    return np.stack(sums), np.stack(asums)
+
+
 def _run_full(dev, cfg):
     """Grid config `cfg` at full size on the GPU; the oracle's windows are fed one integration at a time."""
     from paper_1003_5575_b200 import gridder
     wl = synth.make_workload(cfg)
     nt, nb, nf = wl.n_time, wl.n_baseline, wl.n_chan
+    csum, casum = _table_sums(wl)
+    d_csum = torch.from_numpy(csum.astype(np.complex128)).to(dev).reshape(-1)
+    d_casum = torch.from_numpy(casum).to(dev).reshape(-1)
+    O = wl.oversample
+    want = torch.zeros(4, dtype=torch.complex128, device=dev)      # sum over all cells, per polarisation
+    want_abs = torch.zeros(4, dtype=torch.float64, device=dev)
+    WINDOWS = None
     vis = torch.empty((nt, nb, nf, 4, 2), dtype=torch.float32, device=dev)
     weight = torch.empty((nt, nb, nf), dtype=torch.float32, device=dev) if wl.random_weights else None
     res = None
@@ -53,8 +104,23 @@ def _run_full(dev, cfg):
             weight[t] = wl.weight_block(t, dev)
         h_vis = vis[t].cpu().numpy()
         h_w = None if weight is None else weight[t].cpu().numpy()
+        m = oracle.map_visibilities(wl.uvw[t:t + 1], wl.freq, **kw)          # the ORACLE's mapping
+        if WINDOWS is None:
+            WINDOWS = _windows(wl, m[m[:, 5] == 0])
         res = oracle.grid_windows(wl.uvw[t:t + 1], wl.freq, h_vis, h_w, WINDOWS, out=res, **kw)
-        del h_vis, h_w
+        # expected total of the grid: sum_i w_i V_i * (table sum of (plane, qy, qx) of visibility i, conjugated for w < 0)
+        plane, conj = m[:, 4] & 255, (m[:, 4] >> 8) & 1
+        q = torch.from_numpy(((plane * O + m[:, 3]) * O + m[:, 2]).astype(np.int64)).to(dev)
+        cs = d_csum[q]
+        cs = torch.where(torch.from_numpy(conj.astype(bool)).to(dev), cs.conj(), cs)
+        live = torch.from_numpy((m[:, 5] == 0)).to(dev)
+        wv = torch.view_as_complex(vis[t].reshape(-1, 4, 2).double())
+        if weight is not None:
+            wv = wv * weight[t].reshape(-1, 1).double()
+        wv = torch.where(live[:, None], wv, torch.zeros_like(wv))
+        want += (wv * cs[:, None]).sum(0)
+        want_abs += (wv.abs() * d_casum[q][:, None]).sum(0)
+        del h_vis, h_w, m, q, cs, wv, live
     g = gridder.Gridder(grid_size=wl.grid_size, cell_size=wl.cell_size, oversample=wl.oversample, support=wl.support,
                         kernel=torch.from_numpy(wl.kernel).to(dev), max_vis=wl.n_vis, n_wplanes=wl.n_wplanes,
                         w_max=wl.w_max, kernel_is_complex=wl.kernel_is_complex)
@@ -62,18 +128,20 @@ def _run_full(dev, cfg):
     grid = g.grid(vis, weight)
     st = g.stats()
     first = [grid[:, y0:y1, x0:x1].cpu().numpy() for (y0, y1, x0, x1) in WINDOWS]
+    total = torch.view_as_complex(grid.double()).sum(dim=(1, 2))          # per polarisation, FP64
+    sums = (total.cpu().numpy(), want.cpu().numpy(), want_abs.cpu().numpy())
     checksum = grid.view(torch.int32).sum(dtype=torch.int64).item()
     grid2 = g.grid(vis, weight)
     same = bool(torch.equal(grid, grid2)) and grid2.view(torch.int32).sum(dtype=torch.int64).item() == checksum
     g.destroy()
     del vis, weight, grid, grid2
     torch.cuda.empty_cache()
-    return wl, st, first, res, same
+    return wl, st, first, res, same, WINDOWS, sums
 
 
 @pytest.mark.parametrize("cfg", [2, 3, 4])
 def test_full_size_sampled_windows(dev, cfg):
-    wl, st, got, res, same = _run_full(dev, cfg)
+    wl, st, got, res, same, WINDOWS, (total, want, want_abs) = _run_full(dev, cfg)
     assert same, "rerun at full size is not bit-identical"
     assert st.n_vis == wl.n_vis and st.n_dropped == res["n_dropped"] == 0
     assert st.vis_taps == res["vis_taps"]
@@ -90,5 +158,12 @@ def test_full_size_sampled_windows(dev, cfg):
         worst = max(worst, float((err / tol).max()))
         busiest = max(busiest, float(ab.max()))
     assert busiest > 1e3, "the sampled windows must include heavily loaded cells"
+    assert len(WINDOWS) >= 40
+    # the whole grid.  The per-cell tolerances add up to 1e-5 sum|w V C|; cell errors are rounding errors of either
+    # sign, so the sums agree far better (measured 2e-10), and the bar is set where ONE lost or doubled visibility
+    # of typical size (|w V| sum|C| ~ 1e-9 of the total for config 4, more for the others) already fails
+    gap = np.abs(total - want) / (2e-9 * want_abs + 1e-3)
+    assert (gap <= 1.0).all(), f"config {cfg}: sum over all cells off by {gap} x (2e-9 sum|w V C|) per polarisation"
+    print(f"config {cfg}: whole-grid sums within {gap.max():.3g} x 2e-9 sum|w V C|")
     print(f"config {cfg}: worst err/tol {worst:.3f} over {len(WINDOWS)} windows, busiest cell sum|wVC| {busiest:.3g}, "
           f"{st.n_work_items} work items, max tile load {st.max_tile_load}")
