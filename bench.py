@@ -539,6 +539,46 @@ def run_ours(args) -> dict | None:
             Lc.close()
             del Lc
             torch.cuda.empty_cache()
+    # ---- row f4: the paper's deployment shape, 12 consecutive channels of a GPU, one grid each (PAPER.md :108-120)
+    f4 = None
+    if world == 1 and not args.no_per_config:
+        import synth
+        wl12 = synth.make_workload(4, n_chan=12)
+        v12 = torch.stack([wl12.vis_block(t, dev) for t in range(wl12.n_time)])
+        w12 = torch.stack([wl12.weight_block(t, dev) for t in range(wl12.n_time)])
+        u12, f12 = torch.from_numpy(wl12.uvw).to(dev), torch.from_numpy(wl12.freq).to(dev)
+        tab = torch.from_numpy(wl12.kernel).to(dev)
+        kw12 = dict(grid_size=wl12.grid_size, cell_size=wl12.cell_size, oversample=wl12.oversample, support=wl12.support, kernel=tab)
+        gb = gridder.Gridder(max_vis=wl12.n_vis, max_grids=12, **kw12)
+        grids = torch.empty((12, 4, wl12.grid_size, wl12.grid_size, 2), dtype=torch.float32, device=dev)
+
+        def batched():
+            gb.bin(u12, f12, chans_per_grid=1)
+            gb.grid(v12, w12, out=grids)
+        for _ in range(3):
+            batched()
+        ms_b = timed_steps(batched, 10, barrier)
+        taps12 = gb.stats().vis_taps
+        gb.destroy()
+        g1 = gridder.Gridder(max_vis=wl12.n_vis // 12, **kw12)
+        vc = [v12[:, :, c:c + 1].contiguous() for c in range(12)]
+        wc = [w12[:, :, c:c + 1].contiguous() for c in range(12)]
+
+        def one_by_one():
+            for c in range(12):
+                g1.bin(u12, f12[c:c + 1])
+                g1.grid(vc[c], wc[c], out=grids[c])
+        for _ in range(2):
+            one_by_one()
+        ms_1 = timed_steps(one_by_one, 5, barrier)
+        g1.destroy()
+        f4 = {"workload": "config 4 geometry, first 12 channels, 8 integrations, one 4096^2 grid per channel",
+              "n_vis": wl12.n_vis, "n_grids": 12, "batched_ms_min": min(ms_b), "batched_ms_median": _median(ms_b),
+              "twelve_bin_grid_rounds_ms_min": min(ms_1), "vis_taps_per_s": taps12 / (min(ms_b) * 1e-3),
+              "note": "gridder_bin_channels + gridder_grid_channels: one map, one sort, one set of kernel launches for the "
+                      "12 grids, against 12 gridder_bin + gridder_grid rounds on per-channel copies"}
+        del v12, w12, grids, vc, wc
+        torch.cuda.empty_cache()
     if world > 1:
         dist.destroy_process_group()
     if rank != 0:
@@ -600,6 +640,8 @@ def run_ours(args) -> dict | None:
         out["e2e"] = e2e
     if per_config is not None:
         out["per_config"] = per_config
+    if f4 is not None:
+        out["f4_channel_grids"] = f4
     if world == 1 and not args.no_cpu:
         import oracle
         oracle.build()

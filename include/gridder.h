@@ -84,6 +84,8 @@ typedef struct {
     int64_t max_vis;            /* capacity: upper bound of n_time * n_baseline * n_chan            */
     void *workspace;            /* DEVICE scratch, 256-byte aligned, owned by the caller            */
     size_t workspace_bytes;
+    int32_t max_grids;          /* most output grids of gridder_bin_channels / gridder_grid_channels (one
+                                   grid per block of channels, PAPER.md :108-120); 0 or 1: one grid      */
 } gridder_config;
 
 /* Optional tuning (gridder_plan_tuned).  Every field: 0 = the library's default, so a zeroed struct is
@@ -164,6 +166,19 @@ GRIDDER_API int gridder_bin_tables(gridder_plan_t *plan, const double *uvw_m, in
  * otherwise the result is added to `grid`.  Asynchronous on `cuda_stream`. */
 GRIDDER_API int gridder_grid(gridder_plan_t *plan, const float *vis, const float *weight, float *grid,
                  int32_t accumulate, void *cuda_stream);
+
+/* SURVEY 8(f) row f4, second half -- the paper's own deployment (PAPER.md :108-120, section 3.1): a GPU holds 12
+ * consecutive channels and makes one image per channel.  gridder_bin_channels maps, sorts and tabulates all
+ * n_chan channels ONCE, filing channel f under grid f / chans_per_grid (the grid index becomes part of the
+ * uv-tile id, so one sort and one set of work items serve every grid); gridder_grid_channels then grids them in
+ * the same kernel launches and flushes grid g to grids + g * 8 N^2 floats (DEVICE, [n_grids][4][N][N][2]),
+ * n_grids = ceil(n_chan / chans_per_grid) <= cfg.max_grids (else GRIDDER_ERR_CAPACITY).  Grid g is, bit for bit
+ * up to FP32 summation order, what gridder_bin + gridder_grid give on channels [g, g + 1) * chans_per_grid alone.
+ * After gridder_bin_channels with more than one grid, plain gridder_grid is GRIDDER_ERR_INVALID_ARG. */
+GRIDDER_API int gridder_bin_channels(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
+                                     const double *freq_hz, int32_t n_chan, int32_t chans_per_grid, void *cuda_stream);
+GRIDDER_API int gridder_grid_channels(gridder_plan_t *plan, const float *vis, const float *weight, float *grids,
+                                      int32_t accumulate, void *cuda_stream);
 
 GRIDDER_API int gridder_destroy(gridder_plan_t *plan);
 

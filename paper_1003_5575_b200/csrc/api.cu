@@ -64,9 +64,14 @@ int derive(const gridder_config *cfg, const gridder_tuning *tuning, Plan &p) {
     p.ntx = (cfg->grid_size + p.T - 1) / p.T;
     p.nty = p.ntx;
     p.n_tiles = p.ntx * p.nty;
+    if (cfg->max_grids < 0 || cfg->max_grids > 4096) return GRIDDER_ERR_INVALID_ARG;
+    p.max_grids = cfg->max_grids > 1 ? cfg->max_grids : 1;
+    if ((int64_t)p.n_tiles * p.max_grids > (1ll << 30)) return GRIDDER_ERR_UNSUPPORTED;
+    p.n_tiles_cls = p.n_tiles * p.max_grids;
+    p.n_grids = 1;
     // the fast path keeps the sub-cell offsets in the 32-bit sort key; a grid too large for that
     // (2 log2 N + 2 log2 O + 1 > 32 bits) goes through the general path, whose values carry them
-    if (p.mode == 0 && 2 * q_bits + 1 + 2 * p.tlog + ceil_log2((unsigned long long)p.n_tiles) > 32) {
+    if (p.mode == 0 && 2 * q_bits + 1 + 2 * p.tlog + ceil_log2((unsigned long long)p.n_tiles_cls) > 32) {
         p.mode = 1;
         p.presum = 0;
     }
@@ -137,7 +142,7 @@ int derive(const gridder_config *cfg, const gridder_tuning *tuning, Plan &p) {
     k.aux_bits = p.mode == 0 ? 2 * k.bits_q + 1 : 0;
     k.plane_shift = k.aux_bits + 2 * k.tlog;
     k.plane_bits = cfg->n_wplanes > 1 ? ceil_log2((unsigned long long)cfg->n_wplanes) : 0;
-    k.tile_bits = ceil_log2((unsigned long long)p.n_tiles * p.n_cls);
+    k.tile_bits = ceil_log2((unsigned long long)p.n_tiles_cls * p.n_cls);
     if (k.tile_bits < 1) k.tile_bits = 1;
     // sorting on the plane inside a tile only helps table locality: dropped when the key is full
     if (k.plane_shift + k.plane_bits + k.tile_bits > 32) k.plane_bits = 0;
@@ -147,11 +152,11 @@ int derive(const gridder_config *cfg, const gridder_tuning *tuning, Plan &p) {
     p.key = k;
 
     const int64_t n = cfg->max_vis;
-    const int64_t n_vtiles = (int64_t)p.n_tiles * p.n_cls;
+    const int64_t n_vtiles = (int64_t)p.n_tiles_cls * p.n_cls;
     int64_t occ = n < n_vtiles ? n : n_vtiles;
     p.max_items = occ + n / p.chunk + 1;
     // each class has its own partial-region array, sized for the case that every entry is of that class
-    p.max_items_cls = (n < p.n_tiles ? n : p.n_tiles) + n / p.chunk + 1;
+    p.max_items_cls = (n < p.n_tiles_cls ? n : p.n_tiles_cls) + n / p.chunk + 1;
     if (p.presum) {
         // The sums of a group's partial records live in the group's own visibility slots (presum.cu slot_index), so
         // they need an array as large as the visibilities.  Inputs that merge into more than 3/4 n records take the per-visibility path (decided
@@ -173,7 +178,7 @@ cudaError_t carve(Plan &p, char *base) {
     size_t off = 0;
     auto take = [&](size_t bytes) { char *ptr = base ? base + off : nullptr; off += align_up(bytes); return ptr; };
     const size_t n = (size_t)(p.cfg.max_vis > 0 ? p.cfg.max_vis : 1);
-    const size_t n_vtiles = (size_t)p.n_tiles * p.n_cls;
+    const size_t n_vtiles = (size_t)p.n_tiles_cls * p.n_cls;
     const size_t val_bytes = p.mode == 0 ? sizeof(uint32_t) : sizeof(unsigned long long);
     // (keys[1] and vals[1] next to each other: together they are the staging area of the pre-summed plans)
     p.keys[0] = (uint32_t *)take(n * sizeof(uint32_t));
@@ -278,15 +283,33 @@ int gridder_bin(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32
     return gridder_bin_tables(plan, uvw_m, n_time, n_baseline, freq_hz, n_chan, nullptr, cuda_stream);
 }
 
+static int bin_common(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline, const double *freq_hz,
+                      int32_t n_chan, const int32_t *table_index, int32_t chans_per_grid, void *cuda_stream);
+
 int gridder_bin_tables(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
                        const double *freq_hz, int32_t n_chan, const int32_t *table_index, void *cuda_stream) {
+    return bin_common(plan, uvw_m, n_time, n_baseline, freq_hz, n_chan, table_index, 0, cuda_stream);
+}
+
+int gridder_bin_channels(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline,
+                         const double *freq_hz, int32_t n_chan, int32_t chans_per_grid, void *cuda_stream) {
+    if (chans_per_grid < 1) return GRIDDER_ERR_INVALID_ARG;
+    return bin_common(plan, uvw_m, n_time, n_baseline, freq_hz, n_chan, nullptr, chans_per_grid, cuda_stream);
+}
+
+static int bin_common(gridder_plan_t *plan, const double *uvw_m, int32_t n_time, int32_t n_baseline, const double *freq_hz,
+                      int32_t n_chan, const int32_t *table_index, int32_t chans_per_grid, void *cuda_stream) {
     Plan *p = reinterpret_cast<Plan *>(plan);
     if (!p || n_time < 0 || n_baseline < 0 || n_chan < 0) return GRIDDER_ERR_INVALID_ARG;
+    const int32_t n_grids = chans_per_grid > 0 && n_chan > 0 ? (n_chan + chans_per_grid - 1) / chans_per_grid : 1;
+    if (n_grids > p->max_grids) return GRIDDER_ERR_CAPACITY;
     const int64_t n = (int64_t)n_time * n_baseline * n_chan;
     if (n > 0 && (!uvw_m || !freq_hz)) return GRIDDER_ERR_INVALID_ARG;
     if (n > p->cfg.max_vis) return GRIDDER_ERR_CAPACITY;
     if (n_chan > kMaxChannels) return GRIDDER_ERR_UNSUPPORTED;
     p->binned = false;
+    p->n_grids = n_grids;
+    p->chans_per_grid = chans_per_grid;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     cudaError_t e = launch_bin(*p, uvw_m, n_time, n_baseline, freq_hz, n_chan, table_index, s);
     if (e != cudaSuccess) return cuda_fail(p, e);
@@ -298,6 +321,13 @@ int gridder_bin_tables(gridder_plan_t *plan, const double *uvw_m, int32_t n_time
 
 int gridder_grid(gridder_plan_t *plan, const float *vis, const float *weight, float *grid,
                  int32_t accumulate, void *cuda_stream) {
+    Plan *p = reinterpret_cast<Plan *>(plan);
+    if (p && p->binned && p->n_grids > 1) return GRIDDER_ERR_INVALID_ARG;       // binned for several grids
+    return gridder_grid_channels(plan, vis, weight, grid, accumulate, cuda_stream);
+}
+
+int gridder_grid_channels(gridder_plan_t *plan, const float *vis, const float *weight, float *grid,
+                          int32_t accumulate, void *cuda_stream) {
     Plan *p = reinterpret_cast<Plan *>(plan);
     if (!p || !grid) return GRIDDER_ERR_INVALID_ARG;
     if (!p->binned) return GRIDDER_ERR_NOT_BINNED;

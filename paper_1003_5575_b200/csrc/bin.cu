@@ -89,7 +89,8 @@ __global__ void __launch_bounds__(256) map_kernel(const double *__restrict__ uvw
             taps_here += (unsigned long long)(m.S * m.S);
             const uint32_t x0 = (uint32_t)m.x0, y0 = (uint32_t)m.y0;
             const uint32_t tile = (y0 >> p.key.tlog) * (uint32_t)p.ntx + (x0 >> p.key.tlog);
-            const uint32_t vtile = (uint32_t)(p.cls_slot[m.plane] * p.n_tiles) + tile;
+            const uint32_t gtile = p.chans_per_grid ? (f / (uint32_t)p.chans_per_grid) * (uint32_t)p.grid_tiles : 0u;
+            const uint32_t vtile = (uint32_t)(p.cls_slot[m.plane] * p.n_tiles) + gtile + tile;
             key = (vtile << p.key.tile_shift) | ((y0 & tmask) << (p.key.aux_bits + p.key.tlog)) |
                   ((x0 & tmask) << p.key.aux_bits);
             if (p.key.plane_bits) key |= (uint32_t)m.plane << p.key.plane_shift;
@@ -138,7 +139,9 @@ MapParams make_map_params(const Plan &p) {
     mp.n_grid = p.cfg.grid_size;
     mp.oversample = p.cfg.oversample;
     mp.ntx = p.ntx;
-    mp.n_tiles = p.n_tiles;
+    mp.n_tiles = p.n_tiles_cls;
+    mp.grid_tiles = p.n_tiles;
+    mp.chans_per_grid = p.n_grids > 1 ? p.chans_per_grid : 0;
     mp.n_planes = p.cfg.n_wplanes;
     mp.general = p.mode != 0;
     mp.is_complex = p.cfg.kernel_is_complex ? 1 : 0;
@@ -287,7 +290,7 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
                        const int32_t *table_index, cudaStream_t s) {
     const long long n_tb = (long long)n_time * n_bl;
     const long long n = n_tb * n_chan;
-    const int n_vtiles = p.n_tiles * p.n_cls;
+    const int n_vtiles = p.n_tiles_cls * p.n_cls;
     GR_TRY(cudaMemsetAsync(p.counters, 0, sizeof(Counters), s));
     // tile_start and tile_end are adjacent: [2][n_vtiles]
     GR_TRY(cudaMemsetAsync(p.tile_start, 0, sizeof(uint32_t) * 2 * (size_t)n_vtiles, s));
@@ -368,7 +371,7 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
     size_t tb = p.cub_temp_bytes;
     GR_TRY(cub::DeviceScan::ExclusiveSum(p.cub_temp, tb, (const unsigned long long *)p.tile_chunks,
                                          p.tile_chunks_scan, (long long)nt1, s));
-    item_fill_kernel<<<(nt1 + 255) / 256, 256, 0, s>>>(p.tile_start, tile_end, p.tile_chunks_scan, p.n_tiles,
+    item_fill_kernel<<<(nt1 + 255) / 256, 256, 0, s>>>(p.tile_start, tile_end, p.tile_chunks_scan, p.n_tiles_cls,
                                                          p.n_cls, p.chunk, p.tile_info, p.items, p.counters);
     GR_TRY(cudaGetLastError());
     p.n_launches += 3;

@@ -807,35 +807,38 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         p.n_launches += 1;
     }
     stage_mark(p, 5, s);
+    const size_t grid_floats = (size_t)8 * p.cfg.grid_size * p.cfg.grid_size;
     for (int c = 0; c < p.n_cls; ++c) {
         const ClassGeo &g = p.cls[c];
         flush_fn_t ffn = pick_flush(g, p.tlog);
         if (!ffn) return cudaErrorInvalidConfiguration;
-        FlushParams fp;
-        fp.tiles = p.tile_info + (size_t)c * p.n_tiles;
-        fp.partials = p.partials + g.part_off_f4;
-        fp.counters = p.counters;
-        fp.cls = c;
-        fp.grid = reinterpret_cast<float2 *>(grid);
-        fp.n_grid = p.cfg.grid_size;
-        fp.ntx = p.ntx;
-        fp.nty = p.nty;
-        fp.accumulate = (c > 0 || accumulate) ? 1 : 0;
-        fp.cover = nullptr;
-        if (c > 0) {
-            // a later class only adds: cells no region of the class can reach are skipped (sparse classes)
-            const int reach = (g.RW - 1 + (g.nsub - 1) * 8 * g.NA + p.T - 1) / p.T;
-            tile_cover_kernel<<<(p.n_tiles + 255) / 256, 256, 0, s>>>(fp.tiles, p.ntx, p.nty, reach, p.tile_cover);
+        for (int gi = 0; gi < p.n_grids; ++gi) {         // (one grid, or one per channel block: gridder_bin_channels)
+            FlushParams fp;
+            fp.tiles = p.tile_info + (size_t)c * p.n_tiles_cls + (size_t)gi * p.n_tiles;
+            fp.partials = p.partials + g.part_off_f4;
+            fp.counters = p.counters;
+            fp.cls = c;
+            fp.grid = reinterpret_cast<float2 *>(grid + gi * grid_floats);
+            fp.n_grid = p.cfg.grid_size;
+            fp.ntx = p.ntx;
+            fp.nty = p.nty;
+            fp.accumulate = (c > 0 || accumulate) ? 1 : 0;
+            fp.cover = nullptr;
+            if (c > 0) {
+                // a later class only adds: cells no region of the class can reach are skipped (sparse classes)
+                const int reach = (g.RW - 1 + (g.nsub - 1) * 8 * g.NA + p.T - 1) / p.T;
+                tile_cover_kernel<<<(p.n_tiles + 255) / 256, 256, 0, s>>>(fp.tiles, p.ntx, p.nty, reach, p.tile_cover);
+                e = cudaGetLastError();
+                if (e != cudaSuccess) return e;
+                fp.cover = p.tile_cover;
+                p.n_launches += 1;
+            }
+            dim3 blk(32, 8), grd((p.cfg.grid_size + 31) / 32, (p.cfg.grid_size + 7) / 8);
+            ffn<<<grd, blk, 0, s>>>(fp);
             e = cudaGetLastError();
             if (e != cudaSuccess) return e;
-            fp.cover = p.tile_cover;
             p.n_launches += 1;
         }
-        dim3 blk(32, 8), grd((p.cfg.grid_size + 31) / 32, (p.cfg.grid_size + 7) / 8);
-        ffn<<<grd, blk, 0, s>>>(fp);
-        e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
-        p.n_launches += 1;
     }
     stage_mark(p, 6, s);
     if (p.profiling) p.prof_grid_calls++;

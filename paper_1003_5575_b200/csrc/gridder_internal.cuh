@@ -56,7 +56,9 @@ struct MapParams {
     int32_t n_grid;          // N
     int32_t oversample;      // O
     int32_t ntx;             // tiles per grid row
-    int32_t n_tiles;
+    int32_t n_tiles;         // tile ids per patch class: tiles of one grid x grids of the plan
+    int32_t grid_tiles;      // tiles of one grid
+    int32_t chans_per_grid;  // channels filed under one grid (gridder_bin_channels); 0: one grid
     int32_t n_planes;
     int32_t general;         // 0: fast path key/value format
     int32_t is_complex;
@@ -147,6 +149,9 @@ struct Plan {
     int32_t plane_slot[kMaxPlanes];
     uint32_t plane_off256[kMaxPlanes];
     int32_t tlog, T, ntx, nty, n_tiles;
+    int32_t max_grids;             // output grids the tile tables have room for (cfg.max_grids, at least 1)
+    int32_t n_tiles_cls;           // n_tiles * max_grids: tile ids per patch class
+    int32_t n_grids, chans_per_grid;      // of the last bin (1, 0: plain gridder_bin)
     int32_t chunk;                 // K
     int32_t merge;                 // tuning.merge (default on)
     // pre-summation in input order (presum.cu); presum == 0: not used by this plan
@@ -242,7 +247,7 @@ cudaError_t launch_scatter_atomic(Plan &p, const double *uvw, int n_time, int n_
 // grid.cu
 cudaError_t configure_grid_kernel(Plan &p);          // picks warps/smem per class, sets the smem attribute
 cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *grid, int accumulate,
-                        cudaStream_t s);
+                        cudaStream_t s);      // grid: [p.n_grids][4][N][N][2]
 size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps);
 
 }  // namespace gridder

@@ -115,68 +115,17 @@ __device__ __forceinline__ VisMap map_vis(double u_m, double v_m, double w_m, do
 
 // Fast-path sort key of a mapped visibility (KeyLayout): tile, origin inside the
 // tile, and -- not sorted on -- drop flag and sub-cell offsets.
-__device__ __forceinline__ uint32_t fast_key(const VisMap &m, const MapParams &p) {
+// `gtile`: first tile id of the visibility's grid (gridder_bin_channels; 0 for one grid).
+__device__ __forceinline__ uint32_t fast_key(const VisMap &m, const MapParams &p, uint32_t gtile = 0) {
     if (m.dropped)      // filed under tile 0, origin (0, 0)
         return ((uint32_t)(p.drop_slot * p.n_tiles) << p.key.tile_shift) | (1u << (2 * p.key.bits_q));
     const uint32_t tmask = (1u << p.key.tlog) - 1u;
     const uint32_t x0 = (uint32_t)m.x0, y0 = (uint32_t)m.y0;
     const uint32_t tile = (y0 >> p.key.tlog) * (uint32_t)p.ntx + (x0 >> p.key.tlog);
-    const uint32_t vtile = (uint32_t)(p.cls_slot[m.plane] * p.n_tiles) + tile;
+    const uint32_t vtile = (uint32_t)(p.cls_slot[m.plane] * p.n_tiles) + gtile + tile;
     return (vtile << p.key.tile_shift) | ((y0 & tmask) << (p.key.aux_bits + p.key.tlog)) |
            ((x0 & tmask) << p.key.aux_bits) | ((uint32_t)m.qy << p.key.bits_q) | (uint32_t)m.qx;
 }
-
-// The fast path's mapper with its constants in registers (one real table, power-of-two oversampling).
-// Bit for bit the result of map_vis + fast_key: it accepts a position only under a STRICTER screening
-// margin than map_axis (2^-48 * 2 N O >= 2^-48 (|h| + N O) for |h| < N O), where map_axis takes the same
-// multiply-by-reciprocal value and the same 32-bit algebra; everything else goes to map_vis itself.
-struct FastMap {
-    double rcp_cell, half_n, d_o, eps, one_minus_eps, span;
-    int o_shift, o_minus_1, half_so, n_minus_s, s2;
-    uint32_t ntx, tmask, tlog, aux_bits, bits_q, tile_shift;
-
-    __device__ __forceinline__ void init(const MapParams &p) {
-        rcp_cell = p.rcp_cell; half_n = (double)(p.n_grid / 2); d_o = (double)p.oversample; span = p.span;
-        eps = p.span * 7.1054273576010019e-15;                 // 2^-48 * 2 N O
-        one_minus_eps = 1.0 - eps;
-        o_shift = p.o_shift; o_minus_1 = p.oversample - 1;
-        half_so = (p.support[0] * p.oversample) >> 1;
-        n_minus_s = p.n_grid - p.support[0];
-        s2 = p.support[0] * p.support[0];
-        ntx = (uint32_t)p.ntx; tlog = (uint32_t)p.key.tlog; tmask = (1u << p.key.tlog) - 1u;
-        aux_bits = (uint32_t)p.key.aux_bits; bits_q = (uint32_t)p.key.bits_q; tile_shift = (uint32_t)p.key.tile_shift;
-    }
-    __device__ __forceinline__ bool axis(double coord_lambda, int &x0, int &q) const {
-        const double h1 = __dmul_rn(__dadd_rn(__dmul_rn(coord_lambda, rcp_cell), half_n), d_o);
-        const double t1 = __dadd_rn(h1, 0.5);
-        const double r = floor(t1);
-        const double fr = t1 - r;
-        if (!(fabs(h1) < span && fr > eps && fr < one_minus_eps)) return false;
-        const int a = (int)r - half_so;
-        x0 = (a + o_minus_1) >> o_shift;                        // ceil(a / O), arithmetic shift = floor division
-        q = (x0 << o_shift) - a;
-        return true;
-    }
-    // sort key of the visibility (fast_key's layout); `taps` gets S^2 or 0 (dropped)
-    __device__ __forceinline__ uint32_t key(double u_m, double v_m, double s, const MapParams &p, int &taps) const {
-        int x0, y0, qx, qy;
-        const bool okx = axis(__dmul_rn(u_m, s), x0, qx), oky = axis(__dmul_rn(v_m, s), y0, qy);
-        if (okx && oky) {
-            if ((unsigned)x0 > (unsigned)n_minus_s || (unsigned)y0 > (unsigned)n_minus_s) {     // off the grid
-                taps = 0;
-                return 1u << (2 * bits_q);                      // drop slot 0, tile 0, origin (0, 0)
-            }
-            taps = s2;
-            const uint32_t ux = (uint32_t)x0, uy = (uint32_t)y0;
-            const uint32_t tile = (uy >> tlog) * ntx + (ux >> tlog);
-            return (tile << tile_shift) | ((uy & tmask) << (aux_bits + tlog)) | ((ux & tmask) << aux_bits) |
-                   ((uint32_t)qy << bits_q) | (uint32_t)qx;
-        }
-        const VisMap m = map_vis(u_m, v_m, 0.0, s, p);          // rare: near a rounding boundary, or far away
-        taps = m.dropped ? 0 : m.S * m.S;
-        return fast_key(m, p);
-    }
-};
 
 // The production mapper of the pre-summed path: ONE fused multiply-add per axis.  Per channel the scale
 // ks = RN(RN(s rcp_cell) O) is formed once (O a power of two: the last product is exact); per visibility and axis
@@ -210,7 +159,7 @@ struct FastMap2 {
     // sort key of the visibility (fast_key's layout; a dropped visibility has the drop bit, 1 << 2 bits_q, set).
     // Both axes are computed first and tested together: one branch per visibility.  Returns kUndecided where the
     // screen does not decide: the caller then takes slow_key.
-    __device__ __forceinline__ uint32_t key(double u_m, double v_m, double ks) const {
+    __device__ __forceinline__ uint32_t key(double u_m, double v_m, double ks, uint32_t gtile = 0) const {
         const double kMagic = 6755399441055744.0;               // 1.5 * 2^52
         const double tx = __fma_rn(u_m, ks, chalf), ty = __fma_rn(v_m, ks, chalf);
         const double mx = __dadd_rn(tx, kMagic), my = __dadd_rn(ty, kMagic);
@@ -224,15 +173,15 @@ struct FastMap2 {
                 return 1u << (2 * bits_q);                      // drop slot 0, tile 0, origin (0, 0)
             const uint32_t qx = (uint32_t)((x0 << o_shift) - ax), qy = (uint32_t)((y0 << o_shift) - ay);
             const uint32_t ux = (uint32_t)x0, uy = (uint32_t)y0;
-            const uint32_t tile = (uy >> tlog) * ntx + (ux >> tlog);
+            const uint32_t tile = gtile + (uy >> tlog) * ntx + (ux >> tlog);
             return (tile << tile_shift) | ((uy & tmask) << (aux_bits + tlog)) | ((ux & tmask) << aux_bits) |
                    (qy << bits_q) | qx;
         }
         return kUndecided;                                      // rare: near a rounding boundary, or far away
     }
     // what the caller maps such a visibility with (kept out of key() so that unrolled callers inline it once)
-    static __device__ __forceinline__ uint32_t slow_key(double u_m, double v_m, double s, const MapParams &p) {
-        return fast_key(map_vis(u_m, v_m, 0.0, s, p), p);
+    static __device__ __forceinline__ uint32_t slow_key(double u_m, double v_m, double s, const MapParams &p, uint32_t gtile = 0) {
+        return fast_key(map_vis(u_m, v_m, 0.0, s, p), p, gtile);
     }
     static constexpr uint32_t kUndecided = 0xFFFFFFFEu;         // never a key (nor kAbsent of presum.cu)
 };

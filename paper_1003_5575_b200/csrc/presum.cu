@@ -132,6 +132,8 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
         const bool col = f < geo.n_chan;
         const double s = col ? scale[f] : 0.0;
         const double ks = FAST ? fm.chan_scale(s) : 0.0;
+        // (gridder_bin_channels: the channel's grid is part of the tile id, so nothing merges across grids)
+        const uint32_t gtile = p.chans_per_grid ? (f / (uint32_t)p.chans_per_grid) * (uint32_t)p.grid_tiles : 0u;
         uint32_t key[8];
         uint32_t valid = 0, slow = 0;
 #pragma unroll
@@ -140,7 +142,7 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
             uint32_t row;
             if (row_index<RT>(geo, r, t0, b0, row) && col) {
                 const double *L = uvw + (size_t)row * 3;
-                key[r] = FAST ? fm.key(__ldg(L), __ldg(L + 1), ks) : FastMap2::kUndecided;
+                key[r] = FAST ? fm.key(__ldg(L), __ldg(L + 1), ks, gtile) : FastMap2::kUndecided;
                 if (key[r] == FastMap2::kUndecided) slow |= 1u << r;
                 valid |= 1u << r;
             }
@@ -151,7 +153,7 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
             uint32_t row;
             row_index<RT>(geo, r, t0, b0, row);
             const double *L = uvw + (size_t)row * 3;
-            const uint32_t k = FastMap2::slow_key(__ldg(L), __ldg(L + 1), s, p);
+            const uint32_t k = FastMap2::slow_key(__ldg(L), __ldg(L + 1), s, p, gtile);
 #pragma unroll
             for (int rr = 0; rr < 8; ++rr)
                 if (rr == r) key[rr] = k;

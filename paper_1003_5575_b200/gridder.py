@@ -17,7 +17,7 @@ LIB_PATH = _HERE / "libgridder.so"
 
 OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_WORKSPACE, ERR_CUDA, ERR_NOT_BINNED, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 
-EXPORTS = ("gridder_workspace_size", "gridder_plan", "gridder_workspace_size_tuned", "gridder_plan_tuned", "gridder_map_presum",
+EXPORTS = ("gridder_bin_channels", "gridder_grid_channels", "gridder_workspace_size", "gridder_plan", "gridder_workspace_size_tuned", "gridder_plan_tuned", "gridder_map_presum",
            "gridder_bin", "gridder_bin_tables", "gridder_grid", "gridder_destroy",
            "gridder_get_stats", "gridder_map", "gridder_scatter_atomic", "gridder_image_workspace_size", "gridder_image",
            "gridder_run_host", "gridder_sum_parts", "gridder_set_profiling",
@@ -35,7 +35,8 @@ class _Config(C.Structure):
     _fields_ = [("grid_size", C.c_int32), ("cell_size", C.c_double), ("n_pol", C.c_int32),
                 ("oversample", C.c_int32), ("n_wplanes", C.c_int32), ("support", C.POINTER(C.c_int32)),
                 ("w_max", C.c_double), ("kernel_is_complex", C.c_int32), ("kernel", C.c_void_p),
-                ("max_vis", C.c_int64), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t)]
+                ("max_vis", C.c_int64), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+                ("max_grids", C.c_int32)]
 
 
 class _Tuning(C.Structure):
@@ -77,6 +78,9 @@ def load_library() -> C.CDLL:
         lib.gridder_bin_tables.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
                                            C.c_void_p, C.c_void_p]
         lib.gridder_grid.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+        lib.gridder_bin_channels.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32, C.c_int32,
+                                             C.c_void_p]
+        lib.gridder_grid_channels.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
         lib.gridder_destroy.argtypes = [C.c_void_p]
         lib.gridder_get_stats.argtypes = [C.c_void_p, C.POINTER(_Stats)]
         lib.gridder_map.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
@@ -155,7 +159,7 @@ class Gridder:
 
     def __init__(self, *, grid_size: int, cell_size: float, oversample: int, support, kernel: torch.Tensor,
                  max_vis: int, n_wplanes: int = 1, w_max: float = 1.0, kernel_is_complex: bool = False,
-                 device=None, tuning: dict | None = None):
+                 device=None, tuning: dict | None = None, max_grids: int = 1):
         """`tuning`: optional {field of gridder_tuning: value} (include/gridder.h); absent fields are defaults."""
         lib = load_library()
         self._lib = lib
@@ -168,7 +172,9 @@ class Gridder:
         self._kernel = kernel.to(self.device, torch.float32).contiguous()
         self.grid_size = int(grid_size)
         cfg = _Config(int(grid_size), float(cell_size), 4, int(oversample), int(n_wplanes), self._support,
-                      float(w_max), int(bool(kernel_is_complex)), self._kernel.data_ptr(), int(max_vis), None, 0)
+                      float(w_max), int(bool(kernel_is_complex)), self._kernel.data_ptr(), int(max_vis), None, 0,
+                      int(max_grids))
+        self.n_grids = 1                 # of the last bin
         tune = _Tuning()
         for k, v in (tuning or {}).items():
             if k not in TUNING_FIELDS:
@@ -193,9 +199,10 @@ class Gridder:
         self._keep = []
 
     # -- the four calls ---------------------------------------------------------------------
-    def bin(self, uvw_m: torch.Tensor, freq_hz: torch.Tensor, stream=None, table_index=None) -> None:
+    def bin(self, uvw_m: torch.Tensor, freq_hz: torch.Tensor, stream=None, table_index=None, chans_per_grid=None) -> None:
         """uvw_m float64 [n_time][n_baseline][3] (metres), freq_hz float64 [n_chan]; table_index (row f3):
-        int32 [n_time][n_baseline] choosing each baseline's table from the plan's bank, or None."""
+        int32 [n_time][n_baseline] choosing each baseline's table from the plan's bank, or None;
+        chans_per_grid (row f4): one output grid per block of that many channels (gridder_bin_channels)."""
         if uvw_m.dim() == 2:
             uvw_m = uvw_m[None]
         n_time, n_bl, three = uvw_m.shape
@@ -203,6 +210,18 @@ class Gridder:
             raise ValueError("uvw_m must be [n_time][n_baseline][3]")
         self._keep = [uvw_m, freq_hz, table_index]
         self._binned = None
+        if chans_per_grid is not None:
+            if table_index is not None:
+                raise ValueError("chans_per_grid and table_index cannot be combined")
+            rc = self._lib.gridder_bin_channels(self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m", self.device), n_time, n_bl,
+                                                _dev_ptr(freq_hz, torch.float64, "freq_hz", self.device), freq_hz.numel(),
+                                                int(chans_per_grid), _stream_ptr(stream))
+            if rc != OK:
+                raise GridderError(rc, "gridder_bin_channels")
+            self.n_grids = max(1, -(-freq_hz.numel() // int(chans_per_grid)))
+            self._binned = (n_time, n_bl, freq_hz.numel())
+            return
+        self.n_grids = 1
         rc = self._lib.gridder_bin_tables(self._plan, _dev_ptr(uvw_m, torch.float64, "uvw_m", self.device), n_time, n_bl,
                                           _dev_ptr(freq_hz, torch.float64, "freq_hz", self.device), freq_hz.numel(),
                                           _dev_ptr(table_index, torch.int32, "table_index", self.device, n_time * n_bl),
@@ -212,18 +231,21 @@ class Gridder:
         self._binned = (n_time, n_bl, freq_hz.numel())
 
     def grid(self, vis: torch.Tensor, weight=None, out=None, accumulate: bool = False, stream=None) -> torch.Tensor:
-        """vis float32 [...][4][2]; returns the grid float32 [4][N][N][2]; asynchronous."""
+        """vis float32 [...][4][2]; returns the grid float32 [4][N][N][2] (after a bin with chans_per_grid:
+        [n_grids][4][N][N][2]); asynchronous."""
+        shape = (4, self.grid_size, self.grid_size, 2) if self.n_grids == 1 else (self.n_grids, 4, self.grid_size, self.grid_size, 2)
         if out is None:
             if accumulate:
                 raise ValueError("accumulate needs an existing grid")
-            out = torch.empty((4, self.grid_size, self.grid_size, 2), dtype=torch.float32, device=self.device)
+            out = torch.empty(shape, dtype=torch.float32, device=self.device)
         if self._binned is None:
             raise GridderError(ERR_NOT_BINNED, "gridder_grid")
         n = self._binned[0] * self._binned[1] * self._binned[2]
-        rc = self._lib.gridder_grid(self._plan, _dev_ptr(vis, torch.float32, "vis", self.device, 8 * n),
-                                    _dev_ptr(weight, torch.float32, "weight", self.device, n),
-                                    _dev_ptr(out, torch.float32, "grid", self.device, 8 * self.grid_size ** 2),
-                                    int(accumulate), _stream_ptr(stream))
+        fn = self._lib.gridder_grid if self.n_grids == 1 else self._lib.gridder_grid_channels
+        rc = fn(self._plan, _dev_ptr(vis, torch.float32, "vis", self.device, 8 * n),
+                _dev_ptr(weight, torch.float32, "weight", self.device, n),
+                _dev_ptr(out, torch.float32, "grid", self.device, 8 * self.grid_size ** 2 * self.n_grids),
+                int(accumulate), _stream_ptr(stream))
         if rc != OK:
             raise GridderError(rc, "gridder_grid")
         return out

@@ -42,7 +42,7 @@ def test_null_and_invalid_arguments_need_no_device(lib):
     sup = (C.c_int32 * 1)(16)
     def cfg(**kw):
         base = dict(grid_size=256, cell_size=1.0, n_pol=4, oversample=4, n_wplanes=1, support=sup, w_max=1.0,
-                    kernel_is_complex=0, kernel=None, max_vis=1000, workspace=None, workspace_bytes=0)
+                    kernel_is_complex=0, kernel=None, max_vis=1000, workspace=None, workspace_bytes=0, max_grids=0)
         base.update(kw)
         return gridder._Config(*[base[f[0]] for f in gridder._Config._fields_])
     for bad in (dict(grid_size=255), dict(grid_size=0), dict(cell_size=0.0), dict(n_pol=2), dict(oversample=0),
@@ -60,6 +60,18 @@ def test_null_and_invalid_arguments_need_no_device(lib):
     sup64 = (C.c_int32 * 64)(*([32] * 64))
     assert lib.gridder_workspace_size(C.byref(cfg(n_wplanes=64, support=sup64, oversample=64, kernel_is_complex=1,
                                                   w_max=1.0)), C.byref(need)) == gridder.ERR_UNSUPPORTED
+    # tuning: a zeroed struct is the default plan, a field outside its range is refused, several grids are sized
+    tune = gridder._Tuning()
+    assert lib.gridder_workspace_size_tuned(C.byref(cfg()), C.byref(tune), C.byref(need)) == gridder.OK
+    one = need.value
+    assert lib.gridder_workspace_size(C.byref(cfg()), C.byref(need)) == gridder.OK and need.value == one
+    for field, bad in (("tile_log2", 5), ("chunk", 7), ("merge", 3), ("presum", -1), ("fold_batches", 3), ("table_in_tmem", 9)):
+        t = gridder._Tuning()
+        setattr(t, field, bad)
+        assert lib.gridder_workspace_size_tuned(C.byref(cfg()), C.byref(t), C.byref(need)) == gridder.ERR_INVALID_ARG, field
+    assert lib.gridder_workspace_size(C.byref(cfg(max_grids=12)), C.byref(need)) == gridder.OK and need.value > one
+    assert lib.gridder_workspace_size(C.byref(cfg(max_grids=-1)), C.byref(need)) == gridder.ERR_INVALID_ARG
+    assert lib.gridder_bin_channels(None, None, 1, 1, None, 1, 1, None) == gridder.ERR_INVALID_ARG
     plan = C.c_void_p()
     assert lib.gridder_plan(C.byref(cfg(grid_size=255)), C.byref(plan), None) == gridder.ERR_INVALID_ARG
     assert lib.gridder_plan(C.byref(cfg()), None, None) == gridder.ERR_INVALID_ARG
