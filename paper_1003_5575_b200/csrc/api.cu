@@ -130,7 +130,7 @@ int derive(const gridder_config *cfg, const gridder_tuning *tuning, Plan &p) {
     // short items so that a hot tile still spreads over the ~1800 resident warps; the largest get 8192
     // (2048 when the entries are partial records: shorter items balance the end of the grid kernel), which bounds the partial regions the flush has to sum for
     // the cells of a hot tile (the accuracy budget of DESIGN.md section 7 holds up to 8192)
-    int k_auto = p.presum ? 2048 : 8192;
+    int k_auto = 2048;
     while (k_auto > 256 && (int64_t)k_auto * 16384 > cfg->max_vis) k_auto >>= 1;
     p.chunk = t.chunk ? t.chunk : k_auto;
     p.warps_forced = t.max_warps;
