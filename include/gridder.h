@@ -268,6 +268,11 @@ GRIDDER_API const char *gridder_strerror(int code);
 GRIDDER_API int gridder_last_cuda_error(const gridder_plan_t *plan);
 /* "major.minor.patch" of the library. */
 GRIDDER_API const char *gridder_version(void);
+/* Builds with -DGRIDDER_CHECKED (libgridder_checked.so; `python -m paper_1003_5575_b200.build --checked`) check
+ * every index their kernels compute -- shared memory, workspace arrays, the caller's buffers -- against its bound
+ * and count the failures: this returns the count over all plans of the process so far (collected at gridder_bin
+ * and gridder_destroy).  The normal build has no checks and returns -1. */
+GRIDDER_API long long gridder_check_violations(void);
 
 #ifdef __cplusplus
 }

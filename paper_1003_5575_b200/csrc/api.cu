@@ -223,6 +223,24 @@ cudaError_t carve(Plan &p, char *base) {
     return cudaSuccess;
 }
 
+// GRIDDER_CHECKED builds: failed index checks of all plans of this process (see gridder_internal.cuh GR_CHECK)
+long long g_check_violations = 0;
+
+// Adds the device counter of the plan's last bin / grid to the process total (synchronises the device).
+void collect_violations(Plan *p) {
+#ifdef GRIDDER_CHECKED
+    if (!p || !p->counters) return;
+    unsigned int v = 0;
+    if (cudaDeviceSynchronize() == cudaSuccess &&
+        cudaMemcpy(&v, &p->counters->violations, sizeof(v), cudaMemcpyDeviceToHost) == cudaSuccess && v) {
+        g_check_violations += v;
+        cudaMemset(&p->counters->violations, 0, sizeof(v));
+    }
+#else
+    (void)p;
+#endif
+}
+
 int cuda_fail(Plan *p, cudaError_t e) {
     if (p) p->last_cuda_error = (int)e;
     return GRIDDER_ERR_CUDA;
@@ -307,6 +325,7 @@ static int bin_common(gridder_plan_t *plan, const double *uvw_m, int32_t n_time,
     if (n > 0 && (!uvw_m || !freq_hz)) return GRIDDER_ERR_INVALID_ARG;
     if (n > p->cfg.max_vis) return GRIDDER_ERR_CAPACITY;
     if (n_chan > kMaxChannels) return GRIDDER_ERR_UNSUPPORTED;
+    collect_violations(p);           // (the bin resets the device counters)
     p->binned = false;
     p->n_grids = n_grids;
     p->chans_per_grid = chans_per_grid;
@@ -344,6 +363,7 @@ int gridder_destroy(gridder_plan_t *plan) {
     Plan *p = reinterpret_cast<Plan *>(plan);
     if (!p) return GRIDDER_ERR_INVALID_ARG;
     cudaError_t e = cudaDeviceSynchronize();     // the caller may free the workspace after this
+    collect_violations(p);
     image_destroy(*p);
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
     for (int r = 0; r < kProfRing; ++r)
@@ -595,6 +615,14 @@ int gridder_last_cuda_error(const gridder_plan_t *plan) {
     return p ? p->last_cuda_error : 0;
 }
 
-const char *gridder_version(void) { return "0.1.0"; }
+const char *gridder_version(void) { return "0.2.0"; }
+
+long long gridder_check_violations(void) {
+#ifdef GRIDDER_CHECKED
+    return g_check_violations;
+#else
+    return -1;
+#endif
+}
 
 }  // extern "C"

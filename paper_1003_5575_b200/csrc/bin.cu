@@ -222,7 +222,7 @@ __global__ void __launch_bounds__(256) item_fill_kernel(const uint32_t *__restri
                                                          const uint32_t *__restrict__ tile_end,
                                                          const unsigned long long *__restrict__ scan, int n_tiles,
                                                          int n_cls, int chunk, TileInfo *__restrict__ info,
-                                                         WorkItem *__restrict__ items, Counters *counters) {
+                                                         WorkItem *__restrict__ items, Counters *counters, unsigned int max_items) {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     const int n_vtiles = n_tiles * n_cls;
     if (t == 0) {
@@ -255,6 +255,7 @@ __global__ void __launch_bounds__(256) item_fill_kernel(const uint32_t *__restri
     ti.n_full = nf;
     ti.tail_item = rem ? tail_id : 0xFFFFFFFFu;
     info[t] = ti;
+    GR_CHECK(counters, (unsigned long long)full_base + nf <= max_items && (!rem || tail_id < max_items));
     for (uint32_t k = 0; k < nf; ++k) {
         WorkItem w;
         w.start = start + k * chunk; w.len = chunk; w.tile = t; w.pad = 0;
@@ -372,7 +373,7 @@ cudaError_t launch_bin(Plan &p, const double *uvw, int n_time, int n_bl, const d
     GR_TRY(cub::DeviceScan::ExclusiveSum(p.cub_temp, tb, (const unsigned long long *)p.tile_chunks,
                                          p.tile_chunks_scan, (long long)nt1, s));
     item_fill_kernel<<<(nt1 + 255) / 256, 256, 0, s>>>(p.tile_start, tile_end, p.tile_chunks_scan, p.n_tiles_cls,
-                                                         p.n_cls, p.chunk, p.tile_info, p.items, p.counters);
+                                                         p.n_cls, p.chunk, p.tile_info, p.items, p.counters, (unsigned int)p.max_items);
     GR_TRY(cudaGetLastError());
     p.n_launches += 3;
     stage_mark(p, 3, s);

@@ -164,6 +164,7 @@ __device__ __forceinline__ Entry load_entry(const GridParams &p, unsigned e, boo
     Entry k;
     k.key = k.idx = k.aux = 0u;
     if (valid) {
+        GR_CHECK(p.counters, e < p.n_sorted);
         k.key = __ldg(p.keys + e);
         if (GEN) {
             const uint2 v = __ldg(reinterpret_cast<const uint2 *>(p.vals) + e);
@@ -182,6 +183,7 @@ template <bool GEN>
 __device__ __forceinline__ void issue_vis(const GridParams &p, float4 *raw, int lane, const Entry k, bool valid) {
     const bool dropped = GEN ? ((k.aux >> 30) & 1u) : ((k.key >> (2 * p.key.bits_q)) & 1u);
     const bool live = valid && !dropped;
+    GR_CHECK(p.counters, !live || k.idx < p.n_src);
     const float4 *src = p.vis + 2 * (size_t)(live ? k.idx : 0u);
     cp_async_16(raw + lane, src, live);                // two planes of 32 float4: conflict-free to read back
     cp_async_16(raw + 32 + lane, src + 1, live);
@@ -260,6 +262,7 @@ __device__ __forceinline__ int stage_write(const GridParams &p, const float4 *ra
     int next_coff = __shfl_sync(0xffffffffu, coff, above ? __ffs(above) - 1 : lane);
     if (!above) next_coff = 0;
     const int last_poff = __shfl_sync(0xffffffffu, poff, 31 - __clz(kept | 1u));
+    GR_CHECK(p.counters, n_rec + 2 <= G::SLOTS);
     if (keep) {
         // slot r carries the table offset of record r + 1 (the consumer loads taps one record ahead)
         // and the origin of record r; every slot also carries its own table offset (slot 0's is used)
@@ -360,7 +363,8 @@ struct RecRegs {
 // cleared.  A long single chain is not good enough: neighbouring channels of one baseline give
 // nearly equal terms, whose rounding errors do not cancel (measured 1.2e-5 relative at 2048 terms).
 template <int NA, int NB, int RW, bool CIRC>
-__device__ __forceinline__ void fold_patch(float4 *regA, float4 *regB, int cur, int lane, float (&acc)[NA][NB][8]) {
+__device__ __forceinline__ void fold_patch(float4 *regA, float4 *regB, int cur, int lane, float (&acc)[NA][NB][8],
+                                           Counters *ck) {
     __syncwarp();       // a cell changes owner lane from one origin to the next
     constexpr int SPY = 4 * NB, CB = RW * (CIRC ? SPY : 1);     // (CB: plane stride is passed by the caller via regB)
     (void)CB;
@@ -371,6 +375,7 @@ __device__ __forceinline__ void fold_patch(float4 *regA, float4 *regB, int cur, 
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
             const int o = CIRC ? ((y0 + rq + 4 * b) & (SPY - 1)) * RW + xo + 8 * a : xo + 4 * b * RW + 8 * a;
+            GR_CHECK(ck, o >= 0 && o < (int)(regB - regA) && (!CIRC || xo + 8 * a < RW));
             float4 x = regA[o], y = regB[o];
             x.x += acc[a][b][0]; x.y += acc[a][b][1]; x.z += acc[a][b][2]; x.w += acc[a][b][3];
             y.x += acc[a][b][4]; y.y += acc[a][b][5]; y.z += acc[a][b][6]; y.w += acc[a][b][7];
@@ -382,8 +387,9 @@ __device__ __forceinline__ void fold_patch(float4 *regA, float4 *regB, int cur, 
 
 // Ring of region rows: rows [from, to) of the item's region are complete -- to the item's partial, slots cleared.
 template <int RW, int SPY, int CELLS>
-__device__ __forceinline__ void flush_rows(float4 *regA, float4 *regB, float4 *dst, int from, int to, int lane) {
+__device__ __forceinline__ void flush_rows(float4 *regA, float4 *regB, float4 *dst, int from, int to, int lane, Counters *ck) {
     __syncwarp();
+    GR_CHECK(ck, from >= 0 && from <= to && to * RW <= CELLS);
     for (int y = from; y < to; ++y) {
         if (lane < RW) {
             const int o = (y & (SPY - 1)) * RW + lane;
@@ -412,12 +418,12 @@ __device__ __forceinline__ void ffma2(float &d0, float &d1, float c, float v0, f
 template <int NA, int NB, int RW, int CELLS, int MODE>
 __device__ __forceinline__ void consume(const RecRegs<NA, NB, MODE> &R, const int poff, int &cur, int &cmp,
                                         float4 *regA, float4 *regB, int lane, float (&acc)[NA][NB][8],
-                                        int &rows_done, float4 *dst) {
+                                        int &rows_done, float4 *dst, Counters *ck) {
     constexpr bool CIRC = MODE == 0 || MODE == 3;
     if (poff != cmp) {                                      // warp-uniform
-        if (cur >= 0) fold_patch<NA, NB, RW, CIRC>(regA, regB, cur, lane, acc);
+        if (cur >= 0) fold_patch<NA, NB, RW, CIRC>(regA, regB, cur, lane, acc, ck);
         if (CIRC && poff >= 0 && (poff >> 8) > rows_done) {     // the origin moved up: the rows below it are complete
-            flush_rows<RW, 4 * NB, CELLS>(regA, regB, dst, rows_done, poff >> 8, lane);
+            flush_rows<RW, 4 * NB, CELLS>(regA, regB, dst, rows_done, poff >> 8, lane, ck);
             rows_done = poff >> 8;
         }
         cur = cmp = poff;
@@ -589,11 +595,11 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
                     mB = *reinterpret_cast<const int2 *>(sp + G::SLOT_F4 + G::VF4);
                     A.wait();
                     B.fetch(sp + G::SLOT_F4, mA.x, cl);
-                    consume<NA, NB, G::RW, G::CELLS, MODE>(A, mA.y + sub_poff, cur, cmp, regA, regB, lane, acc, rows_done, dst);
+                    consume<NA, NB, G::RW, G::CELLS, MODE>(A, mA.y + sub_poff, cur, cmp, regA, regB, lane, acc, rows_done, dst, p.counters);
                     mA = *reinterpret_cast<const int2 *>(sp + 2 * G::SLOT_F4 + G::VF4);
                     B.wait();
                     A.fetch(sp + 2 * G::SLOT_F4, mB.x, cl);
-                    consume<NA, NB, G::RW, G::CELLS, MODE>(B, mB.y + sub_poff, cur, cmp, regA, regB, lane, acc, rows_done, dst);
+                    consume<NA, NB, G::RW, G::CELLS, MODE>(B, mB.y + sub_poff, cur, cmp, regA, regB, lane, acc, rows_done, dst, p.counters);
                     sp += 2 * G::SLOT_F4;
                 } while (sp < send);
             }
@@ -604,10 +610,11 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
                 cmp = kSentinel;
                 __syncwarp();
                 float4 *dst = p.partials + (size_t)dC.item * (2 * G::CELLS);      // (virtual) item id inside the class
+                GR_CHECK(p.counters, (dC.item >> G::VSHIFT) < p.max_items_cls);
                 if (G::CIRC) {
                     // the rest of the region: the rows still in the ring, then rows no entry reached (their slots
                     // were cleared when the rows SPY below them were written: zeros)
-                    flush_rows<G::RW, G::SPY, G::CELLS>(regA, regB, dst, rows_done, G::RH, lane);
+                    flush_rows<G::RW, G::SPY, G::CELLS>(regA, regB, dst, rows_done, G::RH, lane, p.counters);
                     rows_done = 0;
                 } else {
                     for (int i = lane; i < 2 * G::CELLS; i += 32) {
@@ -690,6 +697,7 @@ __global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
                 for (uint32_t c = 0; c < n_it; ++c) {
                     const uint32_t item = c < ti.n_full ? ti.full_base + c : ti.tail_item;
                     const size_t vitem = (size_t)(item - first_item) * (G::NSUB * G::NSUB) + sub;
+                    GR_CHECK(const_cast<Counters *>(p.counters), item >= first_item && item - first_item < p.max_items_cls && cell >= 0 && cell < G::CELLS);
                     const float4 *part = p.partials + vitem * (2 * G::CELLS);
                     const float4 a = __ldcs(part + cell), b = __ldcs(part + G::CELLS + cell);
                     acc[0] += (double)a.x; acc[1] += (double)a.y; acc[2] += (double)a.z; acc[3] += (double)a.w;
@@ -840,6 +848,9 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         gp.tmem_cols = p.tmem_cols;
         gp.merge = p.merge;
         gp.n_q = p.cfg.oversample * p.cfg.oversample;
+        gp.n_sorted = (uint32_t)p.n_sorted;
+        gp.n_src = (uint32_t)p.n_vis;                    // (record sums live in visibility slots: the same bound)
+        gp.max_items_cls = (uint32_t)p.max_items_cls;
         if (p.presum_active) {       // the sorted list names partial records: their sums are the "visibilities"
             gp.vis = p.ps_sum;
             gp.weight = nullptr;
@@ -868,6 +879,7 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
             fp.nty = p.nty;
             fp.accumulate = (c > 0 || accumulate) ? 1 : 0;
             fp.cover = nullptr;
+            fp.max_items_cls = (uint32_t)p.max_items_cls;
             if (c > 0) {
                 // a later class only adds: cells no region of the class can reach are skipped (sparse classes)
                 const int reach = (g.RW - 1 + (g.nsub - 1) * 8 * g.NA + p.T - 1) / p.T;

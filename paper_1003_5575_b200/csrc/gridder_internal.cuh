@@ -19,6 +19,16 @@
 
 #include "../../include/gridder.h"
 
+// GRIDDER_CHECKED builds (python -m paper_1003_5575_b200.build --checked -> libgridder_checked.so): every index the
+// kernels compute for shared memory, the workspace arrays and the caller's buffers is checked against its bound
+// and failures are COUNTED (Counters::violations, summed per process by gridder_check_violations) -- the pool's
+// compute-sanitizer is closed, so this is the memcheck the tests run (tests/test_gpu_checked_build.py).
+#ifdef GRIDDER_CHECKED
+#define GR_CHECK(counters, cond) do { if (!(cond)) atomicAdd(&(counters)->violations, 1u); } while (0)
+#else
+#define GR_CHECK(counters, cond) do { } while (0)
+#endif
+
 namespace gridder {
 
 constexpr int kProfRing = 32;                     // calls remembered by the stage timers
@@ -102,7 +112,8 @@ struct Counters {
     unsigned int cls_begin[kMaxClasses];      // work-item range of each class slot
     unsigned int cls_end[kMaxClasses];
     unsigned int queue_head[kMaxClasses];     // work queues of the grid kernel launches
-    unsigned int pad[2];
+    unsigned int violations;                  // GRIDDER_CHECKED builds: index checks that failed (see GR_CHECK)
+    unsigned int pad[1];
     unsigned long long n_exec[kMaxClasses];   // records gridded per class by the last gridder_grid (after merging)
 };
 
@@ -122,6 +133,7 @@ struct GridParams {
     int32_t tmem_cols;             // tensor-memory columns to allocate (MODE 3)
     int32_t n_q;                   // O^2 sub-tables
     int32_t merge;                 // sum entries of a batch with equal origin and table offset before gridding
+    uint32_t n_sorted, n_src, max_items_cls;      // bounds (GRIDDER_CHECKED builds): sorted entries, gatherable slots, items
     KeyLayout key;
 };
 
@@ -135,6 +147,7 @@ struct FlushParams {
     int32_t ntx, nty;
     int32_t accumulate;
     const unsigned char *cover;    // null, or [n_tiles]: 0 = no region of this class reaches the tile's cells
+    uint32_t max_items_cls;        // bound (GRIDDER_CHECKED builds)
 };
 
 struct Plan {

@@ -52,6 +52,7 @@ struct PsGeo {
     uint32_t n_tblock;          // ceil(n_time / rt)
     uint32_t n_bgroup;          // ceil(n_bl / rb)
     uint32_t n_groups;          // n_tblock * n_bgroup * n_fchunk; group g = (tb * n_bgroup + bg) * n_fchunk + fc
+    uint32_t n_vis;             // n_time * n_bl * n_chan
 };
 
 __device__ __forceinline__ void group_coords(const PsGeo &g, uint32_t grp, uint32_t &t0, uint32_t &b0, uint32_t &f0) {
@@ -210,8 +211,12 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
             if (valid & bit) {
                 uint32_t row;
                 row_index<RT>(geo, r, t0, b0, row);
+                GR_CHECK(counters, row * geo.n_chan + f < geo.n_vis);
                 flags[row * geo.n_chan + f] = (unsigned char)((r < 4 ? w_lo : w_hi) >> (8 * (r & 3)));
-                if (head & bit) st[idx++] = key[r];
+                if (head & bit) {
+                    GR_CHECK(counters, (size_t)(st - stage) + idx < geo.n_vis);
+                    st[idx++] = key[r];
+                }
             }
         }
     }
@@ -230,7 +235,8 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
 __global__ void __launch_bounds__(256) presum_compact_kernel(const uint32_t *__restrict__ stage,
                                                               const uint32_t *__restrict__ count,
                                                               const uint32_t *__restrict__ base, const PsGeo geo,
-                                                              uint32_t *__restrict__ rec_key, uint32_t *__restrict__ rec_idx) {
+                                                              uint32_t *__restrict__ rec_key, uint32_t *__restrict__ rec_idx,
+                                                              Counters *counters) {
     const int lane = threadIdx.x & 31;
     const uint32_t nw = gridDim.x * 8u;
     for (uint32_t grp = blockIdx.x * 8u + (threadIdx.x >> 5); grp < geo.n_groups; grp += nw) {
@@ -239,6 +245,7 @@ __global__ void __launch_bounds__(256) presum_compact_kernel(const uint32_t *__r
         group_coords(geo, grp, t0, b0, f0);
         const uint32_t *st = stage + stage_offset(geo, t0, b0, f0);
         for (uint32_t j = lane; j < cnt; j += 32) {
+            GR_CHECK(counters, dst + j < geo.n_vis && slot_index(geo, t0, b0, f0, j) < geo.n_vis && (size_t)(st - stage) + j < geo.n_vis);
             rec_key[dst + j] = st[j];
             rec_idx[dst + j] = slot_index(geo, t0, b0, f0, j);
         }
@@ -262,7 +269,7 @@ __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefe
 template <bool WEIGHTED, int RT>
 __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__restrict__ vis, const float *__restrict__ weight,
                                                                const unsigned char *__restrict__ flags, const PsGeo geo,
-                                                               float4 *__restrict__ rec_sum) {
+                                                               float4 *__restrict__ rec_sum, Counters *counters) {
     __shared__ float4 smem[kPsWarps * kPsWarpF4];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     float4 *slotA = smem + warp * kPsWarpF4, *slotB = slotA + 8 * 32;
@@ -305,6 +312,7 @@ __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__r
             uint32_t row;
             if (row_index<RT>(geo, r, t0, b0, row) && col) {
                 const size_t i = (size_t)(row * geo.n_chan + f);
+                GR_CHECK(counters, i < geo.n_vis);
                 va[r] = ld_stream4(vis + 2 * i);
                 vb[r] = ld_stream4(vis + 2 * i + 1);
                 w[r] = WEIGHTED ? __ldcs(weight + i) : 1.0f;
@@ -346,12 +354,14 @@ __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__r
             while (cf & kFlagLink) {
                 const int rr = (int)((cf >> 1) & 7u);
                 ++c;
+                GR_CHECK(counters, c < 32);
                 const float4 ta = slotA[rr * 32 + c], tb4 = slotB[rr * 32 + c];
                 sa.x += ta.x; sa.y += ta.y; sa.z += ta.z; sa.w += ta.w;
                 sb.x += tb4.x; sb.y += tb4.y; sb.z += tb4.z; sb.w += tb4.w;
                 cf = sflag[rr * 32 + c];
             }
             const size_t idx = (size_t)slot_index(geo, t0, b0, f0, j++);
+            GR_CHECK(counters, idx < geo.n_vis && j <= total);
             rec_sum[2 * idx] = sa;
             rec_sum[2 * idx + 1] = sb;
         }
@@ -410,6 +420,7 @@ static PsGeo make_geo(int n_time, int n_bl, int n_chan) {
     g.n_tblock = ((uint32_t)n_time + g.rt - 1) / g.rt;
     g.n_bgroup = ((uint32_t)n_bl + g.rb - 1) / g.rb;
     g.n_groups = g.n_tblock * g.n_bgroup * g.n_fchunk;
+    g.n_vis = g.n_time * g.n_bl * g.n_chan;
     return g;
 }
 
@@ -456,7 +467,7 @@ cudaError_t launch_presum_plan(Plan &p, const double *uvw, const double *scale, 
                                          (long long)geo.n_groups + 1, s));
     unsigned int total = 0;
     GR_TRY(cudaMemcpyAsync(&total, p.ps_base + geo.n_groups, sizeof(unsigned int), cudaMemcpyDeviceToHost, s));
-    presum_compact_kernel<<<blocks, 256, 0, s>>>(stage, p.ps_count, p.ps_base, geo, p.keys[0], (uint32_t *)p.vals[0]);
+    presum_compact_kernel<<<blocks, 256, 0, s>>>(stage, p.ps_count, p.ps_base, geo, p.keys[0], (uint32_t *)p.vals[0], p.counters);
     GR_TRY(cudaGetLastError());
     GR_TRY(cudaStreamSynchronize(s));
     p.n_launches += 3;
@@ -469,7 +480,7 @@ cudaError_t launch_presum(Plan &p, const float *vis, const float *weight, cudaSt
     const PsGeo geo = make_geo(p.ps_n_time, p.ps_n_bl, p.ps_n_chan);
     const int blocks = (int)min((long long)(geo.n_groups + kPsWarps - 1) / kPsWarps, (long long)p.n_sm * 32);
     const float4 *v4 = reinterpret_cast<const float4 *>(vis);
-#define PS_SUM(W, R) presum_kernel<W, R><<<blocks, kPsWarps * 32, 0, s>>>(v4, weight, p.ps_flags, geo, p.ps_sum)
+#define PS_SUM(W, R) presum_kernel<W, R><<<blocks, kPsWarps * 32, 0, s>>>(v4, weight, p.ps_flags, geo, p.ps_sum, p.counters)
     if (weight) {
         switch (geo.rt) {
             case 8: PS_SUM(true, 8); break;

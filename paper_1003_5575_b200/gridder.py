@@ -17,7 +17,7 @@ LIB_PATH = _HERE / "libgridder.so"
 
 OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_WORKSPACE, ERR_CUDA, ERR_NOT_BINNED, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 
-EXPORTS = ("gridder_bin_channels", "gridder_grid_channels", "gridder_workspace_size", "gridder_plan", "gridder_workspace_size_tuned", "gridder_plan_tuned", "gridder_map_presum",
+EXPORTS = ("gridder_check_violations", "gridder_bin_channels", "gridder_grid_channels", "gridder_workspace_size", "gridder_plan", "gridder_workspace_size_tuned", "gridder_plan_tuned", "gridder_map_presum",
            "gridder_bin", "gridder_bin_tables", "gridder_grid", "gridder_destroy",
            "gridder_get_stats", "gridder_map", "gridder_scatter_atomic", "gridder_image_workspace_size", "gridder_image",
            "gridder_run_host", "gridder_sum_parts", "gridder_set_profiling",
@@ -58,6 +58,19 @@ class _Stats(C.Structure):
 
 
 _lib = None
+
+
+def select_library(path) -> None:
+    """Use another build of the library (the GRIDDER_CHECKED one) -- before the first load_library()."""
+    global LIB_PATH
+    if _lib is not None:
+        raise RuntimeError("the library is loaded already")
+    LIB_PATH = Path(path)
+
+
+def check_violations() -> int:
+    """Failed index checks so far (GRIDDER_CHECKED build), -1 for the normal build."""
+    return int(load_library().gridder_check_violations())
 
 
 def load_library() -> C.CDLL:
@@ -101,6 +114,7 @@ def load_library() -> C.CDLL:
         lib.gridder_strerror.restype = C.c_char_p
         lib.gridder_last_cuda_error.argtypes = [C.c_void_p]
         lib.gridder_version.restype = C.c_char_p
+        lib.gridder_check_violations.restype = C.c_longlong
         for name in EXPORTS:
             getattr(lib, name)
         _lib = lib
