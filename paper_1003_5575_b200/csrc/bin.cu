@@ -153,6 +153,11 @@ MapParams make_map_params(const Plan &p) {
     mp.rcp_cell = 1.0 / p.cfg.cell_size;
     mp.span = (double)p.cfg.grid_size * p.cfg.oversample;
     mp.w_max = p.cfg.w_max;
+    mp.fm_chalf = (double)(p.cfg.grid_size / 2) * (double)p.cfg.oversample + 0.5;
+    mp.fm_eps = mp.span * 7.1054273576010019e-15;             // 2^-47 N O
+    mp.fm_span2 = 2.0 * mp.span;
+    mp.fm_half_so = (p.support_copy[0] * p.cfg.oversample) >> 1;
+    mp.fm_n_minus_s = p.cfg.grid_size - p.support_copy[0];
     mp.key = p.key;
     for (int i = 0; i < p.cfg.n_wplanes; ++i) {
         mp.support[i] = p.support_copy[i];

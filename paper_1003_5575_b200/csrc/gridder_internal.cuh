@@ -78,6 +78,9 @@ struct MapParams {
     double rcp_cell;         // RN(1 / du): screening value only, never decides a rounding (map.cuh)
     double span;             // N O: scale of the screening margin
     double w_max;
+    // FastMap2's constants (map.cuh), made on the host so that no kernel recomputes them
+    double fm_chalf, fm_eps, fm_span2;
+    int32_t fm_half_so, fm_n_minus_s;
     const int32_t *table_index;   // null, or DEVICE [n_time][n_baseline]: the table of each baseline (row f3)
     KeyLayout key;
     int32_t support[kMaxPlanes];

@@ -140,18 +140,17 @@ __device__ __forceinline__ uint32_t fast_key(const VisMap &m, const MapParams &p
 // 1.5 * 2^52 trick: m = RN(t1 + M) holds RN(t1) in its low mantissa bits, d = t1 - (m - M) is exact.
 struct FastMap2 {
     double rcp_cell, d_o, chalf, eps, span2;
-    int o_shift, o_minus_1, half_so, n_minus_s, s2;
+    int o_shift, o_minus_1, half_so, n_minus_s;
     uint32_t ntx, tmask, tlog, aux_bits, bits_q, tile_shift;
 
     __device__ __forceinline__ void init(const MapParams &p) {
         rcp_cell = p.rcp_cell; d_o = (double)p.oversample;
-        chalf = (double)(p.n_grid / 2) * (double)p.oversample + 0.5;
-        eps = p.span * 7.1054273576010019e-15;                 // 2^-47 N O
-        span2 = 2.0 * p.span;
+        chalf = p.fm_chalf;                                     // N/2 O + 1/2
+        eps = p.fm_eps;                                         // 2^-47 N O
+        span2 = p.fm_span2;
         o_shift = p.o_shift; o_minus_1 = p.oversample - 1;
-        half_so = (p.support[0] * p.oversample) >> 1;
-        n_minus_s = p.n_grid - p.support[0];
-        s2 = p.support[0] * p.support[0];
+        half_so = p.fm_half_so;                                 // S O / 2
+        n_minus_s = p.fm_n_minus_s;
         ntx = (uint32_t)p.ntx; tlog = (uint32_t)p.key.tlog; tmask = (1u << p.key.tlog) - 1u;
         aux_bits = (uint32_t)p.key.aux_bits; bits_q = (uint32_t)p.key.bits_q; tile_shift = (uint32_t)p.key.tile_shift;
     }

@@ -8,26 +8,29 @@
 // inside a group of 32 channels x 8 integrations of one baseline; config 2, one integration: 2.0).
 //
 // So the visibilities are never sorted.  They are streamed once, in the order they are stored:
-//   gridder_bin   presum_plan_kernel   geometry only: per GROUP (one baseline, 32 consecutive channels, up to 8
-//                                      consecutive integrations) the exact map of every visibility, then which
+//   gridder_bin   presum_plan_kernel   geometry only: per GROUP (8 rows x 32 consecutive channels; a row is one
+//                                      (integration, baseline)) the exact map of every visibility, then which
 //                                      visibilities share a lattice point -> one FLAG BYTE per visibility and
 //                                      one key per partial RECORD
 //                 scan + compact       record keys to their final places (group order)
-//                 radix sort           of the RECORDS (key, record index) by tile and origin
-//   gridder_grid  presum_kernel        warp per group: lane = channel, 8 integrations in registers; visibilities,
-//                                      weights and flags are read fully coalesced, once; writes sum of w V per record
-//                 grid_kernel          on the sorted records (gathered through the index), then the flush
+//                 radix sort           of the RECORDS (key, slot of the record's sum) by tile and origin
+//   gridder_grid  presum_kernel        warp per group: lane = channel, 8 rows in registers; visibilities, weights and
+//                                      flags are read fully coalesced, once; writes sum of w V per record
+//                 grid_kernel          on the sorted records (gathered through the slot index), then the flush
 //
 // How a group finds its records (both kernels follow the same rules, the plan kernel from the keys, the
 // pre-summation kernel from the flag bytes):
-//   * lane = channel (column), rows r = 0..7 = integrations.  A T-RUN is a maximal run of equal keys down a
-//     column (the uv point moves on a line, so a lattice point is met once: a run).
-//   * a t-run of column f LINKS FORWARD to the t-run of column f + 1 with the same key, if there is one.  Only
-//     the first t-run of a key in its column takes part in links (a second one -- possible for adversarial
-//     inputs only -- becomes a record of its own), so every t-run has at most one predecessor.
+//   * lane = channel (column), rows r = 0..7.  A T-RUN is a maximal run of equal keys down a column (the uv point
+//     of a baseline moves on a line with the integration, so a lattice point is met once: a run).
+//   * a t-run of column f LINKS FORWARD to the t-run of column f + 1 that holds the same key in one of the run's
+//     own rows (the first such row decides).  Runs of one lattice point in neighbouring columns overlap in their
+//     rows or are strangers to each other -- then they stay two records, which costs a record, never correctness.
+//     A t-run of column f + 1 is linked to at most once (the first claimant in row order), so every t-run has at
+//     most one predecessor and chains cannot merge or loop.
 //   * a t-run with no predecessor is a CHAIN HEAD = one record; the record is the sum over its chain of
 //     t-runs, added in chain order: a fixed order, so results are bit-identical from run to run.
-//   * records of a group are numbered in (column, row) order of their heads.
+//   * records of a group are numbered in (column, row) order of their heads; record j's sum lives in the group's
+//     own visibility slots (slot_index), its staged key at a closed-form offset (stage_offset).
 // Flag byte of visibility (t, b, f), meaningful where a t-run starts (0 elsewhere):
 //   bit 0 has a forward link | bits 1-3 row where the linked t-run of column f + 1 starts |
 //   bit 4 t-run starts here | bit 5 chain head | bit 6 dropped (off the grid).
@@ -42,8 +45,9 @@ constexpr uint32_t kFlagLink = 1u, kFlagStart = 16u, kFlagHead = 32u, kFlagDrop 
 constexpr uint32_t kAbsent = 0xFFFFFFFFu;      // no visibility here (ragged group); never a key (see fast_key)
 
 // A group is 8 ROWS x 32 channels; a row is one (integration, baseline).  Rows of a group: rt integrations
-// (rt = min(8, n_time)) of each of rb = 8 / rt consecutive baselines, the integrations of a baseline next to each
-// other -- so 8 integrations of one baseline when there are that many, 8 baselines when there is one integration.
+// (at most 8, in t-blocks of equal size: make_geo) of each of rb = 8 / rt consecutive baselines, the integrations of
+// a baseline next to each other -- so 8 integrations of one baseline when there are that many, 8 baselines when
+// there is one integration.
 // (Summing visibilities with equal keys is valid whatever rows they come from.)
 struct PsGeo {
     uint32_t n_time, n_bl, n_chan;
