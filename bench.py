@@ -37,11 +37,12 @@ FLOP_PER_VIS_TAP = 16            # 4 pol x complex x (mul + add), real GCF table
 FP32_LANES_PER_SM = 128          # guide: 4 SMSP x 32 lanes, one FFMA per lane per clock
 BAND_HZ = 768 * 40.0e3           # one rank's band; rank r starts at 140 MHz + r * BAND_HZ
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures of this round
-# (profiles/r02_*_ncu_full.csv; historical, i.e. not measured by this run), keyed by kernel and config.
+# (profiles/r02_kernels_config4_ncu_full.csv; historical, i.e. not measured by this run), keyed by kernel and config.
 NCU_TRAFFIC_BYTES = {
-    ("presum_kernel", 4): 32_558_710_000,     # 29.794871 GB read + 2.763839 GB written
-    ("grid_kernel", 4): 5_966_465_000,        # 3.673973 GB read + 2.292492 GB written
-    ("presum_plan_kernel", 4): 1_285_268_000,  # 0.122242 GB read + 1.163026 GB written
+    # profiles/r02_kernels_config4_ncu_full.csv
+    ("presum_kernel", 4): 32_740_711_000,      # 29.974770 GB read + 2.765941 GB written
+    ("grid_kernel", 4): 6_326_859_000,         # 3.882851 GB read + 2.444008 GB written
+    ("presum_plan_kernel", 4): 1_298_758_000,  # 0.131762 GB read + 1.166996 GB written
 }
 
 
