@@ -278,11 +278,11 @@ def spawn_check(args) -> dict | None:
 class Loaded:
     """One config resident in HBM: inputs, plan, output grid."""
 
-    def __init__(self, cfg: int, dev, band: int = 0, tuning=None):
+    def __init__(self, cfg: int, dev, band: int = 0, tuning=None, n_bands: int = 1):
         import torch
         import synth
         from paper_1003_5575_b200 import gridder
-        wl = synth.make_workload(cfg, band=band)
+        wl = synth.make_workload(cfg, band=band, n_bands=n_bands)       # one cell size for all ranks' bands
         self.wl = wl
         nt, nb, nf = wl.n_time, wl.n_baseline, wl.n_chan
         self.vis = torch.empty((nt, nb, nf, 4, 2), dtype=torch.float32, device=dev)
@@ -421,7 +421,7 @@ def run_ours(args) -> dict | None:
     gridder.load_library()                       # fails loudly if libgridder.so is missing
 
     shard = shard_plan(world, rank)
-    L = Loaded(args.config, dev, band=shard["band"])
+    L = Loaded(args.config, dev, band=shard["band"], n_bands=world)
     wl, g = L.wl, L.g
     nt, nb, nf, n = wl.n_time, wl.n_baseline, wl.n_chan, wl.n_vis
     mfs_on = bool(args.mfs and world > 1)

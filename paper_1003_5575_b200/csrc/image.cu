@@ -54,7 +54,7 @@ CufftApi &cufft_api() {
 
 // out = in * (-1)^(x+y) [* corr[y] corr[x]]; float4 = two complex cells (x even, x+1), so the signs
 // inside one float4 are (s, s, -s, -s) with s = (-1)^y.
-__global__ void __launch_bounds__(256) centre_kernel(const float4 *__restrict__ in, float4 *__restrict__ out,
+__global__ void __launch_bounds__(256) centre_kernel(const float4 *in, float4 *out,       // (may be the same buffer: no __restrict__)
                                                       const float *__restrict__ corr, int n_grid, size_t n_f4) {
     const int half = n_grid >> 1;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_f4; i += (size_t)gridDim.x * blockDim.x) {

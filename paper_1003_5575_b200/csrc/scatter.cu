@@ -93,8 +93,8 @@ cudaError_t launch_scatter_atomic(Plan &p, const double *uvw, int n_time, int n_
 // Row f4: out[i] = (float) sum over the parts, in part order, in double (include/gridder.h).  One float4
 // per thread and part: HBM-bound, (n_parts + 1) x 4 len bytes.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) sum_parts_kernel(const float4 *__restrict__ parts, int n_parts, long long len4,
-                                                         long long stride4, float4 *__restrict__ out) {
+__global__ void __launch_bounds__(256) sum_parts_kernel(const float4 *parts, int n_parts, long long len4,
+                                                         long long stride4, float4 *out) {     // (out may alias part 0)
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < len4; i += (long long)gridDim.x * blockDim.x) {
         double a = 0.0, b = 0.0, c = 0.0, d = 0.0;
         for (int p = 0; p < n_parts; ++p) {

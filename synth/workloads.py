@@ -169,11 +169,13 @@ def config_shape(cfg: int) -> dict:
     return sp
 
 
-def make_workload(cfg: int, n_time: int | None = None, n_chan: int | None = None, band: int = 0) -> Workload:
+def make_workload(cfg: int, n_time: int | None = None, n_chan: int | None = None, band: int = 0, n_bands: int = 1) -> Workload:
     """Build config ``cfg``.  ``n_time`` / ``n_chan`` may shrink the sample axes (bounded CPU
     samples of the same workload); geometry, cell size and tables stay those of the full config.
     ``band`` > 0 moves the whole band up by ``band`` bandwidths (another GPU's channel block in the
-    paper's channel decomposition, PAPER.md :112-118); the cell size is fitted to that band."""
+    paper's channel decomposition, PAPER.md :112-118).  ``n_bands`` is the number of bands of the whole job: the
+    cell size is fitted to the top of the highest one, so that all ranks of a channel-sharded job grid onto the
+    SAME uv cells and their grids may be summed (multi-frequency synthesis)."""
     sp = _SPEC[cfg]
     rng = np.random.default_rng(SEED0 + cfg)
     enu = _antennas(cfg, rng, sp["n_ant"])
@@ -193,7 +195,8 @@ def make_workload(cfg: int, n_time: int | None = None, n_chan: int | None = None
         table = kernels.spheroidal_table(sp["support"], o).ravel()
         w_max, is_complex = 1.0, False
     # fit-to-grid cell size: no visibility of the full config is dropped
-    max_uv = float(np.abs(uvw[:, :, :2]).max() * freq.max() / C_M_PER_S)
+    top = sp["f0"] + (max(n_bands, band + 1) * sp["n_chan"] - 1) * sp["df"] if sp["n_chan"] > 1 else freq.max()
+    max_uv = float(np.abs(uvw[:, :, :2]).max() * max(top, freq.max()) / C_M_PER_S)
     n = sp["grid"]
     cell = max_uv / (n / 2 - max(support) / 2 - 2)
     # 20 sources, dN/dS ~ S^-2 on [0.1, 10] Jy, (l, m) uniform in (-0.3, 0.3)
