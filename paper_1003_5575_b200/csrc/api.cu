@@ -134,6 +134,8 @@ int derive(const gridder_config *cfg, const gridder_tuning *tuning, Plan &p) {
     while (k_auto > 256 && (int64_t)k_auto * 16384 > cfg->max_vis) k_auto >>= 1;
     p.chunk = t.chunk ? t.chunk : k_auto;
     p.warps_forced = t.max_warps;
+    // per-origin bins carried across the batches of the grid kernel (grid.cu stage_write_bins)
+    p.bins = (p.mode == 0 && p.merge && oo <= 16) ? 1 : 0;
     p.fold_batches = t.fold_batches ? t.fold_batches : 8;
 
     KeyLayout k;

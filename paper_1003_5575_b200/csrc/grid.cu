@@ -54,9 +54,12 @@ struct Geo {
     static constexpr int VF4 = 2;                              // float4 per staged visibility
     static constexpr int SLOT_F4 = VF4 + 1;                    // + (table offset of the NEXT record, origin)
     static constexpr int SLOTS = 36;                           // 32 records + sentinel + pad + look-ahead
-    static constexpr int RING_F4 = 2 * SLOTS * SLOT_F4;        // two halves
+    static constexpr int SLOTS_BINS = 52;                      // ... + the 16 records a carried origin's bins may add
     static constexpr int RAW_F4 = 32 * 2 + 8;                  // cp.async landing: 32 x {a, b}, 32 weights
-    static constexpr int WARP_F4 = 2 * CELLS_B + RING_F4 + RAW_F4;
+    static constexpr int BINS_F4 = 2 * 16;                     // per-origin bins (kernels with p.bins): [16 q][2] float4
+    __host__ __device__ static constexpr int warp_f4(bool bins) {
+        return 2 * CELLS_B + 2 * (bins ? SLOTS_BINS : SLOTS) * SLOT_F4 + RAW_F4 + (bins ? BINS_F4 : 0);
+    }
     static constexpr int SUB_BYTES = NA * NB * 32 * (CPLX ? 8 : 4);   // one (plane, sub-patch, q) sub-table
 };
 
@@ -280,6 +283,107 @@ __device__ __forceinline__ int stage_write(const GridParams &p, const float4 *ra
     return n_rec;
 }
 
+// stage_write with PER-ORIGIN BINS carried from batch to batch (fast path, O^2 <= 16, merging on).  A hot origin
+// has hundreds of entries but only O^2 different sets of taps; merging inside a batch of 32 still leaves up to
+// O^2 records per batch.  Here the records of the batch's LAST origin are not handed to the consumer: they go to
+// O^2 bins in shared memory (lane-distinct offsets after the batch merge: no two lanes touch a bin), the next
+// batches add to them while the origin lasts, and when it ends the non-empty bins become its records, in offset
+// order, ahead of the batch's own records -- the sorted order, so results stay bit-identical from run to run.
+// Every (item, origin, offset) is then gridded exactly once.  The last batch of an item carries nothing over.
+template <int NA, int NB, int NSUB, int TLOG, int MODE>
+__device__ __forceinline__ int stage_write_bins(const GridParams &p, const float4 *raw, float4 *half, int lane,
+                                                const Desc d, const Entry k, float4 *bins, int &bin_org, unsigned &bin_occ) {
+    using G = Geo<NA, NB, NSUB, TLOG, MODE>;
+    const int cnt = d.cnt();
+    const uint32_t tmask = (1u << TLOG) - 1u, qmask = (1u << (2 * p.key.bits_q)) - 1u;
+    const uint32_t x0l = (k.key >> p.key.aux_bits) & tmask, y0l = (k.key >> (p.key.aux_bits + TLOG)) & tmask;
+    const int q = (int)(k.key & qmask);
+    const int cstride = G::TMEM ? NA * NB : G::SUB_BYTES;            // table offset of offset q: q * cstride
+    const int poff = G::CIRC ? (int)((y0l << 8) | x0l) : (int)(y0l * G::RW + x0l);
+    const bool valid = lane < cnt;
+    const float4 ra = raw[lane], rb = raw[32 + lane];
+    const float w = p.weight ? reinterpret_cast<const float *>(raw + 64)[lane] : 1.0f;
+    const float o[8] = {ra.x * w, ra.y * w, ra.z * w, ra.w * w, rb.x * w, rb.y * w, rb.z * w, rb.w * w};
+    float sum[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) sum[i] = o[i];
+    // merge inside the batch (as stage_write)
+    const unsigned gkey = valid ? (((unsigned)poff << 8) | (unsigned)q) : (0xFFFF0000u | (unsigned)lane);
+    const unsigned grp = __match_any_sync(0xffffffffu, gkey);
+    bool keep = valid && (__ffs(grp) - 1 == lane);
+    unsigned rest = keep ? (grp & ~(1u << lane)) : 0u;
+    while (__any_sync(0xffffffffu, rest != 0u)) {
+        const int src = rest ? __ffs(rest) - 1 : lane;
+        const bool add = rest != 0u;
+        rest &= rest - 1u;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const float t = __shfl_sync(0xffffffffu, o[i], src);
+            if (add) sum[i] += t;
+        }
+    }
+    // (a) records of the carried origin join its bins
+    const bool to_old = keep && poff == bin_org;
+    if (to_old) {
+        float4 a = bins[2 * q], b = bins[2 * q + 1];
+        a.x += sum[0]; a.y += sum[1]; a.z += sum[2]; a.w += sum[3];
+        b.x += sum[4]; b.y += sum[5]; b.z += sum[6]; b.w += sum[7];
+        bins[2 * q] = a; bins[2 * q + 1] = b;
+    }
+    bin_occ |= __reduce_or_sync(0xffffffffu, to_old ? (1u << q) : 0u);
+    keep = keep && !to_old;
+    // (b) does the carried origin end here, and which origin is carried on?
+    const int tail_org = __shfl_sync(0xffffffffu, poff, cnt - 1);
+    const bool carry = !d.last();                              // the last batch of an item hands everything over
+    const bool flush_bins = bin_org >= 0 && (!carry || tail_org != bin_org);
+    const bool to_new = keep && carry && poff == tail_org && tail_org != bin_org;
+    const bool emit = keep && !to_new;
+    // (c) the ring: first the finished origin's bins in offset order, then the batch's own records
+    const unsigned occ = flush_bins ? bin_occ : 0u;
+    const int n_bin = __popc(occ);
+    const unsigned kept = __ballot_sync(0xffffffffu, emit);
+    const int n_rec = n_bin + __popc(kept);
+    GR_CHECK(p.counters, n_rec + 2 <= G::SLOTS_BINS);
+    const int first_kept_coff = kept ? __shfl_sync(0xffffffffu, q, __ffs(kept) - 1) * cstride : 0;
+    __syncwarp();
+    if (lane < 16 && ((occ >> lane) & 1u)) {
+        const unsigned higher = occ & ~((2u << lane) - 1u);
+        const int next_coff = higher ? (__ffs(higher) - 1) * cstride : first_kept_coff;
+        float4 *slot = half + __popc(occ & ((1u << lane) - 1u)) * G::SLOT_F4;
+        slot[0] = bins[2 * lane];
+        slot[1] = bins[2 * lane + 1];
+        slot[G::VF4] = make_float4(__int_as_float(next_coff), __int_as_float(bin_org), __int_as_float(lane * cstride), 0.f);
+        bins[2 * lane] = make_float4(0.f, 0.f, 0.f, 0.f);
+        bins[2 * lane + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    const unsigned above = kept & ~((2u << lane) - 1u);             // emitted lanes after this one
+    int next_coff = __shfl_sync(0xffffffffu, q, above ? __ffs(above) - 1 : lane) * cstride;
+    if (!above) next_coff = 0;
+    int last_poff = kept ? __shfl_sync(0xffffffffu, poff, 31 - __clz(kept | 1u)) : bin_org;
+    if (emit) {
+        float4 *slot = half + (n_bin + __popc(kept & ((1u << lane) - 1u))) * G::SLOT_F4;
+        slot[0] = make_float4(sum[0], sum[1], sum[2], sum[3]);
+        slot[1] = make_float4(sum[4], sum[5], sum[6], sum[7]);
+        slot[G::VF4] = make_float4(__int_as_float(next_coff), __int_as_float(poff), __int_as_float(q * cstride), 0.f);
+    }
+    if (lane < 2) {          // sentinel + pad (last batch of an item) or pad (odd count)
+        float4 *s2 = half + (n_rec + lane) * G::SLOT_F4;
+#pragma unroll
+        for (int i = 0; i < G::VF4; ++i) s2[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        s2[G::VF4] = make_float4(__int_as_float(0), __int_as_float(d.last() ? kSentinel : last_poff), __int_as_float(0), 0.f);
+    }
+    if (flush_bins) { bin_org = -1; bin_occ = 0; }
+    __syncwarp();
+    // (d) the batch's last origin moves into the (now empty) bins
+    if (to_new) {
+        bins[2 * q] = make_float4(sum[0], sum[1], sum[2], sum[3]);
+        bins[2 * q + 1] = make_float4(sum[4], sum[5], sum[6], sum[7]);
+    }
+    const unsigned moved = __reduce_or_sync(0xffffffffu, to_new ? (1u << q) : 0u);
+    if (moved) { bin_org = tail_org; bin_occ = moved; }
+    return n_rec;
+}
+
 // One staged record in registers: the weighted visibility (broadcast loads) and this lane's taps.
 template <int NA, int NB, int MODE>
 struct RecRegs {
@@ -474,16 +578,19 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
     extern __shared__ float4 smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int table_f4 = MODE == 0 ? p.coef_f4 : 0;
-    float4 *region = smem + table_f4 + warp * G::WARP_F4;      // plane A (XX, XY) then plane B (YX, YY)
+    const bool bins_on = !G::GEN && p.bins != 0;
+    const int slots = bins_on ? G::SLOTS_BINS : G::SLOTS, warp_f4 = G::warp_f4(bins_on);
+    float4 *region = smem + table_f4 + warp * warp_f4;         // plane A (XX, XY) then plane B (YX, YY)
     float4 *regA = region, *regB = region + G::CELLS_B;
     float4 *ring = region + 2 * G::CELLS_B;                    // 2 halves x SLOTS x VF4
-    float4 *raw = ring + G::RING_F4;                           // cp.async landing buffer
+    float4 *raw = ring + 2 * slots * G::SLOT_F4;               // cp.async landing buffer
+    float4 *bins = raw + G::RAW_F4;                            // (bins_on) sums of w V of the carried origin, per offset
 
     if (MODE == 0)
         for (int i = threadIdx.x; i < p.coef_f4; i += blockDim.x) smem[i] = p.coef[i];
     // everything is cleared: records are fetched one ahead, also past the end of a batch, and
     // whatever a slot holds must be a valid table offset
-    for (int i = lane; i < G::WARP_F4; i += 32) region[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int i = lane; i < warp_f4; i += 32) region[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     __syncthreads();
 
     const char *coef_lane;
@@ -550,17 +657,20 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
     eL.key = eL.idx = eL.aux = 0u;
     int par = 0, cur = -1, cmp = kSentinel;
     int rows_done = 0;                   // ring of rows: region rows of the current item already in its partial
+    int bin_org = -1;                    // (bins_on) origin the bins hold, -1: none
+    unsigned bin_occ = 0;                // ... and which of its offsets have something
     unsigned long long n_exec = 0;       // records gridded by this warp (after merging)
 
     while (true) {
-        const float4 *half = ring + par * (G::SLOTS * G::SLOT_F4);
+        const float4 *half = ring + par * (slots * G::SLOT_F4);
         // the batch that landed goes to the other half (last read one iteration ago)
         cp_async_wait_all();
         __syncwarp();
         Desc dS = dL;
         if (dS.cnt() > 0) {
-            const int n_rec = stage_write<NA, NB, NSUB, TLOG, MODE>(p, raw, ring + (par ^ 1) * (G::SLOTS * G::SLOT_F4),
-                                                                   lane, dS, eL);
+            float4 *other = ring + (par ^ 1) * (slots * G::SLOT_F4);
+            const int n_rec = bins_on ? stage_write_bins<NA, NB, NSUB, TLOG, MODE>(p, raw, other, lane, dS, eL, bins, bin_org, bin_occ)
+                                      : stage_write<NA, NB, NSUB, TLOG, MODE>(p, raw, other, lane, dS, eL);
             dS.bits = (dS.bits & ~63) | n_rec;          // the consumer sees the merged records
             n_exec += (unsigned)n_rec;
         }
@@ -723,10 +833,10 @@ __global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
 // Host side: kernel selection.  The register patch (NA x NB), the sub-patch count and the table
 // mode follow from the plan; TLOG is a plan parameter; the block size is chosen at run time.
 // ------------------------------------------------------------------------------------------
-size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps) {
+size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps, bool bins) {
     const int vf4 = 2;
     const int rows = (mode == 0 || mode == 3) ? 4 * g.NB : g.RH;       // fast path: a ring of SPY region rows (Geo::RHB)
-    const size_t per_warp = (size_t)(2 * g.RW * rows + 2 * 36 * (vf4 + 1) + 32 * 2 + 8) * sizeof(float4);   // Geo::WARP_F4
+    const size_t per_warp = (size_t)(2 * g.RW * rows + 2 * (bins ? 52 : 36) * (vf4 + 1) + 32 * 2 + 8 + (bins ? 32 : 0)) * sizeof(float4);   // Geo::warp_f4
     (void)tlog;
     return (mode == 0 ? table_bytes : 0) + per_warp * warps;
 }
@@ -802,11 +912,11 @@ cudaError_t configure_grid_kernel(Plan &p) {
         for (int w : kWarpChoices) {
             if (w > cap) continue;
             if (p.warps_forced > 0 && w > p.warps_forced) continue;      // the caller's limit (tuning, tests)
-            if (grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, w) <= (size_t)smem_max) { chosen = w; break; }
+            if (grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, w, p.bins != 0) <= (size_t)smem_max) { chosen = w; break; }
         }
         if (!chosen) return cudaErrorInvalidConfiguration;
         g.warps = chosen;
-        g.smem_bytes = (int)grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, chosen);
+        g.smem_bytes = (int)grid_smem_bytes(g, p.tlog, kernel_mode(p), p.coef_bytes, chosen, p.bins != 0);
         grid_fn_t fn = pick_grid(g, p.tlog, kernel_mode(p));
         if (!fn) return cudaErrorInvalidConfiguration;
         e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, g.smem_bytes);
@@ -848,6 +958,7 @@ cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *g
         gp.tmem_cols = p.tmem_cols;
         gp.merge = p.merge;
         gp.n_q = p.cfg.oversample * p.cfg.oversample;
+        gp.bins = p.bins;
         gp.n_sorted = (uint32_t)p.n_sorted;
         gp.n_src = (uint32_t)p.n_vis;                    // (record sums live in visibility slots: the same bound)
         gp.max_items_cls = (uint32_t)p.max_items_cls;

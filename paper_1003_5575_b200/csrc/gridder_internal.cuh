@@ -136,6 +136,7 @@ struct GridParams {
     int32_t tmem_cols;             // tensor-memory columns to allocate (MODE 3)
     int32_t n_q;                   // O^2 sub-tables
     int32_t merge;                 // sum entries of a batch with equal origin and table offset before gridding
+    int32_t bins;                  // ... and carry the last origin's sums from batch to batch (stage_write_bins)
     uint32_t n_sorted, n_src, max_items_cls;      // bounds (GRIDDER_CHECKED builds): sorted entries, gatherable slots, items
     KeyLayout key;
 };
@@ -170,6 +171,7 @@ struct Plan {
     int32_t n_grids, chans_per_grid;      // of the last bin (1, 0: plain gridder_bin)
     int32_t chunk;                 // K
     int32_t merge;                 // tuning.merge (default on)
+    int32_t bins;                  // per-origin bins in the grid kernel: fast path, merging on, O^2 <= 16
     // pre-summation in input order (presum.cu); presum == 0: not used by this plan
     int32_t presum;
     int32_t presum_active;         // the last gridder_bin took it: keys / vals hold the sorted RECORDS
@@ -264,6 +266,6 @@ cudaError_t launch_scatter_atomic(Plan &p, const double *uvw, int n_time, int n_
 cudaError_t configure_grid_kernel(Plan &p);          // picks warps/smem per class, sets the smem attribute
 cudaError_t launch_grid(Plan &p, const float *vis, const float *weight, float *grid, int accumulate,
                         cudaStream_t s);      // grid: [p.n_grids][4][N][N][2]
-size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps);
+size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps, bool bins);
 
 }  // namespace gridder
