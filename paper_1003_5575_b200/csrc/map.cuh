@@ -113,20 +113,6 @@ __device__ __forceinline__ VisMap map_vis(double u_m, double v_m, double w_m, do
     return m;
 }
 
-// Fast-path sort key of a mapped visibility (KeyLayout): tile, origin inside the
-// tile, and -- not sorted on -- drop flag and sub-cell offsets.
-// `gtile`: first tile id of the visibility's grid (gridder_bin_channels; 0 for one grid).
-__device__ __forceinline__ uint32_t fast_key(const VisMap &m, const MapParams &p, uint32_t gtile = 0) {
-    if (m.dropped)      // filed under tile 0, origin (0, 0)
-        return ((uint32_t)(p.drop_slot * p.n_tiles) << p.key.tile_shift) | (1u << (2 * p.key.bits_q));
-    const uint32_t tmask = (1u << p.key.tlog) - 1u;
-    const uint32_t x0 = (uint32_t)m.x0, y0 = (uint32_t)m.y0;
-    const uint32_t tile = (y0 >> p.key.tlog) * (uint32_t)p.ntx + (x0 >> p.key.tlog);
-    const uint32_t vtile = (uint32_t)(p.cls_slot[m.plane] * p.n_tiles) + gtile + tile;
-    return (vtile << p.key.tile_shift) | ((y0 & tmask) << (p.key.aux_bits + p.key.tlog)) |
-           ((x0 & tmask) << p.key.aux_bits) | ((uint32_t)m.qy << p.key.bits_q) | (uint32_t)m.qx;
-}
-
 // The production mapper of the pre-summed path: ONE fused multiply-add per axis.  Per channel the scale
 // ks = RN(RN(s rcp_cell) O) is formed once (O a power of two: the last product is exact); per visibility and axis
 //     t1 = RN(coord_m ks + (N/2 O + 1/2)).
@@ -140,49 +126,58 @@ __device__ __forceinline__ uint32_t fast_key(const VisMap &m, const MapParams &p
 // 1.5 * 2^52 trick: m = RN(t1 + M) holds RN(t1) in its low mantissa bits, d = t1 - (m - M) is exact.
 struct FastMap2 {
     double rcp_cell, d_o, chalf, eps, span2;
-    int o_shift, o_minus_1, half_so, n_minus_s;
-    uint32_t ntx, tmask, tlog, aux_bits, bits_q, tile_shift;
+    int b_off;                                                  // O - 1 - S O / 2
+    uint32_t b_lim;                                             // (N - S) O + O - 1: largest b on the grid
 
     __device__ __forceinline__ void init(const MapParams &p) {
         rcp_cell = p.rcp_cell; d_o = (double)p.oversample;
         chalf = p.fm_chalf;                                     // N/2 O + 1/2
         eps = p.fm_eps;                                         // 2^-47 N O
         span2 = p.fm_span2;
-        o_shift = p.o_shift; o_minus_1 = p.oversample - 1;
-        half_so = p.fm_half_so;                                 // S O / 2
-        n_minus_s = p.fm_n_minus_s;
-        ntx = (uint32_t)p.ntx; tlog = (uint32_t)p.key.tlog; tmask = (1u << p.key.tlog) - 1u;
-        aux_bits = (uint32_t)p.key.aux_bits; bits_q = (uint32_t)p.key.bits_q; tile_shift = (uint32_t)p.key.tile_shift;
+        b_off = p.oversample - 1 - p.fm_half_so;
+        b_lim = (uint32_t)(p.fm_n_minus_s * p.oversample + p.oversample - 1);
     }
     __device__ __forceinline__ double chan_scale(double s) const { return __dmul_rn(__dmul_rn(s, rcp_cell), d_o); }
-    // sort key of the visibility (fast_key's layout; a dropped visibility has the drop bit, 1 << 2 bits_q, set).
-    // Both axes are computed first and tested together: one branch per visibility.  Returns kUndecided where the
-    // screen does not decide: the caller then takes slow_key.
-    __device__ __forceinline__ uint32_t key(double u_m, double v_m, double ks, uint32_t gtile = 0) const {
+    // LATTICE CODE of the visibility: (by << 16) | bx with b = floor(t) - S O / 2 + O - 1 >= 0, i.e. patch origin
+    // x0 = bx / O and offset qx = x0 O + O - 1 - bx -- one word that is equal for two visibilities exactly when
+    // their sort keys are (N O <= 46340 on the fast path, so each axis fits 16 bits), and ten integer instructions
+    // cheaper to make than the key; key_of() turns it into the key where one is needed (the head of a record).
+    // kDropped: off the grid; kUndecided: the screen does not decide, the caller takes slow_lat.
+    // Both axes are computed first and tested together: one branch per visibility.
+    __device__ __forceinline__ uint32_t lat(double u_m, double v_m, double ks) const {
         const double kMagic = 6755399441055744.0;               // 1.5 * 2^52
         const double tx = __fma_rn(u_m, ks, chalf), ty = __fma_rn(v_m, ks, chalf);
         const double mx = __dadd_rn(tx, kMagic), my = __dadd_rn(ty, kMagic);
         const double dx = __dadd_rn(tx, -__dadd_rn(mx, -kMagic)), dy = __dadd_rn(ty, -__dadd_rn(my, -kMagic));
         if (fabs(tx) < span2 && fabs(ty) < span2 && fabs(dx) > eps && fabs(dy) > eps) {
             // floor(t) = RN(t) - (d < 0): the sign of d is the top bit of its high word
-            const int ax = __double2loint(mx) + (__double2hiint(dx) >> 31) - half_so;
-            const int ay = __double2loint(my) + (__double2hiint(dy) >> 31) - half_so;
-            const int x0 = (ax + o_minus_1) >> o_shift, y0 = (ay + o_minus_1) >> o_shift;     // ceil(a / O)
-            if ((unsigned)x0 > (unsigned)n_minus_s || (unsigned)y0 > (unsigned)n_minus_s)     // off the grid
-                return 1u << (2 * bits_q);                      // drop slot 0, tile 0, origin (0, 0)
-            const uint32_t qx = (uint32_t)((x0 << o_shift) - ax), qy = (uint32_t)((y0 << o_shift) - ay);
-            const uint32_t ux = (uint32_t)x0, uy = (uint32_t)y0;
-            const uint32_t tile = gtile + (uy >> tlog) * ntx + (ux >> tlog);
-            return (tile << tile_shift) | ((uy & tmask) << (aux_bits + tlog)) | ((ux & tmask) << aux_bits) |
-                   (qy << bits_q) | qx;
+            const int bx = __double2loint(mx) + (__double2hiint(dx) >> 31) + b_off;
+            const int by = __double2loint(my) + (__double2hiint(dy) >> 31) + b_off;
+            if ((unsigned)bx > b_lim || (unsigned)by > b_lim) return kDropped;       // off the grid
+            return ((uint32_t)by << 16) | (uint32_t)bx;
         }
         return kUndecided;                                      // rare: near a rounding boundary, or far away
     }
-    // what the caller maps such a visibility with (kept out of key() so that unrolled callers inline it once)
-    static __device__ __forceinline__ uint32_t slow_key(double u_m, double v_m, double s, const MapParams &p, uint32_t gtile = 0) {
-        return fast_key(map_vis(u_m, v_m, 0.0, s, p), p, gtile);
+    // the same from the definition's own mapper (kept out of lat() so that unrolled callers inline it once)
+    static __device__ __forceinline__ uint32_t slow_lat(double u_m, double v_m, double s, const MapParams &p) {
+        const VisMap m = map_vis(u_m, v_m, 0.0, s, p);
+        if (m.dropped) return kDropped;
+        const int o = p.oversample;
+        return ((uint32_t)(m.y0 * o - m.qy + o - 1) << 16) | (uint32_t)(m.x0 * o - m.qx + o - 1);
     }
-    static constexpr uint32_t kUndecided = 0xFFFFFFFEu;         // never a key (nor kAbsent of presum.cu)
+    // sort key (fast_key's layout) of a lattice code; `gtile`: first tile id of the visibility's grid
+    static __device__ __forceinline__ uint32_t key_of(uint32_t c, const MapParams &p, uint32_t gtile = 0) {
+        const uint32_t bx = c & 0xFFFFu, by = c >> 16, om1 = (uint32_t)p.oversample - 1u;
+        uint32_t x0, y0;
+        if (p.o_shift >= 0) { x0 = bx >> p.o_shift; y0 = by >> p.o_shift; }
+        else { x0 = bx / (uint32_t)p.oversample; y0 = by / (uint32_t)p.oversample; }
+        const uint32_t qx = x0 * (uint32_t)p.oversample + om1 - bx, qy = y0 * (uint32_t)p.oversample + om1 - by;
+        const uint32_t tmask = (1u << p.key.tlog) - 1u;
+        const uint32_t tile = gtile + (y0 >> p.key.tlog) * (uint32_t)p.ntx + (x0 >> p.key.tlog);
+        return (tile << p.key.tile_shift) | ((y0 & tmask) << (p.key.aux_bits + p.key.tlog)) | ((x0 & tmask) << p.key.aux_bits) |
+               (qy << p.key.bits_q) | qx;
+    }
+    static constexpr uint32_t kUndecided = 0xFFFFFFFEu, kDropped = 0xFFFFFFFDu;     // never lattice codes (nor kAbsent)
 };
 
 }  // namespace gridder

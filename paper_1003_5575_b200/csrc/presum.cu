@@ -42,7 +42,7 @@
 namespace gridder {
 
 constexpr uint32_t kFlagLink = 1u, kFlagStart = 16u, kFlagHead = 32u, kFlagDrop = 64u;
-constexpr uint32_t kAbsent = 0xFFFFFFFFu;      // no visibility here (ragged group); never a key (see fast_key)
+constexpr uint32_t kAbsent = 0xFFFFFFFFu;      // no visibility here (ragged group); never a lattice code (map.cuh)
 
 // A group is 8 ROWS x 32 channels; a row is one (integration, baseline).  Rows of a group: rt integrations
 // (at most 8, in t-blocks of equal size: make_geo) of each of rb = 8 / rt consecutive baselines, the integrations of
@@ -125,7 +125,6 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
                                                            uint32_t *__restrict__ count, Counters *counters) {
     const int lane = threadIdx.x & 31;
     const uint32_t gw = blockIdx.x * 8u + (threadIdx.x >> 5), nw = gridDim.x * 8u;
-    const uint32_t dropbit = 1u << (2 * p.key.bits_q);
     FastMap2 fm;
     if (FAST) fm.init(p);
     unsigned int dropped_here = 0, mapped_here = 0;
@@ -139,7 +138,7 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
         const double ks = FAST ? fm.chan_scale(s) : 0.0;
         // (gridder_bin_channels: the channel's grid is part of the tile id, so nothing merges across grids)
         const uint32_t gtile = p.chans_per_grid ? (f / (uint32_t)p.chans_per_grid) * (uint32_t)p.grid_tiles : 0u;
-        uint32_t key[8];
+        uint32_t key[8];                 // lattice codes (FastMap2::lat): equal exactly when the sort keys are
         uint32_t valid = 0, slow = 0;
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
@@ -147,7 +146,7 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
             uint32_t row;
             if (row_index<RT>(geo, r, t0, b0, row) && col) {
                 const double *L = uvw + (size_t)row * 3;
-                key[r] = FAST ? fm.key(__ldg(L), __ldg(L + 1), ks, gtile) : FastMap2::kUndecided;
+                key[r] = FAST ? fm.lat(__ldg(L), __ldg(L + 1), ks) : FastMap2::kUndecided;
                 if (key[r] == FastMap2::kUndecided) slow |= 1u << r;
                 valid |= 1u << r;
             }
@@ -158,20 +157,23 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
             uint32_t row;
             row_index<RT>(geo, r, t0, b0, row);
             const double *L = uvw + (size_t)row * 3;
-            const uint32_t k = FastMap2::slow_key(__ldg(L), __ldg(L + 1), s, p, gtile);
+            const uint32_t k = FastMap2::slow_lat(__ldg(L), __ldg(L + 1), s, p);
 #pragma unroll
             for (int rr = 0; rr < 8; ++rr)
                 if (rr == r) key[rr] = k;
         }
         // t-runs (bit r of th: a run starts in row r), dropped visibilities, rows whose key equals the next column's
         uint32_t th = 0, dropv = 0, eq = 0;
+        // (a chain stays inside one output grid: gridder_bin_channels)
+        const uint32_t next_gtile = __shfl_down_sync(0xffffffffu, gtile, 1);       // (every lane takes part)
+        const bool same_grid = lane < 31 && next_gtile == gtile;
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
             const uint32_t nk = __shfl_down_sync(0xffffffffu, key[r], 1);
             if (!((valid >> r) & 1u)) continue;
             if (r == 0 || key[r] != key[r - 1]) th |= 1u << r;
-            if (key[r] & dropbit) dropv |= 1u << r;
-            if (nk == key[r] && lane < 31) eq |= 1u << r;
+            if (key[r] == FastMap2::kDropped) dropv |= 1u << r;
+            if (nk == key[r] && same_grid) eq |= 1u << r;
         }
         const uint32_t drop = th & dropv;                   // dropped runs
         mapped_here += (unsigned)__popc(valid);
@@ -217,11 +219,17 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
                 row_index<RT>(geo, r, t0, b0, row);
                 GR_CHECK(counters, row * geo.n_chan + f < geo.n_vis);
                 flags[row * geo.n_chan + f] = (unsigned char)((r < 4 ? w_lo : w_hi) >> (8 * (r & 3)));
-                if (head & bit) {
-                    GR_CHECK(counters, (size_t)(st - stage) + idx < geo.n_vis);
-                    st[idx++] = key[r];
-                }
             }
+        }
+        // the sort keys of the records: only the heads need one (a ninth of the visibilities in config 4)
+        for (uint32_t m = head; m; m &= m - 1u) {
+            const int r = __ffs(m) - 1;
+            uint32_t c = key[0];
+#pragma unroll
+            for (int rr = 1; rr < 8; ++rr)
+                if (rr == r) c = key[rr];
+            GR_CHECK(counters, (size_t)(st - stage) + idx < geo.n_vis);
+            st[idx++] = FastMap2::key_of(c, p, gtile);
         }
     }
     for (int o = 16; o > 0; o >>= 1) {
@@ -384,10 +392,11 @@ __global__ void __launch_bounds__(256) map_presum_debug_kernel(const double *__r
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
         const long long tb = i / n_chan;
         const double s = __ddiv_rn(freq[(int)(i - tb * n_chan)], kSpeedOfLight);
-        uint32_t key = fm.key(uvw[tb * 3], uvw[tb * 3 + 1], fm.chan_scale(s));
-        if (key == FastMap2::kUndecided) key = FastMap2::slow_key(uvw[tb * 3], uvw[tb * 3 + 1], s, p);
+        uint32_t c = fm.lat(uvw[tb * 3], uvw[tb * 3 + 1], fm.chan_scale(s));
+        if (c == FastMap2::kUndecided) c = FastMap2::slow_lat(uvw[tb * 3], uvw[tb * 3 + 1], s, p);
+        const uint32_t key = c == FastMap2::kDropped ? 0u : FastMap2::key_of(c, p);
         int32_t *o = out + i * 6;
-        if (key & (1u << (2 * p.key.bits_q))) {
+        if (c == FastMap2::kDropped) {
             o[0] = o[1] = o[2] = o[3] = o[4] = 0; o[5] = 1;
         } else {
             const uint32_t tile = key >> p.key.tile_shift;
