@@ -86,6 +86,20 @@ __device__ __forceinline__ bool row_index(const PsGeo &g, int r, uint32_t t0, ui
     row = (t0 + rt) * g.n_bl + (b0 + rb);
     return (RT > 0 || rb < g.rb) && t0 + rt < g.n_time && b0 + rb < g.n_bl;
 }
+// The same relative to the group's first row: row = row0 + row_step<RT>(g, r), valid iff row_ok<RT>(g, r, nrt, nrb)
+// with nrt = n_time - t0, nrb = n_bl - b0 -- a multiply-add and a compare or two of uniform values per row.
+template <int RT>
+__device__ __forceinline__ uint32_t row_step(const PsGeo &g, int r) {
+    uint32_t rt, rb;
+    row_of<RT>(g, r, rt, rb);
+    return rt * g.n_bl + rb;
+}
+template <int RT>
+__device__ __forceinline__ bool row_ok(const PsGeo &g, int r, uint32_t nrt, uint32_t nrb) {
+    uint32_t rt, rb;
+    row_of<RT>(g, r, rt, rb);
+    return (RT > 0 || rb < g.rb) && rt < nrt && rb < nrb;
+}
 
 // Where the sum of record j of a group lives in ps_sum (an array as large as the visibility array): in the group's
 // own visibility slots, filled row segment by row segment -- so a group's records are contiguous runs of up to 32,
@@ -140,12 +154,13 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
         const uint32_t gtile = p.chans_per_grid ? (f / (uint32_t)p.chans_per_grid) * (uint32_t)p.grid_tiles : 0u;
         uint32_t key[8];                 // lattice codes (FastMap2::lat): equal exactly when the sort keys are
         uint32_t valid = 0, slow = 0;
+        const uint32_t row0 = t0 * geo.n_bl + b0, nrt = geo.n_time - t0, nrb = geo.n_bl - b0;
+        const double *L0 = uvw + (size_t)row0 * 3;
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
             key[r] = kAbsent;
-            uint32_t row;
-            if (row_index<RT>(geo, r, t0, b0, row) && col) {
-                const double *L = uvw + (size_t)row * 3;
+            if (row_ok<RT>(geo, r, nrt, nrb) && col) {
+                const double *L = L0 + (size_t)row_step<RT>(geo, r) * 3;
                 key[r] = FAST ? fm.lat(__ldg(L), __ldg(L + 1), ks) : FastMap2::kUndecided;
                 if (key[r] == FastMap2::kUndecided) slow |= 1u << r;
                 valid |= 1u << r;
@@ -168,13 +183,14 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
         const uint32_t next_gtile = __shfl_down_sync(0xffffffffu, gtile, 1);       // (every lane takes part)
         const bool same_grid = lane < 31 && next_gtile == gtile;
 #pragma unroll
-        for (int r = 0; r < 8; ++r) {
+        for (int r = 0; r < 8; ++r) {          // (branch-free: the masks are cut to the valid rows afterwards)
             const uint32_t nk = __shfl_down_sync(0xffffffffu, key[r], 1);
-            if (!((valid >> r) & 1u)) continue;
-            if (r == 0 || key[r] != key[r - 1]) th |= 1u << r;
-            if (key[r] == FastMap2::kDropped) dropv |= 1u << r;
-            if (nk == key[r] && same_grid) eq |= 1u << r;
+            th |= (uint32_t)(r == 0 || key[r] != key[r - 1]) << r;
+            dropv |= (uint32_t)(key[r] == FastMap2::kDropped) << r;
+            eq |= (uint32_t)(nk == key[r]) << r;
         }
+        th &= valid;
+        eq &= same_grid ? valid : 0u;
         const uint32_t drop = th & dropv;                   // dropped runs
         mapped_here += (unsigned)__popc(valid);
         dropped_here += (unsigned)__popc(dropv);
@@ -215,10 +231,9 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
         for (int r = 0; r < 8; ++r) {
             const uint32_t bit = 1u << r;
             if (valid & bit) {
-                uint32_t row;
-                row_index<RT>(geo, r, t0, b0, row);
-                GR_CHECK(counters, row * geo.n_chan + f < geo.n_vis);
-                flags[row * geo.n_chan + f] = (unsigned char)((r < 4 ? w_lo : w_hi) >> (8 * (r & 3)));
+                const uint32_t i = (row0 + row_step<RT>(geo, r)) * geo.n_chan + f;
+                GR_CHECK(counters, i < geo.n_vis);
+                flags[i] = (unsigned char)((r < 4 ? w_lo : w_hi) >> (8 * (r & 3)));
             }
         }
         // the sort keys of the records: only the heads need one (a ninth of the visibilities in config 4)
@@ -313,6 +328,7 @@ __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__r
         const uint32_t f = f0 + (uint32_t)lane;
         const bool col = f < geo.n_chan;
         // everything the group needs is requested at once: 8 rows x (32 B + 4 B + 1 B) per lane
+        const uint32_t row0 = t0 * geo.n_bl + b0, nrt = geo.n_time - t0, nrb = geo.n_bl - b0;
         float4 va[8], vb[8];
         float w[8];
         uint32_t fl[8];
@@ -321,9 +337,8 @@ __global__ void __launch_bounds__(kPsWarps * 32) presum_kernel(const float4 *__r
             va[r] = vb[r] = make_float4(0.f, 0.f, 0.f, 0.f);
             w[r] = 0.f;
             fl[r] = 0u;
-            uint32_t row;
-            if (row_index<RT>(geo, r, t0, b0, row) && col) {
-                const size_t i = (size_t)(row * geo.n_chan + f);
+            if (row_ok<RT>(geo, r, nrt, nrb) && col) {
+                const size_t i = (size_t)((row0 + row_step<RT>(geo, r)) * geo.n_chan + f);
                 GR_CHECK(counters, i < geo.n_vis);
                 va[r] = ld_stream4(vis + 2 * i);
                 vb[r] = ld_stream4(vis + 2 * i + 1);
