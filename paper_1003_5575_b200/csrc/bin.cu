@@ -192,11 +192,25 @@ cudaError_t launch_map_debug(const Plan &p, const double *uvw, int n_time, int n
 __global__ void __launch_bounds__(256) tile_bounds_kernel(const uint32_t *__restrict__ keys, long long n,
                                                            int tile_shift, uint32_t *__restrict__ tile_start,
                                                            uint32_t *__restrict__ tile_end) {
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
-         i += (long long)gridDim.x * blockDim.x) {
-        const uint32_t t = keys[i] >> tile_shift;
-        if (i == 0 || (keys[i - 1] >> tile_shift) != t) tile_start[t] = (uint32_t)i;
-        if (i == n - 1 || (keys[i + 1] >> tile_shift) != t) tile_end[t] = (uint32_t)(i + 1);
+    // four keys per thread (one 16-byte load), the neighbours of the quad with two scalar loads
+    const long long n4 = (n + 3) / 4;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n4; q += (long long)gridDim.x * blockDim.x) {
+        const long long i0 = 4 * q;
+        uint32_t t[6];                                        // tiles of entries i0 - 1 .. i0 + 4 (0xFFFFFFFF: none)
+        if (i0 + 4 <= n) {
+            const uint4 k = *reinterpret_cast<const uint4 *>(keys + i0);
+            t[1] = k.x >> tile_shift; t[2] = k.y >> tile_shift; t[3] = k.z >> tile_shift; t[4] = k.w >> tile_shift;
+        } else {
+            for (int j = 0; j < 4; ++j) t[1 + j] = i0 + j < n ? keys[i0 + j] >> tile_shift : 0xFFFFFFFFu;
+        }
+        t[0] = i0 > 0 ? keys[i0 - 1] >> tile_shift : 0xFFFFFFFFu;
+        t[5] = i0 + 4 < n ? keys[i0 + 4] >> tile_shift : 0xFFFFFFFFu;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (i0 + j >= n) break;
+            if (t[j] != t[1 + j]) tile_start[t[1 + j]] = (uint32_t)(i0 + j);
+            if (t[2 + j] != t[1 + j]) tile_end[t[1 + j]] = (uint32_t)(i0 + j + 1);
+        }
     }
 }
 
