@@ -370,6 +370,7 @@ int gridder_destroy(gridder_plan_t *plan) {
     collect_violations(p);
     image_destroy(*p);
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+    if (p->count_ev) cudaEventDestroy(p->count_ev);
     for (int r = 0; r < kProfRing; ++r)
         for (int i = 0; i < 10; ++i) if (p->ev[r][i]) cudaEventDestroy(p->ev[r][i]);
     delete p;

@@ -182,6 +182,7 @@ struct Plan {
     int64_t n_sorted;              // entries of the sorted list of the last bin (records, or visibilities)
     unsigned char *ps_flags;       // [max_vis] one flag byte per visibility
     uint32_t *ps_count, *ps_base;  // [ps_group_cap + 1] records per group and their exclusive scan
+    cudaEvent_t count_ev;          // recorded when the record count has reached the host (the one wait of gridder_bin)
     int32_t fold_batches;          // longest FP32 register chain, in batches of 32 entries (power of 2)
     int32_t warps_forced, n_sm;
     int64_t max_items;             // capacity of the work-item table (all classes)

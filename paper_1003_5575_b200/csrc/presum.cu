@@ -133,7 +133,7 @@ __device__ __forceinline__ uint32_t warp_excl(uint32_t x, int lane, uint32_t &to
 }
 
 template <bool FAST, int RT>
-__global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__restrict__ uvw, const double *__restrict__ scale,
+__global__ void __launch_bounds__(256, 5) presum_plan_kernel(const double *__restrict__ uvw, const double *__restrict__ scale,
                                                            const PsGeo geo, const MapParams p,
                                                            unsigned char *__restrict__ flags, uint32_t *__restrict__ stage,
                                                            uint32_t *__restrict__ count, Counters *counters) {
@@ -143,6 +143,7 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
     if (FAST) fm.init(p);
     unsigned int dropped_here = 0, mapped_here = 0;
 
+    const uint32_t g_end_all = geo.n_groups;
     for (uint32_t grp = gw; grp < geo.n_groups; grp += nw) {
         uint32_t t0, b0, f0;
         group_coords(geo, grp, t0, b0, f0);
@@ -156,6 +157,11 @@ __global__ void __launch_bounds__(256, 4) presum_plan_kernel(const double *__res
         uint32_t valid = 0, slow = 0;
         const uint32_t row0 = t0 * geo.n_bl + b0, nrt = geo.n_time - t0, nrb = geo.n_bl - b0;
         const double *L0 = uvw + (size_t)row0 * 3;
+        if (grp + nw < g_end_all && lane < 8) {         // the uvw rows of the group this warp takes next: into L1 now
+            uint32_t nt0, nb0, nf0, nrow;
+            group_coords(geo, grp + nw, nt0, nb0, nf0);
+            if (row_index<RT>(geo, lane, nt0, nb0, nrow)) asm volatile("prefetch.global.L1 [%0];" :: "l"(uvw + (size_t)nrow * 3));
+        }
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
             key[r] = kAbsent;
@@ -469,7 +475,7 @@ cudaError_t presum_scan_temp_bytes(int64_t n, size_t *bytes) {
 }
 
 // gridder_bin of a pre-summed plan, first half: flags, record keys (compacted into keys[0] / vals[0]) and the
-// record count (*n_rec, read back: the stream is synchronised once).
+// record count (*n_rec, read back: the host waits once, for the count; the compaction is still running then).
 cudaError_t launch_presum_plan(Plan &p, const double *uvw, const double *scale, int n_time, int n_bl, int n_chan,
                                cudaStream_t s, long long *n_rec) {
     const PsGeo geo = make_geo(n_time, n_bl, n_chan);
@@ -493,11 +499,15 @@ cudaError_t launch_presum_plan(Plan &p, const double *uvw, const double *scale, 
     size_t tb = p.cub_temp_bytes;
     GR_TRY(cub::DeviceScan::ExclusiveSum(p.cub_temp, tb, (const uint32_t *)p.ps_count, p.ps_base,
                                          (long long)geo.n_groups + 1, s));
+    // the record count goes to the host as soon as the scan is done; the host waits for THAT (an event), not for the
+    // compaction enqueued behind it, so the sort is enqueued while the compaction still runs and the GPU never idles
     unsigned int total = 0;
+    if (!p.count_ev) GR_TRY(cudaEventCreateWithFlags(&p.count_ev, cudaEventDisableTiming));
     GR_TRY(cudaMemcpyAsync(&total, p.ps_base + geo.n_groups, sizeof(unsigned int), cudaMemcpyDeviceToHost, s));
+    GR_TRY(cudaEventRecord(p.count_ev, s));
     presum_compact_kernel<<<blocks, 256, 0, s>>>(stage, p.ps_count, p.ps_base, geo, p.keys[0], (uint32_t *)p.vals[0], p.counters);
     GR_TRY(cudaGetLastError());
-    GR_TRY(cudaStreamSynchronize(s));
+    GR_TRY(cudaEventSynchronize(p.count_ev));
     p.n_launches += 3;
     *n_rec = (long long)total;
     return cudaSuccess;
