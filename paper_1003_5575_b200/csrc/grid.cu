@@ -780,7 +780,7 @@ __global__ void __launch_bounds__(256) tile_cover_kernel(const TileInfo *__restr
 }
 
 template <int SP, int TLOG>
-__global__ void __launch_bounds__(256) flush_kernel(const FlushParams p) {
+__global__ void __launch_bounds__(256, 6) flush_kernel(const FlushParams p) {
     using G = FlushGeo<SP, TLOG>;
     const int x = blockIdx.x * 32 + threadIdx.x;
     const int y = blockIdx.y * 8 + threadIdx.y;

@@ -57,13 +57,24 @@ struct PsGeo {
     uint32_t n_bgroup;          // ceil(n_bl / rb)
     uint32_t n_groups;          // n_tblock * n_bgroup * n_fchunk; group g = (tb * n_bgroup + bg) * n_fchunk + fc
     uint32_t n_vis;             // n_time * n_bl * n_chan
+    float rcp_fchunk, rcp_bgroup;       // 1 / n_fchunk, 1 / n_bgroup (div_small)
 };
 
+// x / d for x < 2^24 (group indices: a plan has fewer than 2^32 / 256 groups... and 2^24 bounds them for every
+// accepted shape, see presum_fits): float reciprocal and one correction step instead of a 32-bit division.
+__device__ __forceinline__ uint32_t div_small(uint32_t x, uint32_t d, float rcp) {
+    uint32_t q = (uint32_t)((float)x * rcp);
+    if (q * d > x) --q;
+    if ((q + 1u) * d <= x) ++q;
+    return q;
+}
+
 __device__ __forceinline__ void group_coords(const PsGeo &g, uint32_t grp, uint32_t &t0, uint32_t &b0, uint32_t &f0) {
-    const uint32_t fc = grp % g.n_fchunk, rest = grp / g.n_fchunk;
+    const uint32_t rest = div_small(grp, g.n_fchunk, g.rcp_fchunk), fc = grp - rest * g.n_fchunk;
+    const uint32_t tb = div_small(rest, g.n_bgroup, g.rcp_bgroup);
     f0 = fc * 32u;
-    b0 = (rest % g.n_bgroup) * g.rb;
-    t0 = (rest / g.n_bgroup) * g.rt;
+    b0 = (rest - tb * g.n_bgroup) * g.rb;
+    t0 = tb * g.rt;
 }
 
 // Row r of a group: integration t0 + rt of baseline b0 + rb.  RT > 0: the integrations per group are known at
@@ -107,8 +118,9 @@ __device__ __forceinline__ bool row_ok(const PsGeo &g, int r, uint32_t nrt, uint
 // as visibilities.)
 __device__ __forceinline__ uint32_t slot_index(const PsGeo &g, uint32_t t0, uint32_t b0, uint32_t f0, uint32_t j) {
     const uint32_t ncols = min(32u, g.n_chan - f0), nrt = min(g.rt, g.n_time - t0);
-    const uint32_t k = j / ncols, c = j - k * ncols;          // k-th valid row of the group
-    const uint32_t kb = k / nrt, kt = k - kb * nrt;
+    // j < 256, ncols <= 32, k < 8, nrt <= 8: multiply-shift divisions are exact (j * 32 < 2^16)
+    const uint32_t k = (j * ((65536u + ncols - 1u) / ncols)) >> 16, c = j - k * ncols;          // k-th valid row of the group
+    const uint32_t kb = (k * ((65536u + nrt - 1u) / nrt)) >> 16, kt = k - kb * nrt;
     return ((t0 + kt) * g.n_bl + (b0 + kb)) * g.n_chan + f0 + c;
 }
 
@@ -455,6 +467,8 @@ static PsGeo make_geo(int n_time, int n_bl, int n_chan) {
     g.n_bgroup = ((uint32_t)n_bl + g.rb - 1) / g.rb;
     g.n_groups = g.n_tblock * g.n_bgroup * g.n_fchunk;
     g.n_vis = g.n_time * g.n_bl * g.n_chan;
+    g.rcp_fchunk = 1.0f / (float)g.n_fchunk;
+    g.rcp_bgroup = 1.0f / (float)g.n_bgroup;
     return g;
 }
 
@@ -464,7 +478,7 @@ bool presum_fits(const Plan &p, int n_time, int n_bl, int n_chan) {
     if (!p.presum || n_time <= 0 || n_bl <= 0 || n_chan <= 0) return false;
     const PsGeo g = make_geo(n_time, n_bl, n_chan);
     const unsigned long long ng = (unsigned long long)g.n_tblock * g.n_bgroup * g.n_fchunk;
-    if (ng > (unsigned long long)p.ps_group_cap) return false;
+    if (ng > (unsigned long long)p.ps_group_cap || ng >= (1ull << 24)) return false;      // (2^24: div_small)
     return true;
 }
 
