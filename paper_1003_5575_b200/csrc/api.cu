@@ -128,11 +128,12 @@ int derive(const gridder_config *cfg, const gridder_tuning *tuning, Plan &p) {
             while ((size_t)p.tmem_cols < cols) p.tmem_cols *= 2;
         }
     }
-    // K: most entries per work item, ~ max_vis / 2^14 as a power of two in [256, 8192]: small inputs get
-    // short items so that a hot tile still spreads over the ~1800 resident warps; the largest get 8192
-    // (2048 when the entries are partial records: shorter items balance the end of the grid kernel), which bounds the partial regions the flush has to sum for
-    // the cells of a hot tile (the accuracy budget of DESIGN.md section 7 holds up to 8192)
-    int k_auto = 2048;
+    // K: most entries per work item, ~ max_vis / 2^14 as a power of two in [256, 4096]: small inputs get
+    // short items so that a hot tile still spreads over the ~1800 resident warps; larger K means fewer partial
+    // regions for the flush, smaller K a better balanced end of the grid kernel (warps claim one item at a time);
+    // measured on configs 3 and 4, 2048 .. 8192 are within 1 % of each other (the accuracy budget of DESIGN.md
+    // section 7 holds up to 8192)
+    int k_auto = 4096;
     while (k_auto > 256 && (int64_t)k_auto * 16384 > cfg->max_vis) k_auto >>= 1;
     p.chunk = t.chunk ? t.chunk : k_auto;
     p.warps_forced = t.max_warps;
