@@ -138,7 +138,7 @@ int derive(const gridder_config *cfg, const gridder_tuning *tuning, Plan &p) {
     p.chunk = t.chunk ? t.chunk : k_auto;
     p.warps_forced = t.max_warps;
     // per-origin bins carried across the batches of the grid kernel (grid.cu stage_write_bins)
-    p.bins = (p.mode == 0 && p.merge && oo <= 16) ? 1 : 0;
+    p.bins = (p.merge && oo <= 16) ? 1 : 0;
     p.fold_batches = t.fold_batches ? t.fold_batches : 8;
 
     KeyLayout k;
@@ -155,6 +155,8 @@ int derive(const gridder_config *cfg, const gridder_tuning *tuning, Plan &p) {
     k.total_bits = k.tile_shift + k.tile_bits;
     if (k.total_bits > 32) return GRIDDER_ERR_UNSUPPORTED;
     p.key = k;
+    // general path: a carried run is (plane, origin), so the sort must keep the entries of a plane together
+    if (p.mode != 0 && ((cfg->n_wplanes > 1 && k.plane_bits == 0) || k.tile_shift > 26)) p.bins = 0;
 
     const int64_t n = cfg->max_vis;
     const int64_t n_vtiles = (int64_t)p.n_tiles_cls * p.n_cls;

@@ -33,10 +33,14 @@ __global__ void relayout_kernel(const float *__restrict__ table, float *__restri
         const int qy = q / O, qx = q % O;
         const int ty = 4 * NB * (sub / nsub) + (lane >> 3) + 4 * b;
         const int tx = 8 * NA * (sub % nsub) + (lane & 7) + 8 * a;
+        // a lane's NB * E floats: contiguous, except 8 floats (complex, NB = 4) = two float4 kept 32 lanes apart
+        // ([a][j][lane][4]) so that each of the warp's two 128-bit loads is one contiguous 512-byte run
+        size_t o = (size_t)i * E;
+        if (NB * E == 8) o = ((((size_t)(sub * O * O + q) * NA + a) * 2 + (b >> 1)) * 32 + lane) * 4 + (b & 1) * 2;
         for (int e = 0; e < E; ++e) {
             float v = 0.f;
             if (ty < S && tx < S) v = table[((size_t)(qy + ty * O) * (S * O) + (qx + tx * O)) * E + e];
-            coef[(size_t)i * E + e] = v;
+            coef[o + e] = v;
         }
     }
 }
@@ -98,8 +102,8 @@ __global__ void __launch_bounds__(256) map_kernel(const double *__restrict__ uvw
         }
         keys[i] = key;
         if (GENERAL) {
-            uint32_t aux = m.dropped ? (1u << 30)
-                                     : p.tab_off256[m.plane] + (uint32_t)(m.qy * p.oversample + m.qx) * p.q_units[m.plane];
+            const uint32_t q = (uint32_t)(m.qy * p.oversample + m.qx);
+            uint32_t aux = m.dropped ? (1u << 30) : (p.tab_off256[m.plane] + q * p.q_units[m.plane]) | ((q & 63u) << kAuxQShift);
             if (m.conj) aux |= 1u << 31;
             reinterpret_cast<uint2 *>(vals)[i] = make_uint2(i, aux);
         } else {

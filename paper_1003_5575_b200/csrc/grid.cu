@@ -54,9 +54,11 @@ struct Geo {
     static constexpr int VF4 = 2;                              // float4 per staged visibility
     static constexpr int SLOT_F4 = VF4 + 1;                    // + (table offset of the NEXT record, origin)
     static constexpr int SLOTS = 36;                           // 32 records + sentinel + pad + look-ahead
-    static constexpr int SLOTS_BINS = 52;                      // ... + the 16 records a carried origin's bins may add
+    static constexpr int NBINS = GEN ? 32 : 16;                // bins of a carried run: sub-cell offsets (x conjugate)
+    static constexpr int SLOTS_BINS = SLOTS + NBINS;           // ... + the records a carried run's bins may add
     static constexpr int RAW_F4 = 32 * 2 + 8;                  // cp.async landing: 32 x {a, b}, 32 weights
-    static constexpr int BINS_F4 = 2 * 16;                     // per-origin bins (kernels with p.bins): [16 q][2] float4
+    static constexpr int BINS_F4 = 2 * NBINS + (GEN ? NBINS / 4 : 0);   // per-run bins (kernels with p.bins): [bin][2] float4
+                                                               // (+ general path: the table offset of each bin)
     __host__ __device__ static constexpr int warp_f4(bool bins) {
         return 2 * CELLS_B + 2 * (bins ? SLOTS_BINS : SLOTS) * SLOT_F4 + RAW_F4 + (bins ? BINS_F4 : 0);
     }
@@ -221,7 +223,7 @@ __device__ __forceinline__ int stage_write(const GridParams &p, const float4 *ra
     if (G::GEN) {
         x0l = k.key & tmask;
         y0l = (k.key >> TLOG) & tmask;
-        coff = (int)((k.aux & 0x3fffffffu) << 8);          // table offset in 256-byte units
+        coff = (int)((k.aux & kAuxOffMask) << 8);          // table offset in 256-byte units
         if (G::CPLX) coff |= (int)(k.aux >> 31);           // bit 0: use the conjugate table (w < 0)
     } else {
         const uint32_t qmask = (1u << (2 * p.key.bits_q)) - 1u;
@@ -284,23 +286,37 @@ __device__ __forceinline__ int stage_write(const GridParams &p, const float4 *ra
     return n_rec;
 }
 
-// stage_write with PER-ORIGIN BINS carried from batch to batch (fast path, O^2 <= 16, merging on).  A hot origin
-// has hundreds of entries but only O^2 different sets of taps; merging inside a batch of 32 still leaves up to
-// O^2 records per batch.  Here the records of the batch's LAST origin are not handed to the consumer: they go to
-// O^2 bins in shared memory (lane-distinct offsets after the batch merge: no two lanes touch a bin), the next
-// batches add to them while the origin lasts, and when it ends the non-empty bins become its records, in offset
+// stage_write with PER-ORIGIN BINS carried from batch to batch (O^2 <= 16, merging on).  A hot origin
+// has hundreds of entries but only O^2 different sets of taps (x 2 with conjugated w-planes); merging inside a
+// batch of 32 still leaves up to that many records per batch.  Here the records of the batch's LAST run -- entries
+// of one origin (general path: one origin of one plane; the sort puts them next to each other) -- are not handed to
+// the consumer: they go to bins in shared memory (lane-distinct after the batch merge: no two lanes touch a bin),
+// the next batches add to them while the run lasts, and when it ends the non-empty bins become its records, in bin
 // order, ahead of the batch's own records -- the sorted order, so results stay bit-identical from run to run.
-// Every (item, origin, offset) is then gridded exactly once.  The last batch of an item carries nothing over.
+// Every (item, plane, origin, offset) is then gridded exactly once.  The last batch of an item carries nothing over.
 template <int NA, int NB, int NSUB, int TLOG, int MODE>
 __device__ __forceinline__ int stage_write_bins(const GridParams &p, const float4 *raw, float4 *half, int lane,
-                                                const Desc d, const Entry k, float4 *bins, int &bin_org, unsigned &bin_occ) {
+                                                const Desc d, const Entry k, float4 *bins, int &bin_org, int &bin_poff,
+                                                unsigned &bin_occ) {
     using G = Geo<NA, NB, NSUB, TLOG, MODE>;
     const int cnt = d.cnt();
-    const uint32_t tmask = (1u << TLOG) - 1u, qmask = (1u << (2 * p.key.bits_q)) - 1u;
-    const uint32_t x0l = (k.key >> p.key.aux_bits) & tmask, y0l = (k.key >> (p.key.aux_bits + TLOG)) & tmask;
-    const int q = (int)(k.key & qmask);
-    const int cstride = G::TMEM ? NA * NB : G::SUB_BYTES;            // table offset of offset q: q * cstride
-    const int poff = G::CIRC ? (int)((y0l << 8) | x0l) : (int)(y0l * G::RW + x0l);
+    const uint32_t tmask = (1u << TLOG) - 1u;
+    int poff, org, bin, coff;           // region offset of the origin | identity of the run | bin of the run | table offset
+    if (G::GEN) {
+        const uint32_t x0l = k.key & tmask, y0l = (k.key >> TLOG) & tmask;
+        poff = (int)(y0l * G::RW + x0l);
+        org = (int)(k.key & ((1u << p.key.tile_shift) - 1u));                  // plane | y0l | x0l
+        bin = (int)(((k.aux >> kAuxQShift) & 15u) | ((k.aux >> 31) << 4));      // offset, conjugate
+        coff = (int)((k.aux & kAuxOffMask) << 8) | (int)(k.aux >> 31);
+    } else {
+        const uint32_t qmask = (1u << (2 * p.key.bits_q)) - 1u;
+        const uint32_t x0l = (k.key >> p.key.aux_bits) & tmask, y0l = (k.key >> (p.key.aux_bits + TLOG)) & tmask;
+        poff = (int)((y0l << 8) | x0l);
+        org = poff;
+        bin = (int)(k.key & qmask);
+        coff = bin * (G::TMEM ? NA * NB : G::SUB_BYTES);
+    }
+    int *bin_coff = reinterpret_cast<int *>(bins + 2 * G::NBINS);             // (general path) table offset of a bin
     const bool valid = lane < cnt;
     const float4 ra = raw[lane], rb = raw[32 + lane];
     const float w = p.weight ? reinterpret_cast<const float *>(raw + 64)[lane] : 1.0f;
@@ -309,7 +325,7 @@ __device__ __forceinline__ int stage_write_bins(const GridParams &p, const float
 #pragma unroll
     for (int i = 0; i < 8; ++i) sum[i] = o[i];
     // merge inside the batch (as stage_write)
-    const unsigned gkey = valid ? (((unsigned)poff << 8) | (unsigned)q) : (0xFFFF0000u | (unsigned)lane);
+    const unsigned gkey = valid ? (((unsigned)org << 5) | (unsigned)bin) : (0xF0000000u | (unsigned)lane);
     const unsigned grp = __match_any_sync(0xffffffffu, gkey);
     bool keep = valid && (__ffs(grp) - 1 == lane);
     unsigned rest = keep ? (grp & ~(1u << lane)) : 0u;
@@ -323,49 +339,54 @@ __device__ __forceinline__ int stage_write_bins(const GridParams &p, const float
             if (add) sum[i] += t;
         }
     }
-    // (a) records of the carried origin join its bins
-    const bool to_old = keep && poff == bin_org;
+    // (a) records of the carried run join its bins
+    const bool to_old = keep && org == bin_org;
     if (to_old) {
-        float4 a = bins[2 * q], b = bins[2 * q + 1];
+        float4 a = bins[2 * bin], b = bins[2 * bin + 1];
         a.x += sum[0]; a.y += sum[1]; a.z += sum[2]; a.w += sum[3];
         b.x += sum[4]; b.y += sum[5]; b.z += sum[6]; b.w += sum[7];
-        bins[2 * q] = a; bins[2 * q + 1] = b;
+        bins[2 * bin] = a; bins[2 * bin + 1] = b;
+        if (G::GEN) bin_coff[bin] = coff;
     }
-    bin_occ |= __reduce_or_sync(0xffffffffu, to_old ? (1u << q) : 0u);
+    bin_occ |= __reduce_or_sync(0xffffffffu, to_old ? (1u << bin) : 0u);
     keep = keep && !to_old;
-    // (b) does the carried origin end here, and which origin is carried on?
-    const int tail_org = __shfl_sync(0xffffffffu, poff, cnt - 1);
+    // (b) does the carried run end here, and which run is carried on?
+    const int tail_org = __shfl_sync(0xffffffffu, org, cnt - 1);
+    const int tail_poff = __shfl_sync(0xffffffffu, poff, cnt - 1);
     const bool carry = !d.last();                              // the last batch of an item hands everything over
     const bool flush_bins = bin_org >= 0 && (!carry || tail_org != bin_org);
-    const bool to_new = keep && carry && poff == tail_org && tail_org != bin_org;
+    const bool to_new = keep && carry && org == tail_org && tail_org != bin_org;
     const bool emit = keep && !to_new;
-    // (c) the ring: first the finished origin's bins in offset order, then the batch's own records
+    // (c) the ring: first the finished run's bins in bin order, then the batch's own records
     const unsigned occ = flush_bins ? bin_occ : 0u;
     const int n_bin = __popc(occ);
     const unsigned kept = __ballot_sync(0xffffffffu, emit);
     const int n_rec = n_bin + __popc(kept);
     GR_CHECK(p.counters, n_rec + 2 <= G::SLOTS_BINS);
-    const int first_kept_coff = kept ? __shfl_sync(0xffffffffu, q, __ffs(kept) - 1) * cstride : 0;
+    const int first_kept_coff = kept ? __shfl_sync(0xffffffffu, coff, __ffs(kept) - 1) : 0;
     __syncwarp();
-    if (lane < 16 && ((occ >> lane) & 1u)) {
+    if (lane < G::NBINS && ((occ >> lane) & 1u)) {
         const unsigned higher = occ & ~((2u << lane) - 1u);
-        const int next_coff = higher ? (__ffs(higher) - 1) * cstride : first_kept_coff;
+        const int hb = higher ? __ffs(higher) - 1 : 0;
+        const int cstride = G::TMEM ? NA * NB : G::SUB_BYTES;
+        const int next_coff = higher ? (G::GEN ? bin_coff[hb] : hb * cstride) : first_kept_coff;
         float4 *slot = half + __popc(occ & ((1u << lane) - 1u)) * G::SLOT_F4;
         slot[0] = bins[2 * lane];
         slot[1] = bins[2 * lane + 1];
-        slot[G::VF4] = make_float4(__int_as_float(next_coff), __int_as_float(bin_org), __int_as_float(lane * cstride), 0.f);
+        slot[G::VF4] = make_float4(__int_as_float(next_coff), __int_as_float(bin_poff),
+                                   __int_as_float(G::GEN ? bin_coff[lane] : lane * cstride), 0.f);
         bins[2 * lane] = make_float4(0.f, 0.f, 0.f, 0.f);
         bins[2 * lane + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
     const unsigned above = kept & ~((2u << lane) - 1u);             // emitted lanes after this one
-    int next_coff = __shfl_sync(0xffffffffu, q, above ? __ffs(above) - 1 : lane) * cstride;
+    int next_coff = __shfl_sync(0xffffffffu, coff, above ? __ffs(above) - 1 : lane);
     if (!above) next_coff = 0;
-    int last_poff = kept ? __shfl_sync(0xffffffffu, poff, 31 - __clz(kept | 1u)) : bin_org;
+    int last_poff = kept ? __shfl_sync(0xffffffffu, poff, 31 - __clz(kept | 1u)) : bin_poff;
     if (emit) {
         float4 *slot = half + (n_bin + __popc(kept & ((1u << lane) - 1u))) * G::SLOT_F4;
         slot[0] = make_float4(sum[0], sum[1], sum[2], sum[3]);
         slot[1] = make_float4(sum[4], sum[5], sum[6], sum[7]);
-        slot[G::VF4] = make_float4(__int_as_float(next_coff), __int_as_float(poff), __int_as_float(q * cstride), 0.f);
+        slot[G::VF4] = make_float4(__int_as_float(next_coff), __int_as_float(poff), __int_as_float(coff), 0.f);
     }
     if (lane < 2) {          // sentinel + pad (last batch of an item) or pad (odd count)
         float4 *s2 = half + (n_rec + lane) * G::SLOT_F4;
@@ -375,13 +396,14 @@ __device__ __forceinline__ int stage_write_bins(const GridParams &p, const float
     }
     if (flush_bins) { bin_org = -1; bin_occ = 0; }
     __syncwarp();
-    // (d) the batch's last origin moves into the (now empty) bins
+    // (d) the batch's last run moves into the (now empty) bins
     if (to_new) {
-        bins[2 * q] = make_float4(sum[0], sum[1], sum[2], sum[3]);
-        bins[2 * q + 1] = make_float4(sum[4], sum[5], sum[6], sum[7]);
+        bins[2 * bin] = make_float4(sum[0], sum[1], sum[2], sum[3]);
+        bins[2 * bin + 1] = make_float4(sum[4], sum[5], sum[6], sum[7]);
+        if (G::GEN) bin_coff[bin] = coff;
     }
-    const unsigned moved = __reduce_or_sync(0xffffffffu, to_new ? (1u << q) : 0u);
-    if (moved) { bin_org = tail_org; bin_occ = moved; }
+    const unsigned moved = __reduce_or_sync(0xffffffffu, to_new ? (1u << bin) : 0u);
+    if (moved) { bin_org = tail_org; bin_poff = tail_poff; bin_occ = moved; }
     return n_rec;
 }
 
@@ -436,9 +458,11 @@ struct RecRegs {
                     asm("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(c[a][0]), "=f"(c[a][1]) : "r"(sa));
                 }
             } else {                                           // global memory through L1
+                // (CF == 8: the two float4 of a lane are 512 bytes apart, [j][lane][4], so that each warp load is one
+                // contiguous 512-byte run -- bin.cu relayout_kernel)
 #pragma unroll
                 for (int j = 0; j < CF / 4; ++j) {
-                    const float4 t = __ldg(reinterpret_cast<const float4 *>(ca) + j);
+                    const float4 t = __ldg(reinterpret_cast<const float4 *>(ca) + j * 32);
                     c[a][4 * j] = t.x; c[a][4 * j + 1] = t.y; c[a][4 * j + 2] = t.z; c[a][4 * j + 3] = t.w;
                 }
                 if (CF == 2) {
@@ -579,7 +603,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
     extern __shared__ float4 smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int table_f4 = MODE == 0 ? p.coef_f4 : 0;
-    const bool bins_on = !G::GEN && p.bins != 0;
+    const bool bins_on = p.bins != 0;
     const int slots = bins_on ? G::SLOTS_BINS : G::SLOTS, warp_f4 = G::warp_f4(bins_on);
     float4 *region = smem + table_f4 + warp * warp_f4;         // plane A (XX, XY) then plane B (YX, YY)
     float4 *regA = region, *regB = region + G::CELLS_B;
@@ -636,7 +660,8 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
         coef_lane = reinterpret_cast<const char *>((uintptr_t)((uint32_t)__cvta_generic_to_shared(smem) +
                                                               lane * RecRegs<NA, NB, MODE>::CF * (int)sizeof(float)));
     else
-        coef_lane = reinterpret_cast<const char *>(p.coef) + lane * RecRegs<NA, NB, MODE>::CF * (int)sizeof(float);
+        coef_lane = reinterpret_cast<const char *>(p.coef) +
+                    lane * (RecRegs<NA, NB, MODE>::CF > 4 ? 4 : RecRegs<NA, NB, MODE>::CF) * (int)sizeof(float);
 
     float acc[NA][NB][8];
 #pragma unroll
@@ -658,7 +683,8 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
     eL.key = eL.idx = eL.aux = 0u;
     int par = 0, cur = -1, cmp = kSentinel;
     int rows_done = 0;                   // ring of rows: region rows of the current item already in its partial
-    int bin_org = -1;                    // (bins_on) origin the bins hold, -1: none
+    int bin_org = -1;                    // (bins_on) run the bins hold (origin; general path: plane | origin), -1: none
+    int bin_poff = 0;                    // ... and its origin's region offset
     unsigned bin_occ = 0;                // ... and which of its offsets have something
     unsigned long long n_exec = 0;       // records gridded by this warp (after merging)
 
@@ -670,7 +696,7 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
         Desc dS = dL;
         if (dS.cnt() > 0) {
             float4 *other = ring + (par ^ 1) * (slots * G::SLOT_F4);
-            const int n_rec = bins_on ? stage_write_bins<NA, NB, NSUB, TLOG, MODE>(p, raw, other, lane, dS, eL, bins, bin_org, bin_occ)
+            const int n_rec = bins_on ? stage_write_bins<NA, NB, NSUB, TLOG, MODE>(p, raw, other, lane, dS, eL, bins, bin_org, bin_poff, bin_occ)
                                       : stage_write<NA, NB, NSUB, TLOG, MODE>(p, raw, other, lane, dS, eL);
             dS.bits = (dS.bits & ~63) | n_rec;          // the consumer sees the merged records
             n_exec += (unsigned)n_rec;
@@ -836,8 +862,10 @@ __global__ void __launch_bounds__(256, 6) flush_kernel(const FlushParams p) {
 // ------------------------------------------------------------------------------------------
 size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes, int warps, bool bins) {
     const int vf4 = 2;
+    const bool gen = mode == 1 || mode == 2;
+    const int nbins = gen ? 32 : 16;                                   // Geo::NBINS
     const int rows = (mode == 0 || mode == 3) ? 4 * g.NB : g.RH;       // fast path: a ring of SPY region rows (Geo::RHB)
-    const size_t per_warp = (size_t)(2 * g.RW * rows + 2 * (bins ? 52 : 36) * (vf4 + 1) + 32 * 2 + 8 + (bins ? 32 : 0)) * sizeof(float4);   // Geo::warp_f4
+    const size_t per_warp = (size_t)(2 * g.RW * rows + 2 * (bins ? 36 + nbins : 36) * (vf4 + 1) + 32 * 2 + 8 + (bins ? 2 * nbins + (gen ? nbins / 4 : 0) : 0)) * sizeof(float4);   // Geo::warp_f4
     (void)tlog;
     return (mode == 0 ? table_bytes : 0) + per_warp * warps;
 }

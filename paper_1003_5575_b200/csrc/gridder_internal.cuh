@@ -37,6 +37,12 @@ constexpr int kMaxPlanes = 64;
 constexpr int kMaxChannels = 1 << 16;              // per gridder_bin call (frequency scale table)
 constexpr int kMaxClasses = 3;                    // padded patch 8 (S <= 8), 16 (S <= 16), 32 = 2x2 x 16
 
+// General path, second word of a sorted value ("aux"): bits 0..23 table offset in 256-byte units (tables < 2 GB:
+// derive()), 24..29 sub-cell offset q = qy O + qx (names a bin of the carried run, grid.cu stage_write_bins),
+// 30 dropped, 31 conjugate table (w < 0).
+constexpr int kAuxQShift = 24;
+constexpr uint32_t kAuxOffMask = (1u << kAuxQShift) - 1u;
+
 // Bit layout of a sort key (LSB first): [aux: qx, qy (bits_q each), drop flag -- fast path only],
 // x0l, y0l (tlog each), plane (plane_bits, may be 0), virtual tile = class slot * n_tiles + tile.
 struct KeyLayout {
