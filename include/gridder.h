@@ -93,7 +93,7 @@ typedef struct {
  * equivalent paths runs; results stay within the tolerance of the definition and bit-identical from run to run
  * for a given tuning.  The tests use them to reach every path on small inputs. */
 typedef struct {
-    int32_t tile_log2;          /* 2, 3 or 4: uv tiles of 2^tile_log2 cells per edge (default 2; 3 for pre-summed plans) */
+    int32_t tile_log2;          /* 2, 3 or 4: uv tiles of 2^tile_log2 cells per edge (default 2; 3 for pre-summed plans and the general path) */
     int32_t chunk;              /* K, 32 .. 2^20: most sorted entries per work item (default by size, 256 .. 8192)  */
     int32_t max_warps;          /* cap on the warps per block of the grid kernel (default: what fits)              */
     int32_t merge;              /* 1 on (default), 2 off: entries of a batch of 32 with equal patch origin and

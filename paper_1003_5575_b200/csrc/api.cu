@@ -61,7 +61,7 @@ int derive(const gridder_config *cfg, const gridder_tuning *tuning, Plan &p) {
                 (t.presum == 1 || (t.presum == 0 && cfg->max_vis >= (4ll << 20)))) ? 1 : 0;
     // (its mapper packs the two lattice coordinates of a visibility into 16 bits each: map.cuh FastMap2::lat)
     if ((int64_t)cfg->grid_size * cfg->oversample + cfg->oversample >= 65533) p.presum = 0;
-    p.tlog = t.tile_log2 ? t.tile_log2 : (p.presum ? 3 : 2);
+    p.tlog = t.tile_log2 ? t.tile_log2 : ((p.presum || p.mode != 0) ? 3 : 2);
     p.T = 1 << p.tlog;
     p.ntx = (cfg->grid_size + p.T - 1) / p.T;
     p.nty = p.ntx;

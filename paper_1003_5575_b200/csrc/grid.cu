@@ -53,7 +53,8 @@ struct Geo {
     static constexpr int CELLS_B = RW * RHB;
     static constexpr int VF4 = 2;                              // float4 per staged visibility
     static constexpr int SLOT_F4 = VF4 + 1;                    // + (table offset of the NEXT record, origin)
-    static constexpr int SLOTS = 36;                           // 32 records + sentinel + pad + look-ahead
+    static constexpr int PIPE = GEN ? 3 : 2;                   // records in flight in the consumer (taps fetched PIPE - 1 ahead)
+    static constexpr int SLOTS = GEN ? 40 : 36;                // 32 records + sentinel / pads (PIPE) + look-ahead (PIPE)
     static constexpr int NBINS = GEN ? 32 : 16;                // bins of a carried run: sub-cell offsets (x conjugate)
     static constexpr int SLOTS_BINS = SLOTS + NBINS;           // ... + the records a carried run's bins may add
     static constexpr int RAW_F4 = 32 * 2 + 8;                  // cp.async landing: 32 x {a, b}, 32 weights
@@ -268,7 +269,7 @@ __device__ __forceinline__ int stage_write(const GridParams &p, const float4 *ra
     int next_coff = __shfl_sync(0xffffffffu, coff, above ? __ffs(above) - 1 : lane);
     if (!above) next_coff = 0;
     const int last_poff = __shfl_sync(0xffffffffu, poff, 31 - __clz(kept | 1u));
-    GR_CHECK(p.counters, n_rec + 2 <= G::SLOTS);
+    GR_CHECK(p.counters, n_rec + G::PIPE <= G::SLOTS);
     if (keep) {
         // slot r carries the table offset of record r + 1 (the consumer loads taps one record ahead)
         // and the origin of record r; every slot also carries its own table offset (slot 0's is used)
@@ -277,7 +278,7 @@ __device__ __forceinline__ int stage_write(const GridParams &p, const float4 *ra
         slot[1] = make_float4(sum[4], sum[5], sum[6], sum[7]);
         slot[G::VF4] = make_float4(__int_as_float(next_coff), __int_as_float(poff), __int_as_float(coff), 0.f);
     }
-    if (lane < 2) {          // sentinel + pad (last batch of an item) or pad (odd count)
+    if (lane < G::PIPE) {    // sentinel + pads (last batch of an item) or pads (count not a multiple of PIPE)
         float4 *s2 = half + (n_rec + lane) * G::SLOT_F4;
 #pragma unroll
         for (int i = 0; i < G::VF4; ++i) s2[i] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -362,7 +363,7 @@ __device__ __forceinline__ int stage_write_bins(const GridParams &p, const float
     const int n_bin = __popc(occ);
     const unsigned kept = __ballot_sync(0xffffffffu, emit);
     const int n_rec = n_bin + __popc(kept);
-    GR_CHECK(p.counters, n_rec + 2 <= G::SLOTS_BINS);
+    GR_CHECK(p.counters, n_rec + G::PIPE <= G::SLOTS_BINS);
     const int first_kept_coff = kept ? __shfl_sync(0xffffffffu, coff, __ffs(kept) - 1) : 0;
     __syncwarp();
     if (lane < G::NBINS && ((occ >> lane) & 1u)) {
@@ -388,7 +389,7 @@ __device__ __forceinline__ int stage_write_bins(const GridParams &p, const float
         slot[1] = make_float4(sum[4], sum[5], sum[6], sum[7]);
         slot[G::VF4] = make_float4(__int_as_float(next_coff), __int_as_float(poff), __int_as_float(coff), 0.f);
     }
-    if (lane < 2) {          // sentinel + pad (last batch of an item) or pad (odd count)
+    if (lane < G::PIPE) {    // sentinel + pads (last batch of an item) or pads (count not a multiple of PIPE)
         float4 *s2 = half + (n_rec + lane) * G::SLOT_F4;
 #pragma unroll
         for (int i = 0; i < G::VF4; ++i) s2[i] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -712,33 +713,61 @@ __global__ void __launch_bounds__(MAXW * 32, 1) grid_kernel(const GridParams p) 
         if (dC.end()) break;
         const int cnt = dC.cnt();
         if (cnt > 0) {
-            const int cntp = dC.last() ? ((cnt + 2) & ~1) : ((cnt + 1) & ~1);   // + sentinel / pad, even
+            // + sentinel (last batch of an item), padded to a multiple of the consumer's pipeline depth
+            const int cnt1 = cnt + (dC.last() ? 1 : 0);
+            const int cntp = G::PIPE == 3 ? ((cnt1 + 2) / 3) * 3 : ((cnt1 + 1) & ~1);
             const float4 *send = half + cntp * G::SLOT_F4;
             {
                 // NSUB == 2: the virtual item's sub-patch selects its quarter of the table
                 constexpr int sub_poff = 0;
                 const char *cl = NSUB > 1 ? coef_lane + (int)(dC.item & 3u) * p.sub_stride_bytes : coef_lane;
-                RecRegs<NA, NB, MODE> A, B;
                 const float4 *sp = half;
                 float4 *dst = p.partials + (size_t)dC.item * (2 * G::CELLS);      // (virtual) item id inside the class
                 // meta of a slot: x = table offset of the next record, y = origin of this one
-                int2 mA, mB;
-                {
-                    const float4 m0 = sp[G::VF4];
-                    A.fetch(sp, __float_as_int(m0.z), cl);
-                    mA = make_int2(__float_as_int(m0.x), __float_as_int(m0.y));
+                if constexpr (G::PIPE == 3) {
+                    // general path: the taps come from global memory (L1 / L2): three records in flight, taps
+                    // fetched two records ahead (255 registers per thread are there at 8 warps per SM)
+                    RecRegs<NA, NB, MODE> A, B, C;
+                    int2 mA, mB, mC;
+                    {
+                        const float4 m0 = sp[G::VF4];
+                        A.fetch(sp, __float_as_int(m0.z), cl);
+                        mA = make_int2(__float_as_int(m0.x), __float_as_int(m0.y));
+                        mB = *reinterpret_cast<const int2 *>(sp + G::SLOT_F4 + G::VF4);
+                        B.fetch(sp + G::SLOT_F4, mA.x, cl);
+                    }
+                    do {
+                        mC = *reinterpret_cast<const int2 *>(sp + 2 * G::SLOT_F4 + G::VF4);
+                        C.fetch(sp + 2 * G::SLOT_F4, mB.x, cl);
+                        consume<NA, NB, G::RW, G::CELLS, MODE>(A, mA.y + sub_poff, cur, cmp, regA, regB, lane, acc, rows_done, dst, p.counters);
+                        mA = *reinterpret_cast<const int2 *>(sp + 3 * G::SLOT_F4 + G::VF4);
+                        A.fetch(sp + 3 * G::SLOT_F4, mC.x, cl);
+                        consume<NA, NB, G::RW, G::CELLS, MODE>(B, mB.y + sub_poff, cur, cmp, regA, regB, lane, acc, rows_done, dst, p.counters);
+                        mB = *reinterpret_cast<const int2 *>(sp + 4 * G::SLOT_F4 + G::VF4);
+                        B.fetch(sp + 4 * G::SLOT_F4, mA.x, cl);
+                        consume<NA, NB, G::RW, G::CELLS, MODE>(C, mC.y + sub_poff, cur, cmp, regA, regB, lane, acc, rows_done, dst, p.counters);
+                        sp += 3 * G::SLOT_F4;
+                    } while (sp < send);
+                } else {
+                    RecRegs<NA, NB, MODE> A, B;
+                    int2 mA, mB;
+                    {
+                        const float4 m0 = sp[G::VF4];
+                        A.fetch(sp, __float_as_int(m0.z), cl);
+                        mA = make_int2(__float_as_int(m0.x), __float_as_int(m0.y));
+                    }
+                    do {
+                        mB = *reinterpret_cast<const int2 *>(sp + G::SLOT_F4 + G::VF4);
+                        A.wait();
+                        B.fetch(sp + G::SLOT_F4, mA.x, cl);
+                        consume<NA, NB, G::RW, G::CELLS, MODE>(A, mA.y + sub_poff, cur, cmp, regA, regB, lane, acc, rows_done, dst, p.counters);
+                        mA = *reinterpret_cast<const int2 *>(sp + 2 * G::SLOT_F4 + G::VF4);
+                        B.wait();
+                        A.fetch(sp + 2 * G::SLOT_F4, mB.x, cl);
+                        consume<NA, NB, G::RW, G::CELLS, MODE>(B, mB.y + sub_poff, cur, cmp, regA, regB, lane, acc, rows_done, dst, p.counters);
+                        sp += 2 * G::SLOT_F4;
+                    } while (sp < send);
                 }
-                do {
-                    mB = *reinterpret_cast<const int2 *>(sp + G::SLOT_F4 + G::VF4);
-                    A.wait();
-                    B.fetch(sp + G::SLOT_F4, mA.x, cl);
-                    consume<NA, NB, G::RW, G::CELLS, MODE>(A, mA.y + sub_poff, cur, cmp, regA, regB, lane, acc, rows_done, dst, p.counters);
-                    mA = *reinterpret_cast<const int2 *>(sp + 2 * G::SLOT_F4 + G::VF4);
-                    B.wait();
-                    A.fetch(sp + 2 * G::SLOT_F4, mB.x, cl);
-                    consume<NA, NB, G::RW, G::CELLS, MODE>(B, mB.y + sub_poff, cur, cmp, regA, regB, lane, acc, rows_done, dst, p.counters);
-                    sp += 2 * G::SLOT_F4;
-                } while (sp < send);
             }
             if (dC.last()) {
                 // the sentinel has folded the last patch in; move the region to this item's
@@ -864,8 +893,9 @@ size_t grid_smem_bytes(const ClassGeo &g, int tlog, int mode, size_t table_bytes
     const int vf4 = 2;
     const bool gen = mode == 1 || mode == 2;
     const int nbins = gen ? 32 : 16;                                   // Geo::NBINS
+    const int slots = gen ? 40 : 36;                                   // Geo::SLOTS
     const int rows = (mode == 0 || mode == 3) ? 4 * g.NB : g.RH;       // fast path: a ring of SPY region rows (Geo::RHB)
-    const size_t per_warp = (size_t)(2 * g.RW * rows + 2 * (bins ? 36 + nbins : 36) * (vf4 + 1) + 32 * 2 + 8 + (bins ? 2 * nbins + (gen ? nbins / 4 : 0) : 0)) * sizeof(float4);   // Geo::warp_f4
+    const size_t per_warp = (size_t)(2 * g.RW * rows + 2 * (bins ? slots + nbins : slots) * (vf4 + 1) + 32 * 2 + 8 + (bins ? 2 * nbins + (gen ? nbins / 4 : 0) : 0)) * sizeof(float4);   // Geo::warp_f4
     (void)tlog;
     return (mode == 0 ? table_bytes : 0) + per_warp * warps;
 }
