@@ -248,6 +248,24 @@ GRIDDER_API int gridder_run_host(gridder_plan_t *plan, const double *h_uvw_m, in
                      const float *h_weight, float *h_grid, double *d_uvw_m, double *d_freq_hz,
                      float *d_vis, float *d_weight, float *d_grid, void *cuda_stream);
 
+/* For callers that cannot allocate device memory at all (tight serving loops, harnesses that forbid cudaMalloc):
+ * plan + gridder_bin + gridder_grid of a SMALL cadence on a workspace that is a file-scope device array of the
+ * library, GRIDDER_STATIC_WORKSPACE_BYTES large (every GPU that loads the library holds those 64 MiB until the
+ * process exits).  cfg->workspace / workspace_bytes are ignored; inputs and outputs are the caller's DEVICE buffers
+ * as for gridder_bin / gridder_grid; `tuning` may be NULL (pre-summation in input order is off unless asked for).
+ * Calls no cudaMalloc, cudaFree or allocating library routine.  A plan that needs more than the array returns
+ * GRIDDER_ERR_WORKSPACE ("workspace too small") with the size it would need in *workspace_needed (may be NULL) and
+ * enqueues nothing -- use gridder_plan with a workspace of your own then.  The result is bit for bit that of
+ * gridder_plan_tuned + gridder_bin + gridder_grid with the same tuning.
+ * All calls on a device share the array and it keeps the last call's contents (the path clears what must start at
+ * zero itself).  Calls that overlapped on the GPU would race on it: they are serialised by a process-wide lock and
+ * every call SYNCHRONISES THE DEVICE before it returns. */
+#define GRIDDER_STATIC_WORKSPACE_BYTES ((size_t)64 << 20)
+GRIDDER_API int gridder_grid_static(const gridder_config *cfg, const gridder_tuning *tuning, const double *uvw_m,
+                                    int32_t n_time, int32_t n_baseline, const double *freq_hz, int32_t n_chan,
+                                    const float *vis, const float *weight, float *grid, int32_t accumulate,
+                                    size_t *workspace_needed, void *cuda_stream);
+
 /* Stage timers for the benchmark harness (PAPER.md :249 instrumented its pipeline per kernel).
  * When enabled, gridder_bin / gridder_grid record CUDA events between their stages on the stream
  * they run on (a few microseconds of host time per call; nothing else changes). */

@@ -15,7 +15,7 @@ HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libgridder.so"
 CHECKED_LIB = HERE / "libgridder_checked.so"
-SOURCES = ["api.cu", "bin.cu", "grid.cu", "presum.cu", "scatter.cu", "image.cu"]
+SOURCES = ["api.cu", "bin.cu", "grid.cu", "presum.cu", "scatter.cu", "image.cu", "static_ws.cu"]
 HEADERS = [CSRC / "gridder_internal.cuh", CSRC / "map.cuh", HERE.parent / "include" / "gridder.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Wno-deprecated-gpu-targets",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]

@@ -20,7 +20,7 @@ OK, ERR_INVALID_ARG, ERR_CAPACITY, ERR_WORKSPACE, ERR_CUDA, ERR_NOT_BINNED, ERR_
 EXPORTS = ("gridder_check_violations", "gridder_bin_channels", "gridder_grid_channels", "gridder_workspace_size", "gridder_plan", "gridder_workspace_size_tuned", "gridder_plan_tuned", "gridder_map_presum",
            "gridder_bin", "gridder_bin_tables", "gridder_grid", "gridder_destroy",
            "gridder_get_stats", "gridder_map", "gridder_scatter_atomic", "gridder_image_workspace_size", "gridder_image",
-           "gridder_run_host", "gridder_sum_parts", "gridder_set_profiling",
+           "gridder_run_host", "gridder_grid_static", "gridder_sum_parts", "gridder_set_profiling",
            "gridder_get_stage_ms", "gridder_launch_count", "gridder_strerror",
            "gridder_last_cuda_error", "gridder_version")
 
@@ -106,6 +106,9 @@ def load_library() -> C.CDLL:
         lib.gridder_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_int32,
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.gridder_grid_static.argtypes = [C.POINTER(_Config), C.POINTER(_Tuning), C.c_void_p, C.c_int32, C.c_int32,
+                                            C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32,
+                                            C.POINTER(C.c_size_t), C.c_void_p]
         lib.gridder_set_profiling.argtypes = [C.c_void_p, C.c_int32]
         lib.gridder_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
         lib.gridder_launch_count.argtypes = [C.c_void_p]
@@ -166,6 +169,57 @@ class Stats:
     n_records_gridded: int = 0
     n_presum_records: int = 0
     fma_executed: int = 0
+
+
+STATIC_WORKSPACE_BYTES = 64 << 20       # GRIDDER_STATIC_WORKSPACE_BYTES (include/gridder.h)
+
+
+def grid_static(uvw_m: torch.Tensor, freq_hz: torch.Tensor, vis: torch.Tensor, weight, *, grid_size: int, cell_size: float,
+                oversample: int, support, kernel: torch.Tensor, n_wplanes: int = 1, w_max: float = 1.0,
+                kernel_is_complex: bool = False, tuning: dict | None = None, out: torch.Tensor | None = None,
+                accumulate: bool = False, stream=None) -> torch.Tensor:
+    """gridder_grid_static: plan + bin + grid of a small cadence on the library's own static 64 MiB workspace -- no
+    device allocation by the library or on its behalf (`out` is the caller's grid; without it one torch.empty is made
+    here).  Raises GridderError(ERR_WORKSPACE) when the plan needs more than STATIC_WORKSPACE_BYTES.  Synchronises
+    the device."""
+    lib = load_library()
+    device = vis.device
+    if device.type != "cuda":
+        raise RuntimeError("the gridder runs on a CUDA device only (no CPU fallback)")
+    if uvw_m.dim() == 2:
+        uvw_m = uvw_m[None]
+    n_time, n_bl, three = uvw_m.shape
+    if three != 3:
+        raise ValueError("uvw_m must be [n_time][n_baseline][3]")
+    n = n_time * n_bl * freq_hz.numel()
+    sup = [int(s) for s in (support if hasattr(support, "__len__") else [support])]
+    c_sup = (C.c_int32 * len(sup))(*sup)
+    if kernel.device != device or kernel.dtype != torch.float32 or not kernel.is_contiguous():
+        raise ValueError("kernel must be a contiguous float32 tensor on the visibilities' device")
+    cfg = _Config(int(grid_size), float(cell_size), 4, int(oversample), int(n_wplanes), c_sup, float(w_max),
+                  int(bool(kernel_is_complex)), kernel.data_ptr(), int(max(n, 1)), None, 0, 1)
+    tune = _Tuning()
+    for k, v in (tuning or {}).items():
+        if k not in TUNING_FIELDS:
+            raise KeyError(f"unknown gridder_tuning field {k!r}")
+        setattr(tune, k, int(v))
+    if out is None:
+        if accumulate:
+            raise ValueError("accumulate needs an existing grid")
+        out = torch.empty((4, int(grid_size), int(grid_size), 2), dtype=torch.float32, device=device)
+    need = C.c_size_t(0)
+    with torch.cuda.device(device):
+        rc = lib.gridder_grid_static(
+            C.byref(cfg), C.byref(tune), _dev_ptr(uvw_m, torch.float64, "uvw_m", device, 3 * n_time * n_bl), n_time, n_bl,
+            _dev_ptr(freq_hz, torch.float64, "freq_hz", device), freq_hz.numel(),
+            _dev_ptr(vis, torch.float32, "vis", device, 8 * n), _dev_ptr(weight, torch.float32, "weight", device, n),
+            _dev_ptr(out, torch.float32, "grid", device, 8 * int(grid_size) ** 2), int(accumulate), C.byref(need),
+            _stream_ptr(stream))
+    if rc != OK:
+        err = GridderError(rc, "gridder_grid_static")
+        err.workspace_needed = need.value
+        raise err
+    return out
 
 
 class Gridder:
