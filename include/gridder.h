@@ -99,7 +99,7 @@ typedef struct {
     int32_t merge;              /* 1 on (default), 2 off: entries of a batch of 32 with equal patch origin and
                                    sub-cell offset are summed before they are gridded (exact by linearity)        */
     int32_t presum;             /* pre-summation in input order (one real table, S <= 16, O <= 8): 1 always,
-                                   2 never; default: plans of max_vis >= 4 Mi, where the one synchronisation
+                                   2 never; default: plans of max_vis >= 1 Mi, where the one synchronisation
                                    it costs gridder_bin is cheaper than sorting every visibility                   */
     int32_t table_in_tmem;      /* 1 on, 2 off: GCF table in tensor memory instead of shared memory (one real
                                    table with O^2 x 8 <= 512 columns; default: on for pre-summed plans)            */

@@ -53,12 +53,12 @@ int derive(const gridder_config *cfg, const gridder_tuning *tuning, Plan &p) {
     // fast path: one real table with S <= 16 (table in shared or tensor memory, 32-bit sort values)
     p.mode = cplx ? 2 : ((cfg->n_wplanes == 1 && cfg->support[0] <= 16 && !t.force_general) ? 0 : 1);
     // PRE-SUMMATION IN INPUT ORDER (presum.cu): fast path, merging allowed (a per-visibility GCF forbids it),
-    // sub-cell offsets and drop flag in one byte.  By default for plans of 4 Mi visibilities and more: below
+    // sub-cell offsets and drop flag in one byte.  By default for plans of 1 Mi visibilities and more: below
     // that sorting every visibility is cheap and the one host synchronisation it costs gridder_bin is not.
     // Whether an input then really takes it is decided per gridder_bin, from its shape and the number of partial
     // records the plan kernel COUNTED (the data, not the capacity): see launch_bin.
     p.presum = (p.mode == 0 && p.merge && 2 * q_bits + 1 <= 8 &&
-                (t.presum == 1 || (t.presum == 0 && cfg->max_vis >= (4ll << 20)))) ? 1 : 0;
+                (t.presum == 1 || (t.presum == 0 && cfg->max_vis >= (1ll << 20)))) ? 1 : 0;
     // (its mapper packs the two lattice coordinates of a visibility into 16 bits each: map.cuh FastMap2::lat)
     if ((int64_t)cfg->grid_size * cfg->oversample + cfg->oversample >= 65533) p.presum = 0;
     p.tlog = t.tile_log2 ? t.tile_log2 : ((p.presum || p.mode != 0) ? 3 : 2);
