@@ -40,9 +40,9 @@ BAND_HZ = 768 * 40.0e3           # one rank's band; rank r starts at 140 MHz + r
 # (profiles/r02_kernels_config4_ncu_full.csv; historical, i.e. not measured by this run), keyed by kernel and config.
 NCU_TRAFFIC_BYTES = {
     # profiles/r02_kernels_config4_ncu_full.csv
-    ("presum_kernel", 4): 32_740_711_000,      # 29.974770 GB read + 2.765941 GB written
-    ("grid_kernel", 4): 6_326_859_000,         # 3.882851 GB read + 2.444008 GB written
-    ("presum_plan_kernel", 4): 1_298_758_000,  # 0.131762 GB read + 1.166996 GB written
+    ("presum_kernel", 4): 32_686_298_000,      # 29.923058 GB read + 2.763240 GB written
+    ("grid_kernel", 4): 6_077_384_000,         # 3.773518 GB read + 2.303866 GB written
+    ("presum_plan_kernel", 4): 1_299_012_000,  # 0.116209 GB read + 1.182803 GB written
 }
 
 
