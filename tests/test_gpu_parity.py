@@ -384,6 +384,14 @@ def test_merging_of_equal_origin_and_offset_entries(dev):
     assert st_b.n_records_gridded == st_b.n_vis == n                 # unmerged: one record per entry (none dropped)
     assert st_b.fma_executed == n * 256 * 8
     assert st_a.n_records_gridded < n // 3 and st_a.fma_executed == st_a.n_records_gridded * 256 * 8
+    # one work item per tile: with the per-origin bins carried from batch to batch the grid kernel grids every
+    # distinct (origin, offset) exactly once -- the count is the oracle's number of distinct lattice points
+    c, st_c = _run(dev, uvw, [C], vis, w, tuning={"chunk": 32768}, **kw)
+    m = oracle.map_visibilities(np.ascontiguousarray(uvw), [C], grid_size=N, cell_size=1.0, oversample=O, support=[S],
+                                kernel=np.ascontiguousarray(table, np.float32).ravel())
+    live = m[m[:, 5] == 0]
+    assert st_c.n_records_gridded == len(np.unique(live[:, :4], axis=0))
+    assert_parity(c, ref, ab, "merging on, one item per tile")
 
 
 @pytest.mark.parametrize("S,O,N,n,tuning", [(16, 4, 96, 6000, {}), (12, 4, 66, 3000, {"merge": 2}),

@@ -198,3 +198,32 @@ def test_per_baseline_tables_bank_of_one_on_the_fast_path(dev, presum):
     n_bad = int(((idx < 0) | (idx > 0)).sum()) * nf
     assert st.n_dropped == ost["n_dropped"] == n_bad and st.vis_taps == ost["vis_taps"] and st.n_presum_records == 0
     assert_parity(out, ref, ab, "bank of one table with indices outside it")
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+def test_carried_bins_grid_every_plane_origin_offset_once(dev, cplx):
+    """Long runs of one (plane, origin) across many batches, both signs of w, every sub-cell offset: with the per-run
+    bins (grid.cu stage_write_bins) the grid kernel grids each distinct (plane, conjugate, origin, offset) of a work
+    item exactly once -- the count is pinned against the oracle's mapping -- and the sums stay within tolerance."""
+    rng = np.random.default_rng(91 + cplx)
+    supports = [12, 16]                                       # one patch class (16 cells), two tables
+    O, N, n, w_max = 4, 64, 7000, 2.0
+    table = _tables(rng, supports, O, cplx)
+    uvw = np.zeros((1, n, 3))
+    uvw[0, :, :2] = rng.uniform(-1.4, 1.4, (n, 2))            # a handful of origins, all of one 8 x 8 tile or two
+    uvw[0, :, 2] = rng.uniform(-2.0, 2.0, n)
+    uvw[0, :200, :2] = 0.3                                    # and one lattice point met 200 times
+    vis = rng.standard_normal((n, 4, 2)).astype(np.float32)
+    w = rng.uniform(0.5, 1.5, n).astype(np.float32)
+    got, ref, ab, st, ost = _both(dev, uvw, [C], vis, w, N=N, du=1.0, O=O, supports=supports, table=table, w_max=w_max,
+                                  cplx=cplx, tuning={"chunk": 16384})
+    m = oracle.map_visibilities(uvw, [C], grid_size=N, cell_size=1.0, oversample=O, support=supports, kernel=table,
+                                w_max=w_max, kernel_is_complex=cplx)
+    live = m[m[:, 5] == 0]
+    if not cplx:
+        live = live.copy()
+        live[:, 4] &= 255                                     # real tables: the sign of w changes nothing
+    distinct = len(np.unique(live[:, :5], axis=0))
+    assert st.n_dropped == 0 and st.n_work_items <= 4
+    assert st.n_records_gridded == distinct < n // 4
+    assert_parity(got, ref, ab, f"carried bins cplx={cplx}")
